@@ -1,0 +1,208 @@
+"""CPU oracle for the CLTDSE hot path -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+ctypes front-end of oracle/tdse_oracle.cpp (see tdse_oracle.h for the citations).
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs may import this package; it imports nothing from paper_1308_1856_b200.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+from .build import build as _build
+
+_lib = None
+
+
+class Grid(C.Structure):
+    _fields_ = [("n_r", C.c_int), ("dr", C.c_double), ("n_l", C.c_int), ("fd_order", C.c_int),
+                ("z_nuc", C.c_double), ("batch", C.c_int), ("r_offset", C.c_double)]
+
+
+class Pulse(C.Structure):
+    _fields_ = [("e0", C.c_double), ("omega", C.c_double), ("n_cycles", C.c_double), ("cep", C.c_double)]
+
+
+class Obs(C.Structure):
+    _fields_ = [("n_states", C.c_int), ("l_of_state", C.POINTER(C.c_int)), ("phi", C.POINTER(C.c_double)),
+                ("obs_every", C.c_int), ("obs_out", C.POINTER(C.c_double))]
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build())
+        _lib.oracle_pulse_E.restype = C.c_double
+        _lib.oracle_pulse_E.argtypes = [C.POINTER(Pulse), C.c_double]
+    return _lib
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def make_grid(n_r, dr, n_l, fd_order, z_nuc=1.0, batch=1, r_offset=0.0):
+    return Grid(int(n_r), float(dr), int(n_l), int(fd_order), float(z_nuc), int(batch), float(r_offset))
+
+
+def _pulses(g, pulses):
+    """pulses: iterable of (e0, omega, n_cycles, cep) per member (or one tuple for all)."""
+    if isinstance(pulses, tuple) and not isinstance(pulses[0], (tuple, list)):
+        pulses = [pulses] * g.batch
+    assert len(pulses) == g.batch
+    arr = (Pulse * g.batch)()
+    for i, p in enumerate(pulses):
+        arr[i] = Pulse(*[float(x) for x in p])
+    return arr
+
+
+def _state(g, psi):
+    psi = np.ascontiguousarray(psi, dtype=np.complex128).reshape(g.batch, g.n_l, g.n_r).copy()
+    return psi
+
+
+def _obs(g, states, obs_every, nsteps):
+    """states: None or (l_of_state int array, phi [n][n_r]) -> (Obs struct or None, out array, keepalive)."""
+    if not obs_every:
+        return None, None, None
+    if states is None:
+        l_arr = np.zeros(0, dtype=np.int32)
+        phi = np.zeros((0, g.n_r))
+    else:
+        l_arr = np.ascontiguousarray(states[0], dtype=np.int32)
+        phi = np.ascontiguousarray(states[1], dtype=np.float64).reshape(len(l_arr), g.n_r)
+    n_blocks = nsteps // obs_every
+    out = np.zeros((n_blocks, g.batch, 3 + len(l_arr)))
+    o = Obs(len(l_arr), l_arr.ctypes.data_as(C.POINTER(C.c_int)), _dp(phi), int(obs_every), _dp(out))
+    return o, out, (l_arr, phi)
+
+
+def set_threads(n):
+    lib().oracle_set_threads(int(n))
+
+
+def pulse_E(pulse, t):
+    p = Pulse(*[float(x) for x in pulse])
+    return lib().oracle_pulse_E(C.byref(p), float(t))
+
+
+def coupling(n_l):
+    c = np.zeros(n_l)
+    lib().oracle_coupling(int(n_l), _dp(c))
+    return c
+
+
+def apply_H(g, psi, e_field):
+    psi = _state(g, psi)
+    e = np.ascontiguousarray(np.broadcast_to(np.asarray(e_field, dtype=np.float64), (g.batch,)))
+    out = np.empty_like(psi)
+    rc = lib().oracle_apply_H(C.byref(g), _dp(psi.view(np.float64)), _dp(e), _dp(out.view(np.float64)))
+    assert rc == 0, rc
+    return out
+
+
+def dense_H(g, e_field):
+    n = g.n_r * g.n_l
+    h = np.zeros((n, n))
+    rc = lib().oracle_dense_H(C.byref(g), C.c_double(e_field), _dp(h))
+    assert rc == 0, rc
+    return h
+
+
+def bound_states(g, l, n_want, only_negative=False):
+    en = np.zeros(n_want)
+    phi = np.zeros((n_want, g.n_r))
+    n = lib().oracle_bound_states(C.byref(g), int(l), int(n_want), int(bool(only_negative)), _dp(en), _dp(phi))
+    assert n >= 0, n
+    return en[:n].copy(), phi[:n].copy()
+
+
+def observables(g, psi, e_now, states=None):
+    psi = _state(g, psi)
+    e = np.ascontiguousarray(np.broadcast_to(np.asarray(e_now, dtype=np.float64), (g.batch,)))
+    if states is None:
+        l_arr, phi = np.zeros(0, dtype=np.int32), np.zeros((0, g.n_r))
+    else:
+        l_arr = np.ascontiguousarray(states[0], dtype=np.int32)
+        phi = np.ascontiguousarray(states[1], dtype=np.float64).reshape(len(l_arr), g.n_r)
+    out = np.zeros((g.batch, 3 + len(l_arr)))
+    rc = lib().oracle_observables(C.byref(g), _dp(psi.view(np.float64)), _dp(e), len(l_arr),
+                                  l_arr.ctypes.data_as(C.POINTER(C.c_int)), _dp(phi), _dp(out))
+    assert rc == 0, rc
+    return out
+
+
+def step_taylor(g, pulses, psi, order, t0, dt, nsteps, field_sample=0, states=None, obs_every=0):
+    psi = _state(g, psi)
+    pa = _pulses(g, pulses)
+    o, out, keep = _obs(g, states, obs_every, nsteps)
+    rc = lib().oracle_step_taylor(C.byref(g), pa, _dp(psi.view(np.float64)), int(order), C.c_double(t0),
+                                  C.c_double(dt), C.c_long(nsteps), int(field_sample),
+                                  C.byref(o) if o else None)
+    assert rc == 0, rc
+    return psi, out
+
+
+def step_rk_fixed(g, pulses, psi, tableau, t0, dt, nsteps, states=None, obs_every=0):
+    """tableau: 0 = ClassicRK4, 1 = DormandPrince (5th-order weights). Returns psi, err[nsteps], obs."""
+    psi = _state(g, psi)
+    pa = _pulses(g, pulses)
+    o, out, keep = _obs(g, states, obs_every, nsteps)
+    err = np.zeros(max(nsteps, 1))
+    rc = lib().oracle_step_rk_fixed(C.byref(g), pa, _dp(psi.view(np.float64)), int(tableau), C.c_double(t0),
+                                    C.c_double(dt), C.c_long(nsteps), _dp(err), C.byref(o) if o else None)
+    assert rc == 0, rc
+    return psi, err[:nsteps], out
+
+
+def step_rk4(g, pulses, psi, t0, dt, nsteps, states=None, obs_every=0):
+    psi, _, out = step_rk_fixed(g, pulses, psi, 0, t0, dt, nsteps, states, obs_every)
+    return psi, out
+
+
+def step_rk45(g, pulses, psi, t0, t_end, dt_init, rtol, dt_max=0.0, dt_replay=None, max_log=1 << 20):
+    """Returns psi, dict(n_accept, n_reject, dt[], err[])."""
+    psi = _state(g, psi)
+    pa = _pulses(g, pulses)
+    na, nr = C.c_long(0), C.c_long(0)
+    if dt_replay is not None:
+        rep = np.ascontiguousarray(dt_replay, dtype=np.float64)
+        max_log = max(len(rep), 1)
+    dt_log, err_log = np.zeros(max_log), np.zeros(max_log)
+    rc = lib().oracle_step_rk45(C.byref(g), pa, _dp(psi.view(np.float64)), C.c_double(t0), C.c_double(t_end),
+                                C.c_double(dt_init), C.c_double(rtol), C.c_double(dt_max),
+                                _dp(rep) if dt_replay is not None else None,
+                                C.c_long(len(rep) if dt_replay is not None else 0),
+                                C.byref(na), C.byref(nr), _dp(dt_log), _dp(err_log), C.c_long(max_log))
+    assert rc == 0, rc
+    n = min(na.value, max_log)
+    return psi, {"n_accept": na.value, "n_reject": nr.value, "dt": dt_log[:n].copy(), "err": err_log[:n].copy()}
+
+
+def step_lanczos(g, pulses, psi, krylov_dim, taylor_order, t0, dt, nsteps, field_sample=0, beta_tol=1e-12,
+                 states=None, obs_every=0):
+    psi = _state(g, psi)
+    pa = _pulses(g, pulses)
+    o, out, keep = _obs(g, states, obs_every, nsteps)
+    rc = lib().oracle_step_lanczos(C.byref(g), pa, _dp(psi.view(np.float64)), int(krylov_dim), int(taylor_order),
+                                   C.c_double(t0), C.c_double(dt), C.c_long(nsteps), int(field_sample),
+                                   C.c_double(beta_tol), C.byref(o) if o else None)
+    assert rc == 0, rc
+    return psi, out
+
+
+def lanczos_internals(g, psi, e_field, krylov_dim, taylor_order, dt, beta_tol=1e-12):
+    """One member. Returns dict(m, q[K][L][N], alpha[K], beta[K], coef[K] complex, n_sub)."""
+    assert g.batch == 1
+    psi = _state(g, psi)
+    K = int(krylov_dim)
+    q = np.zeros((K, g.n_l, g.n_r), dtype=np.complex128)
+    alpha, beta = np.zeros(K), np.zeros(K)
+    coef = np.zeros(K, dtype=np.complex128)
+    n_sub = C.c_int(0)
+    m = lib().oracle_lanczos_internals(C.byref(g), _dp(psi.view(np.float64)), C.c_double(e_field), K,
+                                       int(taylor_order), C.c_double(dt), C.c_double(beta_tol),
+                                       _dp(q.view(np.float64)), _dp(alpha), _dp(beta),
+                                       _dp(coef.view(np.float64)), C.byref(n_sub))
+    assert m >= 1, m
+    return {"m": m, "q": q, "alpha": alpha, "beta": beta, "coef": coef, "n_sub": n_sub.value}

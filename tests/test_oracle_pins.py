@@ -1,0 +1,549 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (-m "not gpu").
+
+Every oracle function is checked against something other than itself: values the paper prints
+(tests/golden/), closed forms, LAPACK on a dense matrix, brute force on the tiny grid, invariants.
+Pin numbers P1..P10 refer to DESIGN.md "Oracle pins".
+"""
+import math
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+import scipy.linalg as sla
+
+import oracle
+from paper_1308_1856_b200 import workloads as wl
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def read_golden(name):
+    rows = []
+    for line in open(os.path.join(GOLD, name)):
+        line = line.split("#")[0].strip()
+        if line:
+            rows.append(line.split())
+    return rows
+
+
+def tiny(fd_order, n_l=3, n_r=100, dr=0.2):
+    return oracle.make_grid(n_r, dr, n_l, fd_order)
+
+
+def rand_state(shape, seed):
+    u = wl.splitmix64_uniform(seed, 2 * int(np.prod(shape)))
+    v = 2 * u - 1
+    return (v[0::2] + 1j * v[1::2]).reshape(shape)
+
+
+def dense_propagate(h, psi, dt):
+    """exp(-i H dt) psi by LAPACK eigen-decomposition of the dense real-symmetric H."""
+    w, v = np.linalg.eigh(h)
+    return v @ (np.exp(-1j * w * dt) * (v.T @ psi))
+
+
+# ---------------------------------------------------------------- coupling, pulse
+def test_coupling_is_cos_theta_matrix_element():
+    """c_l = <l 0|cos(theta)|l+1 0> (Eq. 9): Gauss-Legendre quadrature of normalised Legendre polynomials."""
+    x, w = np.polynomial.legendre.leggauss(80)
+    c = oracle.coupling(12)
+    for l in range(12):
+        pl = np.polynomial.legendre.Legendre.basis(l)(x) * math.sqrt((2 * l + 1) / 2)
+        pn = np.polynomial.legendre.Legendre.basis(l + 1)(x) * math.sqrt((2 * l + 3) / 2)
+        assert abs(np.sum(w * pl * x * pn) - c[l]) < 1e-13
+    assert abs(c[0] - 1 / math.sqrt(3)) < 1e-16
+
+
+def test_pulse_properties():
+    """E(t) = e0 sin^2(w t/2n_c) cos(w t + cep) on [0, T] (Eq. 19): zero at the ends and outside,
+    |E(T/2)| = e0 for integer n_c, zero time integral, carrier at omega."""
+    e0, om, nc = 0.0534, 0.057, 4.0
+    T = 2 * math.pi * nc / om
+    p = (e0, om, nc, 0.0)
+    assert oracle.pulse_E(p, 0.0) == 0.0
+    assert abs(oracle.pulse_E(p, T)) < 1e-15
+    assert oracle.pulse_E(p, -1e-9) == 0.0 and oracle.pulse_E(p, T * (1 + 1e-12) + 1e-9) == 0.0
+    assert abs(abs(oracle.pulse_E(p, T / 2)) - e0) < 1e-15
+    t = np.linspace(0, T, 20001)
+    e = np.array([oracle.pulse_E(p, x) for x in t])
+    assert abs(np.trapezoid(e, t)) < 1e-9 * e0 * T           # no DC component for n_c >= 2
+    # the spectrum peaks at the carrier
+    f = np.abs(np.fft.rfft(e, 8 * len(e)))
+    om_peak = 2 * math.pi * np.argmax(f) / (8 * len(e) * (t[1] - t[0]))
+    assert abs(om_peak - om) < 0.02 * om
+    # cep shifts the carrier: cep = pi/2 makes the centre a zero crossing
+    assert abs(oracle.pulse_E((e0, om, nc, math.pi / 2), T / 2)) < 1e-15
+    # test aid: omega = 0 is a static field
+    assert oracle.pulse_E((0.05, 0.0, 1.0, 0.0), 123.4) == 0.05
+
+
+# ---------------------------------------------------------------- P1: Hermiticity, dense == matrix-free
+@pytest.mark.parametrize("fd", [3, 5])
+def test_P1_dense_H_symmetric_and_equals_matrix_free(fd):
+    g = tiny(fd)
+    h = oracle.dense_H(g, 0.05)
+    assert np.array_equal(h, h.T)                               # exactly symmetric
+    psi = rand_state((1, g.n_l, g.n_r), 11 + fd)
+    ref = (h @ psi.reshape(-1)).reshape(psi.shape)
+    out = oracle.apply_H(g, psi, 0.05)
+    assert np.linalg.norm(out - ref) <= 1e-14 * np.linalg.norm(ref)
+
+
+@pytest.mark.parametrize("fd", [3, 5])
+def test_P1_band_structure(fd):
+    """P:134/Fig. 1: diagonal blocks are (2w+1)-diagonal, length-gauge off-diagonal blocks are diagonal,
+    blocks with |l-l'| > 1 vanish; off-diagonal blocks scale linearly with E and vanish at E = 0."""
+    g = tiny(fd)
+    n, L, w = g.n_r, g.n_l, (1 if fd == 3 else 2)
+    h = oracle.dense_H(g, 0.05).reshape(L, n, L, n)
+    h0 = oracle.dense_H(g, 0.0).reshape(L, n, L, n)
+    jj = np.abs(np.arange(n)[:, None] - np.arange(n)[None, :])
+    for l in range(L):
+        for lp in range(L):
+            blk = h[l, :, lp, :]
+            if l == lp:
+                assert np.all(blk[jj > w] == 0) and np.all(blk[jj <= w] != 0)
+                assert np.array_equal(blk, h0[l, :, lp, :])
+            elif abs(l - lp) == 1:
+                assert np.all(blk[jj > 0] == 0) and np.all(np.diag(blk) != 0)
+                assert np.all(h0[l, :, lp, :] == 0)
+                r = 0.2 * np.arange(1, n + 1)
+                assert np.allclose(np.diag(blk), 0.05 * r * oracle.coupling(L)[min(l, lp)], rtol=1e-15)
+            else:
+                assert np.all(blk == 0)
+
+
+@pytest.mark.parametrize("shape", [(500, 0.2, 8, 3, 1), (700, 0.1, 5, 5, 1), (64, 0.1, 4, 3, 3), (257, 0.1, 7, 5, 2)])
+def test_P1_matrix_free_hermitian(shape):
+    n_r, dr, n_l, fd, b = shape
+    g = oracle.make_grid(n_r, dr, n_l, fd, batch=b)
+    x = rand_state((b, n_l, n_r), 3)
+    y = rand_state((b, n_l, n_r), 4)
+    e = 0.01 + 0.0004 * np.arange(b)
+    hx, hy = oracle.apply_H(g, x, e), oracle.apply_H(g, y, e)
+    for m in range(b):
+        lhs, rhs = np.vdot(x[m], hy[m]), np.vdot(hx[m], y[m])
+        assert abs(lhs - rhs) <= 1e-13 * abs(lhs)
+    # batched call == per-member calls
+    g1 = oracle.make_grid(n_r, dr, n_l, fd, batch=1)
+    for m in range(b):
+        assert np.array_equal(oracle.apply_H(g1, x[m], e[m])[0], hx[m])
+
+
+# ---------------------------------------------------------------- P2/P3: energies
+def test_P2_closed_form_3point_ground_state():
+    for dr_s, e_s in read_golden("closed_form_energies.txt"):
+        dr, e_gold = float(dr_s), float(e_s)
+        assert abs(e_gold + 1 / (1 + math.sqrt(1 + dr * dr))) < 1e-12
+        g = oracle.make_grid(int(round(100 / dr)), dr, 1, 3)
+        en, phi = oracle.bound_states(g, 0, 1)
+        assert abs(en[0] - e_gold) < 1e-11
+        # the eigenvector is j q^j
+        q = math.sqrt(1 + dr * dr) - dr
+        j = np.arange(1, g.n_r + 1)
+        ref = wl.grid_normalised(j * q ** j, dr)
+        assert np.max(np.abs(phi[0] - ref)) < 1e-9
+        assert abs(dr * np.sum(phi[0] ** 2) - 1) < 1e-13 and phi[0, 0] > 0
+        # H phi = E phi with the matrix-free operator (pins kinetic sign, Coulomb term, grid origin)
+        res = oracle.apply_H(g, phi[0][None, None, :], 0.0)[0, 0] - en[0] * phi[0]
+        assert np.linalg.norm(res) < 1e-10
+    # O(dr^2) convergence to -0.5 (NS)
+    errs = [abs(-1 / (1 + math.sqrt(1 + d * d)) + 0.5) for d in (0.2, 0.1, 0.05)]
+    assert 3.9 < errs[0] / errs[1] < 4.1 and 3.9 < errs[1] / errs[2] < 4.1
+
+
+@pytest.mark.parametrize("fd,dr,l", [(3, 0.2, 0), (3, 0.2, 1), (3, 0.1, 3), (5, 0.2, 0), (5, 0.2, 1), (5, 0.1, 2)])
+def test_P2b_eigensolver_vs_lapack(fd, dr, l):
+    """Bound states of h_l against LAPACK on the same band (scipy.linalg.eig_banded)."""
+    n = 600
+    g = oracle.make_grid(n, dr, l + 1, fd)
+    r = dr * np.arange(1, n + 1)
+    v = l * (l + 1) / (2 * r * r) - 1 / r
+    if fd == 3:
+        band = np.zeros((2, n)); band[0] = 1 / dr ** 2 + v; band[1, :-1] = -0.5 / dr ** 2
+    else:
+        band = np.zeros((3, n)); band[0] = 30 / (24 * dr ** 2) + v
+        band[1, :-1] = -16 / (24 * dr ** 2); band[2, :-2] = 1 / (24 * dr ** 2)
+    w, vec = sla.eig_banded(band, lower=True, select="i", select_range=(0, 3))
+    en, phi = oracle.bound_states(g, l, 4)
+    assert np.max(np.abs(en - w)) < 1e-10
+    for k in range(4):
+        ref = vec[:, k] / math.sqrt(dr) * np.sign(vec[0, k])
+        assert np.max(np.abs(phi[k] - ref)) < 1e-7
+    # the oracle's own H agrees: ||H phi - E phi|| small for block l
+    psi = np.zeros((1, l + 1, n), dtype=complex); psi[0, l] = phi[0]
+    res = oracle.apply_H(g, psi, 0.0)[0, l] - en[0] * phi[0]
+    assert np.linalg.norm(res) < 1e-9
+    # only_negative stops at the continuum
+    en_neg, _ = oracle.bound_states(g, l, 40, only_negative=True)
+    assert len(en_neg) < 40 and np.all(en_neg < 0)
+    w_all = sla.eig_banded(band, lower=True, eigvals_only=True)
+    assert len(en_neg) == int(np.sum(w_all < 0))
+
+
+def test_P3_paper_printed_energies_5point():
+    """E_1s ~ -0.47 on (R = 800, dr = 0.2) and ~ -0.5 with Offset -0.02: pins the 5-point coefficients and
+    the zero-extension inner boundary (reading G4); odd extension would give -0.4896 / -0.5241."""
+    for n_r, dr, fd, off, e_print, tol in read_golden("paper_energies.txt"):
+        g = oracle.make_grid(int(n_r), float(dr), 1, int(fd), r_offset=float(off))
+        en, _ = oracle.bound_states(g, 0, 1)
+        assert abs(en[0] - float(e_print)) < float(tol), en
+    g = oracle.make_grid(4000, 0.2, 1, 5)
+    assert abs(oracle.bound_states(g, 0, 1)[0][0] - (-0.4714542027)) < 1e-9
+
+
+# ---------------------------------------------------------------- P6: structural zeros / reality
+@pytest.mark.parametrize("fd", [3, 5])
+def test_P6_structural_zeros_and_reality(fd):
+    g = oracle.make_grid(120, 0.2, 6, fd)
+    psi = np.zeros((1, 6, 120), dtype=complex)
+    psi[0, 0] = rand_state((120,), 5).real
+    cur = psi
+    for k in range(1, 5):
+        cur = oracle.apply_H(g, cur, 0.07)
+        assert np.all(cur[0, k + 1:] == 0)                     # coupling only l <-> l +- 1
+        assert np.any(cur[0, k] != 0)
+        assert np.all(cur.imag == 0)                           # H real: real in, real out
+    # i * real in -> purely imaginary out
+    out = oracle.apply_H(g, 1j * psi, 0.07)
+    assert np.all(out.real == 0)
+
+
+# ---------------------------------------------------------------- P4: dense exponential on the tiny grid
+STATIC = lambda e: (e, 0.0, 1.0, 0.0)       # omega = 0: static field
+
+
+@pytest.mark.parametrize("fd", [3, 5])
+@pytest.mark.parametrize("order", [2, 4, 6, 10])
+def test_P4_taylor_vs_dense_exponential(fd, order):
+    g = tiny(fd)
+    h = oracle.dense_H(g, 0.05)
+    rho = np.max(np.abs(np.linalg.eigvalsh(h)))
+    dt = 0.004
+    y = dt * rho
+    psi = rand_state((1, g.n_l, g.n_r), 21)
+    psi /= np.linalg.norm(psi)
+    exact = dense_propagate(h, psi.reshape(-1), dt)
+    got, _ = oracle.step_taylor(g, STATIC(0.05), psi, order, 0.0, dt, 1)
+    err = np.linalg.norm(got.reshape(-1) - exact)
+    bound = 1.01 * y ** (order + 1) / math.factorial(order + 1)
+    assert err <= bound + 1e-15
+    # ... and it IS of order P: the error is the first dropped term (next one is y/(P+2) smaller)
+    lead = psi.reshape(-1).copy()
+    for k in range(order + 1):
+        lead = dt * (h @ lead)
+    lead = np.linalg.norm(lead) / math.factorial(order + 1)
+    assert 0.7 * lead - 2e-15 <= err <= 1.3 * lead + 2e-15
+    # exact polynomial: sum_k (-i H dt)^k / k!
+    acc, term = psi.reshape(-1).copy(), psi.reshape(-1).copy()
+    for k in range(1, order + 1):
+        term = (-1j * dt / k) * (h @ term); acc = acc + term
+    assert np.linalg.norm(got.reshape(-1) - acc) < 1e-14
+
+
+@pytest.mark.parametrize("fd", [3, 5])
+def test_P4_rk4_and_dp5_stability_polynomials(fd):
+    """Constant field: RK4 == Taylor-4 polynomial; DP5 == sum_{k<=5} z^k/k! + z^6/600 (its stability function)."""
+    g = tiny(fd)
+    h = oracle.dense_H(g, 0.05)
+    dt = 0.004
+    psi = rand_state((1, g.n_l, g.n_r), 22); psi /= np.linalg.norm(psi)
+    v = psi.reshape(-1)
+    pw = [v]
+    for k in range(1, 7):
+        pw.append(-1j * dt * (h @ pw[-1]))
+    t4 = sum(pw[k] / math.factorial(k) for k in range(5))
+    r5 = sum(pw[k] / math.factorial(k) for k in range(6)) + pw[6] / 600
+    got4, _ = oracle.step_rk4(g, STATIC(0.05), psi, 0.0, dt, 1)
+    assert np.linalg.norm(got4.reshape(-1) - t4) < 2e-15
+    got5, err, _ = oracle.step_rk_fixed(g, STATIC(0.05), psi, 1, 0.0, dt, 1)
+    assert np.linalg.norm(got5.reshape(-1) - r5) < 2e-15
+    # embedded 4th-order solution: R4hat = sum_{k<=4} z^k/k! + (1097/120000) z^5 + (161/120000) z^6 + z^7/24000
+    pw.append(-1j * dt * (h @ pw[-1]))
+    r4 = sum(pw[k] / math.factorial(k) for k in range(5)) + 1097 / 120000 * pw[5] + 161 / 120000 * pw[6] + pw[7] / 24000
+    want = np.linalg.norm(r5 - r4) / np.linalg.norm(r5)
+    assert abs(err[0] - want) < 1e-3 * want
+
+
+def test_dormand_prince_order_conditions():
+    """The tableau satisfies the order conditions in exact rational arithmetic: row sums = c; b up to order 5."""
+    F = Fraction
+    c = [F(0), F(1, 5), F(3, 10), F(4, 5), F(8, 9), F(1), F(1)]
+    a = [[], [F(1, 5)], [F(3, 40), F(9, 40)], [F(44, 45), F(-56, 15), F(32, 9)],
+         [F(19372, 6561), F(-25360, 2187), F(64448, 6561), F(-212, 729)],
+         [F(9017, 3168), F(-355, 33), F(46732, 5247), F(49, 176), F(-5103, 18656)],
+         [F(35, 384), F(0), F(500, 1113), F(125, 192), F(-2187, 6784), F(11, 84)]]
+    b = [F(35, 384), F(0), F(500, 1113), F(125, 192), F(-2187, 6784), F(11, 84), F(0)]
+    bh = [F(5179, 57600), F(0), F(7571, 16695), F(393, 640), F(-92097, 339200), F(187, 2100), F(1, 40)]
+    for i in range(7):
+        assert sum(a[i]) == c[i]
+    for q in range(1, 6):                                       # quadrature conditions
+        assert sum(bi * ci ** (q - 1) for bi, ci in zip(b, c)) == F(1, q)
+    for q in range(1, 5):
+        assert sum(bi * ci ** (q - 1) for bi, ci in zip(bh, c)) == F(1, q)
+    assert sum(bi * ci ** 4 for bi, ci in zip(bh, c)) != F(1, 5)
+    ac = [sum(aij * c[j] for j, aij in enumerate(a[i])) for i in range(7)]
+    assert sum(bi * x for bi, x in zip(b, ac)) == F(1, 6)        # order 3
+    assert sum(bi * ci * x for bi, ci, x in zip(b, c, ac)) == F(1, 8)   # order 4
+    # the stability function the oracle is pinned to in test_P4: coefficient of z^6 is 1/600
+    # (b . A^5 . 1 = 1/600)
+    vec = [F(1)] * 7
+    for _ in range(5):
+        vec = [sum(aij * vec[j] for j, aij in enumerate(a[i])) for i in range(7)]
+    assert sum(bi * x for bi, x in zip(b, vec)) == F(1, 600)
+
+
+@pytest.mark.parametrize("fd", [3, 5])
+def test_P4_lanczos_vs_dense_exponential(fd):
+    g = tiny(fd)
+    h = oracle.dense_H(g, 0.05)
+    dt = 0.004
+    psi = rand_state((1, g.n_l, g.n_r), 23); psi /= np.linalg.norm(psi)
+    exact = dense_propagate(h, psi.reshape(-1), dt)
+    got, _ = oracle.step_lanczos(g, STATIC(0.05), psi, 16, 12, 0.0, dt, 1)
+    assert np.linalg.norm(got.reshape(-1) - exact) < 1e-12
+    # several steps, against the dense propagator applied repeatedly
+    got, _ = oracle.step_lanczos(g, STATIC(0.05), psi, 16, 12, 0.0, dt, 25)
+    assert np.linalg.norm(got.reshape(-1) - dense_propagate(h, psi.reshape(-1), 25 * dt)) < 1e-11
+
+
+# ---------------------------------------------------------------- P9: Lanczos internals
+@pytest.mark.parametrize("fd", [3, 5])
+def test_P9_lanczos_internals(fd):
+    g = tiny(fd)
+    h = oracle.dense_H(g, 0.05)
+    psi = rand_state((1, g.n_l, g.n_r), 24)
+    K = 16
+    r = oracle.lanczos_internals(g, psi, 0.05, K, 12, 0.004)
+    assert r["m"] == K
+    Q = r["q"].reshape(K, -1)
+    # three-term recurrence in the order of reading G16:  H q_p = beta_{p-1} q_{p-1} + alpha_p q_p + beta_p q_{p+1}
+    hn = np.max(np.abs(np.linalg.eigvalsh(h)))
+    for p in range(K - 1):
+        lhs = h @ Q[p]
+        rhs = r["alpha"][p] * Q[p] + r["beta"][p] * Q[p + 1] + (r["beta"][p - 1] * Q[p - 1] if p else 0)
+        assert np.linalg.norm(lhs - rhs) < 1e-13 * hn
+        assert abs(r["alpha"][p] - np.vdot(Q[p], lhs).real) < 1e-12 * hn
+    G = Q.conj() @ Q.T
+    assert np.max(np.abs(np.diag(G) - 1)) < 1e-13                   # unit vectors
+    assert np.max(np.abs(np.diag(G, 1))) < 1e-12 and np.max(np.abs(np.diag(G, 2))) < 1e-12   # local orthogonality
+    # no re-orthogonalisation in the paper: global orthogonality decays as Ritz values converge, but stays small
+    assert np.max(np.abs(G[:8, :8] - np.eye(8))) < 1e-11 and np.max(np.abs(G - np.eye(K))) < 1e-6
+    T = Q.conj() @ (h @ Q.T)
+    Tref = np.diag(r["alpha"]) + np.diag(r["beta"][:K - 1], 1) + np.diag(r["beta"][:K - 1], -1)
+    assert np.max(np.abs(T - Tref)) < 1e-6 * np.max(np.abs(Tref))  # Q^H H Q = tridiag(beta, alpha, beta)
+    assert abs(np.vdot(Q[0], psi.reshape(-1)) - np.linalg.norm(psi)) < 1e-12
+    # coefficients = exp(-i T dt) e_1 (LAPACK), sub-stepping per the Gershgorin rule
+    w, v = np.linalg.eigh(Tref)
+    cref = v @ (np.exp(-1j * w * 0.004) * v[0])
+    assert np.max(np.abs(r["coef"] - cref)) < 1e-13
+    gr = max(abs(r["alpha"][i]) + (r["beta"][i - 1] if i else 0) + (r["beta"][i] if i < K - 1 else 0) for i in range(K))
+    assert r["n_sub"] == max(1, math.ceil(0.004 * gr / 3.0))
+    # K = 1: psi * R(-i alpha dt), R the truncated exponential
+    r1 = oracle.lanczos_internals(g, psi, 0.05, 1, 12, 0.004)
+    a = np.vdot(psi, (h @ psi.reshape(-1)).reshape(psi.shape)).real / np.vdot(psi, psi).real
+    assert abs(r1["alpha"][0] - a) < 1e-12 * abs(a)
+    z = -1j * a * 0.004 / r1["n_sub"]
+    R = sum(z ** k / math.factorial(k) for k in range(13)) ** r1["n_sub"]
+    assert abs(r1["coef"][0] - R) < 1e-14
+    got, _ = oracle.step_lanczos(g, STATIC(0.05), psi, 1, 12, 0.0, 0.004, 1)
+    assert np.linalg.norm(got - psi * R) < 1e-13 * np.linalg.norm(psi)
+
+
+def test_lanczos_substepping_large_dt():
+    """Reading G18: with Ritz values * dt above the Taylor-12 stability limit the small system is sub-stepped;
+    the step stays unitary in the Krylov space (|c| = 1) and exact for a state inside an invariant subspace."""
+    g = tiny(3)
+    h = oracle.dense_H(g, 0.0)
+    w, v = np.linalg.eigh(h)
+    # state spanned by 3 eigenvectors with large eigenvalues: Krylov space closes at m = 3
+    idx = [len(w) - 1, len(w) - 7, 5]
+    psi = (v[:, idx] @ np.array([0.6, 0.5 + 0.2j, 0.3j])).reshape(1, g.n_l, g.n_r)
+    dt = 0.5
+    assert dt * w[-1] > 3.4
+    r = oracle.lanczos_internals(g, psi, 0.0, 8, 12, dt, beta_tol=1e-9)
+    assert r["m"] == 3 and r["n_sub"] > 1
+    # each sub-step has y <= 3: Taylor-12 is stable there (|R| <= 1) and accurate to y^13/13! ~ 2.6e-4
+    assert 1 - 1e-3 * r["n_sub"] < np.linalg.norm(r["coef"]) <= 1 + 1e-12
+    got, _ = oracle.step_lanczos(g, STATIC(0.0), psi, 8, 12, 0.0, dt, 1, beta_tol=1e-9)
+    assert np.linalg.norm(got.reshape(-1) - dense_propagate(h, psi.reshape(-1), dt)) < 1e-3 * r["n_sub"]
+    # without sub-stepping the same step would blow up: |R_12(-i y)| > 1 for y = dt * lambda_max
+    y = dt * w[-1]
+    assert abs(sum((-1j * y) ** k / math.factorial(k) for k in range(13))) > 1.0 + 1e-3
+
+
+# ---------------------------------------------------------------- P5: field-free eigenstate phase
+@pytest.mark.parametrize("prop", ["taylor4", "taylor6", "rk4", "dp5", "lanczos"])
+def test_P5_field_free_phase(prop):
+    dr, n_r = 0.2, 500
+    g = oracle.make_grid(n_r, dr, 3, 3)
+    e1s = -1 / (1 + math.sqrt(1 + dr * dr))                       # closed form, not the oracle's eigenvalue
+    en, phi = oracle.bound_states(g, 0, 1)
+    psi0 = np.zeros((1, 3, n_r), dtype=complex); psi0[0, 0] = phi[0]
+    dt, n = 0.01, 200
+    off = (0.0, 0.057, 2.0, 0.0)
+    trunc = lambda z, p: sum(z ** k / math.factorial(k) for k in range(p + 1))
+    z = -1j * e1s * dt
+    if prop.startswith("taylor"):
+        p = int(prop[6:]); psi, _ = oracle.step_taylor(g, off, psi0, p, 0.0, dt, n); R = trunc(z, p)
+    elif prop == "rk4":
+        psi, _ = oracle.step_rk4(g, off, psi0, 0.0, dt, n); R = trunc(z, 4)
+    elif prop == "dp5":
+        psi, _, _ = oracle.step_rk_fixed(g, off, psi0, 1, 0.0, dt, n); R = trunc(z, 5) + z ** 6 / 600
+    else:
+        psi, _ = oracle.step_lanczos(g, off, psi0, 16, 12, 0.0, dt, n); R = trunc(z, 12)
+    amp = dr * np.sum(phi[0] * psi[0, 0])
+    assert abs(amp - R ** n) < 1e-12
+    assert abs(amp - np.exp(-1j * e1s * dt * n)) < 1e-6          # e^{-i E0 t} phase (NS)
+    obs = oracle.observables(g, psi, 0.0, ([0], phi[:1]))
+    assert abs(obs[0, 0] - abs(R) ** (2 * n)) < 1e-12            # norm = |R|^{2n}
+    assert abs(obs[0, 3] - abs(R) ** (2 * n)) < 1e-12            # 1s population
+    assert np.all(np.abs(psi[0, 1:]) < 1e-300)                   # no field: other blocks stay empty
+
+
+# ---------------------------------------------------------------- time-dependent H: order of convergence
+def _td_reference(g, pulse, psi, t0, t1, n):
+    """Independent reference for time-dependent H: product of dense midpoint exponentials, Richardson-extrapolated."""
+    def run(m):
+        v = psi.reshape(-1).copy()
+        dt = (t1 - t0) / m
+        h0 = oracle.dense_H(g, 0.0)
+        h1 = oracle.dense_H(g, 1.0) - h0
+        for k in range(m):
+            e = oracle.pulse_E(pulse, t0 + (k + 0.5) * dt)
+            v = dense_propagate(h0 + e * h1, v, dt)
+        return v
+    a, b = run(n), run(2 * n)
+    return (4 * b - a) / 3                                       # midpoint rule is O(dt^2)
+
+
+def test_time_dependent_convergence_orders():
+    g = oracle.make_grid(40, 0.4, 3, 3)                            # small so that dense references are cheap
+    pulse = (0.3, 1.5, 2.0, 0.3)                                   # strong, fast pulse: time dependence matters
+    t0, t1 = 1.0, 3.0
+    psi = rand_state((1, 3, 40), 31); psi /= np.linalg.norm(psi)
+    ref = _td_reference(g, pulse, psi, t0, t1, 400)
+    def err(fn, n):
+        return np.linalg.norm(fn(n).reshape(-1) - ref)
+    rk4 = lambda n: oracle.step_rk4(g, pulse, psi, t0, (t1 - t0) / n, n)[0]
+    dp5 = lambda n: oracle.step_rk_fixed(g, pulse, psi, 1, t0, (t1 - t0) / n, n)[0]
+    tay = lambda n: oracle.step_taylor(g, pulse, psi, 8, t0, (t1 - t0) / n, n)[0]
+    lan = lambda n: oracle.step_lanczos(g, pulse, psi, 12, 12, t0, (t1 - t0) / n, n)[0]
+    tay_start = lambda n: oracle.step_taylor(g, pulse, psi, 8, t0, (t1 - t0) / n, n, field_sample=1)[0]
+    e1, e2 = err(rk4, 400), err(rk4, 800)
+    assert 14 < e1 / e2 < 18, (e1, e2)                           # 4th order: pins the stage times c_i
+    e1, e2 = err(dp5, 200), err(dp5, 400)
+    assert 27 < e1 / e2 < 37, (e1, e2)                           # 5th order
+    for fn in (tay, lan):                                        # midpoint-frozen H: 2nd order
+        e1, e2 = err(fn, 400), err(fn, 800)
+        assert 3.8 < e1 / e2 < 4.2, (e1, e2)
+    e1, e2 = err(tay_start, 400), err(tay_start, 800)
+    assert 1.9 < e1 / e2 < 2.1                                   # start-frozen H: 1st order
+    assert err(dp5, 800) < 1e-7 and err(rk4, 800) < 1e-6
+
+
+# ---------------------------------------------------------------- RK45 controller
+def test_rk45_controller_and_replay():
+    g = oracle.make_grid(200, 0.2, 4, 5)
+    pulse = (0.05, 0.057, 2.0, 0.0)
+    en, phi = oracle.bound_states(g, 0, 1)
+    psi0 = np.zeros((1, 4, 200), dtype=complex); psi0[0, 0] = phi[0]
+    t0, t1 = 100.0, 101.0
+    psi, info = oracle.step_rk45(g, pulse, psi0, t0, t1, 1e-4, 1e-8)
+    assert info["n_accept"] == len(info["dt"]) and info["n_accept"] > 10
+    assert abs(np.sum(info["dt"]) - (t1 - t0)) < 1e-12          # lands on t_end
+    assert np.all(info["err"] <= 1.0)
+    assert np.all(info["dt"][1:] <= 5.0 * info["dt"][:-1] * (1 + 1e-12))
+    # replaying the accepted steps reproduces the state bit for bit and never exceeds err 1
+    psi_r, info_r = oracle.step_rk45(g, pulse, psi0, t0, t1, 1e-4, 1e-8, dt_replay=info["dt"])
+    assert np.array_equal(psi_r, psi)
+    assert np.allclose(info_r["err"], info["err"], rtol=1e-12)
+    # against a fine fixed-step RK4 run: error ~ n_accept * rtol (tolerance is per step)
+    n = 40000
+    ref, _ = oracle.step_rk4(g, pulse, psi0, t0, (t1 - t0) / n, n)
+    assert np.linalg.norm(psi - ref) < 5 * info["n_accept"] * 1e-8
+    # dt_max caps every step
+    _, info_c = oracle.step_rk45(g, pulse, psi0, t0, t1, 1e-4, 1e-8, dt_max=2e-3)
+    assert np.max(info_c["dt"]) <= 2e-3 * (1 + 1e-15)
+    # fixed-step DP5 reports the same error estimate as the adaptive call's first step
+    _, err, _ = oracle.step_rk_fixed(g, pulse, psi0, 1, t0, 1e-4, 1)
+    assert abs(err[0] / 1e-8 - info["err"][0]) < 1e-9 * info["err"][0] + 1e-30
+
+
+# ---------------------------------------------------------------- observables
+def test_observables_textbook_matrix_elements():
+    """<z> and <z''> of a 1s + 2p0 superposition of analytic hydrogen functions against the textbook integrals."""
+    gold = {k: float(v) for k, v in read_golden("hydrogen_matrix_elements.txt")}
+    dr, n_r = 0.01, 6000
+    g = oracle.make_grid(n_r, dr, 3, 3)
+    r = dr * np.arange(1, n_r + 1)
+    u1s, u2p = wl.hydrogen_u(1, 0, r), wl.hydrogen_u(2, 1, r)
+    a, b = 0.8, 0.6 * np.exp(0.4j)
+    psi = np.zeros((1, 3, n_r), dtype=complex); psi[0, 0] = a * u1s; psi[0, 1] = b * u2p
+    e_now = 0.0123
+    obs = oracle.observables(g, psi, e_now, ([0, 1, 2], np.stack([u1s, u2p, wl.hydrogen_u(3, 2, r)])))
+    re_ab = (np.conj(a) * b).real
+    assert abs(obs[0, 0] - 1.0) < 1e-6                                    # norm
+    assert abs(obs[0, 1] - 2 * re_ab * gold["z_1s_2p"]) < 1e-6            # P:294 Eq. 34
+    assert abs(obs[0, 2] - (-e_now - 2 * re_ab * gold["acc_1s_2p"])) < 1e-5   # P:302 Eq. 36
+    assert abs(obs[0, 3] - 0.64) < 1e-6 and abs(obs[0, 4] - 0.36) < 1e-6   # P:227 Eq. 25 (|.|^2)
+    assert obs[0, 5] < 1e-20
+    # Z scales the acceleration's Coulomb term (R-G14)
+    g2 = oracle.make_grid(n_r, dr, 3, 3, z_nuc=2.0)
+    obs2 = oracle.observables(g2, psi, e_now)
+    assert abs((obs2[0, 2] + e_now) - 2 * (obs[0, 2] + e_now)) < 1e-12
+    # batch rows are independent
+    g3 = oracle.make_grid(n_r, dr, 3, 3, batch=2)
+    two = np.concatenate([psi, 0.5 * psi])
+    o3 = oracle.observables(g3, two, [e_now, 0.0])
+    assert abs(o3[1, 0] - 0.25 * obs[0, 0]) < 1e-15 and abs(o3[0, 1] - obs[0, 1]) < 1e-15
+
+
+# ---------------------------------------------------------------- P7: first-order perturbation theory
+def test_P7_resonant_1s_2p_perturbation_theory():
+    dr, n_r = 0.2, 500
+    g = oracle.make_grid(n_r, dr, 3, 3)
+    e1s, p1s = oracle.bound_states(g, 0, 1)
+    e2p, p2p = oracle.bound_states(g, 1, 1)
+    om = e2p[0] - e1s[0]
+    assert abs(om - 0.369992762914) < 1e-9
+    r = dr * np.arange(1, n_r + 1)
+    d = (1 / math.sqrt(3)) * dr * np.sum(p2p[0] * r * p1s[0])    # textbook c_0 = 1/sqrt 3
+    nc = 10.0
+    T = 2 * math.pi * nc / om
+    nsteps = int(round(T / 0.0035))
+    dt = T / nsteps
+    psi0 = np.zeros((1, 3, n_r), dtype=complex); psi0[0, 0] = p1s[0]
+    res = {}
+    for e0 in (1e-4, 1e-3):
+        pulse = (e0, om, nc, 0.0)
+        psi, _ = oracle.step_taylor(g, pulse, psi0, 4, 0.0, dt, nsteps)
+        pop = oracle.observables(g, psi, 0.0, ([0, 1], np.stack([p1s[0], p2p[0]])))[0, 4]
+        t = np.linspace(0, T, 400001)
+        et = e0 * np.sin(om * t / (2 * nc)) ** 2 * np.cos(om * t)   # independent quadrature of the pulse
+        pt = d * d * abs(np.trapezoid(et * np.exp(1j * om * t), t)) ** 2
+        res[e0] = (pop - pt) / pt
+    assert abs(res[1e-4]) < 1e-5, res
+    assert 50 < res[1e-3] / res[1e-4] < 200, res                    # deviation is the E0^2 correction
+
+
+# ---------------------------------------------------------------- P8 / P10: Ehrenfest, norm conservation
+def test_P8_ehrenfest_and_P10_norm():
+    c = wl.config("cfg1", n_l=4)
+    g = oracle.make_grid(c["n_r"], c["dr"], c["n_l"], c["fd_order"])
+    en, phi = oracle.bound_states(g, 0, 1)
+    psi0 = wl.ground_state(c, phi[0])
+    pulse = wl.pulses(c)[0]
+    dt = wl.dt_eff(c)
+    t0 = 0.25 * c["t_pulse"]
+    n = 6000
+    psi, obs = oracle.step_taylor(g, pulse, psi0, 4, t0, dt, n, states=([0], phi[:1]), obs_every=1)
+    norm, z, acc = obs[:, 0, 0], obs[:, 0, 1], obs[:, 0, 2]
+    assert np.max(np.abs(norm - 1)) < 1e-11                        # P10
+    s = 50                                                         # second difference on a coarser stride
+    zz = z[::s]
+    d2 = (zz[2:] - 2 * zz[1:-1] + zz[:-2]) / (s * dt) ** 2
+    a = acc[::s][1:-1]
+    assert np.max(np.abs(d2 - a)) < 0.02 * np.max(np.abs(a))      # P8 (soft): signs/factors of Eq. 34/36
+    assert np.max(np.abs(a)) > 1e-3
