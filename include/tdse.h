@@ -1,0 +1,138 @@
+/*
+ * tdse.h -- C ABI of the B200-native TDSE hot path (libtdse_b200.so).
+ *
+ * Method: O Broin & Nikolopoulos, "A GPGPU based program to solve the TDSE in intense laser
+ * fields through the finite difference approach" (arXiv:1308.1856).  P:<n> below is line n of the
+ * paper text; readings of garbled or silent passages are R-* in DESIGN.md.
+ *
+ * What the library does: applies the matrix-free finite-difference Hamiltonian
+ *     (H f)_{l,j} = -1/2 D2 f_l |_j + [ l(l+1)/(2 r_j^2) - Z/r_j ] f_{l,j}
+ *                   + E(t) r_j [ c_{l-1} f_{l-1,j} + c_l f_{l+1,j} ]                 (Eq. 11, Eq. 7)
+ * with D2 the 3-point or the 5-point (Eq. 15) second difference, c_l = (l+1)/sqrt((2l+1)(2l+3))
+ * (Eq. 9 at m = 0), r_j = j*dr, j = 1..n_r, f = 0 outside the index box, and advances
+ * i dF/dt = H(t) F (Eq. 17) with the paper's propagators.  Every step runs in CUDA kernels for
+ * sm_100a; there is no CPU fallback: without a CUDA device every compute entry point returns
+ * TDSE_ERR_CUDA.
+ *
+ * Data layout.  A state is psi[b][l][j-1]: b = 0..batch-1 independent members, l = 0..n_l-1
+ * partial waves (block-contiguous in r), complex128 stored as interleaved (re, im) doubles,
+ * 16-byte aligned.  "dev" pointers are CUDA device pointers owned by the caller (e.g. torch tensors);
+ * "host" pointers are ordinary host memory owned by the caller, only touched during the call.
+ *
+ * Streams.  `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Work is
+ * enqueued asynchronously on it unless the call returns data to the host, in which case the call
+ * synchronises that stream before returning.
+ *
+ * Errors.  Every function returns 0 (TDSE_OK) or a negative code; no exceptions cross the ABI, nothing
+ * aborts, and the handle stays valid after an error.
+ */
+#ifndef TDSE_B200_H
+#define TDSE_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TDSE_OK               0
+#define TDSE_ERR_ARG         (-1)   /* null pointer, non-positive size, order < 1, ...           */
+#define TDSE_ERR_ALLOC       (-2)   /* host or device allocation failed                           */
+#define TDSE_ERR_CUDA        (-3)   /* CUDA runtime error (no device, launch failure)             */
+#define TDSE_ERR_NONFINITE   (-4)   /* a logged norm is NaN/Inf (unstable step size)       */
+#define TDSE_ERR_UNSUPPORTED (-5)   /* gauge != length, fd_order not 3/5, krylov_dim > 32         */
+
+typedef struct tdse_handle tdse_handle;   /* opaque; owns the state, all scratch, tables and CUDA graphs */
+
+typedef struct {
+    int    n_r;       /* radial points N_r; r_j = j*dr, j = 1..n_r (reading R-G1)          */
+    double dr;        /* radial spacing                                                           */
+    int    n_l;       /* number of partial-wave blocks L, l = 0..n_l-1 (`NumBlocks`)       */
+    int    fd_order;  /* 3 or 5 point second derivative (Eq. 15)                            */
+    int    gauge;     /* 0 = length gauge (Eq. 11); anything else: TDSE_ERR_UNSUPPORTED     */
+    double z_nuc;     /* V(r) = -z_nuc/r                                                   */
+    int    batch;     /* B >= 1 independent members sharing the grid                      */
+} tdse_grid;
+
+typedef struct {      /* E(t) = e0 sin^2(omega t/(2 n_cycles)) cos(omega t + cep) on 0 <= t <= 2 pi n_cycles/omega, */
+    double e0, omega, n_cycles, cep;   /* else 0 (Eq. 19; R-G8).  omega == 0: static field e0 */
+} tdse_pulse;
+
+/* Create / destroy.  tdse_create builds the device tables (diagonal of h_l, c_l) and allocates the state
+ * (zero-initialised).  Survives repeated create/destroy cycles (the paper's program was not tested for
+ * that). */
+int  tdse_create (const tdse_grid *grid, tdse_handle **out);
+void tdse_destroy(tdse_handle *h);
+
+/* Options (all default to the value in brackets):
+ *   "field_sample"     [0] 0: H frozen at t_n + dt/2 in Taylor/Lanczos steps, 1: at t_n (R-G7)
+ *   "use_graph"        [1] capture blocks of steps in a CUDA graph
+ *   "graph_steps"      [16] steps per captured graph
+ *   "taylor_block"     [1] 0: one kernel per Taylor order; 1: temporally blocked kernel when the
+ *                          tile fits shared memory (all n_l rows resident), else falls back to 0
+ *   "lanczos_beta_tol" [1e-12] breakdown threshold on beta ("if beta = 0 then quit", R-G17)
+ *   "rk45_dt_max"      [0 = none] cap on the adaptive step
+ *   "rk45_check_every" [8] attempted steps enqueued between host checks of the device `done` flag */
+int  tdse_set_option(tdse_handle *h, const char *key, double value);
+
+/* One pulse per member, host array [batch]. */
+int  tdse_set_pulse(tdse_handle *h, const tdse_pulse *per_member_host);
+
+/* Real bound-state vectors for the population observable p_s = |dr sum_j phi_s[j] f_{l_s,j}|^2
+ * (Eq. 25 with the modulus squared, R-G12).  l_of_state: host [n_states]; phi: host [n_states][n_r]. */
+int  tdse_set_bound_states(tdse_handle *h, int n_states, const int *l_of_state, const double *phi);
+
+/* Copy the whole state [batch][n_l][n_r] complex128 in / out.  is_device = 0: host pointer (the call
+ * synchronises `stream`), 1: device pointer (asynchronous on `stream`). */
+int  tdse_set_state(tdse_handle *h, const void *psi, int is_device, void *stream);
+int  tdse_get_state(tdse_handle *h, void *psi, int is_device, void *stream);
+
+/* out = H(E) psi for caller-owned device arrays (must not alias); e_field_host: host [batch], the field
+ * value each member sees (Eq. 11).  Asynchronous on `stream`. */
+int  tdse_apply_H(tdse_handle *h, const void *psi_dev, void *out_dev, const double *e_field_host, void *stream);
+
+/* Propagators.  All advance the handle's state in place over nsteps steps of size dt starting at t0;
+ * member b sees pulse b.  If obs_every > 0 an observable row block is logged after every obs_every-th
+ * step (evaluated at t_{n+1}); the log restarts at row 0 on every call.  Asynchronous on `stream`.
+ *   taylor : F_{n+1} = sum_{k=0..order} F^(k), F^(k) = (-i dt/k) H F^(k-1)         (Eq. 37, R-G6)
+ *   rk4    : classic Runge-Kutta through the stage loop of P:462 Eq. 38 / P:469-478
+ *   lanczos: Krylov basis by the three-term recurrence, c = exp(-i T dt) e_1 by a (sub-stepped) Taylor
+ *            series of order taylor_order on the tridiagonal T, F_{n+1} = ||F|| sum_p c_p q_p
+ *            (App. B, R-C5); krylov_dim <= 32. */
+int  tdse_step_taylor (tdse_handle *h, int order, double t0, double dt, long nsteps, int obs_every, void *stream);
+int  tdse_step_rk4    (tdse_handle *h, double t0, double dt, long nsteps, int obs_every, void *stream);
+int  tdse_step_lanczos(tdse_handle *h, int krylov_dim, int taylor_order, double t0, double dt, long nsteps,
+                       int obs_every, void *stream);
+
+/* Embedded Dormand-Prince 5(4) (named P:796; error estimate P:813-833; the adaptive controller is ours,
+ * R-C4, the paper's is "not implemented"): err = max_b ||Delta_b||_2 / (rtol ||psi_new,b||_2), accept iff
+ * err <= 1, dt_next = dt clamp(0.9 err^(-1/5), 0.2, 5) (<= 1 right after a reject), last step clipped to t_end,
+ * FSAL.  If dt_replay != NULL (host [n_replay]) exactly those steps are taken, all accepted.
+ * Synchronises `stream`; n_accept / n_reject may be NULL. */
+int  tdse_step_rk45(tdse_handle *h, double t0, double t_end, double dt_init, double rtol,
+                    const double *dt_replay, long n_replay, long *n_accept, long *n_reject, void *stream);
+
+/* Observable row of member b: { norm, <z>, <z''>, pop[0..n_states-1] }:
+ *   norm = dr sum |f|^2;  <z> = 2 dr sum_l c_l sum_j r_j Re(conj f_{l,j} f_{l+1,j})          (Eq. 34)
+ *   <z''> = -E(t) - 2 Z dr sum_l c_l sum_j r_j^-2 Re(conj f_{l,j} f_{l+1,j})                  (Eq. 36)
+ * tdse_observables: current state, field taken at time t; out_host: [batch][3 + n_states]; synchronises. */
+int  tdse_observables(tdse_handle *h, double t, double *out_host, void *stream);
+/* Rows logged by the last step call: out_host [rows][batch][3+n_states]; at most max_rows row blocks are
+ * copied, *rows = number logged.  Synchronises the device.  TDSE_ERR_NONFINITE if a logged norm is not finite. */
+int  tdse_obs_log(tdse_handle *h, double *out_host, long max_rows, long *rows);
+/* Accepted step sizes (and their err values; err_host may be NULL) of the last tdse_step_rk45 call. */
+int  tdse_dt_log(tdse_handle *h, double *dt_host, double *err_host, long max, long *n);
+/* Krylov data of the LAST Lanczos step: alpha, beta host [batch][krylov_dim]; coef host [batch][krylov_dim]
+ * complex (re, im); m_used, n_sub host [batch] (dimension used after breakdown, Taylor sub-steps). Any may be NULL. */
+int  tdse_lanczos_info(tdse_handle *h, double *alpha, double *beta, double *coef, int *m_used, int *n_sub);
+
+/* Number of CUDA kernels this handle has launched so far (graph nodes counted per graph launch). */
+long tdse_launch_count(tdse_handle *h);
+/* Shared-memory-resident temporally blocked Taylor kernel: 1 if the last tdse_step_taylor call used it. */
+int  tdse_taylor_was_blocked(tdse_handle *h);
+
+const char *tdse_strerror(int code);
+const char *tdse_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,793 @@
+// tdse_api.cu -- host side of libtdse_b200: the C ABI of include/tdse.h, buffer ownership, the time loops
+// (CUDA-graph captured blocks of steps) and the launch sequences of every propagator.
+// Product path: there is no CPU fallback; without a CUDA device every compute entry point fails loudly.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <new>
+#include <string>
+#include <tuple>
+#include <vector>
+
+#include "tdse_kernels.cuh"
+#include "tdse_taylor_blocked.cuh"
+
+using namespace tdse;
+
+#define CU(call)                                                            \
+    do {                                                                    \
+        cudaError_t e_ = (call);                                            \
+        if (e_ != cudaSuccess) {                                            \
+            h->last_cuda = e_;                                              \
+            return (e_ == cudaErrorMemoryAllocation) ? TDSE_ERR_ALLOC : TDSE_ERR_CUDA; \
+        }                                                                   \
+    } while (0)
+
+#define RC(call)                     \
+    do {                             \
+        int rc_ = (call);            \
+        if (rc_ != TDSE_OK) return rc_; \
+    } while (0)
+
+namespace {
+enum Role { R_PSI = 0, R_G0 = 1, R_G1 = 2, R_K0 = 3 };
+
+// Butcher tableaux (P:796-797 names them; coefficients: classic RK4 and Dormand & Prince 1980, R-C4)
+const double RK4_A[4][4] = {{0, 0, 0, 0}, {0.5, 0, 0, 0}, {0, 0.5, 0, 0}, {0, 0, 1.0, 0}};
+const double RK4_B[4] = {1.0 / 6, 1.0 / 3, 1.0 / 3, 1.0 / 6};
+const double DP_A[7][7] = {
+    {0, 0, 0, 0, 0, 0, 0},
+    {1.0 / 5, 0, 0, 0, 0, 0, 0},
+    {3.0 / 40, 9.0 / 40, 0, 0, 0, 0, 0},
+    {44.0 / 45, -56.0 / 15, 32.0 / 9, 0, 0, 0, 0},
+    {19372.0 / 6561, -25360.0 / 2187, 64448.0 / 6561, -212.0 / 729, 0, 0, 0},
+    {9017.0 / 3168, -355.0 / 33, 46732.0 / 5247, 49.0 / 176, -5103.0 / 18656, 0, 0},
+    {35.0 / 384, 0, 500.0 / 1113, 125.0 / 192, -2187.0 / 6784, 11.0 / 84, 0}};
+const double DP_B[7] = {35.0 / 384, 0, 500.0 / 1113, 125.0 / 192, -2187.0 / 6784, 11.0 / 84, 0};
+const double DP_BH[7] = {5179.0 / 57600, 0, 7571.0 / 16695, 393.0 / 640, -92097.0 / 339200, 187.0 / 2100, 1.0 / 40};
+}  // namespace
+
+struct tdse_handle {
+    tdse_grid grid{};
+    GridDev gd{};
+    size_t n_state = 0;                 // complex elements per state vector (B*L*N)
+    cudaError_t last_cuda = cudaSuccess;
+    // options
+    int field_sample = 0, use_graph = 1, graph_steps = 16, taylor_block = 1, rk45_check_every = 8;
+    double beta_tol = 1e-12, rk45_dt_max = 0.0;
+    // device tables
+    double *d_vj = nullptr, *d_cen = nullptr, *d_cl = nullptr;
+    tdse_pulse *d_pulse = nullptr;
+    // state vector pool; pool[psi_slot] is the state
+    std::vector<double2 *> pool;
+    int psi_slot = 0;
+    double2 **d_bufs = nullptr;         // device copy of the role -> pointer table (RK)
+    int role_slot[kRkRoles];
+    // control, fields, reductions
+    Ctl *d_ctl = nullptr;
+    double *d_etab = nullptr; size_t etab_cap = 0;
+    double *d_eapply = nullptr; std::vector<double> eapply_host; bool eapply_valid = false;
+    double *d_partials = nullptr; size_t partials_cap = 0;
+    unsigned int *d_counter = nullptr;
+    // observables
+    int n_states = 0; double *d_phi = nullptr; int *d_lstate = nullptr;
+    double *d_obs_partials = nullptr; double2 *d_amp = nullptr;
+    double *d_rows = nullptr; size_t rows_cap = 0; long log_rows = 0; double *d_row_direct = nullptr;
+    // rk45 logs
+    double *d_dtlog = nullptr, *d_errlog = nullptr, *d_replay = nullptr; long log_cap = 0, replay_cap = 0;
+    long last_accept = 0;
+    // lanczos scalars
+    int lz_K = 0; double *d_alpha = nullptr, *d_beta = nullptr, *d_nrm = nullptr, *d_inv = nullptr;
+    double2 *d_coef = nullptr; int *d_m = nullptr, *d_nsub = nullptr; double2 *d_basis = nullptr;
+    // graphs
+    cudaStream_t cap_stream = nullptr;
+    std::map<std::tuple<int, int, int, int, int, int>, cudaGraphExec_t> graphs;
+    std::map<std::tuple<int, int, int, int, int, int>, long> graph_nodes;
+    long launches = 0; long pending = 0; bool capturing = false;
+    int taylor_blocked_last = 0;
+    // blocked Taylor configuration
+    BlockedCfg bcfg{};
+};
+
+namespace {
+
+inline void count(tdse_handle *h) { ++h->pending; }
+
+void free_graphs(tdse_handle *h) {
+    for (auto &kv : h->graphs) cudaGraphExecDestroy(kv.second);
+    h->graphs.clear();
+    h->graph_nodes.clear();
+}
+
+int ensure_pool(tdse_handle *h, int n) {
+    while ((int)h->pool.size() < n) {
+        double2 *p = nullptr;
+        CU(cudaMalloc(&p, h->n_state * sizeof(double2)));
+        CU(cudaMemset(p, 0, h->n_state * sizeof(double2)));
+        h->pool.push_back(p);
+    }
+    return TDSE_OK;
+}
+
+template <class T>
+int ensure_buf(tdse_handle *h, T **p, size_t *cap, size_t need) {
+    if (*cap >= need && *p) return TDSE_OK;
+    if (*p) { cudaDeviceSynchronize(); cudaFree(*p); *p = nullptr; free_graphs(h); }
+    CU(cudaMalloc(p, need * sizeof(T)));
+    CU(cudaMemset(*p, 0, need * sizeof(T)));
+    *cap = need;
+    return TDSE_OK;
+}
+
+dim3 tile_grid(const tdse_handle *h) {
+    const int tw = 128, tl = 8;
+    return dim3((h->grid.n_r + tw - 1) / tw, (h->grid.n_l + tl - 1) / tl, h->grid.batch);
+}
+int tile_ctas_per_member(const tdse_handle *h) { dim3 g = tile_grid(h); return (int)(g.x * g.y); }
+long long pts_per_member(const tdse_handle *h) { return (long long)h->grid.n_l * h->grid.n_r; }
+dim3 ew_grid(const tdse_handle *h) {
+    return dim3((unsigned)((pts_per_member(h) + EW_CHUNK - 1) / EW_CHUNK), 1, h->grid.batch);
+}
+
+template <class Epi>
+int launch_tile(tdse_handle *h, const Epi &epi, cudaStream_t s) {
+    RedCtx rc{h->d_partials, h->d_counter, tile_ctas_per_member(h)};
+    if (h->grid.fd_order == 3) tile_kernel<3, Epi><<<tile_grid(h), 256, 0, s>>>(h->gd, epi, rc);
+    else tile_kernel<5, Epi><<<tile_grid(h), 256, 0, s>>>(h->gd, epi, rc);
+    count(h);
+    CU(cudaGetLastError());
+    return TDSE_OK;
+}
+
+template <class Op>
+int launch_ew(tdse_handle *h, const Op &op, cudaStream_t s) {
+    dim3 g = ew_grid(h);
+    RedCtx rc{h->d_partials, h->d_counter, (int)g.x};
+    ew_kernel<Op><<<g, EW_NT, 0, s>>>(pts_per_member(h), h->grid.batch, op, rc);
+    count(h);
+    CU(cudaGetLastError());
+    return TDSE_OK;
+}
+
+int obs_chunks(const tdse_handle *h) { return (h->grid.n_r + 255) / 256; }
+
+// Observable kernels for the state `psi`; logged row (predicated on the device step counter) or direct.
+int enqueue_obs(tdse_handle *h, const double2 *psi, int step_off, int predicated, int use_direct, double t_direct,
+                double *rows, cudaStream_t s) {
+    const int B = h->grid.batch;
+    obs_main_kernel<<<dim3(obs_chunks(h), B), 256, 0, s>>>(h->gd, psi, h->d_ctl, step_off, predicated,
+                                                             h->d_obs_partials);
+    count(h);
+    if (h->n_states > 0) {
+        obs_pop_kernel<<<dim3(h->n_states, B), 128, 0, s>>>(h->gd, psi, h->d_phi, h->d_lstate, h->n_states, h->d_ctl,
+                                                             step_off, predicated, h->d_amp);
+        count(h);
+    }
+    obs_final_kernel<<<B, 128, 0, s>>>(h->gd, h->d_obs_partials, obs_chunks(h), h->d_amp, h->n_states, h->d_pulse,
+                                       h->d_ctl, step_off, predicated, use_direct, t_direct, rows);
+    count(h);
+    CU(cudaGetLastError());
+    return TDSE_OK;
+}
+
+int ensure_rows(tdse_handle *h, long nsteps, int obs_every) {
+    const size_t W = 3 + h->n_states;
+    size_t need = (size_t)h->grid.batch * W;
+    if (obs_every > 0) need *= (size_t)std::max(1L, nsteps / obs_every);
+    return ensure_buf(h, &h->d_rows, &h->rows_cap, need);
+}
+
+int init_ctl(tdse_handle *h, const CtlInit &v, cudaStream_t s) {
+    ctl_init_kernel<<<1, 32, 0, s>>>(h->d_ctl, v);
+    count(h);
+    CU(cudaGetLastError());
+    return TDSE_OK;
+}
+
+// ---- blocks of steps --------------------------------------------------------------------------------
+// Each enqueue_* function enqueues `n` consecutive steps (reading t0, dt and the step counter from the device
+// control block) and ends by advancing the counter; it is either captured into a graph or run eagerly.
+
+int enqueue_taylor_block(tdse_handle *h, int order, int n, int obs, cudaStream_t s) {
+    const int B = h->grid.batch;
+    field_table_kernel<<<(n * B + 255) / 256, 256, 0, s>>>(h->d_ctl, h->d_pulse, B, n, 0, h->d_etab);
+    count(h);
+    double2 *psi = h->pool[h->psi_slot];
+    // scratch: three further pool slots
+    int sl[3], c = 0;
+    for (int i = 0; c < 3; ++i) if (i != h->psi_slot) sl[c++] = i;
+    double2 *ta = h->pool[sl[0]], *tb = h->pool[sl[1]], *acc = h->pool[sl[2]];
+    for (int i = 0; i < n; ++i) {
+        const double *ef = h->d_etab + (size_t)i * B;
+        if (h->taylor_blocked_last) {
+            // ping-pong psi <-> acc: even steps read psi, odd steps read acc (n is even inside graphs)
+            double2 *src = (i & 1) ? acc : psi, *dst = (i & 1) ? psi : acc;
+            RC(launch_taylor_blocked(h->bcfg, h->gd, src, dst, ef, &h->d_ctl->dt, order, s));
+            count(h);
+            if (obs) RC(enqueue_obs(h, dst, i, 1, 0, 0.0, h->d_rows, s));
+            continue;
+        }
+        for (int k = 1; k <= order; ++k) {
+            EpiTaylor e{};
+            e.in = (k == 1) ? psi : ((k & 1) ? tb : ta);       // term_{k-1}: k-1 odd -> ta, even -> tb
+            e.ef = ef; e.dtp = &h->d_ctl->dt; e.k = k; e.first = (k == 1); e.write_term = (k < order);
+            e.term_out = (k & 1) ? ta : tb;
+            e.acc_in = acc;
+            e.acc_out = (k == order && order > 1) ? psi : acc;  // the last order reads acc point-wise: write psi in place
+            RC(launch_tile(h, e, s));
+        }
+        if (order == 1) {
+            OpCopy cp{}; cp.dst = psi; cp.src = acc;
+            RC(launch_ew(h, cp, s));
+        }
+        if (obs) RC(enqueue_obs(h, psi, i, 1, 0, 0.0, h->d_rows, s));
+    }
+    if (h->taylor_blocked_last && (n & 1)) {   // odd eager remainder: bring the state back into the psi slot
+        OpCopy cp{}; cp.dst = psi; cp.src = acc;
+        RC(launch_ew(h, cp, s));
+    }
+    ctl_advance_kernel<<<1, 32, 0, s>>>(h->d_ctl, n);
+    count(h);
+    CU(cudaGetLastError());
+    return TDSE_OK;
+}
+
+void rk_roles(tdse_handle *h) {
+    // role r lives in pool slot: PSI -> psi_slot, the others in increasing slot order
+    int c = 0;
+    for (int r = 0; r < kRkRoles; ++r) {
+        if (r == R_PSI) { h->role_slot[r] = h->psi_slot; continue; }
+        if (c == h->psi_slot) ++c;
+        h->role_slot[r] = c++;
+    }
+}
+
+int upload_bufs(tdse_handle *h, int n_roles, cudaStream_t s) {
+    std::vector<double2 *> tab(kRkRoles, nullptr);
+    for (int r = 0; r < n_roles; ++r) tab[r] = h->pool[h->role_slot[r]];
+    CU(cudaMemcpyAsync(h->d_bufs, tab.data(), sizeof(double2 *) * kRkRoles, cudaMemcpyHostToDevice, s));
+    CU(cudaStreamSynchronize(s));   // tab is a stack object
+    return TDSE_OK;
+}
+
+template <bool EMBED>
+void fill_rk_common(tdse_handle *h, EpiRK<EMBED> &e, int stage, const double *ef, const double *hptr) {
+    e.ctl = h->d_ctl; e.bufs = h->d_bufs; e.ef = ef; e.hptr = hptr; e.stage = stage;
+    e.psi_role = R_PSI;
+    for (int j = 0; j < 7; ++j) { e.k_role[j] = -1; e.a_next[j] = 0.0; e.d_err[j] = 0.0; }
+    e.check_done = 0; e.dt_log = h->d_dtlog; e.err_log = h->d_errlog;
+}
+
+int enqueue_rk4_block(tdse_handle *h, int n, int obs, cudaStream_t s) {
+    const int B = h->grid.batch;
+    field_table_kernel<<<(n * 4 * B + 255) / 256, 256, 0, s>>>(h->d_ctl, h->d_pulse, B, n, 1, h->d_etab);
+    count(h);
+    double2 *psi = h->pool[h->psi_slot];
+    for (int i = 0; i < n; ++i) {
+        for (int st = 0; st < 4; ++st) {
+            EpiRK<false> e{};
+            fill_rk_common(h, e, st, h->d_etab + ((size_t)i * 4 + st) * B, &h->d_ctl->dt);
+            e.in_role = (st == 0) ? R_PSI : ((st & 1) ? R_G1 : R_G0);      // stage st reads what stage st-1 wrote
+            for (int j = 0; j < 3; ++j) e.k_role[j] = R_K0 + j;
+            if (st < 3) {
+                e.store_k = 1;
+                e.out_role = ((st + 1) & 1) ? R_G1 : R_G0;
+                for (int j = 0; j <= st; ++j) e.a_next[j] = RK4_A[st + 1][j];
+            } else {
+                e.store_k = 0;
+                e.out_role = R_PSI;                                         // psi is read point-wise only: in place
+                for (int j = 0; j < 4; ++j) e.a_next[j] = RK4_B[j];
+            }
+            RC(launch_tile(h, e, s));
+        }
+        if (obs) RC(enqueue_obs(h, psi, i, 1, 0, 0.0, h->d_rows, s));
+    }
+    ctl_advance_kernel<<<1, 32, 0, s>>>(h->d_ctl, n);
+    count(h);
+    CU(cudaGetLastError());
+    return TDSE_OK;
+}
+
+// Dormand-Prince stages [first_stage, 7) of `n` attempted steps; every kernel exits at once when ctl->done.
+int enqueue_rk45_block(tdse_handle *h, int n, int first_stage, cudaStream_t s) {
+    const int B = h->grid.batch;
+    for (int i = 0; i < n; ++i) {
+        rk45_begin_kernel<<<1, 256, 0, s>>>(h->d_ctl, h->d_pulse, B, h->d_replay, h->d_etab);
+        count(h);
+        for (int st = (i == 0 ? first_stage : 1); st < 7; ++st) {
+            const double *ef = h->d_etab + (size_t)st * B;
+            if (st < 6) {
+                EpiRK<false> e{};
+                fill_rk_common(h, e, st, ef, &h->d_ctl->h);
+                e.check_done = 1;
+                e.in_role = (st == 0) ? R_PSI : ((st & 1) ? R_G1 : R_G0);
+                for (int j = 0; j < 7; ++j) e.k_role[j] = R_K0 + j;
+                e.store_k = 1;
+                e.out_role = ((st + 1) & 1) ? R_G1 : R_G0;
+                for (int j = 0; j <= st; ++j) e.a_next[j] = DP_A[st + 1][j];
+                RC(launch_tile(h, e, s));
+            } else {
+                EpiRK<true> e{};
+                fill_rk_common(h, e, st, ef, &h->d_ctl->h);
+                e.check_done = 1;
+                e.in_role = R_G0;                                           // stage 5 wrote psi_new = g_7 into G0
+                for (int j = 0; j < 7; ++j) e.k_role[j] = R_K0 + j;
+                e.store_k = 1;
+                e.out_role = -1;
+                for (int j = 0; j < 7; ++j) e.d_err[j] = DP_B[j] - DP_BH[j];
+                RC(launch_tile(h, e, s));
+            }
+        }
+    }
+    CU(cudaGetLastError());
+    return TDSE_OK;
+}
+
+// Lanczos step: per Krylov vector one tile kernel (matvec + alpha) and one element-wise kernel
+// (orthogonalise + beta); then the one-warp exponential and the back-expansion.  The normalisation of q_{p+1}
+// is folded into the next tile load.  w ping-pongs between two buffers because a tile source must not be
+// written by the same kernel (halo race).
+int enqueue_lanczos_block(tdse_handle *h, int K, int order, int n, int obs, cudaStream_t s) {
+    const int B = h->grid.batch;
+    field_table_kernel<<<(n * B + 255) / 256, 256, 0, s>>>(h->d_ctl, h->d_pulse, B, n, 0, h->d_etab);
+    count(h);
+    double2 *psi = h->pool[h->psi_slot];
+    double2 *wbuf[2]; int c = 0;
+    for (int i = 0; c < 2; ++i) if (i != h->psi_slot) wbuf[c++] = h->pool[i];
+    double2 *basis = h->d_basis;
+    for (int i = 0; i < n; ++i) {
+        const double *ef = h->d_etab + (size_t)i * B;
+        OpNorm on{}; on.psi = psi; on.nrm = h->d_nrm; on.inv = h->d_inv; on.m_used = h->d_m; on.K = K;
+        RC(launch_ew(h, on, s));
+        for (int p = 0; p < K; ++p) {
+            double2 *q_p = basis + (size_t)p * h->n_state;
+            EpiLanczosA a{};
+            a.in = (p == 0) ? psi : wbuf[p & 1];
+            a.ef = ef; a.inv = h->d_inv; a.m_used = h->d_m; a.p = p; a.K = K;
+            a.q_out = q_p; a.w_out = (p < K - 1) ? wbuf[(p + 1) & 1] : nullptr; a.alpha = h->d_alpha;
+            RC(launch_tile(h, a, s));
+            if (p < K - 1) {
+                OpLanczosB bb{};
+                bb.w = wbuf[(p + 1) & 1]; bb.q = q_p; bb.q_prev = (p > 0) ? q_p - h->n_state : nullptr;
+                bb.alpha = h->d_alpha; bb.beta = h->d_beta; bb.inv = h->d_inv; bb.m_used = h->d_m;
+                bb.p = p; bb.K = K; bb.tol = h->beta_tol;
+                RC(launch_ew(h, bb, s));
+            }
+        }
+        small_exp_kernel<<<B, 32, 0, s>>>(h->d_alpha, h->d_beta, h->d_m, &h->d_ctl->dt, K, order, h->d_coef, h->d_nsub);
+        count(h);
+        OpCombine oc{};
+        oc.psi = psi; oc.q = basis; oc.q_stride = h->n_state; oc.coef = h->d_coef; oc.nrm = h->d_nrm;
+        oc.m_used = h->d_m; oc.K = K;
+        RC(launch_ew(h, oc, s));
+        if (obs) RC(enqueue_obs(h, psi, i, 1, 0, 0.0, h->d_rows, s));
+    }
+    ctl_advance_kernel<<<1, 32, 0, s>>>(h->d_ctl, n);
+    count(h);
+    CU(cudaGetLastError());
+    return TDSE_OK;
+}
+
+// ---- graph-captured time loop (row a7; NS: "the time loop is captured in a CUDA graph") ------------------
+enum Kind { KIND_TAYLOR = 1, KIND_RK4 = 2, KIND_LANCZOS = 3, KIND_RK45 = 4 };
+
+int enqueue_block(tdse_handle *h, int kind, int p1, int p2, int n, int obs, cudaStream_t s) {
+    switch (kind) {
+        case KIND_TAYLOR: return enqueue_taylor_block(h, p1, n, obs, s);
+        case KIND_RK4: return enqueue_rk4_block(h, n, obs, s);
+        case KIND_LANCZOS: return enqueue_lanczos_block(h, p1, p2, n, obs, s);
+        case KIND_RK45: return enqueue_rk45_block(h, n, 1, s);
+    }
+    return TDSE_ERR_ARG;
+}
+
+// Run `nblocks` blocks of `n` steps each on `stream`, through a cached graph when enabled.
+int run_blocks(tdse_handle *h, int kind, int p1, int p2, int n, int obs, long nblocks, cudaStream_t stream) {
+    if (nblocks <= 0) return TDSE_OK;
+    if (!h->use_graph) {
+        for (long i = 0; i < nblocks; ++i) {
+            h->pending = 0;
+            RC(enqueue_block(h, kind, p1, p2, n, obs, stream));
+            h->launches += h->pending;
+        }
+        return TDSE_OK;
+    }
+    const auto key = std::make_tuple(kind, p1, p2, n, obs + 2 * h->taylor_blocked_last, h->psi_slot);
+    auto it = h->graphs.find(key);
+    if (it == h->graphs.end()) {
+        cudaGraph_t g = nullptr;
+        CU(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeRelaxed));
+        h->pending = 0;
+        const int rc = enqueue_block(h, kind, p1, p2, n, obs, h->cap_stream);
+        const cudaError_t ce = cudaStreamEndCapture(h->cap_stream, &g);
+        if (rc != TDSE_OK) { if (g) cudaGraphDestroy(g); return rc; }
+        CU(ce);
+        cudaGraphExec_t ex = nullptr;
+        const cudaError_t ie = cudaGraphInstantiate(&ex, g, 0);
+        cudaGraphDestroy(g);
+        CU(ie);
+        h->graph_nodes[key] = h->pending;
+        it = h->graphs.emplace(key, ex).first;
+    }
+    const long nodes = h->graph_nodes[key];
+    for (long i = 0; i < nblocks; ++i) {
+        CU(cudaGraphLaunch(it->second, stream));
+        h->launches += nodes;
+    }
+    return TDSE_OK;
+}
+
+int run_fixed(tdse_handle *h, int kind, int p1, int p2, double t0, double dt, long nsteps, int obs_every,
+              cudaStream_t stream) {
+    const int B = h->grid.batch;
+    int G = std::max(1, h->graph_steps);
+    if (h->taylor_blocked_last) G = (G + 1) & ~1;       // ping-pong needs an even block
+    RC(ensure_buf(h, &h->d_etab, &h->etab_cap, (size_t)G * 7 * B));
+    RC(ensure_rows(h, nsteps, obs_every));
+    CtlInit v{};
+    v.t0 = t0; v.dt = dt; v.obs_every = obs_every; v.field_sample = h->field_sample;
+    h->pending = 0;
+    RC(init_ctl(h, v, stream));
+    h->launches += h->pending;
+    const int obs = obs_every > 0 ? 1 : 0;
+    RC(run_blocks(h, kind, p1, p2, G, obs, nsteps / G, stream));
+    const int rem = (int)(nsteps % G);
+    if (rem) {
+        const int ug = h->use_graph; h->use_graph = 0;
+        const int rc = run_blocks(h, kind, p1, p2, rem, obs, 1, stream);
+        h->use_graph = ug;
+        RC(rc);
+    }
+    h->log_rows = obs ? nsteps / obs_every : 0;
+    return TDSE_OK;
+}
+
+bool grid_valid(const tdse_grid *g) {
+    return g && g->n_r >= 1 && g->n_l >= 1 && g->dr > 0.0 && g->batch >= 1 && g->batch <= 65535 &&
+           (long long)g->n_r * g->n_l * g->batch < (1LL << 31) * 8;
+}
+
+}  // namespace
+
+// =========================================================================================================
+extern "C" {
+
+const char *tdse_version(void) { return "tdse_b200 0.1 (sm_100a)"; }
+
+const char *tdse_strerror(int code) {
+    switch (code) {
+        case TDSE_OK: return "ok";
+        case TDSE_ERR_ARG: return "invalid argument";
+        case TDSE_ERR_ALLOC: return "allocation failed";
+        case TDSE_ERR_CUDA: return "CUDA error (no device or launch failure)";
+        case TDSE_ERR_NONFINITE: return "non-finite norm logged (unstable step size?)";
+        case TDSE_ERR_UNSUPPORTED: return "unsupported configuration";
+    }
+    return "unknown error";
+}
+
+int tdse_create(const tdse_grid *grid, tdse_handle **out) {
+    if (!out) return TDSE_ERR_ARG;
+    *out = nullptr;
+    if (!grid_valid(grid)) return TDSE_ERR_ARG;
+    if (grid->gauge != 0 || (grid->fd_order != 3 && grid->fd_order != 5)) return TDSE_ERR_UNSUPPORTED;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return TDSE_ERR_CUDA; }
+    tdse_handle *h = new (std::nothrow) tdse_handle();
+    if (!h) return TDSE_ERR_ALLOC;
+    h->grid = *grid;
+    const int N = grid->n_r, L = grid->n_l, B = grid->batch;
+    h->n_state = (size_t)N * L * B;
+    auto fail = [&](int rc) { tdse_destroy(h); return rc; };
+    auto body = [&]() -> int {
+        // tables of the diagonal of h_l (Eq. 7) and the coupling (Eq. 9)
+        std::vector<double> vj(N), cen(N), cl(L);
+        const double dr2 = grid->dr * grid->dr;
+        const double kd = (grid->fd_order == 3) ? 1.0 / dr2 : 30.0 / (24.0 * dr2);
+        for (int j = 0; j < N; ++j) {
+            const double r = (j + 1) * grid->dr;
+            vj[j] = kd - grid->z_nuc / r;
+            cen[j] = 1.0 / (2.0 * r * r);
+        }
+        for (int l = 0; l < L; ++l) cl[l] = (l + 1) / std::sqrt((2.0 * l + 1.0) * (2.0 * l + 3.0));
+        CU(cudaMalloc(&h->d_vj, sizeof(double) * N));
+        CU(cudaMalloc(&h->d_cen, sizeof(double) * N));
+        CU(cudaMalloc(&h->d_cl, sizeof(double) * L));
+        CU(cudaMemcpy(h->d_vj, vj.data(), sizeof(double) * N, cudaMemcpyHostToDevice));
+        CU(cudaMemcpy(h->d_cen, cen.data(), sizeof(double) * N, cudaMemcpyHostToDevice));
+        CU(cudaMemcpy(h->d_cl, cl.data(), sizeof(double) * L, cudaMemcpyHostToDevice));
+        GridDev &g = h->gd;
+        g.n_r = N; g.n_l = L; g.batch = B; g.fd = grid->fd_order; g.dr = grid->dr; g.z = grid->z_nuc;
+        if (grid->fd_order == 3) { g.c1 = -0.5 / dr2; g.c2 = 0.0; }
+        else { g.c1 = -16.0 / (24.0 * dr2); g.c2 = 1.0 / (24.0 * dr2); }
+        g.vj = h->d_vj; g.cen = h->d_cen; g.cl = h->d_cl;
+        CU(cudaMalloc(&h->d_pulse, sizeof(tdse_pulse) * B));
+        CU(cudaMemset(h->d_pulse, 0, sizeof(tdse_pulse) * B));
+        CU(cudaMalloc(&h->d_ctl, sizeof(Ctl)));
+        CU(cudaMemset(h->d_ctl, 0, sizeof(Ctl)));
+        CU(cudaMalloc(&h->d_bufs, sizeof(double2 *) * kRkRoles));
+        CU(cudaMalloc(&h->d_counter, sizeof(unsigned int)));
+        CU(cudaMemset(h->d_counter, 0, sizeof(unsigned int)));
+        CU(cudaMalloc(&h->d_eapply, sizeof(double) * B));
+        // reduction partials: the larger of the tile grid and the element-wise grid, 4 values per CTA
+        const size_t ctas = std::max((size_t)tile_ctas_per_member(h), (size_t)ew_grid(h).x) * B;
+        size_t cap = 0;
+        RC(ensure_buf(h, &h->d_partials, &cap, ctas * 4));
+        CU(cudaMalloc(&h->d_obs_partials, sizeof(double) * 3 * obs_chunks(h) * B));
+        CU(cudaMalloc(&h->d_row_direct, sizeof(double) * 3 * B));
+        CU(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
+        RC(ensure_pool(h, 1));
+        RC(blocked_configure(&h->bcfg, h->grid));
+        return TDSE_OK;
+    };
+    const int rc = body();
+    if (rc != TDSE_OK) return fail(rc);
+    *out = h;
+    return TDSE_OK;
+}
+
+void tdse_destroy(tdse_handle *h) {
+    if (!h) return;
+    cudaDeviceSynchronize();
+    free_graphs(h);
+    for (double2 *p : h->pool) cudaFree(p);
+    void *ptrs[] = {h->d_vj, h->d_cen, h->d_cl, h->d_pulse, h->d_bufs, h->d_ctl, h->d_etab, h->d_eapply, h->d_partials,
+                    h->d_counter, h->d_phi, h->d_lstate, h->d_obs_partials, h->d_amp, h->d_rows, h->d_row_direct,
+                    h->d_dtlog, h->d_errlog, h->d_replay, h->d_alpha, h->d_beta, h->d_nrm, h->d_inv, h->d_coef,
+                    h->d_m, h->d_nsub, h->d_basis};
+    for (void *p : ptrs) if (p) cudaFree(p);
+    if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+    cudaGetLastError();
+    delete h;
+}
+
+int tdse_set_option(tdse_handle *h, const char *key, double value) {
+    if (!h || !key) return TDSE_ERR_ARG;
+    const std::string k(key);
+    if (k == "field_sample") { if (value != 0.0 && value != 1.0) return TDSE_ERR_ARG; h->field_sample = (int)value; }
+    else if (k == "use_graph") h->use_graph = value != 0.0;
+    else if (k == "graph_steps") { if (value < 1 || value > 4096) return TDSE_ERR_ARG; h->graph_steps = (int)value; }
+    else if (k == "taylor_block") h->taylor_block = value != 0.0;
+    else if (k == "lanczos_beta_tol") { if (!(value >= 0.0)) return TDSE_ERR_ARG; h->beta_tol = value; free_graphs(h); }
+    else if (k == "rk45_dt_max") { if (!(value >= 0.0)) return TDSE_ERR_ARG; h->rk45_dt_max = value; }
+    else if (k == "rk45_check_every") { if (value < 1 || value > 1024) return TDSE_ERR_ARG; h->rk45_check_every = (int)value; }
+    else return TDSE_ERR_ARG;
+    return TDSE_OK;
+}
+
+int tdse_set_pulse(tdse_handle *h, const tdse_pulse *p) {
+    if (!h || !p) return TDSE_ERR_ARG;
+    CU(cudaDeviceSynchronize());
+    CU(cudaMemcpy(h->d_pulse, p, sizeof(tdse_pulse) * h->grid.batch, cudaMemcpyHostToDevice));
+    return TDSE_OK;
+}
+
+int tdse_set_bound_states(tdse_handle *h, int n_states, const int *l_of_state, const double *phi) {
+    if (!h || n_states < 0 || (n_states > 0 && (!l_of_state || !phi))) return TDSE_ERR_ARG;
+    for (int s = 0; s < n_states; ++s) if (l_of_state[s] < 0 || l_of_state[s] >= h->grid.n_l) return TDSE_ERR_ARG;
+    CU(cudaDeviceSynchronize());
+    free_graphs(h);
+    if (h->d_phi) { cudaFree(h->d_phi); h->d_phi = nullptr; }
+    if (h->d_lstate) { cudaFree(h->d_lstate); h->d_lstate = nullptr; }
+    if (h->d_amp) { cudaFree(h->d_amp); h->d_amp = nullptr; }
+    if (h->d_rows) { cudaFree(h->d_rows); h->d_rows = nullptr; h->rows_cap = 0; }
+    if (h->d_row_direct) { cudaFree(h->d_row_direct); h->d_row_direct = nullptr; }
+    h->n_states = n_states;
+    h->log_rows = 0;
+    CU(cudaMalloc(&h->d_row_direct, sizeof(double) * (3 + n_states) * h->grid.batch));
+    if (n_states > 0) {
+        CU(cudaMalloc(&h->d_phi, sizeof(double) * (size_t)n_states * h->grid.n_r));
+        CU(cudaMalloc(&h->d_lstate, sizeof(int) * n_states));
+        CU(cudaMalloc(&h->d_amp, sizeof(double2) * (size_t)n_states * h->grid.batch));
+        CU(cudaMemcpy(h->d_phi, phi, sizeof(double) * (size_t)n_states * h->grid.n_r, cudaMemcpyHostToDevice));
+        CU(cudaMemcpy(h->d_lstate, l_of_state, sizeof(int) * n_states, cudaMemcpyHostToDevice));
+    }
+    return TDSE_OK;
+}
+
+int tdse_set_state(tdse_handle *h, const void *psi, int is_device, void *stream) {
+    if (!h || !psi) return TDSE_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    CU(cudaMemcpyAsync(h->pool[h->psi_slot], psi, h->n_state * sizeof(double2),
+                       is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s));
+    if (!is_device) CU(cudaStreamSynchronize(s));
+    return TDSE_OK;
+}
+
+int tdse_get_state(tdse_handle *h, void *psi, int is_device, void *stream) {
+    if (!h || !psi) return TDSE_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    CU(cudaMemcpyAsync(psi, h->pool[h->psi_slot], h->n_state * sizeof(double2),
+                       is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, s));
+    if (!is_device) CU(cudaStreamSynchronize(s));
+    return TDSE_OK;
+}
+
+int tdse_apply_H(tdse_handle *h, const void *psi_dev, void *out_dev, const double *e_field_host, void *stream) {
+    if (!h || !psi_dev || !out_dev || !e_field_host || psi_dev == out_dev) return TDSE_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    const int B = h->grid.batch;
+    if (!h->eapply_valid || std::memcmp(h->eapply_host.data(), e_field_host, sizeof(double) * B) != 0) {
+        // the staging copy must not race with an earlier launch still reading d_eapply
+        CU(cudaStreamSynchronize(s));
+        h->eapply_host.assign(e_field_host, e_field_host + B);
+        CU(cudaMemcpy(h->d_eapply, h->eapply_host.data(), sizeof(double) * B, cudaMemcpyHostToDevice));
+        h->eapply_valid = true;
+    }
+    EpiApply e{};
+    e.in = (const double2 *)psi_dev; e.ef = h->d_eapply; e.out = (double2 *)out_dev;
+    h->pending = 0;
+    RC(launch_tile(h, e, s));
+    h->launches += h->pending;
+    return TDSE_OK;
+}
+
+int tdse_step_taylor(tdse_handle *h, int order, double t0, double dt, long nsteps, int obs_every, void *stream) {
+    if (!h || order < 1 || order > 64 || nsteps < 0 || obs_every < 0 || !(dt == dt)) return TDSE_ERR_ARG;
+    RC(ensure_pool(h, 4));
+    h->taylor_blocked_last = (h->taylor_block && blocked_supported(h->bcfg, order)) ? 1 : 0;
+    return run_fixed(h, KIND_TAYLOR, order, 0, t0, dt, nsteps, obs_every, (cudaStream_t)stream);
+}
+
+int tdse_step_rk4(tdse_handle *h, double t0, double dt, long nsteps, int obs_every, void *stream) {
+    if (!h || nsteps < 0 || obs_every < 0) return TDSE_ERR_ARG;
+    RC(ensure_pool(h, 6));
+    h->taylor_blocked_last = 0;
+    rk_roles(h);
+    RC(upload_bufs(h, 6, (cudaStream_t)stream));
+    return run_fixed(h, KIND_RK4, 0, 0, t0, dt, nsteps, obs_every, (cudaStream_t)stream);
+}
+
+int tdse_step_lanczos(tdse_handle *h, int K, int order, double t0, double dt, long nsteps, int obs_every, void *stream) {
+    if (!h || K < 1 || order < 1 || nsteps < 0 || obs_every < 0) return TDSE_ERR_ARG;
+    if (K > kMaxKrylov) return TDSE_ERR_UNSUPPORTED;
+    RC(ensure_pool(h, 3));
+    h->taylor_blocked_last = 0;
+    const int B = h->grid.batch;
+    if (h->lz_K != K) {
+        CU(cudaDeviceSynchronize());
+        free_graphs(h);
+        void *old[] = {h->d_alpha, h->d_beta, h->d_nrm, h->d_inv, h->d_coef, h->d_m, h->d_nsub, h->d_basis};
+        for (void *p : old) if (p) cudaFree(p);
+        h->d_alpha = h->d_beta = h->d_nrm = h->d_inv = nullptr; h->d_coef = nullptr; h->d_m = h->d_nsub = nullptr;
+        h->d_basis = nullptr; h->lz_K = 0;
+        CU(cudaMalloc(&h->d_alpha, sizeof(double) * B * K));
+        CU(cudaMalloc(&h->d_beta, sizeof(double) * B * K));
+        CU(cudaMalloc(&h->d_nrm, sizeof(double) * B));
+        CU(cudaMalloc(&h->d_inv, sizeof(double) * B));
+        CU(cudaMalloc(&h->d_coef, sizeof(double2) * B * K));
+        CU(cudaMalloc(&h->d_m, sizeof(int) * B));
+        CU(cudaMalloc(&h->d_nsub, sizeof(int) * B));
+        CU(cudaMalloc(&h->d_basis, sizeof(double2) * h->n_state * K));
+        h->lz_K = K;
+    }
+    CU(cudaMemsetAsync(h->d_alpha, 0, sizeof(double) * B * K, (cudaStream_t)stream));
+    CU(cudaMemsetAsync(h->d_beta, 0, sizeof(double) * B * K, (cudaStream_t)stream));
+    return run_fixed(h, KIND_LANCZOS, K, order, t0, dt, nsteps, obs_every, (cudaStream_t)stream);
+}
+
+int tdse_step_rk45(tdse_handle *h, double t0, double t_end, double dt_init, double rtol, const double *dt_replay,
+                   long n_replay, long *n_accept, long *n_reject, void *stream) {
+    if (!h || !(rtol > 0.0)) return TDSE_ERR_ARG;
+    const bool replay = dt_replay != nullptr;
+    if (replay ? (n_replay < 0) : (!(dt_init > 0.0) || !(t_end > t0))) return TDSE_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    const int B = h->grid.batch;
+    RC(ensure_pool(h, kRkRoles));
+    h->taylor_blocked_last = 0;
+    rk_roles(h);
+    RC(upload_bufs(h, kRkRoles, s));
+    RC(ensure_buf(h, &h->d_etab, &h->etab_cap, (size_t)std::max(1, h->graph_steps) * 7 * B));
+    // logs
+    const long want_log = replay ? std::max(1L, n_replay) : (1L << 20);
+    if (h->log_cap < want_log) {
+        CU(cudaDeviceSynchronize());
+        free_graphs(h);
+        if (h->d_dtlog) cudaFree(h->d_dtlog);
+        if (h->d_errlog) cudaFree(h->d_errlog);
+        h->d_dtlog = h->d_errlog = nullptr; h->log_cap = 0;
+        CU(cudaMalloc(&h->d_dtlog, sizeof(double) * want_log));
+        CU(cudaMalloc(&h->d_errlog, sizeof(double) * want_log));
+        h->log_cap = want_log;
+    }
+    if (replay && n_replay > 0) {
+        if (h->replay_cap < n_replay) {
+            CU(cudaDeviceSynchronize());
+            free_graphs(h);
+            if (h->d_replay) cudaFree(h->d_replay);
+            h->d_replay = nullptr; h->replay_cap = 0;
+            CU(cudaMalloc(&h->d_replay, sizeof(double) * n_replay));
+            h->replay_cap = n_replay;
+        }
+        CU(cudaMemcpy(h->d_replay, dt_replay, sizeof(double) * n_replay, cudaMemcpyHostToDevice));
+    }
+    h->last_accept = 0;
+    if (n_accept) *n_accept = 0;
+    if (n_reject) *n_reject = 0;
+    if (replay && n_replay == 0) return TDSE_OK;
+    CtlInit v{};
+    v.t = t0; v.t_end = t_end; v.rtol = rtol; v.dt_max = h->rk45_dt_max; v.replay = replay ? 1 : 0;
+    v.n_replay = n_replay; v.max_log = h->log_cap;
+    v.h = dt_init;
+    if (!replay && v.dt_max > 0.0 && v.h > v.dt_max) v.h = v.dt_max;
+    h->pending = 0;
+    RC(init_ctl(h, v, s));
+    // the first attempted step needs k_1 (no FSAL yet): run it eagerly with stage 0 included
+    RC(enqueue_rk45_block(h, 1, 0, s));
+    h->launches += h->pending;
+    const int G = std::max(1, h->rk45_check_every);
+    Ctl hc{};
+    for (;;) {
+        CU(cudaMemcpyAsync(&hc, h->d_ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, s));
+        CU(cudaStreamSynchronize(s));
+        if (hc.done) break;
+        if (!(hc.h > 0.0) || hc.n_attempt > (1LL << 40)) return TDSE_ERR_NONFINITE;
+        RC(run_blocks(h, KIND_RK45, 0, 0, G, 0, 1, s));
+    }
+    // the device swapped roles on every accept: make the host's view of "the state" follow
+    h->psi_slot = h->role_slot[hc.perm[R_PSI]];
+    h->last_accept = (long)hc.n_accept;
+    if (n_accept) *n_accept = (long)hc.n_accept;
+    if (n_reject) *n_reject = (long)hc.n_reject;
+    return TDSE_OK;
+}
+
+int tdse_observables(tdse_handle *h, double t, double *out_host, void *stream) {
+    if (!h || !out_host) return TDSE_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    h->pending = 0;
+    RC(enqueue_obs(h, h->pool[h->psi_slot], 0, 0, 1, t, h->d_row_direct, s));
+    h->launches += h->pending;
+    CU(cudaMemcpyAsync(out_host, h->d_row_direct, sizeof(double) * (3 + h->n_states) * h->grid.batch,
+                       cudaMemcpyDeviceToHost, s));
+    CU(cudaStreamSynchronize(s));
+    return TDSE_OK;
+}
+
+int tdse_obs_log(tdse_handle *h, double *out_host, long max_rows, long *rows) {
+    if (!h || !rows || max_rows < 0 || (max_rows > 0 && !out_host)) return TDSE_ERR_ARG;
+    CU(cudaDeviceSynchronize());
+    *rows = h->log_rows;
+    const long n = std::min(max_rows, h->log_rows);
+    const size_t W = 3 + h->n_states, per = W * h->grid.batch;
+    if (n > 0) {
+        CU(cudaMemcpy(out_host, h->d_rows, sizeof(double) * per * n, cudaMemcpyDeviceToHost));
+        for (long r = 0; r < n; ++r)
+            for (int b = 0; b < h->grid.batch; ++b)
+                if (!std::isfinite(out_host[r * per + b * W])) return TDSE_ERR_NONFINITE;
+    }
+    return TDSE_OK;
+}
+
+int tdse_dt_log(tdse_handle *h, double *dt_host, double *err_host, long max, long *n) {
+    if (!h || !n || max < 0 || (max > 0 && !dt_host)) return TDSE_ERR_ARG;
+    CU(cudaDeviceSynchronize());
+    *n = h->last_accept;
+    const long c = std::min(std::min(max, h->last_accept), h->log_cap);
+    if (c > 0) {
+        CU(cudaMemcpy(dt_host, h->d_dtlog, sizeof(double) * c, cudaMemcpyDeviceToHost));
+        if (err_host) CU(cudaMemcpy(err_host, h->d_errlog, sizeof(double) * c, cudaMemcpyDeviceToHost));
+    }
+    return TDSE_OK;
+}
+
+int tdse_lanczos_info(tdse_handle *h, double *alpha, double *beta, double *coef, int *m_used, int *n_sub) {
+    if (!h) return TDSE_ERR_ARG;
+    if (h->lz_K == 0) return TDSE_ERR_ARG;
+    CU(cudaDeviceSynchronize());
+    const size_t n = (size_t)h->grid.batch * h->lz_K;
+    if (alpha) CU(cudaMemcpy(alpha, h->d_alpha, sizeof(double) * n, cudaMemcpyDeviceToHost));
+    if (beta) CU(cudaMemcpy(beta, h->d_beta, sizeof(double) * n, cudaMemcpyDeviceToHost));
+    if (coef) CU(cudaMemcpy(coef, h->d_coef, sizeof(double2) * n, cudaMemcpyDeviceToHost));
+    if (m_used) CU(cudaMemcpy(m_used, h->d_m, sizeof(int) * h->grid.batch, cudaMemcpyDeviceToHost));
+    if (n_sub) CU(cudaMemcpy(n_sub, h->d_nsub, sizeof(int) * h->grid.batch, cudaMemcpyDeviceToHost));
+    return TDSE_OK;
+}
+
+long tdse_launch_count(tdse_handle *h) { return h ? h->launches : 0; }
+int tdse_taylor_was_blocked(tdse_handle *h) { return h ? h->taylor_blocked_last : 0; }
+
+}  // extern "C"

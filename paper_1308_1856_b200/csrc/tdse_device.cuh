@@ -1,0 +1,136 @@
+// tdse_device.cuh -- device-side data structures and helpers shared by all kernels of libtdse_b200.
+// Part of the CUDA product path; shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/tdse.h"
+
+namespace tdse {
+
+constexpr int kMaxKrylov = 32;     // one lane per Krylov coefficient in the small exponential
+constexpr int kRkRoles   = 10;     // PSI, G0, G1, K0..K6
+
+// Grid description and device tables handed to every kernel by value.
+struct GridDev {
+    int n_r, n_l, batch, fd;
+    double dr, z;
+    double c1, c2;          // off-diagonal stencil weights of -1/2 D2: 3-point c1 = -1/(2dr^2); 5-point c1 = -16/(24dr^2), c2 = +1/(24dr^2)
+    const double *vj;       // [n_r]  kinetic diagonal - Z/r_j          (Eq. 7, Eq. 15)
+    const double *cen;      // [n_r]  1/(2 r_j^2)                       (centrifugal factor, Eq. 7)
+    const double *cl;       // [n_l]  c_l = (l+1)/sqrt((2l+1)(2l+3))    (Eq. 9, m = 0)
+};
+
+// Device-resident control block: everything a captured graph must be able to re-read at launch time.
+struct Ctl {
+    // fixed-step propagators
+    double t0, dt;
+    long long step_base;            // index (within this call) of the first step of the running block
+    int obs_every, field_sample;
+    // adaptive / replayed Dormand-Prince
+    double t, h, t_end, rtol, dt_max;
+    int done, last, after_reject, replay;
+    long long n_accept, n_reject, n_attempt, n_replay, max_log;
+    int perm[kRkRoles];             // role -> buffer index (swapped on accept: psi <-> psi_new, k1 <-> k7)
+};
+
+struct CtlInit {
+    double t0, dt; int obs_every, field_sample;
+    double t, h, t_end, rtol, dt_max; int replay; long long n_replay, max_log;
+};
+
+// Reduction context of a kernel launch: per-CTA partial sums, a ticket counter, and the CTA count.
+struct RedCtx {
+    double *partials;               // [ctas][NRED]
+    unsigned int *counter;          // zero before the launch; reset by the last CTA
+    int ctas_per_member;
+};
+
+__device__ __forceinline__ double2 ldcg2(const double2 *p) { return __ldcg(p); }
+
+__device__ __forceinline__ double2 cadd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
+// a + s*b, s real
+__device__ __forceinline__ double2 caxpy_r(double s, double2 b, double2 a) {
+    return make_double2(fma(s, b.x, a.x), fma(s, b.y, a.y));
+}
+
+// E(t) of one member (Eq. 19 with the Hann envelope of P:166; reading R-G8).  The time bookkeeping uses
+// explicitly rounded operations so that t itself carries no contraction-dependent bits.
+__device__ inline double pulse_E(const tdse_pulse &p, double t) {
+    if (p.omega == 0.0) return p.e0;
+    const double T = __ddiv_rn(__dmul_rn(2.0 * 3.14159265358979323846, p.n_cycles), p.omega);
+    if (t < 0.0 || t > T) return 0.0;
+    const double wt = __dmul_rn(p.omega, t);
+    const double s = sin(__ddiv_rn(wt, __dmul_rn(2.0, p.n_cycles)));
+    return __dmul_rn(__dmul_rn(__dmul_rn(p.e0, s), s), cos(__dadd_rn(wt, p.cep)));
+}
+
+// t0 + x*dt with two roundings (never contracted)
+__device__ __forceinline__ double time_at(double t0, double x, double dt) { return __dadd_rn(t0, __dmul_rn(x, dt)); }
+
+// Deterministic block reduction of NRED doubles per thread: warp shuffle tree, then a fixed-order pass over
+// the per-warp results.  Result valid in thread 0.  scratch: NRED * (NT/32) doubles of shared memory.
+template <int NT, int NRED>
+__device__ __forceinline__ void block_reduce(double (&v)[NRED], double *scratch) {
+    constexpr int NW = NT / 32;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int r = 0; r < NRED; ++r) {
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) v[r] += __shfl_down_sync(0xffffffffu, v[r], off);
+    }
+    __syncthreads();   // scratch may still be in use by a previous call
+    if (lane == 0) {
+#pragma unroll
+        for (int r = 0; r < NRED; ++r) scratch[r * NW + warp] = v[r];
+    }
+    __syncthreads();
+    if (warp == 0) {
+#pragma unroll
+        for (int r = 0; r < NRED; ++r) {
+            double x = (lane < NW) ? scratch[r * NW + lane] : 0.0;
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) x += __shfl_down_sync(0xffffffffu, x, off);
+            v[r] = x;
+        }
+    }
+}
+
+// Two-stage grid reduction with a "last CTA finishes" second stage (replaces the paper's redundant
+// per-work-group second stage).  Every CTA of the launch must call this exactly once.
+// cta_linear = member * ctas_per_member + tile.  The last CTA sums the partials of every member in a fixed
+// order and calls fin.finish_member(b, sums) for each, then fin.finish_all(), from thread 0.
+template <int NT, int NRED, class Fin>
+__device__ __forceinline__ void grid_reduce_finish(double (&red)[NRED], const RedCtx &rc, int cta_linear,
+                                                   int total_ctas, int n_members, Fin &fin, double *scratch,
+                                                   int *flag) {
+    block_reduce<NT, NRED>(red, scratch);
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int r = 0; r < NRED; ++r) rc.partials[(size_t)cta_linear * NRED + r] = red[r];
+        __threadfence();
+        const unsigned int ticket = atomicAdd(rc.counter, 1u);
+        *flag = (ticket == (unsigned int)(total_ctas - 1));
+    }
+    __syncthreads();
+    if (!*flag) return;
+    __threadfence();
+    for (int b = 0; b < n_members; ++b) {
+        double s[NRED];
+#pragma unroll
+        for (int r = 0; r < NRED; ++r) s[r] = 0.0;
+        const double *p = rc.partials + (size_t)b * rc.ctas_per_member * NRED;
+        for (int i = threadIdx.x; i < rc.ctas_per_member; i += NT) {
+#pragma unroll
+            for (int r = 0; r < NRED; ++r) s[r] += __ldcg(p + (size_t)i * NRED + r);
+        }
+        block_reduce<NT, NRED>(s, scratch);
+        if (threadIdx.x == 0) fin.finish_member(b, s);
+    }
+    if (threadIdx.x == 0) {
+        fin.finish_all();
+        *rc.counter = 0u;
+    }
+}
+
+}  // namespace tdse

@@ -1,0 +1,559 @@
+// tdse_kernels.cuh -- the sm_100a kernels of the one-pass path: H.psi on shared-memory (l, r) tiles with the
+// propagator arithmetic fused into the epilogue, element-wise/reduction kernels, observables, the one-warp
+// tridiagonal exponential and the control kernels.  Product path; shares nothing with oracle/.
+#pragma once
+#include "tdse_device.cuh"
+
+namespace tdse {
+
+// ------------------------------------------------------------------------------------------------------
+// Tile geometry: TL partial waves x TW radial points of complex128 per CTA, staged in shared memory with
+// a radial halo of HW points on both sides and the l-1 / l+1 rows (NS: "(l, r) tiles ... staged with their
+// radial halo and l+-1 neighbours").  256 threads; each thread owns one column and marches RPT rows, keeping
+// the l-1, l, l+1 values in registers.
+// ------------------------------------------------------------------------------------------------------
+template <int FD>
+struct Tile {
+    static constexpr int HW = (FD == 3) ? 1 : 2;
+    static constexpr int TW = 128, TL = 8, NT = 256;
+    static constexpr int RPT = TL / (NT / TW);          // rows per thread
+    static constexpr int PITCH = TW + 2 * HW;           // double2 elements per shared row
+    static constexpr int ROWS = TL + 2;
+    static constexpr int ELEMS = ROWS * PITCH;
+};
+
+// (H f)_{l,j} from the five/seven neighbouring values (Eq. 11).  d = l(l+1)/(2r^2) - Z/r + kinetic diagonal.
+template <int FD>
+__device__ __forceinline__ double2 h_point(const GridDev &g, double d, double er, double cm, double cp,
+                                           double2 f, double2 fm1, double2 fp1, double2 fm2, double2 fp2,
+                                           double2 lo, double2 up) {
+    double2 h;
+    double kx = g.c1 * (fp1.x + fm1.x), ky = g.c1 * (fp1.y + fm1.y);
+    if (FD == 5) {
+        kx = fma(g.c2, fp2.x + fm2.x, kx);
+        ky = fma(g.c2, fp2.y + fm2.y, ky);
+    }
+    const double cx = fma(cp, up.x, cm * lo.x), cy = fma(cp, up.y, cm * lo.y);
+    h.x = fma(er, cx, fma(d, f.x, kx));
+    h.y = fma(er, cy, fma(d, f.y, ky));
+    return h;
+}
+
+// One pass: out/epilogue <- H(E_b) in, for every member b.  grid = (ceil(n_r/TW), ceil(n_l/TL), batch).
+// Epi supplies: NRED, SCALED; begin(); skip_all(); member_active(b); input(); in_scale(b); efield(b);
+// point(b,l,j,idx,f,h,red); finish_member(b,s); finish_all().
+template <int FD, class Epi>
+__global__ void __launch_bounds__(256, 3) tile_kernel(GridDev g, Epi epi_in, RedCtx rc) {
+    using T = Tile<FD>;
+    __shared__ double2 tile[T::ELEMS];
+    __shared__ double red_s[(Epi::NRED > 0 ? Epi::NRED : 1) * (T::NT / 32)];
+    __shared__ int last_flag;
+    Epi epi = epi_in;
+    epi.begin();
+    if (epi.skip_all()) return;
+
+    const int tid = threadIdx.x;
+    const int b = blockIdx.z, l0 = blockIdx.y * T::TL, j0 = blockIdx.x * T::TW;
+    double red[Epi::NRED > 0 ? Epi::NRED : 1];
+#pragma unroll
+    for (int r = 0; r < (Epi::NRED > 0 ? Epi::NRED : 1); ++r) red[r] = 0.0;
+
+    if (epi.member_active(b)) {
+        const double2 *base = epi.input() + (size_t)b * g.n_l * g.n_r;
+        const double sc = Epi::SCALED ? epi.in_scale(b) : 1.0;
+        // stage the tile (zero outside the index box: Dirichlet walls, f_{-1} = f_L = 0)
+#pragma unroll
+        for (int it = 0; it < (T::ELEMS + T::NT - 1) / T::NT; ++it) {
+            const int i = tid + it * T::NT;
+            if (i < T::ELEMS) {
+                const int rr = i / T::PITCH, cc = i - rr * T::PITCH;
+                const int l = l0 - 1 + rr, j = j0 - T::HW + cc;
+                double2 v = make_double2(0.0, 0.0);
+                if (l >= 0 && l < g.n_l && j >= 0 && j < g.n_r) v = __ldg(base + (size_t)l * g.n_r + j);
+                if (Epi::SCALED) { v.x *= sc; v.y *= sc; }
+                tile[i] = v;
+            }
+        }
+        __syncthreads();
+
+        const int tx = tid % T::TW, ty = tid / T::TW;
+        const int j = j0 + tx;
+        if (j < g.n_r) {
+            const double vj = __ldg(g.vj + j), cen = __ldg(g.cen + j);
+            const double er = epi.efield(b) * (g.dr * (double)(j + 1));
+            const int r0 = ty * T::RPT;
+            const double2 *col = tile + (r0 + 1) * T::PITCH + T::HW + tx;
+            double2 lo = col[-T::PITCH], f = col[0];
+#pragma unroll
+            for (int rr = 0; rr < T::RPT; ++rr) {
+                const int l = l0 + r0 + rr;
+                if (l >= g.n_l) break;
+                const double2 *c = col + rr * T::PITCH;
+                const double2 up = c[T::PITCH];
+                const double2 fm1 = c[-1], fp1 = c[1];
+                double2 fm2 = fm1, fp2 = fp1;
+                if (FD == 5) { fm2 = c[-2]; fp2 = c[2]; }
+                const double d = fma((double)(l * (l + 1)), cen, vj);
+                const double cm = (l > 0) ? __ldg(g.cl + l - 1) : 0.0;
+                const double cp = __ldg(g.cl + l);
+                const double2 h = h_point<FD>(g, d, er, cm, cp, f, fm1, fp1, fm2, fp2, lo, up);
+                const size_t idx = ((size_t)b * g.n_l + l) * g.n_r + j;
+                epi.point(b, l, j, idx, f, h, red);
+                lo = f; f = up;
+            }
+        }
+    }
+    if (Epi::NRED > 0) {
+        const int cta = (b * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+        grid_reduce_finish<T::NT, (Epi::NRED > 0 ? Epi::NRED : 1)>(red, rc, cta, gridDim.x * gridDim.y * gridDim.z,
+                                                                  g.batch, epi, red_s, &last_flag);
+    }
+}
+
+// Defaults shared by the epilogues.
+struct EpiBase {
+    static constexpr int NRED = 0;
+    static constexpr bool SCALED = false;
+    __device__ __forceinline__ void begin() {}
+    __device__ __forceinline__ bool skip_all() const { return false; }
+    __device__ __forceinline__ bool member_active(int) const { return true; }
+    __device__ __forceinline__ double in_scale(int) const { return 1.0; }
+    __device__ __forceinline__ void finish_member(int, const double *) {}
+    __device__ __forceinline__ void finish_all() {}
+};
+
+// out = H in  (tdse_apply_H)
+struct EpiApply : EpiBase {
+    const double2 *in; const double *ef; double2 *out;
+    __device__ __forceinline__ const double2 *input() const { return in; }
+    __device__ __forceinline__ double efield(int b) const { return __ldg(ef + b); }
+    __device__ __forceinline__ void point(int, int, int, size_t idx, double2, double2 h, double *) { out[idx] = h; }
+};
+
+// One Taylor order (Eq. 37, "only one kernel"): term_k = (-i dt/k) H term_{k-1}; acc += term_k.
+struct EpiTaylor : EpiBase {
+    const double2 *in; const double *ef; const double *dtp; int k, first, write_term;
+    double2 *term_out; const double2 *acc_in; double2 *acc_out;
+    double s;
+    __device__ __forceinline__ void begin() { s = *dtp / (double)k; }
+    __device__ __forceinline__ const double2 *input() const { return in; }
+    __device__ __forceinline__ double efield(int b) const { return __ldg(ef + b); }
+    __device__ __forceinline__ void point(int, int, int, size_t idx, double2 f, double2 h, double *) {
+        const double2 t = make_double2(s * h.y, -s * h.x);      // (-i s)(x + i y) = s y - i s x
+        if (write_term) term_out[idx] = t;
+        const double2 a = first ? f : acc_in[idx];
+        acc_out[idx] = cadd(a, t);
+    }
+};
+
+// One explicit Runge-Kutta stage (Eq. 38, stage loop P:469-478) with the next stage vector formed in the
+// epilogue: k_i = -i H(t_n + c_i h) g_i;  g_{i+1} = psi + sum_{j<=i} (h a_{i+1,j}) k_j  (or psi_new with the b row).
+// Buffers are addressed through roles so that the adaptive driver can swap psi/psi_new and k1/k7 on the device.
+template <bool EMBED>
+struct EpiRK : EpiBase {
+    static constexpr int NRED = EMBED ? 2 : 0;
+    Ctl *ctl; double2 *const *bufs; const double *ef; const double *hptr;
+    int stage;              // i (0-based)
+    int in_role;            // role of the tile source
+    int k_role[7];          // roles of k_0..k_6
+    int store_k;            // write k_i
+    int out_role;           // role receiving g_{i+1} / psi_new, -1: none
+    int psi_role;
+    double a_next[7];       // a_{i+1,j} (or b_j), j = 0..i; 0 entries are skipped like in the paper's loop
+    double d_err[7];        // b_j - bhat_j  (embedded pair difference)
+    int check_done;
+    double *dt_log, *err_log;
+    // resolved at begin()
+    const double2 *in_p; double2 *out_p; const double2 *psi_p; double2 *k_p[7]; double hh; double emax;
+
+    __device__ __forceinline__ void begin() {
+        in_p = bufs[ctl->perm[in_role]];
+        out_p = out_role >= 0 ? bufs[ctl->perm[out_role]] : nullptr;
+        psi_p = bufs[ctl->perm[psi_role]];
+#pragma unroll
+        for (int j = 0; j < 7; ++j) k_p[j] = (k_role[j] >= 0) ? bufs[ctl->perm[k_role[j]]] : nullptr;
+        hh = *hptr;
+        emax = 0.0;
+    }
+    __device__ __forceinline__ bool skip_all() const { return check_done && ctl->done; }
+    __device__ __forceinline__ const double2 *input() const { return in_p; }
+    __device__ __forceinline__ double efield(int b) const { return __ldg(ef + b); }
+    __device__ __forceinline__ void point(int, int, int, size_t idx, double2 f, double2 h, double *red) {
+        const double2 k = make_double2(h.y, -h.x);              // -i H g
+        if (store_k) k_p[stage][idx] = k;
+        if (out_role >= 0) {
+            double2 acc = (stage == 0) ? f : psi_p[idx];
+#pragma unroll
+            for (int j = 0; j < 7; ++j) {
+                if (j < stage && a_next[j] != 0.0) acc = caxpy_r(hh * a_next[j], k_p[j][idx], acc);
+            }
+            if (a_next[stage] != 0.0) acc = caxpy_r(hh * a_next[stage], k, acc);
+            out_p[idx] = acc;
+        }
+        if (EMBED) {
+            double2 d = make_double2(0.0, 0.0);
+#pragma unroll
+            for (int j = 0; j < 7; ++j) {
+                if (j < stage && d_err[j] != 0.0) d = caxpy_r(hh * d_err[j], k_p[j][idx], d);
+            }
+            if (d_err[stage] != 0.0) d = caxpy_r(hh * d_err[stage], k, d);
+            red[0] += d.x * d.x + d.y * d.y;
+            red[1] += f.x * f.x + f.y * f.y;                    // the tile source of the last stage is psi_new
+        }
+    }
+    // controller (R-C4): runs once per attempted step in the last CTA
+    __device__ __forceinline__ void finish_member(int, const double *s) {
+        if (EMBED) { const double e = sqrt(s[0]) / sqrt(s[1]); if (!(e <= emax)) emax = e; }
+    }
+    __device__ __forceinline__ void finish_all() {
+        if (!EMBED) return;
+        Ctl &c = *ctl;
+        const double err = emax / c.rtol;
+        const long long slot = c.n_accept;
+        const double h = c.h;
+        bool accept = c.replay || (err <= 1.0);
+        if (accept) {
+            if (slot < c.max_log) { dt_log[slot] = h; err_log[slot] = err; }
+            c.n_accept = slot + 1;
+            // psi <- psi_new (held by the last stage's tile source), k1 <- k7 (FSAL: same time t_{n+1})
+            int tmp = c.perm[psi_role]; c.perm[psi_role] = c.perm[in_role]; c.perm[in_role] = tmp;
+            tmp = c.perm[k_role[0]]; c.perm[k_role[0]] = c.perm[k_role[6]]; c.perm[k_role[6]] = tmp;
+            c.t = c.last ? c.t_end : __dadd_rn(c.t, h);
+        } else {
+            c.n_reject += 1;
+        }
+        c.n_attempt += 1;
+        if (c.replay) {
+            if (c.n_attempt >= c.n_replay) c.done = 1;
+            return;
+        }
+        double fac = 0.9 * pow(err, -0.2);
+        if (!(fac >= 0.2)) fac = 0.2;
+        if (fac > 5.0) fac = 5.0;
+        if (accept) {
+            if (c.after_reject && fac > 1.0) fac = 1.0;
+            c.after_reject = 0;
+            if (!(c.t < c.t_end)) c.done = 1;
+        } else {
+            if (fac > 1.0) fac = 1.0;
+            c.after_reject = 1;
+        }
+        double hn = __dmul_rn(h, fac);
+        if (c.dt_max > 0.0 && hn > c.dt_max) hn = c.dt_max;
+        c.h = hn;
+    }
+};
+
+// Lanczos matvec with the alpha reduction fused (LanczosLoop1): q_p = in * inv_b; w = H q_p; alpha_p = Re<q_p|w>.
+struct EpiLanczosA : EpiBase {
+    static constexpr int NRED = 1;
+    static constexpr bool SCALED = true;
+    const double2 *in; const double *ef; const double *inv; const int *m_used; int p, K;
+    double2 *q_out; double2 *w_out; double *alpha;
+    __device__ __forceinline__ bool member_active(int b) const { return m_used[b] > p; }
+    __device__ __forceinline__ const double2 *input() const { return in; }
+    __device__ __forceinline__ double in_scale(int b) const { return inv[b]; }
+    __device__ __forceinline__ double efield(int b) const { return __ldg(ef + b); }
+    __device__ __forceinline__ void point(int, int, int, size_t idx, double2 f, double2 h, double *red) {
+        q_out[idx] = f;
+        if (w_out) w_out[idx] = h;
+        red[0] += f.x * h.x + f.y * h.y;
+    }
+    __device__ __forceinline__ void finish_member(int b, const double *s) { if (m_used[b] > p) alpha[b * K + p] = s[0]; }
+};
+
+// ------------------------------------------------------------------------------------------------------
+// Element-wise kernels with optional fused reduction.  grid = (chunks, 1, batch); a CTA handles EW_CHUNK
+// consecutive points of one member.
+// ------------------------------------------------------------------------------------------------------
+constexpr int EW_NT = 256, EW_PER = 8, EW_CHUNK = EW_NT * EW_PER;
+
+template <class Op>
+__global__ void __launch_bounds__(EW_NT) ew_kernel(long long n_per_member, int n_members, Op op_in, RedCtx rc) {
+    __shared__ double red_s[(Op::NRED > 0 ? Op::NRED : 1) * (EW_NT / 32)];
+    __shared__ int last_flag;
+    Op op = op_in;
+    op.begin();
+    const int b = blockIdx.z;
+    double red[Op::NRED > 0 ? Op::NRED : 1];
+#pragma unroll
+    for (int r = 0; r < (Op::NRED > 0 ? Op::NRED : 1); ++r) red[r] = 0.0;
+    if (op.member_active(b)) {
+        const long long base = (long long)blockIdx.x * EW_CHUNK;
+#pragma unroll
+        for (int u = 0; u < EW_PER; ++u) {
+            const long long i = base + threadIdx.x + u * EW_NT;
+            if (i < n_per_member) op.point(b, (size_t)b * n_per_member + i, red);
+        }
+    }
+    if (Op::NRED > 0) {
+        const int cta = b * gridDim.x + blockIdx.x;
+        grid_reduce_finish<EW_NT, (Op::NRED > 0 ? Op::NRED : 1)>(red, rc, cta, gridDim.x * gridDim.z, n_members, op,
+                                                              red_s, &last_flag);
+    }
+}
+
+struct OpBase {
+    static constexpr int NRED = 0;
+    __device__ __forceinline__ void begin() {}
+    __device__ __forceinline__ bool member_active(int) const { return true; }
+    __device__ __forceinline__ void finish_member(int, const double *) {}
+    __device__ __forceinline__ void finish_all() {}
+};
+
+// ||F|| at the start of a Lanczos step: nrm_b, inv_b = 1/nrm_b, m_b = K.
+struct OpNorm : OpBase {
+    static constexpr int NRED = 1;
+    const double2 *psi; double *nrm, *inv; int *m_used; int K;
+    __device__ __forceinline__ void point(int, size_t idx, double *red) {
+        const double2 v = psi[idx];
+        red[0] += v.x * v.x + v.y * v.y;
+    }
+    __device__ __forceinline__ void finish_member(int b, const double *s) {
+        const double n = sqrt(s[0]);
+        nrm[b] = n; inv[b] = 1.0 / n; m_used[b] = K;
+    }
+};
+
+// Orthogonalisation and beta (LanczosLoop2 + NormKrylov): w -= alpha_p q_p + beta_{p-1} q_{p-1};
+// beta_p = ||w||; breakdown if beta_p < tol (R-G17); inv_b = 1/beta_p scales the next tile load.
+struct OpLanczosB : OpBase {
+    static constexpr int NRED = 1;
+    double2 *w; const double2 *q, *q_prev; const double *alpha; double *beta; double *inv; int *m_used;
+    int p, K; double tol;
+    __device__ __forceinline__ bool member_active(int b) const { return m_used[b] > p; }
+    __device__ __forceinline__ void point(int b, size_t idx, double *red) {
+        double2 v = w[idx];
+        v = caxpy_r(-alpha[b * K + p], q[idx], v);
+        if (p > 0) v = caxpy_r(-beta[b * K + p - 1], q_prev[idx], v);
+        w[idx] = v;
+        red[0] += v.x * v.x + v.y * v.y;
+    }
+    __device__ __forceinline__ void finish_member(int b, const double *s) {
+        if (m_used[b] <= p) return;
+        const double bt = sqrt(s[0]);
+        beta[b * K + p] = bt;
+        if (bt < tol) m_used[b] = p + 1;
+        inv[b] = 1.0 / bt;
+    }
+};
+
+// F(t+dt) = ||F|| sum_{p<m} c_p q_p  (Taylor2)
+struct OpCombine : OpBase {
+    double2 *psi; const double2 *q; size_t q_stride; const double2 *coef; const double *nrm; const int *m_used; int K;
+    __device__ __forceinline__ void point(int b, size_t idx, double *) {
+        const int m = m_used[b];
+        const double n = nrm[b];
+        double2 acc = make_double2(0.0, 0.0);
+        for (int p = 0; p < m; ++p) {
+            const double2 c = coef[b * K + p];
+            const double ar = n * c.x, ai = n * c.y;
+            const double2 x = q[(size_t)p * q_stride + idx];
+            acc.x += ar * x.x - ai * x.y;
+            acc.y += ar * x.y + ai * x.x;
+        }
+        psi[idx] = acc;
+    }
+};
+
+struct OpCopy : OpBase {
+    double2 *dst; const double2 *src;
+    __device__ __forceinline__ void point(int, size_t idx, double *) { dst[idx] = src[idx]; }
+};
+
+// ------------------------------------------------------------------------------------------------------
+// c = exp(-i T dt) e_1 on the K x K real tridiagonal T by a sub-stepped Taylor series (Taylor1, P:511:
+// "only one work group" -> one warp, lane i owns coefficient i; R-G18 for the sub-step count).
+// grid = batch, block = 32.
+// ------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(32) small_exp_kernel(const double *alpha, const double *beta, const int *m_used,
+                                                       const double *dtp, int K, int order, double2 *coef,
+                                                       int *n_sub_out) {
+    const int b = blockIdx.x, i = threadIdx.x;
+    const int m = m_used[b];
+    const double dt = *dtp;
+    const bool on = i < m;
+    const double a = on ? alpha[b * K + i] : 0.0;
+    const double bl = (on && i > 0) ? beta[b * K + i - 1] : 0.0;        // beta_{i-1}
+    const double br = (on && i < m - 1) ? beta[b * K + i] : 0.0;        // beta_i
+    double gr = on ? (fabs(a) + bl + br) : 0.0;                          // Gershgorin radius of row i
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) gr = fmax(gr, __shfl_xor_sync(0xffffffffu, gr, off));
+    int s = (int)ceil(dt * gr / 3.0);
+    if (s < 1) s = 1;
+    const double h = dt / (double)s;
+    double2 c = make_double2(i == 0 ? 1.0 : 0.0, 0.0);
+    for (int rep = 0; rep < s; ++rep) {
+        double2 t = c;
+        for (int k = 1; k <= order; ++k) {
+            const double tlx = __shfl_up_sync(0xffffffffu, t.x, 1), tly = __shfl_up_sync(0xffffffffu, t.y, 1);
+            const double trx = __shfl_down_sync(0xffffffffu, t.x, 1), try_ = __shfl_down_sync(0xffffffffu, t.y, 1);
+            double ux = a * t.x, uy = a * t.y;
+            if (i > 0) { ux += bl * tlx; uy += bl * tly; }
+            if (i < m - 1) { ux += br * trx; uy += br * try_; }
+            const double f = h / (double)k;
+            t = on ? make_double2(f * uy, -f * ux) : make_double2(0.0, 0.0);
+            c.x += t.x; c.y += t.y;
+        }
+    }
+    if (i < K) coef[b * K + i] = on ? c : make_double2(0.0, 0.0);
+    if (i == 0) n_sub_out[b] = s;
+}
+
+// ------------------------------------------------------------------------------------------------------
+// Field tables and control kernels (time loop, row a7).
+// ------------------------------------------------------------------------------------------------------
+// mode 0: Taylor/Lanczos (one value per step, at t_n + dt/2 or t_n);  mode 1: RK4 (4 stage times).
+// e_tab[(step*n_stage + stage)*B + b]
+__global__ void field_table_kernel(const Ctl *ctl, const tdse_pulse *pulse, int B, int n_steps, int mode,
+                                   double *e_tab) {
+    const int n_stage = (mode == 1) ? 4 : 1;
+    const int total = n_steps * n_stage * B;
+    const double t0 = ctl->t0, dt = ctl->dt;
+    const long long base = ctl->step_base;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < total; i += gridDim.x * blockDim.x) {
+        const int b = i % B, st = (i / B) % n_stage, s = i / (B * n_stage);
+        const double n = (double)(base + s);
+        double t;
+        if (mode == 1) {
+            const double c = (st == 0) ? 0.0 : (st == 3 ? 1.0 : 0.5);
+            t = __dadd_rn(time_at(t0, n, dt), __dmul_rn(c, dt));
+        } else {
+            t = ctl->field_sample == 1 ? time_at(t0, n, dt) : time_at(t0, n + 0.5, dt);
+        }
+        e_tab[i] = pulse_E(pulse[b], t);
+    }
+}
+
+__global__ void ctl_init_kernel(Ctl *c, CtlInit v) {
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        c->t0 = v.t0; c->dt = v.dt; c->step_base = 0; c->obs_every = v.obs_every; c->field_sample = v.field_sample;
+        c->t = v.t; c->h = v.h; c->t_end = v.t_end; c->rtol = v.rtol; c->dt_max = v.dt_max;
+        c->done = 0; c->last = 0; c->after_reject = 0; c->replay = v.replay;
+        c->n_accept = 0; c->n_reject = 0; c->n_attempt = 0; c->n_replay = v.n_replay; c->max_log = v.max_log;
+        for (int i = 0; i < kRkRoles; ++i) c->perm[i] = i;
+    }
+}
+
+__global__ void ctl_advance_kernel(Ctl *c, int n) {
+    if (threadIdx.x == 0 && blockIdx.x == 0) c->step_base += n;
+}
+
+// Start of an attempted Dormand-Prince step: clip the step to t_end (or take the replayed one) and tabulate
+// E_b(t + c_i h) for the 7 stages.  e_tab[stage*B + b].  One block.
+__global__ void rk45_begin_kernel(Ctl *c, const tdse_pulse *pulse, int B, const double *replay, double *e_tab) {
+    if (c->done) return;
+    __shared__ double sh_h;
+    if (threadIdx.x == 0) {
+        double h = c->h;
+        if (c->replay) {
+            h = replay[c->n_attempt];
+            c->last = 0;
+        } else if (__dadd_rn(c->t, h) >= c->t_end) {
+            h = c->t_end - c->t; c->last = 1;
+        } else {
+            c->last = 0;
+        }
+        c->h = h;
+        sh_h = h;
+    }
+    __syncthreads();
+    const double h = sh_h, t = c->t;
+    const double cs[7] = {0.0, 1.0 / 5, 3.0 / 10, 4.0 / 5, 8.0 / 9, 1.0, 1.0};
+    for (int i = threadIdx.x; i < 7 * B; i += blockDim.x) {
+        const int st = i / B, b = i - st * B;
+        e_tab[i] = pulse_E(pulse[b], __dadd_rn(t, __dmul_rn(cs[st], h)));
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------
+// Observables (row a6).  obs_main: norm, dipole and acceleration sums by marching l along a column (each
+// element read once).  grid = (ceil(n_r/256), batch).  partials[(b*chunks + chunk)*3 + {0,1,2}].
+// ------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) obs_main_kernel(GridDev g, const double2 *psi, const Ctl *ctl, int step_off,
+                                                       int predicated, double *partials) {
+    __shared__ double red_s[3 * 8];
+    if (predicated) {
+        const long long n = ctl->step_base + step_off + 1;
+        if (ctl->obs_every <= 0 || (n % ctl->obs_every) != 0) return;
+    }
+    const int b = blockIdx.y, j = blockIdx.x * 256 + threadIdx.x;
+    double red[3] = {0.0, 0.0, 0.0};
+    if (j < g.n_r) {
+        const double2 *p = psi + (size_t)b * g.n_l * g.n_r + j;
+        double2 cur = p[0];
+        double nn = cur.x * cur.x + cur.y * cur.y, sz = 0.0;
+        for (int l = 0; l + 1 < g.n_l; ++l) {
+            const double2 nx = p[(size_t)(l + 1) * g.n_r];
+            sz = fma(__ldg(g.cl + l), cur.x * nx.x + cur.y * nx.y, sz);
+            nn += nx.x * nx.x + nx.y * nx.y;
+            cur = nx;
+        }
+        const double r = g.dr * (double)(j + 1);
+        red[0] = nn; red[1] = r * sz; red[2] = sz / (r * r);
+    }
+    block_reduce<256, 3>(red, red_s);
+    if (threadIdx.x == 0) {
+        double *o = partials + ((size_t)b * gridDim.x + blockIdx.x) * 3;
+        o[0] = red[0]; o[1] = red[1]; o[2] = red[2];
+    }
+}
+
+// amplitude_s = sum_j phi_s[j] f_{l_s,j}  (Eq. 25).  grid = (n_states, batch), block 128.
+__global__ void __launch_bounds__(128) obs_pop_kernel(GridDev g, const double2 *psi, const double *phi,
+                                                      const int *l_of_state, int n_states, const Ctl *ctl,
+                                                      int step_off, int predicated, double2 *amp) {
+    __shared__ double red_s[2 * 4];
+    if (predicated) {
+        const long long n = ctl->step_base + step_off + 1;
+        if (ctl->obs_every <= 0 || (n % ctl->obs_every) != 0) return;
+    }
+    const int s = blockIdx.x, b = blockIdx.y;
+    const double2 *f = psi + ((size_t)b * g.n_l + l_of_state[s]) * g.n_r;
+    const double *ph = phi + (size_t)s * g.n_r;
+    double red[2] = {0.0, 0.0};
+    for (int j = threadIdx.x; j < g.n_r; j += 128) {
+        const double w = __ldg(ph + j);
+        const double2 v = f[j];
+        red[0] = fma(w, v.x, red[0]); red[1] = fma(w, v.y, red[1]);
+    }
+    block_reduce<128, 2>(red, red_s);
+    if (threadIdx.x == 0) amp[(size_t)b * n_states + s] = make_double2(red[0], red[1]);
+}
+
+// Assemble the row {norm, <z>, <z''>, pop...} of every member (Eq. 34, Eq. 36).  grid = batch, block 128.
+// t_direct: if use_direct, the time for -E(t); else t_{n+1} = t0 + (n+1) dt of the step being logged.
+__global__ void __launch_bounds__(128) obs_final_kernel(GridDev g, const double *partials, int chunks,
+                                                        const double2 *amp, int n_states, const tdse_pulse *pulse,
+                                                        const Ctl *ctl, int step_off, int predicated, int use_direct,
+                                                        double t_direct, double *rows) {
+    __shared__ double red_s[3 * 4];
+    long long row = 0;
+    double t = t_direct;
+    if (!use_direct) {
+        const long long n = ctl->step_base + step_off + 1;
+        if (predicated && (ctl->obs_every <= 0 || (n % ctl->obs_every) != 0)) return;
+        row = n / ctl->obs_every - 1;
+        t = time_at(ctl->t0, (double)n, ctl->dt);
+    }
+    const int b = blockIdx.x, W = 3 + n_states;
+    double red[3] = {0.0, 0.0, 0.0};
+    for (int i = threadIdx.x; i < chunks; i += 128) {
+        const double *p = partials + ((size_t)b * chunks + i) * 3;
+        red[0] += p[0]; red[1] += p[1]; red[2] += p[2];
+    }
+    block_reduce<128, 3>(red, red_s);
+    double *o = rows + ((size_t)row * g.batch + b) * W;
+    if (threadIdx.x == 0) {
+        o[0] = g.dr * red[0];
+        o[1] = 2.0 * g.dr * red[1];
+        o[2] = -pulse_E(pulse[b], t) - 2.0 * g.z * g.dr * red[2];
+    }
+    for (int s = threadIdx.x; s < n_states; s += 128) {
+        const double2 a = amp[(size_t)b * n_states + s];
+        const double ar = g.dr * a.x, ai = g.dr * a.y;
+        o[3 + s] = ar * ar + ai * ai;
+    }
+}
+
+}  // namespace tdse

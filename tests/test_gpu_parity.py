@@ -1,0 +1,446 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same seeded
+inputs.  Tolerances are the north star's: rel-L2 <= 1e-13 per H.psi, <= 1e-9 on a propagated wavefunction,
+norm and populations within 1e-10 absolute (fp64 throughout).  Run with `-m gpu` on the B200 box.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1308_1856_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL_H = 1e-13
+TOL_PSI = 1e-9
+TOL_OBS = 1e-10
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_1308_1856_b200 import binding
+    oracle.set_threads(8)
+    return binding
+
+
+def rel_l2(a, b):
+    return float(np.linalg.norm((a - b).ravel()) / max(np.linalg.norm(b.ravel()), 1e-300))
+
+
+def cfg_shape(n_r, dr, n_l, fd, batch=1, index=0):
+    return dict(index=index, n_r=n_r, dr=dr, n_l=n_l, fd_order=fd, batch=batch, name="adhoc")
+
+
+def both(B, c):
+    g = oracle.make_grid(c["n_r"], c["dr"], c["n_l"], c["fd_order"], batch=c["batch"])
+    h = B.Tdse(c["n_r"], c["dr"], c["n_l"], c["fd_order"], batch=c["batch"])
+    return g, h
+
+
+def bound_pack(g, specs):
+    """specs: [(l, n_index)] -> (l_of_state, phi) from the oracle's eigen-solver (inputs to both sides)."""
+    ls, phis = [], []
+    for l, k in specs:
+        _, phi = oracle.bound_states(g, l, k + 1)
+        ls.append(l)
+        phis.append(phi[k])
+    return np.array(ls, dtype=np.int32), np.array(phis)
+
+
+# ------------------------------------------------------------------------------------------------- H.psi
+SHAPES_H = [
+    (100, 0.2, 3, 3, 1), (100, 0.2, 3, 5, 1),           # the tiny grid of the dense pins
+    (500, 0.2, 8, 3, 1),                                # CFG1
+    (257, 0.1, 7, 5, 2), (129, 0.1, 9, 3, 3),           # ragged in r and l, batched
+    (1, 0.3, 1, 3, 1), (2, 0.3, 2, 5, 1), (3, 0.1, 17, 5, 2),   # degenerate sizes
+    (4000, 0.1, 32, 5, 1),                              # CFG2
+    (1000, 0.1, 33, 3, 1),
+]
+
+
+@pytest.mark.parametrize("shape", SHAPES_H)
+def test_apply_H_parity(B, shape):
+    import torch
+    n_r, dr, n_l, fd, batch = shape
+    c = cfg_shape(n_r, dr, n_l, fd, batch, index=n_r % 7)
+    g, h = both(B, c)
+    psi = wl.random_state(c)
+    e = wl.random_fields(c)
+    ref = oracle.apply_H(g, psi, e)
+    d_in = torch.from_numpy(psi).cuda()
+    d_out = torch.full_like(d_in, float("nan"))
+    h.apply_H(d_in, d_out, e)
+    torch.cuda.synchronize()
+    got = d_out.cpu().numpy()
+    assert np.isfinite(got.view(np.float64)).all()
+    assert rel_l2(got, ref) <= TOL_H
+    # per l-block as well: a wrong centrifugal or coupling term in one block must not hide in the total
+    for l in range(n_l):
+        assert rel_l2(got[:, l], ref[:, l]) <= TOL_H
+    # the input is untouched and a second field value takes effect
+    assert np.array_equal(d_in.cpu().numpy(), psi)
+    h.apply_H(d_in, d_out, e * -2.0)
+    torch.cuda.synchronize()
+    assert rel_l2(d_out.cpu().numpy(), oracle.apply_H(g, psi, e * -2.0)) <= TOL_H
+    h.close()
+
+
+@pytest.mark.parametrize("name", ["cfg3", "cfg4", "cfg5"])
+def test_apply_H_full_size(B, name):
+    """BASELINE's full sizes, in the launch configuration bench.py times."""
+    import torch
+    c = wl.config(name)
+    g, h = both(B, c)
+    psi = wl.random_state(c)
+    e = wl.random_fields(c)
+    ref = oracle.apply_H(g, psi, e)
+    d_in = torch.from_numpy(psi).cuda()
+    d_out = torch.empty_like(d_in)
+    h.apply_H(d_in, d_out, e)
+    torch.cuda.synchronize()
+    got = d_out.cpu().numpy()
+    assert rel_l2(got, ref) <= TOL_H
+    worst = max(rel_l2(got[b, l], ref[b, l]) for b in range(0, c["batch"], 37) for l in range(c["n_l"]))
+    assert worst <= TOL_H
+    h.close()
+
+
+def test_apply_H_hermitian_and_structural_zeros(B):
+    """Properties that hold at any size: <x|Hy> = <Hx|y>; H^k of an l=0 state leaves blocks l>k exactly zero."""
+    import torch
+    c = cfg_shape(777, 0.1, 6, 5, 1, index=3)
+    _, h = both(B, c)
+    x = torch.from_numpy(wl.random_state(c)).cuda()
+    y = torch.from_numpy(wl.random_state(c, seed_extra=11)).cuda()
+    hx, hy = torch.empty_like(x), torch.empty_like(y)
+    h.apply_H(x, hx, 0.07)
+    h.apply_H(y, hy, 0.07)
+    a = torch.vdot(x.flatten(), hy.flatten()).item()
+    b = torch.vdot(hx.flatten(), y.flatten()).item()
+    assert abs(a - b) <= 1e-12 * abs(a)
+    z = torch.zeros_like(x)
+    z[:, 0, :] = x[:, 0, :]
+    w = torch.empty_like(z)
+    for k in range(1, 4):
+        h.apply_H(z, w, 0.05)
+        torch.cuda.synchronize()
+        assert torch.count_nonzero(w[:, k + 1:, :]).item() == 0
+        z, w = w, z
+    h.close()
+
+
+# ------------------------------------------------------------------------------------------------- steppers
+def stepping_case(name="cfg1", **over):
+    c = wl.config(name, **over)
+    return c
+
+
+def run_pair_fixed(B, c, prop, nsteps, psi0, t0, dt, obs_every=1, states=None, opts=None, **kw):
+    g, h = both(B, c)
+    for k, v in (opts or {}).items():
+        h.set_option(k, v)
+    pulses = wl.pulses(c)
+    h.set_pulse(pulses)
+    st = None
+    if states is not None:
+        st = bound_pack(g, states)
+        h.set_bound_states(*st)
+    h.set_state(psi0)
+    if prop == "taylor":
+        ref, robs = oracle.step_taylor(g, pulses, psi0, kw["order"], t0, dt, nsteps, states=st, obs_every=obs_every)
+        h.step_taylor(kw["order"], t0, dt, nsteps, obs_every)
+    elif prop == "rk4":
+        ref, robs = oracle.step_rk4(g, pulses, psi0, t0, dt, nsteps, states=st, obs_every=obs_every)
+        h.step_rk4(t0, dt, nsteps, obs_every)
+    elif prop == "lanczos":
+        ref, robs = oracle.step_lanczos(g, pulses, psi0, kw["K"], kw["order"], t0, dt, nsteps, states=st,
+                                        obs_every=obs_every)
+        h.step_lanczos(kw["K"], kw["order"], t0, dt, nsteps, obs_every)
+    got = h.get_state()
+    gobs = h.obs_log() if obs_every else None
+    return h, got, ref, gobs, robs
+
+
+def check_fixed(got, ref, gobs, robs):
+    assert np.isfinite(got.view(np.float64)).all()
+    assert rel_l2(got, ref) <= TOL_PSI
+    if gobs is not None:
+        assert gobs.shape == robs.shape
+        assert np.max(np.abs(gobs[..., 0] - robs[..., 0])) <= TOL_OBS          # norm
+        assert np.max(np.abs(gobs[..., 3:] - robs[..., 3:]), initial=0.0) <= TOL_OBS   # populations
+        scale = max(1.0, float(np.max(np.abs(robs[..., 1:3]))))
+        assert np.max(np.abs(gobs[..., 1:3] - robs[..., 1:3])) <= 1e-9 * scale  # dipole, acceleration
+
+
+@pytest.mark.parametrize("order,fd,use_graph,nsteps", [(4, 3, 1, 203), (4, 3, 0, 37), (1, 3, 1, 33), (2, 5, 1, 64),
+                                                       (6, 5, 1, 75), (10, 3, 1, 50)])
+def test_taylor_cfg1_window(B, order, fd, use_graph, nsteps):
+    """CFG1 shape, stable dt (dt_eff rule), window at the pulse peak from the populated state S4."""
+    c = stepping_case("cfg1", fd_order=fd, order=order)
+    dt = wl.dt_eff(c, "taylor", order)
+    t0 = wl.window(c, nsteps, dt)
+    psi0 = wl.populated_state(c)
+    h, got, ref, gobs, robs = run_pair_fixed(B, c, "taylor", nsteps, psi0, t0, dt, 1, [(0, 0), (1, 0)],
+                                             {"use_graph": use_graph, "taylor_block": 0}, order=order)
+    check_fixed(got, ref, gobs, robs)
+    assert h.launch_count() > 0
+    h.close()
+
+
+def test_taylor_batched_ragged_obs_every(B):
+    c = wl.config("cfg5", n_r=300, batch=5, n_l=11)
+    dt = wl.dt_eff(c)
+    nsteps = 90
+    t0 = wl.window(c, nsteps, dt)
+    psi0 = wl.populated_state(c)
+    h, got, ref, gobs, robs = run_pair_fixed(B, c, "taylor", nsteps, psi0, t0, dt, 7, [(0, 0), (0, 1), (3, 0)],
+                                             {"taylor_block": 0}, order=6)
+    assert gobs.shape[0] == nsteps // 7
+    check_fixed(got, ref, gobs, robs)
+    # per-member parity: members see different intensities
+    for b in range(c["batch"]):
+        assert rel_l2(got[b], ref[b]) <= TOL_PSI
+    h.close()
+
+
+def test_taylor_field_sample_start_and_continuation(B):
+    """field_sample = 1 (H frozen at t_n) and two consecutive calls equal one long call."""
+    c = wl.config("tiny")
+    dt = wl.dt_eff(c)
+    psi0 = wl.populated_state(c)
+    g, h = both(B, c)
+    h.set_option("field_sample", 1)
+    h.set_option("taylor_block", 0)
+    pulses = wl.pulses(c)
+    h.set_pulse(pulses)
+    h.set_state(psi0)
+    t0 = wl.window(c, 60, dt)
+    h.step_taylor(4, t0, dt, 25)
+    h.step_taylor(4, t0 + 25 * dt, dt, 35)
+    ref, _ = oracle.step_taylor(g, pulses, psi0, 4, t0, dt, 25, field_sample=1)
+    ref, _ = oracle.step_taylor(g, pulses, ref, 4, t0 + 25 * dt, dt, 35, field_sample=1)
+    assert rel_l2(h.get_state(), ref) <= TOL_PSI
+    h.close()
+
+
+@pytest.mark.parametrize("fd,batch,use_graph", [(5, 1, 1), (3, 2, 0)])
+def test_rk4_parity(B, fd, batch, use_graph):
+    c = wl.config("cfg2", n_r=600, n_l=9, fd_order=fd, batch=batch)
+    dt = wl.dt_eff(c, "rk4", 4)
+    nsteps = 70
+    t0 = wl.window(c, nsteps, dt)
+    psi0 = wl.populated_state(c)
+    h, got, ref, gobs, robs = run_pair_fixed(B, c, "rk4", nsteps, psi0, t0, dt, 5, [(0, 0)], {"use_graph": use_graph})
+    check_fixed(got, ref, gobs, robs)
+    h.close()
+
+
+@pytest.mark.parametrize("fd,K", [(3, 16), (5, 7)])
+def test_lanczos_parity_and_internals(B, fd, K):
+    c = wl.config("cfg4", n_r=700, n_l=10, fd_order=fd)
+    dt = wl.dt_eff(c, "lanczos", 12)
+    nsteps = 20
+    t0 = wl.window(c, nsteps, dt)
+    psi0 = wl.populated_state(c)
+    h, got, ref, gobs, robs = run_pair_fixed(B, c, "lanczos", nsteps, psi0, t0, dt, 4, [(0, 0)], None, K=K, order=12)
+    check_fixed(got, ref, gobs, robs)
+    # internals of one step from the same start (alpha, beta, coefficients, sub-step count)
+    g = oracle.make_grid(c["n_r"], c["dr"], c["n_l"], fd)
+    pulses = wl.pulses(c)
+    e_mid = oracle.pulse_E(pulses[0], t0 + 0.5 * dt)
+    info = oracle.lanczos_internals(g, psi0, e_mid, K, 12, dt)
+    h.set_state(psi0)
+    h.step_lanczos(K, 12, t0, dt, 1)
+    gi = h.lanczos_info(K)
+    assert gi["m"][0] == info["m"] and gi["n_sub"][0] == info["n_sub"]
+    scale = np.max(np.abs(info["alpha"]))
+    assert np.max(np.abs(gi["alpha"][0] - info["alpha"])) <= 1e-11 * scale
+    assert np.max(np.abs(gi["beta"][0, :K - 1] - info["beta"][:K - 1])) <= 1e-9 * scale
+    assert np.max(np.abs(gi["coef"][0] - info["coef"])) <= 1e-9
+    h.close()
+
+
+def test_lanczos_breakdown_field_free_eigenstate(B):
+    """E = 0 and psi = discrete 1s: beta_1 is at rounding level -> breakdown path (R-G17); the state only gets a phase."""
+    c = wl.config("tiny", intensity=0.0)
+    g, h = both(B, c)
+    en, phi = oracle.bound_states(g, 0, 1)
+    psi0 = wl.ground_state(c, phi[0])
+    pulses = wl.pulses(c)
+    h.set_pulse(pulses)
+    h.set_bound_states(np.array([0], dtype=np.int32), phi)
+    h.set_option("lanczos_beta_tol", 1e-9)
+    h.set_state(psi0)
+    dt, n = 0.01, 40
+    h.step_lanczos(8, 12, 0.0, dt, n, 1)
+    got = h.get_state()
+    assert h.lanczos_info(8)["m"][0] == 1
+    expect = np.exp(-1j * en[0] * dt * n)
+    amp = c["dr"] * np.sum(phi[0] * got[0, 0])
+    assert abs(amp - expect) <= 1e-10
+    rows = h.obs_log()
+    assert np.max(np.abs(rows[:, 0, 0] - 1.0)) <= TOL_OBS and np.max(np.abs(rows[:, 0, 3] - 1.0)) <= TOL_OBS
+    ref, _ = oracle.step_lanczos(g, pulses, psi0, 8, 12, 0.0, dt, n, beta_tol=1e-9)
+    assert rel_l2(got, ref) <= TOL_PSI
+    h.close()
+
+
+def test_rk45_adaptive_replay_parity(B):
+    """Adaptive DP5(4) on the GPU; the oracle replays the GPU's accepted-dt sequence (R-G20) and must agree on the final
+    state; the oracle's own adaptive run must make the same number of decisions; the GPU replays the oracle's list."""
+    c = wl.config("cfg2", n_r=500, n_l=6)
+    g, h = both(B, c)
+    pulses = wl.pulses(c)
+    h.set_pulse(pulses)
+    psi0 = wl.populated_state(c)
+    t0 = 0.5 * c["t_pulse"]
+    t1 = t0 + 0.05
+    rtol = 1e-8
+    h.set_state(psi0)
+    info = h.step_rk45(t0, t1, 1e-4, rtol)
+    got = h.get_state()
+    assert info["n_accept"] > 20 and len(info["dt"]) == info["n_accept"]
+    assert abs(np.sum(info["dt"]) - (t1 - t0)) <= 1e-12
+    assert np.all(info["err"] <= 1.0)
+    ref, rinfo = oracle.step_rk45(g, pulses, psi0, t0, t1, 1e-4, rtol, dt_replay=info["dt"])
+    assert np.max(rinfo["err"]) <= 1.05
+    assert rel_l2(got, ref) <= TOL_PSI
+    own, oinfo = oracle.step_rk45(g, pulses, psi0, t0, t1, 1e-4, rtol)
+    assert abs(oinfo["n_accept"] - info["n_accept"]) <= 2 and abs(oinfo["n_reject"] - info["n_reject"]) <= 2
+    assert rel_l2(got, own) <= 1e-7
+    # GPU replay of the oracle's sequence, then a fixed-step propagator from the swapped state slot
+    h.set_state(psi0)
+    rep = h.step_rk45(t0, t1, 1e-4, rtol, dt_replay=oinfo["dt"])
+    assert rep["n_accept"] == oinfo["n_accept"] and rep["n_reject"] == 0
+    assert rel_l2(h.get_state(), own) <= TOL_PSI
+    dt = wl.dt_eff(c, "rk4", 4)
+    h.step_rk4(t1, dt, 10)
+    ref2, _ = oracle.step_rk4(g, pulses, own, t1, dt, 10)
+    assert rel_l2(h.get_state(), ref2) <= TOL_PSI
+    h.step_taylor(4, t1, dt, 11)
+    ref3, _ = oracle.step_taylor(g, pulses, ref2, 4, t1, dt, 11)
+    assert rel_l2(h.get_state(), ref3) <= TOL_PSI
+    h.close()
+
+
+def test_rk45_batched_with_rejects(B):
+    c = wl.config("cfg5", n_r=200, n_l=5, batch=3, fd_order=5)
+    g, h = both(B, c)
+    pulses = wl.pulses(c)
+    h.set_pulse(pulses)
+    psi0 = wl.populated_state(c)
+    t0 = 0.5 * c["t_pulse"]
+    h.set_state(psi0)
+    info = h.step_rk45(t0, t0 + 0.02, 5e-3, 1e-9)     # dt_init far too large: forces rejects
+    assert info["n_reject"] >= 1
+    ref, rinfo = oracle.step_rk45(g, pulses, psi0, t0, t0 + 0.02, 5e-3, 1e-9, dt_replay=info["dt"])
+    assert rel_l2(h.get_state(), ref) <= TOL_PSI
+    h.close()
+
+
+def test_observables_direct(B):
+    c = wl.config("cfg1", batch=2)
+    g, h = both(B, c)
+    st = bound_pack(g, [(0, 0), (1, 0), (0, 1)])
+    h.set_bound_states(*st)
+    pulses = wl.pulses(c)
+    h.set_pulse(pulses)
+    psi = wl.populated_state(c)
+    h.set_state(psi)
+    t = 0.37 * c["t_pulse"]
+    got = h.observables(t)
+    e_now = [oracle.pulse_E(p, t) for p in pulses]
+    ref = oracle.observables(g, psi, e_now, st)
+    assert np.max(np.abs(got[:, 0] - ref[:, 0])) <= TOL_OBS
+    assert np.max(np.abs(got[:, 3:] - ref[:, 3:])) <= TOL_OBS
+    assert np.max(np.abs(got[:, 1:3] - ref[:, 1:3])) <= 1e-10 * max(1.0, np.max(np.abs(ref[:, 1:3])))
+    h.close()
+
+
+# ------------------------------------------------------------------------------------------------- full sizes
+def test_full_size_cfg5_taylor_steps(B):
+    """CFG5 at full size (256 members x 16 x 2000) in the configuration bench.py times: a few steps against the oracle."""
+    c = wl.config("cfg5")
+    dt = wl.dt_eff(c)
+    nsteps = 4
+    t0 = wl.window(c, nsteps, dt)
+    psi0 = wl.populated_state(c)
+    g, h = both(B, c)
+    pulses = wl.pulses(c)
+    h.set_pulse(pulses)
+    h.set_state(psi0)
+    h.step_taylor(6, t0, dt, nsteps)
+    got = h.get_state()
+    ref, _ = oracle.step_taylor(g, pulses, psi0, 6, t0, dt, nsteps)
+    assert rel_l2(got, ref) <= TOL_PSI
+    for b in (0, 17, 255):
+        assert rel_l2(got[b], ref[b]) <= TOL_PSI
+    e_now = [oracle.pulse_E(p, t0 + nsteps * dt) for p in pulses]
+    obs = h.observables(t0 + nsteps * dt)
+    robs = oracle.observables(g, ref, e_now)
+    assert np.max(np.abs(obs[:, 0] - robs[:, 0])) <= TOL_OBS
+    h.close()
+
+
+def test_full_size_cfg3_taylor10_and_cfg2_rk4(B):
+    for name, prop, kw in (("cfg3", "taylor", dict(order=10)), ("cfg2", "rk4", {})):
+        c = wl.config(name)
+        dt = wl.dt_eff(c)
+        nsteps = 3
+        t0 = wl.window(c, nsteps, dt)
+        psi0 = wl.populated_state(c)
+        h, got, ref, gobs, robs = run_pair_fixed(B, c, prop, nsteps, psi0, t0, dt, 1, None, None, **kw)
+        check_fixed(got, ref, gobs, robs)
+        h.close()
+
+
+def test_full_size_cfg4_lanczos_step(B):
+    c = wl.config("cfg4")
+    dt = wl.dt_eff(c)
+    t0 = wl.window(c, 1, dt)
+    psi0 = wl.populated_state(c)
+    h, got, ref, gobs, robs = run_pair_fixed(B, c, "lanczos", 1, psi0, t0, dt, 1, None, None, K=16, order=12)
+    check_fixed(got, ref, gobs, robs)
+    h.close()
+
+
+# ------------------------------------------------------------------------------------------------- ABI behaviour
+def test_error_codes_and_lifecycle(B):
+    import ctypes as C
+    L = B.lib()
+    hp = C.c_void_p()
+    bad = B.Grid(100, 0.1, 3, 4, 0, 1.0, 1)
+    assert L.tdse_create(C.byref(bad), C.byref(hp)) == -5          # fd_order 4
+    bad = B.Grid(100, 0.1, 3, 3, 1, 1.0, 1)
+    assert L.tdse_create(C.byref(bad), C.byref(hp)) == -5          # velocity gauge: not built
+    bad = B.Grid(0, 0.1, 3, 3, 0, 1.0, 1)
+    assert L.tdse_create(C.byref(bad), C.byref(hp)) == -1
+    for _ in range(20):                                            # create/destroy cycles
+        h = B.Tdse(300, 0.1, 4, 5, batch=2)
+        h.set_pulse((0.05, 0.057, 2.0, 0.0))
+        h.set_state(np.ones(h.shape, dtype=np.complex128))
+        h.step_taylor(4, 0.0, 1e-4, 3, 1)
+        h.close()
+    h = B.Tdse(300, 0.1, 4, 5)
+    with pytest.raises(B.TdseError):
+        h.step_taylor(0, 0.0, 1e-3, 1)
+    with pytest.raises(B.TdseError):
+        h.step_lanczos(33, 12, 0.0, 1e-3, 1)
+    with pytest.raises(B.TdseError):
+        h.set_option("no_such_option", 1.0)
+    h.step_taylor(4, 0.0, 1e-3, 0)                                 # zero steps: no-op
+    assert np.count_nonzero(h.get_state()) == 0
+    # unstable literal step size overflows and is reported ("not always stable")
+    c = wl.config("cfg1")
+    h2 = B.Tdse(c["n_r"], c["dr"], c["n_l"], 3)
+    h2.set_pulse(wl.pulses(c))
+    h2.set_state(wl.populated_state(c))
+    h2.step_taylor(4, 0.0, c["dt_cfg"], 400, 50)
+    with pytest.raises(B.TdseError) as ei:
+        h2.obs_log()
+    assert ei.value.code == -4
+    h.close()
+    h2.close()
