@@ -1,0 +1,370 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the TDSE hot path on B200 (one JSON line on stdout, rank 0).
+
+Own arm (default): workload CFG5 of BASELINE.json (256 independent hydrogen wavefunctions per GPU, N_r = 2000,
+L = 16, 3-point stencil, Taylor order 6; the largest Taylor grid, sharded over ranks by members, weak scaling).
+A "step" is one Taylor time step of the whole batch: field table -> H.psi x order with the propagator arithmetic
+fused -> state update.  `value` = Gpoint-updates/s of H(t)psi = members * L * N_r * order * steps / device time.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg5] [--impl reference] [--no-extra]
+
+Reference arm (--impl reference): the CPU oracle (oracle/), as it stands, on the host cores, on a bounded sample
+of the same workload.  See DESIGN.md "Measurement".
+"""
+import argparse
+import json
+import math
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1308_1856_b200 import workloads as wl  # noqa: E402
+
+METRIC = "Gpoint-updates/s of H(t)psi (Taylor step)"
+UNIT = "Gpoint-updates/s"
+
+
+def host_cores():
+    try:
+        return len(os.sched_getaffinity(0))
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+# ------------------------------------------------------------------------------------------ clocks sampler
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons of one GPU during the timed region (NVML; nvidia-smi fallback)."""
+
+    def __init__(self, index, period=0.02):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.samples, self.reasons, self.stop_flag = [], set(), False
+        self.max_mhz = None
+        self.nv = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.dev = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.dev, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        names = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+                 0x80: "hw_power_brake", 0x2: "applications_clocks_setting"}
+        while not self.stop_flag:
+            if self.nv is not None:
+                try:
+                    self.samples.append(self.nv.nvmlDeviceGetClockInfo(self.dev, self.nv.NVML_CLOCK_SM))
+                    r = self.nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.dev)
+                    for bit, nm in names.items():
+                        if r & bit:
+                            self.reasons.add(nm)
+                except Exception:
+                    pass
+            else:
+                try:
+                    import subprocess
+                    out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=clocks.sm,clocks.max.sm,"
+                                          "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+                                          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap",
+                                          "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5)
+                    f = [x.strip() for x in out.stdout.strip().split(",")]
+                    self.samples.append(int(f[0]))
+                    self.max_mhz = int(f[1])
+                    for nm, v in zip(["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"], f[2:]):
+                        if v.lower().startswith("active"):
+                            self.reasons.add(nm)
+                except Exception:
+                    pass
+            time.sleep(self.period)
+
+    def result(self):
+        self.stop_flag = True
+        self.join(timeout=5)
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------------------ CPU oracle timing
+def time_oracle(c, order, dt, t0, members, steps, warmup, threads):
+    """Oracle Taylor steps on `members` members of the workload; returns (seconds for `steps` steps)."""
+    import oracle
+    oracle.set_threads(threads)
+    cs = dict(c)
+    cs["batch"] = members
+    g = oracle.make_grid(cs["n_r"], cs["dr"], cs["n_l"], cs["fd_order"], batch=members)
+    pulses = wl.pulses(c)[:members]
+    psi = wl.populated_state(cs)
+    if warmup:
+        psi, _ = oracle.step_taylor(g, pulses, psi, order, t0, dt, warmup)
+    t = time.perf_counter()
+    psi, _ = oracle.step_taylor(g, pulses, psi, order, t0 + warmup * dt, dt, steps)
+    el = time.perf_counter() - t
+    assert np.isfinite(psi.view(np.float64)).all()
+    return el
+
+
+def cpu_baseline(c, order, dt, t0, budget_s=12.0):
+    cores = host_cores()
+    members = min(c["batch"], 16)
+    pts = members * c["n_l"] * c["n_r"]
+    probe = time_oracle(c, order, dt, t0, members, 2, 1, cores)
+    steps = int(max(2, min(2000, budget_s / max(probe / 2, 1e-6))))
+    el = time_oracle(c, order, dt, t0, members, steps, 0, cores)
+    return {"value": pts * order * steps / el / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{members} of {c['batch']} members x {steps} Taylor-{order} steps (same grid, dt, pulses), "
+                      f"OpenMP over l rows, {el:.1f} s", "s_per_step_full_batch": el / steps * c["batch"] / members}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    c = wl.config(args.workload)
+    order = c["order"]
+    dt = wl.dt_eff(c)
+    t0 = wl.window(c, args.steps + args.warmup, dt)
+    cores = host_cores()
+    members = min(c["batch"], 16)
+    el = time_oracle(c, order, dt, t0, members, args.steps, args.warmup, cores)
+    pts = members * c["n_l"] * c["n_r"]
+    val = pts * order * args.steps / el / 1e9
+    sample = f"{members} of {c['batch']} members per step (same grid, dt, pulses); oracle/ as it stands, OpenMP over l rows"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": el / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{args.workload} (BASELINE.json configs[{c['index'] - 1}]), bounded sample",
+                       "taylor_order": order, "dt_eff": dt},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------ own arm
+def run_own(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1308_1856_b200 import binding, sharding
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback "
+                         "(use --impl reference for the oracle arm)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    c = wl.config(args.workload)
+    order, B, L, N = c["order"], c["batch"], c["n_l"], c["n_r"]
+    dt = wl.dt_eff(c)
+    K, W = args.steps, args.warmup
+    t0 = wl.window(c, K + W, dt)
+    # weak scaling: every rank runs a full batch; rank r takes members [r*B, (r+1)*B) of a world*B-member scan
+    cg = wl.config(args.workload, batch=B * world)
+    first, cnt = sharding.member_slice(B * world, rank, world)
+    pulses = wl.pulses(cg)[first:first + cnt]
+    psi0 = wl.populated_state(c)                       # S3/S4 state: every l block populated (no denormals)
+    pts = B * L * N
+
+    h = binding.Tdse(N, c["dr"], L, c["fd_order"], batch=B)
+    h.set_option("taylor_block", 0 if args.no_block else 1)
+    h.set_option("graph_steps", args.graph_steps)
+    h.set_pulse(pulses)
+    stream = torch.cuda.Stream()
+    pinned = torch.empty((B, L, N), dtype=torch.complex128).pin_memory()
+    pinned.numpy()[...] = psi0
+    pin_out = torch.empty((B, L, N), dtype=torch.complex128).pin_memory()
+
+    with torch.cuda.stream(stream):
+        h.set_state(pinned.numpy(), stream=stream)
+        # ---- device-resident timing
+        h.step_taylor(order, t0, dt, W, 0, stream=stream)
+        stream.synchronize()
+        sharding.barrier()
+        torch.cuda.synchronize()
+        sampler = ClockSampler(local)
+        sampler.start()
+        l0 = h.launch_count()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record(stream)
+        h.step_taylor(order, t0 + W * dt, dt, K, 0, stream=stream)
+        ev1.record(stream)
+        stream.synchronize()
+        torch.cuda.synchronize()
+        sharding.barrier()
+        ms = ev0.elapsed_time(ev1)
+        launches = h.launch_count() - l0
+        clocks = sampler.result()
+        blocked = h.taylor_was_blocked()
+        obs = h.observables(t0 + (W + K) * dt, stream=stream)
+        norm_dev = float(np.max(np.abs(obs[:, 0] - 1.0)))
+        ms = sharding.max_over_ranks(ms)
+
+        # ---- end to end through the C ABI with host buffers: upload state + pulses, K steps, download rows + state
+        sharding.barrier()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        tw0 = time.perf_counter()
+        e0.record(stream)
+        h.set_pulse(pulses)
+        h.set_state(pinned.numpy(), stream=stream)
+        h.step_taylor(order, t0, dt, K, 0, stream=stream)
+        rows = h.observables(t0 + K * dt, stream=stream)
+        h.get_state(pin_out.numpy(), stream=stream)
+        e1.record(stream)
+        stream.synchronize()
+        tw1 = time.perf_counter()
+        ms_e2e = max(e0.elapsed_time(e1), (tw1 - tw0) * 1e3)
+        ms_e2e = sharding.max_over_ranks(ms_e2e)
+        h2d = (pinned.numel() * 16 + 32 * B) / K
+        d2h = (pin_out.numel() * 16 + rows.size * 8) / K
+
+    total_pts = pts * world
+    value = total_pts * order * K / (ms * 1e-3) / 1e9
+    e2e_val = total_pts * order * K / (ms_e2e * 1e-3) / 1e9
+
+    # ---- roofline of the dominant kernel (per launch): algorithmic bytes / average launch duration
+    peak, peak_src = measured_peaks()
+    if blocked:
+        bytes_step = 32.0 * pts                         # read psi once, write psi once (all orders in shared memory)
+        kname, n_dom = "taylor_blocked_kernel", K
+    else:
+        bytes_step = (64.0 * order - 32.0) * pts        # k=1: 16R+32W, 1<k<P: 32R+32W, k=P: 32R+16W
+        kname, n_dom = "tile_kernel<EpiTaylor>", K * order
+    achieved = bytes_step * K / (ms * 1e-3) / 1e9
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        try:
+            traffic = json.load(open(tpath)).get(kname)
+        except Exception:
+            traffic = None
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": traffic, "kernel": kname, "launches": n_dom, "us_per_launch": ms * 1e3 / n_dom,
+                "algorithmic_bytes_per_launch": bytes_step * K / n_dom, "peak_source": peak_src}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": f"{args.workload} (BASELINE.json configs[{c['index'] - 1}]): {B} members/GPU x L={L} x "
+                                   f"N_r={N}, {c['fd_order']}-point, Taylor order {order}",
+                       "dt_cfg": c["dt_cfg"], "dt_eff": dt, "window": "pulse peak", "state": "S4 populated",
+                       "points_per_gpu": pts, "taylor_blocked": bool(blocked), "graph_steps": args.graph_steps,
+                       "l2": "inputs_exceed_l2 (state arrays 131 MB each > 126 MB L2)", "parallelism": f"batch x{world}"},
+            "clocks": clocks, "roofline": roofline,
+            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "what": "set_pulse + set_state(host, pinned) + K steps + observables + get_state(host) via the C ABI"},
+            "gpu_launches": int(launches), "max_norm_drift": norm_dev}
+
+    if rank == 0 and not args.no_extra and world == 1:
+        line["extra"] = extra_measurements(binding, torch, stream)
+    if rank == 0 and world == 1 and not args.no_cpu:
+        line["cpu_baseline"] = cpu_baseline(c, order, dt, t0)
+    h.close()
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def extra_measurements(binding, torch, stream):
+    """Secondary figures (not the headline): bare H.psi on the CFG4 grid and s/step of the other configs."""
+    out = {}
+    peak, _ = measured_peaks()
+    with torch.cuda.stream(stream):
+        for name in ("cfg4", "cfg3"):
+            c = wl.config(name)
+            h = binding.Tdse(c["n_r"], c["dr"], c["n_l"], c["fd_order"], batch=c["batch"])
+            x = torch.from_numpy(wl.random_state(c)).cuda()
+            y = torch.empty_like(x)
+            for _ in range(5):
+                h.apply_H(x, y, 0.05, stream=stream)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            n = 50
+            e0.record(stream)
+            for _ in range(n):
+                h.apply_H(x, y, 0.05, stream=stream)
+            e1.record(stream)
+            stream.synchronize()
+            us = e0.elapsed_time(e1) * 1e3 / n
+            pts = x.numel()
+            out[f"apply_H_{name}"] = {"us": us, "gpoints_per_s": pts / us / 1e3, "gbs_algorithmic": 32.0 * pts / us / 1e3,
+                                      "frac_of_hbm_peak": 32.0 * pts / us / 1e3 / peak,
+                                      "note": "L2-resident" if pts * 32 < 100e6 else "exceeds L2"}
+            del x, y
+            h.close()
+        for name, nsteps in (("cfg1", 2000), ("cfg2", 400), ("cfg3", 100), ("cfg4", 10)):
+            c = wl.config(name)
+            h = binding.Tdse(c["n_r"], c["dr"], c["n_l"], c["fd_order"], batch=c["batch"])
+            h.set_pulse(wl.pulses(c))
+            h.set_state(wl.populated_state(c), stream=stream)
+            dt = wl.dt_eff(c)
+            t0 = wl.window(c, 2 * nsteps, dt)
+
+            def go(n, t):
+                if c["propagator"] == "taylor":
+                    h.step_taylor(c["order"], t, dt, n, 1 if name in ("cfg1", "cfg3") else 0, stream=stream)
+                elif c["propagator"] == "rk4":
+                    h.step_rk4(t, dt, n, 0, stream=stream)
+                else:
+                    h.step_lanczos(c["krylov_dim"], c["order"], t, dt, n, 0, stream=stream)
+            go(max(2, nsteps // 10), t0)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            go(nsteps, t0)
+            e1.record(stream)
+            stream.synchronize()
+            ms = e0.elapsed_time(e1)
+            n_h = {"taylor": c["order"], "rk4": 4, "lanczos": c.get("krylov_dim", 0)}[c["propagator"]]
+            pts = c["batch"] * c["n_l"] * c["n_r"]
+            out[f"step_{name}"] = {"propagator": c["propagator"], "us_per_step": ms * 1e3 / nsteps, "dt_eff": dt,
+                                   "gpoint_updates_per_s": pts * n_h * nsteps / (ms * 1e-3) / 1e9,
+                                   "blocked": h.taylor_was_blocked() if c["propagator"] == "taylor" else None}
+            h.close()
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
+    ap.add_argument("--impl", default="own", choices=["own", "reference"])
+    ap.add_argument("--workload", default="cfg5")
+    ap.add_argument("--graph-steps", type=int, default=16)
+    ap.add_argument("--no-block", action="store_true", help="one kernel per Taylor order (no temporal blocking)")
+    ap.add_argument("--no-extra", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        args.steps = 20 if args.steps is None else args.steps
+        args.warmup = 3 if args.warmup is None else max(args.warmup, 0)
+        run_reference(args)
+    else:
+        args.steps = 2000 if args.steps is None else args.steps
+        args.warmup = 64 if args.warmup is None else max(args.warmup, 3)
+        run_own(args)
+
+
+if __name__ == "__main__":
+    main()

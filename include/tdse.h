@@ -68,6 +68,7 @@ void tdse_destroy(tdse_handle *h);
  *   "graph_steps"      [16] steps per captured graph
  *   "taylor_block"     [1] 0: one kernel per Taylor order; 1: temporally blocked kernel when the
  *                          tile fits shared memory (all n_l rows resident), else falls back to 0
+ *   "taylor_block_width" [0] interior tile width W of the blocked kernel (0: heuristic)
  *   "lanczos_beta_tol" [1e-12] breakdown threshold on beta ("if beta = 0 then quit", R-G17)
  *   "rk45_dt_max"      [0 = none] cap on the adaptive step
  *   "rk45_check_every" [8] attempted steps enqueued between host checks of the device `done` flag */

@@ -253,8 +253,8 @@ int upload_bufs(tdse_handle *h, int n_roles, cudaStream_t s) {
     return TDSE_OK;
 }
 
-template <bool EMBED>
-void fill_rk_common(tdse_handle *h, EpiRK<EMBED> &e, int stage, const double *ef, const double *hptr) {
+template <class E>
+void fill_rk_common(tdse_handle *h, E &e, int stage, const double *ef, const double *hptr) {
     e.ctl = h->d_ctl; e.bufs = h->d_bufs; e.ef = ef; e.hptr = hptr; e.stage = stage;
     e.psi_role = R_PSI;
     for (int j = 0; j < 7; ++j) { e.k_role[j] = -1; e.a_next[j] = 0.0; e.d_err[j] = 0.0; }
@@ -299,7 +299,24 @@ int enqueue_rk45_block(tdse_handle *h, int n, int first_stage, cudaStream_t s) {
         count(h);
         for (int st = (i == 0 ? first_stage : 1); st < 7; ++st) {
             const double *ef = h->d_etab + (size_t)st * B;
-            if (st < 6) {
+            if (st == 0) {
+                // only the very first attempted step: k_1 = -i H(t) psi (afterwards FSAL supplies it); g_2 is
+                // formed by stage 1 while loading its tile, because h changes between attempts
+                EpiRK<false> e{};
+                fill_rk_common(h, e, st, ef, &h->d_ctl->h);
+                e.check_done = 1; e.in_role = R_PSI; e.k_role[0] = R_K0; e.store_k = 1; e.out_role = -1;
+                RC(launch_tile(h, e, s));
+            } else if (st == 1) {
+                EpiRK<false, true> e{};
+                fill_rk_common(h, e, st, ef, &h->d_ctl->h);
+                e.check_done = 1;
+                e.in_role = R_PSI; e.in2_role = R_K0; e.in2_a = DP_A[1][0];     // g_2 = psi + h a_21 k_1
+                for (int j = 0; j < 7; ++j) e.k_role[j] = R_K0 + j;
+                e.store_k = 1;
+                e.out_role = R_G0;
+                for (int j = 0; j <= st; ++j) e.a_next[j] = DP_A[st + 1][j];
+                RC(launch_tile(h, e, s));
+            } else if (st < 6) {
                 EpiRK<false> e{};
                 fill_rk_common(h, e, st, ef, &h->d_ctl->h);
                 e.check_done = 1;
@@ -551,6 +568,7 @@ int tdse_set_option(tdse_handle *h, const char *key, double value) {
     else if (k == "use_graph") h->use_graph = value != 0.0;
     else if (k == "graph_steps") { if (value < 1 || value > 4096) return TDSE_ERR_ARG; h->graph_steps = (int)value; }
     else if (k == "taylor_block") h->taylor_block = value != 0.0;
+    else if (k == "taylor_block_width") { if (value < 0 || value > 4096) return TDSE_ERR_ARG; h->bcfg.width_override = (int)value; free_graphs(h); }
     else if (k == "lanczos_beta_tol") { if (!(value >= 0.0)) return TDSE_ERR_ARG; h->beta_tol = value; free_graphs(h); }
     else if (k == "rk45_dt_max") { if (!(value >= 0.0)) return TDSE_ERR_ARG; h->rk45_dt_max = value; }
     else if (k == "rk45_check_every") { if (value < 1 || value > 1024) return TDSE_ERR_ARG; h->rk45_check_every = (int)value; }

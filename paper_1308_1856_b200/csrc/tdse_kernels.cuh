@@ -61,6 +61,9 @@ __global__ void __launch_bounds__(256, 3) tile_kernel(GridDev g, Epi epi_in, Red
     if (epi.member_active(b)) {
         const double2 *base = epi.input() + (size_t)b * g.n_l * g.n_r;
         const double sc = Epi::SCALED ? epi.in_scale(b) : 1.0;
+        // optional second source: the tile holds in + c2in * in2 (a stage vector formed while loading)
+        const double2 *base2 = Epi::TWO_IN ? epi.input2() + (size_t)b * g.n_l * g.n_r : nullptr;
+        const double c2in = Epi::TWO_IN ? epi.in2_coef() : 0.0;
         // stage the tile (zero outside the index box: Dirichlet walls, f_{-1} = f_L = 0)
 #pragma unroll
         for (int it = 0; it < (T::ELEMS + T::NT - 1) / T::NT; ++it) {
@@ -69,7 +72,10 @@ __global__ void __launch_bounds__(256, 3) tile_kernel(GridDev g, Epi epi_in, Red
                 const int rr = i / T::PITCH, cc = i - rr * T::PITCH;
                 const int l = l0 - 1 + rr, j = j0 - T::HW + cc;
                 double2 v = make_double2(0.0, 0.0);
-                if (l >= 0 && l < g.n_l && j >= 0 && j < g.n_r) v = __ldg(base + (size_t)l * g.n_r + j);
+                if (l >= 0 && l < g.n_l && j >= 0 && j < g.n_r) {
+                    v = __ldg(base + (size_t)l * g.n_r + j);
+                    if (Epi::TWO_IN) v = caxpy_r(c2in, __ldg(base2 + (size_t)l * g.n_r + j), v);
+                }
                 if (Epi::SCALED) { v.x *= sc; v.y *= sc; }
                 tile[i] = v;
             }
@@ -114,6 +120,9 @@ __global__ void __launch_bounds__(256, 3) tile_kernel(GridDev g, Epi epi_in, Red
 struct EpiBase {
     static constexpr int NRED = 0;
     static constexpr bool SCALED = false;
+    static constexpr bool TWO_IN = false;
+    __device__ __forceinline__ const double2 *input2() const { return nullptr; }
+    __device__ __forceinline__ double in2_coef() const { return 0.0; }
     __device__ __forceinline__ void begin() {}
     __device__ __forceinline__ bool skip_all() const { return false; }
     __device__ __forceinline__ bool member_active(int) const { return true; }
@@ -149,9 +158,11 @@ struct EpiTaylor : EpiBase {
 // One explicit Runge-Kutta stage (Eq. 38, stage loop P:469-478) with the next stage vector formed in the
 // epilogue: k_i = -i H(t_n + c_i h) g_i;  g_{i+1} = psi + sum_{j<=i} (h a_{i+1,j}) k_j  (or psi_new with the b row).
 // Buffers are addressed through roles so that the adaptive driver can swap psi/psi_new and k1/k7 on the device.
-template <bool EMBED>
+template <bool EMBED, bool TWO = false>
 struct EpiRK : EpiBase {
     static constexpr int NRED = EMBED ? 2 : 0;
+    static constexpr bool TWO_IN = TWO;     // tile = bufs[in_role] + (h * in2_a) * bufs[in2_role]
+    int in2_role; double in2_a;
     Ctl *ctl; double2 *const *bufs; const double *ef; const double *hptr;
     int stage;              // i (0-based)
     int in_role;            // role of the tile source
@@ -164,10 +175,11 @@ struct EpiRK : EpiBase {
     int check_done;
     double *dt_log, *err_log;
     // resolved at begin()
-    const double2 *in_p; double2 *out_p; const double2 *psi_p; double2 *k_p[7]; double hh; double emax;
+    const double2 *in_p; const double2 *in2_p; double2 *out_p; const double2 *psi_p; double2 *k_p[7]; double hh; double emax;
 
     __device__ __forceinline__ void begin() {
         in_p = bufs[ctl->perm[in_role]];
+        in2_p = TWO ? bufs[ctl->perm[in2_role]] : nullptr;
         out_p = out_role >= 0 ? bufs[ctl->perm[out_role]] : nullptr;
         psi_p = bufs[ctl->perm[psi_role]];
 #pragma unroll
@@ -177,6 +189,8 @@ struct EpiRK : EpiBase {
     }
     __device__ __forceinline__ bool skip_all() const { return check_done && ctl->done; }
     __device__ __forceinline__ const double2 *input() const { return in_p; }
+    __device__ __forceinline__ const double2 *input2() const { return in2_p; }
+    __device__ __forceinline__ double in2_coef() const { return hh * in2_a; }
     __device__ __forceinline__ double efield(int b) const { return __ldg(ef + b); }
     __device__ __forceinline__ void point(int, int, int, size_t idx, double2 f, double2 h, double *red) {
         const double2 k = make_double2(h.y, -h.x);              // -i H g

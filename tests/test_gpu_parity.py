@@ -190,6 +190,48 @@ def test_taylor_cfg1_window(B, order, fd, use_graph, nsteps):
     h.close()
 
 
+BLOCKED_CASES = [
+    # n_r, dr, n_l, fd, batch, order, nsteps, obs_every, width(0 = heuristic), use_graph
+    (500, 0.2, 8, 3, 1, 4, 101, 1, 0, 1),        # CFG1
+    (500, 0.2, 8, 3, 1, 4, 7, 1, 0, 0),          # eager, odd number of steps
+    (333, 0.1, 11, 5, 3, 6, 40, 4, 0, 1),        # ragged everything, 5-point, batched
+    (333, 0.1, 11, 3, 2, 5, 33, 0, 0, 1),        # odd order: the valid region straddles column pairs
+    (700, 0.1, 16, 3, 4, 6, 30, 0, 0, 1),        # CFG5 rows
+    (420, 0.1, 33, 5, 1, 10, 12, 3, 0, 1),       # n_l > 16: 8 rows per thread
+    (300, 0.1, 64, 5, 1, 10, 6, 0, 0, 1),        # CFG3 rows
+    (37, 0.2, 3, 3, 1, 1, 9, 1, 0, 1),           # order 1, grid smaller than a tile
+    (500, 0.2, 8, 5, 1, 3, 20, 5, 2, 1),         # narrowest tile: W = 2
+    (500, 0.2, 8, 3, 2, 4, 20, 5, 46, 1),        # width override, last tile ragged
+]
+
+
+@pytest.mark.parametrize("case", BLOCKED_CASES)
+def test_taylor_blocked_parity(B, case):
+    """The temporally blocked kernel (all orders in shared memory) against the oracle's order-by-order recursion."""
+    n_r, dr, n_l, fd, batch, order, nsteps, obs_every, width, use_graph = case
+    c = wl.config("cfg5" if batch > 1 else "cfg1", n_r=n_r, dr=dr, n_l=n_l, fd_order=fd, batch=batch, order=order)
+    c["propagator"] = "taylor"
+    dt = wl.dt_eff(c, "taylor", order)
+    t0 = wl.window(c, nsteps, dt)
+    psi0 = wl.populated_state(c)
+    opts = {"taylor_block": 1, "use_graph": use_graph}
+    if width:
+        opts["taylor_block_width"] = width
+    h, got, ref, gobs, robs = run_pair_fixed(B, c, "taylor", nsteps, psi0, t0, dt, obs_every, [(0, 0)], opts, order=order)
+    assert h.taylor_was_blocked()
+    check_fixed(got, ref, gobs, robs)
+    for b in range(batch):
+        for l in range(n_l):
+            assert np.linalg.norm(got[b, l] - ref[b, l]) <= TOL_PSI * max(np.linalg.norm(ref[b, l]), 1e-3)
+    # the blocked and the per-order path agree with each other far below the parity gate
+    h.set_option("taylor_block", 0)
+    h.set_state(psi0)
+    h.step_taylor(order, t0, dt, nsteps)
+    assert not h.taylor_was_blocked()
+    assert rel_l2(h.get_state(), got) <= 1e-12
+    h.close()
+
+
 def test_taylor_batched_ragged_obs_every(B):
     c = wl.config("cfg5", n_r=300, batch=5, n_l=11)
     dt = wl.dt_eff(c)
@@ -256,9 +298,15 @@ def test_lanczos_parity_and_internals(B, fd, K):
     h.step_lanczos(K, 12, t0, dt, 1)
     gi = h.lanczos_info(K)
     assert gi["m"][0] == info["m"] and gi["n_sub"][0] == info["n_sub"]
+    # the three-term recurrence amplifies rounding differences with p (loss of orthogonality, no
+    # re-orthogonalisation in the paper): the early coefficients agree to rounding, the late ones loosely, and
+    # the Krylov coefficients c_p -- what the step actually uses -- agree absolutely
     scale = np.max(np.abs(info["alpha"]))
-    assert np.max(np.abs(gi["alpha"][0] - info["alpha"])) <= 1e-11 * scale
-    assert np.max(np.abs(gi["beta"][0, :K - 1] - info["beta"][:K - 1])) <= 1e-9 * scale
+    nt = min(6, K - 1)
+    assert np.max(np.abs(gi["alpha"][0, :nt] - info["alpha"][:nt])) <= 1e-11 * scale
+    assert np.max(np.abs(gi["beta"][0, :nt] - info["beta"][:nt])) <= 1e-11 * scale
+    assert np.max(np.abs(gi["alpha"][0] - info["alpha"])) <= 1e-5 * scale
+    assert np.max(np.abs(gi["beta"][0, :K - 1] - info["beta"][:K - 1])) <= 1e-5 * scale
     assert np.max(np.abs(gi["coef"][0] - info["coef"])) <= 1e-9
     h.close()
 
@@ -373,6 +421,7 @@ def test_full_size_cfg5_taylor_steps(B):
     h.set_pulse(pulses)
     h.set_state(psi0)
     h.step_taylor(6, t0, dt, nsteps)
+    assert h.taylor_was_blocked()                      # the configuration bench.py times
     got = h.get_state()
     ref, _ = oracle.step_taylor(g, pulses, psi0, 6, t0, dt, nsteps)
     assert rel_l2(got, ref) <= TOL_PSI
