@@ -187,7 +187,8 @@ def run_own(args):
     pts = B * L * N
 
     h = binding.Tdse(N, c["dr"], L, c["fd_order"], batch=B)
-    h.set_option("taylor_block", 0 if args.no_block else 1)
+    h.set_option("taylor_block", 0 if args.no_block else args.taylor_block)
+    h.set_option("taylor_rt_variant", args.rt_variant)
     h.set_option("graph_steps", args.graph_steps)
     h.set_pulse(pulses)
     stream = torch.cuda.Stream()
@@ -215,7 +216,7 @@ def run_own(args):
         ms = ev0.elapsed_time(ev1)
         launches = h.launch_count() - l0
         clocks = sampler.result()
-        blocked = h.taylor_was_blocked()
+        blocked = h.taylor_kernel()
         obs = h.observables(t0 + (W + K) * dt, stream=stream)
         norm_dev = float(np.max(np.abs(obs[:, 0] - 1.0)))
         ms = sharding.max_over_ranks(ms)
@@ -247,7 +248,7 @@ def run_own(args):
     peak, peak_src = measured_peaks()
     if blocked:
         bytes_step = 32.0 * pts                         # read psi once, write psi once (all orders in shared memory)
-        kname, n_dom = "taylor_blocked_kernel", K
+        kname, n_dom = ("taylor_rt_kernel" if blocked == 2 else "taylor_blocked_kernel"), K
     else:
         bytes_step = (64.0 * order - 32.0) * pts        # k=1: 16R+32W, 1<k<P: 32R+32W, k=P: 32R+16W
         kname, n_dom = "tile_kernel<EpiTaylor>", K * order
@@ -269,7 +270,7 @@ def run_own(args):
             "config": {"workload": f"{args.workload} (BASELINE.json configs[{c['index'] - 1}]): {B} members/GPU x L={L} x "
                                    f"N_r={N}, {c['fd_order']}-point, Taylor order {order}",
                        "dt_cfg": c["dt_cfg"], "dt_eff": dt, "window": "pulse peak", "state": "S4 populated",
-                       "points_per_gpu": pts, "taylor_blocked": bool(blocked), "graph_steps": args.graph_steps,
+                       "points_per_gpu": pts, "taylor_blocked": bool(blocked), "taylor_kernel": kname, "graph_steps": args.graph_steps,
                        "l2": "inputs_exceed_l2 (state arrays 131 MB each > 126 MB L2)", "parallelism": f"batch x{world}"},
             "clocks": clocks, "roofline": roofline,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
@@ -353,6 +354,8 @@ def main():
     ap.add_argument("--workload", default="cfg5")
     ap.add_argument("--graph-steps", type=int, default=16)
     ap.add_argument("--no-block", action="store_true", help="one kernel per Taylor order (no temporal blocking)")
+    ap.add_argument("--taylor-block", type=int, default=1, help="1 auto, 2 shared-memory tile kernel, 3 register tiles")
+    ap.add_argument("--rt-variant", type=int, default=-1, help="instantiation of the register-tile kernel")
     ap.add_argument("--no-extra", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()

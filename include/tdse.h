@@ -66,9 +66,12 @@ void tdse_destroy(tdse_handle *h);
  *   "field_sample"     [0] 0: H frozen at t_n + dt/2 in Taylor/Lanczos steps, 1: at t_n (R-G7)
  *   "use_graph"        [1] capture blocks of steps in a CUDA graph
  *   "graph_steps"      [16] steps per captured graph
- *   "taylor_block"     [1] 0: one kernel per Taylor order; 1: temporally blocked kernel when the
- *                          tile fits shared memory (all n_l rows resident), else falls back to 0
- *   "taylor_block_width" [0] interior tile width W of the blocked kernel (0: heuristic)
+ *   "taylor_block"     [1] 0: one kernel per Taylor order; 1: temporally blocked step, all orders in one
+ *                          pass (register-tile kernel when n_l <= 32, else the shared-memory tile kernel when the
+ *                          tile fits, else falls back to 0); 2: shared-memory tile kernel only; 3: register-tile
+ *                          kernel only (each falls back to 0 when it does not apply)
+ *   "taylor_block_width" [0] interior tile width W of the shared-memory tile kernel (0: heuristic)
+ *   "taylor_rt_variant" [-1] instantiation of the register-tile kernel (-1: heuristic)
  *   "lanczos_beta_tol" [1e-12] breakdown threshold on beta ("if beta = 0 then quit", R-G17)
  *   "rk45_dt_max"      [0 = none] cap on the adaptive step
  *   "rk45_check_every" [8] attempted steps enqueued between host checks of the device `done` flag */
@@ -127,7 +130,8 @@ int  tdse_lanczos_info(tdse_handle *h, double *alpha, double *beta, double *coef
 
 /* Number of CUDA kernels this handle has launched so far (graph nodes counted per graph launch). */
 long tdse_launch_count(tdse_handle *h);
-/* Shared-memory-resident temporally blocked Taylor kernel: 1 if the last tdse_step_taylor call used it. */
+/* Kernel used by the last tdse_step_taylor call: 0 one kernel per order, 1 shared-memory tile kernel (all orders in
+ * one pass), 2 register-tile kernel (all orders in one pass). */
 int  tdse_taylor_was_blocked(tdse_handle *h);
 
 const char *tdse_strerror(int code);

@@ -248,3 +248,7 @@ class Tdse:
 
     def taylor_was_blocked(self):
         return bool(lib().tdse_taylor_was_blocked(self._h))
+
+    def taylor_kernel(self):
+        """0: one kernel per order, 1: shared-memory tile kernel, 2: register-tile kernel (last step_taylor call)."""
+        return int(lib().tdse_taylor_was_blocked(self._h))

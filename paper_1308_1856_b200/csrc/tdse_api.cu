@@ -14,6 +14,7 @@
 
 #include "tdse_kernels.cuh"
 #include "tdse_taylor_blocked.cuh"
+#include "tdse_taylor_rt.cuh"
 
 using namespace tdse;
 
@@ -87,9 +88,10 @@ struct tdse_handle {
     std::map<std::tuple<int, int, int, int, int, int>, cudaGraphExec_t> graphs;
     std::map<std::tuple<int, int, int, int, int, int>, long> graph_nodes;
     long launches = 0; long pending = 0; bool capturing = false;
-    int taylor_blocked_last = 0;
+    int taylor_blocked_last = 0;        // 0: one kernel per order, 1: shared-memory tile kernel, 2: register-tile kernel
     // blocked Taylor configuration
     BlockedCfg bcfg{};
+    RtPlan rtp{}; int rt_variant = -1;
 };
 
 namespace {
@@ -205,7 +207,8 @@ int enqueue_taylor_block(tdse_handle *h, int order, int n, int obs, cudaStream_t
         if (h->taylor_blocked_last) {
             // ping-pong psi <-> acc: even steps read psi, odd steps read acc (n is even inside graphs)
             double2 *src = (i & 1) ? acc : psi, *dst = (i & 1) ? psi : acc;
-            RC(launch_taylor_blocked(h->bcfg, h->gd, src, dst, ef, &h->d_ctl->dt, order, s));
+            if (h->taylor_blocked_last == 2) RC(launch_taylor_rt(h->gd, h->rtp, src, dst, ef, &h->d_ctl->dt, order, s));
+            else RC(launch_taylor_blocked(h->bcfg, h->gd, src, dst, ef, &h->d_ctl->dt, order, s));
             count(h);
             if (obs) RC(enqueue_obs(h, dst, i, 1, 0, 0.0, h->d_rows, s));
             continue;
@@ -412,7 +415,7 @@ int run_blocks(tdse_handle *h, int kind, int p1, int p2, int n, int obs, long nb
         }
         return TDSE_OK;
     }
-    const auto key = std::make_tuple(kind, p1, p2, n, obs + 2 * h->taylor_blocked_last, h->psi_slot);
+    const auto key = std::make_tuple(kind, p1, p2, n, obs + 2 * h->taylor_blocked_last + 8 * (h->rtp.variant + 1), h->psi_slot);
     auto it = h->graphs.find(key);
     if (it == h->graphs.end()) {
         cudaGraph_t g = nullptr;
@@ -567,7 +570,8 @@ int tdse_set_option(tdse_handle *h, const char *key, double value) {
     if (k == "field_sample") { if (value != 0.0 && value != 1.0) return TDSE_ERR_ARG; h->field_sample = (int)value; }
     else if (k == "use_graph") h->use_graph = value != 0.0;
     else if (k == "graph_steps") { if (value < 1 || value > 4096) return TDSE_ERR_ARG; h->graph_steps = (int)value; }
-    else if (k == "taylor_block") h->taylor_block = value != 0.0;
+    else if (k == "taylor_block") { if (value < 0 || value > 3) return TDSE_ERR_ARG; h->taylor_block = (int)value; }
+    else if (k == "taylor_rt_variant") { if (value < -1 || value >= kNumRtVariants) return TDSE_ERR_ARG; h->rt_variant = (int)value; free_graphs(h); }
     else if (k == "taylor_block_width") { if (value < 0 || value > 4096) return TDSE_ERR_ARG; h->bcfg.width_override = (int)value; free_graphs(h); }
     else if (k == "lanczos_beta_tol") { if (!(value >= 0.0)) return TDSE_ERR_ARG; h->beta_tol = value; free_graphs(h); }
     else if (k == "rk45_dt_max") { if (!(value >= 0.0)) return TDSE_ERR_ARG; h->rk45_dt_max = value; }
@@ -646,7 +650,17 @@ int tdse_apply_H(tdse_handle *h, const void *psi_dev, void *out_dev, const doubl
 int tdse_step_taylor(tdse_handle *h, int order, double t0, double dt, long nsteps, int obs_every, void *stream) {
     if (!h || order < 1 || order > 64 || nsteps < 0 || obs_every < 0 || !(dt == dt)) return TDSE_ERR_ARG;
     RC(ensure_pool(h, 4));
-    h->taylor_blocked_last = (h->taylor_block && blocked_supported(h->bcfg, order)) ? 1 : 0;
+    // taylor_block: 0 one kernel per order; 1 auto (register tiles, else shared-memory tile, else per order);
+    // 2 shared-memory tile kernel only; 3 register-tile kernel only
+    h->taylor_blocked_last = 0;
+    h->rtp = RtPlan{};
+    if (h->taylor_block == 1 || h->taylor_block == 3) {
+        h->rtp = rt_plan(h->grid, order, h->rt_variant);
+        if (h->rtp.ok) h->taylor_blocked_last = 2;
+    }
+    if (!h->taylor_blocked_last && (h->taylor_block == 1 || h->taylor_block == 2) && blocked_supported(h->bcfg, order))
+        h->taylor_blocked_last = 1;
+    if (h->taylor_blocked_last != 2) h->rtp = RtPlan{};
     return run_fixed(h, KIND_TAYLOR, order, 0, t0, dt, nsteps, obs_every, (cudaStream_t)stream);
 }
 

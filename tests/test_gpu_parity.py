@@ -205,20 +205,63 @@ BLOCKED_CASES = [
 ]
 
 
+RT_CASES = [
+    # n_r, dr, n_l, fd, batch, order, nsteps, obs_every, variant(-1 = heuristic), use_graph
+    (500, 0.2, 8, 3, 1, 4, 101, 1, -1, 1),       # CFG1: two tiles of 256 columns, both at a wall
+    (2000, 0.1, 16, 3, 3, 6, 12, 0, 1, 1),       # CFG5 rows and width: 18 tiles of 128 columns, clamped last tile
+    (2000, 0.1, 16, 3, 2, 6, 9, 4, 2, 0),        # same, 256-column tiles, eager, odd number of steps
+    (333, 0.1, 11, 5, 3, 6, 40, 4, -1, 1),       # ragged rows (11 of 16), 5-point, batched
+    (333, 0.1, 11, 3, 2, 5, 33, 0, 1, 1),        # odd order
+    (257, 0.1, 16, 5, 1, 10, 10, 0, 2, 1),       # grid one column wider than a tile, halo 20
+    (256, 0.1, 13, 5, 1, 12, 6, 2, 2, 1),        # grid exactly one tile: walls on both sides, no mask
+    (100, 0.2, 3, 3, 1, 4, 20, 1, -1, 1),        # grid narrower than a tile: masked instantiation
+    (37, 0.2, 3, 5, 2, 1, 9, 1, 0, 1),           # order 1, masked, 5-point
+    (420, 0.1, 32, 5, 1, 10, 8, 3, 3, 1),        # 32 rows, one CTA per SM
+    (420, 0.1, 29, 3, 2, 7, 8, 0, 4, 1),         # 29 of 32 rows, 64-column tiles
+    (1000, 0.1, 5, 3, 1, 8, 8, 0, 0, 1),         # 5 of 8 rows
+    (1000, 0.1, 24, 5, 1, 4, 8, 0, -1, 1),       # 24 of 32 rows
+]
+
+
+@pytest.mark.parametrize("case", RT_CASES)
+def test_taylor_register_tile_parity(B, case):
+    """The register-tile kernel (all orders in one pass, term and accumulator in registers) against the oracle's
+    order-by-order recursion, on every instantiation, at walls, with ragged rows and columns."""
+    n_r, dr, n_l, fd, batch, order, nsteps, obs_every, variant, use_graph = case
+    c = wl.config("cfg5" if batch > 1 else "cfg1", n_r=n_r, dr=dr, n_l=n_l, fd_order=fd, batch=batch, order=order)
+    c["propagator"] = "taylor"
+    dt = wl.dt_eff(c, "taylor", order)
+    t0 = wl.window(c, nsteps, dt)
+    psi0 = wl.populated_state(c)
+    opts = {"taylor_block": 3, "use_graph": use_graph, "taylor_rt_variant": variant}
+    h, got, ref, gobs, robs = run_pair_fixed(B, c, "taylor", nsteps, psi0, t0, dt, obs_every, [(0, 0)], opts, order=order)
+    assert h.taylor_kernel() == 2
+    check_fixed(got, ref, gobs, robs)
+    for b in range(batch):
+        for l in range(n_l):
+            assert np.linalg.norm(got[b, l] - ref[b, l]) <= TOL_PSI * max(np.linalg.norm(ref[b, l]), 1e-3)
+    h.set_option("taylor_block", 0)
+    h.set_state(psi0)
+    h.step_taylor(order, t0, dt, nsteps)
+    assert h.taylor_kernel() == 0
+    assert rel_l2(h.get_state(), got) <= 1e-12
+    h.close()
+
+
 @pytest.mark.parametrize("case", BLOCKED_CASES)
 def test_taylor_blocked_parity(B, case):
-    """The temporally blocked kernel (all orders in shared memory) against the oracle's order-by-order recursion."""
+    """The shared-memory tile kernel (all orders in shared memory) against the oracle's order-by-order recursion."""
     n_r, dr, n_l, fd, batch, order, nsteps, obs_every, width, use_graph = case
     c = wl.config("cfg5" if batch > 1 else "cfg1", n_r=n_r, dr=dr, n_l=n_l, fd_order=fd, batch=batch, order=order)
     c["propagator"] = "taylor"
     dt = wl.dt_eff(c, "taylor", order)
     t0 = wl.window(c, nsteps, dt)
     psi0 = wl.populated_state(c)
-    opts = {"taylor_block": 1, "use_graph": use_graph}
+    opts = {"taylor_block": 2, "use_graph": use_graph}
     if width:
         opts["taylor_block_width"] = width
     h, got, ref, gobs, robs = run_pair_fixed(B, c, "taylor", nsteps, psi0, t0, dt, obs_every, [(0, 0)], opts, order=order)
-    assert h.taylor_was_blocked()
+    assert h.taylor_kernel() == 1
     check_fixed(got, ref, gobs, robs)
     for b in range(batch):
         for l in range(n_l):
