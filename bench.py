@@ -248,7 +248,7 @@ def run_own(args):
     peak, peak_src = measured_peaks()
     if blocked:
         bytes_step = 32.0 * pts                         # read psi once, write psi once (all orders in shared memory)
-        kname, n_dom = ("taylor_rt_kernel" if blocked == 2 else "taylor_blocked_kernel"), K
+        kname, n_dom = {3: "taylor_rp_kernel", 2: "taylor_rt_kernel"}.get(blocked, "taylor_blocked_kernel"), K
     else:
         bytes_step = (64.0 * order - 32.0) * pts        # k=1: 16R+32W, 1<k<P: 32R+32W, k=P: 32R+16W
         kname, n_dom = "tile_kernel<EpiTaylor>", K * order
@@ -354,7 +354,7 @@ def main():
     ap.add_argument("--workload", default="cfg5")
     ap.add_argument("--graph-steps", type=int, default=16)
     ap.add_argument("--no-block", action="store_true", help="one kernel per Taylor order (no temporal blocking)")
-    ap.add_argument("--taylor-block", type=int, default=1, help="1 auto, 2 shared-memory tile kernel, 3 register tiles")
+    ap.add_argument("--taylor-block", type=int, default=1, help="1 auto, 2 shared-memory tile kernel, 3 register tiles (v2), 4 persistent register patches (v3)")
     ap.add_argument("--rt-variant", type=int, default=-1, help="instantiation of the register-tile kernel")
     ap.add_argument("--no-extra", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")

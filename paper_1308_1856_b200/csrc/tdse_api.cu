@@ -14,6 +14,7 @@
 
 #include "tdse_kernels.cuh"
 #include "tdse_taylor_blocked.cuh"
+#include "tdse_taylor_rp.cuh"
 #include "tdse_taylor_rt.cuh"
 
 using namespace tdse;
@@ -88,10 +89,11 @@ struct tdse_handle {
     std::map<std::tuple<int, int, int, int, int, int>, cudaGraphExec_t> graphs;
     std::map<std::tuple<int, int, int, int, int, int>, long> graph_nodes;
     long launches = 0; long pending = 0; bool capturing = false;
-    int taylor_blocked_last = 0;        // 0: one kernel per order, 1: shared-memory tile kernel, 2: register-tile kernel
+    int taylor_blocked_last = 0;        // 0: one kernel per order, 1: shared-memory tile kernel, 2: register-tile kernel (v2), 3: persistent register patches (v3)
     // blocked Taylor configuration
     BlockedCfg bcfg{};
     RtPlan rtp{}; int rt_variant = -1;
+    RpPlan rpp{}; int n_sm = 148;
 };
 
 namespace {
@@ -207,7 +209,8 @@ int enqueue_taylor_block(tdse_handle *h, int order, int n, int obs, cudaStream_t
         if (h->taylor_blocked_last) {
             // ping-pong psi <-> acc: even steps read psi, odd steps read acc (n is even inside graphs)
             double2 *src = (i & 1) ? acc : psi, *dst = (i & 1) ? psi : acc;
-            if (h->taylor_blocked_last == 2) RC(launch_taylor_rt(h->gd, h->rtp, src, dst, ef, &h->d_ctl->dt, order, s));
+            if (h->taylor_blocked_last == 3) RC(launch_taylor_rp(h->gd, h->rpp, src, dst, ef, &h->d_ctl->dt, order, s));
+            else if (h->taylor_blocked_last == 2) RC(launch_taylor_rt(h->gd, h->rtp, src, dst, ef, &h->d_ctl->dt, order, s));
             else RC(launch_taylor_blocked(h->bcfg, h->gd, src, dst, ef, &h->d_ctl->dt, order, s));
             count(h);
             if (obs) RC(enqueue_obs(h, dst, i, 1, 0, 0.0, h->d_rows, s));
@@ -415,7 +418,7 @@ int run_blocks(tdse_handle *h, int kind, int p1, int p2, int n, int obs, long nb
         }
         return TDSE_OK;
     }
-    const auto key = std::make_tuple(kind, p1, p2, n, obs + 2 * h->taylor_blocked_last + 8 * (h->rtp.variant + 1), h->psi_slot);
+    const auto key = std::make_tuple(kind, p1, p2, n, obs + 2 * h->taylor_blocked_last + 16 * (h->rtp.variant + 1), h->psi_slot);
     auto it = h->graphs.find(key);
     if (it == h->graphs.end()) {
         cudaGraph_t g = nullptr;
@@ -499,6 +502,12 @@ int tdse_create(const tdse_grid *grid, tdse_handle **out) {
     tdse_handle *h = new (std::nothrow) tdse_handle();
     if (!h) return TDSE_ERR_ALLOC;
     h->grid = *grid;
+    {
+        int dev = 0, n_sm = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n_sm > 0)
+            h->n_sm = n_sm;
+    }
     const int N = grid->n_r, L = grid->n_l, B = grid->batch;
     h->n_state = (size_t)N * L * B;
     auto fail = [&](int rc) { tdse_destroy(h); return rc; };
@@ -570,7 +579,7 @@ int tdse_set_option(tdse_handle *h, const char *key, double value) {
     if (k == "field_sample") { if (value != 0.0 && value != 1.0) return TDSE_ERR_ARG; h->field_sample = (int)value; }
     else if (k == "use_graph") h->use_graph = value != 0.0;
     else if (k == "graph_steps") { if (value < 1 || value > 4096) return TDSE_ERR_ARG; h->graph_steps = (int)value; }
-    else if (k == "taylor_block") { if (value < 0 || value > 3) return TDSE_ERR_ARG; h->taylor_block = (int)value; }
+    else if (k == "taylor_block") { if (value < 0 || value > 4) return TDSE_ERR_ARG; h->taylor_block = (int)value; }
     else if (k == "taylor_rt_variant") { if (value < -1 || value >= kNumRtVariants) return TDSE_ERR_ARG; h->rt_variant = (int)value; free_graphs(h); }
     else if (k == "taylor_block_width") { if (value < 0 || value > 4096) return TDSE_ERR_ARG; h->bcfg.width_override = (int)value; free_graphs(h); }
     else if (k == "lanczos_beta_tol") { if (!(value >= 0.0)) return TDSE_ERR_ARG; h->beta_tol = value; free_graphs(h); }
@@ -650,11 +659,17 @@ int tdse_apply_H(tdse_handle *h, const void *psi_dev, void *out_dev, const doubl
 int tdse_step_taylor(tdse_handle *h, int order, double t0, double dt, long nsteps, int obs_every, void *stream) {
     if (!h || order < 1 || order > 64 || nsteps < 0 || obs_every < 0 || !(dt == dt)) return TDSE_ERR_ARG;
     RC(ensure_pool(h, 4));
-    // taylor_block: 0 one kernel per order; 1 auto (register tiles, else shared-memory tile, else per order);
-    // 2 shared-memory tile kernel only; 3 register-tile kernel only
+    // taylor_block: 0 one kernel per order; 1 auto (persistent register patches, else register tiles, else
+    // shared-memory tile, else per order); 2 shared-memory tile kernel only; 3 register-tile kernel (v2) only;
+    // 4 persistent register-patch kernel (v3) only
     h->taylor_blocked_last = 0;
     h->rtp = RtPlan{};
-    if (h->taylor_block == 1 || h->taylor_block == 3) {
+    h->rpp = RpPlan{};
+    if (h->taylor_block == 1 || h->taylor_block == 4) {
+        h->rpp = rp_plan(h->grid, order, h->n_sm);
+        if (h->rpp.ok) h->taylor_blocked_last = 3;
+    }
+    if (!h->taylor_blocked_last && (h->taylor_block == 1 || h->taylor_block == 3)) {
         h->rtp = rt_plan(h->grid, order, h->rt_variant);
         if (h->rtp.ok) h->taylor_blocked_last = 2;
     }

@@ -248,6 +248,52 @@ def test_taylor_register_tile_parity(B, case):
     h.close()
 
 
+RP_CASES = [
+    # n_r, dr, n_l, fd, batch, order, nsteps, obs_every, use_graph
+    (500, 0.2, 8, 3, 1, 4, 101, 1, 1),           # CFG1: 2 warps, 5 tiles of 128 columns
+    (2000, 0.1, 16, 3, 3, 6, 12, 0, 1),          # CFG5 rows and width: 18 tiles, clamped last tile
+    (2000, 0.1, 16, 3, 2, 6, 9, 4, 0),           # same, eager, odd number of steps
+    (333, 0.1, 11, 5, 3, 6, 40, 4, 1),           # ragged rows (11 of 16), 5-point, batched
+    (333, 0.1, 11, 3, 2, 5, 33, 0, 1),           # odd order
+    (129, 0.1, 16, 5, 1, 10, 10, 0, 1),          # grid one column wider than a tile, halo 20
+    (128, 0.1, 13, 5, 1, 12, 6, 2, 1),           # grid exactly one tile: walls on both sides, no mask
+    (100, 0.2, 3, 3, 1, 4, 20, 1, 1),            # grid narrower than a tile: masked instantiation, 1 warp
+    (37, 0.2, 3, 5, 2, 1, 9, 1, 1),              # order 1, masked, 5-point
+    (420, 0.1, 32, 5, 1, 10, 8, 3, 1),           # 32 rows: 8 warps, one CTA per SM
+    (420, 0.1, 29, 3, 2, 7, 8, 0, 1),            # 29 of 32 rows
+    (1000, 0.1, 5, 3, 1, 8, 8, 0, 1),            # 5 of 8 rows
+    (1000, 0.1, 24, 5, 1, 4, 8, 0, 1),           # 24 of 32 rows
+    (700, 0.1, 4, 3, 300, 6, 6, 0, 1),           # more work items than resident CTAs: persistent loop + L2 prefetch
+    (3000, 0.1, 16, 5, 40, 3, 5, 0, 1),          # several items per CTA, 5-point
+]
+
+
+@pytest.mark.parametrize("case", RP_CASES)
+def test_taylor_register_patch_parity(B, case):
+    """The persistent register-patch kernel (v3: shuffle radial exchange, scaled operator H/c1, direct global
+    loads) against the oracle's order-by-order recursion: every warp count, walls, ragged rows and columns,
+    masked grids, and more work items than resident CTAs."""
+    n_r, dr, n_l, fd, batch, order, nsteps, obs_every, use_graph = case
+    c = wl.config("cfg5" if batch > 1 else "cfg1", n_r=n_r, dr=dr, n_l=n_l, fd_order=fd, batch=batch, order=order)
+    c["propagator"] = "taylor"
+    dt = wl.dt_eff(c, "taylor", order)
+    t0 = wl.window(c, nsteps, dt)
+    psi0 = wl.populated_state(c)
+    opts = {"taylor_block": 4, "use_graph": use_graph}
+    h, got, ref, gobs, robs = run_pair_fixed(B, c, "taylor", nsteps, psi0, t0, dt, obs_every, [(0, 0)], opts, order=order)
+    assert h.taylor_kernel() == 3
+    check_fixed(got, ref, gobs, robs)
+    for b in range(batch):
+        for l in range(n_l):
+            assert np.linalg.norm(got[b, l] - ref[b, l]) <= TOL_PSI * max(np.linalg.norm(ref[b, l]), 1e-3)
+    h.set_option("taylor_block", 0)
+    h.set_state(psi0)
+    h.step_taylor(order, t0, dt, nsteps)
+    assert h.taylor_kernel() == 0
+    assert rel_l2(h.get_state(), got) <= 1e-12
+    h.close()
+
+
 @pytest.mark.parametrize("case", BLOCKED_CASES)
 def test_taylor_blocked_parity(B, case):
     """The shared-memory tile kernel (all orders in shared memory) against the oracle's order-by-order recursion."""
