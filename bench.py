@@ -189,6 +189,7 @@ def run_own(args):
     h = binding.Tdse(N, c["dr"], L, c["fd_order"], batch=B)
     h.set_option("taylor_block", 0 if args.no_block else args.taylor_block)
     h.set_option("taylor_rt_variant", args.rt_variant)
+    h.set_option("taylor_rp_variant", args.rp_variant)
     h.set_option("graph_steps", args.graph_steps)
     h.set_pulse(pulses)
     stream = torch.cuda.Stream()
@@ -356,6 +357,7 @@ def main():
     ap.add_argument("--no-block", action="store_true", help="one kernel per Taylor order (no temporal blocking)")
     ap.add_argument("--taylor-block", type=int, default=1, help="1 auto, 2 shared-memory tile kernel, 3 register tiles (v2), 4 persistent register patches (v3)")
     ap.add_argument("--rt-variant", type=int, default=-1, help="instantiation of the register-tile kernel")
+    ap.add_argument("--rp-variant", type=int, default=-1, help="instantiation of the register-patch kernel")
     ap.add_argument("--no-extra", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()

@@ -67,11 +67,13 @@ void tdse_destroy(tdse_handle *h);
  *   "use_graph"        [1] capture blocks of steps in a CUDA graph
  *   "graph_steps"      [16] steps per captured graph
  *   "taylor_block"     [1] 0: one kernel per Taylor order; 1: temporally blocked step, all orders in one
- *                          pass (register-tile kernel when n_l <= 32, else the shared-memory tile kernel when the
- *                          tile fits, else falls back to 0); 2: shared-memory tile kernel only; 3: register-tile
- *                          kernel only (each falls back to 0 when it does not apply)
+ *                          pass (persistent register-patch kernel when n_l <= 32, else the shared-memory tile
+ *                          kernel when the tile fits, else falls back to 0); 2: shared-memory tile kernel only;
+ *                          3: register-tile kernel (v2) only; 4: persistent register-patch kernel (v3) only
+ *                          (each falls back to 0 when it does not apply)
  *   "taylor_block_width" [0] interior tile width W of the shared-memory tile kernel (0: heuristic)
  *   "taylor_rt_variant" [-1] instantiation of the register-tile kernel (-1: heuristic)
+ *   "taylor_rp_variant" [-1] instantiation of the register-patch kernel (-1: heuristic)
  *   "lanczos_beta_tol" [1e-12] breakdown threshold on beta ("if beta = 0 then quit", R-G17)
  *   "rk45_dt_max"      [0 = none] cap on the adaptive step
  *   "rk45_check_every" [8] attempted steps enqueued between host checks of the device `done` flag */

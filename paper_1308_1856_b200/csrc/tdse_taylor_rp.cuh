@@ -3,16 +3,15 @@
 // Method: Eq. 37 (reading R-G6): F(t+dt) = sum_{k=0..P} F^(k), F^(k) = (-i dt/k) H F^(k-1); all P orders of a
 // step are applied in ONE pass over HBM (32 B/point/step; the paper launches one kernel per order).
 //
-// Work item = (member b, radial tile t).  A warp owns 4 partial waves x 128 radial columns of the tile, a thread a
-// patch of 4 rows x 4 adjacent columns whose current term u_k AND accumulator stay in registers for the whole
-// step.  What differs from v2 (tdse_taylor_rt.cuh):
-//   * no shared-memory tile: a thread loads its patch straight from global memory (64 contiguous bytes per row,
-//     a warp reads 2 KB contiguous) and stores the result the same way;
-//   * radial neighbours (columns c0-1, c0+4 [, c0-2, c0+5]) come from the adjacent LANES by warp shuffle;
-//     only the l-1 / l+1 rows cross warps, through a small double-buffered shared-memory exchange
-//     (lane-contiguous, conflict free) -- 16 instead of 28 shared-memory accesses per thread and order;
-//   * CTAs are persistent (grid = resident CTAs), the zero rows / coefficient table are set up once, and the next
-//     work item is prefetched into L2 (cp.async.bulk.prefetch.L2) while the current one is being computed;
+// Work item = (member b, radial tile t).  A CTA is NWR x NWC warps; a warp owns 4 partial waves x 32*CP radial
+// columns, a thread a patch of 4 rows x CP adjacent columns (CP = 2 or 4) whose current term u_k AND accumulator
+// stay in registers for the whole step.  What differs from v2 (tdse_taylor_rt.cuh):
+//   * no shared-memory tile: a thread loads its patch straight from global memory (CP*16 contiguous bytes per
+//     row, 256-bit accesses when aligned; a warp reads 32*CP*16 contiguous bytes) and stores the result likewise;
+//   * radial neighbours come from the adjacent LANES by warp shuffle; only the l-1 / l+1 rows (and, for NWC > 1,
+//     the two edge lanes of a warp) go through a small double-buffered shared-memory exchange;
+//   * CTAs are persistent (grid = resident CTAs, a multiple of the tile count so that a CTA stays on one radial
+//     tile and keeps its per-column coefficients);
 //   * the operator is applied as H' = H / c1 (c1 = first off-diagonal stencil weight), so the radial part is
 //     (f_{j-1} + f_{j+1}) + d' f_j with no multiply on the neighbours; u'_k = H'^k psi and the accumulator takes
 //     (-i)^k (dt c1)^k / k! u'_k -- the same polynomial as Eq. 37 in another rounding order.  The coupling weight
@@ -25,13 +24,24 @@
 
 namespace tdse {
 
-constexpr int kRpRows = 4, kRpCols = 4, kRpWT = 128;     // patch rows, patch columns, tile columns (32 lanes x 4)
+constexpr int kRpRows = 4;     // patch rows
 
-// shared memory: exchange buffers [2 parities][NW warps][2 (top,bottom)][4 planes][32 lanes] double2, row table
-template <int NW>
+template <int FD, int CP, int NWR, int NWC>
+struct RpGeom {
+    static constexpr int HW = (FD == 3) ? 1 : 2;
+    static constexpr int NT = NWR * NWC * 32;
+    static constexpr int WT = 32 * CP * NWC;           // tile columns
+    static constexpr int ROWS = kRpRows * NWR;
+    static_assert(HW <= CP, "radial halo wider than the patch");
+};
+
+// shared memory: vertical exchange [parity][warp][top,bottom][CP planes][32 lanes], radial edge exchange between
+// the warps of a row group [parity][warp][left,right][4 rows][HW], row table
+template <int FD, int CP, int NWR, int NWC>
 struct RpSmem {
-    double2 xch[2][NW][2][kRpCols][32];
-    double rowtab[NW * kRpRows][4];        // {c_{l-1}, c_l, l(l+1), 0}
+    double2 xch[2][NWR * NWC][2][CP][32];
+    double2 edge[2][NWR * NWC][2][kRpRows][(FD == 3) ? 1 : 2];
+    double rowtab[NWR * kRpRows][4];        // {c_{l-1}, c_l, l(l+1), 0}
 };
 
 __device__ __forceinline__ double2 shfl_up2(double2 v) {
@@ -40,34 +50,40 @@ __device__ __forceinline__ double2 shfl_up2(double2 v) {
 __device__ __forceinline__ double2 shfl_dn2(double2 v) {
     return make_double2(__shfl_down_sync(0xffffffffu, v.x, 1), __shfl_down_sync(0xffffffffu, v.y, 1));
 }
-__device__ __forceinline__ void l2_prefetch_bulk(const void *p, unsigned bytes) {
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+__device__ __forceinline__ void ldg256(const double2 *p, double2 &a, double2 &b) {
+    asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a.x), "=d"(a.y), "=d"(b.x), "=d"(b.y) : "l"(p));
+}
+__device__ __forceinline__ void stg256(double2 *p, const double2 &a, const double2 &b) {
+    asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a.x), "d"(a.y), "d"(b.x), "d"(b.y) : "memory");
 }
 
 // tile start of tile t: interior [t*W, (t+1)*W) plus H halo columns per side, clamped so that a tile at a wall
 // starts (ends) exactly at the wall: the zero beyond the tile IS the Dirichlet wall.
-__device__ __forceinline__ int rp_start(int t, int W, int H, int N) {
+__device__ __forceinline__ int rp_start(int t, int W, int H, int N, int WT) {
     int start = t * W - H;
-    if (start > N - kRpWT) start = N - kRpWT;
+    if (start > N - WT) start = N - WT;
     if (start < 0) start = 0;
     return start;
 }
 
-// grid = persistent CTAs, block = NW*32.  n_l <= 4*NW.  MASK: n_r < 128 (single tile, columns >= n_r held at zero).
-template <int FD, int NW, bool MASK, int MINB>
-__global__ void __launch_bounds__(NW * 32, MINB)
+// grid = persistent CTAs, block = NT.  n_l <= 4*NWR.  H = halo columns per side (>= order * HW; even when n_r is
+// even so that every patch row is 32-byte aligned).  MASK: n_r < WT (single tile, columns >= n_r held at zero).
+template <int FD, int CP, int NWR, int NWC, bool MASK, int MINB>
+__global__ void __launch_bounds__(NWR * NWC * 32, MINB)
 taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict__ out, const double *__restrict__ ef,
-                 const double *__restrict__ dtp, int order, int W, int n_tiles, int n_items) {
-    constexpr int RP = kRpRows, CP = kRpCols, WT = kRpWT, HW = (FD == 3) ? 1 : 2;
+                 const double *__restrict__ dtp, int order, int W, int H, int n_tiles, int n_items) {
+    using G = RpGeom<FD, CP, NWR, NWC>;
+    constexpr int RP = kRpRows, WT = G::WT, HW = G::HW;
     extern __shared__ __align__(16) unsigned char rp_smem_raw[];
-    RpSmem<NW> &sm = *reinterpret_cast<RpSmem<NW> *>(rp_smem_raw);
+    RpSmem<FD, CP, NWR, NWC> &sm = *reinterpret_cast<RpSmem<FD, CP, NWR, NWC> *>(rp_smem_raw);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int wr = warp / NWC, wc = warp - wr * NWC;
     const int L = g.n_l, N = g.n_r;
-    const int H = order * HW;
-    const int r0 = warp * RP, c0 = lane * CP;
+    const int r0 = wr * RP, c0 = (wc * 32 + lane) * CP;
     const double2 z2 = make_double2(0.0, 0.0);
+    const bool al32 = !MASK && ((N & 1) == 0) && ((H & 1) == 0) && ((W & 1) == 0);
 
-    for (int r = threadIdx.x; r < NW * RP; r += NW * 32) {
+    for (int r = threadIdx.x; r < NWR * RP; r += G::NT) {
         sm.rowtab[r][0] = (r >= 1 && r < L) ? __ldg(g.cl + r - 1) : 0.0;
         sm.rowtab[r][1] = (r + 1 < L) ? __ldg(g.cl + r) : 0.0;
         sm.rowtab[r][2] = (double)(r * (r + 1));
@@ -79,62 +95,85 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
     const double inv_c1 = 1.0 / g.c1;
     const double kappa = dt * g.c1;                 // u'_k = (H/c1)^k psi  ->  weight (dt c1)^k / k!
     const double c2p = g.c2 * inv_c1;               // 5-point: second off-diagonal weight / c1 (= -1/16)
+    // radial exchange across warps: lane 0 reads the right edge of warp wc-1, lane 31 the left edge of warp wc+1
+    const bool is_edge = (NWC > 1) && (lane == 0 || lane == 31);
+    const bool has_nb = (NWC > 1) && ((lane == 0 && wc > 0) || (lane == 31 && wc < NWC - 1));
+    const int nb_warp = has_nb ? ((lane == 0) ? warp - 1 : warp + 1) : warp;
+    const int nb_side = (lane == 0) ? 1 : 0, my_side = (lane == 0) ? 0 : 1;
+
+    int t_cur = -1;
+    double Dq[CP], Cq[CP], Eq[CP];
+    bool dom[CP];
+#pragma unroll
+    for (int q = 0; q < CP; ++q) { Dq[q] = 0.0; Cq[q] = 0.0; dom[q] = true; }
 
     for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
         const int b = item / n_tiles, t = item - b * n_tiles;
-        const int start = rp_start(t, W, H, N);
-        const double2 *src_g = in + (size_t)b * L * N + start;
-        // ---- prefetch the next item of this CTA into L2 (one lane per row) ------------------------------------
-        {
-            const int nitem = item + gridDim.x;
-            if (nitem < n_items && threadIdx.x < L) {
-                const int nb = nitem / n_tiles, nt = nitem - nb * n_tiles;
-                const int ns = rp_start(nt, W, H, N);
-                const int ncols = (N < WT) ? N : WT;
-                l2_prefetch_bulk(in + ((size_t)nb * L + threadIdx.x) * N + ns, (unsigned)(ncols * sizeof(double2)));
-            }
-        }
-        // ---- per-column coefficients (scaled by 1/c1) ----------------------------------------------------------
-        const double e_b = __ldg(ef + b);
-        double Dq[CP], Cq[CP], Eq[CP];
-        bool dom[CP];
-#pragma unroll
-        for (int q = 0; q < CP; ++q) {
-            const int j = start + c0 + q;
-            dom[q] = !MASK || j < N;
-            const int jj = dom[q] ? j : 0;
-            Dq[q] = inv_c1 * __ldg(g.vj + jj);
-            Cq[q] = inv_c1 * __ldg(g.cen + jj);
-            Eq[q] = inv_c1 * (e_b * (g.dr * (double)(jj + 1)));
-        }
+        const int start = rp_start(t, W, H, N, WT);
+        const double2 *src_g = in + (size_t)b * L * N + start + c0;
         // ---- own patch straight from global memory -------------------------------------------------------------
         double2 T[RP][CP], A[RP][CP];
 #pragma unroll
-        for (int r = 0; r < RP; ++r)
+        for (int r = 0; r < RP; ++r) {
+            const double2 *p = src_g + (size_t)(r0 + r) * N;
+            if (r0 + r < L) {
+                if (al32) {
+#pragma unroll
+                    for (int q = 0; q < CP; q += 2) ldg256(p + q, T[r][q], T[r][q + 1]);
+                } else {
+#pragma unroll
+                    for (int q = 0; q < CP; ++q) T[r][q] = (!MASK || start + c0 + q < N) ? __ldg(p + q) : z2;
+                }
+            } else {
+#pragma unroll
+                for (int q = 0; q < CP; ++q) T[r][q] = z2;
+            }
+        }
+        // ---- per-column coefficients (scaled by 1/c1): reloaded only when the radial tile changes ----------------
+        if (t != t_cur) {
+            t_cur = t;
 #pragma unroll
             for (int q = 0; q < CP; ++q) {
-                double2 v = z2;
-                if (r0 + r < L && dom[q]) v = __ldg(src_g + (size_t)(r0 + r) * N + c0 + q);
-                T[r][q] = v;
-                A[r][q] = v;
+                const int j = start + c0 + q;
+                dom[q] = !MASK || j < N;
+                const int jj = dom[q] ? j : 0;
+                Dq[q] = inv_c1 * __ldg(g.vj + jj);
+                Cq[q] = inv_c1 * __ldg(g.cen + jj);
             }
-        // publish rows 0 and RP-1 of u_0 for the neighbouring warps
+        }
+        {
+            const double es = inv_c1 * (__ldg(ef + b) * g.dr);
+#pragma unroll
+            for (int q = 0; q < CP; ++q) Eq[q] = es * (double)(dom[q] ? start + c0 + q + 1 : 1);
+        }
+#pragma unroll
+        for (int r = 0; r < RP; ++r)
+#pragma unroll
+            for (int q = 0; q < CP; ++q) A[r][q] = T[r][q];
+        // publish u_0: rows 0 and RP-1 for the warps above / below, edge columns for the warps left / right
 #pragma unroll
         for (int q = 0; q < CP; ++q) {
             sm.xch[0][warp][0][q][lane] = T[0][q];
             sm.xch[0][warp][1][q][lane] = T[RP - 1][q];
         }
+        if (is_edge) {
+#pragma unroll
+            for (int r = 0; r < RP; ++r)
+#pragma unroll
+                for (int h = 0; h < HW; ++h) sm.edge[0][warp][my_side][r][h] = (lane == 0) ? T[r][h] : T[r][CP - 1 - h];
+        }
         __syncthreads();
 
-        double sk = 1.0;
-        for (int k = 1; k <= order; ++k) {
+        // One order: To = H' Ti (rows in increasing l), A += weight * To, publish To's outer rows / edge columns.
+        // The order loop below is unrolled by two with the roles of T and U swapped, so that the new term is
+        // written where the term before last lived and no register copies are needed at the loop back-edge.
+        auto sweep = [&](const double2 (&Ti)[RP][CP], double2 (&To)[RP][CP], const int k, const bool odd, const double s) {
             const int pr = (k - 1) & 1, pw = k & 1;
-            sk = sk * (kappa / (double)k);
             double2 lo[CP], below[CP];
 #pragma unroll
             for (int q = 0; q < CP; ++q) {
-                lo[q] = (warp > 0) ? sm.xch[pr][warp > 0 ? warp - 1 : 0][1][q][lane] : z2;
-                below[q] = (warp < NW - 1) ? sm.xch[pr][warp < NW - 1 ? warp + 1 : 0][0][q][lane] : z2;
+                lo[q] = (wr > 0) ? sm.xch[pr][wr > 0 ? warp - NWC : 0][1][q][lane] : z2;
+                below[q] = (wr < NWR - 1) ? sm.xch[pr][wr < NWR - 1 ? warp + NWC : 0][0][q][lane] : z2;
             }
             double alo[CP];
             {
@@ -146,30 +185,36 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
             for (int r = 0; r < RP; ++r) {
                 const double cup = sm.rowtab[r0 + r][1];
                 const double ll1 = sm.rowtab[r0 + r][2];
-                double2 lf1 = shfl_up2(T[r][CP - 1]);       // column c0 - 1 from lane - 1
-                double2 rg1 = shfl_dn2(T[r][0]);            // column c0 + CP from lane + 1
-                if (lane == 0) lf1 = z2;
-                if (lane == 31) rg1 = z2;
+                // columns beyond the warp: zero at a tile edge, else the neighbouring warp's edge column
+                double2 ev1 = z2, ev2 = z2;
+                if (NWC > 1 && has_nb) {
+                    ev1 = sm.edge[pr][nb_warp][nb_side][r][0];
+                    if (FD == 5) ev2 = sm.edge[pr][nb_warp][nb_side][r][HW - 1];
+                }
+                double2 lf1 = shfl_up2(Ti[r][CP - 1]);       // column c0 - 1 from lane - 1
+                double2 rg1 = shfl_dn2(Ti[r][0]);            // column c0 + CP from lane + 1
+                if (lane == 0) lf1 = ev1;
+                if (lane == 31) rg1 = ev1;
                 double2 lf2 = z2, rg2 = z2;
                 if (FD == 5) {
-                    lf2 = shfl_up2(T[r][CP - 2]);
-                    rg2 = shfl_dn2(T[r][1]);
-                    if (lane == 0) lf2 = z2;
-                    if (lane == 31) rg2 = z2;
+                    lf2 = shfl_up2(Ti[r][CP - 2]);
+                    rg2 = shfl_dn2(Ti[r][1]);
+                    if (lane == 0) lf2 = ev2;
+                    if (lane == 31) rg2 = ev2;
                 }
-                double2 nw[CP];
 #pragma unroll
                 for (int q = 0; q < CP; ++q) {
-                    const double2 f = T[r][q];
-                    const double2 m1 = (q > 0) ? T[r][q > 0 ? q - 1 : 0] : lf1;
-                    const double2 p1 = (q < CP - 1) ? T[r][q < CP - 1 ? q + 1 : 0] : rg1;
-                    const double2 up = (r < RP - 1) ? T[r < RP - 1 ? r + 1 : 0][q] : below[q];
+                    const double2 f = Ti[r][q];
+                    const double2 m1 = (q > 0) ? Ti[r][q > 0 ? q - 1 : 0] : lf1;
+                    const double2 p1 = (q < CP - 1) ? Ti[r][q < CP - 1 ? q + 1 : 0] : rg1;
+                    const double2 up = (r < RP - 1) ? Ti[r < RP - 1 ? r + 1 : 0][q] : below[q];
+                    const double2 dn = (r > 0) ? Ti[r > 0 ? r - 1 : 0][q] : lo[q];
                     const double d = fma(ll1, Cq[q], Dq[q]);
                     const double aup = cup * Eq[q];
                     double hx = m1.x + p1.x, hy = m1.y + p1.y;
                     if (FD == 5) {
-                        const double2 m2 = (q > 1) ? T[r][q > 1 ? q - 2 : 0] : ((q == 1) ? lf1 : lf2);
-                        const double2 p2 = (q < CP - 2) ? T[r][q < CP - 2 ? q + 2 : 0] : ((q == CP - 2) ? rg1 : rg2);
+                        const double2 m2 = (q > 1) ? Ti[r][q > 1 ? q - 2 : 0] : ((q == 1) ? lf1 : lf2);
+                        const double2 p2 = (q < CP - 2) ? Ti[r][q < CP - 2 ? q + 2 : 0] : ((q == CP - 2) ? rg1 : rg2);
                         hx = fma(c2p, m2.x + p2.x, hx);
                         hy = fma(c2p, m2.y + p2.y, hy);
                     }
@@ -177,51 +222,45 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                     hy = fma(d, f.y, hy);
                     hx = fma(aup, up.x, hx);
                     hy = fma(aup, up.y, hy);
-                    hx = fma(alo[q], lo[q].x, hx);
-                    hy = fma(alo[q], lo[q].y, hy);
-                    nw[q] = make_double2(hx, hy);
-                    if (MASK && !dom[q]) nw[q] = z2;
+                    hx = fma(alo[q], dn.x, hx);
+                    hy = fma(alo[q], dn.y, hy);
+                    if (MASK && !dom[q]) { hx = 0.0; hy = 0.0; }
+                    To[r][q] = make_double2(hx, hy);
                     alo[q] = aup;                           // c_l E r / c1 couples row l+1 back to row l
+                    // acc += (-i)^k (dt c1)^k / k! * u'_k; s carries the sign: odd k: -+i, even k: -+1
+                    if (odd) { A[r][q].x = fma(s, hy, A[r][q].x); A[r][q].y = fma(-s, hx, A[r][q].y); }
+                    else { A[r][q].x = fma(s, hx, A[r][q].x); A[r][q].y = fma(s, hy, A[r][q].y); }
                 }
-#pragma unroll
-                for (int q = 0; q < CP; ++q) { lo[q] = T[r][q]; T[r][q] = nw[q]; }
             }
             if (k < order) {
 #pragma unroll
                 for (int q = 0; q < CP; ++q) {
-                    sm.xch[pw][warp][0][q][lane] = T[0][q];
-                    sm.xch[pw][warp][1][q][lane] = T[RP - 1][q];
+                    sm.xch[pw][warp][0][q][lane] = To[0][q];
+                    sm.xch[pw][warp][1][q][lane] = To[RP - 1][q];
+                }
+                if (is_edge) {
+#pragma unroll
+                    for (int r = 0; r < RP; ++r)
+#pragma unroll
+                        for (int h = 0; h < HW; ++h)
+                            sm.edge[pw][warp][my_side][r][h] = (lane == 0) ? To[r][h] : To[r][CP - 1 - h];
                 }
             }
-            // acc += (-i)^k (dt c1)^k / k! * u'_k
-            const double s = sk;
-            switch (k & 3) {
-                case 0:
-#pragma unroll
-                    for (int r = 0; r < RP; ++r)
-#pragma unroll
-                        for (int q = 0; q < CP; ++q) { A[r][q].x = fma(s, T[r][q].x, A[r][q].x); A[r][q].y = fma(s, T[r][q].y, A[r][q].y); }
-                    break;
-                case 1:   // -i (x + i y) = y - i x
-#pragma unroll
-                    for (int r = 0; r < RP; ++r)
-#pragma unroll
-                        for (int q = 0; q < CP; ++q) { A[r][q].x = fma(s, T[r][q].y, A[r][q].x); A[r][q].y = fma(-s, T[r][q].x, A[r][q].y); }
-                    break;
-                case 2:
-#pragma unroll
-                    for (int r = 0; r < RP; ++r)
-#pragma unroll
-                        for (int q = 0; q < CP; ++q) { A[r][q].x = fma(-s, T[r][q].x, A[r][q].x); A[r][q].y = fma(-s, T[r][q].y, A[r][q].y); }
-                    break;
-                default:  // +i (x + i y) = -y + i x
-#pragma unroll
-                    for (int r = 0; r < RP; ++r)
-#pragma unroll
-                        for (int q = 0; q < CP; ++q) { A[r][q].x = fma(-s, T[r][q].y, A[r][q].x); A[r][q].y = fma(s, T[r][q].x, A[r][q].y); }
-                    break;
-            }
             __syncthreads();
+        };
+
+        double2 U[RP][CP];
+        double sk = 1.0;
+        int k = 1;
+        for (; k + 1 <= order; k += 2) {
+            sk = sk * (kappa / (double)k);
+            sweep(T, U, k, true, (k & 2) ? -sk : sk);
+            sk = sk * (kappa / (double)(k + 1));
+            sweep(U, T, k + 1, false, ((k + 1) & 2) ? -sk : sk);
+        }
+        if (k <= order) {
+            sk = sk * (kappa / (double)k);
+            sweep(T, U, k, true, (k & 2) ? -sk : sk);
         }
 
         // ---- psi(t + dt): interior columns of the tile straight from registers ---------------------------------
@@ -229,14 +268,21 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
             const int lo_c = t * W - start;                  // first interior column (tile coordinates)
             int wint = N - t * W;
             if (wint > W) wint = W;
-            double2 *dst_g = out + (size_t)b * L * N + start;
+            double2 *dst_g = out + (size_t)b * L * N + start + c0;
 #pragma unroll
-            for (int q = 0; q < CP; ++q) {
+            for (int q = 0; q < CP; q += 2) {
                 const int c = c0 + q;
-                if (c >= lo_c && c < lo_c + wint) {
+                const bool in0 = c >= lo_c && c < lo_c + wint, in1 = c + 1 >= lo_c && c + 1 < lo_c + wint;
 #pragma unroll
-                    for (int r = 0; r < RP; ++r)
-                        if (r0 + r < L) dst_g[(size_t)(r0 + r) * N + c] = A[r][q];
+                for (int r = 0; r < RP; ++r) {
+                    if (r0 + r >= L) continue;
+                    double2 *p = dst_g + (size_t)(r0 + r) * N + q;
+                    if (al32) {
+                        if (in0) stg256(p, A[r][q], A[r][q + 1]);      // interior bounds are even: in0 == in1
+                    } else {
+                        if (in0) p[0] = A[r][q];
+                        if (in1) p[1] = A[r][q + 1];
+                    }
                 }
             }
         }
@@ -246,59 +292,93 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
 // ------------------------------------------------------------------------------------------------------
 // Host side
 // ------------------------------------------------------------------------------------------------------
-struct RpPlan { int ok, nw, W, n_tiles, n_items, grid, minb; };
+struct RpVariant { int cp, nwr, nwc, minb; };
+// instantiations: (patch columns, row-group warps, column-segment warps, min CTAs/SM)
+constexpr RpVariant kRpVariants[] = {
+    {4, 1, 1, 8}, {4, 2, 1, 4}, {4, 4, 1, 2}, {4, 8, 1, 1},      // 128-column tiles, 16 points per thread
+    {2, 1, 2, 8}, {2, 2, 2, 4}, {2, 4, 2, 2}, {2, 8, 2, 1},      // 128-column tiles,  8 points per thread
+    {2, 4, 4, 1},                                                // 256-column tile, 8 points per thread, n_l <= 16
+};
+constexpr int kNumRpVariants = sizeof(kRpVariants) / sizeof(kRpVariants[0]);
 
-inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm) {
-    RpPlan p{};
-    if (g.n_l > 32) return p;
-    const int hw = (g.fd_order == 3) ? 1 : 2, H = order * hw;
-    p.nw = (g.n_l <= 4) ? 1 : (g.n_l <= 8) ? 2 : (g.n_l <= 16) ? 4 : 8;
-    p.minb = 8 / p.nw;
-    if (g.n_r <= kRpWT) { p.W = g.n_r; p.n_tiles = 1; }
-    else {
-        p.W = kRpWT - 2 * H;
-        if (p.W < kRpWT / 4) return p;
-        p.n_tiles = (g.n_r + p.W - 1) / p.W;
+struct RpPlan { int ok, variant, W, H, WT, n_tiles, n_items, grid, threads; };
+
+inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant) {
+    RpPlan best{};
+    const int hw = (g.fd_order == 3) ? 1 : 2;
+    int H = order * hw;
+    if ((g.n_r & 1) == 0) H = (H + 1) & ~1;             // even halo: every patch row starts 32-byte aligned
+    double best_cost = 0.0;
+    for (int i = 0; i < kNumRpVariants; ++i) {
+        if (force_variant >= 0 && i != force_variant) continue;
+        const RpVariant &v = kRpVariants[i];
+        const int rows = kRpRows * v.nwr, WT = 32 * v.cp * v.nwc;
+        if (rows < g.n_l || v.cp < hw) continue;
+        if (rows >= 2 * g.n_l && v.nwr > 1) continue;      // more than half of the rows would be padding
+        RpPlan p{};
+        p.variant = i; p.H = H; p.WT = WT; p.threads = 32 * v.nwr * v.nwc;
+        if (g.n_r <= WT) { p.W = g.n_r; p.n_tiles = 1; }
+        else {
+            p.W = WT - 2 * H;
+            if (p.W < WT / 4) continue;
+            p.n_tiles = (g.n_r + p.W - 1) / p.W;
+        }
+        p.n_items = p.n_tiles * g.batch;
+        p.grid = std::min(p.n_items, n_sm * v.minb);
+        // a grid that is a multiple of n_tiles keeps every CTA on one radial tile (coefficients loaded once)
+        if (p.n_tiles * 4 <= p.grid) p.grid = p.grid / p.n_tiles * p.n_tiles;
+        p.ok = 1;
+        // cost: columns computed in total; 8 points per thread hides latency better on 3-point stencils, the
+        // 5-point stencil needs twice the shuffles with 2-column patches
+        double cost = (double)p.n_tiles * WT * rows;
+        if (force_variant < 0) {
+            if (g.fd_order == 5 && v.cp == 2) cost *= 1.5;
+            if (g.fd_order == 3 && v.cp == 4) cost *= 1.2;
+        }
+        if (!best.ok || cost < best_cost) { best = p; best_cost = cost; }
     }
-    p.n_items = p.n_tiles * g.batch;
-    p.grid = std::min(p.n_items, n_sm * p.minb);
-    p.ok = 1;
-    return p;
+    return best;
 }
 
-template <int FD, int NW, int MINB>
+template <int FD, int CP, int NWR, int NWC, int MINB>
 inline int rp_launch_one(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
                          const double *dtp, int order, cudaStream_t s) {
-    const bool mask = g.n_r < kRpWT;
-    const int smem = (int)sizeof(RpSmem<NW>);
+    if (FD == 5 && CP < 2) return TDSE_ERR_UNSUPPORTED;
+    const bool mask = g.n_r < 32 * CP * NWC;
+    const int smem = (int)sizeof(RpSmem<FD, CP, NWR, NWC>);
     static bool attr_set[2] = {false, false};
     if (!attr_set[mask]) {
-        cudaError_t e = mask ? cudaFuncSetAttribute(taylor_rp_kernel<FD, NW, true, MINB>,
+        cudaError_t e = mask ? cudaFuncSetAttribute(taylor_rp_kernel<FD, CP, NWR, NWC, true, MINB>,
                                                     cudaFuncAttributeMaxDynamicSharedMemorySize, smem)
-                             : cudaFuncSetAttribute(taylor_rp_kernel<FD, NW, false, MINB>,
+                             : cudaFuncSetAttribute(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB>,
                                                     cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return TDSE_ERR_CUDA;
         attr_set[mask] = true;
     }
     if (mask)
-        taylor_rp_kernel<FD, NW, true, MINB><<<p.grid, NW * 32, smem, s>>>(g, in, out, ef, dtp, order, p.W, p.n_tiles, p.n_items);
+        taylor_rp_kernel<FD, CP, NWR, NWC, true, MINB><<<p.grid, p.threads, smem, s>>>(g, in, out, ef, dtp, order, p.W, p.H, p.n_tiles, p.n_items);
     else
-        taylor_rp_kernel<FD, NW, false, MINB><<<p.grid, NW * 32, smem, s>>>(g, in, out, ef, dtp, order, p.W, p.n_tiles, p.n_items);
+        taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB><<<p.grid, p.threads, smem, s>>>(g, in, out, ef, dtp, order, p.W, p.H, p.n_tiles, p.n_items);
     return cudaGetLastError() == cudaSuccess ? TDSE_OK : TDSE_ERR_CUDA;
 }
 
 inline int launch_taylor_rp(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
                             const double *dtp, int order, cudaStream_t s) {
     if (!p.ok) return TDSE_ERR_UNSUPPORTED;
-#define TDSE_RP_CASE(NW, MINB)                                                                     \
-    case NW:                                                                                       \
-        return (g.fd == 3) ? rp_launch_one<3, NW, MINB>(g, p, in, out, ef, dtp, order, s)          \
-                           : rp_launch_one<5, NW, MINB>(g, p, in, out, ef, dtp, order, s);
-    switch (p.nw) {
-        TDSE_RP_CASE(1, 8)
-        TDSE_RP_CASE(2, 4)
-        TDSE_RP_CASE(4, 2)
-        TDSE_RP_CASE(8, 1)
+#define TDSE_RP_CASE(I, CP, NWR, NWC, MINB)                                                                  \
+    case I:                                                                                                  \
+        return (g.fd == 3) ? rp_launch_one<3, CP, NWR, NWC, MINB>(g, p, in, out, ef, dtp, order, s)          \
+                           : rp_launch_one<5, CP, NWR, NWC, MINB>(g, p, in, out, ef, dtp, order, s);
+    switch (p.variant) {
+        TDSE_RP_CASE(0, 4, 1, 1, 8)
+        TDSE_RP_CASE(1, 4, 2, 1, 4)
+        TDSE_RP_CASE(2, 4, 4, 1, 2)
+        TDSE_RP_CASE(3, 4, 8, 1, 1)
+        TDSE_RP_CASE(4, 2, 1, 2, 8)
+        TDSE_RP_CASE(5, 2, 2, 2, 4)
+        TDSE_RP_CASE(6, 2, 4, 2, 2)
+        TDSE_RP_CASE(7, 2, 8, 2, 1)
+        TDSE_RP_CASE(8, 2, 4, 4, 1)
     }
 #undef TDSE_RP_CASE
     return TDSE_ERR_UNSUPPORTED;

@@ -249,22 +249,26 @@ def test_taylor_register_tile_parity(B, case):
 
 
 RP_CASES = [
-    # n_r, dr, n_l, fd, batch, order, nsteps, obs_every, use_graph
-    (500, 0.2, 8, 3, 1, 4, 101, 1, 1),           # CFG1: 2 warps, 5 tiles of 128 columns
-    (2000, 0.1, 16, 3, 3, 6, 12, 0, 1),          # CFG5 rows and width: 18 tiles, clamped last tile
-    (2000, 0.1, 16, 3, 2, 6, 9, 4, 0),           # same, eager, odd number of steps
-    (333, 0.1, 11, 5, 3, 6, 40, 4, 1),           # ragged rows (11 of 16), 5-point, batched
-    (333, 0.1, 11, 3, 2, 5, 33, 0, 1),           # odd order
-    (129, 0.1, 16, 5, 1, 10, 10, 0, 1),          # grid one column wider than a tile, halo 20
-    (128, 0.1, 13, 5, 1, 12, 6, 2, 1),           # grid exactly one tile: walls on both sides, no mask
-    (100, 0.2, 3, 3, 1, 4, 20, 1, 1),            # grid narrower than a tile: masked instantiation, 1 warp
-    (37, 0.2, 3, 5, 2, 1, 9, 1, 1),              # order 1, masked, 5-point
-    (420, 0.1, 32, 5, 1, 10, 8, 3, 1),           # 32 rows: 8 warps, one CTA per SM
-    (420, 0.1, 29, 3, 2, 7, 8, 0, 1),            # 29 of 32 rows
-    (1000, 0.1, 5, 3, 1, 8, 8, 0, 1),            # 5 of 8 rows
-    (1000, 0.1, 24, 5, 1, 4, 8, 0, 1),           # 24 of 32 rows
-    (700, 0.1, 4, 3, 300, 6, 6, 0, 1),           # more work items than resident CTAs: persistent loop + L2 prefetch
-    (3000, 0.1, 16, 5, 40, 3, 5, 0, 1),          # several items per CTA, 5-point
+    # n_r, dr, n_l, fd, batch, order, nsteps, obs_every, variant(-1 = heuristic), use_graph
+    (500, 0.2, 8, 3, 1, 4, 101, 1, -1, 1),       # CFG1
+    (2000, 0.1, 16, 3, 3, 6, 12, 0, -1, 1),      # CFG5 rows and width, clamped last tile
+    (2000, 0.1, 16, 3, 2, 6, 9, 4, 2, 0),        # same, 16-point patches, eager, odd number of steps
+    (2000, 0.1, 16, 3, 2, 6, 8, 0, 8, 1),        # same, 256-column tile of 16 warps
+    (2000, 0.1, 16, 5, 2, 6, 8, 0, 6, 1),        # 5-point stencil on 2-column patches (4 shuffled columns per row)
+    (333, 0.1, 11, 5, 3, 6, 40, 4, -1, 1),       # ragged rows (11 of 16), 5-point, batched, odd n_r (128-bit path)
+    (333, 0.1, 11, 3, 2, 5, 33, 0, -1, 1),       # odd order, odd n_r
+    (334, 0.1, 11, 3, 2, 5, 20, 0, -1, 1),       # odd order, even n_r: halo rounded up to even (256-bit path)
+    (129, 0.1, 16, 5, 1, 10, 10, 0, 2, 1),       # grid one column wider than a tile, halo 20
+    (128, 0.1, 13, 5, 1, 12, 6, 2, 2, 1),        # grid exactly one tile: walls on both sides, no mask
+    (100, 0.2, 3, 3, 1, 4, 20, 1, -1, 1),        # grid narrower than a tile: masked instantiation
+    (37, 0.2, 3, 5, 2, 1, 9, 1, 0, 1),           # order 1, masked, 5-point, one warp
+    (420, 0.1, 32, 5, 1, 10, 8, 3, 3, 1),        # 32 rows: 8 warps of 16-point patches
+    (420, 0.1, 29, 3, 2, 7, 8, 0, 7, 1),         # 29 of 32 rows: 16 warps of 8-point patches
+    (1000, 0.1, 5, 3, 1, 8, 8, 0, 1, 1),         # 5 of 8 rows
+    (1000, 0.1, 5, 3, 1, 8, 8, 0, 5, 1),         # 5 of 8 rows, 8-point patches
+    (1000, 0.1, 24, 5, 1, 4, 8, 0, -1, 1),       # 24 of 32 rows
+    (700, 0.1, 4, 3, 300, 6, 6, 0, 4, 1),        # more work items than resident CTAs: persistent loop
+    (3000, 0.1, 16, 5, 40, 3, 5, 0, -1, 1),      # several items per CTA, 5-point
 ]
 
 
@@ -273,13 +277,13 @@ def test_taylor_register_patch_parity(B, case):
     """The persistent register-patch kernel (v3: shuffle radial exchange, scaled operator H/c1, direct global
     loads) against the oracle's order-by-order recursion: every warp count, walls, ragged rows and columns,
     masked grids, and more work items than resident CTAs."""
-    n_r, dr, n_l, fd, batch, order, nsteps, obs_every, use_graph = case
+    n_r, dr, n_l, fd, batch, order, nsteps, obs_every, variant, use_graph = case
     c = wl.config("cfg5" if batch > 1 else "cfg1", n_r=n_r, dr=dr, n_l=n_l, fd_order=fd, batch=batch, order=order)
     c["propagator"] = "taylor"
     dt = wl.dt_eff(c, "taylor", order)
     t0 = wl.window(c, nsteps, dt)
     psi0 = wl.populated_state(c)
-    opts = {"taylor_block": 4, "use_graph": use_graph}
+    opts = {"taylor_block": 4, "use_graph": use_graph, "taylor_rp_variant": variant}
     h, got, ref, gobs, robs = run_pair_fixed(B, c, "taylor", nsteps, psi0, t0, dt, obs_every, [(0, 0)], opts, order=order)
     assert h.taylor_kernel() == 3
     check_fixed(got, ref, gobs, robs)
