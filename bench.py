@@ -190,6 +190,7 @@ def run_own(args):
     h.set_option("taylor_block", 0 if args.no_block else args.taylor_block)
     h.set_option("taylor_rt_variant", args.rt_variant)
     h.set_option("taylor_rp_variant", args.rp_variant)
+    h.set_option("taylor_rp_tma", args.rp_tma)
     h.set_option("graph_steps", args.graph_steps)
     h.set_pulse(pulses)
     stream = torch.cuda.Stream()
@@ -249,7 +250,7 @@ def run_own(args):
     peak, peak_src = measured_peaks()
     if blocked:
         bytes_step = 32.0 * pts                         # read psi once, write psi once (all orders in shared memory)
-        kname, n_dom = {3: "taylor_rp_kernel", 2: "taylor_rt_kernel"}.get(blocked, "taylor_blocked_kernel"), K
+        kname, n_dom = {4: "taylor_rp_kernel (TMA)", 3: "taylor_rp_kernel", 2: "taylor_rt_kernel"}.get(blocked, "taylor_blocked_kernel"), K
     else:
         bytes_step = (64.0 * order - 32.0) * pts        # k=1: 16R+32W, 1<k<P: 32R+32W, k=P: 32R+16W
         kname, n_dom = "tile_kernel<EpiTaylor>", K * order
@@ -358,6 +359,7 @@ def main():
     ap.add_argument("--taylor-block", type=int, default=1, help="1 auto, 2 shared-memory tile kernel, 3 register tiles (v2), 4 persistent register patches (v3)")
     ap.add_argument("--rt-variant", type=int, default=-1, help="instantiation of the register-tile kernel")
     ap.add_argument("--rp-variant", type=int, default=-1, help="instantiation of the register-patch kernel")
+    ap.add_argument("--rp-tma", type=int, default=-1, help="register-patch kernel: -1 auto, 0 direct loads, 1 TMA")
     ap.add_argument("--no-extra", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()

@@ -74,6 +74,8 @@ void tdse_destroy(tdse_handle *h);
  *   "taylor_block_width" [0] interior tile width W of the shared-memory tile kernel (0: heuristic)
  *   "taylor_rt_variant" [-1] instantiation of the register-tile kernel (-1: heuristic)
  *   "taylor_rp_variant" [-1] instantiation of the register-patch kernel (-1: heuristic)
+ *   "taylor_rp_tma"    [-1] register-patch kernel: fetch tiles by TMA tensor copies (-1: heuristic, 0: never,
+ *                          1: whenever n_r % 8 == 0 and the grid is wider than a tile)
  *   "lanczos_beta_tol" [1e-12] breakdown threshold on beta ("if beta = 0 then quit", R-G17)
  *   "rk45_dt_max"      [0 = none] cap on the adaptive step
  *   "rk45_check_every" [8] attempted steps enqueued between host checks of the device `done` flag */
@@ -133,7 +135,8 @@ int  tdse_lanczos_info(tdse_handle *h, double *alpha, double *beta, double *coef
 /* Number of CUDA kernels this handle has launched so far (graph nodes counted per graph launch). */
 long tdse_launch_count(tdse_handle *h);
 /* Kernel used by the last tdse_step_taylor call: 0 one kernel per order, 1 shared-memory tile kernel (all orders in
- * one pass), 2 register-tile kernel (all orders in one pass). */
+ * one pass), 2 register-tile kernel v2, 3 persistent register-patch kernel v3 with direct global loads, 4 the same
+ * with TMA tile fetches (1-4: all orders in one pass). */
 int  tdse_taylor_was_blocked(tdse_handle *h);
 
 const char *tdse_strerror(int code);

@@ -93,7 +93,7 @@ struct tdse_handle {
     // blocked Taylor configuration
     BlockedCfg bcfg{};
     RtPlan rtp{}; int rt_variant = -1;
-    RpPlan rpp{}; int n_sm = 148; int rp_variant = -1;
+    RpPlan rpp{}; int n_sm = 148; int rp_variant = -1, rp_tma = -1;
 };
 
 namespace {
@@ -418,7 +418,7 @@ int run_blocks(tdse_handle *h, int kind, int p1, int p2, int n, int obs, long nb
         }
         return TDSE_OK;
     }
-    const auto key = std::make_tuple(kind, p1, p2, n, obs + 2 * h->taylor_blocked_last + 16 * (h->rtp.variant + 1) + 256 * (h->rpp.variant + 1), h->psi_slot);
+    const auto key = std::make_tuple(kind, p1, p2, n, obs + 2 * h->taylor_blocked_last + 16 * (h->rtp.variant + 1) + 256 * (h->rpp.variant + 1) + 8192 * h->rpp.tma, h->psi_slot);
     auto it = h->graphs.find(key);
     if (it == h->graphs.end()) {
         cudaGraph_t g = nullptr;
@@ -582,6 +582,7 @@ int tdse_set_option(tdse_handle *h, const char *key, double value) {
     else if (k == "taylor_block") { if (value < 0 || value > 4) return TDSE_ERR_ARG; h->taylor_block = (int)value; }
     else if (k == "taylor_rt_variant") { if (value < -1 || value >= kNumRtVariants) return TDSE_ERR_ARG; h->rt_variant = (int)value; free_graphs(h); }
     else if (k == "taylor_rp_variant") { if (value < -1 || value >= kNumRpVariants) return TDSE_ERR_ARG; h->rp_variant = (int)value; free_graphs(h); }
+    else if (k == "taylor_rp_tma") { if (value < -1 || value > 1) return TDSE_ERR_ARG; h->rp_tma = (int)value; free_graphs(h); }
     else if (k == "taylor_block_width") { if (value < 0 || value > 4096) return TDSE_ERR_ARG; h->bcfg.width_override = (int)value; free_graphs(h); }
     else if (k == "lanczos_beta_tol") { if (!(value >= 0.0)) return TDSE_ERR_ARG; h->beta_tol = value; free_graphs(h); }
     else if (k == "rk45_dt_max") { if (!(value >= 0.0)) return TDSE_ERR_ARG; h->rk45_dt_max = value; }
@@ -667,7 +668,7 @@ int tdse_step_taylor(tdse_handle *h, int order, double t0, double dt, long nstep
     h->rtp = RtPlan{};
     h->rpp = RpPlan{};
     if (h->taylor_block == 1 || h->taylor_block == 4) {
-        h->rpp = rp_plan(h->grid, order, h->n_sm, h->rp_variant);
+        h->rpp = rp_plan(h->grid, order, h->n_sm, h->rp_variant, h->rp_tma);
         if (h->rpp.ok) h->taylor_blocked_last = 3;
     }
     if (!h->taylor_blocked_last && (h->taylor_block == 1 || h->taylor_block == 3)) {
@@ -836,6 +837,6 @@ int tdse_lanczos_info(tdse_handle *h, double *alpha, double *beta, double *coef,
 }
 
 long tdse_launch_count(tdse_handle *h) { return h ? h->launches : 0; }
-int tdse_taylor_was_blocked(tdse_handle *h) { return h ? h->taylor_blocked_last : 0; }
+int tdse_taylor_was_blocked(tdse_handle *h) { return h ? h->taylor_blocked_last + ((h->taylor_blocked_last == 3 && h->rpp.tma) ? 1 : 0) : 0; }
 
 }  // extern "C"

@@ -18,7 +18,12 @@
 //     c_l E r_j / c1 of the (l, l+1) pair is formed once and used for both rows.  12.25 (3-point) / 16.25 (5-point)
 //     FP64 instructions per point-update instead of 16.3 / 20.
 #pragma once
+#include <cuda.h>
+
 #include <algorithm>
+#include <map>
+#include <mutex>
+#include <tuple>
 
 #include "tdse_device.cuh"
 
@@ -37,8 +42,12 @@ struct RpGeom {
 
 // shared memory: vertical exchange [parity][warp][top,bottom][CP planes][32 lanes], radial edge exchange between
 // the warps of a row group [parity][warp][left,right][4 rows][HW], row table
-template <int FD, int CP, int NWR, int NWC>
+template <int FD, int CP, int NWR, int NWC, bool TMA>
 struct RpSmem {
+    // TMA landing zone of the next item: [row][128-byte column group][8 columns], 128-byte swizzled; first member
+    // so that it is 1024-byte aligned
+    double2 stage[TMA ? kRpRows * NWR * 32 * CP * NWC : 1];
+    unsigned long long mbar;
     double2 xch[2][NWR * NWC][2][CP][32];
     double2 edge[2][NWR * NWC][2][kRpRows][(FD == 3) ? 1 : 2];
     double rowtab[NWR * kRpRows][4];        // {c_{l-1}, c_l, l(l+1), 0}
@@ -57,6 +66,30 @@ __device__ __forceinline__ void stg256(double2 *p, const double2 &a, const doubl
     asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a.x), "d"(a.y), "d"(b.x), "d"(b.y) : "memory");
 }
 
+// ---- TMA (cp.async.bulk.tensor) + mbarrier helpers ---------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity) {
+    unsigned ok;
+    do {
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    } while (!ok);
+}
+// 3-D tiled tensor load global -> shared, completion on an mbarrier
+__device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, int c0, int c1, int c2, unsigned long long *bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+        ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
 // tile start of tile t: interior [t*W, (t+1)*W) plus H halo columns per side, clamped so that a tile at a wall
 // starts (ends) exactly at the wall: the zero beyond the tile IS the Dirichlet wall.
 __device__ __forceinline__ int rp_start(int t, int W, int H, int N, int WT) {
@@ -68,14 +101,20 @@ __device__ __forceinline__ int rp_start(int t, int W, int H, int N, int WT) {
 
 // grid = persistent CTAs, block = NT.  n_l <= 4*NWR.  H = halo columns per side (>= order * HW; even when n_r is
 // even so that every patch row is 32-byte aligned).  MASK: n_r < WT (single tile, columns >= n_r held at zero).
-template <int FD, int CP, int NWR, int NWC, bool MASK, int MINB>
+// TMA: the next item's tile is fetched by one cp.async.bulk.tensor (3-D view [row][n_r/8][8 columns], 128-byte
+// swizzle so that the per-thread patch reads are bank-conflict free) while the current item is computed; needs
+// n_r % 8 == 0, H % 8 == 0, W % 8 == 0 and n_r >= WT.
+template <int FD, int CP, int NWR, int NWC, bool MASK, int MINB, bool TMA>
 __global__ void __launch_bounds__(NWR * NWC * 32, MINB)
 taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict__ out, const double *__restrict__ ef,
-                 const double *__restrict__ dtp, int order, int W, int H, int n_tiles, int n_items) {
+                 const double *__restrict__ dtp, int order, int W, int H, int n_tiles, int n_items,
+                 const __grid_constant__ CUtensorMap tmap) {
+    static_assert(!(TMA && MASK), "the TMA path needs a full tile");
     using G = RpGeom<FD, CP, NWR, NWC>;
     constexpr int RP = kRpRows, WT = G::WT, HW = G::HW;
-    extern __shared__ __align__(16) unsigned char rp_smem_raw[];
-    RpSmem<FD, CP, NWR, NWC> &sm = *reinterpret_cast<RpSmem<FD, CP, NWR, NWC> *>(rp_smem_raw);
+    extern __shared__ __align__(1024) unsigned char rp_smem_raw[];
+    using Smem = RpSmem<FD, CP, NWR, NWC, TMA>;
+    Smem &sm = *reinterpret_cast<Smem *>((reinterpret_cast<uintptr_t>(rp_smem_raw) + 1023) & ~(uintptr_t)1023);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int wr = warp / NWC, wc = warp - wr * NWC;
     const int L = g.n_l, N = g.n_r;
@@ -101,6 +140,18 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
     const int nb_warp = has_nb ? ((lane == 0) ? warp - 1 : warp + 1) : warp;
     const int nb_side = (lane == 0) ? 1 : 0, my_side = (lane == 0) ? 0 : 1;
 
+    constexpr unsigned kStageBytes = (unsigned)(sizeof(double2) * RP * NWR * WT);
+    unsigned tma_phase = 0;
+    if (TMA) {
+        if (threadIdx.x == 0) mbar_init(&sm.mbar, 1);
+        __syncthreads();
+        if (threadIdx.x == 0 && (int)blockIdx.x < n_items) {
+            const int b0 = blockIdx.x / n_tiles, t0 = blockIdx.x - b0 * n_tiles;
+            mbar_expect_tx(&sm.mbar, kStageBytes);
+            tma_load_3d(sm.stage, &tmap, 0, rp_start(t0, W, H, N, WT) >> 3, b0 * L, &sm.mbar);
+        }
+    }
+
     int t_cur = -1;
     double Dq[CP], Cq[CP], Eq[CP];
     bool dom[CP];
@@ -113,6 +164,18 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
         const double2 *src_g = in + (size_t)b * L * N + start + c0;
         // ---- own patch straight from global memory -------------------------------------------------------------
         double2 T[RP][CP], A[RP][CP];
+        if (TMA) {
+            mbar_wait(&sm.mbar, tma_phase);
+            tma_phase ^= 1u;
+            const int gidx = (wc * 32 + lane) * CP / 8, chunk0 = ((wc * 32 + lane) * CP) & 7;
+#pragma unroll
+            for (int r = 0; r < RP; ++r)
+#pragma unroll
+                for (int q = 0; q < CP; ++q) {
+                    const double2 v = sm.stage[((r0 + r) * (WT / 8) + gidx) * 8 + ((chunk0 + q) ^ (gidx & 7))];
+                    T[r][q] = (r0 + r < L) ? v : z2;
+                }
+        } else {
 #pragma unroll
         for (int r = 0; r < RP; ++r) {
             const double2 *p = src_g + (size_t)(r0 + r) * N;
@@ -128,6 +191,7 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
 #pragma unroll
                 for (int q = 0; q < CP; ++q) T[r][q] = z2;
             }
+        }
         }
         // ---- per-column coefficients (scaled by 1/c1): reloaded only when the radial tile changes ----------------
         if (t != t_cur) {
@@ -247,6 +311,13 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                 }
             }
             __syncthreads();
+            // every value of the stage has been consumed by the arithmetic of order 1: fetch the next item
+            if (TMA && k == 1 && threadIdx.x == 0 && item + (int)gridDim.x < n_items) {
+                const int ni = item + gridDim.x, nb = ni / n_tiles, nt = ni - nb * n_tiles;
+                fence_proxy_async_smem();
+                mbar_expect_tx(&sm.mbar, kStageBytes);
+                tma_load_3d(sm.stage, &tmap, 0, rp_start(nt, W, H, N, WT) >> 3, nb * L, &sm.mbar);
+            }
         };
 
         double2 U[RP][CP];
@@ -301,13 +372,12 @@ constexpr RpVariant kRpVariants[] = {
 };
 constexpr int kNumRpVariants = sizeof(kRpVariants) / sizeof(kRpVariants[0]);
 
-struct RpPlan { int ok, variant, W, H, WT, n_tiles, n_items, grid, threads; };
+struct RpPlan { int ok, variant, tma, W, H, WT, n_tiles, n_items, grid, threads; };
 
-inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant) {
+// use_tma: -1 heuristic, 0 never, 1 whenever the layout allows it (n_r % 8 == 0, a full tile, 4-column patches)
+inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant, int use_tma) {
     RpPlan best{};
     const int hw = (g.fd_order == 3) ? 1 : 2;
-    int H = order * hw;
-    if ((g.n_r & 1) == 0) H = (H + 1) & ~1;             // even halo: every patch row starts 32-byte aligned
     double best_cost = 0.0;
     for (int i = 0; i < kNumRpVariants; ++i) {
         if (force_variant >= 0 && i != force_variant) continue;
@@ -315,29 +385,70 @@ inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant
         const int rows = kRpRows * v.nwr, WT = 32 * v.cp * v.nwc;
         if (rows < g.n_l || v.cp < hw) continue;
         if (rows >= 2 * g.n_l && v.nwr > 1) continue;      // more than half of the rows would be padding
-        RpPlan p{};
-        p.variant = i; p.H = H; p.WT = WT; p.threads = 32 * v.nwr * v.nwc;
-        if (g.n_r <= WT) { p.W = g.n_r; p.n_tiles = 1; }
-        else {
-            p.W = WT - 2 * H;
-            if (p.W < WT / 4) continue;
-            p.n_tiles = (g.n_r + p.W - 1) / p.W;
+        for (int tma = 0; tma <= 1; ++tma) {
+            if (tma && (use_tma == 0 || v.cp != 4 || (g.n_r & 7) || g.n_r <= WT)) continue;
+            if (!tma && use_tma == 1 && v.cp == 4 && !(g.n_r & 7) && g.n_r > WT) continue;
+            int H = order * hw;
+            if (tma) H = (H + 7) & ~7;                      // tile starts on a 128-byte column group
+            else if ((g.n_r & 1) == 0) H = (H + 1) & ~1;    // even halo: every patch row starts 32-byte aligned
+            RpPlan p{};
+            p.variant = i; p.tma = tma; p.H = H; p.WT = WT; p.threads = 32 * v.nwr * v.nwc;
+            if (g.n_r <= WT) { p.W = g.n_r; p.n_tiles = 1; }
+            else {
+                p.W = WT - 2 * H;
+                if (p.W < WT / 4) continue;
+                p.n_tiles = (g.n_r + p.W - 1) / p.W;
+            }
+            p.n_items = p.n_tiles * g.batch;
+            p.grid = std::min(p.n_items, n_sm * v.minb);
+            // a grid that is a multiple of n_tiles keeps every CTA on one radial tile (coefficients loaded once)
+            if (p.n_tiles * 4 <= p.grid) p.grid = p.grid / p.n_tiles * p.n_tiles;
+            p.ok = 1;
+            // cost: columns computed in total; 8-point patches measured 1.5x slower per column than 16-point
+            // patches (twice the exchange per point, spills at 128 registers); the asynchronous tile fetch hides
+            // the load latency of the next item
+            double cost = (double)p.n_tiles * WT * rows;
+            if (force_variant < 0 && v.cp == 2) cost *= 1.5;
+            if (tma) cost *= 0.85;
+            if (!best.ok || cost < best_cost) { best = p; best_cost = cost; }
         }
-        p.n_items = p.n_tiles * g.batch;
-        p.grid = std::min(p.n_items, n_sm * v.minb);
-        // a grid that is a multiple of n_tiles keeps every CTA on one radial tile (coefficients loaded once)
-        if (p.n_tiles * 4 <= p.grid) p.grid = p.grid / p.n_tiles * p.n_tiles;
-        p.ok = 1;
-        // cost: columns computed in total; 8 points per thread hides latency better on 3-point stencils, the
-        // 5-point stencil needs twice the shuffles with 2-column patches
-        double cost = (double)p.n_tiles * WT * rows;
-        if (force_variant < 0) {
-            if (g.fd_order == 5 && v.cp == 2) cost *= 1.5;
-            if (g.fd_order == 3 && v.cp == 4) cost *= 1.2;
-        }
-        if (!best.ok || cost < best_cost) { best = p; best_cost = cost; }
     }
     return best;
+}
+
+// cuTensorMapEncodeTiled through the runtime (no link against libcuda)
+typedef CUresult (*RpEncodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// tensor map of a state array seen as [batch*n_l rows][n_r/8 groups][16 doubles], box = rows x WT/8 x 16, cached
+inline const CUtensorMap *rp_tensor_map(const void *base, int n_r, int total_rows, int box_rows, int WT) {
+    static std::map<std::tuple<const void *, int, int, int, int>, CUtensorMap> cache;
+    static std::mutex mu;
+    static RpEncodeTiled encode = nullptr;
+    std::lock_guard<std::mutex> lock(mu);
+    const auto key = std::make_tuple(base, n_r, total_rows, box_rows, WT);
+    auto it = cache.find(key);
+    if (it != cache.end()) return &it->second;
+    if (!encode) {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+            qres != cudaDriverEntryPointSuccess)
+            return nullptr;
+        encode = (RpEncodeTiled)fn;
+    }
+    CUtensorMap m;
+    const cuuint64_t dims[3] = {16, (cuuint64_t)(n_r / 8), (cuuint64_t)total_rows};
+    const cuuint64_t strides[2] = {128, (cuuint64_t)n_r * 16};          // bytes, dims 1 and 2
+    const cuuint32_t box[3] = {16, (cuuint32_t)(WT / 8), (cuuint32_t)box_rows};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    if (encode(&m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void *>(base), dims, strides, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return nullptr;
+    if (cache.size() > 64) cache.clear();
+    return &(cache[key] = m);
 }
 
 template <int FD, int CP, int NWR, int NWC, int MINB>
@@ -345,20 +456,32 @@ inline int rp_launch_one(const GridDev &g, const RpPlan &p, const double2 *in, d
                          const double *dtp, int order, cudaStream_t s) {
     if (FD == 5 && CP < 2) return TDSE_ERR_UNSUPPORTED;
     const bool mask = g.n_r < 32 * CP * NWC;
-    const int smem = (int)sizeof(RpSmem<FD, CP, NWR, NWC>);
-    static bool attr_set[2] = {false, false};
-    if (!attr_set[mask]) {
-        cudaError_t e = mask ? cudaFuncSetAttribute(taylor_rp_kernel<FD, CP, NWR, NWC, true, MINB>,
-                                                    cudaFuncAttributeMaxDynamicSharedMemorySize, smem)
-                             : cudaFuncSetAttribute(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB>,
-                                                    cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return TDSE_ERR_CUDA;
-        attr_set[mask] = true;
+    const int mode = (p.tma && CP == 4) ? 2 : (mask ? 1 : 0);
+    auto set_attr = [](const void *fn, int smem) {
+        return cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) == cudaSuccess;
+    };
+    static bool attr_set[3] = {false, false, false};
+    CUtensorMap dummy{};
+    if (mode == 2) {
+        if (CP != 4) return TDSE_ERR_UNSUPPORTED;
+        constexpr bool kTma = (CP == 4);
+        auto kern = taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, kTma>;
+        const int smem = (int)sizeof(RpSmem<FD, CP, NWR, NWC, kTma>) + 1024;
+        if (!attr_set[2]) { if (!set_attr((const void *)kern, smem)) return TDSE_ERR_CUDA; attr_set[2] = true; }
+        const CUtensorMap *tm = rp_tensor_map(in, g.n_r, g.batch * g.n_l, kRpRows * NWR, 32 * CP * NWC);
+        if (!tm) return TDSE_ERR_CUDA;
+        kern<<<p.grid, p.threads, smem, s>>>(g, in, out, ef, dtp, order, p.W, p.H, p.n_tiles, p.n_items, *tm);
+    } else if (mode == 1) {
+        auto kern = taylor_rp_kernel<FD, CP, NWR, NWC, true, MINB, false>;
+        const int smem = (int)sizeof(RpSmem<FD, CP, NWR, NWC, false>) + 1024;
+        if (!attr_set[1]) { if (!set_attr((const void *)kern, smem)) return TDSE_ERR_CUDA; attr_set[1] = true; }
+        kern<<<p.grid, p.threads, smem, s>>>(g, in, out, ef, dtp, order, p.W, p.H, p.n_tiles, p.n_items, dummy);
+    } else {
+        auto kern = taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false>;
+        const int smem = (int)sizeof(RpSmem<FD, CP, NWR, NWC, false>) + 1024;
+        if (!attr_set[0]) { if (!set_attr((const void *)kern, smem)) return TDSE_ERR_CUDA; attr_set[0] = true; }
+        kern<<<p.grid, p.threads, smem, s>>>(g, in, out, ef, dtp, order, p.W, p.H, p.n_tiles, p.n_items, dummy);
     }
-    if (mask)
-        taylor_rp_kernel<FD, CP, NWR, NWC, true, MINB><<<p.grid, p.threads, smem, s>>>(g, in, out, ef, dtp, order, p.W, p.H, p.n_tiles, p.n_items);
-    else
-        taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB><<<p.grid, p.threads, smem, s>>>(g, in, out, ef, dtp, order, p.W, p.H, p.n_tiles, p.n_items);
     return cudaGetLastError() == cudaSuccess ? TDSE_OK : TDSE_ERR_CUDA;
 }
 

@@ -272,8 +272,9 @@ RP_CASES = [
 ]
 
 
+@pytest.mark.parametrize("tma", [0, 1])
 @pytest.mark.parametrize("case", RP_CASES)
-def test_taylor_register_patch_parity(B, case):
+def test_taylor_register_patch_parity(B, case, tma):
     """The persistent register-patch kernel (v3: shuffle radial exchange, scaled operator H/c1, direct global
     loads) against the oracle's order-by-order recursion: every warp count, walls, ragged rows and columns,
     masked grids, and more work items than resident CTAs."""
@@ -283,9 +284,10 @@ def test_taylor_register_patch_parity(B, case):
     dt = wl.dt_eff(c, "taylor", order)
     t0 = wl.window(c, nsteps, dt)
     psi0 = wl.populated_state(c)
-    opts = {"taylor_block": 4, "use_graph": use_graph, "taylor_rp_variant": variant}
+    opts = {"taylor_block": 4, "use_graph": use_graph, "taylor_rp_variant": variant, "taylor_rp_tma": tma}
     h, got, ref, gobs, robs = run_pair_fixed(B, c, "taylor", nsteps, psi0, t0, dt, obs_every, [(0, 0)], opts, order=order)
-    assert h.taylor_kernel() == 3
+    tma_applies = bool(tma) and n_r % 8 == 0 and n_r > 128 and variant in (-1, 0, 1, 2, 3)
+    assert h.taylor_kernel() == (4 if tma_applies else 3)
     check_fixed(got, ref, gobs, robs)
     for b in range(batch):
         for l in range(n_l):
