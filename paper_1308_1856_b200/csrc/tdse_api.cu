@@ -508,6 +508,7 @@ int tdse_create(const tdse_grid *grid, tdse_handle **out) {
             cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n_sm > 0)
             h->n_sm = n_sm;
     }
+    if (rp_init_tables() != TDSE_OK) { delete h; return TDSE_ERR_CUDA; }
     const int N = grid->n_r, L = grid->n_l, B = grid->batch;
     h->n_state = (size_t)N * L * B;
     auto fail = [&](int rc) { tdse_destroy(h); return rc; };

@@ -30,6 +30,7 @@
 namespace tdse {
 
 constexpr int kRpRows = 4;     // patch rows
+__constant__ double kRpInvK[65];   // 1/k, k = 1..64 (filled by rp_init_tables)
 
 template <int FD, int CP, int NWR, int NWC>
 struct RpGeom {
@@ -110,11 +111,13 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                  const double *__restrict__ dtp, int order, int W, int H, int n_tiles, int n_items,
                  const __grid_constant__ CUtensorMap tmap) {
     static_assert(!(TMA && MASK), "the TMA path needs a full tile");
+    static_assert(NWC > 1 || CP == 4, "one-warp-wide tiles use the edge-weight trick, which needs 4-column patches");
     using G = RpGeom<FD, CP, NWR, NWC>;
     constexpr int RP = kRpRows, WT = G::WT, HW = G::HW;
     extern __shared__ __align__(1024) unsigned char rp_smem_raw[];
     using Smem = RpSmem<FD, CP, NWR, NWC, TMA>;
-    Smem &sm = *reinterpret_cast<Smem *>((reinterpret_cast<uintptr_t>(rp_smem_raw) + 1023) & ~(uintptr_t)1023);
+    Smem &sm = *reinterpret_cast<Smem *>(rp_smem_raw);     // dynamic shared memory starts 1024-byte aligned
+    if (TMA && (smem_u32(rp_smem_raw) & 1023u)) __trap();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int wr = warp / NWC, wc = warp - wr * NWC;
     const int L = g.n_l, N = g.n_r;
@@ -151,6 +154,8 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
             tma_load_3d(sm.stage, &tmap, 0, rp_start(t0, W, H, N, WT) >> 3, b0 * L, &sm.mbar);
         }
     }
+
+    const double wl = (lane == 0) ? 0.0 : 1.0, wrt = (lane == 31) ? 0.0 : 1.0;
 
     int t_cur = -1;
     double Dq[CP], Cq[CP], Eq[CP];
@@ -236,8 +241,12 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
             double2 lo[CP], below[CP];
 #pragma unroll
             for (int q = 0; q < CP; ++q) {
+#ifdef RP_EXP_NOXCH
+                lo[q] = Ti[3][q]; below[q] = Ti[0][q];
+#else
                 lo[q] = (wr > 0) ? sm.xch[pr][wr > 0 ? warp - NWC : 0][1][q][lane] : z2;
                 below[q] = (wr < NWR - 1) ? sm.xch[pr][wr < NWR - 1 ? warp + NWC : 0][0][q][lane] : z2;
+#endif
             }
             double alo[CP];
             {
@@ -257,14 +266,14 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                 }
                 double2 lf1 = shfl_up2(Ti[r][CP - 1]);       // column c0 - 1 from lane - 1
                 double2 rg1 = shfl_dn2(Ti[r][0]);            // column c0 + CP from lane + 1
-                if (lane == 0) lf1 = ev1;
-                if (lane == 31) rg1 = ev1;
                 double2 lf2 = z2, rg2 = z2;
                 if (FD == 5) {
                     lf2 = shfl_up2(Ti[r][CP - 2]);
                     rg2 = shfl_dn2(Ti[r][1]);
-                    if (lane == 0) lf2 = ev2;
-                    if (lane == 31) rg2 = ev2;
+                }
+                if (NWC > 1) {      // NWC == 1: the tile edge is zero through the weights wl / wrt below
+                    if (lane == 0) { lf1 = ev1; lf2 = ev2; }
+                    if (lane == 31) { rg1 = ev1; rg2 = ev2; }
                 }
 #pragma unroll
                 for (int q = 0; q < CP; ++q) {
@@ -275,12 +284,20 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                     const double2 dn = (r > 0) ? Ti[r > 0 ? r - 1 : 0][q] : lo[q];
                     const double d = fma(ll1, Cq[q], Dq[q]);
                     const double aup = cup * Eq[q];
-                    double hx = m1.x + p1.x, hy = m1.y + p1.y;
+                    // lanes 0 / 31 of a one-warp-wide tile got their own value back from the shuffle: weight 0
+                    double hx, hy;
+                    if (NWC == 1 && q == 0) { hx = fma(wl, m1.x, p1.x); hy = fma(wl, m1.y, p1.y); }
+                    else if (NWC == 1 && q == CP - 1) { hx = fma(wrt, p1.x, m1.x); hy = fma(wrt, p1.y, m1.y); }
+                    else { hx = m1.x + p1.x; hy = m1.y + p1.y; }
                     if (FD == 5) {
                         const double2 m2 = (q > 1) ? Ti[r][q > 1 ? q - 2 : 0] : ((q == 1) ? lf1 : lf2);
                         const double2 p2 = (q < CP - 2) ? Ti[r][q < CP - 2 ? q + 2 : 0] : ((q == CP - 2) ? rg1 : rg2);
-                        hx = fma(c2p, m2.x + p2.x, hx);
-                        hy = fma(c2p, m2.y + p2.y, hy);
+                        double sx, sy;
+                        if (NWC == 1 && q <= 1) { sx = fma(wl, m2.x, p2.x); sy = fma(wl, m2.y, p2.y); }
+                        else if (NWC == 1 && q >= CP - 2) { sx = fma(wrt, p2.x, m2.x); sy = fma(wrt, p2.y, m2.y); }
+                        else { sx = m2.x + p2.x; sy = m2.y + p2.y; }
+                        hx = fma(c2p, sx, hx);
+                        hy = fma(c2p, sy, hy);
                     }
                     hx = fma(d, f.x, hx);
                     hy = fma(d, f.y, hy);
@@ -296,7 +313,11 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                     else { A[r][q].x = fma(s, hx, A[r][q].x); A[r][q].y = fma(s, hy, A[r][q].y); }
                 }
             }
+#ifdef RP_EXP_NOXCH
+            if (false) {
+#else
             if (k < order) {
+#endif
 #pragma unroll
                 for (int q = 0; q < CP; ++q) {
                     sm.xch[pw][warp][0][q][lane] = To[0][q];
@@ -310,7 +331,9 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                             sm.edge[pw][warp][my_side][r][h] = (lane == 0) ? To[r][h] : To[r][CP - 1 - h];
                 }
             }
+#ifndef RP_EXP_NOBAR
             __syncthreads();
+#endif
             // every value of the stage has been consumed by the arithmetic of order 1: fetch the next item
             if (TMA && k == 1 && threadIdx.x == 0 && item + (int)gridDim.x < n_items) {
                 const int ni = item + gridDim.x, nb = ni / n_tiles, nt = ni - nb * n_tiles;
@@ -324,13 +347,13 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
         double sk = 1.0;
         int k = 1;
         for (; k + 1 <= order; k += 2) {
-            sk = sk * (kappa / (double)k);
+            sk = sk * (kappa * kRpInvK[k]);
             sweep(T, U, k, true, (k & 2) ? -sk : sk);
-            sk = sk * (kappa / (double)(k + 1));
+            sk = sk * (kappa * kRpInvK[k + 1]);
             sweep(U, T, k + 1, false, ((k + 1) & 2) ? -sk : sk);
         }
         if (k <= order) {
-            sk = sk * (kappa / (double)k);
+            sk = sk * (kappa * kRpInvK[k]);
             sweep(T, U, k, true, (k & 2) ? -sk : sk);
         }
 
@@ -371,6 +394,13 @@ constexpr RpVariant kRpVariants[] = {
     {2, 4, 4, 1},                                                // 256-column tile, 8 points per thread, n_l <= 16
 };
 constexpr int kNumRpVariants = sizeof(kRpVariants) / sizeof(kRpVariants[0]);
+
+inline int rp_init_tables() {
+    double h[65];
+    h[0] = 0.0;
+    for (int k = 1; k <= 64; ++k) h[k] = 1.0 / (double)k;
+    return cudaMemcpyToSymbol(kRpInvK, h, sizeof(h)) == cudaSuccess ? TDSE_OK : TDSE_ERR_CUDA;
+}
 
 struct RpPlan { int ok, variant, tma, W, H, WT, n_tiles, n_items, grid, threads; };
 
@@ -466,19 +496,19 @@ inline int rp_launch_one(const GridDev &g, const RpPlan &p, const double2 *in, d
         if (CP != 4) return TDSE_ERR_UNSUPPORTED;
         constexpr bool kTma = (CP == 4);
         auto kern = taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, kTma>;
-        const int smem = (int)sizeof(RpSmem<FD, CP, NWR, NWC, kTma>) + 1024;
+        const int smem = (int)sizeof(RpSmem<FD, CP, NWR, NWC, kTma>) + 0;
         if (!attr_set[2]) { if (!set_attr((const void *)kern, smem)) return TDSE_ERR_CUDA; attr_set[2] = true; }
         const CUtensorMap *tm = rp_tensor_map(in, g.n_r, g.batch * g.n_l, kRpRows * NWR, 32 * CP * NWC);
         if (!tm) return TDSE_ERR_CUDA;
         kern<<<p.grid, p.threads, smem, s>>>(g, in, out, ef, dtp, order, p.W, p.H, p.n_tiles, p.n_items, *tm);
     } else if (mode == 1) {
         auto kern = taylor_rp_kernel<FD, CP, NWR, NWC, true, MINB, false>;
-        const int smem = (int)sizeof(RpSmem<FD, CP, NWR, NWC, false>) + 1024;
+        const int smem = (int)sizeof(RpSmem<FD, CP, NWR, NWC, false>) + 0;
         if (!attr_set[1]) { if (!set_attr((const void *)kern, smem)) return TDSE_ERR_CUDA; attr_set[1] = true; }
         kern<<<p.grid, p.threads, smem, s>>>(g, in, out, ef, dtp, order, p.W, p.H, p.n_tiles, p.n_items, dummy);
     } else {
         auto kern = taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false>;
-        const int smem = (int)sizeof(RpSmem<FD, CP, NWR, NWC, false>) + 1024;
+        const int smem = (int)sizeof(RpSmem<FD, CP, NWR, NWC, false>) + 0;
         if (!attr_set[0]) { if (!set_attr((const void *)kern, smem)) return TDSE_ERR_CUDA; attr_set[0] = true; }
         kern<<<p.grid, p.threads, smem, s>>>(g, in, out, ef, dtp, order, p.W, p.H, p.n_tiles, p.n_items, dummy);
     }
