@@ -51,7 +51,8 @@ struct RpSmem {
     unsigned long long mbar;
     double2 xch[2][NWR * NWC][2][CP][32];
     double2 edge[2][NWR * NWC][2][kRpRows][(FD == 3) ? 1 : 2];
-    double rowtab[NWR * kRpRows][4];        // {c_{l-1}, c_l, l(l+1), 0}
+    double2 zrow[CP][32];                   // zeros for ever: the rows above l = 0 and below the last row group
+    double rowtab[NWR * kRpRows][4];        // {c_l, l(l+1), c_{l-1}, 0}
 };
 
 __device__ __forceinline__ double2 shfl_up2(double2 v) {
@@ -126,11 +127,12 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
     const bool al32 = !MASK && ((N & 1) == 0) && ((H & 1) == 0) && ((W & 1) == 0);
 
     for (int r = threadIdx.x; r < NWR * RP; r += G::NT) {
-        sm.rowtab[r][0] = (r >= 1 && r < L) ? __ldg(g.cl + r - 1) : 0.0;
-        sm.rowtab[r][1] = (r + 1 < L) ? __ldg(g.cl + r) : 0.0;
-        sm.rowtab[r][2] = (double)(r * (r + 1));
+        sm.rowtab[r][0] = (r + 1 < L) ? __ldg(g.cl + r) : 0.0;
+        sm.rowtab[r][1] = (double)(r * (r + 1));
+        sm.rowtab[r][2] = (r >= 1 && r < L) ? __ldg(g.cl + r - 1) : 0.0;
         sm.rowtab[r][3] = 0.0;
     }
+    for (int i = threadIdx.x; i < CP * 32; i += G::NT) sm.zrow[i / 32][i % 32] = make_double2(0.0, 0.0);
     __syncthreads();
 
     const double dt = *dtp;
@@ -156,6 +158,11 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
     }
 
     const double wl = (lane == 0) ? 0.0 : 1.0, wrt = (lane == 31) ? 0.0 : 1.0;
+    // l-1 / l+1 rows of the neighbouring row groups (or the zero row); the parity offset is 0 for the zero row
+    constexpr int kParStride = (int)(sizeof(sm.xch[0]) / sizeof(double2));
+    const double2 *lo_base = (wr > 0) ? &sm.xch[0][wr > 0 ? warp - NWC : 0][1][0][lane] : &sm.zrow[0][lane];
+    const double2 *up_base = (wr < NWR - 1) ? &sm.xch[0][wr < NWR - 1 ? warp + NWC : 0][0][0][lane] : &sm.zrow[0][lane];
+    const int lo_par = (wr > 0) ? kParStride : 0, up_par = (wr < NWR - 1) ? kParStride : 0;
 
     int t_cur = -1;
     double Dq[CP], Cq[CP], Eq[CP];
@@ -215,10 +222,6 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
 #pragma unroll
             for (int q = 0; q < CP; ++q) Eq[q] = es * (double)(dom[q] ? start + c0 + q + 1 : 1);
         }
-#pragma unroll
-        for (int r = 0; r < RP; ++r)
-#pragma unroll
-            for (int q = 0; q < CP; ++q) A[r][q] = T[r][q];
         // publish u_0: rows 0 and RP-1 for the warps above / below, edge columns for the warps left / right
 #pragma unroll
         for (int q = 0; q < CP; ++q) {
@@ -236,28 +239,24 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
         // One order: To = H' Ti (rows in increasing l), A += weight * To, publish To's outer rows / edge columns.
         // The order loop below is unrolled by two with the roles of T and U swapped, so that the new term is
         // written where the term before last lived and no register copies are needed at the loop back-edge.
-        auto sweep = [&](const double2 (&Ti)[RP][CP], double2 (&To)[RP][CP], const int k, const bool odd, const double s) {
+        auto sweep = [&](const double2 (&Ti)[RP][CP], double2 (&To)[RP][CP], const int k, const bool odd, const bool first, const double s) {
             const int pr = (k - 1) & 1, pw = k & 1;
             double2 lo[CP], below[CP];
 #pragma unroll
             for (int q = 0; q < CP; ++q) {
-#ifdef RP_EXP_NOXCH
-                lo[q] = Ti[3][q]; below[q] = Ti[0][q];
-#else
-                lo[q] = (wr > 0) ? sm.xch[pr][wr > 0 ? warp - NWC : 0][1][q][lane] : z2;
-                below[q] = (wr < NWR - 1) ? sm.xch[pr][wr < NWR - 1 ? warp + NWC : 0][0][q][lane] : z2;
-#endif
+                lo[q] = lo_base[pr * lo_par + q * 32];
+                below[q] = up_base[pr * up_par + q * 32];
             }
             double alo[CP];
             {
-                const double clo = sm.rowtab[r0][0];
+                const double clo = sm.rowtab[r0][2];
 #pragma unroll
                 for (int q = 0; q < CP; ++q) alo[q] = clo * Eq[q];
             }
 #pragma unroll
             for (int r = 0; r < RP; ++r) {
-                const double cup = sm.rowtab[r0 + r][1];
-                const double ll1 = sm.rowtab[r0 + r][2];
+                const double2 rt = *reinterpret_cast<const double2 *>(&sm.rowtab[r0 + r][0]);
+                const double cup = rt.x, ll1 = rt.y;
                 // columns beyond the warp: zero at a tile edge, else the neighbouring warp's edge column
                 double2 ev1 = z2, ev2 = z2;
                 if (NWC > 1 && has_nb) {
@@ -309,15 +308,13 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                     To[r][q] = make_double2(hx, hy);
                     alo[q] = aup;                           // c_l E r / c1 couples row l+1 back to row l
                     // acc += (-i)^k (dt c1)^k / k! * u'_k; s carries the sign: odd k: -+i, even k: -+1
-                    if (odd) { A[r][q].x = fma(s, hy, A[r][q].x); A[r][q].y = fma(-s, hx, A[r][q].y); }
+                    // (order 1 starts the sum from psi itself: A = u_0 + ..., no separate copy)
+                    if (first) { A[r][q].x = fma(s, hy, f.x); A[r][q].y = fma(-s, hx, f.y); }
+                    else if (odd) { A[r][q].x = fma(s, hy, A[r][q].x); A[r][q].y = fma(-s, hx, A[r][q].y); }
                     else { A[r][q].x = fma(s, hx, A[r][q].x); A[r][q].y = fma(s, hy, A[r][q].y); }
                 }
             }
-#ifdef RP_EXP_NOXCH
-            if (false) {
-#else
             if (k < order) {
-#endif
 #pragma unroll
                 for (int q = 0; q < CP; ++q) {
                     sm.xch[pw][warp][0][q][lane] = To[0][q];
@@ -331,9 +328,7 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                             sm.edge[pw][warp][my_side][r][h] = (lane == 0) ? To[r][h] : To[r][CP - 1 - h];
                 }
             }
-#ifndef RP_EXP_NOBAR
             __syncthreads();
-#endif
             // every value of the stage has been consumed by the arithmetic of order 1: fetch the next item
             if (TMA && k == 1 && threadIdx.x == 0 && item + (int)gridDim.x < n_items) {
                 const int ni = item + gridDim.x, nb = ni / n_tiles, nt = ni - nb * n_tiles;
@@ -344,17 +339,18 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
         };
 
         double2 U[RP][CP];
-        double sk = 1.0;
-        int k = 1;
+        double sk = kappa;
+        sweep(T, U, 1, true, true, sk);                       // order 1: -i
+        int k = 2;
         for (; k + 1 <= order; k += 2) {
             sk = sk * (kappa * kRpInvK[k]);
-            sweep(T, U, k, true, (k & 2) ? -sk : sk);
+            sweep(U, T, k, false, false, (k & 2) ? -sk : sk);
             sk = sk * (kappa * kRpInvK[k + 1]);
-            sweep(U, T, k + 1, false, ((k + 1) & 2) ? -sk : sk);
+            sweep(T, U, k + 1, true, false, ((k + 1) & 2) ? -sk : sk);
         }
         if (k <= order) {
             sk = sk * (kappa * kRpInvK[k]);
-            sweep(T, U, k, true, (k & 2) ? -sk : sk);
+            sweep(U, T, k, false, false, (k & 2) ? -sk : sk);
         }
 
         // ---- psi(t + dt): interior columns of the tile straight from registers ---------------------------------
