@@ -48,7 +48,8 @@ struct RpSmem {
     // TMA landing zone of the next item: [row][128-byte column group][8 columns], 128-byte swizzled; first member
     // so that it is 1024-byte aligned
     double2 stage[TMA ? kRpRows * NWR * 32 * CP * NWC : 1];
-    unsigned long long mbar;
+    unsigned long long mbar;                // completion of the TMA tile fetch
+    unsigned long long cbar;                // CTA-wide split barrier of the order loop (arrive after publishing, wait before reading)
     double2 xch[2][NWR * NWC][2][CP][32];
     double2 edge[2][NWR * NWC][2][kRpRows][(FD == 3) ? 1 : 2];
     double2 zrow[CP][32];                   // zeros for ever: the rows above l = 0 and below the last row group
@@ -92,6 +93,26 @@ __device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, i
 }
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
+// ---- thread-block cluster helpers (distributed shared memory) ----------------------------------------------------
+__device__ __forceinline__ unsigned cluster_ctarank() { unsigned r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ unsigned cluster_nctarank() { unsigned r; asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r)); return r; }
+// shared::cluster address of the same shared-memory offset in CTA `rank` of the cluster
+__device__ __forceinline__ unsigned dsmem_addr(const void *p, unsigned rank) {
+    unsigned r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_u32(p)), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ double2 ld_dsmem2(unsigned addr) {
+    double2 v;
+    asm volatile("ld.shared::cluster.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+__device__ __forceinline__ void mbar_arrive(unsigned long long *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
 // tile start of tile t: interior [t*W, (t+1)*W) plus H halo columns per side, clamped so that a tile at a wall
 // starts (ends) exactly at the wall: the zero beyond the tile IS the Dirichlet wall.
 __device__ __forceinline__ int rp_start(int t, int W, int H, int N, int WT) {
@@ -106,7 +127,10 @@ __device__ __forceinline__ int rp_start(int t, int W, int H, int N, int WT) {
 // TMA: the next item's tile is fetched by one cp.async.bulk.tensor (3-D view [row][n_r/8][8 columns], 128-byte
 // swizzle so that the per-thread patch reads are bank-conflict free) while the current item is computed; needs
 // n_r % 8 == 0, H % 8 == 0, W % 8 == 0 and n_r >= WT.
-template <int FD, int CP, int NWR, int NWC, bool MASK, int MINB, bool TMA>
+// CLUSTER: the n_l rows are split over the CTAs of a thread-block cluster (rank = row block of 4*NWR rows); the
+// l-1 / l+1 rows at a CTA boundary are read from the neighbouring CTA's shared memory (DSMEM) and the per-order
+// barrier is a cluster barrier.
+template <int FD, int CP, int NWR, int NWC, bool MASK, int MINB, bool TMA, bool CLUSTER>
 __global__ void __launch_bounds__(NWR * NWC * 32, MINB)
 taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict__ out, const double *__restrict__ ef,
                  const double *__restrict__ dtp, int order, int W, int H, int n_tiles, int n_items,
@@ -122,14 +146,19 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int wr = warp / NWC, wc = warp - wr * NWC;
     const int L = g.n_l, N = g.n_r;
+    const int crank = CLUSTER ? (int)cluster_ctarank() : 0, csize = CLUSTER ? (int)cluster_nctarank() : 1;
+    const int rbase = crank * NWR * RP;                        // global row of this CTA's row 0
+    const int cid = CLUSTER ? (int)blockIdx.x / csize : (int)blockIdx.x, ncl = CLUSTER ? (int)gridDim.x / csize : (int)gridDim.x;
     const int r0 = wr * RP, c0 = (wc * 32 + lane) * CP;
+    const int gr0 = rbase + r0;                                // global row of this thread's patch row 0
     const double2 z2 = make_double2(0.0, 0.0);
     const bool al32 = !MASK && ((N & 1) == 0) && ((H & 1) == 0) && ((W & 1) == 0);
 
     for (int r = threadIdx.x; r < NWR * RP; r += G::NT) {
-        sm.rowtab[r][0] = (r + 1 < L) ? __ldg(g.cl + r) : 0.0;
-        sm.rowtab[r][1] = (double)(r * (r + 1));
-        sm.rowtab[r][2] = (r >= 1 && r < L) ? __ldg(g.cl + r - 1) : 0.0;
+        const int l = rbase + r;
+        sm.rowtab[r][0] = (l + 1 < L) ? __ldg(g.cl + l) : 0.0;
+        sm.rowtab[r][1] = (double)l * (double)(l + 1);
+        sm.rowtab[r][2] = (l >= 1 && l < L) ? __ldg(g.cl + l - 1) : 0.0;
         sm.rowtab[r][3] = 0.0;
     }
     for (int i = threadIdx.x; i < CP * 32; i += G::NT) sm.zrow[i / 32][i % 32] = make_double2(0.0, 0.0);
@@ -147,15 +176,32 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
 
     constexpr unsigned kStageBytes = (unsigned)(sizeof(double2) * RP * NWR * WT);
     unsigned tma_phase = 0;
-    if (TMA) {
-        if (threadIdx.x == 0) mbar_init(&sm.mbar, 1);
-        __syncthreads();
-        if (threadIdx.x == 0 && (int)blockIdx.x < n_items) {
-            const int b0 = blockIdx.x / n_tiles, t0 = blockIdx.x - b0 * n_tiles;
-            mbar_expect_tx(&sm.mbar, kStageBytes);
-            tma_load_3d(sm.stage, &tmap, 0, rp_start(t0, W, H, N, WT) >> 3, b0 * L, &sm.mbar);
-        }
+    if (threadIdx.x == 0) {
+        mbar_init(&sm.mbar, 1);
+        mbar_init(&sm.cbar, G::NT);
     }
+    __syncthreads();
+    unsigned cphase = 0;
+    bool armed = false;                      // a barrier arrival of this thread has not been waited for yet
+    auto bar_arrive = [&]() {
+        if (CLUSTER) cluster_arrive(); else mbar_arrive(&sm.cbar);
+        armed = true;
+    };
+    auto bar_wait = [&]() {
+        if (CLUSTER) cluster_wait();
+        else { mbar_wait(&sm.cbar, cphase); cphase ^= 1u; }
+        armed = false;
+    };
+    // tile of work item `it` -> stage (one thread; the stage must have been consumed by every thread)
+    auto fetch_item = [&](const int it) {
+        if (TMA && threadIdx.x == 0 && it < n_items) {
+            const int fb = it / n_tiles, ft = it - fb * n_tiles;
+            fence_proxy_async_smem();
+            mbar_expect_tx(&sm.mbar, kStageBytes);
+            tma_load_3d(sm.stage, &tmap, 0, rp_start(ft, W, H, N, WT) >> 3, fb * L + rbase, &sm.mbar);
+        }
+    };
+    fetch_item(cid);
 
     const double wl = (lane == 0) ? 0.0 : 1.0, wrt = (lane == 31) ? 0.0 : 1.0;
     // l-1 / l+1 rows of the neighbouring row groups (or the zero row); the parity offset is 0 for the zero row
@@ -163,6 +209,13 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
     const double2 *lo_base = (wr > 0) ? &sm.xch[0][wr > 0 ? warp - NWC : 0][1][0][lane] : &sm.zrow[0][lane];
     const double2 *up_base = (wr < NWR - 1) ? &sm.xch[0][wr < NWR - 1 ? warp + NWC : 0][0][0][lane] : &sm.zrow[0][lane];
     const int lo_par = (wr > 0) ? kParStride : 0, up_par = (wr < NWR - 1) ? kParStride : 0;
+    // CLUSTER: the row groups at the CTA boundary read the neighbouring CTA's exchange buffer through DSMEM
+    const bool lo_remote = CLUSTER && wr == 0 && crank > 0, up_remote = CLUSTER && wr == NWR - 1 && crank < csize - 1;
+    unsigned lo_dsm = 0, up_dsm = 0;
+    if (CLUSTER) {
+        if (lo_remote) lo_dsm = dsmem_addr(&sm.xch[0][(NWR - 1) * NWC + wc][1][0][lane], (unsigned)(crank - 1));
+        if (up_remote) up_dsm = dsmem_addr(&sm.xch[0][wc][0][0][lane], (unsigned)(crank + 1));
+    }
 
     int t_cur = -1;
     double Dq[CP], Cq[CP], Eq[CP];
@@ -170,13 +223,17 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
 #pragma unroll
     for (int q = 0; q < CP; ++q) { Dq[q] = 0.0; Cq[q] = 0.0; dom[q] = true; }
 
-    for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+    for (int item = cid; item < n_items; item += ncl) {
         const int b = item / n_tiles, t = item - b * n_tiles;
         const int start = rp_start(t, W, H, N, WT);
-        const double2 *src_g = in + (size_t)b * L * N + start + c0;
+        const double2 *src_g = in + ((size_t)b * L + rbase) * N + start + c0;
         // ---- own patch straight from global memory -------------------------------------------------------------
         double2 T[RP][CP], A[RP][CP];
         if (TMA) {
+            if (order < 2 && item != cid) {      // no second order whose barrier could have covered the refill
+                if (armed) bar_wait();
+                fetch_item(item);
+            }
             mbar_wait(&sm.mbar, tma_phase);
             tma_phase ^= 1u;
             const int gidx = (wc * 32 + lane) * CP / 8, chunk0 = ((wc * 32 + lane) * CP) & 7;
@@ -185,13 +242,13 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
 #pragma unroll
                 for (int q = 0; q < CP; ++q) {
                     const double2 v = sm.stage[((r0 + r) * (WT / 8) + gidx) * 8 + ((chunk0 + q) ^ (gidx & 7))];
-                    T[r][q] = (r0 + r < L) ? v : z2;
+                    T[r][q] = (gr0 + r < L) ? v : z2;
                 }
         } else {
 #pragma unroll
         for (int r = 0; r < RP; ++r) {
             const double2 *p = src_g + (size_t)(r0 + r) * N;
-            if (r0 + r < L) {
+            if (gr0 + r < L) {
                 if (al32) {
 #pragma unroll
                     for (int q = 0; q < CP; q += 2) ldg256(p + q, T[r][q], T[r][q + 1]);
@@ -223,6 +280,8 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
             for (int q = 0; q < CP; ++q) Eq[q] = es * (double)(dom[q] ? start + c0 + q + 1 : 1);
         }
         // publish u_0: rows 0 and RP-1 for the warps above / below, edge columns for the warps left / right
+        // (after every thread has finished reading the previous item's last exchange)
+        if (armed) bar_wait();
 #pragma unroll
         for (int q = 0; q < CP; ++q) {
             sm.xch[0][warp][0][q][lane] = T[0][q];
@@ -234,86 +293,108 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
 #pragma unroll
                 for (int h = 0; h < HW; ++h) sm.edge[0][warp][my_side][r][h] = (lane == 0) ? T[r][h] : T[r][CP - 1 - h];
         }
-        __syncthreads();
+        bar_arrive();
 
-        // One order: To = H' Ti (rows in increasing l), A += weight * To, publish To's outer rows / edge columns.
-        // The order loop below is unrolled by two with the roles of T and U swapped, so that the new term is
-        // written where the term before last lived and no register copies are needed at the loop back-edge.
-        auto sweep = [&](const double2 (&Ti)[RP][CP], double2 (&To)[RP][CP], const int k, const bool odd, const bool first, const double s) {
-            const int pr = (k - 1) & 1, pw = k & 1;
-            double2 lo[CP], below[CP];
-#pragma unroll
-            for (int q = 0; q < CP; ++q) {
-                lo[q] = lo_base[pr * lo_par + q * 32];
-                below[q] = up_base[pr * up_par + q * 32];
+        // One row of one order: To[r] = (H' Ti)[r], A[r] += weight * To[r].  dn / up = rows l-1 / l+1, alo / aup =
+        // their coupling weights c_{l-1} E r / c1 and c_l E r / c1; ev1 / ev2 = edge columns of the neighbouring warp.
+        auto do_row = [&](const double2 (&Ti)[RP][CP], double2 (&To)[RP][CP], const int r, const double2 (&dn)[CP],
+                          const double2 (&up)[CP], const double (&alo)[CP], const double (&aup)[CP], const double ll1,
+                          const int pr, const bool odd, const bool first, const double s) {
+            double2 lf1 = shfl_up2(Ti[r][CP - 1]);       // column c0 - 1 from lane - 1
+            double2 rg1 = shfl_dn2(Ti[r][0]);            // column c0 + CP from lane + 1
+            double2 lf2 = z2, rg2 = z2;
+            if (FD == 5) {
+                lf2 = shfl_up2(Ti[r][CP - 2]);
+                rg2 = shfl_dn2(Ti[r][1]);
             }
-            double alo[CP];
-            {
-                const double clo = sm.rowtab[r0][2];
-#pragma unroll
-                for (int q = 0; q < CP; ++q) alo[q] = clo * Eq[q];
-            }
-#pragma unroll
-            for (int r = 0; r < RP; ++r) {
-                const double2 rt = *reinterpret_cast<const double2 *>(&sm.rowtab[r0 + r][0]);
-                const double cup = rt.x, ll1 = rt.y;
-                // columns beyond the warp: zero at a tile edge, else the neighbouring warp's edge column
+            if (NWC > 1) {      // NWC == 1: the tile edge is zero through the weights wl / wrt below
                 double2 ev1 = z2, ev2 = z2;
-                if (NWC > 1 && has_nb) {
+                if (has_nb) {
                     ev1 = sm.edge[pr][nb_warp][nb_side][r][0];
                     if (FD == 5) ev2 = sm.edge[pr][nb_warp][nb_side][r][HW - 1];
                 }
-                double2 lf1 = shfl_up2(Ti[r][CP - 1]);       // column c0 - 1 from lane - 1
-                double2 rg1 = shfl_dn2(Ti[r][0]);            // column c0 + CP from lane + 1
-                double2 lf2 = z2, rg2 = z2;
-                if (FD == 5) {
-                    lf2 = shfl_up2(Ti[r][CP - 2]);
-                    rg2 = shfl_dn2(Ti[r][1]);
-                }
-                if (NWC > 1) {      // NWC == 1: the tile edge is zero through the weights wl / wrt below
-                    if (lane == 0) { lf1 = ev1; lf2 = ev2; }
-                    if (lane == 31) { rg1 = ev1; rg2 = ev2; }
-                }
-#pragma unroll
-                for (int q = 0; q < CP; ++q) {
-                    const double2 f = Ti[r][q];
-                    const double2 m1 = (q > 0) ? Ti[r][q > 0 ? q - 1 : 0] : lf1;
-                    const double2 p1 = (q < CP - 1) ? Ti[r][q < CP - 1 ? q + 1 : 0] : rg1;
-                    const double2 up = (r < RP - 1) ? Ti[r < RP - 1 ? r + 1 : 0][q] : below[q];
-                    const double2 dn = (r > 0) ? Ti[r > 0 ? r - 1 : 0][q] : lo[q];
-                    const double d = fma(ll1, Cq[q], Dq[q]);
-                    const double aup = cup * Eq[q];
-                    // lanes 0 / 31 of a one-warp-wide tile got their own value back from the shuffle: weight 0
-                    double hx, hy;
-                    if (NWC == 1 && q == 0) { hx = fma(wl, m1.x, p1.x); hy = fma(wl, m1.y, p1.y); }
-                    else if (NWC == 1 && q == CP - 1) { hx = fma(wrt, p1.x, m1.x); hy = fma(wrt, p1.y, m1.y); }
-                    else { hx = m1.x + p1.x; hy = m1.y + p1.y; }
-                    if (FD == 5) {
-                        const double2 m2 = (q > 1) ? Ti[r][q > 1 ? q - 2 : 0] : ((q == 1) ? lf1 : lf2);
-                        const double2 p2 = (q < CP - 2) ? Ti[r][q < CP - 2 ? q + 2 : 0] : ((q == CP - 2) ? rg1 : rg2);
-                        double sx, sy;
-                        if (NWC == 1 && q <= 1) { sx = fma(wl, m2.x, p2.x); sy = fma(wl, m2.y, p2.y); }
-                        else if (NWC == 1 && q >= CP - 2) { sx = fma(wrt, p2.x, m2.x); sy = fma(wrt, p2.y, m2.y); }
-                        else { sx = m2.x + p2.x; sy = m2.y + p2.y; }
-                        hx = fma(c2p, sx, hx);
-                        hy = fma(c2p, sy, hy);
-                    }
-                    hx = fma(d, f.x, hx);
-                    hy = fma(d, f.y, hy);
-                    hx = fma(aup, up.x, hx);
-                    hy = fma(aup, up.y, hy);
-                    hx = fma(alo[q], dn.x, hx);
-                    hy = fma(alo[q], dn.y, hy);
-                    if (MASK && !dom[q]) { hx = 0.0; hy = 0.0; }
-                    To[r][q] = make_double2(hx, hy);
-                    alo[q] = aup;                           // c_l E r / c1 couples row l+1 back to row l
-                    // acc += (-i)^k (dt c1)^k / k! * u'_k; s carries the sign: odd k: -+i, even k: -+1
-                    // (order 1 starts the sum from psi itself: A = u_0 + ..., no separate copy)
-                    if (first) { A[r][q].x = fma(s, hy, f.x); A[r][q].y = fma(-s, hx, f.y); }
-                    else if (odd) { A[r][q].x = fma(s, hy, A[r][q].x); A[r][q].y = fma(-s, hx, A[r][q].y); }
-                    else { A[r][q].x = fma(s, hx, A[r][q].x); A[r][q].y = fma(s, hy, A[r][q].y); }
-                }
+                if (lane == 0) { lf1 = ev1; lf2 = ev2; }
+                if (lane == 31) { rg1 = ev1; rg2 = ev2; }
             }
+#pragma unroll
+            for (int q = 0; q < CP; ++q) {
+                const double2 f = Ti[r][q];
+                const double2 m1 = (q > 0) ? Ti[r][q > 0 ? q - 1 : 0] : lf1;
+                const double2 p1 = (q < CP - 1) ? Ti[r][q < CP - 1 ? q + 1 : 0] : rg1;
+                const double d = fma(ll1, Cq[q], Dq[q]);
+                // lanes 0 / 31 of a one-warp-wide tile got their own value back from the shuffle: weight 0
+                double hx, hy;
+                if (NWC == 1 && q == 0) { hx = fma(wl, m1.x, p1.x); hy = fma(wl, m1.y, p1.y); }
+                else if (NWC == 1 && q == CP - 1) { hx = fma(wrt, p1.x, m1.x); hy = fma(wrt, p1.y, m1.y); }
+                else { hx = m1.x + p1.x; hy = m1.y + p1.y; }
+                if (FD == 5) {
+                    const double2 m2 = (q > 1) ? Ti[r][q > 1 ? q - 2 : 0] : ((q == 1) ? lf1 : lf2);
+                    const double2 p2 = (q < CP - 2) ? Ti[r][q < CP - 2 ? q + 2 : 0] : ((q == CP - 2) ? rg1 : rg2);
+                    double sx, sy;
+                    if (NWC == 1 && q <= 1) { sx = fma(wl, m2.x, p2.x); sy = fma(wl, m2.y, p2.y); }
+                    else if (NWC == 1 && q >= CP - 2) { sx = fma(wrt, p2.x, m2.x); sy = fma(wrt, p2.y, m2.y); }
+                    else { sx = m2.x + p2.x; sy = m2.y + p2.y; }
+                    hx = fma(c2p, sx, hx);
+                    hy = fma(c2p, sy, hy);
+                }
+                hx = fma(d, f.x, hx);
+                hy = fma(d, f.y, hy);
+                hx = fma(aup[q], up[q].x, hx);
+                hy = fma(aup[q], up[q].y, hy);
+                hx = fma(alo[q], dn[q].x, hx);
+                hy = fma(alo[q], dn[q].y, hy);
+                if (MASK && !dom[q]) { hx = 0.0; hy = 0.0; }
+                To[r][q] = make_double2(hx, hy);
+                // acc += (-i)^k (dt c1)^k / k! * u'_k; s carries the sign: odd k: -+i, even k: -+1
+                // (order 1 starts the sum from psi itself: A = u_0 + ..., no separate copy)
+                if (first) { A[r][q].x = fma(s, hy, f.x); A[r][q].y = fma(-s, hx, f.y); }
+                else if (odd) { A[r][q].x = fma(s, hy, A[r][q].x); A[r][q].y = fma(-s, hx, A[r][q].y); }
+                else { A[r][q].x = fma(s, hx, A[r][q].x); A[r][q].y = fma(s, hy, A[r][q].y); }
+            }
+        };
+
+        // One order.  The rows that need nothing from other warps (1 and 2 of a one-warp-wide tile) are computed
+        // BEFORE waiting on the barrier that publishes the other warps' rows; then rows 0 and 3, then this warp's
+        // outer rows are published and the barrier is signalled (split arrive / wait).  The order loop below is
+        // unrolled by two with the roles of T and U swapped, so that the new term is written where the term before
+        // last lived and no register copies are needed at the loop back-edge.
+        auto sweep = [&](const double2 (&Ti)[RP][CP], double2 (&To)[RP][CP], const int k, const bool odd, const bool first, const double s) {
+            const int pr = (k - 1) & 1, pw = k & 1;
+            double cup[RP], ll1[RP];
+#pragma unroll
+            for (int r = 0; r < RP; ++r) {
+                const double2 rt = *reinterpret_cast<const double2 *>(&sm.rowtab[r0 + r][0]);
+                cup[r] = rt.x; ll1[r] = rt.y;
+            }
+            double a0[CP], a1[CP], a2[CP], a3[CP], ac[CP];
+#pragma unroll
+            for (int q = 0; q < CP; ++q) { a0[q] = cup[0] * Eq[q]; a1[q] = cup[1] * Eq[q]; a2[q] = cup[2] * Eq[q]; }
+            if (NWC == 1) {
+                do_row(Ti, To, 1, Ti[0], Ti[2], a0, a1, ll1[1], pr, odd, first, s);
+                do_row(Ti, To, 2, Ti[1], Ti[3], a1, a2, ll1[2], pr, odd, first, s);
+            }
+            bar_wait();
+            // every value of the stage was consumed by the arithmetic of order 1: fetch the next item
+            if (TMA && k == 2) fetch_item(item + ncl);
+            double2 lo[CP], below[CP];
+#pragma unroll
+            for (int q = 0; q < CP; ++q) {
+                if (CLUSTER && lo_remote) lo[q] = ld_dsmem2(lo_dsm + (unsigned)((pr * kParStride + q * 32) * sizeof(double2)));
+                else lo[q] = lo_base[pr * lo_par + q * 32];
+                if (CLUSTER && up_remote) below[q] = ld_dsmem2(up_dsm + (unsigned)((pr * kParStride + q * 32) * sizeof(double2)));
+                else below[q] = up_base[pr * up_par + q * 32];
+            }
+            {
+                const double clo = sm.rowtab[r0][2];
+#pragma unroll
+                for (int q = 0; q < CP; ++q) { ac[q] = clo * Eq[q]; a3[q] = cup[3] * Eq[q]; }
+            }
+            do_row(Ti, To, 0, lo, Ti[1], ac, a0, ll1[0], pr, odd, first, s);
+            if (NWC > 1) {
+                do_row(Ti, To, 1, Ti[0], Ti[2], a0, a1, ll1[1], pr, odd, first, s);
+                do_row(Ti, To, 2, Ti[1], Ti[3], a1, a2, ll1[2], pr, odd, first, s);
+            }
+            do_row(Ti, To, 3, Ti[2], below, a2, a3, ll1[3], pr, odd, first, s);
             if (k < order) {
 #pragma unroll
                 for (int q = 0; q < CP; ++q) {
@@ -328,14 +409,7 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                             sm.edge[pw][warp][my_side][r][h] = (lane == 0) ? To[r][h] : To[r][CP - 1 - h];
                 }
             }
-            __syncthreads();
-            // every value of the stage has been consumed by the arithmetic of order 1: fetch the next item
-            if (TMA && k == 1 && threadIdx.x == 0 && item + (int)gridDim.x < n_items) {
-                const int ni = item + gridDim.x, nb = ni / n_tiles, nt = ni - nb * n_tiles;
-                fence_proxy_async_smem();
-                mbar_expect_tx(&sm.mbar, kStageBytes);
-                tma_load_3d(sm.stage, &tmap, 0, rp_start(nt, W, H, N, WT) >> 3, nb * L, &sm.mbar);
-            }
+            bar_arrive();
         };
 
         double2 U[RP][CP];
@@ -352,20 +426,21 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
             sk = sk * (kappa * kRpInvK[k]);
             sweep(U, T, k, false, false, (k & 2) ? -sk : sk);
         }
+        // the barrier signalled by the last order is waited for before the next item publishes (or at the end)
 
         // ---- psi(t + dt): interior columns of the tile straight from registers ---------------------------------
         {
             const int lo_c = t * W - start;                  // first interior column (tile coordinates)
             int wint = N - t * W;
             if (wint > W) wint = W;
-            double2 *dst_g = out + (size_t)b * L * N + start + c0;
+            double2 *dst_g = out + ((size_t)b * L + rbase) * N + start + c0;
 #pragma unroll
             for (int q = 0; q < CP; q += 2) {
                 const int c = c0 + q;
                 const bool in0 = c >= lo_c && c < lo_c + wint, in1 = c + 1 >= lo_c && c + 1 < lo_c + wint;
 #pragma unroll
                 for (int r = 0; r < RP; ++r) {
-                    if (r0 + r >= L) continue;
+                    if (gr0 + r >= L) continue;
                     double2 *p = dst_g + (size_t)(r0 + r) * N + q;
                     if (al32) {
                         if (in0) stg256(p, A[r][q], A[r][q + 1]);      // interior bounds are even: in0 == in1
@@ -377,6 +452,7 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
             }
         }
     }
+    if (armed) bar_wait();     // (cluster: no CTA may exit while a neighbour can still read its shared memory)
 }
 
 // ------------------------------------------------------------------------------------------------------
@@ -388,8 +464,11 @@ constexpr RpVariant kRpVariants[] = {
     {4, 1, 1, 8}, {4, 2, 1, 4}, {4, 4, 1, 2}, {4, 8, 1, 1},      // 128-column tiles, 16 points per thread
     {2, 1, 2, 8}, {2, 2, 2, 4}, {2, 4, 2, 2}, {2, 8, 2, 1},      // 128-column tiles,  8 points per thread
     {2, 4, 4, 1},                                                // 256-column tile, 8 points per thread, n_l <= 16
+    {4, 4, 2, 1},                                                // 256-column tile, 16 points per thread, n_l <= 16
 };
 constexpr int kNumRpVariants = sizeof(kRpVariants) / sizeof(kRpVariants[0]);
+// the instantiations that also exist as cluster kernels (16 rows per CTA)
+constexpr bool rp_clusterable(int variant) { return variant == 2 || variant == 9; }
 
 inline int rp_init_tables() {
     double h[65];
@@ -398,7 +477,7 @@ inline int rp_init_tables() {
     return cudaMemcpyToSymbol(kRpInvK, h, sizeof(h)) == cudaSuccess ? TDSE_OK : TDSE_ERR_CUDA;
 }
 
-struct RpPlan { int ok, variant, tma, W, H, WT, n_tiles, n_items, grid, threads; };
+struct RpPlan { int ok, variant, tma, cl, W, H, WT, n_tiles, n_items, grid, threads; };   // cl: CTAs per cluster (1: none)
 
 // use_tma: -1 heuristic, 0 never, 1 whenever the layout allows it (n_r % 8 == 0, a full tile, 4-column patches)
 inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant, int use_tma) {
@@ -408,8 +487,16 @@ inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant
     for (int i = 0; i < kNumRpVariants; ++i) {
         if (force_variant >= 0 && i != force_variant) continue;
         const RpVariant &v = kRpVariants[i];
-        const int rows = kRpRows * v.nwr, WT = 32 * v.cp * v.nwc;
-        if (rows < g.n_l || v.cp < hw) continue;
+        const int WT = 32 * v.cp * v.nwc;
+        int rows = kRpRows * v.nwr, cl = 1;
+        if (rows < g.n_l) {
+            // more rows than one CTA holds: split them over a cluster of 2, 4 or 8 CTAs (16-row CTAs only)
+            if (!rp_clusterable(i)) continue;
+            while (cl < 8 && rows * cl < g.n_l) cl *= 2;
+            if (rows * cl < g.n_l) continue;
+            rows *= cl;
+        }
+        if (v.cp < hw) continue;
         if (rows >= 2 * g.n_l && v.nwr > 1) continue;      // more than half of the rows would be padding
         for (int tma = 0; tma <= 1; ++tma) {
             if (tma && (use_tma == 0 || v.cp != 4 || (g.n_r & 7) || g.n_r <= WT)) continue;
@@ -418,7 +505,7 @@ inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant
             if (tma) H = (H + 7) & ~7;                      // tile starts on a 128-byte column group
             else if ((g.n_r & 1) == 0) H = (H + 1) & ~1;    // even halo: every patch row starts 32-byte aligned
             RpPlan p{};
-            p.variant = i; p.tma = tma; p.H = H; p.WT = WT; p.threads = 32 * v.nwr * v.nwc;
+            p.variant = i; p.tma = tma; p.cl = cl; p.H = H; p.WT = WT; p.threads = 32 * v.nwr * v.nwc;
             if (g.n_r <= WT) { p.W = g.n_r; p.n_tiles = 1; }
             else {
                 p.W = WT - 2 * H;
@@ -426,15 +513,19 @@ inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant
                 p.n_tiles = (g.n_r + p.W - 1) / p.W;
             }
             p.n_items = p.n_tiles * g.batch;
-            p.grid = std::min(p.n_items, n_sm * v.minb);
+            p.grid = std::min(p.n_items, n_sm * v.minb / cl);       // clusters (= CTAs when cl == 1)
             // a grid that is a multiple of n_tiles keeps every CTA on one radial tile (coefficients loaded once)
             if (p.n_tiles * 4 <= p.grid) p.grid = p.grid / p.n_tiles * p.n_tiles;
+            p.grid *= cl;
             p.ok = 1;
             // cost: columns computed in total; 8-point patches measured 1.5x slower per column than 16-point
             // patches (twice the exchange per point, spills at 128 registers); the asynchronous tile fetch hides
             // the load latency of the next item
             double cost = (double)p.n_tiles * WT * rows;
             if (force_variant < 0 && v.cp == 2) cost *= 1.5;
+            // tiles wider than one warp exchange edge columns through shared memory and cannot start an order
+            // before the barrier: measured 1.3-1.4x slower per column
+            if (force_variant < 0 && v.nwc > 1) cost *= 1.4;
             if (tma) cost *= 0.85;
             if (!best.ok || cost < best_cost) { best = p; best_cost = cost; }
         }
@@ -477,38 +568,56 @@ inline const CUtensorMap *rp_tensor_map(const void *base, int n_r, int total_row
     return &(cache[key] = m);
 }
 
-template <int FD, int CP, int NWR, int NWC, int MINB>
+template <class K>
+inline int rp_launch_kernel(K kern, bool *attr_set, int smem, const RpPlan &p, cudaStream_t s, const GridDev &g,
+                            const double2 *in, double2 *out, const double *ef, const double *dtp, int order,
+                            const CUtensorMap &tm) {
+    if (!*attr_set) {
+        if (cudaFuncSetAttribute((const void *)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
+            return TDSE_ERR_CUDA;
+        *attr_set = true;
+    }
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(p.grid); cfg.blockDim = dim3(p.threads); cfg.dynamicSmemBytes = smem; cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = p.cl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = (p.cl > 1) ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, g, in, out, ef, dtp, order, p.W, p.H, p.n_tiles, p.n_items, tm) == cudaSuccess
+               ? TDSE_OK : TDSE_ERR_CUDA;
+}
+
+template <int FD, int CP, int NWR, int NWC, int MINB, bool CLUSTERABLE>
 inline int rp_launch_one(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
                          const double *dtp, int order, cudaStream_t s) {
     if (FD == 5 && CP < 2) return TDSE_ERR_UNSUPPORTED;
     const bool mask = g.n_r < 32 * CP * NWC;
-    const int mode = (p.tma && CP == 4) ? 2 : (mask ? 1 : 0);
-    auto set_attr = [](const void *fn, int smem) {
-        return cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) == cudaSuccess;
-    };
-    static bool attr_set[3] = {false, false, false};
+    constexpr bool kTma = (CP == 4);
+    static bool attr_set[5] = {false, false, false, false, false};
     CUtensorMap dummy{};
-    if (mode == 2) {
-        if (CP != 4) return TDSE_ERR_UNSUPPORTED;
-        constexpr bool kTma = (CP == 4);
-        auto kern = taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, kTma>;
-        const int smem = (int)sizeof(RpSmem<FD, CP, NWR, NWC, kTma>) + 0;
-        if (!attr_set[2]) { if (!set_attr((const void *)kern, smem)) return TDSE_ERR_CUDA; attr_set[2] = true; }
-        const CUtensorMap *tm = rp_tensor_map(in, g.n_r, g.batch * g.n_l, kRpRows * NWR, 32 * CP * NWC);
+    const CUtensorMap *tm = &dummy;
+    if (p.tma) {
+        if (!kTma || mask) return TDSE_ERR_UNSUPPORTED;
+        tm = rp_tensor_map(in, g.n_r, g.batch * g.n_l, kRpRows * NWR, 32 * CP * NWC);
         if (!tm) return TDSE_ERR_CUDA;
-        kern<<<p.grid, p.threads, smem, s>>>(g, in, out, ef, dtp, order, p.W, p.H, p.n_tiles, p.n_items, *tm);
-    } else if (mode == 1) {
-        auto kern = taylor_rp_kernel<FD, CP, NWR, NWC, true, MINB, false>;
-        const int smem = (int)sizeof(RpSmem<FD, CP, NWR, NWC, false>) + 0;
-        if (!attr_set[1]) { if (!set_attr((const void *)kern, smem)) return TDSE_ERR_CUDA; attr_set[1] = true; }
-        kern<<<p.grid, p.threads, smem, s>>>(g, in, out, ef, dtp, order, p.W, p.H, p.n_tiles, p.n_items, dummy);
-    } else {
-        auto kern = taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false>;
-        const int smem = (int)sizeof(RpSmem<FD, CP, NWR, NWC, false>) + 0;
-        if (!attr_set[0]) { if (!set_attr((const void *)kern, smem)) return TDSE_ERR_CUDA; attr_set[0] = true; }
-        kern<<<p.grid, p.threads, smem, s>>>(g, in, out, ef, dtp, order, p.W, p.H, p.n_tiles, p.n_items, dummy);
     }
-    return cudaGetLastError() == cudaSuccess ? TDSE_OK : TDSE_ERR_CUDA;
+    if (p.cl > 1) {
+        if (!CLUSTERABLE || mask) return TDSE_ERR_UNSUPPORTED;
+        constexpr bool kCl = CLUSTERABLE;
+        if (p.tma)
+            return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, kTma, kCl>, &attr_set[3],
+                                    (int)sizeof(RpSmem<FD, CP, NWR, NWC, kTma>), p, s, g, in, out, ef, dtp, order, *tm);
+        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, kCl>, &attr_set[4],
+                                (int)sizeof(RpSmem<FD, CP, NWR, NWC, false>), p, s, g, in, out, ef, dtp, order, *tm);
+    }
+    if (p.tma)
+        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, kTma, false>, &attr_set[2],
+                                (int)sizeof(RpSmem<FD, CP, NWR, NWC, kTma>), p, s, g, in, out, ef, dtp, order, *tm);
+    if (mask)
+        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, true, MINB, false, false>, &attr_set[1],
+                                (int)sizeof(RpSmem<FD, CP, NWR, NWC, false>), p, s, g, in, out, ef, dtp, order, *tm);
+    return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, false>, &attr_set[0],
+                            (int)sizeof(RpSmem<FD, CP, NWR, NWC, false>), p, s, g, in, out, ef, dtp, order, *tm);
 }
 
 inline int launch_taylor_rp(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
@@ -516,8 +625,8 @@ inline int launch_taylor_rp(const GridDev &g, const RpPlan &p, const double2 *in
     if (!p.ok) return TDSE_ERR_UNSUPPORTED;
 #define TDSE_RP_CASE(I, CP, NWR, NWC, MINB)                                                                  \
     case I:                                                                                                  \
-        return (g.fd == 3) ? rp_launch_one<3, CP, NWR, NWC, MINB>(g, p, in, out, ef, dtp, order, s)          \
-                           : rp_launch_one<5, CP, NWR, NWC, MINB>(g, p, in, out, ef, dtp, order, s);
+        return (g.fd == 3) ? rp_launch_one<3, CP, NWR, NWC, MINB, rp_clusterable(I)>(g, p, in, out, ef, dtp, order, s)  \
+                           : rp_launch_one<5, CP, NWR, NWC, MINB, rp_clusterable(I)>(g, p, in, out, ef, dtp, order, s);
     switch (p.variant) {
         TDSE_RP_CASE(0, 4, 1, 1, 8)
         TDSE_RP_CASE(1, 4, 2, 1, 4)
@@ -528,6 +637,7 @@ inline int launch_taylor_rp(const GridDev &g, const RpPlan &p, const double2 *in
         TDSE_RP_CASE(6, 2, 4, 2, 2)
         TDSE_RP_CASE(7, 2, 8, 2, 1)
         TDSE_RP_CASE(8, 2, 4, 4, 1)
+        TDSE_RP_CASE(9, 4, 4, 2, 1)
     }
 #undef TDSE_RP_CASE
     return TDSE_ERR_UNSUPPORTED;

@@ -269,6 +269,13 @@ RP_CASES = [
     (1000, 0.1, 24, 5, 1, 4, 8, 0, -1, 1),       # 24 of 32 rows
     (700, 0.1, 4, 3, 300, 6, 6, 0, 4, 1),        # more work items than resident CTAs: persistent loop
     (3000, 0.1, 16, 5, 40, 3, 5, 0, -1, 1),      # several items per CTA, 5-point
+    (304, 0.1, 64, 5, 1, 10, 6, 0, -1, 1),       # CFG3 rows: cluster of 4 CTAs, l+-1 rows through DSMEM
+    (300, 0.1, 64, 5, 2, 10, 6, 3, -1, 1),       # same, batched, n_r not a multiple of 8 (no TMA)
+    (264, 0.1, 128, 3, 1, 6, 6, 0, -1, 1),       # CFG4 rows: cluster of 8 CTAs
+    (400, 0.1, 40, 3, 3, 5, 7, 0, -1, 0),        # 40 rows in a cluster of 4 (24 padding rows), eager, odd steps
+    (2000, 0.1, 33, 3, 20, 4, 4, 0, -1, 1),      # more clusters than fit at once: persistent loop over items
+    (2000, 0.1, 16, 3, 2, 6, 8, 0, 9, 1),        # 256-column tiles of 16-point patches (edge exchange between warps)
+    (1000, 0.1, 64, 5, 1, 10, 4, 0, 9, 1),       # the same in a cluster of 4 (CFG3 layout)
 ]
 
 
@@ -286,7 +293,7 @@ def test_taylor_register_patch_parity(B, case, tma):
     psi0 = wl.populated_state(c)
     opts = {"taylor_block": 4, "use_graph": use_graph, "taylor_rp_variant": variant, "taylor_rp_tma": tma}
     h, got, ref, gobs, robs = run_pair_fixed(B, c, "taylor", nsteps, psi0, t0, dt, obs_every, [(0, 0)], opts, order=order)
-    tma_applies = bool(tma) and n_r % 8 == 0 and n_r > 128 and variant in (-1, 0, 1, 2, 3)
+    tma_applies = bool(tma) and n_r % 8 == 0 and n_r > 128 and variant in (-1, 0, 1, 2, 3, 9)
     assert h.taylor_kernel() == (4 if tma_applies else 3)
     check_fixed(got, ref, gobs, robs)
     for b in range(batch):
