@@ -265,6 +265,14 @@ def run_own(args):
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": traffic, "kernel": kname, "launches": n_dom, "us_per_launch": ms * 1e3 / n_dom,
                 "algorithmic_bytes_per_launch": bytes_step * K / n_dom, "peak_source": peak_src}
+    if blocked:
+        # second roof of the all-orders-in-one-pass kernels: FP64 issue.  Algorithmic FP64
+        # instructions per point-update of the scaled operator H/c1 (no halo redundancy counted) against the
+        # measured 18.2 T FP64 instr/s of this B200 (64 lanes/clk/SM x 148 SMs x 1.93 GHz).
+        fp64_per_update = 12.25 if c["fd_order"] == 3 else 16.25
+        alu_rate = pts * order * fp64_per_update * K / (ms * 1e-3)
+        roofline["alu"] = {"fp64_instr_per_point_update": fp64_per_update, "achieved_instr_per_s": alu_rate,
+                           "peak_instr_per_s": 18.2e12, "frac": alu_rate / 18.2e12}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
