@@ -350,7 +350,15 @@ def extra_measurements(binding, torch, stream):
             pts = c["batch"] * c["n_l"] * c["n_r"]
             out[f"step_{name}"] = {"propagator": c["propagator"], "us_per_step": ms * 1e3 / nsteps, "dt_eff": dt,
                                    "gpoint_updates_per_s": pts * n_h * nsteps / (ms * 1e-3) / 1e9,
-                                   "blocked": h.taylor_was_blocked() if c["propagator"] == "taylor" else None}
+                                   "blocked": h.taylor_was_blocked() if c["propagator"] == "taylor" else None,
+                                   "observables_every_step": name in ("cfg1", "cfg3")}
+            if c["propagator"] == "lanczos":
+                # one fused pass per Krylov vector: 32 + (K-2) x 80 + 64 B/point, combine (K+1) x 16
+                K = c["krylov_dim"]
+                bpp = 32.0 + (K - 2) * 80.0 + 64.0 + (K + 1) * 16.0
+                gbs = bpp * pts * nsteps / (ms * 1e-3) / 1e9
+                out[f"step_{name}"].update({"algorithmic_bytes_per_point": bpp, "gbs_algorithmic": gbs,
+                                            "frac_of_hbm_peak": gbs / peak})
             h.close()
     return out
 

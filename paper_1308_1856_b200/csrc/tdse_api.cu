@@ -363,27 +363,22 @@ int enqueue_lanczos_block(tdse_handle *h, int K, int order, int n, int obs, cuda
     double2 *basis = h->d_basis;
     for (int i = 0; i < n; ++i) {
         const double *ef = h->d_etab + (size_t)i * B;
-        OpNorm on{}; on.psi = psi; on.nrm = h->d_nrm; on.inv = h->d_inv; on.m_used = h->d_m; on.K = K;
-        RC(launch_ew(h, on, s));
+        // one fused pass per Krylov vector: v_p formed on load, g_p = H v_p, <v_p|g_p> and ||v_p||^2 reduced
         for (int p = 0; p < K; ++p) {
-            double2 *q_p = basis + (size_t)p * h->n_state;
-            EpiLanczosA a{};
-            a.in = (p == 0) ? psi : wbuf[p & 1];
-            a.ef = ef; a.inv = h->d_inv; a.m_used = h->d_m; a.p = p; a.K = K;
-            a.q_out = q_p; a.w_out = (p < K - 1) ? wbuf[(p + 1) & 1] : nullptr; a.alpha = h->d_alpha;
+            EpiLanczosF a{};
+            a.psi = psi; a.g_in = wbuf[(p + 1) & 1];
+            a.v1 = (p >= 1) ? basis + (size_t)(p - 1) * h->n_state : nullptr;
+            a.v2 = (p >= 2) ? basis + (size_t)(p - 2) * h->n_state : nullptr;
+            a.v_out = basis + (size_t)p * h->n_state;
+            a.g_out = (p < K - 1) ? wbuf[p & 1] : nullptr;
+            a.ef = ef; a.alpha = h->d_alpha; a.beta = h->d_beta; a.sc = h->d_inv; a.nrm = h->d_nrm; a.m_used = h->d_m;
+            a.p = p; a.K = K; a.tol = h->beta_tol;
             RC(launch_tile(h, a, s));
-            if (p < K - 1) {
-                OpLanczosB bb{};
-                bb.w = wbuf[(p + 1) & 1]; bb.q = q_p; bb.q_prev = (p > 0) ? q_p - h->n_state : nullptr;
-                bb.alpha = h->d_alpha; bb.beta = h->d_beta; bb.inv = h->d_inv; bb.m_used = h->d_m;
-                bb.p = p; bb.K = K; bb.tol = h->beta_tol;
-                RC(launch_ew(h, bb, s));
-            }
         }
         small_exp_kernel<<<B, 32, 0, s>>>(h->d_alpha, h->d_beta, h->d_m, &h->d_ctl->dt, K, order, h->d_coef, h->d_nsub);
         count(h);
         OpCombine oc{};
-        oc.psi = psi; oc.q = basis; oc.q_stride = h->n_state; oc.coef = h->d_coef; oc.nrm = h->d_nrm;
+        oc.psi = psi; oc.q = basis; oc.q_stride = h->n_state; oc.coef = h->d_coef; oc.nrm = h->d_nrm; oc.sc = h->d_inv;
         oc.m_used = h->d_m; oc.K = K;
         RC(launch_ew(h, oc, s));
         if (obs) RC(enqueue_obs(h, psi, i, 1, 0, 0.0, h->d_rows, s));
@@ -707,7 +702,7 @@ int tdse_step_lanczos(tdse_handle *h, int K, int order, double t0, double dt, lo
         CU(cudaMalloc(&h->d_alpha, sizeof(double) * B * K));
         CU(cudaMalloc(&h->d_beta, sizeof(double) * B * K));
         CU(cudaMalloc(&h->d_nrm, sizeof(double) * B));
-        CU(cudaMalloc(&h->d_inv, sizeof(double) * B));
+        CU(cudaMalloc(&h->d_inv, sizeof(double) * B * K));
         CU(cudaMalloc(&h->d_coef, sizeof(double2) * B * K));
         CU(cudaMalloc(&h->d_m, sizeof(int) * B));
         CU(cudaMalloc(&h->d_nsub, sizeof(int) * B));

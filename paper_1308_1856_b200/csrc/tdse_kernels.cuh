@@ -43,7 +43,7 @@ __device__ __forceinline__ double2 h_point(const GridDev &g, double d, double er
 // Epi supplies: NRED, SCALED; begin(); skip_all(); member_active(b); input(); in_scale(b); efield(b);
 // point(b,l,j,idx,f,h,red); finish_member(b,s); finish_all().
 template <int FD, class Epi>
-__global__ void __launch_bounds__(256, 3) tile_kernel(GridDev g, Epi epi_in, RedCtx rc) {
+__global__ void __launch_bounds__(256, Epi::MINB) tile_kernel(GridDev g, Epi epi_in, RedCtx rc) {
     using T = Tile<FD>;
     __shared__ double2 tile[T::ELEMS];
     __shared__ double red_s[(Epi::NRED > 0 ? Epi::NRED : 1) * (T::NT / 32)];
@@ -59,6 +59,7 @@ __global__ void __launch_bounds__(256, 3) tile_kernel(GridDev g, Epi epi_in, Red
     for (int r = 0; r < (Epi::NRED > 0 ? Epi::NRED : 1); ++r) red[r] = 0.0;
 
     if (epi.member_active(b)) {
+        epi.prepare(b);
         const double2 *base = epi.input() + (size_t)b * g.n_l * g.n_r;
         const double sc = Epi::SCALED ? epi.in_scale(b) : 1.0;
         // optional second source: the tile holds in + c2in * in2 (a stage vector formed while loading)
@@ -73,8 +74,12 @@ __global__ void __launch_bounds__(256, 3) tile_kernel(GridDev g, Epi epi_in, Red
                 const int l = l0 - 1 + rr, j = j0 - T::HW + cc;
                 double2 v = make_double2(0.0, 0.0);
                 if (l >= 0 && l < g.n_l && j >= 0 && j < g.n_r) {
-                    v = __ldg(base + (size_t)l * g.n_r + j);
-                    if (Epi::TWO_IN) v = caxpy_r(c2in, __ldg(base2 + (size_t)l * g.n_r + j), v);
+                    if (Epi::CUSTOM_LOAD) {
+                        v = epi.load(((size_t)b * g.n_l + l) * g.n_r + j);      // a vector formed from several arrays
+                    } else {
+                        v = __ldg(base + (size_t)l * g.n_r + j);
+                        if (Epi::TWO_IN) v = caxpy_r(c2in, __ldg(base2 + (size_t)l * g.n_r + j), v);
+                    }
                 }
                 if (Epi::SCALED) { v.x *= sc; v.y *= sc; }
                 tile[i] = v;
@@ -121,6 +126,11 @@ struct EpiBase {
     static constexpr int NRED = 0;
     static constexpr bool SCALED = false;
     static constexpr bool TWO_IN = false;
+    static constexpr bool CUSTOM_LOAD = false;
+    static constexpr int MINB = 3;              // CTAs per SM the register budget is set for
+    __device__ __forceinline__ void prepare(int) {}
+    __device__ __forceinline__ double2 load(size_t) const { return make_double2(0.0, 0.0); }
+
     __device__ __forceinline__ const double2 *input2() const { return nullptr; }
     __device__ __forceinline__ double in2_coef() const { return 0.0; }
     __device__ __forceinline__ void begin() {}
@@ -258,23 +268,66 @@ struct EpiRK : EpiBase {
     }
 };
 
-// Lanczos matvec with the alpha reduction fused (LanczosLoop1): q_p = in * inv_b; w = H q_p; alpha_p = Re<q_p|w>.
-struct EpiLanczosA : EpiBase {
-    static constexpr int NRED = 1;
-    static constexpr bool SCALED = true;
-    const double2 *in; const double *ef; const double *inv; const int *m_used; int p, K;
-    double2 *q_out; double2 *w_out; double *alpha;
-    __device__ __forceinline__ bool member_active(int b) const { return m_used[b] > p; }
-    __device__ __forceinline__ const double2 *input() const { return in; }
-    __device__ __forceinline__ double in_scale(int b) const { return inv[b]; }
+// One Lanczos vector per PASS (App. B in reading R-G16; the paper uses 3 kernels per vector).
+// Stored vectors are v_0 = psi and v_p = w_{p-1} (the orthogonalised, UNnormalised residual, norm beta_{p-1});
+// q_p = s_p v_p with s_0 = 1/||psi||, s_p = 1/beta_{p-1}.  Pass p forms, while loading its tile,
+//     v_p = s_{p-1} g_{p-1} - alpha_{p-1} q_{p-1} - beta_{p-2} q_{p-2}          (g_{p-1} = H v_{p-1}, so s g = H q)
+// applies H (g_p = H v_p, linear, so the normalisation can wait), writes v_p and g_p, and reduces BOTH
+// <v_p|g_p> and ||v_p||^2 in the same pass; the last CTA turns them into beta_{p-1} = ||v_p||, s_p, the
+// breakdown flag and alpha_p = s_p^2 Re<v_p|g_p> = Re<q_p|H q_p>.  80 B/point/vector in one kernel instead of
+// 112 B in two; the norm of psi is pass 0's second reduction.
+struct EpiLanczosF : EpiBase {
+    static constexpr int NRED = 2;
+    static constexpr bool CUSTOM_LOAD = true;
+#ifndef TDSE_LZ_MINB
+#define TDSE_LZ_MINB 5
+#endif
+    static constexpr int MINB = TDSE_LZ_MINB;   // latency-bound on HBM: measured 2295 / 1923 / 1776 us per CFG4 step at 3 / 4 / 5
+    const double2 *psi, *g_in, *v1, *v2;       // psi (p = 0); g_{p-1}, v_{p-1}, v_{p-2}
+    double2 *v_out, *g_out;
+    const double *ef; double *alpha, *beta, *sc, *nrm; int *m_used; int p, K; double tol;
+    double s1, a1, b2s2, sc_prev;               // per-member scalars of the load (set by prepare)
+    __device__ __forceinline__ bool member_active(int b) const { return p == 0 || m_used[b] > p; }
+    __device__ __forceinline__ const double2 *input() const { return psi; }
     __device__ __forceinline__ double efield(int b) const { return __ldg(ef + b); }
-    __device__ __forceinline__ void point(int, int, int, size_t idx, double2 f, double2 h, double *red) {
-        q_out[idx] = f;
-        if (w_out) w_out[idx] = h;
-        red[0] += f.x * h.x + f.y * h.y;
+    __device__ __forceinline__ void prepare(int b) {
+        s1 = a1 = b2s2 = 0.0;
+        if (p >= 1) { s1 = sc[b * K + p - 1]; a1 = alpha[b * K + p - 1]; }
+        sc_prev = 0.0;
+        if (p >= 2) { b2s2 = beta[b * K + p - 2]; sc_prev = sc[b * K + p - 2]; }
     }
-    __device__ __forceinline__ void finish_member(int b, const double *s) { if (m_used[b] > p) alpha[b * K + p] = s[0]; }
+    // raw values of (g_{p-1} | psi), v_{p-1}, v_{p-2} at one point -> v_p
+    __device__ __forceinline__ double2 combine(double2 g, double2 x1, double2 x2) const {
+        if (p == 0) return g;
+        double2 w = make_double2(g.x * s1, g.y * s1);                            // H q_{p-1}
+        w = caxpy_r(-a1, make_double2(x1.x * s1, x1.y * s1), w);                 // - alpha_{p-1} q_{p-1}
+        if (p >= 2) w = caxpy_r(-b2s2, make_double2(x2.x * sc_prev, x2.y * sc_prev), w);   // - beta_{p-2} q_{p-2}
+        return w;
+    }
+    __device__ __forceinline__ double2 load(size_t idx) const {
+        const double2 z = make_double2(0.0, 0.0);
+        return combine(__ldg((p == 0 ? psi : g_in) + idx), p >= 1 ? __ldg(v1 + idx) : z, p >= 2 ? __ldg(v2 + idx) : z);
+    }
+    __device__ __forceinline__ void point(int, int, int, size_t idx, double2 f, double2 h, double *red) {
+        v_out[idx] = f;
+        if (g_out) g_out[idx] = h;
+        red[0] += f.x * h.x + f.y * h.y;
+        red[1] += f.x * f.x + f.y * f.y;
+    }
+    __device__ __forceinline__ void finish_member(int b, const double *s) {
+        if (p > 0 && m_used[b] <= p) return;
+        const double n = sqrt(s[1]);
+        const double sp = 1.0 / n;
+        if (p == 0) { nrm[b] = n; m_used[b] = K; }
+        else {
+            beta[b * K + p - 1] = n;
+            if (n < tol) { m_used[b] = p; return; }   // breakdown (R-G17): vectors 0 .. p-1 span the space
+        }
+        sc[b * K + p] = sp;
+        alpha[b * K + p] = (s[0] * sp) * sp;
+    }
 };
+
 
 // ------------------------------------------------------------------------------------------------------
 // Element-wise kernels with optional fused reduction.  grid = (chunks, 1, batch); a CTA handles EW_CHUNK
@@ -315,54 +368,19 @@ struct OpBase {
     __device__ __forceinline__ void finish_all() {}
 };
 
-// ||F|| at the start of a Lanczos step: nrm_b, inv_b = 1/nrm_b, m_b = K.
-struct OpNorm : OpBase {
-    static constexpr int NRED = 1;
-    const double2 *psi; double *nrm, *inv; int *m_used; int K;
-    __device__ __forceinline__ void point(int, size_t idx, double *red) {
-        const double2 v = psi[idx];
-        red[0] += v.x * v.x + v.y * v.y;
-    }
-    __device__ __forceinline__ void finish_member(int b, const double *s) {
-        const double n = sqrt(s[0]);
-        nrm[b] = n; inv[b] = 1.0 / n; m_used[b] = K;
-    }
-};
-
-// Orthogonalisation and beta (LanczosLoop2 + NormKrylov): w -= alpha_p q_p + beta_{p-1} q_{p-1};
-// beta_p = ||w||; breakdown if beta_p < tol (R-G17); inv_b = 1/beta_p scales the next tile load.
-struct OpLanczosB : OpBase {
-    static constexpr int NRED = 1;
-    double2 *w; const double2 *q, *q_prev; const double *alpha; double *beta; double *inv; int *m_used;
-    int p, K; double tol;
-    __device__ __forceinline__ bool member_active(int b) const { return m_used[b] > p; }
-    __device__ __forceinline__ void point(int b, size_t idx, double *red) {
-        double2 v = w[idx];
-        v = caxpy_r(-alpha[b * K + p], q[idx], v);
-        if (p > 0) v = caxpy_r(-beta[b * K + p - 1], q_prev[idx], v);
-        w[idx] = v;
-        red[0] += v.x * v.x + v.y * v.y;
-    }
-    __device__ __forceinline__ void finish_member(int b, const double *s) {
-        if (m_used[b] <= p) return;
-        const double bt = sqrt(s[0]);
-        beta[b * K + p] = bt;
-        if (bt < tol) m_used[b] = p + 1;
-        inv[b] = 1.0 / bt;
-    }
-};
-
 // F(t+dt) = ||F|| sum_{p<m} c_p q_p  (Taylor2)
 struct OpCombine : OpBase {
-    double2 *psi; const double2 *q; size_t q_stride; const double2 *coef; const double *nrm; const int *m_used; int K;
+    double2 *psi; const double2 *q; size_t q_stride; const double2 *coef; const double *nrm, *sc; const int *m_used; int K;
     __device__ __forceinline__ void point(int b, size_t idx, double *) {
         const int m = m_used[b];
         const double n = nrm[b];
         double2 acc = make_double2(0.0, 0.0);
         for (int p = 0; p < m; ++p) {
             const double2 c = coef[b * K + p];
+            const double sp = sc[b * K + p];                    // q_p = s_p v_p
             const double ar = n * c.x, ai = n * c.y;
-            const double2 x = q[(size_t)p * q_stride + idx];
+            double2 x = q[(size_t)p * q_stride + idx];
+            x.x *= sp; x.y *= sp;
             acc.x += ar * x.x - ai * x.y;
             acc.y += ar * x.y + ai * x.x;
         }
