@@ -76,7 +76,7 @@ struct tdse_handle {
     unsigned int *d_counter = nullptr;
     // observables
     int n_states = 0; double *d_phi = nullptr; int *d_lstate = nullptr;
-    double *d_obs_partials = nullptr; double2 *d_amp = nullptr;
+    double *d_obs_partials = nullptr; double2 *d_amp = nullptr; unsigned int *d_obs_counters = nullptr;
     double *d_rows = nullptr; size_t rows_cap = 0; long log_rows = 0; double *d_row_direct = nullptr;
     // rk45 logs
     double *d_dtlog = nullptr, *d_errlog = nullptr, *d_replay = nullptr; long log_cap = 0, replay_cap = 0;
@@ -156,22 +156,24 @@ int launch_ew(tdse_handle *h, const Op &op, cudaStream_t s) {
     return TDSE_OK;
 }
 
-int obs_chunks(const tdse_handle *h) { return (h->grid.n_r + 255) / 256; }
+int obs_chunks_r(const tdse_handle *h) { return (h->grid.n_r + 255) / 256; }
+int obs_chunks_l(const tdse_handle *h) { return (h->grid.n_l + kObsRows - 1) / kObsRows; }
+int obs_chunks(const tdse_handle *h) { return obs_chunks_r(h) * obs_chunks_l(h); }
 
 // Observable kernels for the state `psi`; logged row (predicated on the device step counter) or direct.
 int enqueue_obs(tdse_handle *h, const double2 *psi, int step_off, int predicated, int use_direct, double t_direct,
                 double *rows, cudaStream_t s) {
     const int B = h->grid.batch;
-    obs_main_kernel<<<dim3(obs_chunks(h), B), 256, 0, s>>>(h->gd, psi, h->d_ctl, step_off, predicated,
-                                                             h->d_obs_partials);
-    count(h);
-    if (h->n_states > 0) {
-        obs_pop_kernel<<<dim3(h->n_states, B), 128, 0, s>>>(h->gd, psi, h->d_phi, h->d_lstate, h->n_states, h->d_ctl,
-                                                             step_off, predicated, h->d_amp);
+    if (obs_chunks(h) + h->n_states <= 8) {          // small grid: one CTA per member, no cross-CTA hand-over
+        obs_small_kernel<<<B, 256, 0, s>>>(h->gd, psi, h->d_phi, h->d_lstate, h->n_states, h->d_pulse, h->d_ctl, step_off,
+                                           predicated, use_direct, t_direct, rows);
         count(h);
+        CU(cudaGetLastError());
+        return TDSE_OK;
     }
-    obs_final_kernel<<<B, 128, 0, s>>>(h->gd, h->d_obs_partials, obs_chunks(h), h->d_amp, h->n_states, h->d_pulse,
-                                       h->d_ctl, step_off, predicated, use_direct, t_direct, rows);
+    obs_kernel<<<dim3(obs_chunks_r(h), B, obs_chunks_l(h) + h->n_states), 256, 0, s>>>(
+        h->gd, psi, h->d_phi, h->d_lstate, h->n_states, h->d_pulse, h->d_ctl, step_off, predicated, use_direct, t_direct,
+        h->d_obs_partials, h->d_amp, h->d_obs_counters, rows);
     count(h);
     CU(cudaGetLastError());
     return TDSE_OK;
@@ -542,6 +544,8 @@ int tdse_create(const tdse_grid *grid, tdse_handle **out) {
         size_t cap = 0;
         RC(ensure_buf(h, &h->d_partials, &cap, ctas * 4));
         CU(cudaMalloc(&h->d_obs_partials, sizeof(double) * 3 * obs_chunks(h) * B));
+        CU(cudaMalloc(&h->d_obs_counters, sizeof(unsigned int) * B));
+        CU(cudaMemset(h->d_obs_counters, 0, sizeof(unsigned int) * B));
         CU(cudaMalloc(&h->d_row_direct, sizeof(double) * 3 * B));
         CU(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
         RC(ensure_pool(h, 1));
@@ -560,7 +564,7 @@ void tdse_destroy(tdse_handle *h) {
     free_graphs(h);
     for (double2 *p : h->pool) cudaFree(p);
     void *ptrs[] = {h->d_vj, h->d_cen, h->d_cl, h->d_pulse, h->d_bufs, h->d_ctl, h->d_etab, h->d_eapply, h->d_partials,
-                    h->d_counter, h->d_phi, h->d_lstate, h->d_obs_partials, h->d_amp, h->d_rows, h->d_row_direct,
+                    h->d_counter, h->d_phi, h->d_lstate, h->d_obs_partials, h->d_obs_counters, h->d_amp, h->d_rows, h->d_row_direct,
                     h->d_dtlog, h->d_errlog, h->d_replay, h->d_alpha, h->d_beta, h->d_nrm, h->d_inv, h->d_coef,
                     h->d_m, h->d_nsub, h->d_basis};
     for (void *p : ptrs) if (p) cudaFree(p);
@@ -610,7 +614,7 @@ int tdse_set_bound_states(tdse_handle *h, int n_states, const int *l_of_state, c
     if (n_states > 0) {
         CU(cudaMalloc(&h->d_phi, sizeof(double) * (size_t)n_states * h->grid.n_r));
         CU(cudaMalloc(&h->d_lstate, sizeof(int) * n_states));
-        CU(cudaMalloc(&h->d_amp, sizeof(double2) * (size_t)n_states * h->grid.batch));
+        CU(cudaMalloc(&h->d_amp, sizeof(double2) * (size_t)n_states * h->grid.batch * obs_chunks_r(h)));
         CU(cudaMemcpy(h->d_phi, phi, sizeof(double) * (size_t)n_states * h->grid.n_r, cudaMemcpyHostToDevice));
         CU(cudaMemcpy(h->d_lstate, l_of_state, sizeof(int) * n_states, cudaMemcpyHostToDevice));
     }

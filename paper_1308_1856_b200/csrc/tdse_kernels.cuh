@@ -499,67 +499,111 @@ __global__ void rk45_begin_kernel(Ctl *c, const tdse_pulse *pulse, int B, const 
 }
 
 // ------------------------------------------------------------------------------------------------------
-// Observables (row a6).  obs_main: norm, dipole and acceleration sums by marching l along a column (each
-// element read once).  grid = (ceil(n_r/256), batch).  partials[(b*chunks + chunk)*3 + {0,1,2}].
+// Observables (row a6): norm, dipole and acceleration sums, bound-state overlaps and the row assembly in one launch.
+// A thread takes one radial column of a chunk of kObsRows partial waves (plus the first row of the next chunk for
+// the l, l+1 products) with all its loads issued at once -- a serial march over all l was latency-bound (64
+// dependent iterations on CFG3).  grid = (ceil(n_r/256), batch, ceil(n_l/kObsRows) + n_states).
 // ------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) obs_main_kernel(GridDev g, const double2 *psi, const Ctl *ctl, int step_off,
-                                                       int predicated, double *partials) {
+constexpr int kObsRows = 8;
+
+// ONE launch per logged row: CTAs (chunk_r, b, z < chunks_l) reduce norm / dipole / acceleration sums of a chunk,
+// CTAs (chunk_r, b, chunks_l + s) the overlap of 256 radial points with bound state s (Eq. 25); the last CTA of
+// a member to finish (ticket counter) adds the partials in a fixed order and assembles the row
+// {norm, <z>, <z''>, pop...} (Eq. 34, Eq. 36).  The first version used three launches (sums, overlaps,
+// assembly): 6 us of launch latency per step on CFG1.
+// partials[b][chunks_r*chunks_l][3], amp_part[b][n_states][chunks_r] (re, im), counters[b] (zero between launches).
+// t_direct: if use_direct, the time for -E(t); else t_{n+1} = t0 + (n+1) dt of the step being logged.
+__global__ void __launch_bounds__(256) obs_kernel(GridDev g, const double2 *psi, const double *phi, const int *l_of_state,
+                                                  int n_states, const tdse_pulse *pulse, const Ctl *ctl, int step_off,
+                                                  int predicated, int use_direct, double t_direct, double *partials,
+                                                  double2 *amp_part, unsigned int *counters, double *rows) {
     __shared__ double red_s[3 * 8];
-    if (predicated) {
+    __shared__ int last_flag;
+    long long row = 0;
+    double t = t_direct;
+    if (!use_direct) {
         const long long n = ctl->step_base + step_off + 1;
-        if (ctl->obs_every <= 0 || (n % ctl->obs_every) != 0) return;
+        if (predicated && (ctl->obs_every <= 0 || (n % ctl->obs_every) != 0)) return;
+        row = n / ctl->obs_every - 1;
+        t = time_at(ctl->t0, (double)n, ctl->dt);
     }
+    const int chunks_r = gridDim.x, chunks_l = gridDim.z - n_states;
     const int b = blockIdx.y, j = blockIdx.x * 256 + threadIdx.x;
     double red[3] = {0.0, 0.0, 0.0};
-    if (j < g.n_r) {
-        const double2 *p = psi + (size_t)b * g.n_l * g.n_r + j;
-        double2 cur = p[0];
-        double nn = cur.x * cur.x + cur.y * cur.y, sz = 0.0;
-        for (int l = 0; l + 1 < g.n_l; ++l) {
-            const double2 nx = p[(size_t)(l + 1) * g.n_r];
-            sz = fma(__ldg(g.cl + l), cur.x * nx.x + cur.y * nx.y, sz);
-            nn += nx.x * nx.x + nx.y * nx.y;
-            cur = nx;
+    if ((int)blockIdx.z < chunks_l) {
+        const int l0 = blockIdx.z * kObsRows;
+        if (j < g.n_r) {
+            const double2 *p = psi + ((size_t)b * g.n_l + l0) * g.n_r + j;
+            double2 v[kObsRows + 1];
+#pragma unroll
+            for (int r = 0; r <= kObsRows; ++r)
+                v[r] = (l0 + r < g.n_l) ? p[(size_t)r * g.n_r] : make_double2(0.0, 0.0);
+            double nn = 0.0, sz = 0.0;
+#pragma unroll
+            for (int r = 0; r < kObsRows; ++r) {
+                nn += v[r].x * v[r].x + v[r].y * v[r].y;
+                if (l0 + r + 1 < g.n_l) sz = fma(__ldg(g.cl + l0 + r), v[r].x * v[r + 1].x + v[r].y * v[r + 1].y, sz);
+            }
+            const double r = g.dr * (double)(j + 1);
+            red[0] = nn; red[1] = r * sz; red[2] = sz / (r * r);
         }
-        const double r = g.dr * (double)(j + 1);
-        red[0] = nn; red[1] = r * sz; red[2] = sz / (r * r);
+        block_reduce<256, 3>(red, red_s);
+        if (threadIdx.x == 0) {
+            double *o = partials + (((size_t)b * chunks_r + blockIdx.x) * chunks_l + blockIdx.z) * 3;
+            o[0] = red[0]; o[1] = red[1]; o[2] = red[2];
+        }
+    } else {
+        const int s = blockIdx.z - chunks_l;
+        if (j < g.n_r) {
+            const double w = __ldg(phi + (size_t)s * g.n_r + j);
+            const double2 v = psi[((size_t)b * g.n_l + l_of_state[s]) * g.n_r + j];
+            red[0] = w * v.x; red[1] = w * v.y;
+        }
+        block_reduce<256, 3>(red, red_s);
+        if (threadIdx.x == 0) amp_part[((size_t)b * n_states + s) * chunks_r + blockIdx.x] = make_double2(red[0], red[1]);
     }
-    block_reduce<256, 3>(red, red_s);
+    // ---- last CTA of this member assembles the row -------------------------------------------------------------
     if (threadIdx.x == 0) {
-        double *o = partials + ((size_t)b * gridDim.x + blockIdx.x) * 3;
-        o[0] = red[0]; o[1] = red[1]; o[2] = red[2];
+        __threadfence();
+        const unsigned int ticket = atomicAdd(counters + b, 1u);
+        last_flag = (ticket == (unsigned int)(gridDim.x * gridDim.z - 1));
+    }
+    __syncthreads();
+    if (!last_flag) return;
+    __threadfence();
+    const int W = 3 + n_states, chunks = chunks_r * chunks_l;
+    double sum[3] = {0.0, 0.0, 0.0};
+    for (int i = threadIdx.x; i < chunks; i += 256) {
+        const double *p = partials + ((size_t)b * chunks + i) * 3;
+        sum[0] += __ldcg(p); sum[1] += __ldcg(p + 1); sum[2] += __ldcg(p + 2);
+    }
+    block_reduce<256, 3>(sum, red_s);
+    double *o = rows + ((size_t)row * g.batch + b) * W;
+    if (threadIdx.x == 0) {
+        o[0] = g.dr * sum[0];
+        o[1] = 2.0 * g.dr * sum[1];
+        o[2] = -pulse_E(pulse[b], t) - 2.0 * g.z * g.dr * sum[2];
+        counters[b] = 0u;
+    }
+    for (int s = threadIdx.x; s < n_states; s += 256) {
+        double ax = 0.0, ay = 0.0;
+        for (int c = 0; c < chunks_r; ++c) {
+            const double2 a = __ldcg(amp_part + ((size_t)b * n_states + s) * chunks_r + c);
+            ax += a.x; ay += a.y;
+        }
+        const double ar = g.dr * ax, ai = g.dr * ay;
+        o[3 + s] = ar * ar + ai * ai;
     }
 }
 
-// amplitude_s = sum_j phi_s[j] f_{l_s,j}  (Eq. 25).  grid = (n_states, batch), block 128.
-__global__ void __launch_bounds__(128) obs_pop_kernel(GridDev g, const double2 *psi, const double *phi,
-                                                      const int *l_of_state, int n_states, const Ctl *ctl,
-                                                      int step_off, int predicated, double2 *amp) {
-    __shared__ double red_s[2 * 4];
-    if (predicated) {
-        const long long n = ctl->step_base + step_off + 1;
-        if (ctl->obs_every <= 0 || (n % ctl->obs_every) != 0) return;
-    }
-    const int s = blockIdx.x, b = blockIdx.y;
-    const double2 *f = psi + ((size_t)b * g.n_l + l_of_state[s]) * g.n_r;
-    const double *ph = phi + (size_t)s * g.n_r;
-    double red[2] = {0.0, 0.0};
-    for (int j = threadIdx.x; j < g.n_r; j += 128) {
-        const double w = __ldg(ph + j);
-        const double2 v = f[j];
-        red[0] = fma(w, v.x, red[0]); red[1] = fma(w, v.y, red[1]);
-    }
-    block_reduce<128, 2>(red, red_s);
-    if (threadIdx.x == 0) amp[(size_t)b * n_states + s] = make_double2(red[0], red[1]);
-}
-
-// Assemble the row {norm, <z>, <z''>, pop...} of every member (Eq. 34, Eq. 36).  grid = batch, block 128.
-// t_direct: if use_direct, the time for -E(t); else t_{n+1} = t0 + (n+1) dt of the step being logged.
-__global__ void __launch_bounds__(128) obs_final_kernel(GridDev g, const double *partials, int chunks,
-                                                        const double2 *amp, int n_states, const tdse_pulse *pulse,
+// The same for small grids: ONE CTA per member loops over all chunks and states, so that no cross-CTA hand-over
+// (fence, ticket, second pass over partials) sits on the critical path of a launch-latency-bound step.
+// grid = batch, block = 256.
+__global__ void __launch_bounds__(256) obs_small_kernel(GridDev g, const double2 *psi, const double *phi,
+                                                        const int *l_of_state, int n_states, const tdse_pulse *pulse,
                                                         const Ctl *ctl, int step_off, int predicated, int use_direct,
                                                         double t_direct, double *rows) {
-    __shared__ double red_s[3 * 4];
+    __shared__ double red_s[3 * 8];
     long long row = 0;
     double t = t_direct;
     if (!use_direct) {
@@ -569,22 +613,44 @@ __global__ void __launch_bounds__(128) obs_final_kernel(GridDev g, const double 
         t = time_at(ctl->t0, (double)n, ctl->dt);
     }
     const int b = blockIdx.x, W = 3 + n_states;
-    double red[3] = {0.0, 0.0, 0.0};
-    for (int i = threadIdx.x; i < chunks; i += 128) {
-        const double *p = partials + ((size_t)b * chunks + i) * 3;
-        red[0] += p[0]; red[1] += p[1]; red[2] += p[2];
-    }
-    block_reduce<128, 3>(red, red_s);
     double *o = rows + ((size_t)row * g.batch + b) * W;
+    double red[3] = {0.0, 0.0, 0.0};
+    for (int j = threadIdx.x; j < g.n_r; j += 256) {
+        const double2 *p = psi + (size_t)b * g.n_l * g.n_r + j;
+        double nn = 0.0, sz = 0.0;
+        for (int l0 = 0; l0 < g.n_l; l0 += kObsRows) {
+            double2 v[kObsRows + 1];
+#pragma unroll
+            for (int r = 0; r <= kObsRows; ++r)
+                v[r] = (l0 + r < g.n_l) ? p[(size_t)(l0 + r) * g.n_r] : make_double2(0.0, 0.0);
+#pragma unroll
+            for (int r = 0; r < kObsRows; ++r) {
+                nn += v[r].x * v[r].x + v[r].y * v[r].y;
+                if (l0 + r + 1 < g.n_l) sz = fma(__ldg(g.cl + l0 + r), v[r].x * v[r + 1].x + v[r].y * v[r + 1].y, sz);
+            }
+        }
+        const double r = g.dr * (double)(j + 1);
+        red[0] += nn; red[1] = fma(r, sz, red[1]); red[2] += sz / (r * r);
+    }
+    block_reduce<256, 3>(red, red_s);
     if (threadIdx.x == 0) {
         o[0] = g.dr * red[0];
         o[1] = 2.0 * g.dr * red[1];
         o[2] = -pulse_E(pulse[b], t) - 2.0 * g.z * g.dr * red[2];
     }
-    for (int s = threadIdx.x; s < n_states; s += 128) {
-        const double2 a = amp[(size_t)b * n_states + s];
-        const double ar = g.dr * a.x, ai = g.dr * a.y;
-        o[3 + s] = ar * ar + ai * ai;
+    for (int s = 0; s < n_states; ++s) {
+        double a[3] = {0.0, 0.0, 0.0};
+        const double2 *f = psi + ((size_t)b * g.n_l + l_of_state[s]) * g.n_r;
+        for (int j = threadIdx.x; j < g.n_r; j += 256) {
+            const double w = __ldg(phi + (size_t)s * g.n_r + j);
+            const double2 v = f[j];
+            a[0] = fma(w, v.x, a[0]); a[1] = fma(w, v.y, a[1]);
+        }
+        block_reduce<256, 3>(a, red_s);
+        if (threadIdx.x == 0) {
+            const double ar = g.dr * a[0], ai = g.dr * a[1];
+            o[3 + s] = ar * ar + ai * ai;
+        }
     }
 }
 
