@@ -66,6 +66,8 @@ void tdse_destroy(tdse_handle *h);
  *   "field_sample"     [0] 0: H frozen at t_n + dt/2 in Taylor/Lanczos steps, 1: at t_n (R-G7)
  *   "use_graph"        [1] capture blocks of steps in a CUDA graph
  *   "graph_steps"      [16] steps per captured graph
+ *   "rk4_block"        [1] tdse_step_rk4: 1 all four stages in one pass over HBM (register-patch kernel in RK mode)
+ *                          when the grid is at least one 128-column tile wide; 0 one kernel per stage
  *   "taylor_block"     [1] 0: one kernel per Taylor order; 1: temporally blocked step, all orders in one
  *                          pass (persistent register-patch kernel when n_l <= 32, else the shared-memory tile
  *                          kernel when the tile fits, else falls back to 0); 2: shared-memory tile kernel only;
@@ -134,7 +136,7 @@ int  tdse_lanczos_info(tdse_handle *h, double *alpha, double *beta, double *coef
 
 /* Number of CUDA kernels this handle has launched so far (graph nodes counted per graph launch). */
 long tdse_launch_count(tdse_handle *h);
-/* Kernel used by the last tdse_step_taylor call: 0 one kernel per order, 1 shared-memory tile kernel (all orders in
+/* Kernel used by the last tdse_step_taylor call (after tdse_step_rk4: 3 / 4 if the four stages ran fused, else 0): 0 one kernel per order, 1 shared-memory tile kernel (all orders in
  * one pass), 2 register-tile kernel v2, 3 persistent register-patch kernel v3 with direct global loads, 4 the same
  * with TMA tile fetches (1-4: all orders in one pass). */
 int  tdse_taylor_was_blocked(tdse_handle *h);

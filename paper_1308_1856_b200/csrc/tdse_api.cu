@@ -94,6 +94,7 @@ struct tdse_handle {
     BlockedCfg bcfg{};
     RtPlan rtp{}; int rt_variant = -1;
     RpPlan rpp{}; int n_sm = 148; int rp_variant = -1, rp_tma = -1;
+    int rk4_block = 1, rk4_fused = 0;       // option: fuse the four RK4 stages; what the last tdse_step_rk4 used
 };
 
 namespace {
@@ -274,6 +275,24 @@ int enqueue_rk4_block(tdse_handle *h, int n, int obs, cudaStream_t s) {
     field_table_kernel<<<(n * 4 * B + 255) / 256, 256, 0, s>>>(h->d_ctl, h->d_pulse, B, n, 1, h->d_etab);
     count(h);
     double2 *psi = h->pool[h->psi_slot];
+    if (h->rk4_fused) {
+        // all four stages in one pass over HBM (taylor_rp_kernel in RK mode); ping-pong psi <-> scratch
+        double2 *alt = h->pool[h->psi_slot == 0 ? 1 : 0];
+        for (int i = 0; i < n; ++i) {
+            double2 *src = (i & 1) ? alt : psi, *dst = (i & 1) ? psi : alt;
+            RC(launch_taylor_rp(h->gd, h->rpp, src, dst, h->d_etab + (size_t)i * 4 * B, &h->d_ctl->dt, 4, s));
+            count(h);
+            if (obs) RC(enqueue_obs(h, dst, i, 1, 0, 0.0, h->d_rows, s));
+        }
+        if (n & 1) {   // odd eager remainder: bring the state back into the psi slot
+            OpCopy cp{}; cp.dst = psi; cp.src = alt;
+            RC(launch_ew(h, cp, s));
+        }
+        ctl_advance_kernel<<<1, 32, 0, s>>>(h->d_ctl, n);
+        count(h);
+        CU(cudaGetLastError());
+        return TDSE_OK;
+    }
     for (int i = 0; i < n; ++i) {
         for (int st = 0; st < 4; ++st) {
             EpiRK<false> e{};
@@ -415,7 +434,7 @@ int run_blocks(tdse_handle *h, int kind, int p1, int p2, int n, int obs, long nb
         }
         return TDSE_OK;
     }
-    const auto key = std::make_tuple(kind, p1, p2, n, obs + 2 * h->taylor_blocked_last + 16 * (h->rtp.variant + 1) + 256 * (h->rpp.variant + 1) + 8192 * h->rpp.tma, h->psi_slot);
+    const auto key = std::make_tuple(kind, p1, p2, n, obs + 2 * h->taylor_blocked_last + 16 * (h->rtp.variant + 1) + 256 * (h->rpp.variant + 1) + 8192 * h->rpp.tma + 16384 * h->rk4_fused, h->psi_slot);
     auto it = h->graphs.find(key);
     if (it == h->graphs.end()) {
         cudaGraph_t g = nullptr;
@@ -582,6 +601,7 @@ int tdse_set_option(tdse_handle *h, const char *key, double value) {
     else if (k == "taylor_block") { if (value < 0 || value > 4) return TDSE_ERR_ARG; h->taylor_block = (int)value; }
     else if (k == "taylor_rt_variant") { if (value < -1 || value >= kNumRtVariants) return TDSE_ERR_ARG; h->rt_variant = (int)value; free_graphs(h); }
     else if (k == "taylor_rp_variant") { if (value < -1 || value >= kNumRpVariants) return TDSE_ERR_ARG; h->rp_variant = (int)value; free_graphs(h); }
+    else if (k == "rk4_block") { if (value < 0 || value > 1) return TDSE_ERR_ARG; h->rk4_block = (int)value; free_graphs(h); }
     else if (k == "taylor_rp_tma") { if (value < -1 || value > 1) return TDSE_ERR_ARG; h->rp_tma = (int)value; free_graphs(h); }
     else if (k == "taylor_block_width") { if (value < 0 || value > 4096) return TDSE_ERR_ARG; h->bcfg.width_override = (int)value; free_graphs(h); }
     else if (k == "lanczos_beta_tol") { if (!(value >= 0.0)) return TDSE_ERR_ARG; h->beta_tol = value; free_graphs(h); }
@@ -665,6 +685,7 @@ int tdse_step_taylor(tdse_handle *h, int order, double t0, double dt, long nstep
     // shared-memory tile, else per order); 2 shared-memory tile kernel only; 3 register-tile kernel (v2) only;
     // 4 persistent register-patch kernel (v3) only
     h->taylor_blocked_last = 0;
+    h->rk4_fused = 0;
     h->rtp = RtPlan{};
     h->rpp = RpPlan{};
     if (h->taylor_block == 1 || h->taylor_block == 4) {
@@ -685,6 +706,13 @@ int tdse_step_rk4(tdse_handle *h, double t0, double dt, long nsteps, int obs_eve
     if (!h || nsteps < 0 || obs_every < 0) return TDSE_ERR_ARG;
     RC(ensure_pool(h, 6));
     h->taylor_blocked_last = 0;
+    h->rk4_fused = 0;
+    h->rpp = RpPlan{};
+    if (h->rk4_block) {           // all four stages in one pass (register-patch kernel in RK mode) when it applies
+        h->rpp = rp_plan(h->grid, 4, h->n_sm, -1, h->rp_tma, 1);
+        if (h->rpp.ok) { h->rk4_fused = 1; h->taylor_blocked_last = 3; }
+        else h->rpp = RpPlan{};
+    }
     rk_roles(h);
     RC(upload_bufs(h, 6, (cudaStream_t)stream));
     return run_fixed(h, KIND_RK4, 0, 0, t0, dt, nsteps, obs_every, (cudaStream_t)stream);

@@ -43,7 +43,7 @@ struct RpGeom {
 
 // shared memory: vertical exchange [parity][warp][top,bottom][CP planes][32 lanes], radial edge exchange between
 // the warps of a row group [parity][warp][left,right][4 rows][HW], row table
-template <int FD, int CP, int NWR, int NWC, bool TMA>
+template <int FD, int CP, int NWR, int NWC, bool TMA, bool RK = false>
 struct RpSmem {
     // TMA landing zone of the next item: [row][128-byte column group][8 columns], 128-byte swizzled; first member
     // so that it is 1024-byte aligned
@@ -54,6 +54,7 @@ struct RpSmem {
     double2 edge[2][NWR * NWC][2][kRpRows][(FD == 3) ? 1 : 2];
     double2 zrow[CP][32];                   // zeros for ever: the rows above l = 0 and below the last row group
     double rowtab[NWR * kRpRows][4];        // {c_l, l(l+1), c_{l-1}, 0}
+    double2 psi_s[RK ? kRpRows * CP : 1][NWR * NWC * 32];   // RK4: psi(t_n) of every thread's patch (private slots)
 };
 
 __device__ __forceinline__ double2 shfl_up2(double2 v) {
@@ -130,7 +131,11 @@ __device__ __forceinline__ int rp_start(int t, int W, int H, int N, int WT) {
 // CLUSTER: the n_l rows are split over the CTAs of a thread-block cluster (rank = row block of 4*NWR rows); the
 // l-1 / l+1 rows at a CTA boundary are read from the neighbouring CTA's shared memory (DSMEM) and the per-order
 // barrier is a cluster barrier.
-template <int FD, int CP, int NWR, int NWC, bool MASK, int MINB, bool TMA, bool CLUSTER>
+// RK: classic RK4 (Eq. 38) instead of Taylor: four sweeps with the field at t_n, t_n + h/2 (twice),
+// t_n + h (ef[stage*batch + b]); sweep i forms k_i = -i H g_i, the next stage vector g_{i+1} = psi + a_i h k_i (psi
+// re-read from this thread's private shared-memory slots) and psi_new += b_i h k_i: 32 B/point/step over HBM instead
+// of 272 for one kernel per stage.
+template <int FD, int CP, int NWR, int NWC, bool MASK, int MINB, bool TMA, bool CLUSTER, bool RK = false>
 __global__ void __launch_bounds__(NWR * NWC * 32, MINB)
 taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict__ out, const double *__restrict__ ef,
                  const double *__restrict__ dtp, int order, int W, int H, int n_tiles, int n_items,
@@ -140,7 +145,7 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
     using G = RpGeom<FD, CP, NWR, NWC>;
     constexpr int RP = kRpRows, WT = G::WT, HW = G::HW;
     extern __shared__ __align__(1024) unsigned char rp_smem_raw[];
-    using Smem = RpSmem<FD, CP, NWR, NWC, TMA>;
+    using Smem = RpSmem<FD, CP, NWR, NWC, TMA, RK>;
     Smem &sm = *reinterpret_cast<Smem *>(rp_smem_raw);     // dynamic shared memory starts 1024-byte aligned
     if (TMA && (smem_u32(rp_smem_raw) & 1023u)) __trap();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -274,10 +279,18 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                 Cq[q] = inv_c1 * __ldg(g.cen + jj);
             }
         }
-        {
-            const double es = inv_c1 * (__ldg(ef + b) * g.dr);
+        // coupling weights E r_j / c1 for the field value of this step (Taylor) or of RK stage `st`
+        auto set_field = [&](const int st) {
+            const double es = inv_c1 * (__ldg(ef + st * g.batch + b) * g.dr);
 #pragma unroll
             for (int q = 0; q < CP; ++q) Eq[q] = es * (double)(dom[q] ? start + c0 + q + 1 : 1);
+        };
+        set_field(0);
+        if (RK) {       // psi(t_n) is needed again when the stage vectors g_2..g_4 are formed
+#pragma unroll
+            for (int r = 0; r < RP; ++r)
+#pragma unroll
+                for (int q = 0; q < CP; ++q) sm.psi_s[r * CP + q][threadIdx.x] = T[r][q];
         }
         // publish u_0: rows 0 and RP-1 for the warps above / below, edge columns for the warps left / right
         // (after every thread has finished reading the previous item's last exchange)
@@ -299,7 +312,8 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
         // their coupling weights c_{l-1} E r / c1 and c_l E r / c1; ev1 / ev2 = edge columns of the neighbouring warp.
         auto do_row = [&](const double2 (&Ti)[RP][CP], double2 (&To)[RP][CP], const int r, const double2 (&dn)[CP],
                           const double2 (&up)[CP], const double (&alo)[CP], const double (&aup)[CP], const double ll1,
-                          const int pr, const bool odd, const bool first, const double s) {
+                          const int pr, const bool odd, const bool first, const double s, const bool want_out,
+                          const double cg) {
             double2 lf1 = shfl_up2(Ti[r][CP - 1]);       // column c0 - 1 from lane - 1
             double2 rg1 = shfl_dn2(Ti[r][0]);            // column c0 + CP from lane + 1
             double2 lf2 = z2, rg2 = z2;
@@ -344,7 +358,11 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                 hx = fma(alo[q], dn[q].x, hx);
                 hy = fma(alo[q], dn[q].y, hy);
                 if (MASK && !dom[q]) { hx = 0.0; hy = 0.0; }
-                To[r][q] = make_double2(hx, hy);
+                if (!RK) To[r][q] = make_double2(hx, hy);
+                else if (want_out) {            // g_{i+1} = psi + a_i h k_i,  k_i = -i H g_i = c1 (hy - i hx)
+                    const double2 p0 = first ? f : sm.psi_s[r * CP + q][threadIdx.x];
+                    To[r][q] = make_double2(fma(cg, hy, p0.x), fma(-cg, hx, p0.y));
+                }
                 // acc += (-i)^k (dt c1)^k / k! * u'_k; s carries the sign: odd k: -+i, even k: -+1
                 // (order 1 starts the sum from psi itself: A = u_0 + ..., no separate copy)
                 if (first) { A[r][q].x = fma(s, hy, f.x); A[r][q].y = fma(-s, hx, f.y); }
@@ -358,7 +376,9 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
         // outer rows are published and the barrier is signalled (split arrive / wait).  The order loop below is
         // unrolled by two with the roles of T and U swapped, so that the new term is written where the term before
         // last lived and no register copies are needed at the loop back-edge.
-        auto sweep = [&](const double2 (&Ti)[RP][CP], double2 (&To)[RP][CP], const int k, const bool odd, const bool first, const double s) {
+        auto sweep = [&](const double2 (&Ti)[RP][CP], double2 (&To)[RP][CP], const int k, const bool odd, const bool first, const double s,
+                         const double cg) {
+            const bool want_out = k < order;
             const int pr = (k - 1) & 1, pw = k & 1;
             double cup[RP], ll1[RP];
 #pragma unroll
@@ -370,8 +390,8 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
 #pragma unroll
             for (int q = 0; q < CP; ++q) { a0[q] = cup[0] * Eq[q]; a1[q] = cup[1] * Eq[q]; a2[q] = cup[2] * Eq[q]; }
             if (NWC == 1) {
-                do_row(Ti, To, 1, Ti[0], Ti[2], a0, a1, ll1[1], pr, odd, first, s);
-                do_row(Ti, To, 2, Ti[1], Ti[3], a1, a2, ll1[2], pr, odd, first, s);
+                do_row(Ti, To, 1, Ti[0], Ti[2], a0, a1, ll1[1], pr, odd, first, s, want_out, cg);
+                do_row(Ti, To, 2, Ti[1], Ti[3], a1, a2, ll1[2], pr, odd, first, s, want_out, cg);
             }
             bar_wait();
             // every value of the stage was consumed by the arithmetic of order 1: fetch the next item
@@ -389,12 +409,12 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
 #pragma unroll
                 for (int q = 0; q < CP; ++q) { ac[q] = clo * Eq[q]; a3[q] = cup[3] * Eq[q]; }
             }
-            do_row(Ti, To, 0, lo, Ti[1], ac, a0, ll1[0], pr, odd, first, s);
+            do_row(Ti, To, 0, lo, Ti[1], ac, a0, ll1[0], pr, odd, first, s, want_out, cg);
             if (NWC > 1) {
-                do_row(Ti, To, 1, Ti[0], Ti[2], a0, a1, ll1[1], pr, odd, first, s);
-                do_row(Ti, To, 2, Ti[1], Ti[3], a1, a2, ll1[2], pr, odd, first, s);
+                do_row(Ti, To, 1, Ti[0], Ti[2], a0, a1, ll1[1], pr, odd, first, s, want_out, cg);
+                do_row(Ti, To, 2, Ti[1], Ti[3], a1, a2, ll1[2], pr, odd, first, s, want_out, cg);
             }
-            do_row(Ti, To, 3, Ti[2], below, a2, a3, ll1[3], pr, odd, first, s);
+            do_row(Ti, To, 3, Ti[2], below, a2, a3, ll1[3], pr, odd, first, s, want_out, cg);
             if (k < order) {
 #pragma unroll
                 for (int q = 0; q < CP; ++q) {
@@ -413,18 +433,29 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
         };
 
         double2 U[RP][CP];
-        double sk = kappa;
-        sweep(T, U, 1, true, true, sk);                       // order 1: -i
-        int k = 2;
-        for (; k + 1 <= order; k += 2) {
-            sk = sk * (kappa * kRpInvK[k]);
-            sweep(U, T, k, false, false, (k & 2) ? -sk : sk);
-            sk = sk * (kappa * kRpInvK[k + 1]);
-            sweep(T, U, k + 1, true, false, ((k + 1) & 2) ? -sk : sk);
-        }
-        if (k <= order) {
-            sk = sk * (kappa * kRpInvK[k]);
-            sweep(U, T, k, false, false, (k & 2) ? -sk : sk);
+        if (RK) {
+            // classic RK4: a = (1/2, 1/2, 1), b = (1/6, 1/3, 1/3, 1/6); kappa = h c1 carries k_i's factor c1
+            sweep(T, U, 1, true, true, kappa * (1.0 / 6.0), 0.5 * kappa);
+            set_field(1);
+            sweep(U, T, 2, true, false, kappa * (1.0 / 3.0), 0.5 * kappa);
+            set_field(2);
+            sweep(T, U, 3, true, false, kappa * (1.0 / 3.0), kappa);
+            set_field(3);
+            sweep(U, T, 4, true, false, kappa * (1.0 / 6.0), 0.0);
+        } else {
+            double sk = kappa;
+            sweep(T, U, 1, true, true, sk, 0.0);                  // order 1: -i
+            int k = 2;
+            for (; k + 1 <= order; k += 2) {
+                sk = sk * (kappa * kRpInvK[k]);
+                sweep(U, T, k, false, false, (k & 2) ? -sk : sk, 0.0);
+                sk = sk * (kappa * kRpInvK[k + 1]);
+                sweep(T, U, k + 1, true, false, ((k + 1) & 2) ? -sk : sk, 0.0);
+            }
+            if (k <= order) {
+                sk = sk * (kappa * kRpInvK[k]);
+                sweep(U, T, k, false, false, (k & 2) ? -sk : sk, 0.0);
+            }
         }
         // the barrier signalled by the last order is waited for before the next item publishes (or at the end)
 
@@ -477,10 +508,12 @@ inline int rp_init_tables() {
     return cudaMemcpyToSymbol(kRpInvK, h, sizeof(h)) == cudaSuccess ? TDSE_OK : TDSE_ERR_CUDA;
 }
 
-struct RpPlan { int ok, variant, tma, cl, W, H, WT, n_tiles, n_items, grid, threads; };   // cl: CTAs per cluster (1: none)
+struct RpPlan { int ok, variant, tma, cl, rk, W, H, WT, n_tiles, n_items, grid, threads; };   // cl: CTAs per cluster (1: none)
 
 // use_tma: -1 heuristic, 0 never, 1 whenever the layout allows it (n_r % 8 == 0, a full tile, 4-column patches)
-inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant, int use_tma) {
+// rk: plan the fused RK4 step (order = 4 sweeps; only the one-warp-wide 16-point instantiations, full tiles)
+constexpr bool rp_rk_capable(int variant) { return variant >= 0 && variant <= 3; }
+inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant, int use_tma, int rk = 0) {
     RpPlan best{};
     const int hw = (g.fd_order == 3) ? 1 : 2;
     double best_cost = 0.0;
@@ -488,6 +521,7 @@ inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant
         if (force_variant >= 0 && i != force_variant) continue;
         const RpVariant &v = kRpVariants[i];
         const int WT = 32 * v.cp * v.nwc;
+        if (rk && (!rp_rk_capable(i) || g.n_r < WT)) continue;
         int rows = kRpRows * v.nwr, cl = 1;
         if (rows < g.n_l) {
             // more rows than one CTA holds: split them over a cluster of 2, 4 or 8 CTAs (16-row CTAs only)
@@ -505,7 +539,7 @@ inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant
             if (tma) H = (H + 7) & ~7;                      // tile starts on a 128-byte column group
             else if ((g.n_r & 1) == 0) H = (H + 1) & ~1;    // even halo: every patch row starts 32-byte aligned
             RpPlan p{};
-            p.variant = i; p.tma = tma; p.cl = cl; p.H = H; p.WT = WT; p.threads = 32 * v.nwr * v.nwc;
+            p.variant = i; p.tma = tma; p.cl = cl; p.rk = rk; p.H = H; p.WT = WT; p.threads = 32 * v.nwr * v.nwc;
             if (g.n_r <= WT) { p.W = g.n_r; p.n_tiles = 1; }
             else {
                 p.W = WT - 2 * H;
@@ -518,14 +552,16 @@ inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant
             if (p.n_tiles * 4 <= p.grid) p.grid = p.grid / p.n_tiles * p.n_tiles;
             p.grid *= cl;
             p.ok = 1;
-            // cost: columns computed in total; 8-point patches measured 1.5x slower per column than 16-point
-            // patches (twice the exchange per point, spills at 128 registers); the asynchronous tile fetch hides
-            // the load latency of the next item
-            double cost = (double)p.n_tiles * WT * rows;
+            // cost ~ time: the points one CTA computes per item times the items an SM has to work through (at least
+            // one: a small grid is bound by the serial work of a CTA, so more and smaller CTAs win).  Measured
+            // penalties: 8-point patches 1.5x per column (twice the exchange per point, spills at 128 registers);
+            // tiles wider than one warp 1.4x (edge columns through shared memory, no work before the barrier);
+            // cluster barriers 1.25x; the asynchronous tile fetch hides the load latency of the next item.
+            const double n_ctas = (double)p.n_items * cl;
+            double cost = (double)(rows / cl) * WT * std::max(1.0, n_ctas / n_sm);
             if (force_variant < 0 && v.cp == 2) cost *= 1.5;
-            // tiles wider than one warp exchange edge columns through shared memory and cannot start an order
-            // before the barrier: measured 1.3-1.4x slower per column
             if (force_variant < 0 && v.nwc > 1) cost *= 1.4;
+            if (cl > 1) cost *= 1.25;
             if (tma) cost *= 0.85;
             if (!best.ok || cost < best_cost) { best = p; best_cost = cost; }
         }
@@ -587,7 +623,7 @@ inline int rp_launch_kernel(K kern, bool *attr_set, int smem, const RpPlan &p, c
                ? TDSE_OK : TDSE_ERR_CUDA;
 }
 
-template <int FD, int CP, int NWR, int NWC, int MINB, bool CLUSTERABLE>
+template <int FD, int CP, int NWR, int NWC, int MINB, bool CLUSTERABLE, bool RKABLE>
 inline int rp_launch_one(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
                          const double *dtp, int order, cudaStream_t s) {
     if (FD == 5 && CP < 2) return TDSE_ERR_UNSUPPORTED;
@@ -600,6 +636,19 @@ inline int rp_launch_one(const GridDev &g, const RpPlan &p, const double2 *in, d
         if (!kTma || mask) return TDSE_ERR_UNSUPPORTED;
         tm = rp_tensor_map(in, g.n_r, g.batch * g.n_l, kRpRows * NWR, 32 * CP * NWC);
         if (!tm) return TDSE_ERR_CUDA;
+    }
+    if (p.rk) {
+        if (!RKABLE || mask) return TDSE_ERR_UNSUPPORTED;
+        constexpr bool kRk = RKABLE, kCl = CLUSTERABLE && RKABLE, kT = kTma && RKABLE;
+        static bool rk_attr[4] = {false, false, false, false};
+        const int sm_t = (int)sizeof(RpSmem<FD, CP, NWR, NWC, kT, kRk>), sm_n = (int)sizeof(RpSmem<FD, CP, NWR, NWC, false, kRk>);
+        if (p.cl > 1) {
+            if (!kCl) return TDSE_ERR_UNSUPPORTED;
+            if (p.tma) return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, kT, kCl, kRk>, &rk_attr[3], sm_t, p, s, g, in, out, ef, dtp, order, *tm);
+            return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, kCl, kRk>, &rk_attr[2], sm_n, p, s, g, in, out, ef, dtp, order, *tm);
+        }
+        if (p.tma) return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, kT, false, kRk>, &rk_attr[1], sm_t, p, s, g, in, out, ef, dtp, order, *tm);
+        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, false, kRk>, &rk_attr[0], sm_n, p, s, g, in, out, ef, dtp, order, *tm);
     }
     if (p.cl > 1) {
         if (!CLUSTERABLE || mask) return TDSE_ERR_UNSUPPORTED;
@@ -625,8 +674,8 @@ inline int launch_taylor_rp(const GridDev &g, const RpPlan &p, const double2 *in
     if (!p.ok) return TDSE_ERR_UNSUPPORTED;
 #define TDSE_RP_CASE(I, CP, NWR, NWC, MINB)                                                                  \
     case I:                                                                                                  \
-        return (g.fd == 3) ? rp_launch_one<3, CP, NWR, NWC, MINB, rp_clusterable(I)>(g, p, in, out, ef, dtp, order, s)  \
-                           : rp_launch_one<5, CP, NWR, NWC, MINB, rp_clusterable(I)>(g, p, in, out, ef, dtp, order, s);
+        return (g.fd == 3) ? rp_launch_one<3, CP, NWR, NWC, MINB, rp_clusterable(I), rp_rk_capable(I)>(g, p, in, out, ef, dtp, order, s)  \
+                           : rp_launch_one<5, CP, NWR, NWC, MINB, rp_clusterable(I), rp_rk_capable(I)>(g, p, in, out, ef, dtp, order, s);
     switch (p.variant) {
         TDSE_RP_CASE(0, 4, 1, 1, 8)
         TDSE_RP_CASE(1, 4, 2, 1, 4)

@@ -370,15 +370,34 @@ def test_taylor_field_sample_start_and_continuation(B):
     h.close()
 
 
-@pytest.mark.parametrize("fd,batch,use_graph", [(5, 1, 1), (3, 2, 0)])
-def test_rk4_parity(B, fd, batch, use_graph):
-    c = wl.config("cfg2", n_r=600, n_l=9, fd_order=fd, batch=batch)
+RK4_CASES = [
+    # n_r, n_l, fd, batch, nsteps, obs_every, use_graph
+    (600, 9, 5, 1, 70, 5, 1),          # 9 of 16 rows, ragged last tile, odd n_r/8 (direct loads)
+    (600, 9, 3, 2, 70, 5, 0),          # batched, eager
+    (1000, 16, 5, 1, 41, 0, 1),        # TMA tile fetch, odd number of steps
+    (640, 32, 3, 3, 20, 4, 1),         # 8 warps per CTA
+    (520, 64, 5, 1, 12, 0, 1),         # CFG2-like with 64 rows: cluster of 4 CTAs
+    (100, 5, 3, 1, 30, 1, 1),          # narrower than a tile: falls back to one kernel per stage
+]
+
+
+@pytest.mark.parametrize("fused", [0, 1])
+@pytest.mark.parametrize("case", RK4_CASES)
+def test_rk4_parity(B, case, fused):
+    """Classic RK4 against the oracle's stage-by-stage recursion: one kernel per stage (fused = 0) and all four
+    stages in one pass of the register-patch kernel (fused = 1: direct loads, TMA, 8 warps, clusters)."""
+    n_r, n_l, fd, batch, nsteps, obs_every, use_graph = case
+    c = wl.config("cfg2", n_r=n_r, n_l=n_l, fd_order=fd, batch=batch)
     dt = wl.dt_eff(c, "rk4", 4)
-    nsteps = 70
     t0 = wl.window(c, nsteps, dt)
     psi0 = wl.populated_state(c)
-    h, got, ref, gobs, robs = run_pair_fixed(B, c, "rk4", nsteps, psi0, t0, dt, 5, [(0, 0)], {"use_graph": use_graph})
+    h, got, ref, gobs, robs = run_pair_fixed(B, c, "rk4", nsteps, psi0, t0, dt, obs_every, [(0, 0)],
+                                             {"use_graph": use_graph, "rk4_block": fused})
+    assert (h.taylor_kernel() in (3, 4)) == (bool(fused) and n_r >= 128)
     check_fixed(got, ref, gobs, robs)
+    for b in range(batch):
+        for l in range(n_l):
+            assert np.linalg.norm(got[b, l] - ref[b, l]) <= TOL_PSI * max(np.linalg.norm(ref[b, l]), 1e-3)
     h.close()
 
 
