@@ -143,6 +143,16 @@ def step_taylor(g, pulses, psi, order, t0, dt, nsteps, field_sample=0, states=No
     return psi, out
 
 
+def step_imag(g, psi, order, dt, nsteps):
+    """Imaginary-time propagation with re-normalisation. Returns psi, energy[nsteps][batch]."""
+    psi = _state(g, psi)
+    en = np.zeros((max(nsteps, 1), g.batch))
+    rc = lib().oracle_step_imag(C.byref(g), _dp(psi.view(np.float64)), int(order), C.c_double(dt), C.c_long(nsteps),
+                                _dp(en))
+    assert rc == 0, rc
+    return psi, en[:nsteps]
+
+
 def step_rk_fixed(g, pulses, psi, tableau, t0, dt, nsteps, states=None, obs_every=0):
     """tableau: 0 = ClassicRK4, 1 = DormandPrince (5th-order weights). Returns psi, err[nsteps], obs."""
     psi = _state(g, psi)

@@ -499,6 +499,37 @@ int oracle_step_taylor(const oracle_grid *g, const oracle_pulse *pulse, double *
     return 0;
 }
 
+// Imaginary-time ("diffusion") propagation: the field-free equation with -i -> 1, i.e.
+// F^(k) = (-dt/k) H F^(k-1), F(t+dt) = sum_k F^(k) (the Taylor recursion of P:456 Eq. 37 with the replacement),
+// followed by re-normalisation after every step.  Energy estimate P:212 Eq. 24; the norm taken is that of
+// the whole wavefunction and, since <psi|psi> = exp(-2 E dt) for a normalised eigenstate evolved by exp(-H dt),
+// E = -ln<psi(t+dt)|psi(t+dt)> / (2 dt)  (reading R-G25: the factor 2 is absent from the printed equation; the
+// closed-form ground-state energy of the 3-point scheme pins it).
+int oracle_step_imag(const oracle_grid *g, double *psi, int order, double dt, long nsteps, double *energy_out) {
+    if (!grid_ok(g) || !psi || order < 1 || nsteps < 0 || !(dt > 0.0)) return -1;
+    const long M = n_points(g);
+    std::vector<double> term(2 * M), hterm(2 * M);
+    for (long n = 0; n < nsteps; ++n) {
+        for (int b = 0; b < g->batch; ++b) {
+            double *f = psi + 2 * M * b;
+            std::memcpy(term.data(), f, sizeof(double) * 2 * M);
+            for (int k = 1; k <= order; ++k) {
+                apply_H_member(g, term.data(), 0.0, hterm.data());
+                const double s = dt / k;
+                for (long i = 0; i < 2 * M; ++i) term[i] = -s * hterm[i];
+                for (long i = 0; i < 2 * M; ++i) f[i] += term[i];
+            }
+            double n2 = 0.0;
+            for (long i = 0; i < 2 * M; ++i) n2 += f[i] * f[i];
+            n2 *= g->dr;                                   // rectangle rule (reading R-G13)
+            if (energy_out) energy_out[n * g->batch + b] = -std::log(n2) / (2.0 * dt);
+            const double inv = 1.0 / std::sqrt(n2);
+            for (long i = 0; i < 2 * M; ++i) f[i] *= inv;
+        }
+    }
+    return 0;
+}
+
 int oracle_step_rk_fixed(const oracle_grid *g, const oracle_pulse *pulse, double *psi, int tableau,
                          double t0, double dt, long nsteps, double *err_out, const oracle_obs *obs) {
     if (!grid_ok(g) || !pulse || !psi || nsteps < 0 || tableau < 0 || tableau > 1) return -1;

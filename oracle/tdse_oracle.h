@@ -85,6 +85,11 @@ typedef struct {
     int obs_every; double *obs_out;
 } oracle_obs;
 
+/* Imaginary-time propagation: term_k = (-dt/k) H term_{k-1} with E = 0, psi += term_k, then
+ * psi /= ||psi||; energy_out[n*batch + b] = -ln<psi|psi> / (2 dt) before the re-normalisation (Eq. 24 in
+ * reading R-G25).  psi must be normalised on entry for the first estimate to be meaningful. */
+int oracle_step_imag(const oracle_grid *g, double *psi, int order, double dt, long nsteps, double *energy_out);
+
 /* P:456 Eq. 37 (index corrected): term_k = (-i dt/k) H term_{k-1}, psi += term_k */
 int oracle_step_taylor(const oracle_grid *g, const oracle_pulse *pulse, double *psi,
                        int order, double t0, double dt, long nsteps, int field_sample,

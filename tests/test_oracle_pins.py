@@ -547,3 +547,53 @@ def test_P8_ehrenfest_and_P10_norm():
     a = acc[::s][1:-1]
     assert np.max(np.abs(d2 - a)) < 0.02 * np.max(np.abs(a))      # P8 (soft): signs/factors of Eq. 34/36
     assert np.max(np.abs(a)) > 1e-3
+
+
+# ------------------------------------------------------------------------------------------- imaginary time (P11)
+def _h_l_banded(n_r, dr, l):
+    """diagonal and off-diagonal of the 3-point h_l (Eq. 7, reading R-G5), written out here independently."""
+    r = dr * np.arange(1, n_r + 1)
+    d = 1.0 / dr ** 2 + l * (l + 1) / (2 * r ** 2) - 1.0 / r
+    e = np.full(n_r - 1, -0.5 / dr ** 2)
+    return d, e
+
+
+@pytest.mark.parametrize("l", [0, 1])
+def test_P11_imaginary_time_converges_to_lowest_state_of_l(l):
+    """with -i -> 1 and re-normalisation the state settles into the lowest eigenstate of the populated l
+    block, and -ln<psi|psi>/(2 dt) (Eq. 24, reading R-G25) is its energy: closed form for l = 0, LAPACK for l = 1."""
+    dr, n_r, dt, order = 0.2, 400, 0.01, 4
+    g = oracle.make_grid(n_r, dr, 3, 3)
+    r = dr * np.arange(1, n_r + 1)
+    psi = np.zeros((1, 3, n_r), dtype=np.complex128)
+    psi[0, l] = r ** (l + 1) * np.exp(-r / (l + 1)) * (1 + 0.3j)          # analytic guess with an arbitrary phase
+    psi /= math.sqrt(dr * np.sum(np.abs(psi) ** 2))
+    out, en = oracle.step_imag(g, psi, order, dt, 12000)
+    d, e = _h_l_banded(n_r, dr, l)
+    w, v = sla.eigh_tridiagonal(d, e, select="i", select_range=(0, 0))
+    if l == 0:
+        closed = -1.0 / (1.0 + math.sqrt(1.0 + dr * dr))                # golden/closed_form_energies.txt
+        assert abs(w[0] - closed) < 1e-9                                 # (finite box: 80 au)
+    assert abs(en[-1, 0] - w[0]) < 1e-9
+    assert np.all(np.diff(en[:, 0]) < 1e-11)                              # the estimate decreases monotonically (up to rounding / dt)
+    assert abs(dr * np.sum(np.abs(out) ** 2) - 1.0) < 1e-13              # re-normalised
+    assert np.count_nonzero(out[0, [k for k in range(3) if k != l]]) == 0  # no field: blocks stay uncoupled
+    ov = abs(np.vdot(v[:, 0], out[0, l])) * math.sqrt(dr)
+    assert abs(ov - 1.0) < 1e-9                                           # the state is the LAPACK eigenvector
+
+
+def test_P11_imaginary_time_step_on_an_eigenvector():
+    """One step from an exact eigenvector of the discrete h_0: the state is unchanged and the estimate is
+    -ln(R_P(-E dt)^2)/(2 dt) with R_P the truncated exponential: pins the sign, the 1/k factors and the factor 2."""
+    dr, n_r = 0.2, 300
+    g = oracle.make_grid(n_r, dr, 2, 3)
+    d, e = _h_l_banded(n_r, dr, 0)
+    w, v = sla.eigh_tridiagonal(d, e, select="i", select_range=(0, 1))
+    for dt, order in ((0.02, 3), (0.05, 6)):
+        for idx in (0, 1):
+            psi = np.zeros((1, 2, n_r), dtype=np.complex128)
+            psi[0, 0] = v[:, idx] / math.sqrt(dr)
+            out, en = oracle.step_imag(g, psi, order, dt, 1)
+            rp = sum((-w[idx] * dt) ** k / math.factorial(k) for k in range(order + 1))
+            assert abs(en[0, 0] - (-math.log(rp * rp) / (2 * dt))) < 1e-11
+            assert np.linalg.norm(out - psi) < 1e-11 * np.linalg.norm(psi)
