@@ -112,6 +112,16 @@ int  tdse_step_rk4    (tdse_handle *h, double t0, double dt, long nsteps, int ob
 int  tdse_step_lanczos(tdse_handle *h, int krylov_dim, int taylor_order, double t0, double dt, long nsteps,
                        int obs_every, void *stream);
 
+/* Imaginary-time ("diffusion") propagation for ground states: no field, -i -> 1, i.e.
+ * F^(k) = (-dt/k) H F^(k-1), F_{n+1} = sum_{k<=order} F^(k), then F_{n+1} /= ||F_{n+1}|| (whole wavefunction of the
+ * member, rectangle rule) after every step.  The energy estimate of the step, E = -ln<F_{n+1}|F_{n+1}> / (2 dt)
+ * taken before the re-normalisation (Eq. 24 in reading R-G25), is logged on the device; the state must be
+ * normalised on entry for the first estimate to be meaningful.  Asynchronous on `stream`. */
+int  tdse_step_imag(tdse_handle *h, int order, double dt, long nsteps, void *stream);
+/* Energy estimates of the last tdse_step_imag call: energy_host [rows][batch], at most max_rows rows.
+ * Synchronises `stream`. */
+int  tdse_energy_log(tdse_handle *h, double *energy_host, long max_rows, void *stream);
+
 /* Embedded Dormand-Prince 5(4) (named P:796; error estimate P:813-833; the adaptive controller is ours,
  * R-C4, the paper's is "not implemented"): err = max_b ||Delta_b||_2 / (rtol ||psi_new,b||_2), accept iff
  * err <= 1, dt_next = dt clamp(0.9 err^(-1/5), 0.2, 5) (<= 1 right after a reject), last step clipped to t_end,

@@ -17,7 +17,7 @@ ERRORS = {-1: "TDSE_ERR_ARG", -2: "TDSE_ERR_ALLOC", -3: "TDSE_ERR_CUDA", -4: "TD
 
 # every symbol include/tdse.h declares
 SYMBOLS = ["tdse_create", "tdse_destroy", "tdse_set_option", "tdse_set_pulse", "tdse_set_bound_states",
-           "tdse_set_state", "tdse_get_state", "tdse_apply_H", "tdse_step_taylor", "tdse_step_rk4",
+           "tdse_set_state", "tdse_get_state", "tdse_apply_H", "tdse_step_taylor", "tdse_step_imag", "tdse_energy_log", "tdse_step_rk4",
            "tdse_step_lanczos", "tdse_step_rk45", "tdse_observables", "tdse_obs_log", "tdse_dt_log",
            "tdse_lanczos_info", "tdse_launch_count", "tdse_taylor_was_blocked", "tdse_strerror", "tdse_version"]
 
@@ -59,6 +59,8 @@ def lib():
         L.tdse_get_state.argtypes = [vp, vp, C.c_int, vp]
         L.tdse_apply_H.argtypes = [vp, vp, vp, dp, vp]
         L.tdse_step_taylor.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_long, C.c_int, vp]
+        L.tdse_step_imag.argtypes = [vp, C.c_int, C.c_double, C.c_long, vp]
+        L.tdse_energy_log.argtypes = [vp, C.POINTER(C.c_double), C.c_long, vp]
         L.tdse_step_rk4.argtypes = [vp, C.c_double, C.c_double, C.c_long, C.c_int, vp]
         L.tdse_step_lanczos.argtypes = [vp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_long, C.c_int, vp]
         L.tdse_step_rk45.argtypes = [vp, C.c_double, C.c_double, C.c_double, C.c_double, dp, C.c_long, lp, lp, vp]
@@ -194,6 +196,14 @@ class Tdse:
     def step_taylor(self, order, t0, dt, nsteps, obs_every=0, stream=None):
         _check(lib().tdse_step_taylor(self._h, int(order), float(t0), float(dt), int(nsteps), int(obs_every),
                                       _stream(stream)), "tdse_step_taylor")
+
+    def step_imag(self, order, dt, nsteps, stream=None):
+        """Imaginary-time propagation with re-normalisation; returns the energy estimates [nsteps][batch]."""
+        _check(lib().tdse_step_imag(self._h, int(order), float(dt), int(nsteps), _stream(stream)), "tdse_step_imag")
+        en = np.zeros((max(int(nsteps), 1), self.grid.batch))
+        _check(lib().tdse_energy_log(self._h, en.ctypes.data_as(C.POINTER(C.c_double)), int(nsteps), _stream(stream)),
+               "tdse_energy_log")
+        return en[:int(nsteps)]
 
     def step_rk4(self, t0, dt, nsteps, obs_every=0, stream=None):
         _check(lib().tdse_step_rk4(self._h, float(t0), float(dt), int(nsteps), int(obs_every), _stream(stream)),

@@ -95,6 +95,8 @@ struct tdse_handle {
     RtPlan rtp{}; int rt_variant = -1;
     RpPlan rpp{}; int n_sm = 148; int rp_variant = -1, rp_tma = -1;
     int rk4_block = 1, rk4_fused = 0;       // option: fuse the four RK4 stages; what the last tdse_step_rk4 used
+    int imag = 0;                           // the running Taylor call is an imaginary-time propagation
+    double *d_elog = nullptr, *d_imag_inv = nullptr; size_t elog_cap = 0; long elog_rows = 0;
 };
 
 namespace {
@@ -198,10 +200,26 @@ int init_ctl(tdse_handle *h, const CtlInit &v, cudaStream_t s) {
 // Each enqueue_* function enqueues `n` consecutive steps (reading t0, dt and the step counter from the device
 // control block) and ends by advancing the counter; it is either captured into a graph or run eagerly.
 
+// imaginary time: E and 1/||psi|| of the step just taken, then psi *= 1/||psi||
+int enqueue_imag_norm(tdse_handle *h, double2 *psi, int step_off, cudaStream_t s) {
+    OpImagNorm on{};
+    on.psi = psi; on.ctl = h->d_ctl; on.step_off = step_off; on.batch = h->grid.batch; on.dr = h->grid.dr;
+    on.elog = h->d_elog; on.inv = h->d_imag_inv;
+    RC(launch_ew(h, on, s));
+    OpScaleMember sc{};
+    sc.psi = psi; sc.inv = h->d_imag_inv;
+    RC(launch_ew(h, sc, s));
+    return TDSE_OK;
+}
+
 int enqueue_taylor_block(tdse_handle *h, int order, int n, int obs, cudaStream_t s) {
     const int B = h->grid.batch;
-    field_table_kernel<<<(n * B + 255) / 256, 256, 0, s>>>(h->d_ctl, h->d_pulse, B, n, 0, h->d_etab);
-    count(h);
+    if (h->imag) {
+        CU(cudaMemsetAsync(h->d_etab, 0, sizeof(double) * (size_t)n * B, s));       // no field
+    } else {
+        field_table_kernel<<<(n * B + 255) / 256, 256, 0, s>>>(h->d_ctl, h->d_pulse, B, n, 0, h->d_etab);
+        count(h);
+    }
     double2 *psi = h->pool[h->psi_slot];
     // scratch: three further pool slots
     int sl[3], c = 0;
@@ -216,13 +234,14 @@ int enqueue_taylor_block(tdse_handle *h, int order, int n, int obs, cudaStream_t
             else if (h->taylor_blocked_last == 2) RC(launch_taylor_rt(h->gd, h->rtp, src, dst, ef, &h->d_ctl->dt, order, s));
             else RC(launch_taylor_blocked(h->bcfg, h->gd, src, dst, ef, &h->d_ctl->dt, order, s));
             count(h);
+            if (h->imag) RC(enqueue_imag_norm(h, dst, i, s));
             if (obs) RC(enqueue_obs(h, dst, i, 1, 0, 0.0, h->d_rows, s));
             continue;
         }
         for (int k = 1; k <= order; ++k) {
             EpiTaylor e{};
             e.in = (k == 1) ? psi : ((k & 1) ? tb : ta);       // term_{k-1}: k-1 odd -> ta, even -> tb
-            e.ef = ef; e.dtp = &h->d_ctl->dt; e.k = k; e.first = (k == 1); e.write_term = (k < order);
+            e.ef = ef; e.dtp = &h->d_ctl->dt; e.k = k; e.first = (k == 1); e.write_term = (k < order); e.imag = h->imag;
             e.term_out = (k & 1) ? ta : tb;
             e.acc_in = acc;
             e.acc_out = (k == order && order > 1) ? psi : acc;  // the last order reads acc point-wise: write psi in place
@@ -232,6 +251,7 @@ int enqueue_taylor_block(tdse_handle *h, int order, int n, int obs, cudaStream_t
             OpCopy cp{}; cp.dst = psi; cp.src = acc;
             RC(launch_ew(h, cp, s));
         }
+        if (h->imag) RC(enqueue_imag_norm(h, psi, i, s));
         if (obs) RC(enqueue_obs(h, psi, i, 1, 0, 0.0, h->d_rows, s));
     }
     if (h->taylor_blocked_last && (n & 1)) {   // odd eager remainder: bring the state back into the psi slot
@@ -434,7 +454,7 @@ int run_blocks(tdse_handle *h, int kind, int p1, int p2, int n, int obs, long nb
         }
         return TDSE_OK;
     }
-    const auto key = std::make_tuple(kind, p1, p2, n, obs + 2 * h->taylor_blocked_last + 16 * (h->rtp.variant + 1) + 256 * (h->rpp.variant + 1) + 8192 * h->rpp.tma + 16384 * h->rk4_fused, h->psi_slot);
+    const auto key = std::make_tuple(kind, p1, p2, n, obs + 2 * h->taylor_blocked_last + 16 * (h->rtp.variant + 1) + 256 * (h->rpp.variant + 1) + 8192 * h->rpp.tma + 16384 * h->rk4_fused + 32768 * h->imag, h->psi_slot);
     auto it = h->graphs.find(key);
     if (it == h->graphs.end()) {
         cudaGraph_t g = nullptr;
@@ -583,7 +603,7 @@ void tdse_destroy(tdse_handle *h) {
     free_graphs(h);
     for (double2 *p : h->pool) cudaFree(p);
     void *ptrs[] = {h->d_vj, h->d_cen, h->d_cl, h->d_pulse, h->d_bufs, h->d_ctl, h->d_etab, h->d_eapply, h->d_partials,
-                    h->d_counter, h->d_phi, h->d_lstate, h->d_obs_partials, h->d_obs_counters, h->d_amp, h->d_rows, h->d_row_direct,
+                    h->d_counter, h->d_phi, h->d_lstate, h->d_obs_partials, h->d_obs_counters, h->d_elog, h->d_imag_inv, h->d_amp, h->d_rows, h->d_row_direct,
                     h->d_dtlog, h->d_errlog, h->d_replay, h->d_alpha, h->d_beta, h->d_nrm, h->d_inv, h->d_coef,
                     h->d_m, h->d_nsub, h->d_basis};
     for (void *p : ptrs) if (p) cudaFree(p);
@@ -678,8 +698,38 @@ int tdse_apply_H(tdse_handle *h, const void *psi_dev, void *out_dev, const doubl
     return TDSE_OK;
 }
 
+static int step_taylor_impl(tdse_handle *h, int order, double t0, double dt, long nsteps, int obs_every, void *stream);
+
 int tdse_step_taylor(tdse_handle *h, int order, double t0, double dt, long nsteps, int obs_every, void *stream) {
     if (!h || order < 1 || order > 64 || nsteps < 0 || obs_every < 0 || !(dt == dt)) return TDSE_ERR_ARG;
+    h->imag = 0;
+    return step_taylor_impl(h, order, t0, dt, nsteps, obs_every, stream);
+}
+
+int tdse_step_imag(tdse_handle *h, int order, double dt, long nsteps, void *stream) {
+    if (!h || order < 1 || order > 64 || nsteps < 0 || !(dt > 0.0)) return TDSE_ERR_ARG;
+    const size_t need = (size_t)std::max(1L, nsteps) * h->grid.batch;
+    RC(ensure_buf(h, &h->d_elog, &h->elog_cap, need));
+    if (!h->d_imag_inv) CU(cudaMalloc(&h->d_imag_inv, sizeof(double) * h->grid.batch));
+    h->imag = 1;
+    const int rc = step_taylor_impl(h, order, 0.0, dt, nsteps, 0, stream);
+    h->imag = 0;
+    if (rc == TDSE_OK) h->elog_rows = nsteps;
+    return rc;
+}
+
+int tdse_energy_log(tdse_handle *h, double *energy_host, long max_rows, void *stream) {
+    if (!h || !energy_host || max_rows < 0) return TDSE_ERR_ARG;
+    const long rows = std::min(max_rows, h->elog_rows);
+    if (rows > 0) {
+        CU(cudaMemcpyAsync(energy_host, h->d_elog, sizeof(double) * rows * h->grid.batch, cudaMemcpyDeviceToHost,
+                           (cudaStream_t)stream));
+        CU(cudaStreamSynchronize((cudaStream_t)stream));
+    }
+    return TDSE_OK;
+}
+
+static int step_taylor_impl(tdse_handle *h, int order, double t0, double dt, long nsteps, int obs_every, void *stream) {
     RC(ensure_pool(h, 4));
     // taylor_block: 0 one kernel per order; 1 auto (persistent register patches, else register tiles, else
     // shared-memory tile, else per order); 2 shared-memory tile kernel only; 3 register-tile kernel (v2) only;
@@ -689,14 +739,14 @@ int tdse_step_taylor(tdse_handle *h, int order, double t0, double dt, long nstep
     h->rtp = RtPlan{};
     h->rpp = RpPlan{};
     if (h->taylor_block == 1 || h->taylor_block == 4) {
-        h->rpp = rp_plan(h->grid, order, h->n_sm, h->rp_variant, h->rp_tma);
+        h->rpp = rp_plan(h->grid, order, h->n_sm, h->rp_variant, h->rp_tma, h->imag ? 2 : 0);
         if (h->rpp.ok) h->taylor_blocked_last = 3;
     }
-    if (!h->taylor_blocked_last && (h->taylor_block == 1 || h->taylor_block == 3)) {
+    if (!h->taylor_blocked_last && !h->imag && (h->taylor_block == 1 || h->taylor_block == 3)) {
         h->rtp = rt_plan(h->grid, order, h->rt_variant);
         if (h->rtp.ok) h->taylor_blocked_last = 2;
     }
-    if (!h->taylor_blocked_last && (h->taylor_block == 1 || h->taylor_block == 2) && blocked_supported(h->bcfg, order))
+    if (!h->taylor_blocked_last && !h->imag && (h->taylor_block == 1 || h->taylor_block == 2) && blocked_supported(h->bcfg, order))
         h->taylor_blocked_last = 1;
     if (h->taylor_blocked_last != 2) h->rtp = RtPlan{};
     return run_fixed(h, KIND_TAYLOR, order, 0, t0, dt, nsteps, obs_every, (cudaStream_t)stream);

@@ -152,13 +152,15 @@ struct EpiApply : EpiBase {
 // One Taylor order (Eq. 37, "only one kernel"): term_k = (-i dt/k) H term_{k-1}; acc += term_k.
 struct EpiTaylor : EpiBase {
     const double2 *in; const double *ef; const double *dtp; int k, first, write_term;
+    int imag;               // 1: imaginary time (-i -> 1), term_k = (-dt/k) H term_{k-1}
     double2 *term_out; const double2 *acc_in; double2 *acc_out;
     double s;
     __device__ __forceinline__ void begin() { s = *dtp / (double)k; }
     __device__ __forceinline__ const double2 *input() const { return in; }
     __device__ __forceinline__ double efield(int b) const { return __ldg(ef + b); }
     __device__ __forceinline__ void point(int, int, int, size_t idx, double2 f, double2 h, double *) {
-        const double2 t = make_double2(s * h.y, -s * h.x);      // (-i s)(x + i y) = s y - i s x
+        const double2 t = imag ? make_double2(-s * h.x, -s * h.y)
+                               : make_double2(s * h.y, -s * h.x);      // (-i s)(x + i y) = s y - i s x
         if (write_term) term_out[idx] = t;
         const double2 a = first ? f : acc_in[idx];
         acc_out[idx] = cadd(a, t);
@@ -385,6 +387,32 @@ struct OpCombine : OpBase {
             acc.y += ar * x.y + ai * x.x;
         }
         psi[idx] = acc;
+    }
+};
+
+// Imaginary-time step, part 2 (Eq. 24 in reading R-G25): n2 = dr sum |psi|^2;
+// E = -ln(n2) / (2 dt) logged for the step; inv = 1/sqrt(n2) for the re-normalisation that follows.
+struct OpImagNorm : OpBase {
+    static constexpr int NRED = 1;
+    const double2 *psi; const Ctl *ctl; int step_off, batch; double dr; double *elog, *inv;
+    __device__ __forceinline__ void point(int, size_t idx, double *red) {
+        const double2 v = psi[idx];
+        red[0] += v.x * v.x + v.y * v.y;
+    }
+    __device__ __forceinline__ void finish_member(int b, const double *s) {
+        const double n2 = dr * s[0];
+        elog[(ctl->step_base + step_off) * batch + b] = -log(n2) / (2.0 * ctl->dt);
+        inv[b] = 1.0 / sqrt(n2);
+    }
+};
+
+struct OpScaleMember : OpBase {
+    double2 *psi; const double *inv;
+    __device__ __forceinline__ void point(int b, size_t idx, double *) {
+        const double s = inv[b];
+        double2 v = psi[idx];
+        v.x *= s; v.y *= s;
+        psi[idx] = v;
     }
 };
 

@@ -135,7 +135,9 @@ __device__ __forceinline__ int rp_start(int t, int W, int H, int N, int WT) {
 // t_n + h (ef[stage*batch + b]); sweep i forms k_i = -i H g_i, the next stage vector g_{i+1} = psi + a_i h k_i (psi
 // re-read from this thread's private shared-memory slots) and psi_new += b_i h k_i: 32 B/point/step over HBM instead
 // of 272 for one kernel per stage.
-template <int FD, int CP, int NWR, int NWC, bool MASK, int MINB, bool TMA, bool CLUSTER, bool RK = false>
+// MODE: 0 Taylor in real time, 1 classic RK4 (above), 2 Taylor in IMAGINARY time (-i -> 1, weights
+// (-dt c1)^k / k!; the caller re-normalises).
+template <int FD, int CP, int NWR, int NWC, bool MASK, int MINB, bool TMA, bool CLUSTER, int MODE = 0>
 __global__ void __launch_bounds__(NWR * NWC * 32, MINB)
 taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict__ out, const double *__restrict__ ef,
                  const double *__restrict__ dtp, int order, int W, int H, int n_tiles, int n_items,
@@ -145,6 +147,7 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
     using G = RpGeom<FD, CP, NWR, NWC>;
     constexpr int RP = kRpRows, WT = G::WT, HW = G::HW;
     extern __shared__ __align__(1024) unsigned char rp_smem_raw[];
+    constexpr bool RK = (MODE == 1), IMAG = (MODE == 2);
     using Smem = RpSmem<FD, CP, NWR, NWC, TMA, RK>;
     Smem &sm = *reinterpret_cast<Smem *>(rp_smem_raw);     // dynamic shared memory starts 1024-byte aligned
     if (TMA && (smem_u32(rp_smem_raw) & 1023u)) __trap();
@@ -365,7 +368,8 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                 }
                 // acc += (-i)^k (dt c1)^k / k! * u'_k; s carries the sign: odd k: -+i, even k: -+1
                 // (order 1 starts the sum from psi itself: A = u_0 + ..., no separate copy)
-                if (first) { A[r][q].x = fma(s, hy, f.x); A[r][q].y = fma(-s, hx, f.y); }
+                if (first && odd) { A[r][q].x = fma(s, hy, f.x); A[r][q].y = fma(-s, hx, f.y); }
+                else if (first) { A[r][q].x = fma(s, hx, f.x); A[r][q].y = fma(s, hy, f.y); }
                 else if (odd) { A[r][q].x = fma(s, hy, A[r][q].x); A[r][q].y = fma(-s, hx, A[r][q].y); }
                 else { A[r][q].x = fma(s, hx, A[r][q].x); A[r][q].y = fma(s, hy, A[r][q].y); }
             }
@@ -442,6 +446,20 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
             sweep(T, U, 3, true, false, kappa * (1.0 / 3.0), kappa);
             set_field(3);
             sweep(U, T, 4, true, false, kappa * (1.0 / 6.0), 0.0);
+        } else if (IMAG) {
+            double sk = -kappa;                                   // every order is "even": real weights (-kappa)^k / k!
+            sweep(T, U, 1, false, true, sk, 0.0);
+            int k = 2;
+            for (; k + 1 <= order; k += 2) {
+                sk = sk * (-kappa * kRpInvK[k]);
+                sweep(U, T, k, false, false, sk, 0.0);
+                sk = sk * (-kappa * kRpInvK[k + 1]);
+                sweep(T, U, k + 1, false, false, sk, 0.0);
+            }
+            if (k <= order) {
+                sk = sk * (-kappa * kRpInvK[k]);
+                sweep(U, T, k, false, false, sk, 0.0);
+            }
         } else {
             double sk = kappa;
             sweep(T, U, 1, true, true, sk, 0.0);                  // order 1: -i
@@ -508,7 +526,7 @@ inline int rp_init_tables() {
     return cudaMemcpyToSymbol(kRpInvK, h, sizeof(h)) == cudaSuccess ? TDSE_OK : TDSE_ERR_CUDA;
 }
 
-struct RpPlan { int ok, variant, tma, cl, rk, W, H, WT, n_tiles, n_items, grid, threads; };   // cl: CTAs per cluster (1: none)
+struct RpPlan { int ok, variant, tma, cl, rk, W, H, WT, n_tiles, n_items, grid, threads; };   // rk = kernel MODE (0, 1, 2)   // cl: CTAs per cluster (1: none)
 
 // use_tma: -1 heuristic, 0 never, 1 whenever the layout allows it (n_r % 8 == 0, a full tile, 4-column patches)
 // rk: plan the fused RK4 step (order = 4 sweeps; only the one-warp-wide 16-point instantiations, full tiles)
@@ -623,6 +641,24 @@ inline int rp_launch_kernel(K kern, bool *attr_set, int smem, const RpPlan &p, c
                ? TDSE_OK : TDSE_ERR_CUDA;
 }
 
+// MODE 1 / 2 instantiations exist only for the one-warp-wide 16-point variants (RKABLE) and full tiles
+template <int FD, int CP, int NWR, int NWC, int MINB, bool CLUSTERABLE, bool RKABLE, int MODE>
+inline int rp_launch_mode(const GridDev &g, const RpPlan &p, bool mask, const CUtensorMap *tm, const double2 *in,
+                          double2 *out, const double *ef, const double *dtp, int order, cudaStream_t s) {
+    if (!RKABLE || mask) return TDSE_ERR_UNSUPPORTED;
+    constexpr int kM = RKABLE ? MODE : 0;
+    constexpr bool kCl = CLUSTERABLE && RKABLE, kT = (CP == 4) && RKABLE;
+    static bool attr[4] = {false, false, false, false};
+    const int sm_t = (int)sizeof(RpSmem<FD, CP, NWR, NWC, kT, kM == 1>), sm_n = (int)sizeof(RpSmem<FD, CP, NWR, NWC, false, kM == 1>);
+    if (p.cl > 1) {
+        if (!kCl) return TDSE_ERR_UNSUPPORTED;
+        if (p.tma) return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, kT, kCl, kM>, &attr[3], sm_t, p, s, g, in, out, ef, dtp, order, *tm);
+        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, kCl, kM>, &attr[2], sm_n, p, s, g, in, out, ef, dtp, order, *tm);
+    }
+    if (p.tma) return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, kT, false, kM>, &attr[1], sm_t, p, s, g, in, out, ef, dtp, order, *tm);
+    return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, false, kM>, &attr[0], sm_n, p, s, g, in, out, ef, dtp, order, *tm);
+}
+
 template <int FD, int CP, int NWR, int NWC, int MINB, bool CLUSTERABLE, bool RKABLE>
 inline int rp_launch_one(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
                          const double *dtp, int order, cudaStream_t s) {
@@ -637,19 +673,8 @@ inline int rp_launch_one(const GridDev &g, const RpPlan &p, const double2 *in, d
         tm = rp_tensor_map(in, g.n_r, g.batch * g.n_l, kRpRows * NWR, 32 * CP * NWC);
         if (!tm) return TDSE_ERR_CUDA;
     }
-    if (p.rk) {
-        if (!RKABLE || mask) return TDSE_ERR_UNSUPPORTED;
-        constexpr bool kRk = RKABLE, kCl = CLUSTERABLE && RKABLE, kT = kTma && RKABLE;
-        static bool rk_attr[4] = {false, false, false, false};
-        const int sm_t = (int)sizeof(RpSmem<FD, CP, NWR, NWC, kT, kRk>), sm_n = (int)sizeof(RpSmem<FD, CP, NWR, NWC, false, kRk>);
-        if (p.cl > 1) {
-            if (!kCl) return TDSE_ERR_UNSUPPORTED;
-            if (p.tma) return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, kT, kCl, kRk>, &rk_attr[3], sm_t, p, s, g, in, out, ef, dtp, order, *tm);
-            return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, kCl, kRk>, &rk_attr[2], sm_n, p, s, g, in, out, ef, dtp, order, *tm);
-        }
-        if (p.tma) return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, kT, false, kRk>, &rk_attr[1], sm_t, p, s, g, in, out, ef, dtp, order, *tm);
-        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, false, kRk>, &rk_attr[0], sm_n, p, s, g, in, out, ef, dtp, order, *tm);
-    }
+    if (p.rk == 1) return rp_launch_mode<FD, CP, NWR, NWC, MINB, CLUSTERABLE, RKABLE, 1>(g, p, mask, tm, in, out, ef, dtp, order, s);
+    if (p.rk == 2) return rp_launch_mode<FD, CP, NWR, NWC, MINB, CLUSTERABLE, RKABLE, 2>(g, p, mask, tm, in, out, ef, dtp, order, s);
     if (p.cl > 1) {
         if (!CLUSTERABLE || mask) return TDSE_ERR_UNSUPPORTED;
         constexpr bool kCl = CLUSTERABLE;

@@ -401,6 +401,53 @@ def test_rk4_parity(B, case, fused):
     h.close()
 
 
+IMAG_CASES = [
+    # n_r, dr, n_l, fd, batch, order, nsteps, use_graph
+    (400, 0.2, 3, 3, 1, 4, 300, 1),        # register-patch kernel in imaginary-time mode, direct loads
+    (640, 0.1, 16, 5, 2, 6, 40, 1),        # TMA, batched, 5-point
+    (520, 0.1, 40, 3, 1, 4, 24, 0),        # cluster of 4, eager
+    (100, 0.2, 3, 5, 2, 3, 50, 1),         # narrower than a tile: one kernel per order
+]
+
+
+@pytest.mark.parametrize("case", IMAG_CASES)
+def test_imaginary_time_parity(B, case):
+    """Imaginary-time propagation: state and per-step energy estimates against the oracle."""
+    n_r, dr, n_l, fd, batch, order, nsteps, use_graph = case
+    c = wl.config("cfg5" if batch > 1 else "cfg1", n_r=n_r, dr=dr, n_l=n_l, fd_order=fd, batch=batch, order=order)
+    g, h = both(B, c)
+    h.set_option("use_graph", use_graph)
+    psi0 = wl.populated_state(c)                      # every l block populated, normalised
+    dt = 0.2 * wl.dt_eff(c, "taylor", order)          # well inside the stability interval of the real axis
+    h.set_state(psi0)
+    en = h.step_imag(order, dt, nsteps)
+    got = h.get_state()
+    ref, ren = oracle.step_imag(g, psi0, order, dt, nsteps)
+    assert (h.taylor_kernel() in (3, 4)) == (n_r >= 128)
+    assert rel_l2(got, ref) <= TOL_PSI
+    assert en.shape == ren.shape
+    assert np.max(np.abs(en - ren)) <= 1e-9 * max(1.0, float(np.max(np.abs(ren))))
+    nrm = g.dr * np.sum(np.abs(got) ** 2, axis=(1, 2))
+    assert np.max(np.abs(nrm - 1.0)) <= 1e-12
+    h.close()
+
+
+def test_imaginary_time_ground_state_energy(B):
+    """From the analytic 1s function the device propagation settles on the closed-form ground-state energy of the
+    3-point scheme, -1/(1 + sqrt(1 + dr^2)) (tests/golden/closed_form_energies.txt)."""
+    dr, n_r = 0.2, 512
+    c = wl.config("cfg1", n_r=n_r, dr=dr, n_l=2, fd_order=3, batch=1)
+    g, h = both(B, c)
+    r = dr * np.arange(1, n_r + 1)
+    psi0 = np.zeros((1, 2, n_r), dtype=np.complex128)
+    psi0[0, 0] = 2 * r * np.exp(-r)
+    psi0 /= math.sqrt(dr * np.sum(np.abs(psi0) ** 2))
+    h.set_state(psi0)
+    en = h.step_imag(4, 0.01, 6000)
+    assert abs(en[-1, 0] - (-1.0 / (1.0 + math.sqrt(1.0 + dr * dr)))) <= 1e-9
+    h.close()
+
+
 @pytest.mark.parametrize("fd,K", [(3, 16), (5, 7)])
 def test_lanczos_parity_and_internals(B, fd, K):
     c = wl.config("cfg4", n_r=700, n_l=10, fd_order=fd)
