@@ -216,3 +216,41 @@ def lanczos_internals(g, psi, e_field, krylov_dim, taylor_order, dt, beta_tol=1e
                                        _dp(coef.view(np.float64)), C.byref(n_sub))
     assert m >= 1, m
     return {"m": m, "q": q, "alpha": alpha, "beta": beta, "coef": coef, "n_sub": n_sub.value}
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Absorbing boundary and spatial yields (plain numpy; Eq. 18, Eq. 26, Eq. 27-28)
+# ---------------------------------------------------------------------------------------------------------------
+def absorber_W(g, r_b, p, dt):
+    """W(r_j) of P:146 Eq. 18, literally: (i/dt) ln{1 - cos^p[(pi/2)(1 - r/r_b)]} on r_j = j dr (complex)."""
+    r = g.dr * np.arange(1, g.n_r + 1)
+    arg = 1.0 - np.cos(0.5 * np.pi * (1.0 - r / r_b)) ** p
+    with np.errstate(divide="ignore", invalid="ignore"):
+        return (1j / dt) * np.log(arg.astype(np.complex128))
+
+
+def absorber_mask(g, r_b, p):
+    """exp(-i W dt) of Eq. 18 = 1 - cos^p[(pi/2)(1 - r/r_b)]: the factor one step of the imaginary potential
+    multiplies the wavefunction by (reading R-G26: W enters as a split step after each propagator step, which is
+    what the (i/dt) ln{...} form of Eq. 18 is built for); 0 for r >= r_b."""
+    r = g.dr * np.arange(1, g.n_r + 1)
+    m = 1.0 - np.cos(0.5 * np.pi * (1.0 - r / r_b)) ** p
+    m[r >= r_b] = 0.0
+    return m
+
+
+def step_masked(step_fn, g, psi, mask, t0, dt, nsteps):
+    """nsteps steps of `step_fn(psi, t_start, 1) -> psi`, each followed by psi *= mask (absorbing boundary)."""
+    psi = np.array(psi, dtype=np.complex128, copy=True)
+    for n in range(nsteps):
+        psi = step_fn(psi, t0 + n * dt, 1)
+        psi *= mask[None, None, :]
+    return psi
+
+
+def bound_population(g, psi, r_b):
+    """p_b = sum_l int_0^{r_b} |f_l|^2 dr (Eq. 26; rectangle rule over r_j <= r_b, reading R-G27); the spatial
+    ionisation yield is p_i = 1 - p_b (Eq. 27-28) when no absorber removes norm."""
+    r = g.dr * np.arange(1, g.n_r + 1)
+    psi = np.asarray(psi).reshape(g.batch, g.n_l, g.n_r)
+    return g.dr * np.sum(np.abs(psi[:, :, r <= r_b]) ** 2, axis=(1, 2))

@@ -597,3 +597,48 @@ def test_P11_imaginary_time_step_on_an_eigenvector():
             rp = sum((-w[idx] * dt) ** k / math.factorial(k) for k in range(order + 1))
             assert abs(en[0, 0] - (-math.log(rp * rp) / (2 * dt))) < 1e-11
             assert np.linalg.norm(out - psi) < 1e-11 * np.linalg.norm(psi)
+
+
+# ------------------------------------------------------------------------------------ absorber and yields (P12)
+def test_P12_absorber_mask_is_one_step_of_eq18():
+    """exp(-i W dt) with W of Eq. 18 written out literally equals the real mask 1 - cos^p(...), for any dt; the
+    limits of P:148 (no absorption at r -> 0, complete at r_b) and monotonic decrease hold."""
+    g = oracle.make_grid(500, 0.2, 2, 3)
+    for r_b, p in ((100.0, 8), (80.0, 2), (100.0, 40)):
+        m = oracle.absorber_mask(g, r_b, p)
+        r = g.dr * np.arange(1, g.n_r + 1)
+        inside = r < r_b
+        for dt in (0.01, 0.3):
+            w = oracle.absorber_W(g, r_b, p, dt)
+            assert np.allclose(np.exp(-1j * w[inside] * dt), m[inside], rtol=1e-13, atol=1e-15)
+            assert np.all(w[inside].imag <= 0)                       # absorbing, never amplifying
+        assert abs(m[0] - 1.0) < (0.5 * np.pi * r[0] / r_b) ** p * 1.01 + 1e-15   # 1 - M ~ (pi r / 2 r_b)^p at small r
+        assert np.all(np.diff(m[inside]) <= 0) and m[inside][-1] < (1 - np.cos(0.5 * np.pi * g.dr / r_b) ** p) + 1e-12
+        assert np.all(m[~inside] == 0.0)
+
+
+def test_P12_absorber_removes_the_reflection_and_yields_add_up():
+    """A free-ish outgoing wavepacket in l = 3 (weak Coulomb tail) hits the wall at r_max: without absorber the norm
+    stays 1 and the packet comes back (p_b recovers); with it the outgoing flux is removed.  p_i + p_b = 1 (Eq. 28)."""
+    g = oracle.make_grid(600, 0.25, 4, 3)
+    r = g.dr * np.arange(1, g.n_r + 1)
+    psi = np.zeros((1, 4, g.n_r), dtype=np.complex128)
+    psi[0, 3] = np.exp(-(r - 60.0) ** 2 / 50.0) * np.exp(2.0j * r)           # k = 2 au outwards
+    psi /= math.sqrt(g.dr * np.sum(np.abs(psi) ** 2))
+    pulse = [(0.0, 0.057, 2.0, 0.0)]                                         # no field
+    dt, nsteps = 0.01, 9000                                                  # travels 180 au: to the wall (150) and back
+
+    def step(x, t, n):
+        return oracle.step_taylor(g, pulse, x, 8, t, dt, n)[0]
+    free = step(psi, 0.0, nsteps)
+    assert abs(g.dr * np.sum(np.abs(free) ** 2) - 1.0) < 1e-9
+    pb = oracle.bound_population(g, free, 100.0)
+    assert abs(pb[0] + (g.dr * np.sum(np.abs(free[0][:, r > 100.0]) ** 2)) - 1.0) < 1e-9   # Eq. 28
+    assert pb[0] > 0.5                                                        # reflected: back inside r < 100
+    # p = 200 confines the absorbing layer to the last tenth of the box (1 - M = cos^200 < 1e-9 for r < 0.6 r_b)
+    mask = oracle.absorber_mask(g, g.dr * (g.n_r + 1), 200)
+    early = oracle.step_masked(step, g, psi, mask, 0.0, dt, 1500)            # packet at r ~ 90: not yet in the layer
+    assert abs(g.dr * np.sum(np.abs(early) ** 2) - 1.0) < 1e-6
+    absd = oracle.step_masked(step, g, early, mask, 1500 * dt, dt, nsteps - 1500)
+    assert g.dr * np.sum(np.abs(absd) ** 2) < 0.02                            # the outgoing flux was absorbed
+    assert oracle.bound_population(g, absd, 100.0)[0] < 0.02                  # ... and did not come back
