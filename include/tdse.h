@@ -83,6 +83,13 @@ void tdse_destroy(tdse_handle *h);
  *   "rk45_check_every" [8] attempted steps enqueued between host checks of the device `done` flag */
 int  tdse_set_option(tdse_handle *h, const char *key, double value);
 
+/* Absorbing boundary (Eq. 18): W(r) = (i/dt) ln{1 - cos^p[(pi/2)(1 - r/r_b)]} enters as a split step, i.e.
+ * after every step of tdse_step_taylor / rk4 / lanczos the state is multiplied by exp(-i W(r_j) dt) =
+ * 1 - cos^p[(pi/2)(1 - r_j/r_b)] (0 for r_j >= r_b) -- the factor Eq. 18 is built to give, independent of dt (reading
+ * R-G26).  r_b <= 0 removes the absorber.  tdse_step_rk45 returns TDSE_ERR_UNSUPPORTED while one is set; the
+ * imaginary-time propagation ignores it.  Synchronises the device. */
+int  tdse_set_absorber(tdse_handle *h, double r_b, int p);
+
 /* One pulse per member, host array [batch]. */
 int  tdse_set_pulse(tdse_handle *h, const tdse_pulse *per_member_host);
 
@@ -135,6 +142,10 @@ int  tdse_step_rk45(tdse_handle *h, double t0, double t_end, double dt_init, dou
  *   <z''> = -E(t) - 2 Z dr sum_l c_l sum_j r_j^-2 Re(conj f_{l,j} f_{l+1,j})                  (Eq. 36)
  * tdse_observables: current state, field taken at time t; out_host: [batch][3 + n_states]; synchronises. */
 int  tdse_observables(tdse_handle *h, double t, double *out_host, void *stream);
+/* Bound population by spatial integration, out_host [batch]: p_b = sum_l int_0^{r_b} |f_l|^2 dr (Eq. 26,
+ * rectangle rule over r_j <= r_b, reading R-G27); the spatial ionisation yield is p_i = 1 - p_b (Eq. 27-28),
+ * plus the norm lost to an absorber.  Synchronises `stream`. */
+int  tdse_bound_population(tdse_handle *h, double r_b, double *out_host, void *stream);
 /* Rows logged by the last step call: out_host [rows][batch][3+n_states]; at most max_rows row blocks are
  * copied, *rows = number logged.  Synchronises the device.  TDSE_ERR_NONFINITE if a logged norm is not finite. */
 int  tdse_obs_log(tdse_handle *h, double *out_host, long max_rows, long *rows);

@@ -17,7 +17,7 @@ ERRORS = {-1: "TDSE_ERR_ARG", -2: "TDSE_ERR_ALLOC", -3: "TDSE_ERR_CUDA", -4: "TD
 
 # every symbol include/tdse.h declares
 SYMBOLS = ["tdse_create", "tdse_destroy", "tdse_set_option", "tdse_set_pulse", "tdse_set_bound_states",
-           "tdse_set_state", "tdse_get_state", "tdse_apply_H", "tdse_step_taylor", "tdse_step_imag", "tdse_energy_log", "tdse_step_rk4",
+           "tdse_set_state", "tdse_get_state", "tdse_apply_H", "tdse_set_absorber", "tdse_bound_population", "tdse_step_taylor", "tdse_step_imag", "tdse_energy_log", "tdse_step_rk4",
            "tdse_step_lanczos", "tdse_step_rk45", "tdse_observables", "tdse_obs_log", "tdse_dt_log",
            "tdse_lanczos_info", "tdse_launch_count", "tdse_taylor_was_blocked", "tdse_strerror", "tdse_version"]
 
@@ -60,6 +60,8 @@ def lib():
         L.tdse_apply_H.argtypes = [vp, vp, vp, dp, vp]
         L.tdse_step_taylor.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_long, C.c_int, vp]
         L.tdse_step_imag.argtypes = [vp, C.c_int, C.c_double, C.c_long, vp]
+        L.tdse_set_absorber.argtypes = [vp, C.c_double, C.c_int]
+        L.tdse_bound_population.argtypes = [vp, C.c_double, C.POINTER(C.c_double), vp]
         L.tdse_energy_log.argtypes = [vp, C.POINTER(C.c_double), C.c_long, vp]
         L.tdse_step_rk4.argtypes = [vp, C.c_double, C.c_double, C.c_long, C.c_int, vp]
         L.tdse_step_lanczos.argtypes = [vp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_long, C.c_int, vp]
@@ -196,6 +198,15 @@ class Tdse:
     def step_taylor(self, order, t0, dt, nsteps, obs_every=0, stream=None):
         _check(lib().tdse_step_taylor(self._h, int(order), float(t0), float(dt), int(nsteps), int(obs_every),
                                       _stream(stream)), "tdse_step_taylor")
+
+    def set_absorber(self, r_b, p):
+        _check(lib().tdse_set_absorber(self._h, float(r_b), int(p)), "tdse_set_absorber")
+
+    def bound_population(self, r_b, stream=None):
+        out = np.zeros(self.grid.batch)
+        _check(lib().tdse_bound_population(self._h, float(r_b), out.ctypes.data_as(C.POINTER(C.c_double)),
+                                           _stream(stream)), "tdse_bound_population")
+        return out
 
     def step_imag(self, order, dt, nsteps, stream=None):
         """Imaginary-time propagation with re-normalisation; returns the energy estimates [nsteps][batch]."""

@@ -96,6 +96,7 @@ struct tdse_handle {
     RpPlan rpp{}; int n_sm = 148; int rp_variant = -1, rp_tma = -1;
     int rk4_block = 1, rk4_fused = 0;       // option: fuse the four RK4 stages; what the last tdse_step_rk4 used
     int imag = 0;                           // the running Taylor call is an imaginary-time propagation
+    double *d_mask = nullptr; double *d_pb = nullptr;   // absorber mask [n_r] (or null), bound populations [batch]
     double *d_elog = nullptr, *d_imag_inv = nullptr; size_t elog_cap = 0; long elog_rows = 0;
 };
 
@@ -200,6 +201,14 @@ int init_ctl(tdse_handle *h, const CtlInit &v, cudaStream_t s) {
 // Each enqueue_* function enqueues `n` consecutive steps (reading t0, dt and the step counter from the device
 // control block) and ends by advancing the counter; it is either captured into a graph or run eagerly.
 
+// absorbing boundary after a step whose kernels did not apply it themselves
+int enqueue_mask(tdse_handle *h, double2 *psi, cudaStream_t s) {
+    if (!h->d_mask) return TDSE_OK;
+    OpMask m{};
+    m.psi = psi; m.mask = h->d_mask; m.n_r = h->grid.n_r;
+    return launch_ew(h, m, s);
+}
+
 // imaginary time: E and 1/||psi|| of the step just taken, then psi *= 1/||psi||
 int enqueue_imag_norm(tdse_handle *h, double2 *psi, int step_off, cudaStream_t s) {
     OpImagNorm on{};
@@ -235,6 +244,7 @@ int enqueue_taylor_block(tdse_handle *h, int order, int n, int obs, cudaStream_t
             else RC(launch_taylor_blocked(h->bcfg, h->gd, src, dst, ef, &h->d_ctl->dt, order, s));
             count(h);
             if (h->imag) RC(enqueue_imag_norm(h, dst, i, s));
+            else if (h->taylor_blocked_last != 3) RC(enqueue_mask(h, dst, s));      // (v3 applies it in its store)
             if (obs) RC(enqueue_obs(h, dst, i, 1, 0, 0.0, h->d_rows, s));
             continue;
         }
@@ -252,6 +262,7 @@ int enqueue_taylor_block(tdse_handle *h, int order, int n, int obs, cudaStream_t
             RC(launch_ew(h, cp, s));
         }
         if (h->imag) RC(enqueue_imag_norm(h, psi, i, s));
+        else RC(enqueue_mask(h, psi, s));
         if (obs) RC(enqueue_obs(h, psi, i, 1, 0, 0.0, h->d_rows, s));
     }
     if (h->taylor_blocked_last && (n & 1)) {   // odd eager remainder: bring the state back into the psi slot
@@ -330,6 +341,7 @@ int enqueue_rk4_block(tdse_handle *h, int n, int obs, cudaStream_t s) {
             }
             RC(launch_tile(h, e, s));
         }
+        RC(enqueue_mask(h, psi, s));
         if (obs) RC(enqueue_obs(h, psi, i, 1, 0, 0.0, h->d_rows, s));
     }
     ctl_advance_kernel<<<1, 32, 0, s>>>(h->d_ctl, n);
@@ -422,6 +434,7 @@ int enqueue_lanczos_block(tdse_handle *h, int K, int order, int n, int obs, cuda
         oc.psi = psi; oc.q = basis; oc.q_stride = h->n_state; oc.coef = h->d_coef; oc.nrm = h->d_nrm; oc.sc = h->d_inv;
         oc.m_used = h->d_m; oc.K = K;
         RC(launch_ew(h, oc, s));
+        RC(enqueue_mask(h, psi, s));
         if (obs) RC(enqueue_obs(h, psi, i, 1, 0, 0.0, h->d_rows, s));
     }
     ctl_advance_kernel<<<1, 32, 0, s>>>(h->d_ctl, n);
@@ -603,7 +616,7 @@ void tdse_destroy(tdse_handle *h) {
     free_graphs(h);
     for (double2 *p : h->pool) cudaFree(p);
     void *ptrs[] = {h->d_vj, h->d_cen, h->d_cl, h->d_pulse, h->d_bufs, h->d_ctl, h->d_etab, h->d_eapply, h->d_partials,
-                    h->d_counter, h->d_phi, h->d_lstate, h->d_obs_partials, h->d_obs_counters, h->d_elog, h->d_imag_inv, h->d_amp, h->d_rows, h->d_row_direct,
+                    h->d_counter, h->d_phi, h->d_lstate, h->d_obs_partials, h->d_obs_counters, h->d_elog, h->d_imag_inv, h->d_mask, h->d_pb, h->d_amp, h->d_rows, h->d_row_direct,
                     h->d_dtlog, h->d_errlog, h->d_replay, h->d_alpha, h->d_beta, h->d_nrm, h->d_inv, h->d_coef,
                     h->d_m, h->d_nsub, h->d_basis};
     for (void *p : ptrs) if (p) cudaFree(p);
@@ -799,6 +812,7 @@ int tdse_step_lanczos(tdse_handle *h, int K, int order, double t0, double dt, lo
 int tdse_step_rk45(tdse_handle *h, double t0, double t_end, double dt_init, double rtol, const double *dt_replay,
                    long n_replay, long *n_accept, long *n_reject, void *stream) {
     if (!h || !(rtol > 0.0)) return TDSE_ERR_ARG;
+    if (h->d_mask) return TDSE_ERR_UNSUPPORTED;      // the per-step mask of Eq. 18 presumes a fixed dt
     const bool replay = dt_replay != nullptr;
     if (replay ? (n_replay < 0) : (!(dt_init > 0.0) || !(t_end > t0))) return TDSE_ERR_ARG;
     cudaStream_t s = (cudaStream_t)stream;
@@ -915,6 +929,44 @@ int tdse_lanczos_info(tdse_handle *h, double *alpha, double *beta, double *coef,
 }
 
 long tdse_launch_count(tdse_handle *h) { return h ? h->launches : 0; }
+int tdse_set_absorber(tdse_handle *h, double r_b, int p) {
+    if (!h || (r_b > 0.0 && p < 1)) return TDSE_ERR_ARG;
+    CU(cudaDeviceSynchronize());
+    free_graphs(h);                                   // captured kernels hold the grid description by value
+    if (!(r_b > 0.0)) {
+        if (h->d_mask) cudaFree(h->d_mask);
+        h->d_mask = nullptr; h->gd.mask = nullptr;
+        return TDSE_OK;
+    }
+    const int N = h->grid.n_r;
+    std::vector<double> m(N);
+    for (int j = 0; j < N; ++j) {                      // exp(-i W(r_j) dt) of P:146 Eq. 18 = 1 - cos^p[(pi/2)(1 - r/r_b)]
+        const double r = (j + 1) * h->grid.dr;
+        m[j] = (r >= r_b) ? 0.0 : 1.0 - std::pow(std::cos(0.5 * 3.14159265358979323846 * (1.0 - r / r_b)), (double)p);
+    }
+    if (!h->d_mask) CU(cudaMalloc(&h->d_mask, sizeof(double) * N));
+    CU(cudaMemcpy(h->d_mask, m.data(), sizeof(double) * N, cudaMemcpyHostToDevice));
+    h->gd.mask = h->d_mask;
+    return TDSE_OK;
+}
+
+int tdse_bound_population(tdse_handle *h, double r_b, double *out_host, void *stream) {
+    if (!h || !out_host || !(r_b >= 0.0)) return TDSE_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (!h->d_pb) CU(cudaMalloc(&h->d_pb, sizeof(double) * h->grid.batch));
+    OpBoundPop op{};
+    op.psi = h->pool[h->psi_slot]; op.n_r = h->grid.n_r; op.dr = h->grid.dr; op.out = h->d_pb;
+    int jm = 0;
+    while (jm < h->grid.n_r && (jm + 1) * h->grid.dr <= r_b) ++jm;      // r_j = (j+1) dr <= r_b  (R-G27)
+    op.j_max = jm;
+    h->pending = 0;
+    RC(launch_ew(h, op, s));
+    h->launches += h->pending;
+    CU(cudaMemcpyAsync(out_host, h->d_pb, sizeof(double) * h->grid.batch, cudaMemcpyDeviceToHost, s));
+    CU(cudaStreamSynchronize(s));
+    return TDSE_OK;
+}
+
 int tdse_taylor_was_blocked(tdse_handle *h) { return h ? h->taylor_blocked_last + ((h->taylor_blocked_last == 3 && h->rpp.tma) ? 1 : 0) : 0; }
 
 }  // extern "C"

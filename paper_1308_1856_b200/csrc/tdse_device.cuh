@@ -19,6 +19,8 @@ struct GridDev {
     const double *vj;       // [n_r]  kinetic diagonal - Z/r_j          (Eq. 7, Eq. 15)
     const double *cen;      // [n_r]  1/(2 r_j^2)                       (centrifugal factor, Eq. 7)
     const double *cl;       // [n_l]  c_l = (l+1)/sqrt((2l+1)(2l+3))    (Eq. 9, m = 0)
+    const double *mask;     // [n_r]  absorbing-boundary factor exp(-i W(r_j) dt) of P:146 Eq. 18 applied after every
+                            //        step, or nullptr (no absorber)
 };
 
 // Device-resident control block: everything a captured graph must be able to re-read at launch time.

@@ -416,6 +416,30 @@ struct OpScaleMember : OpBase {
     }
 };
 
+// Absorbing boundary as a split step (Eq. 18, reading R-G26): psi_{l,j} *= mask_j after a propagator step.
+struct OpMask : OpBase {
+    double2 *psi; const double *mask; int n_r;
+    __device__ __forceinline__ void point(int, size_t idx, double *) {
+        const double m = __ldg(mask + (int)(idx % (size_t)n_r));
+        double2 v = psi[idx];
+        v.x *= m; v.y *= m;
+        psi[idx] = v;
+    }
+};
+
+// p_b = dr sum_l sum_{r_j <= r_b} |f_{l,j}|^2  (Eq. 26, reading R-G27)
+struct OpBoundPop : OpBase {
+    static constexpr int NRED = 1;
+    const double2 *psi; int n_r, j_max; double dr; double *out;     // j_max: number of radial points with r_j <= r_b
+    __device__ __forceinline__ void point(int, size_t idx, double *red) {
+        if ((int)(idx % (size_t)n_r) < j_max) {
+            const double2 v = psi[idx];
+            red[0] += v.x * v.x + v.y * v.y;
+        }
+    }
+    __device__ __forceinline__ void finish_member(int b, const double *s) { out[b] = dr * s[0]; }
+};
+
 struct OpCopy : OpBase {
     double2 *dst; const double2 *src;
     __device__ __forceinline__ void point(int, size_t idx, double *) { dst[idx] = src[idx]; }

@@ -483,6 +483,15 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
             int wint = N - t * W;
             if (wint > W) wint = W;
             double2 *dst_g = out + ((size_t)b * L + rbase) * N + start + c0;
+            if (MODE != 2 && g.mask != nullptr) {            // absorbing boundary: psi *= exp(-i W dt) (Eq. 18)
+#pragma unroll
+                for (int q = 0; q < CP; ++q) {
+                    const int jj = start + c0 + q;
+                    const double m = (jj < N) ? __ldg(g.mask + jj) : 0.0;
+#pragma unroll
+                    for (int r = 0; r < RP; ++r) { A[r][q].x *= m; A[r][q].y *= m; }
+                }
+            }
 #pragma unroll
             for (int q = 0; q < CP; q += 2) {
                 const int c = c0 + q;

@@ -448,6 +448,65 @@ def test_imaginary_time_ground_state_energy(B):
     h.close()
 
 
+ABSORBER_CASES = [
+    # propagator, n_r, n_l, fd, batch, options
+    ("taylor", 640, 16, 3, 2, {}),                       # register-patch kernel: mask applied in the store
+    ("taylor", 640, 16, 5, 1, {"taylor_block": 0}),      # one kernel per order + mask kernel
+    ("taylor", 300, 40, 3, 1, {"use_graph": 0}),         # cluster kernel, eager
+    ("rk4", 640, 9, 5, 2, {}),                           # fused RK4
+    ("rk4", 640, 9, 3, 1, {"rk4_block": 0}),             # one kernel per stage + mask kernel
+    ("lanczos", 400, 6, 3, 2, {}),
+]
+
+
+@pytest.mark.parametrize("case", ABSORBER_CASES)
+def test_absorbing_boundary_and_bound_population(B, case):
+    """Absorbing boundary of P:146 Eq. 18 as the per-step mask (R-G26) in every fixed-step propagator, and the
+    spatial bound population of Eq. 26, against the oracle."""
+    prop, n_r, n_l, fd, batch, opts = case
+    c = wl.config("cfg5" if batch > 1 else "cfg1", n_r=n_r, dr=0.1, n_l=n_l, fd_order=fd, batch=batch, order=4)
+    g, h = both(B, c)
+    for k, v in opts.items():
+        h.set_option(k, v)
+    pulses = wl.pulses(c)
+    h.set_pulse(pulses)
+    r_abs, p_abs, nsteps = g.dr * (n_r + 1), 6, 23          # p = 6: the mask is visibly below 1 on the whole box
+    h.set_absorber(r_abs, p_abs)
+    mask = oracle.absorber_mask(g, r_abs, p_abs)
+    psi0 = wl.populated_state(c)
+    dt = wl.dt_eff(c, "lanczos" if prop == "lanczos" else prop, 4)
+    t0 = wl.window(c, nsteps, dt)
+    h.set_state(psi0)
+    if prop == "taylor":
+        h.step_taylor(4, t0, dt, nsteps)
+        step = lambda x, t, n: oracle.step_taylor(g, pulses, x, 4, t, dt, n)[0]
+    elif prop == "rk4":
+        h.step_rk4(t0, dt, nsteps)
+        step = lambda x, t, n: oracle.step_rk4(g, pulses, x, t, dt, n)[0]
+    else:
+        h.step_lanczos(8, 12, t0, dt, nsteps)
+        step = lambda x, t, n: oracle.step_lanczos(g, pulses, x, 8, 12, t, dt, n)[0]
+    got = h.get_state()
+    ref = oracle.step_masked(step, g, psi0, mask, t0, dt, nsteps)
+    assert rel_l2(got, ref) <= TOL_PSI
+    nrm = g.dr * np.sum(np.abs(ref) ** 2, axis=(1, 2))
+    assert np.all(nrm < 0.999)                               # the absorber did remove norm
+    for r_b in (0.0, 7.05, 0.5 * g.dr * n_r, 1e9):
+        pb = h.bound_population(r_b)
+        assert np.max(np.abs(pb - oracle.bound_population(g, ref, r_b))) <= TOL_OBS
+    # with the absorber removed the same call is the plain propagation again
+    h.set_absorber(0.0, 0)
+    h.set_state(psi0)
+    if prop == "taylor":
+        h.step_taylor(4, t0, dt, nsteps)
+    elif prop == "rk4":
+        h.step_rk4(t0, dt, nsteps)
+    else:
+        h.step_lanczos(8, 12, t0, dt, nsteps)
+    assert rel_l2(h.get_state(), step(psi0, t0, nsteps)) <= TOL_PSI        # the unmasked propagation again
+    h.close()
+
+
 @pytest.mark.parametrize("fd,K", [(3, 16), (5, 7)])
 def test_lanczos_parity_and_internals(B, fd, K):
     c = wl.config("cfg4", n_r=700, n_l=10, fd_order=fd)
