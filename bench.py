@@ -360,6 +360,29 @@ def extra_measurements(binding, torch, stream):
                 out[f"step_{name}"].update({"algorithmic_bytes_per_point": bpp, "gbs_algorithmic": gbs,
                                             "frac_of_hbm_peak": gbs / peak})
             h.close()
+        # CFG2, second propagator: adaptive Dormand-Prince 5(4), rtol 1e-8, over a 0.05 au window at the pulse peak
+        c = wl.config("cfg2")
+        h = binding.Tdse(c["n_r"], c["dr"], c["n_l"], c["fd_order"], batch=c["batch"])
+        h.set_pulse(wl.pulses(c))
+        psi0 = wl.populated_state(c)
+        t_a = 0.5 * c["t_pulse"]
+        h.set_state(psi0, stream=stream)
+        h.step_rk45(t_a, t_a + 0.005, 1e-5, 1e-8, stream=stream)          # warm-up (graphs, controller)
+        h.set_state(psi0, stream=stream)
+        stream.synchronize()
+        tw = time.perf_counter()
+        info = h.step_rk45(t_a, t_a + 0.05, 1e-5, 1e-8, stream=stream)
+        stream.synchronize()
+        el = time.perf_counter() - tw
+        att = info["n_accept"] + info["n_reject"]
+        pts = c["batch"] * c["n_l"] * c["n_r"]
+        out["step_cfg2_rk45"] = {"propagator": "rk45 (Dormand-Prince, adaptive, rtol 1e-8)", "window_au": 0.05,
+                                 "n_accept": info["n_accept"], "n_reject": info["n_reject"],
+                                 "us_per_attempted_step": el * 1e6 / max(att, 1),
+                                 "dt_mean": float(np.mean(info["dt"])) if len(info["dt"]) else None,
+                                 "gpoint_updates_per_s": pts * 6 * att / el / 1e9,
+                                 "timing": "host wall clock (the driver polls the device controller)"}
+        h.close()
     return out
 
 

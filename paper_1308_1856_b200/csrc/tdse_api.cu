@@ -131,7 +131,7 @@ int ensure_buf(tdse_handle *h, T **p, size_t *cap, size_t need) {
 }
 
 dim3 tile_grid(const tdse_handle *h) {
-    const int tw = 128, tl = 8;
+    const int tw = Tile<3>::TW, tl = Tile<3>::TL;
     return dim3((h->grid.n_r + tw - 1) / tw, (h->grid.n_l + tl - 1) / tl, h->grid.batch);
 }
 int tile_ctas_per_member(const tdse_handle *h) { dim3 g = tile_grid(h); return (int)(g.x * g.y); }

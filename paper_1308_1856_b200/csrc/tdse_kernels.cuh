@@ -15,7 +15,10 @@ namespace tdse {
 template <int FD>
 struct Tile {
     static constexpr int HW = (FD == 3) ? 1 : 2;
-    static constexpr int TW = 128, TL = 8, NT = 256;
+#ifndef TDSE_TILE_TL
+#define TDSE_TILE_TL 8
+#endif
+    static constexpr int TW = 128, TL = TDSE_TILE_TL, NT = 256;
     static constexpr int RPT = TL / (NT / TW);          // rows per thread
     static constexpr int PITCH = TW + 2 * HW;           // double2 elements per shared row
     static constexpr int ROWS = TL + 2;
