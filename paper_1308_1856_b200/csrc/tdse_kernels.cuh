@@ -380,14 +380,21 @@ struct OpCombine : OpBase {
         const int m = m_used[b];
         const double n = nrm[b];
         double2 acc = make_double2(0.0, 0.0);
-        for (int p = 0; p < m; ++p) {
-            const double2 c = coef[b * K + p];
-            const double sp = sc[b * K + p];                    // q_p = s_p v_p
-            const double ar = n * c.x, ai = n * c.y;
-            double2 x = q[(size_t)p * q_stride + idx];
-            x.x *= sp; x.y *= sp;
-            acc.x += ar * x.x - ai * x.y;
-            acc.y += ar * x.y + ai * x.x;
+        for (int p0 = 0; p0 < m; p0 += 8) {                 // 8 basis vectors' loads in flight per point
+            double2 x[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+                x[i] = (p0 + i < m) ? __ldcs(q + (size_t)(p0 + i) * q_stride + idx) : make_double2(0.0, 0.0);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                if (p0 + i >= m) break;
+                const double2 c = coef[b * K + p0 + i];
+                const double sp = sc[b * K + p0 + i];               // q_p = s_p v_p
+                const double ar = n * c.x, ai = n * c.y;
+                const double vx = x[i].x * sp, vy = x[i].y * sp;
+                acc.x += ar * vx - ai * vy;
+                acc.y += ar * vy + ai * vx;
+            }
         }
         psi[idx] = acc;
     }
