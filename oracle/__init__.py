@@ -16,11 +16,12 @@ _lib = None
 
 class Grid(C.Structure):
     _fields_ = [("n_r", C.c_int), ("dr", C.c_double), ("n_l", C.c_int), ("fd_order", C.c_int),
-                ("z_nuc", C.c_double), ("batch", C.c_int), ("r_offset", C.c_double)]
+                ("z_nuc", C.c_double), ("batch", C.c_int), ("r_offset", C.c_double), ("gauge", C.c_int)]
 
 
 class Pulse(C.Structure):
-    _fields_ = [("e0", C.c_double), ("omega", C.c_double), ("n_cycles", C.c_double), ("cep", C.c_double)]
+    _fields_ = [("e0", C.c_double), ("omega", C.c_double), ("n_cycles", C.c_double), ("cep", C.c_double),
+                ("kind", C.c_int)]
 
 
 class Obs(C.Structure):
@@ -34,6 +35,8 @@ def lib():
         _lib = C.CDLL(_build())
         _lib.oracle_pulse_E.restype = C.c_double
         _lib.oracle_pulse_E.argtypes = [C.POINTER(Pulse), C.c_double]
+        _lib.oracle_pulse_A.restype = C.c_double
+        _lib.oracle_pulse_A.argtypes = [C.POINTER(Pulse), C.c_double]
     return _lib
 
 
@@ -41,18 +44,18 @@ def _dp(a):
     return a.ctypes.data_as(C.POINTER(C.c_double))
 
 
-def make_grid(n_r, dr, n_l, fd_order, z_nuc=1.0, batch=1, r_offset=0.0):
-    return Grid(int(n_r), float(dr), int(n_l), int(fd_order), float(z_nuc), int(batch), float(r_offset))
+def make_grid(n_r, dr, n_l, fd_order, z_nuc=1.0, batch=1, r_offset=0.0, gauge=0):
+    return Grid(int(n_r), float(dr), int(n_l), int(fd_order), float(z_nuc), int(batch), float(r_offset), int(gauge))
 
 
 def _pulses(g, pulses):
-    """pulses: iterable of (e0, omega, n_cycles, cep) per member (or one tuple for all)."""
+    """pulses: iterable of (e0, omega, n_cycles, cep[, kind]) per member (or one tuple for all)."""
     if isinstance(pulses, tuple) and not isinstance(pulses[0], (tuple, list)):
         pulses = [pulses] * g.batch
     assert len(pulses) == g.batch
     arr = (Pulse * g.batch)()
     for i, p in enumerate(pulses):
-        arr[i] = Pulse(*[float(x) for x in p])
+        arr[i] = Pulse(float(p[0]), float(p[1]), float(p[2]), float(p[3]), int(p[4]) if len(p) > 4 else 0)
     return arr
 
 
@@ -81,9 +84,19 @@ def set_threads(n):
     lib().oracle_set_threads(int(n))
 
 
+def _pulse1(pulse):
+    return Pulse(float(pulse[0]), float(pulse[1]), float(pulse[2]), float(pulse[3]), int(pulse[4]) if len(pulse) > 4 else 0)
+
+
 def pulse_E(pulse, t):
-    p = Pulse(*[float(x) for x in pulse])
+    p = _pulse1(pulse)
     return lib().oracle_pulse_E(C.byref(p), float(t))
+
+
+def pulse_A(pulse, t):
+    """A(t) with E = -dA/dt (kind 1 pulses; NaN for kind 0)."""
+    p = _pulse1(pulse)
+    return lib().oracle_pulse_A(C.byref(p), float(t))
 
 
 def coupling(n_l):

@@ -16,6 +16,11 @@
 #include <omp.h>
 #endif
 
+// the time-dependent factor of the coupling: E(t) in the length gauge, A(t) in the velocity gauge
+static double coupling_field(const oracle_grid *g, const oracle_pulse *p, double t) {
+    return g->gauge == 1 ? oracle_pulse_A(p, t) : oracle_pulse_E(p, t);
+}
+
 namespace {
 
 int g_threads = 1;
@@ -61,8 +66,29 @@ void apply_H_member(const oracle_grid *g, const double *f, double e, double *out
                 const double pot = v_eff(l, r, z) * F(j);
                 const double fm = flm ? flm[2 * (j - 1) + c] : 0.0;
                 const double fp = flp ? flp[2 * (j - 1) + c] : 0.0;
-                const double cpl = e * r * (cm * fm + cp * fp);  // P:104 Eq. 11, length gauge
+                const double cpl = (g->gauge == 1) ? 0.0 : e * r * (cm * fm + cp * fp);  // P:104 Eq. 11, length gauge
                 out[2L * l * N + 2 * (j - 1) + c] = kin + pot + cpl;
+            }
+            if (g->gauge == 1) {
+                // P:106 Eq. 12 (e = A(t); the factor 1/c is dropped) in reading R-V2:
+                //   -i A [ (d/dr - l/r) kappa_l f_{l-1} + (d/dr + (l+1)/r) kappa_{l+1} f_{l+1} ].
+                // The printed equation has the two 1/r terms with the opposite signs; d/dz applied to
+                // (f_l / r) Y_l0 gives the signs used here, and only they make the two gauges agree (pin P13).
+                // d/dr by the central formula of the stencil (Eq. 14, reading R-V1), zero outside the box
+                double s[2];
+                for (int c = 0; c < 2; ++c) {
+                    auto G = [&](const double *row, int jj) -> double {
+                        return (row && jj >= 1 && jj <= N) ? row[2 * (jj - 1) + c] : 0.0;
+                    };
+                    auto D1 = [&](const double *row) -> double {
+                        if (g->fd_order == 3) return (G(row, j + 1) - G(row, j - 1)) / (2.0 * dr);
+                        return (-G(row, j + 2) + 8.0 * G(row, j + 1) - 8.0 * G(row, j - 1) + G(row, j - 2)) / (12.0 * dr);
+                    };
+                    s[c] = cm * (D1(flm) - (l / r) * G(flm, j)) + cp * (D1(flp) + ((l + 1) / r) * G(flp, j));
+                }
+                // -i (s0 + i s1) = s1 - i s0
+                out[2L * l * N + 2 * (j - 1)] += e * s[1];
+                out[2L * l * N + 2 * (j - 1) + 1] += -e * s[0];
             }
         }
     }
@@ -175,7 +201,7 @@ void rk_step(const oracle_grid *g, const oracle_pulse *pulse, const Tableau &tb,
         }
         // k_i <- f(t_n + c_i h, g) = -i H(t_n + c_i h) g      (Eq. 17)
         for (int b = 0; b < B; ++b) {
-            const double e = oracle_pulse_E(&pulse[b], t + tb.c[i] * h);
+            const double e = coupling_field(g, &pulse[b], t + tb.c[i] * h);
             apply_H_member(g, gbuf.data() + 2 * M * b, e, hbuf.data() + 2 * M * b);
         }
         double *ki = k[i].data();
@@ -359,8 +385,24 @@ double oracle_pulse_E(const oracle_pulse *p, double t) {
     if (p->omega == 0.0) return p->e0;  // test aid: static field (frozen-H pins), not a paper pulse
     const double T = 2.0 * M_PI * p->n_cycles / p->omega;
     if (t < 0.0 || t > T) return 0.0;
-    const double s = std::sin(p->omega * t / (2.0 * p->n_cycles));
+    const double Om = p->omega / (2.0 * p->n_cycles);
+    if (p->kind == 1) {
+        // E = -dA/dt of A = -(e0/omega) sin^2(Om t) sin(omega t + cep): the expression printed at P:188 with the
+        // normalisation 1/omega_0 restored (reading R-V3)
+        const double s = std::sin(Om * t), c = std::cos(Om * t), ph = p->omega * t + p->cep;
+        return (p->e0 / p->omega) * s * (2.0 * Om * c * std::sin(ph) + p->omega * s * std::cos(ph));
+    }
+    const double s = std::sin(Om * t);
     return p->e0 * s * s * std::cos(p->omega * t + p->cep);
+}
+
+double oracle_pulse_A(const oracle_pulse *p, double t) {
+    if (p->omega == 0.0) return p->e0;  // test aid: static vector potential
+    if (p->kind != 1) return std::nan("");
+    const double T = 2.0 * M_PI * p->n_cycles / p->omega;
+    if (t < 0.0 || t > T) return 0.0;
+    const double s = std::sin(p->omega * t / (2.0 * p->n_cycles));
+    return -(p->e0 / p->omega) * s * s * std::sin(p->omega * t + p->cep);
 }
 
 void oracle_coupling(int n_l, double *c) { for (int l = 0; l < n_l; ++l) c[l] = coupling(l); }
@@ -480,7 +522,7 @@ int oracle_step_taylor(const oracle_grid *g, const oracle_pulse *pulse, double *
         const double ts = field_sample == 1 ? t0 + n * dt : t0 + (n + 0.5) * dt;  // reading R-G7
         for (int b = 0; b < g->batch; ++b) {
             double *f = psi + 2 * M * b;
-            const double e = oracle_pulse_E(&pulse[b], ts);
+            const double e = coupling_field(g, &pulse[b], ts);
             // F^(0) = F_n; F^(k) = (-i dt/k) H F^(k-1); F_{n+1} = sum_k F^(k)   (Eq. 37)
             std::memcpy(term.data(), f, sizeof(double) * 2 * M);
             for (int k = 1; k <= order; ++k) {
@@ -625,7 +667,7 @@ int oracle_step_lanczos(const oracle_grid *g, const oracle_pulse *pulse, double 
         const double ts = field_sample == 1 ? t0 + n * dt : t0 + (n + 0.5) * dt;
         for (int b = 0; b < g->batch; ++b) {
             int n_sub;
-            lanczos_member(g, psi + 2 * M * b, oracle_pulse_E(&pulse[b], ts), krylov_dim, taylor_order,
+            lanczos_member(g, psi + 2 * M * b, coupling_field(g, &pulse[b], ts), krylov_dim, taylor_order,
                            dt, beta_tol, q, w, alpha.data(), beta.data(), coef.data(), &n_sub);
         }
         if (obs && obs->obs_every > 0 && (n + 1) % obs->obs_every == 0)

@@ -39,15 +39,21 @@ typedef struct {
     double z_nuc;     /* V(r) = -z_nuc / r                            */
     int    batch;     /* B independent members                               */
     double r_offset;  /* the paper's grid `Offset`; 0 normally   */
+    int    gauge;     /* 0 length gauge (Eq. 11), 1 velocity gauge (Eq. 12) */
 } oracle_grid;
 
-typedef struct {      /* E(t) = e0 sin^2(omega t/(2 n_c)) cos(omega t + cep) */
+typedef struct {      /* kind 0: E(t) = e0 sin^2(omega t/(2 n_c)) cos(omega t + cep) */
     double e0, omega, n_cycles, cep;   /* on 0 <= t <= 2 pi n_c/omega, else 0 (Eq. 19);
                                           omega == 0: static field E(t) = e0 (test aid)              */
+    int kind;         /* 1: the Hann shape is on the vector potential (reading R-V3):
+                         A(t) = -(e0/omega) sin^2(omega t/(2 n_c)) sin(omega t + cep), E(t) = -dA/dt  */
 } oracle_pulse;
 
 /* --- pieces of H ------------------------------------------------------- */
 double oracle_pulse_E(const oracle_pulse *p, double t);
+/* A(t) with E = -dA/dt (Eq. 20 with the factor c dropped as in P:182); defined for kind 1 pulses and for the
+ * static test aid (omega == 0: A = e0); NaN for kind 0 (the running quadrature of P:180 is not implemented). */
+double oracle_pulse_A(const oracle_pulse *p, double t);
 /* c[l] = (l+1)/sqrt((2l+1)(2l+3)), l = 0..n_l-1: k_{l,l+1}(m=0) of P:94 Eq. 9 */
 void   oracle_coupling(int n_l, double *c);
 

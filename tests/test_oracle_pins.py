@@ -642,3 +642,95 @@ def test_P12_absorber_removes_the_reflection_and_yields_add_up():
     absd = oracle.step_masked(step, g, early, mask, 1500 * dt, dt, nsteps - 1500)
     assert g.dr * np.sum(np.abs(absd) ** 2) < 0.02                            # the outgoing flux was absorbed
     assert oracle.bound_population(g, absd, 100.0)[0] < 0.02                  # ... and did not come back
+
+
+# ------------------------------------------------------------------------------------ velocity gauge (P13, NEXT f1)
+def _dense_velocity_H(n_r, dr, n_l, fd, a_field):
+    """H of P:106 Eq. 12 (1/r terms in reading R-V2) built entry by entry in numpy, independently of the oracle."""
+    r = dr * np.arange(1, n_r + 1)
+    n = n_r * n_l
+    h = np.zeros((n, n), dtype=np.complex128)
+    if fd == 3:
+        d2 = {0: -2.0, 1: 1.0, -1: 1.0}; s2 = 1.0 / dr ** 2
+        d1 = {1: 1.0, -1: -1.0}; s1 = 1.0 / (2 * dr)
+    else:
+        d2 = {0: -30.0, 1: 16.0, -1: 16.0, 2: -1.0, -2: -1.0}; s2 = 1.0 / (12 * dr ** 2)
+        d1 = {1: 8.0, -1: -8.0, 2: -1.0, -2: 1.0}; s1 = 1.0 / (12 * dr)
+    kap = lambda l: l / math.sqrt(4.0 * l * l - 1.0) if l > 0 else 0.0     # kappa_l = k_{l,l-1}(m = 0), P:94 Eq. 9
+    for l in range(n_l):
+        for j in range(n_r):
+            row = l * n_r + j
+            for k, w in d2.items():
+                if 0 <= j + k < n_r:
+                    h[row, l * n_r + j + k] += -0.5 * w * s2
+            h[row, row] += l * (l + 1) / (2 * r[j] ** 2) - 1.0 / r[j]
+            for lp, kp, sgn in ((l - 1, kap(l), -l), (l + 1, kap(l + 1), +(l + 1))):      # reading R-V2
+                if 0 <= lp < n_l:
+                    for k, w in d1.items():
+                        if 0 <= j + k < n_r:
+                            h[row, lp * n_r + j + k] += -1j * a_field * kp * w * s1
+                    h[row, lp * n_r + j] += -1j * a_field * kp * sgn / r[j]
+    return h
+
+
+@pytest.mark.parametrize("fd", [3, 5])
+def test_P13_velocity_gauge_operator(fd):
+    """The oracle's matrix-free velocity-gauge H equals the dense matrix written out from Eq. 12 / Eq. 14 column by
+    column, is Hermitian, and reduces to the field-free h_l at A = 0."""
+    n_r, dr, n_l, a = 14, 0.2, 4, 0.37
+    g = oracle.make_grid(n_r, dr, n_l, fd, gauge=1)
+    h = _dense_velocity_H(n_r, dr, n_l, fd, a)
+    assert np.max(np.abs(h - h.conj().T)) < 1e-12
+    cols = np.zeros((n_r * n_l, n_r * n_l), dtype=np.complex128)
+    for c in range(n_r * n_l):
+        e = np.zeros(n_r * n_l, dtype=np.complex128); e[c] = 1.0
+        cols[:, c] = oracle.apply_H(g, e.reshape(1, n_l, n_r), a).ravel()
+    assert np.max(np.abs(cols - h)) < 1e-12 * np.max(np.abs(h))
+    x = rand_state((1, n_l, n_r), 77)
+    g0 = oracle.make_grid(n_r, dr, n_l, fd, gauge=0)
+    assert np.max(np.abs(oracle.apply_H(g, x, 0.0) - oracle.apply_H(g0, x, 0.0))) == 0.0
+
+
+def test_P13_velocity_gauge_propagators_against_dense_exponential():
+    """Static A (test aid): Taylor, RK4 and Lanczos steps against scipy's expm of the independently built dense H."""
+    n_r, dr, n_l, a, dt = 40, 0.2, 3, 0.25, 0.004
+    g = oracle.make_grid(n_r, dr, n_l, 5, gauge=1)
+    u = sla.expm(-1j * dt * _dense_velocity_H(n_r, dr, n_l, 5, a))
+    psi = rand_state((1, n_l, n_r), 5)
+    ref = (u @ psi.ravel()).reshape(psi.shape)
+    static = [(a, 0.0, 1.0, 0.0, 1)]
+    assert np.linalg.norm(oracle.step_taylor(g, static, psi, 14, 0.0, dt, 1)[0] - ref) < 1e-12 * np.linalg.norm(ref)
+    assert np.linalg.norm(oracle.step_lanczos(g, static, psi, 30, 14, 0.0, dt, 1)[0] - ref) < 1e-9 * np.linalg.norm(ref)
+    y = float(np.max(np.abs(np.linalg.eigvalsh(_dense_velocity_H(n_r, dr, n_l, 5, a))))) * dt
+    assert np.linalg.norm(oracle.step_rk4(g, static, psi, 0.0, dt, 1)[0] - ref) < 1.01 * y ** 5 / 120 * np.linalg.norm(ref)
+
+
+def test_P13_vector_potential_pulse_and_gauge_agreement():
+    """Kind-1 pulse (Hann shape on A, R-V3): E = -dA/dt, A vanishes at both ends, peak field ~ e0; and a
+    short pulse gives the same ground-state depletion in both gauges up to the discretisation (it differs between
+    the gauges at finite dr and l truncation; the paper quotes 0.27145 vs 0.27144 on a converged grid)."""
+    p = (0.0534, 0.057, 4.0, 0.3, 1)
+    T = 2 * math.pi * p[2] / p[1]
+    ts = np.linspace(0.01, T - 0.01, 301)
+    hh = 1e-5
+    num = np.array([-(oracle.pulse_A(p, t + hh) - oracle.pulse_A(p, t - hh)) / (2 * hh) for t in ts])
+    ana = np.array([oracle.pulse_E(p, t) for t in ts])
+    assert np.max(np.abs(num - ana)) < 1e-8
+    assert oracle.pulse_A(p, 0.0) == 0.0 and abs(oracle.pulse_A(p, T)) < 1e-15 and oracle.pulse_A(p, T + 1.0) == 0.0
+    assert 0.9 * p[0] < np.max(np.abs(ana)) <= 1.05 * p[0]
+    assert math.isnan(oracle.pulse_A((0.05, 0.057, 2.0, 0.0, 0), 1.0))          # kind 0: no A(t) (running quadrature absent)
+    # depletion of 1s by a one-cycle pulse at omega = 0.6 au (one-photon ionisation), both gauges
+    n_r, dr, n_l, dt = 400, 0.2, 6, 0.004
+    pulse = [(0.15, 0.6, 3.0, 0.0, 1)]
+    Tp = 2 * math.pi * 3.0 / 0.6
+    nsteps = int(math.ceil(Tp / dt)); dt = Tp / nsteps
+    dep = []
+    for gauge in (0, 1):
+        g = oracle.make_grid(n_r, dr, n_l, 5, gauge=gauge)
+        _, phi = oracle.bound_states(oracle.make_grid(n_r, dr, n_l, 5), 0, 1)
+        psi = np.zeros((1, n_l, n_r), dtype=np.complex128); psi[0, 0] = phi[0]
+        out, _ = oracle.step_taylor(g, pulse, psi, 4, 0.0, dt, nsteps)
+        assert abs(dr * np.sum(np.abs(out) ** 2) - 1.0) < 1e-8
+        dep.append(1.0 - abs(np.vdot(phi[0], out[0, 0]) * dr) ** 2)
+    assert dep[0] > 0.01                                                         # the pulse does ionise
+    assert abs(dep[0] - dep[1]) < 0.05 * dep[0]
