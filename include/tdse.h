@@ -38,7 +38,7 @@ extern "C" {
 #define TDSE_ERR_ALLOC       (-2)   /* host or device allocation failed                           */
 #define TDSE_ERR_CUDA        (-3)   /* CUDA runtime error (no device, launch failure)             */
 #define TDSE_ERR_NONFINITE   (-4)   /* a logged norm is NaN/Inf (unstable step size)       */
-#define TDSE_ERR_UNSUPPORTED (-5)   /* gauge != length, fd_order not 3/5, krylov_dim > 32         */
+#define TDSE_ERR_UNSUPPORTED (-5)   /* gauge not 0/1, fd_order not 3/5, krylov_dim > 32           */
 
 typedef struct tdse_handle tdse_handle;   /* opaque; owns the state, all scratch, tables and CUDA graphs */
 
@@ -47,13 +47,18 @@ typedef struct {
     double dr;        /* radial spacing                                                           */
     int    n_l;       /* number of partial-wave blocks L, l = 0..n_l-1 (`NumBlocks`)       */
     int    fd_order;  /* 3 or 5 point second derivative (Eq. 15)                            */
-    int    gauge;     /* 0 = length gauge (Eq. 11); anything else: TDSE_ERR_UNSUPPORTED     */
+    int    gauge;     /* 0 = length gauge (Eq. 11), 1 = velocity gauge (Eq. 12 in reading R-V2,
+                         first derivative of P:119 Eq. 14; needs kind-1 pulses); else TDSE_ERR_UNSUPPORTED */
     double z_nuc;     /* V(r) = -z_nuc/r                                                   */
     int    batch;     /* B >= 1 independent members sharing the grid                      */
 } tdse_grid;
 
 typedef struct {      /* E(t) = e0 sin^2(omega t/(2 n_cycles)) cos(omega t + cep) on 0 <= t <= 2 pi n_cycles/omega, */
     double e0, omega, n_cycles, cep;   /* else 0 (Eq. 19; R-G8).  omega == 0: static field e0 */
+    int kind;         /* 0: as above.  1: the Hann shape is on the vector potential (R-V3):
+                         A(t) = -(e0/omega) sin^2(omega t/(2 n_cycles)) sin(omega t + cep), E(t) = -dA/dt.
+                         The velocity gauge (tdse_grid.gauge = 1) needs kind 1 (or the static test aid omega = 0,
+                         whose e0 is then the constant A). */
 } tdse_pulse;
 
 /* Create / destroy.  tdse_create builds the device tables (diagonal of h_l, c_l) and allocates the state

@@ -34,7 +34,8 @@ class Grid(C.Structure):
 
 
 class Pulse(C.Structure):
-    _fields_ = [("e0", C.c_double), ("omega", C.c_double), ("n_cycles", C.c_double), ("cep", C.c_double)]
+    _fields_ = [("e0", C.c_double), ("omega", C.c_double), ("n_cycles", C.c_double), ("cep", C.c_double),
+                ("kind", C.c_int)]
 
 
 _lib = None
@@ -143,7 +144,7 @@ class Tdse:
         _check(lib().tdse_set_option(self._h, key.encode(), float(value)), f"tdse_set_option({key})")
 
     def set_pulse(self, pulses):
-        """pulses: one (e0, omega, n_cycles, cep) tuple for all members, or a list of batch tuples."""
+        """pulses: one (e0, omega, n_cycles, cep[, kind]) tuple for all members, or a list of batch tuples."""
         b = self.grid.batch
         if isinstance(pulses, tuple) and not isinstance(pulses[0], (tuple, list)):
             pulses = [pulses] * b
@@ -151,7 +152,7 @@ class Tdse:
             raise ValueError("need one pulse per member")
         arr = (Pulse * b)()
         for i, p in enumerate(pulses):
-            arr[i] = Pulse(*[float(x) for x in p])
+            arr[i] = Pulse(float(p[0]), float(p[1]), float(p[2]), float(p[3]), int(p[4]) if len(p) > 4 else 0)
         _check(lib().tdse_set_pulse(self._h, arr), "tdse_set_pulse")
 
     def set_bound_states(self, l_of_state, phi):

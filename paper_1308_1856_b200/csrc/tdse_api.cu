@@ -143,7 +143,10 @@ dim3 ew_grid(const tdse_handle *h) {
 template <class Epi>
 int launch_tile(tdse_handle *h, const Epi &epi, cudaStream_t s) {
     RedCtx rc{h->d_partials, h->d_counter, tile_ctas_per_member(h)};
-    if (h->grid.fd_order == 3) tile_kernel<3, Epi><<<tile_grid(h), 256, 0, s>>>(h->gd, epi, rc);
+    if (h->grid.gauge == 1) {
+        if (h->grid.fd_order == 3) tile_kernel<3, Epi, true><<<tile_grid(h), 256, 0, s>>>(h->gd, epi, rc);
+        else tile_kernel<5, Epi, true><<<tile_grid(h), 256, 0, s>>>(h->gd, epi, rc);
+    } else if (h->grid.fd_order == 3) tile_kernel<3, Epi><<<tile_grid(h), 256, 0, s>>>(h->gd, epi, rc);
     else tile_kernel<5, Epi><<<tile_grid(h), 256, 0, s>>>(h->gd, epi, rc);
     count(h);
     CU(cudaGetLastError());
@@ -226,7 +229,7 @@ int enqueue_taylor_block(tdse_handle *h, int order, int n, int obs, cudaStream_t
     if (h->imag) {
         CU(cudaMemsetAsync(h->d_etab, 0, sizeof(double) * (size_t)n * B, s));       // no field
     } else {
-        field_table_kernel<<<(n * B + 255) / 256, 256, 0, s>>>(h->d_ctl, h->d_pulse, B, n, 0, h->d_etab);
+        field_table_kernel<<<(n * B + 255) / 256, 256, 0, s>>>(h->d_ctl, h->d_pulse, B, n, 0, h->d_etab, h->gd.gauge);
         count(h);
     }
     double2 *psi = h->pool[h->psi_slot];
@@ -303,7 +306,7 @@ void fill_rk_common(tdse_handle *h, E &e, int stage, const double *ef, const dou
 
 int enqueue_rk4_block(tdse_handle *h, int n, int obs, cudaStream_t s) {
     const int B = h->grid.batch;
-    field_table_kernel<<<(n * 4 * B + 255) / 256, 256, 0, s>>>(h->d_ctl, h->d_pulse, B, n, 1, h->d_etab);
+    field_table_kernel<<<(n * 4 * B + 255) / 256, 256, 0, s>>>(h->d_ctl, h->d_pulse, B, n, 1, h->d_etab, h->gd.gauge);
     count(h);
     double2 *psi = h->pool[h->psi_slot];
     if (h->rk4_fused) {
@@ -354,7 +357,7 @@ int enqueue_rk4_block(tdse_handle *h, int n, int obs, cudaStream_t s) {
 int enqueue_rk45_block(tdse_handle *h, int n, int first_stage, cudaStream_t s) {
     const int B = h->grid.batch;
     for (int i = 0; i < n; ++i) {
-        rk45_begin_kernel<<<1, 256, 0, s>>>(h->d_ctl, h->d_pulse, B, h->d_replay, h->d_etab);
+        rk45_begin_kernel<<<1, 256, 0, s>>>(h->d_ctl, h->d_pulse, B, h->d_replay, h->d_etab, h->gd.gauge);
         count(h);
         for (int st = (i == 0 ? first_stage : 1); st < 7; ++st) {
             const double *ef = h->d_etab + (size_t)st * B;
@@ -408,7 +411,7 @@ int enqueue_rk45_block(tdse_handle *h, int n, int first_stage, cudaStream_t s) {
 // written by the same kernel (halo race).
 int enqueue_lanczos_block(tdse_handle *h, int K, int order, int n, int obs, cudaStream_t s) {
     const int B = h->grid.batch;
-    field_table_kernel<<<(n * B + 255) / 256, 256, 0, s>>>(h->d_ctl, h->d_pulse, B, n, 0, h->d_etab);
+    field_table_kernel<<<(n * B + 255) / 256, 256, 0, s>>>(h->d_ctl, h->d_pulse, B, n, 0, h->d_etab, h->gd.gauge);
     count(h);
     double2 *psi = h->pool[h->psi_slot];
     double2 *wbuf[2]; int c = 0;
@@ -545,7 +548,7 @@ int tdse_create(const tdse_grid *grid, tdse_handle **out) {
     if (!out) return TDSE_ERR_ARG;
     *out = nullptr;
     if (!grid_valid(grid)) return TDSE_ERR_ARG;
-    if (grid->gauge != 0 || (grid->fd_order != 3 && grid->fd_order != 5)) return TDSE_ERR_UNSUPPORTED;
+    if ((grid->gauge != 0 && grid->gauge != 1) || (grid->fd_order != 3 && grid->fd_order != 5)) return TDSE_ERR_UNSUPPORTED;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return TDSE_ERR_CUDA; }
     tdse_handle *h = new (std::nothrow) tdse_handle();
@@ -579,7 +582,7 @@ int tdse_create(const tdse_grid *grid, tdse_handle **out) {
         CU(cudaMemcpy(h->d_cen, cen.data(), sizeof(double) * N, cudaMemcpyHostToDevice));
         CU(cudaMemcpy(h->d_cl, cl.data(), sizeof(double) * L, cudaMemcpyHostToDevice));
         GridDev &g = h->gd;
-        g.n_r = N; g.n_l = L; g.batch = B; g.fd = grid->fd_order; g.dr = grid->dr; g.z = grid->z_nuc;
+        g.n_r = N; g.n_l = L; g.batch = B; g.fd = grid->fd_order; g.gauge = grid->gauge; g.dr = grid->dr; g.z = grid->z_nuc;
         if (grid->fd_order == 3) { g.c1 = -0.5 / dr2; g.c2 = 0.0; }
         else { g.c1 = -16.0 / (24.0 * dr2); g.c2 = 1.0 / (24.0 * dr2); }
         g.vj = h->d_vj; g.cen = h->d_cen; g.cl = h->d_cl;
@@ -751,15 +754,17 @@ static int step_taylor_impl(tdse_handle *h, int order, double t0, double dt, lon
     h->rk4_fused = 0;
     h->rtp = RtPlan{};
     h->rpp = RpPlan{};
-    if (h->taylor_block == 1 || h->taylor_block == 4) {
+    // (the all-orders-in-one-pass kernels implement the length-gauge coupling only; imaginary time has no field)
+    const bool lg = h->grid.gauge == 0 || h->imag;
+    if (lg && (h->taylor_block == 1 || h->taylor_block == 4)) {
         h->rpp = rp_plan(h->grid, order, h->n_sm, h->rp_variant, h->rp_tma, h->imag ? 2 : 0);
         if (h->rpp.ok) h->taylor_blocked_last = 3;
     }
-    if (!h->taylor_blocked_last && !h->imag && (h->taylor_block == 1 || h->taylor_block == 3)) {
+    if (lg && !h->taylor_blocked_last && !h->imag && (h->taylor_block == 1 || h->taylor_block == 3)) {
         h->rtp = rt_plan(h->grid, order, h->rt_variant);
         if (h->rtp.ok) h->taylor_blocked_last = 2;
     }
-    if (!h->taylor_blocked_last && !h->imag && (h->taylor_block == 1 || h->taylor_block == 2) && blocked_supported(h->bcfg, order))
+    if (lg && !h->taylor_blocked_last && !h->imag && (h->taylor_block == 1 || h->taylor_block == 2) && blocked_supported(h->bcfg, order))
         h->taylor_blocked_last = 1;
     if (h->taylor_blocked_last != 2) h->rtp = RtPlan{};
     return run_fixed(h, KIND_TAYLOR, order, 0, t0, dt, nsteps, obs_every, (cudaStream_t)stream);
@@ -771,7 +776,7 @@ int tdse_step_rk4(tdse_handle *h, double t0, double dt, long nsteps, int obs_eve
     h->taylor_blocked_last = 0;
     h->rk4_fused = 0;
     h->rpp = RpPlan{};
-    if (h->rk4_block) {           // all four stages in one pass (register-patch kernel in RK mode) when it applies
+    if (h->rk4_block && h->grid.gauge == 0) {           // all four stages in one pass (register-patch kernel in RK mode) when it applies
         h->rpp = rp_plan(h->grid, 4, h->n_sm, -1, h->rp_tma, 1);
         if (h->rpp.ok) { h->rk4_fused = 1; h->taylor_blocked_last = 3; }
         else h->rpp = RpPlan{};

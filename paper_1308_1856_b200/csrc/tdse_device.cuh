@@ -14,6 +14,7 @@ constexpr int kRkRoles   = 10;     // PSI, G0, G1, K0..K6
 // Grid description and device tables handed to every kernel by value.
 struct GridDev {
     int n_r, n_l, batch, fd;
+    int gauge;              // 0 length gauge (Eq. 11), 1 velocity gauge (Eq. 12 in reading R-V2)
     double dr, z;
     double c1, c2;          // off-diagonal stencil weights of -1/2 D2: 3-point c1 = -1/(2dr^2); 5-point c1 = -16/(24dr^2), c2 = +1/(24dr^2)
     const double *vj;       // [n_r]  kinetic diagonal - Z/r_j          (Eq. 7, Eq. 15)
@@ -63,8 +64,30 @@ __device__ inline double pulse_E(const tdse_pulse &p, double t) {
     const double T = __ddiv_rn(__dmul_rn(2.0 * 3.14159265358979323846, p.n_cycles), p.omega);
     if (t < 0.0 || t > T) return 0.0;
     const double wt = __dmul_rn(p.omega, t);
-    const double s = sin(__ddiv_rn(wt, __dmul_rn(2.0, p.n_cycles)));
+    const double hw = __ddiv_rn(wt, __dmul_rn(2.0, p.n_cycles));
+    if (p.kind == 1) {      // E = -dA/dt of the Hann-shaped vector potential (R-V3)
+        const double Om = __ddiv_rn(p.omega, __dmul_rn(2.0, p.n_cycles));
+        const double s = sin(hw), c = cos(hw), ph = __dadd_rn(wt, p.cep);
+        return (p.e0 / p.omega) * s * (2.0 * Om * c * sin(ph) + p.omega * s * cos(ph));
+    }
+    const double s = sin(hw);
     return __dmul_rn(__dmul_rn(__dmul_rn(p.e0, s), s), cos(__dadd_rn(wt, p.cep)));
+}
+
+// A(t) of a kind-1 pulse (R-V3); the static test aid (omega = 0) has A = e0; kind 0 has no closed form here
+__device__ inline double pulse_A(const tdse_pulse &p, double t) {
+    if (p.omega == 0.0) return p.e0;
+    if (p.kind != 1) return nan("");
+    const double T = __ddiv_rn(__dmul_rn(2.0 * 3.14159265358979323846, p.n_cycles), p.omega);
+    if (t < 0.0 || t > T) return 0.0;
+    const double wt = __dmul_rn(p.omega, t);
+    const double s = sin(__ddiv_rn(wt, __dmul_rn(2.0, p.n_cycles)));
+    return -(p.e0 / p.omega) * s * s * sin(__dadd_rn(wt, p.cep));
+}
+
+// the time-dependent factor of the coupling: E(t) in the length gauge, A(t) in the velocity gauge
+__device__ inline double pulse_field(const tdse_pulse &p, double t, int gauge) {
+    return gauge == 1 ? pulse_A(p, t) : pulse_E(p, t);
 }
 
 // t0 + x*dt with two roundings (never contracted)

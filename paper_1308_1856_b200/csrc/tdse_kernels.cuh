@@ -45,7 +45,9 @@ __device__ __forceinline__ double2 h_point(const GridDev &g, double d, double er
 // One pass: out/epilogue <- H(E_b) in, for every member b.  grid = (ceil(n_r/TW), ceil(n_l/TL), batch).
 // Epi supplies: NRED, SCALED; begin(); skip_all(); member_active(b); input(); in_scale(b); efield(b);
 // point(b,l,j,idx,f,h,red); finish_member(b,s); finish_all().
-template <int FD, class Epi>
+// VG: velocity gauge (the l+-1 rows enter through d/dr -+ l/r instead of r; a template flag so that the
+// length-gauge instantiations keep their register budget).
+template <int FD, class Epi, bool VG = false>
 __global__ void __launch_bounds__(256, Epi::MINB) tile_kernel(GridDev g, Epi epi_in, RedCtx rc) {
     using T = Tile<FD>;
     __shared__ double2 tile[T::ELEMS];
@@ -94,7 +96,8 @@ __global__ void __launch_bounds__(256, Epi::MINB) tile_kernel(GridDev g, Epi epi
         const int j = j0 + tx;
         if (j < g.n_r) {
             const double vj = __ldg(g.vj + j), cen = __ldg(g.cen + j);
-            const double er = epi.efield(b) * (g.dr * (double)(j + 1));
+            const double afield = epi.efield(b), rinv = 1.0 / (g.dr * (double)(j + 1));
+            const double er = afield * (g.dr * (double)(j + 1));
             const int r0 = ty * T::RPT;
             const double2 *col = tile + (r0 + 1) * T::PITCH + T::HW + tx;
             double2 lo = col[-T::PITCH], f = col[0];
@@ -110,7 +113,28 @@ __global__ void __launch_bounds__(256, Epi::MINB) tile_kernel(GridDev g, Epi epi
                 const double d = fma((double)(l * (l + 1)), cen, vj);
                 const double cm = (l > 0) ? __ldg(g.cl + l - 1) : 0.0;
                 const double cp = __ldg(g.cl + l);
-                const double2 h = h_point<FD>(g, d, er, cm, cp, f, fm1, fp1, fm2, fp2, lo, up);
+                double2 h = h_point<FD>(g, d, VG ? 0.0 : er, cm, cp, f, fm1, fp1, fm2, fp2, lo, up);
+                if (VG) {
+                    // velocity gauge (Eq. 12 in reading R-V2; `afield` = A(t)):
+                    //   -i A [ c_{l-1} (d/dr - l/r) f_{l-1} + c_l (d/dr + (l+1)/r) f_{l+1} ],  d/dr by P:119 Eq. 14
+                    const double2 *cl_ = c - T::PITCH, *cu_ = c + T::PITCH;
+                    double dlx, dly, dux, duy;
+                    if (FD == 3) {
+                        const double w = 0.5 / g.dr;
+                        dlx = w * (cl_[1].x - cl_[-1].x); dly = w * (cl_[1].y - cl_[-1].y);
+                        dux = w * (cu_[1].x - cu_[-1].x); duy = w * (cu_[1].y - cu_[-1].y);
+                    } else {
+                        const double w = 1.0 / (12.0 * g.dr);
+                        dlx = w * (8.0 * (cl_[1].x - cl_[-1].x) - (cl_[2].x - cl_[-2].x));
+                        dly = w * (8.0 * (cl_[1].y - cl_[-1].y) - (cl_[2].y - cl_[-2].y));
+                        dux = w * (8.0 * (cu_[1].x - cu_[-1].x) - (cu_[2].x - cu_[-2].x));
+                        duy = w * (8.0 * (cu_[1].y - cu_[-1].y) - (cu_[2].y - cu_[-2].y));
+                    }
+                    const double sx = cm * (dlx - (double)l * rinv * lo.x) + cp * (dux + (double)(l + 1) * rinv * up.x);
+                    const double sy = cm * (dly - (double)l * rinv * lo.y) + cp * (duy + (double)(l + 1) * rinv * up.y);
+                    h.x = fma(afield, sy, h.x);              // -i (sx + i sy) = sy - i sx
+                    h.y = fma(-afield, sx, h.y);
+                }
                 const size_t idx = ((size_t)b * g.n_l + l) * g.n_r + j;
                 epi.point(b, l, j, idx, f, h, red);
                 lo = f; f = up;
@@ -500,7 +524,7 @@ __global__ void __launch_bounds__(32) small_exp_kernel(const double *alpha, cons
 // mode 0: Taylor/Lanczos (one value per step, at t_n + dt/2 or t_n);  mode 1: RK4 (4 stage times).
 // e_tab[(step*n_stage + stage)*B + b]
 __global__ void field_table_kernel(const Ctl *ctl, const tdse_pulse *pulse, int B, int n_steps, int mode,
-                                   double *e_tab) {
+                                   double *e_tab, int gauge) {
     const int n_stage = (mode == 1) ? 4 : 1;
     const int total = n_steps * n_stage * B;
     const double t0 = ctl->t0, dt = ctl->dt;
@@ -515,7 +539,7 @@ __global__ void field_table_kernel(const Ctl *ctl, const tdse_pulse *pulse, int 
         } else {
             t = ctl->field_sample == 1 ? time_at(t0, n, dt) : time_at(t0, n + 0.5, dt);
         }
-        e_tab[i] = pulse_E(pulse[b], t);
+        e_tab[i] = pulse_field(pulse[b], t, gauge);      // E(t), or A(t) in the velocity gauge
     }
 }
 
@@ -535,7 +559,8 @@ __global__ void ctl_advance_kernel(Ctl *c, int n) {
 
 // Start of an attempted Dormand-Prince step: clip the step to t_end (or take the replayed one) and tabulate
 // E_b(t + c_i h) for the 7 stages.  e_tab[stage*B + b].  One block.
-__global__ void rk45_begin_kernel(Ctl *c, const tdse_pulse *pulse, int B, const double *replay, double *e_tab) {
+__global__ void rk45_begin_kernel(Ctl *c, const tdse_pulse *pulse, int B, const double *replay, double *e_tab,
+                                  int gauge) {
     if (c->done) return;
     __shared__ double sh_h;
     if (threadIdx.x == 0) {
@@ -556,7 +581,7 @@ __global__ void rk45_begin_kernel(Ctl *c, const tdse_pulse *pulse, int B, const 
     const double cs[7] = {0.0, 1.0 / 5, 3.0 / 10, 4.0 / 5, 8.0 / 9, 1.0, 1.0};
     for (int i = threadIdx.x; i < 7 * B; i += blockDim.x) {
         const int st = i / B, b = i - st * B;
-        e_tab[i] = pulse_E(pulse[b], __dadd_rn(t, __dmul_rn(cs[st], h)));
+        e_tab[i] = pulse_field(pulse[b], __dadd_rn(t, __dmul_rn(cs[st], h)), gauge);
     }
 }
 

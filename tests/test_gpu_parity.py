@@ -34,9 +34,9 @@ def cfg_shape(n_r, dr, n_l, fd, batch=1, index=0):
     return dict(index=index, n_r=n_r, dr=dr, n_l=n_l, fd_order=fd, batch=batch, name="adhoc")
 
 
-def both(B, c):
-    g = oracle.make_grid(c["n_r"], c["dr"], c["n_l"], c["fd_order"], batch=c["batch"])
-    h = B.Tdse(c["n_r"], c["dr"], c["n_l"], c["fd_order"], batch=c["batch"])
+def both(B, c, gauge=0):
+    g = oracle.make_grid(c["n_r"], c["dr"], c["n_l"], c["fd_order"], batch=c["batch"], gauge=gauge)
+    h = B.Tdse(c["n_r"], c["dr"], c["n_l"], c["fd_order"], batch=c["batch"], gauge=gauge)
     return g, h
 
 
@@ -507,6 +507,79 @@ def test_absorbing_boundary_and_bound_population(B, case):
     h.close()
 
 
+# ------------------------------------------------------------------------------------------------- velocity gauge
+@pytest.mark.parametrize("shape", [(500, 8, 3, 1), (333, 11, 5, 3), (1300, 33, 5, 1), (37, 3, 3, 2)])
+def test_velocity_gauge_apply_H_parity(B, shape):
+    """H psi in the velocity gauge (Eq. 12 in reading R-V2, first derivative of Eq. 14) against the oracle."""
+    import torch
+    n_r, n_l, fd, batch = shape
+    c = wl.config("cfg5" if batch > 1 else "cfg1", n_r=n_r, dr=0.1, n_l=n_l, fd_order=fd, batch=batch)
+    g, h = both(B, c, gauge=1)
+    x = wl.random_state(c)
+    a = [0.3 + 0.07 * b for b in range(batch)]
+    d_in = torch.from_numpy(x).cuda()
+    d_out = torch.empty_like(d_in)
+    h.apply_H(d_in, d_out, a)
+    torch.cuda.synchronize()
+    ref = oracle.apply_H(g, x, a)
+    assert rel_l2(d_out.cpu().numpy(), ref) <= TOL_H
+    h.apply_H(d_in, d_out, [0.0] * batch)                       # A = 0: the field-free operator of either gauge
+    torch.cuda.synchronize()
+    g0 = oracle.make_grid(n_r, 0.1, n_l, fd, batch=batch)
+    assert rel_l2(d_out.cpu().numpy(), oracle.apply_H(g0, x, [0.0] * batch)) <= TOL_H
+    h.close()
+
+
+@pytest.mark.parametrize("prop", ["taylor", "rk4", "lanczos", "rk45"])
+def test_velocity_gauge_propagators(B, prop):
+    """Every propagator in the velocity gauge with the Hann-shaped vector potential (pulse kind 1) against the oracle;
+    the all-orders-in-one-pass kernels do not apply and the per-order / per-stage kernels run."""
+    c = wl.config("cfg5", n_r=420, dr=0.1, n_l=7, fd_order=5, batch=2, order=4)
+    g, h = both(B, c, gauge=1)
+    pulses = [(0.06 + 0.02 * b, 0.3, 3.0, 0.2, 1) for b in range(2)]
+    h.set_pulse(pulses)
+    g0 = oracle.make_grid(c["n_r"], c["dr"], c["n_l"], c["fd_order"], batch=2)
+    st = bound_pack(g0, [(0, 0), (1, 0)])
+    h.set_bound_states(*st)
+    psi0 = wl.populated_state(c)
+    dt = wl.dt_eff(c, "lanczos" if prop == "lanczos" else ("rk4" if prop == "rk45" else prop), 4)
+    t0, nsteps = 20.0, 25
+    h.set_state(psi0)
+    if prop == "taylor":
+        h.step_taylor(4, t0, dt, nsteps, 5)
+        ref, robs = oracle.step_taylor(g, pulses, psi0, 4, t0, dt, nsteps, states=st, obs_every=5)
+        assert h.taylor_kernel() == 0
+    elif prop == "rk4":
+        h.step_rk4(t0, dt, nsteps, 5)
+        ref, robs = oracle.step_rk4(g, pulses, psi0, t0, dt, nsteps, states=st, obs_every=5)
+        assert h.taylor_kernel() == 0
+    elif prop == "lanczos":
+        h.step_lanczos(10, 12, t0, dt, nsteps, 5)
+        ref, robs = oracle.step_lanczos(g, pulses, psi0, 10, 12, t0, dt, nsteps, states=st, obs_every=5)
+    else:
+        info = h.step_rk45(t0, t0 + 0.01, 1e-4, 1e-8)
+        ref, rinfo = oracle.step_rk45(g, pulses, psi0, t0, t0 + 0.01, 1e-4, 1e-8, dt_replay=info["dt"])
+        assert info["n_accept"] > 5 and np.max(rinfo["err"]) <= 1.05
+        robs = None
+    got = h.get_state()
+    assert rel_l2(got, ref) <= TOL_PSI
+    if robs is not None:
+        check_fixed(got, ref, h.obs_log(), robs)
+    h.close()
+
+
+def test_velocity_gauge_needs_a_vector_potential_pulse(B):
+    """A kind-0 pulse has no A(t) here: the run must not silently produce numbers."""
+    c = wl.config("cfg1", n_r=200, dr=0.2, n_l=4, fd_order=3)
+    g, h = both(B, c, gauge=1)
+    h.set_pulse([(0.05, 0.057, 2.0, 0.0)])
+    h.set_state(wl.populated_state(c))
+    h.step_taylor(4, 10.0, 1e-3, 4, 1)
+    with pytest.raises(B.TdseError):
+        h.obs_log()                                   # non-finite norm -> TDSE_ERR_NONFINITE
+    h.close()
+
+
 @pytest.mark.parametrize("fd,K", [(3, 16), (5, 7)])
 def test_lanczos_parity_and_internals(B, fd, K):
     c = wl.config("cfg4", n_r=700, n_l=10, fd_order=fd)
@@ -690,8 +763,8 @@ def test_error_codes_and_lifecycle(B):
     hp = C.c_void_p()
     bad = B.Grid(100, 0.1, 3, 4, 0, 1.0, 1)
     assert L.tdse_create(C.byref(bad), C.byref(hp)) == -5          # fd_order 4
-    bad = B.Grid(100, 0.1, 3, 3, 1, 1.0, 1)
-    assert L.tdse_create(C.byref(bad), C.byref(hp)) == -5          # velocity gauge: not built
+    bad = B.Grid(100, 0.1, 3, 3, 2, 1.0, 1)
+    assert L.tdse_create(C.byref(bad), C.byref(hp)) == -5          # gauge: 0 (length) or 1 (velocity) only
     bad = B.Grid(0, 0.1, 3, 3, 0, 1.0, 1)
     assert L.tdse_create(C.byref(bad), C.byref(hp)) == -1
     for _ in range(20):                                            # create/destroy cycles
