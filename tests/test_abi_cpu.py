@@ -36,7 +36,7 @@ def test_header_symbols_exported(binding):
 
 
 def test_struct_layouts_match_header(binding):
-    assert C.sizeof(binding.Grid) == 48 and C.sizeof(binding.Pulse) == 32
+    assert C.sizeof(binding.Grid) == 48 and C.sizeof(binding.Pulse) == 40      # 4 doubles + int kind (padded)
     assert binding.Grid.dr.offset == 8 and binding.Grid.z_nuc.offset == 32 and binding.Grid.batch.offset == 40
 
 
