@@ -178,6 +178,21 @@ def step_rk_fixed(g, pulses, psi, tableau, t0, dt, nsteps, states=None, obs_ever
     return psi, err[:nsteps], out
 
 
+RK_METHODS = {"rk4": 0, "dormandprince": 1, "euler": 2, "rkf": 3, "cashkarp": 4, "merson": 5}
+
+
+def step_rk_method(g, pulses, psi, method, t0, dt, nsteps, states=None, obs_every=0):
+    """Fixed-step propagation with one of the tableaux of P:796 and the passive error sum sigma[batch]."""
+    psi = _state(g, psi)
+    pa = _pulses(g, pulses)
+    o, out, keep = _obs(g, states, obs_every, nsteps)
+    sigma = np.zeros(g.batch)
+    rc = lib().oracle_step_rk_sigma(C.byref(g), pa, _dp(psi.view(np.float64)), int(RK_METHODS[method]), C.c_double(t0),
+                                    C.c_double(dt), C.c_long(nsteps), _dp(sigma), C.byref(o) if o else None)
+    assert rc == 0, rc
+    return psi, sigma, out
+
+
 def step_rk4(g, pulses, psi, t0, dt, nsteps, states=None, obs_every=0):
     psi, _, out = step_rk_fixed(g, pulses, psi, 0, t0, dt, nsteps, states, obs_every)
     return psi, out

@@ -179,9 +179,53 @@ const double dp_a[49] = {
 const double dp_b[7] = {35.0 / 384, 0, 500.0 / 1113, 125.0 / 192, -2187.0 / 6784, 11.0 / 84, 0};
 const double dp_bh[7] = {5179.0 / 57600, 0, 7571.0 / 16695, 393.0 / 640, -92097.0 / 339200, 187.0 / 2100, 1.0 / 40};
 
+// The other methods named at P:796 / P:813 (coefficients from the literature; the order conditions of every row
+// are verified in exact rationals in tests/test_oracle_pins.py).  b = the higher-order weights, which are the ones
+// propagated (reading R-C4 / R-G28); bh = the lower-order companion.
+const double eu_c[1] = {0.0}, eu_a[1] = {0.0}, eu_b[1] = {1.0};
+// Runge-Kutta-Fehlberg 4(5)
+const double rkf_c[6] = {0.0, 1.0 / 4, 3.0 / 8, 12.0 / 13, 1.0, 1.0 / 2};
+const double rkf_a[36] = {
+    0, 0, 0, 0, 0, 0,
+    1.0 / 4, 0, 0, 0, 0, 0,
+    3.0 / 32, 9.0 / 32, 0, 0, 0, 0,
+    1932.0 / 2197, -7200.0 / 2197, 7296.0 / 2197, 0, 0, 0,
+    439.0 / 216, -8.0, 3680.0 / 513, -845.0 / 4104, 0, 0,
+    -8.0 / 27, 2.0, -3544.0 / 2565, 1859.0 / 4104, -11.0 / 40, 0};
+const double rkf_b[6] = {16.0 / 135, 0, 6656.0 / 12825, 28561.0 / 56430, -9.0 / 50, 2.0 / 55};
+const double rkf_bh[6] = {25.0 / 216, 0, 1408.0 / 2565, 2197.0 / 4104, -1.0 / 5, 0};
+// Cash-Karp 5(4)
+const double ck_c[6] = {0.0, 1.0 / 5, 3.0 / 10, 3.0 / 5, 1.0, 7.0 / 8};
+const double ck_a[36] = {
+    0, 0, 0, 0, 0, 0,
+    1.0 / 5, 0, 0, 0, 0, 0,
+    3.0 / 40, 9.0 / 40, 0, 0, 0, 0,
+    3.0 / 10, -9.0 / 10, 6.0 / 5, 0, 0, 0,
+    -11.0 / 54, 5.0 / 2, -70.0 / 27, 35.0 / 27, 0, 0,
+    1631.0 / 55296, 175.0 / 512, 575.0 / 13824, 44275.0 / 110592, 253.0 / 4096, 0};
+const double ck_b[6] = {37.0 / 378, 0, 250.0 / 621, 125.0 / 594, 0, 512.0 / 1771};
+const double ck_bh[6] = {2825.0 / 27648, 0, 18575.0 / 48384, 13525.0 / 55296, 277.0 / 14336, 1.0 / 4};
+// Kutta-Merson 4(3)
+const double me_c[5] = {0.0, 1.0 / 3, 1.0 / 3, 1.0 / 2, 1.0};
+const double me_a[25] = {
+    0, 0, 0, 0, 0,
+    1.0 / 3, 0, 0, 0, 0,
+    1.0 / 6, 1.0 / 6, 0, 0, 0,
+    1.0 / 8, 0, 3.0 / 8, 0, 0,
+    1.0 / 2, 0, -3.0 / 2, 2.0, 0};
+const double me_b[5] = {1.0 / 6, 0, 0, 2.0 / 3, 1.0 / 6};
+const double me_bh[5] = {1.0 / 10, 0, 3.0 / 10, 2.0 / 5, 1.0 / 5};
+
+// 0 ClassicRK4, 1 DormandPrince, 2 Euler, 3 RKF, 4 CashKarp, 5 Merson (the names of P:796)
 Tableau tableau_of(int id) {
-    if (id == 1) return {7, dp_c, dp_a, dp_b, dp_bh};
-    return {4, rk4_c, rk4_a, rk4_b, nullptr};
+    switch (id) {
+        case 1: return {7, dp_c, dp_a, dp_b, dp_bh};
+        case 2: return {1, eu_c, eu_a, eu_b, nullptr};
+        case 3: return {6, rkf_c, rkf_a, rkf_b, rkf_bh};
+        case 4: return {6, ck_c, ck_a, ck_b, ck_bh};
+        case 5: return {5, me_c, me_a, me_b, me_bh};
+        default: return {4, rk4_c, rk4_a, rk4_b, nullptr};
+    }
 }
 
 // One RK step of size h from t for all members.  k: s arrays of B*L*N complex.
@@ -574,7 +618,7 @@ int oracle_step_imag(const oracle_grid *g, double *psi, int order, double dt, lo
 
 int oracle_step_rk_fixed(const oracle_grid *g, const oracle_pulse *pulse, double *psi, int tableau,
                          double t0, double dt, long nsteps, double *err_out, const oracle_obs *obs) {
-    if (!grid_ok(g) || !pulse || !psi || nsteps < 0 || tableau < 0 || tableau > 1) return -1;
+    if (!grid_ok(g) || !pulse || !psi || nsteps < 0 || tableau < 0 || tableau > 5) return -1;
     const Tableau tb = tableau_of(tableau);
     const long MB = n_points(g) * g->batch;
     std::vector<std::vector<double>> k(tb.s, std::vector<double>(2 * MB));
@@ -594,6 +638,30 @@ int oracle_step_rk_fixed(const oracle_grid *g, const oracle_pulse *pulse, double
 int oracle_step_rk4(const oracle_grid *g, const oracle_pulse *pulse, double *psi,
                     double t0, double dt, long nsteps, const oracle_obs *obs) {
     return oracle_step_rk_fixed(g, pulse, psi, 0, t0, dt, nsteps, nullptr, obs);
+}
+
+// Fixed-step propagation with any of the tableaux and the PASSIVE error sum of P:827-833: per member
+// sigma_n = sqrt(|Delta|^2 / M), Delta = F^(2) - F^(1) = h sum (b_i - bh_i) k_i over the M complex elements of the
+// member's vector (reading R-G19), sigma = sum_n sigma_n.  sigma_out[b] (may be NULL) receives sigma; 0 without a pair.
+int oracle_step_rk_sigma(const oracle_grid *g, const oracle_pulse *pulse, double *psi, int tableau,
+                         double t0, double dt, long nsteps, double *sigma_out, const oracle_obs *obs) {
+    if (!grid_ok(g) || !pulse || !psi || nsteps < 0 || tableau < 0 || tableau > 5) return -1;
+    const Tableau tb = tableau_of(tableau);
+    const long M = n_points(g), MB = M * g->batch;
+    std::vector<std::vector<double>> k(tb.s, std::vector<double>(2 * MB));
+    std::vector<double> gbuf(2 * MB), hbuf(2 * MB), next(2 * MB);
+    if (sigma_out) for (int b = 0; b < g->batch; ++b) sigma_out[b] = 0.0;
+    long block = 0;
+    for (long n = 0; n < nsteps; ++n) {
+        double err;
+        rk_step(g, pulse, tb, psi, t0 + n * dt, dt, k, false, gbuf, hbuf, next.data(), &err);   // gbuf <- Delta
+        std::memcpy(psi, next.data(), sizeof(double) * 2 * MB);
+        if (sigma_out && tb.bh)
+            for (int b = 0; b < g->batch; ++b) sigma_out[b] += std::sqrt(sumsq(M, gbuf.data() + 2 * M * b) / (double)M);
+        if (obs && obs->obs_every > 0 && (n + 1) % obs->obs_every == 0)
+            log_obs(g, pulse, psi, t0 + (n + 1) * dt, obs, block++);
+    }
+    return 0;
 }
 
 int oracle_step_rk45(const oracle_grid *g, const oracle_pulse *pulse, double *psi,

@@ -106,11 +106,17 @@ int oracle_step_rk4(const oracle_grid *g, const oracle_pulse *pulse, double *psi
                     double t0, double dt, long nsteps, const oracle_obs *obs);
 
 /* Any explicit tableau through the same stage loop: tableau id
- * 0 = ClassicRK4, 1 = DormandPrince 5(4) advancing with the 5th-order weights.
+ * 0 = ClassicRK4, 1 = DormandPrince 5(4), 2 = Euler, 3 = RKF 4(5), 4 = CashKarp 5(4), 5 = Merson 4(3) (the methods
+ * named at P:796 / P:813), each advancing with its higher-order weights.
  * err_out (may be NULL) receives, per step, max_b ||Delta_b||_2 / ||psi_new,b||_2
  * (embedded-pair difference; 0 for RK4). */
 int oracle_step_rk_fixed(const oracle_grid *g, const oracle_pulse *pulse, double *psi, int tableau,
                          double t0, double dt, long nsteps, double *err_out, const oracle_obs *obs);
+
+/* The same with the passive error sum of P:827-833: sigma_out[b] = sum_n sqrt(|Delta_n,b|^2 / M), M = complex
+ * elements per member (R-G19); may be NULL; 0 for the methods without an embedded pair. */
+int oracle_step_rk_sigma(const oracle_grid *g, const oracle_pulse *pulse, double *psi, int tableau,
+                         double t0, double dt, long nsteps, double *sigma_out, const oracle_obs *obs);
 
 /* Adaptive Dormand-Prince 5(4) (paper: controller "not implemented"; ours, DESIGN.md R-C4):
  * err = max_b ||Delta_b|| / (rtol ||psi_new,b||); accept iff err <= 1;

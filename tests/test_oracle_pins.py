@@ -734,3 +734,94 @@ def test_P13_vector_potential_pulse_and_gauge_agreement():
         dep.append(1.0 - abs(np.vdot(phi[0], out[0, 0]) * dr) ** 2)
     assert dep[0] > 0.01                                                         # the pulse does ionise
     assert abs(dep[0] - dep[1]) < 0.05 * dep[0]
+
+
+# ------------------------------------------------------------------------------- the other RK methods of P:796 (P14)
+def _order_conditions(c, a, b, order):
+    """Rooted-tree order conditions up to `order` (<= 5) in exact rationals; a as a list of rows."""
+    F = Fraction
+    s = len(c)
+    A = [[a[i][j] if j < len(a[i]) else F(0) for j in range(s)] for i in range(s)]
+    dot = lambda u, v: sum(x * y for x, y in zip(u, v))
+    Av = lambda v: [dot(A[i], v) for i in range(s)]
+    mul = lambda u, v: [x * y for x, y in zip(u, v)]
+    one = [F(1)] * s
+    c2, c3 = mul(c, c), mul(mul(c, c), c)
+    Ac, Ac2, Ac3 = Av(c), Av(c2), Av(c3)
+    AAc, AAc2 = Av(Ac), Av(Ac2)
+    conds = {1: [(one, F(1))],
+             2: [(c, F(1, 2))],
+             3: [(c2, F(1, 3)), (Ac, F(1, 6))],
+             4: [(c3, F(1, 4)), (mul(c, Ac), F(1, 8)), (Ac2, F(1, 12)), (AAc, F(1, 24))],
+             5: [(mul(c3, c), F(1, 5)), (mul(c2, Ac), F(1, 10)), (mul(c, Ac2), F(1, 15)), (mul(c, AAc), F(1, 30)),
+                 (mul(Ac, Ac), F(1, 20)), (Ac3, F(1, 20)), (Av(mul(c, Ac)), F(1, 40)), (AAc2, F(1, 60)),
+                 (Av(AAc), F(1, 120))]}
+    ok = True
+    for q in range(1, order + 1):
+        for vec, rhs in conds[q]:
+            ok = ok and dot(b, vec) == rhs
+    return ok
+
+
+def test_P14_rk_tableaux_order_conditions():
+    """RKF 4(5), Cash-Karp 5(4) and Kutta-Merson 4(3) as typed into the oracle: row sums = c and ALL order conditions of
+    the stated orders for both weight rows, in exact rationals; the lower-order row fails the next order."""
+    F = Fraction
+    tabs = {
+        "rkf": ([F(0), F(1, 4), F(3, 8), F(12, 13), F(1), F(1, 2)],
+                [[], [F(1, 4)], [F(3, 32), F(9, 32)], [F(1932, 2197), F(-7200, 2197), F(7296, 2197)],
+                 [F(439, 216), F(-8), F(3680, 513), F(-845, 4104)],
+                 [F(-8, 27), F(2), F(-3544, 2565), F(1859, 4104), F(-11, 40)]],
+                [F(16, 135), F(0), F(6656, 12825), F(28561, 56430), F(-9, 50), F(2, 55)], 5,
+                [F(25, 216), F(0), F(1408, 2565), F(2197, 4104), F(-1, 5), F(0)], 4),
+        "cashkarp": ([F(0), F(1, 5), F(3, 10), F(3, 5), F(1), F(7, 8)],
+                     [[], [F(1, 5)], [F(3, 40), F(9, 40)], [F(3, 10), F(-9, 10), F(6, 5)],
+                      [F(-11, 54), F(5, 2), F(-70, 27), F(35, 27)],
+                      [F(1631, 55296), F(175, 512), F(575, 13824), F(44275, 110592), F(253, 4096)]],
+                     [F(37, 378), F(0), F(250, 621), F(125, 594), F(0), F(512, 1771)], 5,
+                     [F(2825, 27648), F(0), F(18575, 48384), F(13525, 55296), F(277, 14336), F(1, 4)], 4),
+        "merson": ([F(0), F(1, 3), F(1, 3), F(1, 2), F(1)],
+                   [[], [F(1, 3)], [F(1, 6), F(1, 6)], [F(1, 8), F(0), F(3, 8)], [F(1, 2), F(0), F(-3, 2), F(2)]],
+                   [F(1, 6), F(0), F(0), F(2, 3), F(1, 6)], 4,
+                   [F(1, 10), F(0), F(3, 10), F(2, 5), F(1, 5)], 3),
+    }
+    for name, (c, a, b, pb, bh, pbh) in tabs.items():
+        for i in range(len(c)):
+            assert sum(a[i], F(0)) == c[i], name
+        assert _order_conditions(c, a, b, pb), name
+        assert _order_conditions(c, a, bh, pbh), name
+        assert not _order_conditions(c, a, bh, pbh + 1), name
+        if pb < 5:
+            assert not _order_conditions(c, a, b, pb + 1), name
+
+
+def test_P14_rk_methods_convergence_and_sigma():
+    """Every method of P:796 on the tiny grid against a converged Taylor step: the error falls with its order when dt
+    halves (pins the oracle's typed-in coefficients and stage times); Euler is Taylor order 1 exactly; sigma is the
+    sum over steps of sqrt(|F2 - F1|^2 / M), zero for the methods without a pair."""
+    g = tiny(5)
+    psi = rand_state((1, g.n_l, g.n_r), 3); psi /= math.sqrt(g.dr * np.sum(np.abs(psi) ** 2))
+    pulse = [(0.3, 2.0, 1.0, 0.2)]                                        # fast field: the stage times matter
+    t0, span = 0.4, 0.02
+    ref = oracle.step_taylor(g, pulse, psi, 8, t0, span / 400, 400)[0]
+    order = {"euler": 1, "rk4": 4, "merson": 4, "rkf": 5, "cashkarp": 5, "dormandprince": 5}
+    for m, p in order.items():
+        errs, sig = [], []
+        for n in (10, 20):
+            out, s, _ = oracle.step_rk_method(g, pulse, psi, m, t0, span / n, n)
+            errs.append(np.linalg.norm(out - ref)); sig.append(s[0])
+        assert 0.8 * 2 ** p < errs[0] / errs[1] < 1.25 * 2 ** p, (m, errs)
+        if m in ("euler", "rk4"):
+            assert sig == [0.0, 0.0]
+        else:
+            lo = 3 if m == "merson" else 4      # order of the companion: Delta = O(dt^(lo+1)) per step, n = O(1/dt) steps
+            assert sig[0] > 0 and 0.6 * 2 ** lo < sig[0] / sig[1] < 1.4 * 2 ** (lo + 1), (m, sig)   # (linear ODE: Merson gains one)
+    e1 = oracle.step_rk_method(g, pulse, psi, "euler", t0, 1e-3, 7)[0]
+    t1 = oracle.step_taylor(g, pulse, psi, 1, t0, 1e-3, 7, field_sample=1)[0]
+    assert np.linalg.norm(e1 - t1) <= 1e-15 * np.linalg.norm(t1)
+    # sigma of one Dormand-Prince step against the difference of the two solutions formed by hand from err of
+    # oracle.step_rk_fixed (relative definition) -- same Delta, different normalisation
+    out, s, _ = oracle.step_rk_method(g, pulse, psi, "dormandprince", t0, 2e-3, 1)
+    _, rel, _ = oracle.step_rk_fixed(g, pulse, psi, 1, t0, 2e-3, 1)
+    m_el = g.n_l * g.n_r
+    assert abs(s[0] - rel[0] * np.linalg.norm(out) / math.sqrt(m_el)) <= 1e-12 * s[0]
