@@ -124,6 +124,14 @@ int  tdse_step_rk4    (tdse_handle *h, double t0, double dt, long nsteps, int ob
 int  tdse_step_lanczos(tdse_handle *h, int krylov_dim, int taylor_order, double t0, double dt, long nsteps,
                        int obs_every, void *stream);
 
+/* Fixed-step propagation with any of the Runge-Kutta methods the paper lists: method 0 ClassicRK4,
+ * 1 DormandPrince 5(4), 2 Euler, 3 RKF 4(5), 4 CashKarp 5(4), 5 Merson 4(3), through the stage loop of P:469-478; the
+ * pairs advance with their higher-order weights and accumulate the PASSIVE error sum of P:827-833,
+ * sigma_b = sum_n sqrt(|F2 - F1|^2_{n,b} / M) with M = n_l n_r (reading R-G19), read back by tdse_rk_sigma
+ * (host [batch]; 0 for Euler and ClassicRK4; synchronises `stream`). */
+int  tdse_step_rk(tdse_handle *h, int method, double t0, double dt, long nsteps, int obs_every, void *stream);
+int  tdse_rk_sigma(tdse_handle *h, double *sigma_host, void *stream);
+
 /* Imaginary-time ("diffusion") propagation for ground states: no field, -i -> 1, i.e.
  * F^(k) = (-dt/k) H F^(k-1), F_{n+1} = sum_{k<=order} F^(k), then F_{n+1} /= ||F_{n+1}|| (whole wavefunction of the
  * member, rectangle rule) after every step.  The energy estimate of the step, E = -ln<F_{n+1}|F_{n+1}> / (2 dt)

@@ -17,7 +17,7 @@ ERRORS = {-1: "TDSE_ERR_ARG", -2: "TDSE_ERR_ALLOC", -3: "TDSE_ERR_CUDA", -4: "TD
 
 # every symbol include/tdse.h declares
 SYMBOLS = ["tdse_create", "tdse_destroy", "tdse_set_option", "tdse_set_pulse", "tdse_set_bound_states",
-           "tdse_set_state", "tdse_get_state", "tdse_apply_H", "tdse_set_absorber", "tdse_bound_population", "tdse_step_taylor", "tdse_step_imag", "tdse_energy_log", "tdse_step_rk4",
+           "tdse_set_state", "tdse_get_state", "tdse_apply_H", "tdse_set_absorber", "tdse_bound_population", "tdse_step_taylor", "tdse_step_imag", "tdse_energy_log", "tdse_step_rk4", "tdse_step_rk", "tdse_rk_sigma",
            "tdse_step_lanczos", "tdse_step_rk45", "tdse_observables", "tdse_obs_log", "tdse_dt_log",
            "tdse_lanczos_info", "tdse_launch_count", "tdse_taylor_was_blocked", "tdse_strerror", "tdse_version"]
 
@@ -61,6 +61,8 @@ def lib():
         L.tdse_apply_H.argtypes = [vp, vp, vp, dp, vp]
         L.tdse_step_taylor.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_long, C.c_int, vp]
         L.tdse_step_imag.argtypes = [vp, C.c_int, C.c_double, C.c_long, vp]
+        L.tdse_step_rk.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_long, C.c_int, vp]
+        L.tdse_rk_sigma.argtypes = [vp, C.POINTER(C.c_double), vp]
         L.tdse_set_absorber.argtypes = [vp, C.c_double, C.c_int]
         L.tdse_bound_population.argtypes = [vp, C.c_double, C.POINTER(C.c_double), vp]
         L.tdse_energy_log.argtypes = [vp, C.POINTER(C.c_double), C.c_long, vp]
@@ -220,6 +222,16 @@ class Tdse:
     def step_rk4(self, t0, dt, nsteps, obs_every=0, stream=None):
         _check(lib().tdse_step_rk4(self._h, float(t0), float(dt), int(nsteps), int(obs_every), _stream(stream)),
                "tdse_step_rk4")
+
+    RK_METHODS = {"rk4": 0, "dormandprince": 1, "euler": 2, "rkf": 3, "cashkarp": 4, "merson": 5}
+
+    def step_rk(self, method, t0, dt, nsteps, obs_every=0, stream=None):
+        """Fixed-step Runge-Kutta with one of the paper's methods; returns the passive error sums sigma[batch]."""
+        _check(lib().tdse_step_rk(self._h, int(self.RK_METHODS[method]), float(t0), float(dt), int(nsteps), int(obs_every),
+                                  _stream(stream)), "tdse_step_rk")
+        sig = np.zeros(self.grid.batch)
+        _check(lib().tdse_rk_sigma(self._h, sig.ctypes.data_as(C.POINTER(C.c_double)), _stream(stream)), "tdse_rk_sigma")
+        return sig
 
     def step_lanczos(self, krylov_dim, taylor_order, t0, dt, nsteps, obs_every=0, stream=None):
         _check(lib().tdse_step_lanczos(self._h, int(krylov_dim), int(taylor_order), float(t0), float(dt),

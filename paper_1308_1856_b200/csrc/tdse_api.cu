@@ -50,6 +50,38 @@ const double DP_A[7][7] = {
     {35.0 / 384, 0, 500.0 / 1113, 125.0 / 192, -2187.0 / 6784, 11.0 / 84, 0}};
 const double DP_B[7] = {35.0 / 384, 0, 500.0 / 1113, 125.0 / 192, -2187.0 / 6784, 11.0 / 84, 0};
 const double DP_BH[7] = {5179.0 / 57600, 0, 7571.0 / 16695, 393.0 / 640, -92097.0 / 339200, 187.0 / 2100, 1.0 / 40};
+
+// All methods named at P:796 / P:813 for tdse_step_rk: b = the higher-order weights (propagated), bh = companion.
+struct RkTab { int s, embedded; double c[7]; double a[7][7]; double b[7]; double bh[7]; };
+const RkTab kRkTabs[6] = {
+    // 0 ClassicRK4
+    {4, 0, {0, 0.5, 0.5, 1.0}, {{0}, {0.5}, {0, 0.5}, {0, 0, 1.0}}, {1.0 / 6, 1.0 / 3, 1.0 / 3, 1.0 / 6}, {0}},
+    // 1 DormandPrince 5(4)
+    {7, 1, {0, 1.0 / 5, 3.0 / 10, 4.0 / 5, 8.0 / 9, 1.0, 1.0},
+     {{0}, {1.0 / 5}, {3.0 / 40, 9.0 / 40}, {44.0 / 45, -56.0 / 15, 32.0 / 9},
+      {19372.0 / 6561, -25360.0 / 2187, 64448.0 / 6561, -212.0 / 729},
+      {9017.0 / 3168, -355.0 / 33, 46732.0 / 5247, 49.0 / 176, -5103.0 / 18656},
+      {35.0 / 384, 0, 500.0 / 1113, 125.0 / 192, -2187.0 / 6784, 11.0 / 84}},
+     {35.0 / 384, 0, 500.0 / 1113, 125.0 / 192, -2187.0 / 6784, 11.0 / 84, 0},
+     {5179.0 / 57600, 0, 7571.0 / 16695, 393.0 / 640, -92097.0 / 339200, 187.0 / 2100, 1.0 / 40}},
+    // 2 Euler
+    {1, 0, {0}, {{0}}, {1.0}, {0}},
+    // 3 Runge-Kutta-Fehlberg 4(5)
+    {6, 1, {0, 1.0 / 4, 3.0 / 8, 12.0 / 13, 1.0, 1.0 / 2},
+     {{0}, {1.0 / 4}, {3.0 / 32, 9.0 / 32}, {1932.0 / 2197, -7200.0 / 2197, 7296.0 / 2197},
+      {439.0 / 216, -8.0, 3680.0 / 513, -845.0 / 4104}, {-8.0 / 27, 2.0, -3544.0 / 2565, 1859.0 / 4104, -11.0 / 40}},
+     {16.0 / 135, 0, 6656.0 / 12825, 28561.0 / 56430, -9.0 / 50, 2.0 / 55},
+     {25.0 / 216, 0, 1408.0 / 2565, 2197.0 / 4104, -1.0 / 5, 0}},
+    // 4 Cash-Karp 5(4)
+    {6, 1, {0, 1.0 / 5, 3.0 / 10, 3.0 / 5, 1.0, 7.0 / 8},
+     {{0}, {1.0 / 5}, {3.0 / 40, 9.0 / 40}, {3.0 / 10, -9.0 / 10, 6.0 / 5}, {-11.0 / 54, 5.0 / 2, -70.0 / 27, 35.0 / 27},
+      {1631.0 / 55296, 175.0 / 512, 575.0 / 13824, 44275.0 / 110592, 253.0 / 4096}},
+     {37.0 / 378, 0, 250.0 / 621, 125.0 / 594, 0, 512.0 / 1771},
+     {2825.0 / 27648, 0, 18575.0 / 48384, 13525.0 / 55296, 277.0 / 14336, 1.0 / 4}},
+    // 5 Kutta-Merson 4(3)
+    {5, 1, {0, 1.0 / 3, 1.0 / 3, 1.0 / 2, 1.0}, {{0}, {1.0 / 3}, {1.0 / 6, 1.0 / 6}, {1.0 / 8, 0, 3.0 / 8}, {1.0 / 2, 0, -3.0 / 2, 2.0}},
+     {1.0 / 6, 0, 0, 2.0 / 3, 1.0 / 6}, {1.0 / 10, 0, 3.0 / 10, 2.0 / 5, 1.0 / 5}},
+};
 }  // namespace
 
 struct tdse_handle {
@@ -96,6 +128,7 @@ struct tdse_handle {
     RpPlan rpp{}; int n_sm = 148; int rp_variant = -1, rp_tma = -1;
     int rk4_block = 1, rk4_fused = 0;       // option: fuse the four RK4 stages; what the last tdse_step_rk4 used
     int imag = 0;                           // the running Taylor call is an imaginary-time propagation
+    double *d_sigma = nullptr;              // passive RK error sums [batch] (tdse_step_rk)
     double *d_mask = nullptr; double *d_pb = nullptr;   // absorber mask [n_r] (or null), bound populations [batch]
     double *d_elog = nullptr, *d_imag_inv = nullptr; size_t elog_cap = 0; long elog_rows = 0;
 };
@@ -302,6 +335,7 @@ void fill_rk_common(tdse_handle *h, E &e, int stage, const double *ef, const dou
     e.psi_role = R_PSI;
     for (int j = 0; j < 7; ++j) { e.k_role[j] = -1; e.a_next[j] = 0.0; e.d_err[j] = 0.0; }
     e.check_done = 0; e.dt_log = h->d_dtlog; e.err_log = h->d_errlog;
+    e.passive = 0; e.sigma_acc = nullptr; e.inv_m = 0.0;
 }
 
 int enqueue_rk4_block(tdse_handle *h, int n, int obs, cudaStream_t s) {
@@ -354,6 +388,62 @@ int enqueue_rk4_block(tdse_handle *h, int n, int obs, cudaStream_t s) {
 }
 
 // Dormand-Prince stages [first_stage, 7) of `n` attempted steps; every kernel exits at once when ctl->done.
+// Fixed-step propagation with any tableau of kRkTabs through the stage loop of P:469-478: stage st reads the stage
+// vector its predecessor formed, stores k_st and forms g_{st+1} = psi + h sum_j a_{st+1,j} k_j in its epilogue; the
+// last stage writes psi + h sum_j b_j k_j over psi (read point-wise only) and, for an embedded pair, reduces
+// |Delta|^2 for the passive error sum.
+int enqueue_rk_generic_block(tdse_handle *h, int method, int n, int obs, cudaStream_t s) {
+    const int B = h->grid.batch;
+    const RkTab &tb = kRkTabs[method];
+    StageTimes cs{};
+    for (int i = 0; i < 7; ++i) cs.c[i] = tb.c[i];
+    field_table_rk_kernel<<<(n * tb.s * B + 255) / 256, 256, 0, s>>>(h->d_ctl, h->d_pulse, B, n, tb.s, cs, h->d_etab, h->gd.gauge);
+    count(h);
+    double2 *psi = h->pool[h->psi_slot];
+    for (int i = 0; i < n; ++i) {
+        for (int st = 0; st < tb.s; ++st) {
+            const double *ef = h->d_etab + ((size_t)i * tb.s + st) * B;
+            const bool last = (st == tb.s - 1);
+            auto fill = [&](auto &e) {
+                fill_rk_common(h, e, st, ef, &h->d_ctl->dt);
+                e.in_role = (st == 0) ? R_PSI : ((st & 1) ? R_G1 : R_G0);
+                for (int j = 0; j < 7; ++j) e.k_role[j] = R_K0 + j;
+                if (!last) {
+                    e.store_k = 1;
+                    e.out_role = ((st + 1) & 1) ? R_G1 : R_G0;
+                    for (int j = 0; j <= st; ++j) e.a_next[j] = tb.a[st + 1][j];
+                } else {
+                    e.store_k = 0;
+                    // a one-stage method reads psi through the tile (halo): it must not be overwritten in place
+                    e.out_role = (tb.s == 1) ? R_G0 : R_PSI;
+                    for (int j = 0; j < tb.s; ++j) e.a_next[j] = tb.b[j];
+                }
+            };
+            if (last && tb.embedded) {
+                EpiRK<true> e{};
+                fill(e);
+                for (int j = 0; j < tb.s; ++j) e.d_err[j] = tb.b[j] - tb.bh[j];
+                e.passive = 1; e.sigma_acc = h->d_sigma; e.inv_m = 1.0 / (double)pts_per_member(h);
+                RC(launch_tile(h, e, s));
+            } else {
+                EpiRK<false> e{};
+                fill(e);
+                RC(launch_tile(h, e, s));
+            }
+        }
+        if (tb.s == 1) {
+            OpCopy cp{}; cp.dst = psi; cp.src = h->pool[h->role_slot[R_G0]];
+            RC(launch_ew(h, cp, s));
+        }
+        RC(enqueue_mask(h, psi, s));
+        if (obs) RC(enqueue_obs(h, psi, i, 1, 0, 0.0, h->d_rows, s));
+    }
+    ctl_advance_kernel<<<1, 32, 0, s>>>(h->d_ctl, n);
+    count(h);
+    CU(cudaGetLastError());
+    return TDSE_OK;
+}
+
 int enqueue_rk45_block(tdse_handle *h, int n, int first_stage, cudaStream_t s) {
     const int B = h->grid.batch;
     for (int i = 0; i < n; ++i) {
@@ -447,7 +537,7 @@ int enqueue_lanczos_block(tdse_handle *h, int K, int order, int n, int obs, cuda
 }
 
 // ---- graph-captured time loop (row a7; NS: "the time loop is captured in a CUDA graph") ------------------
-enum Kind { KIND_TAYLOR = 1, KIND_RK4 = 2, KIND_LANCZOS = 3, KIND_RK45 = 4 };
+enum Kind { KIND_TAYLOR = 1, KIND_RK4 = 2, KIND_LANCZOS = 3, KIND_RK45 = 4, KIND_RKGEN = 5 };
 
 int enqueue_block(tdse_handle *h, int kind, int p1, int p2, int n, int obs, cudaStream_t s) {
     switch (kind) {
@@ -455,6 +545,7 @@ int enqueue_block(tdse_handle *h, int kind, int p1, int p2, int n, int obs, cuda
         case KIND_RK4: return enqueue_rk4_block(h, n, obs, s);
         case KIND_LANCZOS: return enqueue_lanczos_block(h, p1, p2, n, obs, s);
         case KIND_RK45: return enqueue_rk45_block(h, n, 1, s);
+        case KIND_RKGEN: return enqueue_rk_generic_block(h, p1, n, obs, s);
     }
     return TDSE_ERR_ARG;
 }
@@ -619,7 +710,7 @@ void tdse_destroy(tdse_handle *h) {
     free_graphs(h);
     for (double2 *p : h->pool) cudaFree(p);
     void *ptrs[] = {h->d_vj, h->d_cen, h->d_cl, h->d_pulse, h->d_bufs, h->d_ctl, h->d_etab, h->d_eapply, h->d_partials,
-                    h->d_counter, h->d_phi, h->d_lstate, h->d_obs_partials, h->d_obs_counters, h->d_elog, h->d_imag_inv, h->d_mask, h->d_pb, h->d_amp, h->d_rows, h->d_row_direct,
+                    h->d_counter, h->d_phi, h->d_lstate, h->d_obs_partials, h->d_obs_counters, h->d_elog, h->d_imag_inv, h->d_mask, h->d_pb, h->d_sigma, h->d_amp, h->d_rows, h->d_row_direct,
                     h->d_dtlog, h->d_errlog, h->d_replay, h->d_alpha, h->d_beta, h->d_nrm, h->d_inv, h->d_coef,
                     h->d_m, h->d_nsub, h->d_basis};
     for (void *p : ptrs) if (p) cudaFree(p);
@@ -812,6 +903,30 @@ int tdse_step_lanczos(tdse_handle *h, int K, int order, double t0, double dt, lo
     CU(cudaMemsetAsync(h->d_alpha, 0, sizeof(double) * B * K, (cudaStream_t)stream));
     CU(cudaMemsetAsync(h->d_beta, 0, sizeof(double) * B * K, (cudaStream_t)stream));
     return run_fixed(h, KIND_LANCZOS, K, order, t0, dt, nsteps, obs_every, (cudaStream_t)stream);
+}
+
+int tdse_step_rk(tdse_handle *h, int method, double t0, double dt, long nsteps, int obs_every, void *stream) {
+    if (!h || method < 0 || method > 5 || nsteps < 0 || obs_every < 0) return TDSE_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (!h->d_sigma) CU(cudaMalloc(&h->d_sigma, sizeof(double) * h->grid.batch));
+    CU(cudaMemsetAsync(h->d_sigma, 0, sizeof(double) * h->grid.batch, s));
+    if (method == 0) return tdse_step_rk4(h, t0, dt, nsteps, obs_every, stream);      // (fused kernel when it applies)
+    RC(ensure_pool(h, kRkRoles));
+    h->taylor_blocked_last = 0;
+    h->rk4_fused = 0;
+    h->imag = 0;
+    rk_roles(h);
+    RC(upload_bufs(h, kRkRoles, s));
+    return run_fixed(h, KIND_RKGEN, method, 0, t0, dt, nsteps, obs_every, s);
+}
+
+int tdse_rk_sigma(tdse_handle *h, double *sigma_host, void *stream) {
+    if (!h || !sigma_host) return TDSE_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (!h->d_sigma) { for (int b = 0; b < h->grid.batch; ++b) sigma_host[b] = 0.0; return TDSE_OK; }
+    CU(cudaMemcpyAsync(sigma_host, h->d_sigma, sizeof(double) * h->grid.batch, cudaMemcpyDeviceToHost, s));
+    CU(cudaStreamSynchronize(s));
+    return TDSE_OK;
 }
 
 int tdse_step_rk45(tdse_handle *h, double t0, double t_end, double dt_init, double rtol, const double *dt_replay,

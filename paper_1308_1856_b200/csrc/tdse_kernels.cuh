@@ -213,6 +213,8 @@ struct EpiRK : EpiBase {
     double d_err[7];        // b_j - bhat_j  (embedded pair difference)
     int check_done;
     double *dt_log, *err_log;
+    int passive;            // EMBED: no controller, only the passive error sum of P:827-833 (fixed-step methods)
+    double *sigma_acc; double inv_m;     // sigma_acc[b] += sqrt(|Delta_b|^2 / M), inv_m = 1/M
     // resolved at begin()
     const double2 *in_p; const double2 *in2_p; double2 *out_p; const double2 *psi_p; double2 *k_p[7]; double hh; double emax;
 
@@ -255,11 +257,12 @@ struct EpiRK : EpiBase {
         }
     }
     // controller (R-C4): runs once per attempted step in the last CTA
-    __device__ __forceinline__ void finish_member(int, const double *s) {
+    __device__ __forceinline__ void finish_member(int b, const double *s) {
+        if (EMBED && passive) { sigma_acc[b] += sqrt(s[0] * inv_m); return; }
         if (EMBED) { const double e = sqrt(s[0]) / sqrt(s[1]); if (!(e <= emax)) emax = e; }
     }
     __device__ __forceinline__ void finish_all() {
-        if (!EMBED) return;
+        if (!EMBED || passive) return;
         Ctl &c = *ctl;
         const double err = emax / c.rtol;
         const long long slot = c.n_accept;
@@ -540,6 +543,20 @@ __global__ void field_table_kernel(const Ctl *ctl, const tdse_pulse *pulse, int 
             t = ctl->field_sample == 1 ? time_at(t0, n, dt) : time_at(t0, n + 0.5, dt);
         }
         e_tab[i] = pulse_field(pulse[b], t, gauge);      // E(t), or A(t) in the velocity gauge
+    }
+}
+
+// field values at the stage times t_n + c_i dt of any tableau: e_tab[(step*n_stage + stage)*B + b]
+struct StageTimes { double c[7]; };
+__global__ void field_table_rk_kernel(const Ctl *ctl, const tdse_pulse *pulse, int B, int n_steps, int n_stage,
+                                      StageTimes cs, double *e_tab, int gauge) {
+    const int total = n_steps * n_stage * B;
+    const double t0 = ctl->t0, dt = ctl->dt;
+    const long long base = ctl->step_base;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < total; i += gridDim.x * blockDim.x) {
+        const int b = i % B, st = (i / B) % n_stage, s = i / (B * n_stage);
+        const double t = __dadd_rn(time_at(t0, (double)(base + s), dt), __dmul_rn(cs.c[st], dt));
+        e_tab[i] = pulse_field(pulse[b], t, gauge);
     }
 }
 

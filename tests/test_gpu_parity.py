@@ -580,6 +580,33 @@ def test_velocity_gauge_needs_a_vector_potential_pulse(B):
     h.close()
 
 
+@pytest.mark.parametrize("gauge", [0, 1])
+@pytest.mark.parametrize("method", ["euler", "rk4", "merson", "rkf", "cashkarp", "dormandprince"])
+def test_rk_methods_parity(B, method, gauge):
+    """Every Runge-Kutta method the paper lists at a fixed step, both gauges: state, observables and the
+    passive error sum sigma against the oracle."""
+    c = wl.config("cfg5", n_r=333, dr=0.1, n_l=6, fd_order=5, batch=2, order=4)
+    g, h = both(B, c, gauge=gauge)
+    pulses = [(0.05 + 0.03 * b, 0.4, 3.0, 0.1, 1) for b in range(2)]
+    h.set_pulse(pulses)
+    g0 = oracle.make_grid(c["n_r"], c["dr"], c["n_l"], c["fd_order"], batch=2)
+    st = bound_pack(g0, [(0, 0)])
+    h.set_bound_states(*st)
+    psi0 = wl.populated_state(c)
+    dt = wl.dt_eff(c, "rk4", 4) * (0.02 if method == "euler" else 0.5)
+    t0, nsteps = 11.0, 19
+    h.set_state(psi0)
+    sig = h.step_rk(method, t0, dt, nsteps, 4)
+    got = h.get_state()
+    ref, rsig, robs = oracle.step_rk_method(g, pulses, psi0, method, t0, dt, nsteps, states=st, obs_every=4)
+    check_fixed(got, ref, h.obs_log(), robs)
+    if method in ("euler", "rk4"):
+        assert np.all(sig == 0.0) and np.all(rsig == 0.0)
+    else:
+        assert np.all(rsig > 0) and np.max(np.abs(sig - rsig) / rsig) <= 1e-6
+    h.close()
+
+
 @pytest.mark.parametrize("fd,K", [(3, 16), (5, 7)])
 def test_lanczos_parity_and_internals(B, fd, K):
     c = wl.config("cfg4", n_r=700, n_l=10, fd_order=fd)
