@@ -197,14 +197,22 @@ int launch_ew(tdse_handle *h, const Op &op, cudaStream_t s) {
 }
 
 int obs_chunks_r(const tdse_handle *h) { return (h->grid.n_r + 255) / 256; }
-int obs_chunks_l(const tdse_handle *h) { return (h->grid.n_l + kObsRows - 1) / kObsRows; }
+// l segments of the observable kernel: as few as keep about two CTAs per SM in flight
+int obs_rows_per(const tdse_handle *h) {
+    const int chunks = (h->grid.n_l + kObsRows - 1) / kObsRows;
+    const long ctas_r = (long)obs_chunks_r(h) * h->grid.batch;
+    int seg = (int)std::min<long>(chunks, std::max<long>(1, (2L * h->n_sm + ctas_r - 1) / ctas_r));
+    const int per = (chunks + seg - 1) / seg;
+    return per * kObsRows;
+}
+int obs_chunks_l(const tdse_handle *h) { return (h->grid.n_l + obs_rows_per(h) - 1) / obs_rows_per(h); }
 int obs_chunks(const tdse_handle *h) { return obs_chunks_r(h) * obs_chunks_l(h); }
 
 // Observable kernels for the state `psi`; logged row (predicated on the device step counter) or direct.
 int enqueue_obs(tdse_handle *h, const double2 *psi, int step_off, int predicated, int use_direct, double t_direct,
                 double *rows, cudaStream_t s) {
     const int B = h->grid.batch;
-    if (obs_chunks(h) + h->n_states <= 8) {          // small grid: one CTA per member, no cross-CTA hand-over
+    if (obs_chunks_r(h) * ((h->grid.n_l + kObsRows - 1) / kObsRows) + h->n_states <= 8) {   // small grid: one CTA per member
         obs_small_kernel<<<B, 256, 0, s>>>(h->gd, psi, h->d_phi, h->d_lstate, h->n_states, h->d_pulse, h->d_ctl, step_off,
                                            predicated, use_direct, t_direct, rows);
         count(h);
@@ -213,7 +221,7 @@ int enqueue_obs(tdse_handle *h, const double2 *psi, int step_off, int predicated
     }
     obs_kernel<<<dim3(obs_chunks_r(h), B, obs_chunks_l(h) + h->n_states), 256, 0, s>>>(
         h->gd, psi, h->d_phi, h->d_lstate, h->n_states, h->d_pulse, h->d_ctl, step_off, predicated, use_direct, t_direct,
-        h->d_obs_partials, h->d_amp, h->d_obs_counters, rows);
+        h->d_obs_partials, h->d_amp, h->d_obs_counters, rows, obs_rows_per(h));
     count(h);
     CU(cudaGetLastError());
     return TDSE_OK;

@@ -620,7 +620,7 @@ constexpr int kObsRows = 8;
 __global__ void __launch_bounds__(256) obs_kernel(GridDev g, const double2 *psi, const double *phi, const int *l_of_state,
                                                   int n_states, const tdse_pulse *pulse, const Ctl *ctl, int step_off,
                                                   int predicated, int use_direct, double t_direct, double *partials,
-                                                  double2 *amp_part, unsigned int *counters, double *rows) {
+                                                  double2 *amp_part, unsigned int *counters, double *rows, int rows_per) {
     __shared__ double red_s[3 * 8];
     __shared__ int last_flag;
     long long row = 0;
@@ -631,22 +631,25 @@ __global__ void __launch_bounds__(256) obs_kernel(GridDev g, const double2 *psi,
         row = n / ctl->obs_every - 1;
         t = time_at(ctl->t0, (double)n, ctl->dt);
     }
-    const int chunks_r = gridDim.x, chunks_l = gridDim.z - n_states;
+    const int chunks_r = gridDim.x, chunks_l = gridDim.z - n_states;     // chunks_l = l segments of rows_per rows
     const int b = blockIdx.y, j = blockIdx.x * 256 + threadIdx.x;
     double red[3] = {0.0, 0.0, 0.0};
     if ((int)blockIdx.z < chunks_l) {
-        const int l0 = blockIdx.z * kObsRows;
+        const int l_lo = blockIdx.z * rows_per, l_hi = min(g.n_l, l_lo + rows_per);
         if (j < g.n_r) {
-            const double2 *p = psi + ((size_t)b * g.n_l + l0) * g.n_r + j;
-            double2 v[kObsRows + 1];
-#pragma unroll
-            for (int r = 0; r <= kObsRows; ++r)
-                v[r] = (l0 + r < g.n_l) ? p[(size_t)r * g.n_r] : make_double2(0.0, 0.0);
             double nn = 0.0, sz = 0.0;
+            for (int l0 = l_lo; l0 < l_hi; l0 += kObsRows) {
+                const double2 *p = psi + ((size_t)b * g.n_l + l0) * g.n_r + j;
+                double2 v[kObsRows + 1];
 #pragma unroll
-            for (int r = 0; r < kObsRows; ++r) {
-                nn += v[r].x * v[r].x + v[r].y * v[r].y;
-                if (l0 + r + 1 < g.n_l) sz = fma(__ldg(g.cl + l0 + r), v[r].x * v[r + 1].x + v[r].y * v[r + 1].y, sz);
+                for (int r = 0; r <= kObsRows; ++r)
+                    v[r] = (l0 + r < g.n_l) ? p[(size_t)r * g.n_r] : make_double2(0.0, 0.0);
+#pragma unroll
+                for (int r = 0; r < kObsRows; ++r) {
+                    if (l0 + r >= l_hi) break;
+                    nn += v[r].x * v[r].x + v[r].y * v[r].y;
+                    if (l0 + r + 1 < g.n_l) sz = fma(__ldg(g.cl + l0 + r), v[r].x * v[r + 1].x + v[r].y * v[r + 1].y, sz);
+                }
             }
             const double r = g.dr * (double)(j + 1);
             red[0] = nn; red[1] = r * sz; red[2] = sz / (r * r);
