@@ -241,6 +241,24 @@ def run_own(args):
         ms_e2e = sharding.max_over_ranks(ms_e2e)
         h2d = (pinned.numel() * 16 + 32 * B) / K
         d2h = (pin_out.numel() * 16 + rows.size * 8) / K
+        # the same round trip for SHORT jobs (one graph block of steps per upload/download): PCIe-bound by design,
+        # reported so that the amortisation in `e2e` is visible
+        ks = max(2, args.graph_steps)
+        reps = 5
+        sharding.barrier()
+        torch.cuda.synchronize()
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s0.record(stream)
+        for _ in range(reps):
+            h.set_state(pinned.numpy(), stream=stream)
+            h.step_taylor(order, t0, dt, ks, 0, stream=stream)
+            h.observables(t0 + ks * dt, stream=stream)
+            h.get_state(pin_out.numpy(), stream=stream)
+        s1.record(stream)
+        stream.synchronize()
+        ms_short = sharding.max_over_ranks(s0.elapsed_time(s1))
+        e2e_short = {"steps_per_round_trip": ks, "value": pts * world * order * ks * reps / (ms_short * 1e-3) / 1e9,
+                     "unit": UNIT, "h2d_bytes_per_step": pinned.numel() * 16 / ks, "d2h_bytes_per_step": pin_out.numel() * 16 / ks}
 
     total_pts = pts * world
     value = total_pts * order * K / (ms * 1e-3) / 1e9
@@ -284,7 +302,8 @@ def run_own(args):
                        "l2": "inputs_exceed_l2 (state arrays 131 MB each > 126 MB L2)", "parallelism": f"batch x{world}"},
             "clocks": clocks, "roofline": roofline,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "what": "set_pulse + set_state(host, pinned) + K steps + observables + get_state(host) via the C ABI"},
+                    "what": "set_pulse + set_state(host, pinned) + K steps + observables + get_state(host) via the C ABI",
+                    "short_jobs": e2e_short},
             "gpu_launches": int(launches), "max_norm_drift": norm_dev}
 
     if rank == 0 and not args.no_extra and world == 1:
