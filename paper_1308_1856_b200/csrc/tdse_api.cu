@@ -15,6 +15,7 @@
 #include "tdse_kernels.cuh"
 #include "tdse_taylor_blocked.cuh"
 #include "tdse_taylor_rp.cuh"
+#include "tdse_tile_tma.cuh"
 #include "tdse_taylor_rt.cuh"
 
 using namespace tdse;
@@ -128,6 +129,7 @@ struct tdse_handle {
     RpPlan rpp{}; int n_sm = 148; int rp_variant = -1, rp_tma = -1;
     int rk4_block = 1, rk4_fused = 0;       // option: fuse the four RK4 stages; what the last tdse_step_rk4 used
     int imag = 0;                           // the running Taylor call is an imaginary-time propagation
+    int apply_tma = 1;                      // tdse_apply_H: TMA-fetched tiles when n_r % 8 == 0
     double *d_sigma = nullptr;              // passive RK error sums [batch] (tdse_step_rk)
     double *d_mask = nullptr; double *d_pb = nullptr;   // absorber mask [n_r] (or null), bound populations [batch]
     double *d_elog = nullptr, *d_imag_inv = nullptr; size_t elog_cap = 0; long elog_rows = 0;
@@ -736,6 +738,7 @@ int tdse_set_option(tdse_handle *h, const char *key, double value) {
     else if (k == "taylor_block") { if (value < 0 || value > 4) return TDSE_ERR_ARG; h->taylor_block = (int)value; }
     else if (k == "taylor_rt_variant") { if (value < -1 || value >= kNumRtVariants) return TDSE_ERR_ARG; h->rt_variant = (int)value; free_graphs(h); }
     else if (k == "taylor_rp_variant") { if (value < -1 || value >= kNumRpVariants) return TDSE_ERR_ARG; h->rp_variant = (int)value; free_graphs(h); }
+    else if (k == "apply_tma") { if (value < 0 || value > 1) return TDSE_ERR_ARG; h->apply_tma = (int)value; }
     else if (k == "rk4_block") { if (value < 0 || value > 1) return TDSE_ERR_ARG; h->rk4_block = (int)value; free_graphs(h); }
     else if (k == "taylor_rp_tma") { if (value < -1 || value > 1) return TDSE_ERR_ARG; h->rp_tma = (int)value; free_graphs(h); }
     else if (k == "taylor_block_width") { if (value < 0 || value > 4096) return TDSE_ERR_ARG; h->bcfg.width_override = (int)value; free_graphs(h); }
@@ -808,6 +811,31 @@ int tdse_apply_H(tdse_handle *h, const void *psi_dev, void *out_dev, const doubl
     EpiApply e{};
     e.in = (const double2 *)psi_dev; e.ef = h->d_eapply; e.out = (double2 *)out_dev;
     h->pending = 0;
+    // tiles fetched by TMA (zero fill outside the index box by the hardware) when the layout allows it
+    // (and the grid is many rounds of resident CTAs: small, L2-resident grids measured 8 % slower this way)
+    const long apply_items = (long)((h->grid.n_r + kTtTW - 1) / kTtTW) * ((h->grid.n_l + kTtTL - 1) / kTtTL) * B;
+    if (h->apply_tma && h->grid.gauge == 0 && (h->grid.n_r & 7) == 0 && ((uintptr_t)psi_dev & 15) == 0 &&
+        apply_items >= 6L * h->n_sm * kTtMinB) {
+        const CUtensorMap *tm = tile_tensor_map(psi_dev, h->grid.n_r, h->grid.n_l, B);
+        if (tm) {
+            const int tiles_r = (h->grid.n_r + kTtTW - 1) / kTtTW, tiles_l = (h->grid.n_l + kTtTL - 1) / kTtTL;
+            const int n_items = tiles_r * tiles_l * B;
+            const int smem = kTtStages * (int)kTtStageBytes + 64;
+            const int grid = std::min(n_items, h->n_sm * kTtMinB);
+            static bool attr_set = false;
+            if (!attr_set) {
+                CU(cudaFuncSetAttribute(tile_tma_kernel<3, EpiApply>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+                CU(cudaFuncSetAttribute(tile_tma_kernel<5, EpiApply>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+                attr_set = true;
+            }
+            if (h->grid.fd_order == 3) tile_tma_kernel<3, EpiApply><<<grid, 256, smem, s>>>(h->gd, e, *tm, tiles_r, tiles_l, n_items);
+            else tile_tma_kernel<5, EpiApply><<<grid, 256, smem, s>>>(h->gd, e, *tm, tiles_r, tiles_l, n_items);
+            count(h);
+            CU(cudaGetLastError());
+            h->launches += h->pending;
+            return TDSE_OK;
+        }
+    }
     RC(launch_tile(h, e, s));
     h->launches += h->pending;
     return TDSE_OK;

@@ -1,0 +1,128 @@
+// tdse_tile_tma.cuh -- H.psi on (l, r) tiles fetched by TMA: the single-source variant of tile_kernel for grids with
+// n_r % 8 == 0 (row a1: tdse_apply_H).
+//
+// tile_kernel stages its tile through registers (ld.global -> st.shared): at 5 CTAs per SM the loads in flight per
+// SM are bounded by registers and the LSU pipe carries every byte twice (66 % busy on CFG4, profiles/).  Here a
+// persistent CTA asks the TMA unit for the whole (8 + 2 rows) x (128 + 16 columns) box of the NEXT two work items
+// while it computes the current one: the state array is described as a 4-D tensor [member][l][n_r/8][8 columns] so
+// that everything outside the index box of a member (the rows l = -1 and l = n_l, the columns beyond the walls) is
+// zero-filled by the hardware -- the Dirichlet walls of P:138-144 and the truncation f_{-1} = f_L = 0 cost nothing.
+// The compute phase and the epilogue interface are those of tile_kernel.
+#pragma once
+#include "tdse_kernels.cuh"
+#include "tdse_taylor_rp.cuh"      // mbarrier / TMA helpers, cuTensorMapEncodeTiled entry point
+
+namespace tdse {
+
+// measured on CFG4 / CFG5 (us): (stages, CTAs/SM, rows) = (2,3,8) 31.3 / 45.7; (3,3,8) 31.5 / 47.6; (2,4,8) 31.5 / 47.3;
+// (2,2,16) 31.9 / 47.0; (4,2,8) 33.4 / 49.0; (3,2,16) 37.3 / 51.0
+constexpr int kTtTW = 128, kTtTL = 8, kTtHalo = 8, kTtCols = kTtTW + 2 * kTtHalo, kTtRows = kTtTL + 2, kTtStages = 2;
+constexpr int kTtMinB = 3;
+constexpr unsigned kTtStageBytes = (unsigned)(kTtRows * kTtCols * sizeof(double2));
+
+__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, int c0, int c1, int c2, int c3,
+                                            unsigned long long *bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+        ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
+}
+
+// grid = persistent CTAs, block = 256, dynamic shared = kTtStages * kTtStageBytes + 64.
+// items = batch x l-tiles x r-tiles (r fastest).  Epi must have NRED == 0 and a plain input.
+template <int FD, class Epi>
+__global__ void __launch_bounds__(256, kTtMinB)
+tile_tma_kernel(GridDev g, Epi epi_in, const __grid_constant__ CUtensorMap tmap, int tiles_r, int tiles_l, int n_items) {
+    static_assert(Epi::NRED == 0 && !Epi::CUSTOM_LOAD && !Epi::TWO_IN && !Epi::SCALED, "single-source epilogues only");
+    constexpr int HW = (FD == 3) ? 1 : 2, COLS = kTtCols;
+    extern __shared__ __align__(1024) unsigned char tt_smem[];
+    double2 *st = reinterpret_cast<double2 *>(tt_smem);
+    unsigned long long *bars = reinterpret_cast<unsigned long long *>(tt_smem + kTtStages * kTtStageBytes);
+    Epi epi = epi_in;
+    epi.begin();
+    if (epi.skip_all()) return;
+    const int tid = threadIdx.x;
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < kTtStages; ++s) mbar_init(&bars[s], 1);
+    }
+    __syncthreads();
+    auto fetch = [&](const int item, const int s) {
+        if (tid == 0 && item < n_items) {
+            const int tr = item % tiles_r, rest = item / tiles_r, tl = rest % tiles_l, b = rest / tiles_l;
+            fence_proxy_async_smem();
+            mbar_expect_tx(&bars[s], kTtStageBytes);
+            tma_load_4d(st + (size_t)s * kTtRows * COLS, &tmap, 0, tr * (kTtTW / 8) - kTtHalo / 8, tl * kTtTL - 1, b, &bars[s]);
+        }
+    };
+#pragma unroll
+    for (int s = 0; s < kTtStages; ++s) fetch(blockIdx.x + s * gridDim.x, s);
+
+    const int tx = tid % kTtTW, ty = tid / kTtTW;
+    unsigned phase = 0;          // bit s = parity of stage s
+    int k = 0;
+    double red[1] = {0.0};
+    for (int item = blockIdx.x; item < n_items; item += gridDim.x, ++k) {
+        const int s = k % kTtStages;
+        const int tr = item % tiles_r, rest = item / tiles_r, tl = rest % tiles_l, b = rest / tiles_l;
+        const int j = tr * kTtTW + tx, l0 = tl * kTtTL;
+        mbar_wait(&bars[s], (phase >> s) & 1u);
+        phase ^= 1u << s;
+        if (j < g.n_r && epi.member_active(b)) {
+            const double vj = __ldg(g.vj + j), cen = __ldg(g.cen + j);
+            const double er = epi.efield(b) * (g.dr * (double)(j + 1));
+            const int r0 = ty * (kTtTL / 2);
+            const double2 *col = st + (size_t)s * kTtRows * COLS + (r0 + 1) * COLS + kTtHalo + tx;
+            double2 lo = col[-COLS], f = col[0];
+#pragma unroll
+            for (int rr = 0; rr < kTtTL / 2; ++rr) {
+                const int l = l0 + r0 + rr;
+                if (l >= g.n_l) break;
+                const double2 *c = col + rr * COLS;
+                const double2 up = c[COLS];
+                const double2 fm1 = c[-1], fp1 = c[1];
+                double2 fm2 = fm1, fp2 = fp1;
+                if (FD == 5) { fm2 = c[-2]; fp2 = c[2]; }
+                const double d = fma((double)(l * (l + 1)), cen, vj);
+                const double cm = (l > 0) ? __ldg(g.cl + l - 1) : 0.0;
+                const double cp = __ldg(g.cl + l);
+                const double2 h = h_point<FD>(g, d, er, cm, cp, f, fm1, fp1, fm2, fp2, lo, up);
+                epi.point(b, l, j, ((size_t)b * g.n_l + l) * g.n_r + j, f, h, red);
+                lo = f; f = up;
+            }
+        }
+        __syncthreads();                                   // every thread is done with stage s
+        fetch(item + kTtStages * gridDim.x, s);
+    }
+}
+
+// 4-D tensor map of a state array: [batch][n_l][n_r/8][16 doubles], box = 1 x kTtRows x kTtCols/8 x 16, no swizzle
+inline const CUtensorMap *tile_tensor_map(const void *base, int n_r, int n_l, int batch) {
+    static std::map<std::tuple<const void *, int, int, int>, CUtensorMap> cache;
+    static std::mutex mu;
+    static RpEncodeTiled encode = nullptr;
+    std::lock_guard<std::mutex> lock(mu);
+    const auto key = std::make_tuple(base, n_r, n_l, batch);
+    auto it = cache.find(key);
+    if (it != cache.end()) return &it->second;
+    if (!encode) {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+            qres != cudaDriverEntryPointSuccess)
+            return nullptr;
+        encode = (RpEncodeTiled)fn;
+    }
+    CUtensorMap m;
+    const cuuint64_t dims[4] = {16, (cuuint64_t)(n_r / 8), (cuuint64_t)n_l, (cuuint64_t)batch};
+    const cuuint64_t strides[3] = {128, (cuuint64_t)n_r * 16, (cuuint64_t)n_r * 16 * (cuuint64_t)n_l};
+    const cuuint32_t box[4] = {16, (cuuint32_t)(kTtCols / 8), (cuuint32_t)kTtRows, 1};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    if (encode(&m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<void *>(base), dims, strides, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return nullptr;
+    if (cache.size() > 64) cache.clear();
+    return &(cache[key] = m);
+}
+
+}  // namespace tdse
