@@ -738,7 +738,7 @@ int tdse_set_option(tdse_handle *h, const char *key, double value) {
     else if (k == "taylor_block") { if (value < 0 || value > 4) return TDSE_ERR_ARG; h->taylor_block = (int)value; }
     else if (k == "taylor_rt_variant") { if (value < -1 || value >= kNumRtVariants) return TDSE_ERR_ARG; h->rt_variant = (int)value; free_graphs(h); }
     else if (k == "taylor_rp_variant") { if (value < -1 || value >= kNumRpVariants) return TDSE_ERR_ARG; h->rp_variant = (int)value; free_graphs(h); }
-    else if (k == "apply_tma") { if (value < 0 || value > 1) return TDSE_ERR_ARG; h->apply_tma = (int)value; }
+    else if (k == "apply_tma") { if (value < 0 || value > 2) return TDSE_ERR_ARG; h->apply_tma = (int)value; }
     else if (k == "rk4_block") { if (value < 0 || value > 1) return TDSE_ERR_ARG; h->rk4_block = (int)value; free_graphs(h); }
     else if (k == "taylor_rp_tma") { if (value < -1 || value > 1) return TDSE_ERR_ARG; h->rp_tma = (int)value; free_graphs(h); }
     else if (k == "taylor_block_width") { if (value < 0 || value > 4096) return TDSE_ERR_ARG; h->bcfg.width_override = (int)value; free_graphs(h); }
@@ -815,7 +815,7 @@ int tdse_apply_H(tdse_handle *h, const void *psi_dev, void *out_dev, const doubl
     // (and the grid is many rounds of resident CTAs: small, L2-resident grids measured 8 % slower this way)
     const long apply_items = (long)((h->grid.n_r + kTtTW - 1) / kTtTW) * ((h->grid.n_l + kTtTL - 1) / kTtTL) * B;
     if (h->apply_tma && h->grid.gauge == 0 && (h->grid.n_r & 7) == 0 && ((uintptr_t)psi_dev & 15) == 0 &&
-        apply_items >= 6L * h->n_sm * kTtMinB) {
+        (h->apply_tma == 2 || apply_items >= 6L * h->n_sm * kTtMinB)) {
         const CUtensorMap *tm = tile_tensor_map(psi_dev, h->grid.n_r, h->grid.n_l, B);
         if (tm) {
             const int tiles_r = (h->grid.n_r + kTtTW - 1) / kTtTW, tiles_l = (h->grid.n_l + kTtTL - 1) / kTtTL;
