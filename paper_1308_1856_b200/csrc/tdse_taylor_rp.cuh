@@ -535,6 +535,26 @@ inline int rp_init_tables() {
     return cudaMemcpyToSymbol(kRpInvK, h, sizeof(h)) == cudaSuccess ? TDSE_OK : TDSE_ERR_CUDA;
 }
 
+// cuTensorMapEncodeTiled through the runtime (no link against libcuda)
+typedef CUresult (*RpEncodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+inline RpEncodeTiled rp_encode_fn() {
+    static RpEncodeTiled fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess && p &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = (RpEncodeTiled)p;
+        cudaGetLastError();
+    }
+    return fn;
+}
+
 struct RpPlan { int ok, variant, tma, cl, rk, W, H, WT, n_tiles, n_items, grid, threads; };   // rk = kernel MODE (0, 1, 2)   // cl: CTAs per cluster (1: none)
 
 // use_tma: -1 heuristic, 0 never, 1 whenever the layout allows it (n_r % 8 == 0, a full tile, 4-column patches)
@@ -560,8 +580,8 @@ inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant
         if (v.cp < hw) continue;
         if (rows >= 2 * g.n_l && v.nwr > 1) continue;      // more than half of the rows would be padding
         for (int tma = 0; tma <= 1; ++tma) {
-            if (tma && (use_tma == 0 || v.cp != 4 || (g.n_r & 7) || g.n_r <= WT)) continue;
-            if (!tma && use_tma == 1 && v.cp == 4 && !(g.n_r & 7) && g.n_r > WT) continue;
+            if (tma && (use_tma == 0 || v.cp != 4 || (g.n_r & 7) || g.n_r <= WT || !rp_encode_fn())) continue;
+            if (!tma && use_tma == 1 && v.cp == 4 && !(g.n_r & 7) && g.n_r > WT && rp_encode_fn()) continue;
             int H = order * hw;
             if (tma) H = (H + 7) & ~7;                      // tile starts on a 128-byte column group
             else if ((g.n_r & 1) == 0) H = (H + 1) & ~1;    // even halo: every patch row starts 32-byte aligned
@@ -596,28 +616,16 @@ inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant
     return best;
 }
 
-// cuTensorMapEncodeTiled through the runtime (no link against libcuda)
-typedef CUresult (*RpEncodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
-                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
 // tensor map of a state array seen as [batch*n_l rows][n_r/8 groups][16 doubles], box = rows x WT/8 x 16, cached
 inline const CUtensorMap *rp_tensor_map(const void *base, int n_r, int total_rows, int box_rows, int WT) {
     static std::map<std::tuple<const void *, int, int, int, int>, CUtensorMap> cache;
     static std::mutex mu;
-    static RpEncodeTiled encode = nullptr;
     std::lock_guard<std::mutex> lock(mu);
     const auto key = std::make_tuple(base, n_r, total_rows, box_rows, WT);
     auto it = cache.find(key);
     if (it != cache.end()) return &it->second;
-    if (!encode) {
-        void *fn = nullptr;
-        cudaDriverEntryPointQueryResult qres;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
-            qres != cudaDriverEntryPointSuccess)
-            return nullptr;
-        encode = (RpEncodeTiled)fn;
-    }
+    const RpEncodeTiled encode = rp_encode_fn();
+    if (!encode) return nullptr;
     CUtensorMap m;
     const cuuint64_t dims[3] = {16, (cuuint64_t)(n_r / 8), (cuuint64_t)total_rows};
     const cuuint64_t strides[2] = {128, (cuuint64_t)n_r * 16};          // bytes, dims 1 and 2

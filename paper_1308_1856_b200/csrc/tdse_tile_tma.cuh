@@ -99,19 +99,12 @@ tile_tma_kernel(GridDev g, Epi epi_in, const __grid_constant__ CUtensorMap tmap,
 inline const CUtensorMap *tile_tensor_map(const void *base, int n_r, int n_l, int batch) {
     static std::map<std::tuple<const void *, int, int, int>, CUtensorMap> cache;
     static std::mutex mu;
-    static RpEncodeTiled encode = nullptr;
     std::lock_guard<std::mutex> lock(mu);
     const auto key = std::make_tuple(base, n_r, n_l, batch);
     auto it = cache.find(key);
     if (it != cache.end()) return &it->second;
-    if (!encode) {
-        void *fn = nullptr;
-        cudaDriverEntryPointQueryResult qres;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
-            qres != cudaDriverEntryPointSuccess)
-            return nullptr;
-        encode = (RpEncodeTiled)fn;
-    }
+    const RpEncodeTiled encode = rp_encode_fn();
+    if (!encode) return nullptr;
     CUtensorMap m;
     const cuuint64_t dims[4] = {16, (cuuint64_t)(n_r / 8), (cuuint64_t)n_l, (cuuint64_t)batch};
     const cuuint64_t strides[3] = {128, (cuuint64_t)n_r * 16, (cuuint64_t)n_r * 16 * (cuuint64_t)n_l};
