@@ -130,6 +130,7 @@ struct tdse_handle {
     int rk4_block = 1, rk4_fused = 0;       // option: fuse the four RK4 stages; what the last tdse_step_rk4 used
     int imag = 0;                           // the running Taylor call is an imaginary-time propagation
     int apply_tma = 1;                      // tdse_apply_H: TMA-fetched tiles when n_r % 8 == 0
+    int lanczos_tma = 1;                    // Lanczos pass: sources fetched by TMA when n_r % 8 == 0
     double *d_sigma = nullptr;              // passive RK error sums [batch] (tdse_step_rk)
     double *d_mask = nullptr; double *d_pb = nullptr;   // absorber mask [n_r] (or null), bound populations [batch]
     double *d_elog = nullptr, *d_imag_inv = nullptr; size_t elog_cap = 0; long elog_rows = 0;
@@ -529,6 +530,36 @@ int enqueue_lanczos_block(tdse_handle *h, int K, int order, int n, int obs, cuda
             a.g_out = (p < K - 1) ? wbuf[p & 1] : nullptr;
             a.ef = ef; a.alpha = h->d_alpha; a.beta = h->d_beta; a.sc = h->d_inv; a.nrm = h->d_nrm; a.m_used = h->d_m;
             a.p = p; a.K = K; a.tol = h->beta_tol;
+            if (h->lanczos_tma && h->grid.gauge == 0 && (h->grid.n_r & 7) == 0 && rp_encode_fn()) {
+                // sources fetched by TMA (tdse_tile_tma.cuh); the maps are copied by value into the launch
+                const int tiles_r = (h->grid.n_r + kTtTW - 1) / kTtTW, tiles_l = (h->grid.n_l + kTtTL - 1) / kTtTL;
+                const int n_items = tiles_r * tiles_l * B;
+                CUtensorMap tm[3] = {};
+                bool ok = true;
+                for (int i = 0; i < 3 && ok; ++i) {
+                    const double2 *src = (i == 0) ? (p == 0 ? psi : a.g_in) : (i == 1 ? a.v1 : a.v2);
+                    if (!src) continue;
+                    const CUtensorMap *m = tile_tensor_map(src, h->grid.n_r, h->grid.n_l, B);
+                    if (m) tm[i] = *m; else ok = false;
+                }
+                if (ok) {
+                    static bool attr_set = false;
+                    if (!attr_set) {
+                        CU(cudaFuncSetAttribute(tile_tma3_kernel<3, EpiLanczosF>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTt3Smem));
+                        CU(cudaFuncSetAttribute(tile_tma3_kernel<5, EpiLanczosF>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTt3Smem));
+                        attr_set = true;
+                    }
+                    RedCtx rc{h->d_partials, h->d_counter, tiles_r * tiles_l};
+                    const int grid = std::min(n_items, h->n_sm * 2);
+                    if (h->grid.fd_order == 3)
+                        tile_tma3_kernel<3, EpiLanczosF><<<grid, 256, kTt3Smem, s>>>(h->gd, a, rc, tm[0], tm[1], tm[2], tiles_r, tiles_l, n_items);
+                    else
+                        tile_tma3_kernel<5, EpiLanczosF><<<grid, 256, kTt3Smem, s>>>(h->gd, a, rc, tm[0], tm[1], tm[2], tiles_r, tiles_l, n_items);
+                    count(h);
+                    CU(cudaGetLastError());
+                    continue;
+                }
+            }
             RC(launch_tile(h, a, s));
         }
         small_exp_kernel<<<B, 32, 0, s>>>(h->d_alpha, h->d_beta, h->d_m, &h->d_ctl->dt, K, order, h->d_coef, h->d_nsub);
@@ -739,6 +770,7 @@ int tdse_set_option(tdse_handle *h, const char *key, double value) {
     else if (k == "taylor_rt_variant") { if (value < -1 || value >= kNumRtVariants) return TDSE_ERR_ARG; h->rt_variant = (int)value; free_graphs(h); }
     else if (k == "taylor_rp_variant") { if (value < -1 || value >= kNumRpVariants) return TDSE_ERR_ARG; h->rp_variant = (int)value; free_graphs(h); }
     else if (k == "apply_tma") { if (value < 0 || value > 2) return TDSE_ERR_ARG; h->apply_tma = (int)value; }
+    else if (k == "lanczos_tma") { if (value < 0 || value > 1) return TDSE_ERR_ARG; h->lanczos_tma = (int)value; free_graphs(h); }
     else if (k == "rk4_block") { if (value < 0 || value > 1) return TDSE_ERR_ARG; h->rk4_block = (int)value; free_graphs(h); }
     else if (k == "taylor_rp_tma") { if (value < -1 || value > 1) return TDSE_ERR_ARG; h->rp_tma = (int)value; free_graphs(h); }
     else if (k == "taylor_block_width") { if (value < 0 || value > 4096) return TDSE_ERR_ARG; h->bcfg.width_override = (int)value; free_graphs(h); }

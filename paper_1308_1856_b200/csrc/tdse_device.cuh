@@ -158,4 +158,43 @@ __device__ __forceinline__ void grid_reduce_finish(double (&red)[NRED], const Re
     }
 }
 
+// The same in two parts for persistent kernels: a CTA stores one partial per WORK ITEM (slot = member *
+// items_per_member + item), and signs off once at its end; the last CTA to sign off finishes as above.
+template <int NT, int NRED>
+__device__ __forceinline__ void grid_store_partial(double (&red)[NRED], const RedCtx &rc, size_t slot, double *scratch) {
+    block_reduce<NT, NRED>(red, scratch);
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int r = 0; r < NRED; ++r) rc.partials[slot * NRED + r] = red[r];
+    }
+}
+template <int NT, int NRED, class Fin>
+__device__ __forceinline__ void grid_finish(const RedCtx &rc, int total_ctas, int n_members, Fin &fin, double *scratch,
+                                            int *flag) {
+    if (threadIdx.x == 0) {
+        __threadfence();
+        const unsigned int ticket = atomicAdd(rc.counter, 1u);
+        *flag = (ticket == (unsigned int)(total_ctas - 1));
+    }
+    __syncthreads();
+    if (!*flag) return;
+    __threadfence();
+    for (int b = 0; b < n_members; ++b) {
+        double s[NRED];
+#pragma unroll
+        for (int r = 0; r < NRED; ++r) s[r] = 0.0;
+        const double *p = rc.partials + (size_t)b * rc.ctas_per_member * NRED;
+        for (int i = threadIdx.x; i < rc.ctas_per_member; i += NT) {
+#pragma unroll
+            for (int r = 0; r < NRED; ++r) s[r] += __ldcg(p + (size_t)i * NRED + r);
+        }
+        block_reduce<NT, NRED>(s, scratch);
+        if (threadIdx.x == 0) fin.finish_member(b, s);
+    }
+    if (threadIdx.x == 0) {
+        fin.finish_all();
+        *rc.counter = 0u;
+    }
+}
+
 }  // namespace tdse

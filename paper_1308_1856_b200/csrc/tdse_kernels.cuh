@@ -328,6 +328,9 @@ struct EpiLanczosF : EpiBase {
         sc_prev = 0.0;
         if (p >= 2) { b2s2 = beta[b * K + p - 2]; sc_prev = sc[b * K + p - 2]; }
     }
+    __device__ __forceinline__ const double2 *src(int i) const {
+        return (i == 0) ? (p == 0 ? psi : g_in) : (i == 1 ? v1 : v2);
+    }
     // raw values of (g_{p-1} | psi), v_{p-1}, v_{p-2} at one point -> v_p
     __device__ __forceinline__ double2 combine(double2 g, double2 x1, double2 x2) const {
         if (p == 0) return g;

@@ -119,3 +119,102 @@ inline const CUtensorMap *tile_tensor_map(const void *base, int n_r, int n_l, in
 }
 
 }  // namespace tdse
+
+namespace tdse {
+
+// ------------------------------------------------------------------------------------------------------
+// The fused Lanczos pass (EpiLanczosF, tdse_kernels.cuh) with TMA-fetched sources: the vector v_p is formed from up to
+// three arrays (g_{p-1}, v_{p-1}, v_{p-2}); each source's box lands in its own raw buffer, the CTA combines them
+// into the tile (halo included; zero-filled raw data combine to zero, so the walls stay exact), and as soon as the
+// raw buffers are consumed the NEXT item's three boxes are requested -- they arrive during the H application,
+// the epilogue and the other resident CTA's phases.  One partial of the two fused reductions per work item; a CTA
+// signs off once (grid_finish).  grid = persistent CTAs, block = 256, 2 CTAs per SM (92 KB of shared memory each).
+// ------------------------------------------------------------------------------------------------------
+constexpr int kTt3Smem = 4 * (int)kTtStageBytes + 256;
+
+template <int FD, class Epi>
+__global__ void __launch_bounds__(256, 2)
+tile_tma3_kernel(GridDev g, Epi epi_in, RedCtx rc, const __grid_constant__ CUtensorMap tm0,
+                 const __grid_constant__ CUtensorMap tm1, const __grid_constant__ CUtensorMap tm2, int tiles_r, int tiles_l,
+                 int n_items) {
+    static_assert(Epi::CUSTOM_LOAD && Epi::NRED > 0, "multi-source epilogues with fused reductions");
+    constexpr int HW = (FD == 3) ? 1 : 2, COLS = kTtCols, ELEMS = kTtRows * kTtCols, NR = Epi::NRED;
+    (void)HW;
+    extern __shared__ __align__(1024) unsigned char t3_smem[];
+    double2 *raw = reinterpret_cast<double2 *>(t3_smem);                       // [3][ELEMS]
+    double2 *tile = raw + 3 * ELEMS;
+    unsigned long long *bar = reinterpret_cast<unsigned long long *>(t3_smem + 4 * kTtStageBytes);
+    double *red_s = reinterpret_cast<double *>(t3_smem + 4 * kTtStageBytes + 16);   // NR * 8 doubles
+    int *flag = reinterpret_cast<int *>(t3_smem + 4 * kTtStageBytes + 16 + sizeof(double) * NR * 8);
+    Epi epi = epi_in;
+    epi.begin();
+    if (epi.skip_all()) return;
+    const int tid = threadIdx.x;
+    if (tid == 0) mbar_init(bar, 1);
+    __syncthreads();
+    const int per_member = tiles_r * tiles_l;
+    const bool has1 = epi.src(1) != nullptr, has2 = epi.src(2) != nullptr;
+    auto fetch = [&](const int item) {
+        if (tid == 0 && item < n_items) {
+            const int b = item / per_member;
+            if (!epi.member_active(b)) return;
+            const int rest = item - b * per_member, tl = rest / tiles_r, tr = rest - tl * tiles_r;
+            const int c1 = tr * (kTtTW / 8) - kTtHalo / 8, c2 = tl * kTtTL - 1;
+            fence_proxy_async_smem();
+            mbar_expect_tx(bar, kTtStageBytes * (1u + (has1 ? 1u : 0u) + (has2 ? 1u : 0u)));
+            tma_load_4d(raw, &tm0, 0, c1, c2, b, bar);
+            if (has1) tma_load_4d(raw + ELEMS, &tm1, 0, c1, c2, b, bar);
+            if (has2) tma_load_4d(raw + 2 * ELEMS, &tm2, 0, c1, c2, b, bar);
+        }
+    };
+    fetch(blockIdx.x);
+
+    const int tx = tid % kTtTW, ty = tid / kTtTW;
+    unsigned phase = 0;
+    const double2 z2 = make_double2(0.0, 0.0);
+    for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+        const int b = item / per_member, rest = item - b * per_member, tl = rest / tiles_r, tr = rest - tl * tiles_r;
+        double red[NR];
+#pragma unroll
+        for (int r = 0; r < NR; ++r) red[r] = 0.0;
+        if (epi.member_active(b)) {
+            epi.prepare(b);
+            mbar_wait(bar, phase);
+            phase ^= 1u;
+            for (int i = tid; i < ELEMS; i += 256)
+                tile[i] = epi.combine(raw[i], has1 ? raw[ELEMS + i] : z2, has2 ? raw[2 * ELEMS + i] : z2);
+            __syncthreads();                               // tile complete, raw buffers consumed
+            fetch(item + gridDim.x);
+            const int j = tr * kTtTW + tx, l0 = tl * kTtTL;
+            if (j < g.n_r) {
+                const double vj = __ldg(g.vj + j), cen = __ldg(g.cen + j);
+                const double er = epi.efield(b) * (g.dr * (double)(j + 1));
+                const int r0 = ty * (kTtTL / 2);
+                const double2 *col = tile + (r0 + 1) * COLS + kTtHalo + tx;
+                double2 lo = col[-COLS], f = col[0];
+#pragma unroll
+                for (int rr = 0; rr < kTtTL / 2; ++rr) {
+                    const int l = l0 + r0 + rr;
+                    if (l >= g.n_l) break;
+                    const double2 *c = col + rr * COLS;
+                    const double2 up = c[COLS];
+                    const double2 fm1 = c[-1], fp1 = c[1];
+                    double2 fm2 = fm1, fp2 = fp1;
+                    if (FD == 5) { fm2 = c[-2]; fp2 = c[2]; }
+                    const double d = fma((double)(l * (l + 1)), cen, vj);
+                    const double cm = (l > 0) ? __ldg(g.cl + l - 1) : 0.0;
+                    const double cp = __ldg(g.cl + l);
+                    const double2 h = h_point<FD>(g, d, er, cm, cp, f, fm1, fp1, fm2, fp2, lo, up);
+                    epi.point(b, l, j, ((size_t)b * g.n_l + l) * g.n_r + j, f, h, red);
+                    lo = f; f = up;
+                }
+            }
+        } else {
+            fetch(item + gridDim.x);
+        }
+        grid_store_partial<256, NR>(red, rc, (size_t)item, red_s);    // (its barriers also fence the tile for the next item)
+    }
+    grid_finish<256, NR>(rc, gridDim.x, g.batch, epi, red_s, flag);
+}
+
+}  // namespace tdse

@@ -637,9 +637,10 @@ def test_rk_methods_parity(B, method, gauge):
     h.close()
 
 
-@pytest.mark.parametrize("fd,K", [(3, 16), (5, 7)])
-def test_lanczos_parity_and_internals(B, fd, K):
-    c = wl.config("cfg4", n_r=700, n_l=10, fd_order=fd)
+@pytest.mark.parametrize("fd,K,n_r", [(3, 16, 700), (5, 7, 700), (3, 16, 704), (5, 7, 704)])
+def test_lanczos_parity_and_internals(B, fd, K, n_r):
+    """n_r = 700: the register-staged pass; n_r = 704 (a multiple of 8): the sources are fetched by TMA."""
+    c = wl.config("cfg4", n_r=n_r, n_l=10, fd_order=fd)
     dt = wl.dt_eff(c, "lanczos", 12)
     nsteps = 20
     t0 = wl.window(c, nsteps, dt)
@@ -665,6 +666,25 @@ def test_lanczos_parity_and_internals(B, fd, K):
     assert np.max(np.abs(gi["alpha"][0] - info["alpha"])) <= 1e-5 * scale
     assert np.max(np.abs(gi["beta"][0, :K - 1] - info["beta"][:K - 1])) <= 1e-5 * scale
     assert np.max(np.abs(gi["coef"][0] - info["coef"])) <= 1e-9
+    h.close()
+
+
+@pytest.mark.parametrize("tma", [0, 1])
+def test_lanczos_batched_ragged_tma_and_staged(B, tma):
+    """Batched members with different fields, 11 of 16 rows, a ragged last column tile, 5-point stencil: the TMA
+    pass and the register-staged pass against the oracle and against each other."""
+    c = wl.config("cfg5", n_r=264, dr=0.1, n_l=11, fd_order=5, batch=3, order=12)
+    dt = wl.dt_eff(c, "lanczos", 12)
+    nsteps = 9
+    t0 = wl.window(c, nsteps, dt)
+    psi0 = wl.populated_state(c)
+    h, got, ref, gobs, robs = run_pair_fixed(B, c, "lanczos", nsteps, psi0, t0, dt, 3, [(0, 0)], {"lanczos_tma": tma},
+                                             K=6, order=12)
+    check_fixed(got, ref, gobs, robs)
+    h.set_option("lanczos_tma", 1 - tma)
+    h.set_state(psi0)
+    h.step_lanczos(6, 12, t0, dt, nsteps)
+    assert rel_l2(h.get_state(), got) <= 1e-12
     h.close()
 
 
