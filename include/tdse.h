@@ -72,10 +72,10 @@ void tdse_destroy(tdse_handle *h);
  *   "use_graph"        [1] capture blocks of steps in a CUDA graph
  *   "graph_steps"      [16] steps per captured graph
  *   "apply_tma"        [1] tdse_apply_H: tiles fetched by TMA tensor copies (zero fill outside the index box by the
- *                          hardware) when n_r % 8 == 0, the gauge is the length gauge and the grid is many rounds of
+ *                          hardware) when n_r % 8 == 0 and the grid is many rounds of
  *                          resident CTAs; 2: whenever the layout allows it; 0: the (l, r) tile kernel
  *   "lanczos_tma"      [1] Lanczos pass: the (up to three) source arrays of a tile are fetched by TMA when
- *                          n_r % 8 == 0 and the gauge is the length gauge; 0: register-staged tile kernel
+ *                          n_r % 8 == 0; 0: register-staged tile kernel
  *   "rk4_block"        [1] tdse_step_rk4: 1 all four stages in one pass over HBM (register-patch kernel in RK mode)
  *                          when the grid is at least one 128-column tile wide; 0 one kernel per stage
  *   "taylor_block"     [1] 0: one kernel per Taylor order; 1: temporally blocked step, all orders in one

@@ -530,7 +530,7 @@ int enqueue_lanczos_block(tdse_handle *h, int K, int order, int n, int obs, cuda
             a.g_out = (p < K - 1) ? wbuf[p & 1] : nullptr;
             a.ef = ef; a.alpha = h->d_alpha; a.beta = h->d_beta; a.sc = h->d_inv; a.nrm = h->d_nrm; a.m_used = h->d_m;
             a.p = p; a.K = K; a.tol = h->beta_tol;
-            if (h->lanczos_tma && h->grid.gauge == 0 && (h->grid.n_r & 7) == 0 && rp_encode_fn()) {
+            if (h->lanczos_tma && (h->grid.n_r & 7) == 0 && rp_encode_fn()) {
                 // sources fetched by TMA (tdse_tile_tma.cuh); the maps are copied by value into the launch
                 const int tiles_r = (h->grid.n_r + kTtTW - 1) / kTtTW, tiles_l = (h->grid.n_l + kTtTL - 1) / kTtTL;
                 const int n_items = tiles_r * tiles_l * B;
@@ -547,11 +547,18 @@ int enqueue_lanczos_block(tdse_handle *h, int K, int order, int n, int obs, cuda
                     if (!attr_set) {
                         CU(cudaFuncSetAttribute(tile_tma3_kernel<3, EpiLanczosF>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTt3Smem));
                         CU(cudaFuncSetAttribute(tile_tma3_kernel<5, EpiLanczosF>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTt3Smem));
+                        CU(cudaFuncSetAttribute(tile_tma3_kernel<3, EpiLanczosF, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTt3Smem));
+                        CU(cudaFuncSetAttribute(tile_tma3_kernel<5, EpiLanczosF, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTt3Smem));
                         attr_set = true;
                     }
                     RedCtx rc{h->d_partials, h->d_counter, tiles_r * tiles_l};
                     const int grid = std::min(n_items, h->n_sm * 2);
-                    if (h->grid.fd_order == 3)
+                    if (h->grid.gauge == 1) {
+                        if (h->grid.fd_order == 3)
+                            tile_tma3_kernel<3, EpiLanczosF, true><<<grid, 256, kTt3Smem, s>>>(h->gd, a, rc, tm[0], tm[1], tm[2], tiles_r, tiles_l, n_items);
+                        else
+                            tile_tma3_kernel<5, EpiLanczosF, true><<<grid, 256, kTt3Smem, s>>>(h->gd, a, rc, tm[0], tm[1], tm[2], tiles_r, tiles_l, n_items);
+                    } else if (h->grid.fd_order == 3)
                         tile_tma3_kernel<3, EpiLanczosF><<<grid, 256, kTt3Smem, s>>>(h->gd, a, rc, tm[0], tm[1], tm[2], tiles_r, tiles_l, n_items);
                     else
                         tile_tma3_kernel<5, EpiLanczosF><<<grid, 256, kTt3Smem, s>>>(h->gd, a, rc, tm[0], tm[1], tm[2], tiles_r, tiles_l, n_items);
@@ -846,7 +853,7 @@ int tdse_apply_H(tdse_handle *h, const void *psi_dev, void *out_dev, const doubl
     // tiles fetched by TMA (zero fill outside the index box by the hardware) when the layout allows it
     // (and the grid is many rounds of resident CTAs: small, L2-resident grids measured 8 % slower this way)
     const long apply_items = (long)((h->grid.n_r + kTtTW - 1) / kTtTW) * ((h->grid.n_l + kTtTL - 1) / kTtTL) * B;
-    if (h->apply_tma && h->grid.gauge == 0 && (h->grid.n_r & 7) == 0 && ((uintptr_t)psi_dev & 15) == 0 &&
+    if (h->apply_tma && (h->grid.n_r & 7) == 0 && ((uintptr_t)psi_dev & 15) == 0 &&
         (h->apply_tma == 2 || apply_items >= 6L * h->n_sm * kTtMinB)) {
         const CUtensorMap *tm = tile_tensor_map(psi_dev, h->grid.n_r, h->grid.n_l, B);
         if (tm) {
@@ -858,9 +865,15 @@ int tdse_apply_H(tdse_handle *h, const void *psi_dev, void *out_dev, const doubl
             if (!attr_set) {
                 CU(cudaFuncSetAttribute(tile_tma_kernel<3, EpiApply>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
                 CU(cudaFuncSetAttribute(tile_tma_kernel<5, EpiApply>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+                CU(cudaFuncSetAttribute(tile_tma_kernel<3, EpiApply, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+                CU(cudaFuncSetAttribute(tile_tma_kernel<5, EpiApply, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
                 attr_set = true;
             }
-            if (h->grid.fd_order == 3) tile_tma_kernel<3, EpiApply><<<grid, 256, smem, s>>>(h->gd, e, *tm, tiles_r, tiles_l, n_items);
+            const bool vg = h->grid.gauge == 1;
+            if (vg) {
+                if (h->grid.fd_order == 3) tile_tma_kernel<3, EpiApply, true><<<grid, 256, smem, s>>>(h->gd, e, *tm, tiles_r, tiles_l, n_items);
+                else tile_tma_kernel<5, EpiApply, true><<<grid, 256, smem, s>>>(h->gd, e, *tm, tiles_r, tiles_l, n_items);
+            } else if (h->grid.fd_order == 3) tile_tma_kernel<3, EpiApply><<<grid, 256, smem, s>>>(h->gd, e, *tm, tiles_r, tiles_l, n_items);
             else tile_tma_kernel<5, EpiApply><<<grid, 256, smem, s>>>(h->gd, e, *tm, tiles_r, tiles_l, n_items);
             count(h);
             CU(cudaGetLastError());

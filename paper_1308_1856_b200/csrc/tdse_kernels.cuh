@@ -42,6 +42,31 @@ __device__ __forceinline__ double2 h_point(const GridDev &g, double d, double er
     return h;
 }
 
+// Velocity-gauge coupling added to h (Eq. 12 in reading R-V2; afield = A(t)):
+//   -i A [ c_{l-1} (d/dr - l/r) f_{l-1} + c_l (d/dr + (l+1)/r) f_{l+1} ],  d/dr by P:119 Eq. 14 (R-V1).
+// c points at (l, j) of a shared-memory tile with row pitch `pitch` that holds the rows l-1 and l+1 with their radial halo.
+template <int FD>
+__device__ __forceinline__ void vg_couple(const GridDev &g, const double2 *c, int pitch, int l, double rinv, double cm,
+                                          double cp, double afield, double2 lo, double2 up, double2 &h) {
+    const double2 *cl_ = c - pitch, *cu_ = c + pitch;
+    double dlx, dly, dux, duy;
+    if (FD == 3) {
+        const double w = 0.5 / g.dr;
+        dlx = w * (cl_[1].x - cl_[-1].x); dly = w * (cl_[1].y - cl_[-1].y);
+        dux = w * (cu_[1].x - cu_[-1].x); duy = w * (cu_[1].y - cu_[-1].y);
+    } else {
+        const double w = 1.0 / (12.0 * g.dr);
+        dlx = w * (8.0 * (cl_[1].x - cl_[-1].x) - (cl_[2].x - cl_[-2].x));
+        dly = w * (8.0 * (cl_[1].y - cl_[-1].y) - (cl_[2].y - cl_[-2].y));
+        dux = w * (8.0 * (cu_[1].x - cu_[-1].x) - (cu_[2].x - cu_[-2].x));
+        duy = w * (8.0 * (cu_[1].y - cu_[-1].y) - (cu_[2].y - cu_[-2].y));
+    }
+    const double sx = cm * (dlx - (double)l * rinv * lo.x) + cp * (dux + (double)(l + 1) * rinv * up.x);
+    const double sy = cm * (dly - (double)l * rinv * lo.y) + cp * (duy + (double)(l + 1) * rinv * up.y);
+    h.x = fma(afield, sy, h.x);              // -i (sx + i sy) = sy - i sx
+    h.y = fma(-afield, sx, h.y);
+}
+
 // One pass: out/epilogue <- H(E_b) in, for every member b.  grid = (ceil(n_r/TW), ceil(n_l/TL), batch).
 // Epi supplies: NRED, SCALED; begin(); skip_all(); member_active(b); input(); in_scale(b); efield(b);
 // point(b,l,j,idx,f,h,red); finish_member(b,s); finish_all().
@@ -114,27 +139,7 @@ __global__ void __launch_bounds__(256, Epi::MINB) tile_kernel(GridDev g, Epi epi
                 const double cm = (l > 0) ? __ldg(g.cl + l - 1) : 0.0;
                 const double cp = __ldg(g.cl + l);
                 double2 h = h_point<FD>(g, d, VG ? 0.0 : er, cm, cp, f, fm1, fp1, fm2, fp2, lo, up);
-                if (VG) {
-                    // velocity gauge (Eq. 12 in reading R-V2; `afield` = A(t)):
-                    //   -i A [ c_{l-1} (d/dr - l/r) f_{l-1} + c_l (d/dr + (l+1)/r) f_{l+1} ],  d/dr by P:119 Eq. 14
-                    const double2 *cl_ = c - T::PITCH, *cu_ = c + T::PITCH;
-                    double dlx, dly, dux, duy;
-                    if (FD == 3) {
-                        const double w = 0.5 / g.dr;
-                        dlx = w * (cl_[1].x - cl_[-1].x); dly = w * (cl_[1].y - cl_[-1].y);
-                        dux = w * (cu_[1].x - cu_[-1].x); duy = w * (cu_[1].y - cu_[-1].y);
-                    } else {
-                        const double w = 1.0 / (12.0 * g.dr);
-                        dlx = w * (8.0 * (cl_[1].x - cl_[-1].x) - (cl_[2].x - cl_[-2].x));
-                        dly = w * (8.0 * (cl_[1].y - cl_[-1].y) - (cl_[2].y - cl_[-2].y));
-                        dux = w * (8.0 * (cu_[1].x - cu_[-1].x) - (cu_[2].x - cu_[-2].x));
-                        duy = w * (8.0 * (cu_[1].y - cu_[-1].y) - (cu_[2].y - cu_[-2].y));
-                    }
-                    const double sx = cm * (dlx - (double)l * rinv * lo.x) + cp * (dux + (double)(l + 1) * rinv * up.x);
-                    const double sy = cm * (dly - (double)l * rinv * lo.y) + cp * (duy + (double)(l + 1) * rinv * up.y);
-                    h.x = fma(afield, sy, h.x);              // -i (sx + i sy) = sy - i sx
-                    h.y = fma(-afield, sx, h.y);
-                }
+                if (VG) vg_couple<FD>(g, c, T::PITCH, l, rinv, cm, cp, afield, lo, up, h);
                 const size_t idx = ((size_t)b * g.n_l + l) * g.n_r + j;
                 epi.point(b, l, j, idx, f, h, red);
                 lo = f; f = up;

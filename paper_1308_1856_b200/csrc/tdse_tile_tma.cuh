@@ -29,7 +29,7 @@ __device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, i
 
 // grid = persistent CTAs, block = 256, dynamic shared = kTtStages * kTtStageBytes + 64.
 // items = batch x l-tiles x r-tiles (r fastest).  Epi must have NRED == 0 and a plain input.
-template <int FD, class Epi>
+template <int FD, class Epi, bool VG = false>
 __global__ void __launch_bounds__(256, kTtMinB)
 tile_tma_kernel(GridDev g, Epi epi_in, const __grid_constant__ CUtensorMap tmap, int tiles_r, int tiles_l, int n_items) {
     static_assert(Epi::NRED == 0 && !Epi::CUSTOM_LOAD && !Epi::TWO_IN && !Epi::SCALED, "single-source epilogues only");
@@ -69,7 +69,8 @@ tile_tma_kernel(GridDev g, Epi epi_in, const __grid_constant__ CUtensorMap tmap,
         phase ^= 1u << s;
         if (j < g.n_r && epi.member_active(b)) {
             const double vj = __ldg(g.vj + j), cen = __ldg(g.cen + j);
-            const double er = epi.efield(b) * (g.dr * (double)(j + 1));
+            const double afield = epi.efield(b), rinv = 1.0 / (g.dr * (double)(j + 1));
+            const double er = afield * (g.dr * (double)(j + 1));
             const int r0 = ty * (kTtTL / 2);
             const double2 *col = st + (size_t)s * kTtRows * COLS + (r0 + 1) * COLS + kTtHalo + tx;
             double2 lo = col[-COLS], f = col[0];
@@ -85,7 +86,8 @@ tile_tma_kernel(GridDev g, Epi epi_in, const __grid_constant__ CUtensorMap tmap,
                 const double d = fma((double)(l * (l + 1)), cen, vj);
                 const double cm = (l > 0) ? __ldg(g.cl + l - 1) : 0.0;
                 const double cp = __ldg(g.cl + l);
-                const double2 h = h_point<FD>(g, d, er, cm, cp, f, fm1, fp1, fm2, fp2, lo, up);
+                double2 h = h_point<FD>(g, d, VG ? 0.0 : er, cm, cp, f, fm1, fp1, fm2, fp2, lo, up);
+                if (VG) vg_couple<FD>(g, c, COLS, l, rinv, cm, cp, afield, lo, up, h);
                 epi.point(b, l, j, ((size_t)b * g.n_l + l) * g.n_r + j, f, h, red);
                 lo = f; f = up;
             }
@@ -132,7 +134,7 @@ namespace tdse {
 // ------------------------------------------------------------------------------------------------------
 constexpr int kTt3Smem = 4 * (int)kTtStageBytes + 256;
 
-template <int FD, class Epi>
+template <int FD, class Epi, bool VG = false>
 __global__ void __launch_bounds__(256, 2)
 tile_tma3_kernel(GridDev g, Epi epi_in, RedCtx rc, const __grid_constant__ CUtensorMap tm0,
                  const __grid_constant__ CUtensorMap tm1, const __grid_constant__ CUtensorMap tm2, int tiles_r, int tiles_l,
@@ -188,7 +190,8 @@ tile_tma3_kernel(GridDev g, Epi epi_in, RedCtx rc, const __grid_constant__ CUten
             const int j = tr * kTtTW + tx, l0 = tl * kTtTL;
             if (j < g.n_r) {
                 const double vj = __ldg(g.vj + j), cen = __ldg(g.cen + j);
-                const double er = epi.efield(b) * (g.dr * (double)(j + 1));
+                const double afield = epi.efield(b), rinv = 1.0 / (g.dr * (double)(j + 1));
+                const double er = afield * (g.dr * (double)(j + 1));
                 const int r0 = ty * (kTtTL / 2);
                 const double2 *col = tile + (r0 + 1) * COLS + kTtHalo + tx;
                 double2 lo = col[-COLS], f = col[0];
@@ -204,7 +207,8 @@ tile_tma3_kernel(GridDev g, Epi epi_in, RedCtx rc, const __grid_constant__ CUten
                     const double d = fma((double)(l * (l + 1)), cen, vj);
                     const double cm = (l > 0) ? __ldg(g.cl + l - 1) : 0.0;
                     const double cp = __ldg(g.cl + l);
-                    const double2 h = h_point<FD>(g, d, er, cm, cp, f, fm1, fp1, fm2, fp2, lo, up);
+                    double2 h = h_point<FD>(g, d, VG ? 0.0 : er, cm, cp, f, fm1, fp1, fm2, fp2, lo, up);
+                    if (VG) vg_couple<FD>(g, c, COLS, l, rinv, cm, cp, afield, lo, up, h);
                     epi.point(b, l, j, ((size_t)b * g.n_l + l) * g.n_r + j, f, h, red);
                     lo = f; f = up;
                 }

@@ -538,13 +538,14 @@ def test_apply_H_tma_tiles_parity(B, shape):
 
 
 # ------------------------------------------------------------------------------------------------- velocity gauge
-@pytest.mark.parametrize("shape", [(500, 8, 3, 1), (333, 11, 5, 3), (1300, 33, 5, 1), (37, 3, 3, 2)])
+@pytest.mark.parametrize("shape", [(500, 8, 3, 1), (333, 11, 5, 3), (1300, 33, 5, 1), (37, 3, 3, 2), (504, 9, 3, 2), (328, 11, 5, 3)])
 def test_velocity_gauge_apply_H_parity(B, shape):
     """H psi in the velocity gauge (Eq. 12 in reading R-V2, first derivative of Eq. 14) against the oracle."""
     import torch
     n_r, n_l, fd, batch = shape
     c = wl.config("cfg5" if batch > 1 else "cfg1", n_r=n_r, dr=0.1, n_l=n_l, fd_order=fd, batch=batch)
     g, h = both(B, c, gauge=1)
+    h.set_option("apply_tma", 2)                                # TMA-fetched tiles where n_r % 8 == 0
     x = wl.random_state(c)
     a = [0.3 + 0.07 * b for b in range(batch)]
     d_in = torch.from_numpy(x).cuda()
@@ -560,11 +561,12 @@ def test_velocity_gauge_apply_H_parity(B, shape):
     h.close()
 
 
+@pytest.mark.parametrize("n_r", [420, 424])
 @pytest.mark.parametrize("prop", ["taylor", "rk4", "lanczos", "rk45"])
-def test_velocity_gauge_propagators(B, prop):
+def test_velocity_gauge_propagators(B, prop, n_r):
     """Every propagator in the velocity gauge with the Hann-shaped vector potential (pulse kind 1) against the oracle;
     the all-orders-in-one-pass kernels do not apply and the per-order / per-stage kernels run."""
-    c = wl.config("cfg5", n_r=420, dr=0.1, n_l=7, fd_order=5, batch=2, order=4)
+    c = wl.config("cfg5", n_r=n_r, dr=0.1, n_l=7, fd_order=5, batch=2, order=4)      # 424: the Lanczos pass uses TMA
     g, h = both(B, c, gauge=1)
     pulses = [(0.06 + 0.02 * b, 0.3, 3.0, 0.2, 1) for b in range(2)]
     h.set_pulse(pulses)
