@@ -65,10 +65,11 @@ tile_tma_kernel(GridDev g, Epi epi_in, const __grid_constant__ CUtensorMap tmap,
         const int s = k % kTtStages;
         const int tr = item % tiles_r, rest = item / tiles_r, tl = rest % tiles_l, b = rest / tiles_l;
         const int j = tr * kTtTW + tx, l0 = tl * kTtTL;
+        // per-column coefficients first: their latency overlaps the wait for the tile
+        const double vj = (j < g.n_r) ? __ldg(g.vj + j) : 0.0, cen = (j < g.n_r) ? __ldg(g.cen + j) : 0.0;
         mbar_wait(&bars[s], (phase >> s) & 1u);
         phase ^= 1u << s;
         if (j < g.n_r && epi.member_active(b)) {
-            const double vj = __ldg(g.vj + j), cen = __ldg(g.cen + j);
             const double afield = epi.efield(b), rinv = 1.0 / (g.dr * (double)(j + 1));
             const double er = afield * (g.dr * (double)(j + 1));
             const int r0 = ty * (kTtTL / 2);
@@ -181,6 +182,9 @@ tile_tma3_kernel(GridDev g, Epi epi_in, RedCtx rc, const __grid_constant__ CUten
         for (int r = 0; r < NR; ++r) red[r] = 0.0;
         if (epi.member_active(b)) {
             epi.prepare(b);
+            // per-column coefficients first: their latency overlaps the wait for the sources
+            const int jc = tr * kTtTW + tx;
+            const double vj = (jc < g.n_r) ? __ldg(g.vj + jc) : 0.0, cen = (jc < g.n_r) ? __ldg(g.cen + jc) : 0.0;
             mbar_wait(bar, phase);
             phase ^= 1u;
             for (int i = tid; i < ELEMS; i += 256)
@@ -189,7 +193,6 @@ tile_tma3_kernel(GridDev g, Epi epi_in, RedCtx rc, const __grid_constant__ CUten
             fetch(item + gridDim.x);
             const int j = tr * kTtTW + tx, l0 = tl * kTtTL;
             if (j < g.n_r) {
-                const double vj = __ldg(g.vj + j), cen = __ldg(g.cen + j);
                 const double afield = epi.efield(b), rinv = 1.0 / (g.dr * (double)(j + 1));
                 const double er = afield * (g.dr * (double)(j + 1));
                 const int r0 = ty * (kTtTL / 2);
