@@ -90,7 +90,7 @@ void tdse_destroy(tdse_handle *h);
  *                          1: whenever n_r % 8 == 0 and the grid is wider than a tile)
  *   "lanczos_beta_tol" [1e-12] breakdown threshold on beta ("if beta = 0 then quit", R-G17)
  *   "rk45_dt_max"      [0 = none] cap on the adaptive step
- *   "rk45_check_every" [8] attempted steps enqueued between host checks of the device `done` flag */
+ *   "rk45_check_every" [32] attempted steps enqueued between host checks of the device `done` flag */
 int  tdse_set_option(tdse_handle *h, const char *key, double value);
 
 /* Absorbing boundary (Eq. 18): W(r) = (i/dt) ln{1 - cos^p[(pi/2)(1 - r/r_b)]} enters as a split step, i.e.

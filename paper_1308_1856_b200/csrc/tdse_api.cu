@@ -91,7 +91,7 @@ struct tdse_handle {
     size_t n_state = 0;                 // complex elements per state vector (B*L*N)
     cudaError_t last_cuda = cudaSuccess;
     // options
-    int field_sample = 0, use_graph = 1, graph_steps = 16, taylor_block = 1, rk45_check_every = 8;
+    int field_sample = 0, use_graph = 1, graph_steps = 16, taylor_block = 1, rk45_check_every = 32;
     double beta_tol = 1e-12, rk45_dt_max = 0.0;
     // device tables
     double *d_vj = nullptr, *d_cen = nullptr, *d_cl = nullptr;
