@@ -79,12 +79,7 @@ void tdse_destroy(tdse_handle *h);
  *   "rk4_block"        [1] tdse_step_rk4: 1 all four stages in one pass over HBM (register-patch kernel in RK mode)
  *                          when the grid is at least one 128-column tile wide; 0 one kernel per stage
  *   "taylor_block"     [1] 0: one kernel per Taylor order; 1: temporally blocked step, all orders in one
- *                          pass (persistent register-patch kernel when n_l <= 32, else the shared-memory tile
- *                          kernel when the tile fits, else falls back to 0); 2: shared-memory tile kernel only;
- *                          3: register-tile kernel (v2) only; 4: persistent register-patch kernel (v3) only
- *                          (each falls back to 0 when it does not apply)
- *   "taylor_block_width" [0] interior tile width W of the shared-memory tile kernel (0: heuristic)
- *   "taylor_rt_variant" [-1] instantiation of the register-tile kernel (-1: heuristic)
+ *                          pass over HBM (persistent register-patch kernel; n_l <= 128, else falls back to 0)
  *   "taylor_rp_variant" [-1] instantiation of the register-patch kernel (-1: heuristic)
  *   "taylor_rp_tma"    [-1] register-patch kernel: fetch tiles by TMA tensor copies (-1: heuristic, 0: never,
  *                          1: whenever n_r % 8 == 0 and the grid is wider than a tile)
@@ -100,7 +95,7 @@ int  tdse_set_option(tdse_handle *h, const char *key, double value);
  * imaginary-time propagation ignores it.  Synchronises the device. */
 int  tdse_set_absorber(tdse_handle *h, double r_b, int p);
 
-/* One pulse per member, host array [batch]. */
+/* One pulse per member, host array [batch].  TDSE_ERR_UNSUPPORTED for a kind-0 pulse on a velocity-gauge handle. */
 int  tdse_set_pulse(tdse_handle *h, const tdse_pulse *per_member_host);
 
 /* Real bound-state vectors for the population observable p_s = |dr sum_j phi_s[j] f_{l_s,j}|^2
@@ -173,11 +168,19 @@ int  tdse_dt_log(tdse_handle *h, double *dt_host, double *err_host, long max, lo
  * complex (re, im); m_used, n_sub host [batch] (dimension used after breakdown, Taylor sub-steps). Any may be NULL. */
 int  tdse_lanczos_info(tdse_handle *h, double *alpha, double *beta, double *coef, int *m_used, int *n_sub);
 
+/* Ionisation yield of the current state from the bound-state populations (CFG5 of BASELINE.json: "final ionisation
+ * yield 1 - sum of bound populations per member"; Eq. 25 generalised to every supplied bound state, reading
+ * R-G23): out_host [batch] = 1 - sum_s p_s over the states of tdse_set_bound_states.  Synchronises `stream`. */
+int  tdse_ionisation_yield(tdse_handle *h, double *out_host, void *stream);
+
 /* Number of CUDA kernels this handle has launched so far (graph nodes counted per graph launch). */
 long tdse_launch_count(tdse_handle *h);
-/* Kernel used by the last tdse_step_taylor call (after tdse_step_rk4: 3 / 4 if the four stages ran fused, else 0): 0 one kernel per order, 1 shared-memory tile kernel (all orders in
- * one pass), 2 register-tile kernel v2, 3 persistent register-patch kernel v3 with direct global loads, 4 the same
- * with TMA tile fetches (1-4: all orders in one pass). */
+/* Number of CUDA graphs this handle has captured and instantiated so far (a step call does that on first use of a
+ * (propagator, order, block length, ...) combination; a timed region should see this number unchanged). */
+long tdse_graph_instantiations(tdse_handle *h);
+/* Kernel used by the last tdse_step_taylor call (after tdse_step_rk4: 3 / 4 if the four stages ran fused, else 0):
+ * 0 one kernel per order, 3 persistent register-patch kernel with direct global loads, 4 the same with TMA tile
+ * fetches (3, 4: all orders in one pass). */
 int  tdse_taylor_was_blocked(tdse_handle *h);
 
 const char *tdse_strerror(int code);

@@ -19,7 +19,7 @@ ERRORS = {-1: "TDSE_ERR_ARG", -2: "TDSE_ERR_ALLOC", -3: "TDSE_ERR_CUDA", -4: "TD
 SYMBOLS = ["tdse_create", "tdse_destroy", "tdse_set_option", "tdse_set_pulse", "tdse_set_bound_states",
            "tdse_set_state", "tdse_get_state", "tdse_apply_H", "tdse_set_absorber", "tdse_bound_population", "tdse_step_taylor", "tdse_step_imag", "tdse_energy_log", "tdse_step_rk4", "tdse_step_rk", "tdse_rk_sigma",
            "tdse_step_lanczos", "tdse_step_rk45", "tdse_observables", "tdse_obs_log", "tdse_dt_log",
-           "tdse_lanczos_info", "tdse_launch_count", "tdse_taylor_was_blocked", "tdse_strerror", "tdse_version"]
+           "tdse_lanczos_info", "tdse_ionisation_yield", "tdse_graph_instantiations", "tdse_launch_count", "tdse_taylor_was_blocked", "tdse_strerror", "tdse_version"]
 
 
 class TdseError(RuntimeError):
@@ -75,6 +75,9 @@ def lib():
         L.tdse_lanczos_info.argtypes = [vp, dp, dp, dp, ip, ip]
         L.tdse_launch_count.argtypes = [vp]
         L.tdse_launch_count.restype = C.c_long
+        L.tdse_graph_instantiations.argtypes = [vp]
+        L.tdse_graph_instantiations.restype = C.c_long
+        L.tdse_ionisation_yield.argtypes = [vp, dp, vp]
         L.tdse_taylor_was_blocked.argtypes = [vp]
         L.tdse_strerror.argtypes = [C.c_int]
         L.tdse_strerror.restype = C.c_char_p
@@ -277,12 +280,21 @@ class Tdse:
                "tdse_lanczos_info")
         return {"alpha": alpha, "beta": beta, "coef": coef, "m": m, "n_sub": ns}
 
+    def ionisation_yield(self, stream=None):
+        """1 - sum of the bound-state populations of the current state, per member."""
+        out = np.zeros(self.grid.batch)
+        _check(lib().tdse_ionisation_yield(self._h, _dp(out), _stream(stream)), "tdse_ionisation_yield")
+        return out
+
     def launch_count(self):
         return int(lib().tdse_launch_count(self._h))
+
+    def graph_instantiations(self):
+        return int(lib().tdse_graph_instantiations(self._h))
 
     def taylor_was_blocked(self):
         return bool(lib().tdse_taylor_was_blocked(self._h))
 
     def taylor_kernel(self):
-        """0: one kernel per order, 1: shared-memory tile kernel, 2: register-tile kernel (last step_taylor call)."""
+        """0: one kernel per order, 3 / 4: all orders in one pass (direct loads / TMA tile fetches)."""
         return int(lib().tdse_taylor_was_blocked(self._h))

@@ -2,30 +2,52 @@
 
 nvcc cross-compiles without a GPU.  The library links the static CUDA runtime, so loading it needs no GPU;
 every compute entry point returns TDSE_ERR_CUDA when no device is present (there is no CPU fallback).
+The translation units are compiled in parallel into paper_1308_1856_b200/build/*.o and linked.
 """
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libtdse_b200.so")
-SOURCES = [os.path.join(CSRC, "tdse_api.cu")]
-DEPS = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(ROOT, "include", "tdse.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 
 
-def nvcc_cmd(extra=()):
-    return [NVCC, "-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-            "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", *extra, "-o", LIB, *SOURCES]
+def sources():
+    return sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith(".cu"))
+
+
+def deps():
+    return [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(ROOT, "include", "tdse.h")]
+
+
+def compile_cmd(src, obj, extra=()):
+    return [NVCC, "-std=c++17", "-O3", *ARCH, "-lineinfo", "-Xcompiler", "-fPIC", *extra, "-c", "-o", obj, src]
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= max(os.path.getmtime(d) for d in DEPS):
+    newest = max(os.path.getmtime(d) for d in deps())
+    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
         return LIB
-    cmd = nvcc_cmd(("-Xptxas", "-v") if verbose else ())
-    subprocess.run(cmd, check=True)
+    os.makedirs(OBJ, exist_ok=True)
+    extra = ("-Xptxas", "-v") if verbose else ()
+    jobs = []
+    for src in sources():
+        obj = os.path.join(OBJ, os.path.basename(src)[:-3] + ".o")
+        if force or not os.path.exists(obj) or os.path.getmtime(obj) < newest:
+            jobs.append(compile_cmd(src, obj, extra))
+    with ThreadPoolExecutor(max_workers=max(1, min(len(jobs), os.cpu_count() or 1))) as ex:
+        for r in ex.map(lambda c: subprocess.run(c, capture_output=not verbose, text=True), jobs):
+            if r.returncode != 0:
+                sys.stderr.write((r.stdout or "") + (r.stderr or ""))
+                raise subprocess.CalledProcessError(r.returncode, r.args)
+    objs = [os.path.join(OBJ, os.path.basename(s)[:-3] + ".o") for s in sources()]
+    subprocess.run([NVCC, *ARCH, "-shared", "-cudart", "static", "-o", LIB, *objs], check=True)
     return LIB
 
 

@@ -13,10 +13,8 @@
 #include <vector>
 
 #include "tdse_kernels.cuh"
-#include "tdse_taylor_blocked.cuh"
-#include "tdse_taylor_rp.cuh"
+#include "tdse_taylor_rp_plan.h"
 #include "tdse_tile_tma.cuh"
-#include "tdse_taylor_rt.cuh"
 
 using namespace tdse;
 
@@ -34,6 +32,10 @@ using namespace tdse;
         int rc_ = (call);            \
         if (rc_ != TDSE_OK) return rc_; \
     } while (0)
+
+namespace tdse {
+bool tma_available() { return tma_encode_fn() != nullptr; }
+}  // namespace tdse
 
 namespace {
 enum Role { R_PSI = 0, R_G0 = 1, R_G1 = 2, R_K0 = 3 };
@@ -109,7 +111,8 @@ struct tdse_handle {
     unsigned int *d_counter = nullptr;
     // observables
     int n_states = 0; double *d_phi = nullptr; int *d_lstate = nullptr;
-    double *d_obs_partials = nullptr; double2 *d_amp = nullptr; unsigned int *d_obs_counters = nullptr;
+    double *d_obs_partials = nullptr; int *d_loff = nullptr, *d_slist = nullptr; unsigned int *d_obs_counters = nullptr;
+    double *d_yield = nullptr;
     double *d_rows = nullptr; size_t rows_cap = 0; long log_rows = 0; double *d_row_direct = nullptr;
     // rk45 logs
     double *d_dtlog = nullptr, *d_errlog = nullptr, *d_replay = nullptr; long log_cap = 0, replay_cap = 0;
@@ -121,11 +124,9 @@ struct tdse_handle {
     cudaStream_t cap_stream = nullptr;
     std::map<std::tuple<int, int, int, int, int, int>, cudaGraphExec_t> graphs;
     std::map<std::tuple<int, int, int, int, int, int>, long> graph_nodes;
-    long launches = 0; long pending = 0; bool capturing = false;
-    int taylor_blocked_last = 0;        // 0: one kernel per order, 1: shared-memory tile kernel, 2: register-tile kernel (v2), 3: persistent register patches (v3)
+    long launches = 0; long pending = 0; long graph_inst = 0; bool capturing = false;
+    int taylor_blocked_last = 0;        // 0: one kernel per order, 3: all orders in one pass (persistent register-patch kernel)
     // blocked Taylor configuration
-    BlockedCfg bcfg{};
-    RtPlan rtp{}; int rt_variant = -1;
     RpPlan rpp{}; int n_sm = 148; int rp_variant = -1, rp_tma = -1;
     int rk4_block = 1, rk4_fused = 0;       // option: fuse the four RK4 stages; what the last tdse_step_rk4 used
     int imag = 0;                           // the running Taylor call is an imaginary-time propagation
@@ -215,17 +216,22 @@ int obs_chunks(const tdse_handle *h) { return obs_chunks_r(h) * obs_chunks_l(h);
 int enqueue_obs(tdse_handle *h, const double2 *psi, int step_off, int predicated, int use_direct, double t_direct,
                 double *rows, cudaStream_t s) {
     const int B = h->grid.batch;
-    if (obs_chunks_r(h) * ((h->grid.n_l + kObsRows - 1) / kObsRows) + h->n_states <= 8) {   // small grid: one CTA per member
+    if (obs_chunks_r(h) * ((h->grid.n_l + kObsRows - 1) / kObsRows) <= 8 && h->n_states <= 4) {   // small grid: one CTA per member
         obs_small_kernel<<<B, 256, 0, s>>>(h->gd, psi, h->d_phi, h->d_lstate, h->n_states, h->d_pulse, h->d_ctl, step_off,
                                            predicated, use_direct, t_direct, rows);
         count(h);
         CU(cudaGetLastError());
         return TDSE_OK;
     }
-    obs_kernel<<<dim3(obs_chunks_r(h), B, obs_chunks_l(h) + h->n_states), 256, 0, s>>>(
-        h->gd, psi, h->d_phi, h->d_lstate, h->n_states, h->d_pulse, h->d_ctl, step_off, predicated, use_direct, t_direct,
-        h->d_obs_partials, h->d_amp, h->d_obs_counters, rows, obs_rows_per(h));
+    obs_kernel<<<dim3(obs_chunks_r(h), B, obs_chunks_l(h)), 256, 0, s>>>(
+        h->gd, psi, h->n_states, h->d_pulse, h->d_ctl, step_off, predicated, use_direct, t_direct, h->d_obs_partials,
+        h->d_obs_counters, rows, obs_rows_per(h));
     count(h);
+    if (h->n_states > 0) {
+        pop_kernel<<<dim3(h->grid.n_l, B), 256, 0, s>>>(h->gd, psi, h->d_phi, h->d_loff, h->d_slist, h->n_states, h->d_ctl,
+                                                         step_off, predicated, use_direct, rows);
+        count(h);
+    }
     CU(cudaGetLastError());
     return TDSE_OK;
 }
@@ -286,12 +292,9 @@ int enqueue_taylor_block(tdse_handle *h, int order, int n, int obs, cudaStream_t
         if (h->taylor_blocked_last) {
             // ping-pong psi <-> acc: even steps read psi, odd steps read acc (n is even inside graphs)
             double2 *src = (i & 1) ? acc : psi, *dst = (i & 1) ? psi : acc;
-            if (h->taylor_blocked_last == 3) RC(launch_taylor_rp(h->gd, h->rpp, src, dst, ef, &h->d_ctl->dt, order, s));
-            else if (h->taylor_blocked_last == 2) RC(launch_taylor_rt(h->gd, h->rtp, src, dst, ef, &h->d_ctl->dt, order, s));
-            else RC(launch_taylor_blocked(h->bcfg, h->gd, src, dst, ef, &h->d_ctl->dt, order, s));
+            RC(launch_taylor_rp(h->gd, h->rpp, src, dst, ef, &h->d_ctl->dt, order, s));
             count(h);
             if (h->imag) RC(enqueue_imag_norm(h, dst, i, s));
-            else if (h->taylor_blocked_last != 3) RC(enqueue_mask(h, dst, s));      // (v3 applies it in its store)
             if (obs) RC(enqueue_obs(h, dst, i, 1, 0, 0.0, h->d_rows, s));
             continue;
         }
@@ -530,7 +533,7 @@ int enqueue_lanczos_block(tdse_handle *h, int K, int order, int n, int obs, cuda
             a.g_out = (p < K - 1) ? wbuf[p & 1] : nullptr;
             a.ef = ef; a.alpha = h->d_alpha; a.beta = h->d_beta; a.sc = h->d_inv; a.nrm = h->d_nrm; a.m_used = h->d_m;
             a.p = p; a.K = K; a.tol = h->beta_tol;
-            if (h->lanczos_tma && (h->grid.n_r & 7) == 0 && rp_encode_fn()) {
+            if (h->lanczos_tma && (h->grid.n_r & 7) == 0 && tma_available()) {
                 // sources fetched by TMA (tdse_tile_tma.cuh); the maps are copied by value into the launch
                 const int tiles_r = (h->grid.n_r + kTtTW - 1) / kTtTW, tiles_l = (h->grid.n_l + kTtTL - 1) / kTtTL;
                 const int n_items = tiles_r * tiles_l * B;
@@ -539,17 +542,15 @@ int enqueue_lanczos_block(tdse_handle *h, int K, int order, int n, int obs, cuda
                 for (int i = 0; i < 3 && ok; ++i) {
                     const double2 *src = (i == 0) ? (p == 0 ? psi : a.g_in) : (i == 1 ? a.v1 : a.v2);
                     if (!src) continue;
-                    const CUtensorMap *m = tile_tensor_map(src, h->grid.n_r, h->grid.n_l, B);
-                    if (m) tm[i] = *m; else ok = false;
+                    ok = tile_tensor_map(&tm[i], src, h->grid.n_r, h->grid.n_l, B);
                 }
                 if (ok) {
-                    static bool attr_set = false;
-                    if (!attr_set) {
+                    static DeviceOnce attr_once;
+                    if (attr_once.first()) {
                         CU(cudaFuncSetAttribute(tile_tma3_kernel<3, EpiLanczosF>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTt3Smem));
                         CU(cudaFuncSetAttribute(tile_tma3_kernel<5, EpiLanczosF>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTt3Smem));
                         CU(cudaFuncSetAttribute(tile_tma3_kernel<3, EpiLanczosF, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTt3Smem));
                         CU(cudaFuncSetAttribute(tile_tma3_kernel<5, EpiLanczosF, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTt3Smem));
-                        attr_set = true;
                     }
                     RedCtx rc{h->d_partials, h->d_counter, tiles_r * tiles_l};
                     const int grid = std::min(n_items, h->n_sm * 2);
@@ -609,7 +610,7 @@ int run_blocks(tdse_handle *h, int kind, int p1, int p2, int n, int obs, long nb
         }
         return TDSE_OK;
     }
-    const auto key = std::make_tuple(kind, p1, p2, n, obs + 2 * h->taylor_blocked_last + 16 * (h->rtp.variant + 1) + 256 * (h->rpp.variant + 1) + 8192 * h->rpp.tma + 16384 * h->rk4_fused + 32768 * h->imag, h->psi_slot);
+    const auto key = std::make_tuple(kind, p1, p2, n, obs + 2 * h->taylor_blocked_last + 256 * (h->rpp.variant + 1) + 8192 * h->rpp.tma + 16384 * h->rk4_fused + 32768 * h->imag, h->psi_slot);
     auto it = h->graphs.find(key);
     if (it == h->graphs.end()) {
         cudaGraph_t g = nullptr;
@@ -624,6 +625,7 @@ int run_blocks(tdse_handle *h, int kind, int p1, int p2, int n, int obs, long nb
         cudaGraphDestroy(g);
         CU(ie);
         h->graph_nodes[key] = h->pending;
+        ++h->graph_inst;
         it = h->graphs.emplace(key, ex).first;
     }
     const long nodes = h->graph_nodes[key];
@@ -699,7 +701,7 @@ int tdse_create(const tdse_grid *grid, tdse_handle **out) {
             cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n_sm > 0)
             h->n_sm = n_sm;
     }
-    if (rp_init_tables() != TDSE_OK) { delete h; return TDSE_ERR_CUDA; }
+    if ((grid->fd_order == 3 ? rp_init_fd3() : rp_init_fd5()) != TDSE_OK) { delete h; return TDSE_ERR_CUDA; }
     const int N = grid->n_r, L = grid->n_l, B = grid->batch;
     h->n_state = (size_t)N * L * B;
     auto fail = [&](int rc) { tdse_destroy(h); return rc; };
@@ -743,7 +745,6 @@ int tdse_create(const tdse_grid *grid, tdse_handle **out) {
         CU(cudaMalloc(&h->d_row_direct, sizeof(double) * 3 * B));
         CU(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
         RC(ensure_pool(h, 1));
-        RC(blocked_configure(&h->bcfg, h->grid));
         return TDSE_OK;
     };
     const int rc = body();
@@ -758,7 +759,7 @@ void tdse_destroy(tdse_handle *h) {
     free_graphs(h);
     for (double2 *p : h->pool) cudaFree(p);
     void *ptrs[] = {h->d_vj, h->d_cen, h->d_cl, h->d_pulse, h->d_bufs, h->d_ctl, h->d_etab, h->d_eapply, h->d_partials,
-                    h->d_counter, h->d_phi, h->d_lstate, h->d_obs_partials, h->d_obs_counters, h->d_elog, h->d_imag_inv, h->d_mask, h->d_pb, h->d_sigma, h->d_amp, h->d_rows, h->d_row_direct,
+                    h->d_counter, h->d_phi, h->d_lstate, h->d_obs_partials, h->d_obs_counters, h->d_elog, h->d_imag_inv, h->d_mask, h->d_pb, h->d_sigma, h->d_loff, h->d_slist, h->d_yield, h->d_rows, h->d_row_direct,
                     h->d_dtlog, h->d_errlog, h->d_replay, h->d_alpha, h->d_beta, h->d_nrm, h->d_inv, h->d_coef,
                     h->d_m, h->d_nsub, h->d_basis};
     for (void *p : ptrs) if (p) cudaFree(p);
@@ -773,14 +774,12 @@ int tdse_set_option(tdse_handle *h, const char *key, double value) {
     if (k == "field_sample") { if (value != 0.0 && value != 1.0) return TDSE_ERR_ARG; h->field_sample = (int)value; }
     else if (k == "use_graph") h->use_graph = value != 0.0;
     else if (k == "graph_steps") { if (value < 1 || value > 4096) return TDSE_ERR_ARG; h->graph_steps = (int)value; }
-    else if (k == "taylor_block") { if (value < 0 || value > 4) return TDSE_ERR_ARG; h->taylor_block = (int)value; }
-    else if (k == "taylor_rt_variant") { if (value < -1 || value >= kNumRtVariants) return TDSE_ERR_ARG; h->rt_variant = (int)value; free_graphs(h); }
+    else if (k == "taylor_block") { if (value != 0.0 && value != 1.0) return TDSE_ERR_ARG; h->taylor_block = (int)value; }
     else if (k == "taylor_rp_variant") { if (value < -1 || value >= kNumRpVariants) return TDSE_ERR_ARG; h->rp_variant = (int)value; free_graphs(h); }
     else if (k == "apply_tma") { if (value < 0 || value > 2) return TDSE_ERR_ARG; h->apply_tma = (int)value; }
     else if (k == "lanczos_tma") { if (value < 0 || value > 1) return TDSE_ERR_ARG; h->lanczos_tma = (int)value; free_graphs(h); }
     else if (k == "rk4_block") { if (value < 0 || value > 1) return TDSE_ERR_ARG; h->rk4_block = (int)value; free_graphs(h); }
     else if (k == "taylor_rp_tma") { if (value < -1 || value > 1) return TDSE_ERR_ARG; h->rp_tma = (int)value; free_graphs(h); }
-    else if (k == "taylor_block_width") { if (value < 0 || value > 4096) return TDSE_ERR_ARG; h->bcfg.width_override = (int)value; free_graphs(h); }
     else if (k == "lanczos_beta_tol") { if (!(value >= 0.0)) return TDSE_ERR_ARG; h->beta_tol = value; free_graphs(h); }
     else if (k == "rk45_dt_max") { if (!(value >= 0.0)) return TDSE_ERR_ARG; h->rk45_dt_max = value; }
     else if (k == "rk45_check_every") { if (value < 1 || value > 1024) return TDSE_ERR_ARG; h->rk45_check_every = (int)value; }
@@ -790,6 +789,9 @@ int tdse_set_option(tdse_handle *h, const char *key, double value) {
 
 int tdse_set_pulse(tdse_handle *h, const tdse_pulse *p) {
     if (!h || !p) return TDSE_ERR_ARG;
+    if (h->grid.gauge == 1)             // the velocity gauge needs A(t): kind-1 pulses (or the static test aid omega = 0)
+        for (int b = 0; b < h->grid.batch; ++b)
+            if (p[b].omega != 0.0 && p[b].kind != 1) return TDSE_ERR_UNSUPPORTED;
     CU(cudaDeviceSynchronize());
     CU(cudaMemcpy(h->d_pulse, p, sizeof(tdse_pulse) * h->grid.batch, cudaMemcpyHostToDevice));
     return TDSE_OK;
@@ -802,7 +804,8 @@ int tdse_set_bound_states(tdse_handle *h, int n_states, const int *l_of_state, c
     free_graphs(h);
     if (h->d_phi) { cudaFree(h->d_phi); h->d_phi = nullptr; }
     if (h->d_lstate) { cudaFree(h->d_lstate); h->d_lstate = nullptr; }
-    if (h->d_amp) { cudaFree(h->d_amp); h->d_amp = nullptr; }
+    if (h->d_loff) { cudaFree(h->d_loff); h->d_loff = nullptr; }
+    if (h->d_slist) { cudaFree(h->d_slist); h->d_slist = nullptr; }
     if (h->d_rows) { cudaFree(h->d_rows); h->d_rows = nullptr; h->rows_cap = 0; }
     if (h->d_row_direct) { cudaFree(h->d_row_direct); h->d_row_direct = nullptr; }
     h->n_states = n_states;
@@ -811,7 +814,16 @@ int tdse_set_bound_states(tdse_handle *h, int n_states, const int *l_of_state, c
     if (n_states > 0) {
         CU(cudaMalloc(&h->d_phi, sizeof(double) * (size_t)n_states * h->grid.n_r));
         CU(cudaMalloc(&h->d_lstate, sizeof(int) * n_states));
-        CU(cudaMalloc(&h->d_amp, sizeof(double2) * (size_t)n_states * h->grid.batch * obs_chunks_r(h)));
+        // states grouped by partial wave for pop_kernel: l_off[l] .. l_off[l+1] indexes state_list
+        std::vector<int> loff(h->grid.n_l + 1, 0), slist(n_states);
+        for (int s = 0; s < n_states; ++s) ++loff[l_of_state[s] + 1];
+        for (int l = 0; l < h->grid.n_l; ++l) loff[l + 1] += loff[l];
+        std::vector<int> fill(loff.begin(), loff.end() - 1);
+        for (int s = 0; s < n_states; ++s) slist[fill[l_of_state[s]]++] = s;
+        CU(cudaMalloc(&h->d_loff, sizeof(int) * loff.size()));
+        CU(cudaMalloc(&h->d_slist, sizeof(int) * n_states));
+        CU(cudaMemcpy(h->d_loff, loff.data(), sizeof(int) * loff.size(), cudaMemcpyHostToDevice));
+        CU(cudaMemcpy(h->d_slist, slist.data(), sizeof(int) * n_states, cudaMemcpyHostToDevice));
         CU(cudaMemcpy(h->d_phi, phi, sizeof(double) * (size_t)n_states * h->grid.n_r, cudaMemcpyHostToDevice));
         CU(cudaMemcpy(h->d_lstate, l_of_state, sizeof(int) * n_states, cudaMemcpyHostToDevice));
     }
@@ -855,19 +867,19 @@ int tdse_apply_H(tdse_handle *h, const void *psi_dev, void *out_dev, const doubl
     const long apply_items = (long)((h->grid.n_r + kTtTW - 1) / kTtTW) * ((h->grid.n_l + kTtTL - 1) / kTtTL) * B;
     if (h->apply_tma && (h->grid.n_r & 7) == 0 && ((uintptr_t)psi_dev & 15) == 0 &&
         (h->apply_tma == 2 || apply_items >= 6L * h->n_sm * kTtMinB)) {
-        const CUtensorMap *tm = tile_tensor_map(psi_dev, h->grid.n_r, h->grid.n_l, B);
-        if (tm) {
+        CUtensorMap tmv{};
+        const CUtensorMap *tm = &tmv;
+        if (tile_tensor_map(&tmv, psi_dev, h->grid.n_r, h->grid.n_l, B)) {
             const int tiles_r = (h->grid.n_r + kTtTW - 1) / kTtTW, tiles_l = (h->grid.n_l + kTtTL - 1) / kTtTL;
             const int n_items = tiles_r * tiles_l * B;
             const int smem = kTtStages * (int)kTtStageBytes + 64;
             const int grid = std::min(n_items, h->n_sm * kTtMinB);
-            static bool attr_set = false;
-            if (!attr_set) {
+            static DeviceOnce attr_once;
+            if (attr_once.first()) {
                 CU(cudaFuncSetAttribute(tile_tma_kernel<3, EpiApply>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
                 CU(cudaFuncSetAttribute(tile_tma_kernel<5, EpiApply>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
                 CU(cudaFuncSetAttribute(tile_tma_kernel<3, EpiApply, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
                 CU(cudaFuncSetAttribute(tile_tma_kernel<5, EpiApply, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-                attr_set = true;
             }
             const bool vg = h->grid.gauge == 1;
             if (vg) {
@@ -919,26 +931,17 @@ int tdse_energy_log(tdse_handle *h, double *energy_host, long max_rows, void *st
 
 static int step_taylor_impl(tdse_handle *h, int order, double t0, double dt, long nsteps, int obs_every, void *stream) {
     RC(ensure_pool(h, 4));
-    // taylor_block: 0 one kernel per order; 1 auto (persistent register patches, else register tiles, else
-    // shared-memory tile, else per order); 2 shared-memory tile kernel only; 3 register-tile kernel (v2) only;
-    // 4 persistent register-patch kernel (v3) only
+    // taylor_block: 0 one kernel per order; 1 all orders in one pass (persistent register-patch kernel) when
+    // the grid allows it (n_l <= 128), else one kernel per order
     h->taylor_blocked_last = 0;
     h->rk4_fused = 0;
-    h->rtp = RtPlan{};
     h->rpp = RpPlan{};
-    // (the all-orders-in-one-pass kernels implement the length-gauge coupling only; imaginary time has no field)
+    // (the all-orders-in-one-pass kernel implements the length-gauge coupling only; imaginary time has no field)
     const bool lg = h->grid.gauge == 0 || h->imag;
-    if (lg && (h->taylor_block == 1 || h->taylor_block == 4)) {
+    if (lg && h->taylor_block == 1) {
         h->rpp = rp_plan(h->grid, order, h->n_sm, h->rp_variant, h->rp_tma, h->imag ? 2 : 0);
         if (h->rpp.ok) h->taylor_blocked_last = 3;
     }
-    if (lg && !h->taylor_blocked_last && !h->imag && (h->taylor_block == 1 || h->taylor_block == 3)) {
-        h->rtp = rt_plan(h->grid, order, h->rt_variant);
-        if (h->rtp.ok) h->taylor_blocked_last = 2;
-    }
-    if (lg && !h->taylor_blocked_last && !h->imag && (h->taylor_block == 1 || h->taylor_block == 2) && blocked_supported(h->bcfg, order))
-        h->taylor_blocked_last = 1;
-    if (h->taylor_blocked_last != 2) h->rtp = RtPlan{};
     return run_fixed(h, KIND_TAYLOR, order, 0, t0, dt, nsteps, obs_every, (cudaStream_t)stream);
 }
 
@@ -1066,7 +1069,10 @@ int tdse_step_rk45(tdse_handle *h, double t0, double t_end, double dt_init, doub
         CU(cudaMemcpyAsync(&hc, h->d_ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, s));
         CU(cudaStreamSynchronize(s));
         if (hc.done) break;
-        if (!(hc.h > 0.0) || hc.n_attempt > (1LL << 40)) return TDSE_ERR_NONFINITE;
+        if (!(hc.h > 0.0) || hc.n_attempt > (1LL << 40)) {
+            h->psi_slot = h->role_slot[hc.perm[R_PSI]];       // the state follows the device's role swaps even on failure
+            return TDSE_ERR_NONFINITE;
+        }
         RC(run_blocks(h, KIND_RK45, 0, 0, G, 0, 1, s));
     }
     // the device swapped roles on every accept: make the host's view of "the state" follow
@@ -1130,6 +1136,23 @@ int tdse_lanczos_info(tdse_handle *h, double *alpha, double *beta, double *coef,
 }
 
 long tdse_launch_count(tdse_handle *h) { return h ? h->launches : 0; }
+long tdse_graph_instantiations(tdse_handle *h) { return h ? h->graph_inst : 0; }
+
+int tdse_ionisation_yield(tdse_handle *h, double *out_host, void *stream) {
+    if (!h || !out_host) return TDSE_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (!h->d_yield) CU(cudaMalloc(&h->d_yield, sizeof(double) * h->grid.batch));
+    h->pending = 0;
+    RC(enqueue_obs(h, h->pool[h->psi_slot], 0, 0, 1, 0.0, h->d_row_direct, s));
+    yield_kernel<<<h->grid.batch, 32, 0, s>>>(h->d_row_direct, h->n_states, h->d_yield);
+    count(h);
+    CU(cudaGetLastError());
+    h->launches += h->pending;
+    CU(cudaMemcpyAsync(out_host, h->d_yield, sizeof(double) * h->grid.batch, cudaMemcpyDeviceToHost, s));
+    CU(cudaStreamSynchronize(s));
+    return TDSE_OK;
+}
+
 int tdse_set_absorber(tdse_handle *h, double r_b, int p) {
     if (!h || (r_b > 0.0 && p < 1)) return TDSE_ERR_ARG;
     CU(cudaDeviceSynchronize());

@@ -618,17 +618,15 @@ __global__ void rk45_begin_kernel(Ctl *c, const tdse_pulse *pulse, int B, const 
 // ------------------------------------------------------------------------------------------------------
 constexpr int kObsRows = 8;
 
-// ONE launch per logged row: CTAs (chunk_r, b, z < chunks_l) reduce norm / dipole / acceleration sums of a chunk,
-// CTAs (chunk_r, b, chunks_l + s) the overlap of 256 radial points with bound state s (Eq. 25); the last CTA of
-// a member to finish (ticket counter) adds the partials in a fixed order and assembles the row
-// {norm, <z>, <z''>, pop...} (Eq. 34, Eq. 36).  The first version used three launches (sums, overlaps,
-// assembly): 6 us of launch latency per step on CFG1.
-// partials[b][chunks_r*chunks_l][3], amp_part[b][n_states][chunks_r] (re, im), counters[b] (zero between launches).
+// ONE launch per logged row for the sums: CTAs (chunk_r, b, z) reduce the norm / dipole / acceleration sums of a chunk;
+// the last CTA of a member to finish (ticket counter) adds the partials in a fixed order and writes
+// {norm, <z>, <z''>} of the row (Eq. 34, Eq. 36).  The bound-state populations of the row are written by
+// pop_kernel below.  partials[b][chunks_r*chunks_l][3], counters[b] (zero between launches).
 // t_direct: if use_direct, the time for -E(t); else t_{n+1} = t0 + (n+1) dt of the step being logged.
-__global__ void __launch_bounds__(256) obs_kernel(GridDev g, const double2 *psi, const double *phi, const int *l_of_state,
-                                                  int n_states, const tdse_pulse *pulse, const Ctl *ctl, int step_off,
-                                                  int predicated, int use_direct, double t_direct, double *partials,
-                                                  double2 *amp_part, unsigned int *counters, double *rows, int rows_per) {
+__global__ void __launch_bounds__(256) obs_kernel(GridDev g, const double2 *psi, int n_states, const tdse_pulse *pulse,
+                                                  const Ctl *ctl, int step_off, int predicated, int use_direct,
+                                                  double t_direct, double *partials, unsigned int *counters,
+                                                  double *rows, int rows_per) {
     __shared__ double red_s[3 * 8];
     __shared__ int last_flag;
     long long row = 0;
@@ -639,10 +637,10 @@ __global__ void __launch_bounds__(256) obs_kernel(GridDev g, const double2 *psi,
         row = n / ctl->obs_every - 1;
         t = time_at(ctl->t0, (double)n, ctl->dt);
     }
-    const int chunks_r = gridDim.x, chunks_l = gridDim.z - n_states;     // chunks_l = l segments of rows_per rows
+    const int chunks_r = gridDim.x, chunks_l = gridDim.z;     // chunks_l = l segments of rows_per rows
     const int b = blockIdx.y, j = blockIdx.x * 256 + threadIdx.x;
     double red[3] = {0.0, 0.0, 0.0};
-    if ((int)blockIdx.z < chunks_l) {
+    {
         const int l_lo = blockIdx.z * rows_per, l_hi = min(g.n_l, l_lo + rows_per);
         if (j < g.n_r) {
             double nn = 0.0, sz = 0.0;
@@ -667,17 +665,8 @@ __global__ void __launch_bounds__(256) obs_kernel(GridDev g, const double2 *psi,
             double *o = partials + (((size_t)b * chunks_r + blockIdx.x) * chunks_l + blockIdx.z) * 3;
             o[0] = red[0]; o[1] = red[1]; o[2] = red[2];
         }
-    } else {
-        const int s = blockIdx.z - chunks_l;
-        if (j < g.n_r) {
-            const double w = __ldg(phi + (size_t)s * g.n_r + j);
-            const double2 v = psi[((size_t)b * g.n_l + l_of_state[s]) * g.n_r + j];
-            red[0] = w * v.x; red[1] = w * v.y;
-        }
-        block_reduce<256, 3>(red, red_s);
-        if (threadIdx.x == 0) amp_part[((size_t)b * n_states + s) * chunks_r + blockIdx.x] = make_double2(red[0], red[1]);
     }
-    // ---- last CTA of this member assembles the row -------------------------------------------------------------
+    // ---- last CTA of this member assembles the sums of the row ---------------------------------------------------
     if (threadIdx.x == 0) {
         __threadfence();
         const unsigned int ticket = atomicAdd(counters + b, 1u);
@@ -700,15 +689,61 @@ __global__ void __launch_bounds__(256) obs_kernel(GridDev g, const double2 *psi,
         o[2] = -pulse_E(pulse[b], t) - 2.0 * g.z * g.dr * sum[2];
         counters[b] = 0u;
     }
-    for (int s = threadIdx.x; s < n_states; s += 256) {
-        double ax = 0.0, ay = 0.0;
-        for (int c = 0; c < chunks_r; ++c) {
-            const double2 a = __ldcg(amp_part + ((size_t)b * n_states + s) * chunks_r + c);
-            ax += a.x; ay += a.y;
-        }
-        const double ar = g.dr * ax, ai = g.dr * ay;
-        o[3 + s] = ar * ar + ai * ai;
+}
+
+// Bound-state populations of a row (Eq. 25 with the modulus squared, R-G12): p_s = |dr sum_j phi_s[j] f_{l_s,j}|^2.
+// grid = (n_l, batch): the CTA of (l, b) walks the states with l_s = l (state_list[l_off[l] .. l_off[l+1])), four at a
+// time, so that the row f_l of a member is read from L1/L2 once per four states and a whole overlap is reduced inside one
+// CTA in a fixed order -- the ~170 bound states of the CFG5 yield (R-G23) cost one launch.
+__global__ void __launch_bounds__(256) pop_kernel(GridDev g, const double2 *psi, const double *phi, const int *l_off,
+                                                  const int *state_list, int n_states, const Ctl *ctl, int step_off,
+                                                  int predicated, int use_direct, double *rows) {
+    __shared__ double red_s[8 * 8];
+    long long row = 0;
+    if (!use_direct) {
+        const long long n = ctl->step_base + step_off + 1;
+        if (predicated && (ctl->obs_every <= 0 || (n % ctl->obs_every) != 0)) return;
+        row = n / ctl->obs_every - 1;
     }
+    const int l = blockIdx.x, b = blockIdx.y;
+    const int s_lo = l_off[l], s_hi = l_off[l + 1];
+    if (s_lo == s_hi) return;
+    const double2 *f = psi + ((size_t)b * g.n_l + l) * g.n_r;
+    double *o = rows + ((size_t)row * g.batch + b) * (3 + n_states) + 3;
+    for (int s0 = s_lo; s0 < s_hi; s0 += 4) {
+        int sid[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) sid[i] = state_list[min(s0 + i, s_hi - 1)];
+        double a[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+        for (int j = threadIdx.x; j < g.n_r; j += 256) {
+            const double2 v = f[j];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const double w = __ldg(phi + (size_t)sid[i] * g.n_r + j);
+                a[2 * i] = fma(w, v.x, a[2 * i]); a[2 * i + 1] = fma(w, v.y, a[2 * i + 1]);
+            }
+        }
+        block_reduce<256, 8>(a, red_s);
+        if (threadIdx.x == 0) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                if (s0 + i < s_hi) {
+                    const double ar = g.dr * a[2 * i], ai = g.dr * a[2 * i + 1];
+                    o[sid[i]] = ar * ar + ai * ai;
+                }
+            }
+        }
+    }
+}
+
+// Ionisation yield from the bound-state populations of a row (CFG5, R-G23): 1 - sum_s p_s.  grid = batch, block = 32.
+__global__ void __launch_bounds__(32) yield_kernel(const double *rows, int n_states, double *out) {
+    const double *o = rows + (size_t)blockIdx.x * (3 + n_states) + 3;
+    double s = 0.0;
+    for (int i = threadIdx.x; i < n_states; i += 32) s += o[i];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) s += __shfl_down_sync(0xffffffffu, s, off);
+    if (threadIdx.x == 0) out[blockIdx.x] = 1.0 - s;
 }
 
 // The same for small grids: ONE CTA per member loops over all chunks and states, so that no cross-CTA hand-over

@@ -18,19 +18,12 @@
 //     c_l E r_j / c1 of the (l, l+1) pair is formed once and used for both rows.  12.25 (3-point) / 16.25 (5-point)
 //     FP64 instructions per point-update instead of 16.3 / 20.
 #pragma once
-#include <cuda.h>
-
-#include <algorithm>
-#include <map>
-#include <mutex>
-#include <tuple>
-
-#include "tdse_device.cuh"
+#include "tdse_taylor_rp_plan.h"
+#include "tdse_tma.cuh"
 
 namespace tdse {
 
-constexpr int kRpRows = 4;     // patch rows
-__constant__ double kRpInvK[65];   // 1/k, k = 1..64 (filled by rp_init_tables)
+static __constant__ double kRpInvK[65];   // 1/k, k = 1..64 (filled by rp_init_tables)
 
 template <int FD, int CP, int NWR, int NWC>
 struct RpGeom {
@@ -68,50 +61,6 @@ __device__ __forceinline__ void ldg256(const double2 *p, double2 &a, double2 &b)
 }
 __device__ __forceinline__ void stg256(double2 *p, const double2 &a, const double2 &b) {
     asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a.x), "d"(a.y), "d"(b.x), "d"(b.y) : "memory");
-}
-
-// ---- TMA (cp.async.bulk.tensor) + mbarrier helpers ---------------------------------------------------------------
-__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity) {
-    unsigned ok;
-    do {
-        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
-                     : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
-    } while (!ok);
-}
-// 3-D tiled tensor load global -> shared, completion on an mbarrier
-__device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, int c0, int c1, int c2, unsigned long long *bar) {
-    asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
-        ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-
-// ---- thread-block cluster helpers (distributed shared memory) ----------------------------------------------------
-__device__ __forceinline__ unsigned cluster_ctarank() { unsigned r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
-__device__ __forceinline__ unsigned cluster_nctarank() { unsigned r; asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r)); return r; }
-// shared::cluster address of the same shared-memory offset in CTA `rank` of the cluster
-__device__ __forceinline__ unsigned dsmem_addr(const void *p, unsigned rank) {
-    unsigned r;
-    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_u32(p)), "r"(rank));
-    return r;
-}
-__device__ __forceinline__ double2 ld_dsmem2(unsigned addr) {
-    double2 v;
-    asm volatile("ld.shared::cluster.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr) : "memory");
-    return v;
-}
-__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
-__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
-__device__ __forceinline__ void mbar_arrive(unsigned long long *bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 
 // tile start of tile t: interior [t*W, (t+1)*W) plus H halo columns per side, clamped so that a tile at a wall
@@ -514,139 +463,26 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
 }
 
 // ------------------------------------------------------------------------------------------------------
-// Host side
+// Host side: launchers of the instantiations of ONE stencil (FD), compiled in tdse_taylor_rp_fd3.cu / _fd5.cu
 // ------------------------------------------------------------------------------------------------------
-struct RpVariant { int cp, nwr, nwc, minb; };
-// instantiations: (patch columns, row-group warps, column-segment warps, min CTAs/SM)
-constexpr RpVariant kRpVariants[] = {
-    {4, 1, 1, 8}, {4, 2, 1, 4}, {4, 4, 1, 2}, {4, 8, 1, 1},      // 128-column tiles, 16 points per thread
-    {2, 1, 2, 8}, {2, 2, 2, 4}, {2, 4, 2, 2}, {2, 8, 2, 1},      // 128-column tiles,  8 points per thread
-    {2, 4, 4, 1},                                                // 256-column tile, 8 points per thread, n_l <= 16
-    {4, 4, 2, 1},                                                // 256-column tile, 16 points per thread, n_l <= 16
-};
-constexpr int kNumRpVariants = sizeof(kRpVariants) / sizeof(kRpVariants[0]);
-// the instantiations that also exist as cluster kernels (16 rows per CTA)
-constexpr bool rp_clusterable(int variant) { return variant == 2 || variant == 9; }
-
+// (one copy of the constant table per translation unit, hence per FD)
+template <int FD>
 inline int rp_init_tables() {
+    static DeviceOnce once;
+    if (!once.first()) return TDSE_OK;
     double h[65];
     h[0] = 0.0;
     for (int k = 1; k <= 64; ++k) h[k] = 1.0 / (double)k;
     return cudaMemcpyToSymbol(kRpInvK, h, sizeof(h)) == cudaSuccess ? TDSE_OK : TDSE_ERR_CUDA;
 }
 
-// cuTensorMapEncodeTiled through the runtime (no link against libcuda)
-typedef CUresult (*RpEncodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
-                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-inline RpEncodeTiled rp_encode_fn() {
-    static RpEncodeTiled fn = nullptr;
-    static bool tried = false;
-    if (!tried) {
-        tried = true;
-        void *p = nullptr;
-        cudaDriverEntryPointQueryResult qres;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess && p &&
-            qres == cudaDriverEntryPointSuccess)
-            fn = (RpEncodeTiled)p;
-        cudaGetLastError();
-    }
-    return fn;
-}
-
-struct RpPlan { int ok, variant, tma, cl, rk, W, H, WT, n_tiles, n_items, grid, threads; };   // rk = kernel MODE (0, 1, 2)   // cl: CTAs per cluster (1: none)
-
-// use_tma: -1 heuristic, 0 never, 1 whenever the layout allows it (n_r % 8 == 0, a full tile, 4-column patches)
-// rk: plan the fused RK4 step (order = 4 sweeps; only the one-warp-wide 16-point instantiations, full tiles)
-constexpr bool rp_rk_capable(int variant) { return variant >= 0 && variant <= 3; }
-inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant, int use_tma, int rk = 0) {
-    RpPlan best{};
-    const int hw = (g.fd_order == 3) ? 1 : 2;
-    double best_cost = 0.0;
-    for (int i = 0; i < kNumRpVariants; ++i) {
-        if (force_variant >= 0 && i != force_variant) continue;
-        const RpVariant &v = kRpVariants[i];
-        const int WT = 32 * v.cp * v.nwc;
-        if (rk && (!rp_rk_capable(i) || g.n_r < WT)) continue;
-        int rows = kRpRows * v.nwr, cl = 1;
-        if (rows < g.n_l) {
-            // more rows than one CTA holds: split them over a cluster of 2, 4 or 8 CTAs (16-row CTAs only)
-            if (!rp_clusterable(i)) continue;
-            while (cl < 8 && rows * cl < g.n_l) cl *= 2;
-            if (rows * cl < g.n_l) continue;
-            rows *= cl;
-        }
-        if (v.cp < hw) continue;
-        if (rows >= 2 * g.n_l && v.nwr > 1) continue;      // more than half of the rows would be padding
-        for (int tma = 0; tma <= 1; ++tma) {
-            if (tma && (use_tma == 0 || v.cp != 4 || (g.n_r & 7) || g.n_r <= WT || !rp_encode_fn())) continue;
-            if (!tma && use_tma == 1 && v.cp == 4 && !(g.n_r & 7) && g.n_r > WT && rp_encode_fn()) continue;
-            int H = order * hw;
-            if (tma) H = (H + 7) & ~7;                      // tile starts on a 128-byte column group
-            else if ((g.n_r & 1) == 0) H = (H + 1) & ~1;    // even halo: every patch row starts 32-byte aligned
-            RpPlan p{};
-            p.variant = i; p.tma = tma; p.cl = cl; p.rk = rk; p.H = H; p.WT = WT; p.threads = 32 * v.nwr * v.nwc;
-            if (g.n_r <= WT) { p.W = g.n_r; p.n_tiles = 1; }
-            else {
-                p.W = WT - 2 * H;
-                if (p.W < WT / 4) continue;
-                p.n_tiles = (g.n_r + p.W - 1) / p.W;
-            }
-            p.n_items = p.n_tiles * g.batch;
-            p.grid = std::min(p.n_items, n_sm * v.minb / cl);       // clusters (= CTAs when cl == 1)
-            // a grid that is a multiple of n_tiles keeps every CTA on one radial tile (coefficients loaded once)
-            if (p.n_tiles * 4 <= p.grid) p.grid = p.grid / p.n_tiles * p.n_tiles;
-            p.grid *= cl;
-            p.ok = 1;
-            // cost ~ time: the points one CTA computes per item times the items an SM has to work through (at least
-            // one: a small grid is bound by the serial work of a CTA, so more and smaller CTAs win).  Measured
-            // penalties: 8-point patches 1.5x per column (twice the exchange per point, spills at 128 registers);
-            // tiles wider than one warp 1.4x (edge columns through shared memory, no work before the barrier);
-            // cluster barriers 1.25x; the asynchronous tile fetch hides the load latency of the next item.
-            const double n_ctas = (double)p.n_items * cl;
-            double cost = (double)(rows / cl) * WT * std::max(1.0, n_ctas / n_sm);
-            if (force_variant < 0 && v.cp == 2) cost *= 1.5;
-            if (force_variant < 0 && v.nwc > 1) cost *= 1.4;
-            if (cl > 1) cost *= 1.25;
-            if (tma) cost *= 0.85;
-            if (!best.ok || cost < best_cost) { best = p; best_cost = cost; }
-        }
-    }
-    return best;
-}
-
-// tensor map of a state array seen as [batch*n_l rows][n_r/8 groups][16 doubles], box = rows x WT/8 x 16, cached
-inline const CUtensorMap *rp_tensor_map(const void *base, int n_r, int total_rows, int box_rows, int WT) {
-    static std::map<std::tuple<const void *, int, int, int, int>, CUtensorMap> cache;
-    static std::mutex mu;
-    std::lock_guard<std::mutex> lock(mu);
-    const auto key = std::make_tuple(base, n_r, total_rows, box_rows, WT);
-    auto it = cache.find(key);
-    if (it != cache.end()) return &it->second;
-    const RpEncodeTiled encode = rp_encode_fn();
-    if (!encode) return nullptr;
-    CUtensorMap m;
-    const cuuint64_t dims[3] = {16, (cuuint64_t)(n_r / 8), (cuuint64_t)total_rows};
-    const cuuint64_t strides[2] = {128, (cuuint64_t)n_r * 16};          // bytes, dims 1 and 2
-    const cuuint32_t box[3] = {16, (cuuint32_t)(WT / 8), (cuuint32_t)box_rows};
-    const cuuint32_t estr[3] = {1, 1, 1};
-    if (encode(&m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void *>(base), dims, strides, box, estr,
-               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-        return nullptr;
-    if (cache.size() > 64) cache.clear();
-    return &(cache[key] = m);
-}
-
 template <class K>
-inline int rp_launch_kernel(K kern, bool *attr_set, int smem, const RpPlan &p, cudaStream_t s, const GridDev &g,
+inline int rp_launch_kernel(K kern, DeviceOnce *once, int smem, const RpPlan &p, cudaStream_t s, const GridDev &g,
                             const double2 *in, double2 *out, const double *ef, const double *dtp, int order,
                             const CUtensorMap &tm) {
-    if (!*attr_set) {
+    if (once->first()) {
         if (cudaFuncSetAttribute((const void *)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
             return TDSE_ERR_CUDA;
-        *attr_set = true;
     }
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(p.grid); cfg.blockDim = dim3(p.threads); cfg.dynamicSmemBytes = smem; cfg.stream = s;
@@ -658,77 +494,68 @@ inline int rp_launch_kernel(K kern, bool *attr_set, int smem, const RpPlan &p, c
                ? TDSE_OK : TDSE_ERR_CUDA;
 }
 
-// MODE 1 / 2 instantiations exist only for the one-warp-wide 16-point variants (RKABLE) and full tiles
+// MODE 1 / 2 instantiations exist only for the one-warp-wide variants (RKABLE) and full tiles
 template <int FD, int CP, int NWR, int NWC, int MINB, bool CLUSTERABLE, bool RKABLE, int MODE>
 inline int rp_launch_mode(const GridDev &g, const RpPlan &p, bool mask, const CUtensorMap *tm, const double2 *in,
                           double2 *out, const double *ef, const double *dtp, int order, cudaStream_t s) {
     if (!RKABLE || mask) return TDSE_ERR_UNSUPPORTED;
     constexpr int kM = RKABLE ? MODE : 0;
-    constexpr bool kCl = CLUSTERABLE && RKABLE, kT = (CP == 4) && RKABLE;
-    static bool attr[4] = {false, false, false, false};
+    constexpr bool kCl = CLUSTERABLE && RKABLE, kT = RKABLE;
+    static DeviceOnce once[4];
     const int sm_t = (int)sizeof(RpSmem<FD, CP, NWR, NWC, kT, kM == 1>), sm_n = (int)sizeof(RpSmem<FD, CP, NWR, NWC, false, kM == 1>);
     if (p.cl > 1) {
         if (!kCl) return TDSE_ERR_UNSUPPORTED;
-        if (p.tma) return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, kT, kCl, kM>, &attr[3], sm_t, p, s, g, in, out, ef, dtp, order, *tm);
-        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, kCl, kM>, &attr[2], sm_n, p, s, g, in, out, ef, dtp, order, *tm);
+        if (p.tma) return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, kT, kCl, kM>, &once[3], sm_t, p, s, g, in, out, ef, dtp, order, *tm);
+        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, kCl, kM>, &once[2], sm_n, p, s, g, in, out, ef, dtp, order, *tm);
     }
-    if (p.tma) return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, kT, false, kM>, &attr[1], sm_t, p, s, g, in, out, ef, dtp, order, *tm);
-    return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, false, kM>, &attr[0], sm_n, p, s, g, in, out, ef, dtp, order, *tm);
+    if (p.tma) return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, kT, false, kM>, &once[1], sm_t, p, s, g, in, out, ef, dtp, order, *tm);
+    return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, false, kM>, &once[0], sm_n, p, s, g, in, out, ef, dtp, order, *tm);
 }
 
 template <int FD, int CP, int NWR, int NWC, int MINB, bool CLUSTERABLE, bool RKABLE>
 inline int rp_launch_one(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
                          const double *dtp, int order, cudaStream_t s) {
-    if (FD == 5 && CP < 2) return TDSE_ERR_UNSUPPORTED;
     const bool mask = g.n_r < 32 * CP * NWC;
-    constexpr bool kTma = (CP == 4);
-    static bool attr_set[5] = {false, false, false, false, false};
-    CUtensorMap dummy{};
-    const CUtensorMap *tm = &dummy;
+    static DeviceOnce once[5];
+    CUtensorMap tmap{};
     if (p.tma) {
-        if (!kTma || mask) return TDSE_ERR_UNSUPPORTED;
-        tm = rp_tensor_map(in, g.n_r, g.batch * g.n_l, kRpRows * NWR, 32 * CP * NWC);
-        if (!tm) return TDSE_ERR_CUDA;
+        if (mask) return TDSE_ERR_UNSUPPORTED;
+        if (!tma_map_rows3d(&tmap, in, g.n_r, g.batch * g.n_l, kRpRows * NWR, 32 * CP * NWC)) return TDSE_ERR_CUDA;
     }
+    const CUtensorMap *tm = &tmap;
     if (p.rk == 1) return rp_launch_mode<FD, CP, NWR, NWC, MINB, CLUSTERABLE, RKABLE, 1>(g, p, mask, tm, in, out, ef, dtp, order, s);
     if (p.rk == 2) return rp_launch_mode<FD, CP, NWR, NWC, MINB, CLUSTERABLE, RKABLE, 2>(g, p, mask, tm, in, out, ef, dtp, order, s);
     if (p.cl > 1) {
         if (!CLUSTERABLE || mask) return TDSE_ERR_UNSUPPORTED;
         constexpr bool kCl = CLUSTERABLE;
         if (p.tma)
-            return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, kTma, kCl>, &attr_set[3],
-                                    (int)sizeof(RpSmem<FD, CP, NWR, NWC, kTma>), p, s, g, in, out, ef, dtp, order, *tm);
-        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, kCl>, &attr_set[4],
+            return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, true, kCl>, &once[3],
+                                    (int)sizeof(RpSmem<FD, CP, NWR, NWC, true>), p, s, g, in, out, ef, dtp, order, *tm);
+        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, kCl>, &once[4],
                                 (int)sizeof(RpSmem<FD, CP, NWR, NWC, false>), p, s, g, in, out, ef, dtp, order, *tm);
     }
     if (p.tma)
-        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, kTma, false>, &attr_set[2],
-                                (int)sizeof(RpSmem<FD, CP, NWR, NWC, kTma>), p, s, g, in, out, ef, dtp, order, *tm);
+        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, true, false>, &once[2],
+                                (int)sizeof(RpSmem<FD, CP, NWR, NWC, true>), p, s, g, in, out, ef, dtp, order, *tm);
     if (mask)
-        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, true, MINB, false, false>, &attr_set[1],
+        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, true, MINB, false, false>, &once[1],
                                 (int)sizeof(RpSmem<FD, CP, NWR, NWC, false>), p, s, g, in, out, ef, dtp, order, *tm);
-    return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, false>, &attr_set[0],
+    return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, false>, &once[0],
                             (int)sizeof(RpSmem<FD, CP, NWR, NWC, false>), p, s, g, in, out, ef, dtp, order, *tm);
 }
 
-inline int launch_taylor_rp(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
-                            const double *dtp, int order, cudaStream_t s) {
+template <int FD>
+inline int launch_taylor_rp_fd(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
+                               const double *dtp, int order, cudaStream_t s) {
     if (!p.ok) return TDSE_ERR_UNSUPPORTED;
-#define TDSE_RP_CASE(I, CP, NWR, NWC, MINB)                                                                  \
-    case I:                                                                                                  \
-        return (g.fd == 3) ? rp_launch_one<3, CP, NWR, NWC, MINB, rp_clusterable(I), rp_rk_capable(I)>(g, p, in, out, ef, dtp, order, s)  \
-                           : rp_launch_one<5, CP, NWR, NWC, MINB, rp_clusterable(I), rp_rk_capable(I)>(g, p, in, out, ef, dtp, order, s);
+#define TDSE_RP_CASE(I, CP, NWR, NWC, MINB) \
+    case I: return rp_launch_one<FD, CP, NWR, NWC, MINB, rp_clusterable(I), rp_rk_capable(I)>(g, p, in, out, ef, dtp, order, s);
     switch (p.variant) {
         TDSE_RP_CASE(0, 4, 1, 1, 8)
         TDSE_RP_CASE(1, 4, 2, 1, 4)
         TDSE_RP_CASE(2, 4, 4, 1, 2)
         TDSE_RP_CASE(3, 4, 8, 1, 1)
-        TDSE_RP_CASE(4, 2, 1, 2, 8)
-        TDSE_RP_CASE(5, 2, 2, 2, 4)
-        TDSE_RP_CASE(6, 2, 4, 2, 2)
-        TDSE_RP_CASE(7, 2, 8, 2, 1)
-        TDSE_RP_CASE(8, 2, 4, 4, 1)
-        TDSE_RP_CASE(9, 4, 4, 2, 1)
+        TDSE_RP_CASE(4, 4, 4, 2, 1)
     }
 #undef TDSE_RP_CASE
     return TDSE_ERR_UNSUPPORTED;

@@ -1,0 +1,11 @@
+// tdse_taylor_rp_fd3.cu -- the 3-point instantiations of the persistent register-patch kernel (own translation unit
+// so that the library builds in parallel).
+#include "tdse_taylor_rp.cuh"
+
+namespace tdse {
+int rp_init_fd3() { return rp_init_tables<3>(); }
+int launch_taylor_rp_fd3(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
+                         const double *dtp, int order, cudaStream_t s) {
+    return launch_taylor_rp_fd<3>(g, p, in, out, ef, dtp, order, s);
+}
+}  // namespace tdse

@@ -1,0 +1,102 @@
+// tdse_taylor_rp_plan.h -- host-side plan of the persistent register-patch kernel (tdse_taylor_rp.cuh): which
+// instantiation, tile geometry and grid a (grid, order) pair runs with.  Plain C++ (no device code) so that the API
+// translation unit does not have to compile the kernels.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <algorithm>
+
+#include "tdse_device.cuh"
+
+namespace tdse {
+
+constexpr int kRpRows = 4;     // patch rows
+
+struct RpVariant { int cp, nwr, nwc, minb; };
+// instantiations: (patch columns, row-group warps, column-segment warps, min CTAs/SM); 16 points per thread
+constexpr RpVariant kRpVariants[] = {
+    {4, 1, 1, 8}, {4, 2, 1, 4}, {4, 4, 1, 2}, {4, 8, 1, 1},      // 128-column tiles, 4 / 8 / 16 / 32 rows
+    {4, 4, 2, 1},                                                // 256-column tile (edge exchange between warps), 16 rows
+};
+constexpr int kNumRpVariants = sizeof(kRpVariants) / sizeof(kRpVariants[0]);
+// the instantiations that also exist as cluster kernels (16 rows per CTA)
+constexpr bool rp_clusterable(int variant) { return variant == 2 || variant == 4; }
+// ... and as fused-RK4 / imaginary-time kernels (one-warp-wide tiles)
+constexpr bool rp_rk_capable(int variant) { return variant >= 0 && variant <= 3; }
+
+// rk = kernel MODE (0 Taylor, 1 classic RK4, 2 imaginary time); cl: CTAs per cluster (1: none)
+struct RpPlan { int ok, variant, tma, cl, rk, W, H, WT, n_tiles, n_items, grid, threads; };
+
+bool tma_available();       // cuTensorMapEncodeTiled could be resolved (tdse_api.cu)
+
+// use_tma: -1 heuristic, 0 never, 1 whenever the layout allows it (n_r % 8 == 0 and more than one tile)
+// rk: plan the fused RK4 / imaginary-time step (only the one-warp-wide instantiations, full tiles)
+inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant, int use_tma, int rk = 0) {
+    RpPlan best{};
+    const int hw = (g.fd_order == 3) ? 1 : 2;
+    double best_cost = 0.0;
+    for (int i = 0; i < kNumRpVariants; ++i) {
+        if (force_variant >= 0 && i != force_variant) continue;
+        const RpVariant &v = kRpVariants[i];
+        const int WT = 32 * v.cp * v.nwc;
+        if (rk && (!rp_rk_capable(i) || g.n_r < WT)) continue;
+        int rows = kRpRows * v.nwr, cl = 1;
+        if (rows < g.n_l) {
+            // more rows than one CTA holds: split them over a cluster of 2, 4 or 8 CTAs (16-row CTAs only)
+            if (!rp_clusterable(i)) continue;
+            while (cl < 8 && rows * cl < g.n_l) cl *= 2;
+            if (rows * cl < g.n_l) continue;
+            rows *= cl;
+        }
+        if (rows >= 2 * g.n_l && v.nwr > 1) continue;      // more than half of the rows would be padding
+        for (int tma = 0; tma <= 1; ++tma) {
+            const bool tma_ok = !(g.n_r & 7) && g.n_r > WT && tma_available();
+            if (tma && (use_tma == 0 || !tma_ok)) continue;
+            if (!tma && use_tma == 1 && tma_ok) continue;
+            int H = order * hw;
+            if (tma) H = (H + 7) & ~7;                      // tile starts on a 128-byte column group
+            else if ((g.n_r & 1) == 0) H = (H + 1) & ~1;    // even halo: every patch row starts 32-byte aligned
+            RpPlan p{};
+            p.variant = i; p.tma = tma; p.cl = cl; p.rk = rk; p.H = H; p.WT = WT; p.threads = 32 * v.nwr * v.nwc;
+            if (g.n_r <= WT) { p.W = g.n_r; p.n_tiles = 1; }
+            else {
+                p.W = WT - 2 * H;
+                if (p.W < WT / 4) continue;
+                p.n_tiles = (g.n_r + p.W - 1) / p.W;
+            }
+            p.n_items = p.n_tiles * g.batch;
+            p.grid = std::min(p.n_items, n_sm * v.minb / cl);       // clusters (= CTAs when cl == 1)
+            // a grid that is a multiple of n_tiles keeps every CTA on one radial tile (coefficients loaded once)
+            if (p.n_tiles * 4 <= p.grid) p.grid = p.grid / p.n_tiles * p.n_tiles;
+            p.grid *= cl;
+            p.ok = 1;
+            // cost ~ time: the points one CTA computes per item times the items an SM has to work through (at least
+            // one: a small grid is bound by the serial work of a CTA, so more and smaller CTAs win).  Measured
+            // penalties: tiles wider than one warp 1.4x (edge columns through shared memory, no work before the
+            // barrier); cluster barriers 1.25x; the asynchronous tile fetch hides the load latency of the next item.
+            const double n_ctas = (double)p.n_items * cl;
+            double cost = (double)(rows / cl) * WT * std::max(1.0, n_ctas / n_sm);
+            if (force_variant < 0 && v.nwc > 1) cost *= 1.4;
+            if (cl > 1) cost *= 1.25;
+            if (tma) cost *= 0.85;
+            if (!best.ok || cost < best_cost) { best = p; best_cost = cost; }
+        }
+    }
+    return best;
+}
+
+// defined in tdse_taylor_rp_fd3.cu / tdse_taylor_rp_fd5.cu
+int rp_init_fd3();          // uploads the 1/k table of that translation unit to the current device (tdse_create)
+int rp_init_fd5();
+int launch_taylor_rp_fd3(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
+                         const double *dtp, int order, cudaStream_t s);
+int launch_taylor_rp_fd5(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
+                         const double *dtp, int order, cudaStream_t s);
+
+inline int launch_taylor_rp(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
+                            const double *dtp, int order, cudaStream_t s) {
+    return g.fd == 3 ? launch_taylor_rp_fd3(g, p, in, out, ef, dtp, order, s)
+                     : launch_taylor_rp_fd5(g, p, in, out, ef, dtp, order, s);
+}
+
+}  // namespace tdse

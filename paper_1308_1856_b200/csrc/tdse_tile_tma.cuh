@@ -10,7 +10,7 @@
 // The compute phase and the epilogue interface are those of tile_kernel.
 #pragma once
 #include "tdse_kernels.cuh"
-#include "tdse_taylor_rp.cuh"      // mbarrier / TMA helpers, cuTensorMapEncodeTiled entry point
+#include "tdse_tma.cuh"            // mbarrier / TMA helpers, tensor maps
 
 namespace tdse {
 
@@ -19,13 +19,6 @@ namespace tdse {
 constexpr int kTtTW = 128, kTtTL = 8, kTtHalo = 8, kTtCols = kTtTW + 2 * kTtHalo, kTtRows = kTtTL + 2, kTtStages = 2;
 constexpr int kTtMinB = 3;
 constexpr unsigned kTtStageBytes = (unsigned)(kTtRows * kTtCols * sizeof(double2));
-
-__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, int c0, int c1, int c2, int c3,
-                                            unsigned long long *bar) {
-    asm volatile(
-        "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
-        ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
-}
 
 // grid = persistent CTAs, block = 256, dynamic shared = kTtStages * kTtStageBytes + 64.
 // items = batch x l-tiles x r-tiles (r fastest).  Epi must have NRED == 0 and a plain input.
@@ -98,27 +91,9 @@ tile_tma_kernel(GridDev g, Epi epi_in, const __grid_constant__ CUtensorMap tmap,
     }
 }
 
-// 4-D tensor map of a state array: [batch][n_l][n_r/8][16 doubles], box = 1 x kTtRows x kTtCols/8 x 16, no swizzle
-inline const CUtensorMap *tile_tensor_map(const void *base, int n_r, int n_l, int batch) {
-    static std::map<std::tuple<const void *, int, int, int>, CUtensorMap> cache;
-    static std::mutex mu;
-    std::lock_guard<std::mutex> lock(mu);
-    const auto key = std::make_tuple(base, n_r, n_l, batch);
-    auto it = cache.find(key);
-    if (it != cache.end()) return &it->second;
-    const RpEncodeTiled encode = rp_encode_fn();
-    if (!encode) return nullptr;
-    CUtensorMap m;
-    const cuuint64_t dims[4] = {16, (cuuint64_t)(n_r / 8), (cuuint64_t)n_l, (cuuint64_t)batch};
-    const cuuint64_t strides[3] = {128, (cuuint64_t)n_r * 16, (cuuint64_t)n_r * 16 * (cuuint64_t)n_l};
-    const cuuint32_t box[4] = {16, (cuuint32_t)(kTtCols / 8), (cuuint32_t)kTtRows, 1};
-    const cuuint32_t estr[4] = {1, 1, 1, 1};
-    if (encode(&m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<void *>(base), dims, strides, box, estr,
-               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-        return nullptr;
-    if (cache.size() > 64) cache.clear();
-    return &(cache[key] = m);
+// 4-D tensor map of a state array for these kernels (by value; tdse_tma.cuh)
+inline bool tile_tensor_map(CUtensorMap *m, const void *base, int n_r, int n_l, int batch) {
+    return tma_map_member4d(m, base, n_r, n_l, batch, kTtRows, kTtCols);
 }
 
 }  // namespace tdse
