@@ -16,7 +16,8 @@ _lib = None
 
 class Grid(C.Structure):
     _fields_ = [("n_r", C.c_int), ("dr", C.c_double), ("n_l", C.c_int), ("fd_order", C.c_int),
-                ("z_nuc", C.c_double), ("batch", C.c_int), ("r_offset", C.c_double), ("gauge", C.c_int)]
+                ("z_nuc", C.c_double), ("batch", C.c_int), ("r_offset", C.c_double), ("gauge", C.c_int),
+                ("cutoff_lambda", C.c_double)]
 
 
 class Pulse(C.Structure):
@@ -44,8 +45,10 @@ def _dp(a):
     return a.ctypes.data_as(C.POINTER(C.c_double))
 
 
-def make_grid(n_r, dr, n_l, fd_order, z_nuc=1.0, batch=1, r_offset=0.0, gauge=0):
-    return Grid(int(n_r), float(dr), int(n_l), int(fd_order), float(z_nuc), int(batch), float(r_offset), int(gauge))
+def make_grid(n_r, dr, n_l, fd_order, z_nuc=1.0, batch=1, r_offset=0.0, gauge=0, cutoff_lambda=0.0):
+    """cutoff_lambda > 0: centrifugal inner cut-off (an extension beyond the paper, see tdse_oracle.h)."""
+    return Grid(int(n_r), float(dr), int(n_l), int(fd_order), float(z_nuc), int(batch), float(r_offset), int(gauge),
+                float(cutoff_lambda))
 
 
 def _pulses(g, pulses):
@@ -112,6 +115,24 @@ def apply_H(g, psi, e_field):
     rc = lib().oracle_apply_H(C.byref(g), _dp(psi.view(np.float64)), _dp(e), _dp(out.view(np.float64)))
     assert rc == 0, rc
     return out
+
+
+def held_mask(g):
+    """[n_l][n_r] bool: the points the centrifugal cut-off holds at zero."""
+    m = np.zeros((g.n_l, g.n_r), dtype=bool)
+    for l in range(g.n_l):
+        for j in range(1, g.n_r + 1):
+            if not lib().oracle_is_held(C.byref(g), l, j):
+                break                      # held points of a row are its first ones
+            m[l, j - 1] = True
+    return m
+
+
+def project(g, psi):
+    psi = _state(g, psi)
+    rc = lib().oracle_project(C.byref(g), _dp(psi.view(np.float64)))
+    assert rc == 0, rc
+    return psi
 
 
 def dense_H(g, e_field):

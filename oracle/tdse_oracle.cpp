@@ -39,7 +39,26 @@ inline double coupling(int l) { return (l + 1) / std::sqrt((2.0 * l + 1.0) * (2.
 // V_l(r) = l(l+1)/(2 r^2) - Z/r  (Eq. 7)
 inline double v_eff(int l, double r, double z) { return l * (l + 1.0) / (2.0 * r * r) - z / r; }
 
-// one member: out = H(E) f.  f, out: [L][N_r] complex
+// centrifugal inner cut-off (extension beyond the paper): point (l, j) is held at zero iff
+// l(l+1)/(2 r_j^2) > Lambda, decided as l(l+1) > (2 Lambda) r_j^2 in this operation order
+inline bool held(const oracle_grid *g, int l, int j) {
+    if (!(g->cutoff_lambda > 0.0)) return false;
+    const double r = r_of(g, j);
+    return (double)(l * (l + 1)) > (2.0 * g->cutoff_lambda) * (r * r);
+}
+
+void project_member(const oracle_grid *g, double *f) {
+    for (int l = 0; l < g->n_l; ++l)
+        for (int j = 1; j <= g->n_r; ++j)
+            if (held(g, l, j)) { f[2L * l * g->n_r + 2 * (j - 1)] = 0.0; f[2L * l * g->n_r + 2 * (j - 1) + 1] = 0.0; }
+}
+void project_all(const oracle_grid *g, double *psi) {
+    if (!(g->cutoff_lambda > 0.0)) return;
+    for (int b = 0; b < g->batch; ++b) project_member(g, psi + 2 * n_points(g) * b);
+}
+
+// one member: out = H(E) f.  f, out: [L][N_r] complex.  With a cut-off: out = P H P f (held points read as zero and
+// come out as zero: the principal sub-matrix of H on the points that are not held).
 void apply_H_member(const oracle_grid *g, const double *f, double e, double *out) {
     const int N = g->n_r, L = g->n_l;
     const double dr = g->dr, z = g->z_nuc;
@@ -53,8 +72,8 @@ void apply_H_member(const oracle_grid *g, const double *f, double e, double *out
         for (int j = 1; j <= N; ++j) {
             const double r = r_of(g, j);
             for (int c = 0; c < 2; ++c) {  // real and imaginary part: H is real
-                auto F = [&](int jj) -> double {  // zero outside the box
-                    return (jj >= 1 && jj <= N) ? fl[2 * (jj - 1) + c] : 0.0;
+                auto F = [&](int jj) -> double {  // zero outside the box and at held points
+                    return (jj >= 1 && jj <= N && !held(g, l, jj)) ? fl[2 * (jj - 1) + c] : 0.0;
                 };
                 double d2;
                 if (g->fd_order == 3)
@@ -64,8 +83,8 @@ void apply_H_member(const oracle_grid *g, const double *f, double e, double *out
                          (12.0 * dr * dr);
                 const double kin = -0.5 * d2;
                 const double pot = v_eff(l, r, z) * F(j);
-                const double fm = flm ? flm[2 * (j - 1) + c] : 0.0;
-                const double fp = flp ? flp[2 * (j - 1) + c] : 0.0;
+                const double fm = (flm && !held(g, l - 1, j)) ? flm[2 * (j - 1) + c] : 0.0;
+                const double fp = (flp && !held(g, l + 1, j)) ? flp[2 * (j - 1) + c] : 0.0;
                 const double cpl = (g->gauge == 1) ? 0.0 : e * r * (cm * fm + cp * fp);  // P:104 Eq. 11, length gauge
                 out[2L * l * N + 2 * (j - 1) + c] = kin + pot + cpl;
             }
@@ -77,19 +96,20 @@ void apply_H_member(const oracle_grid *g, const double *f, double e, double *out
                 // d/dr by the central formula of the stencil (Eq. 14, reading R-V1), zero outside the box
                 double s[2];
                 for (int c = 0; c < 2; ++c) {
-                    auto G = [&](const double *row, int jj) -> double {
-                        return (row && jj >= 1 && jj <= N) ? row[2 * (jj - 1) + c] : 0.0;
+                    auto G = [&](const double *row, int lr, int jj) -> double {
+                        return (row && jj >= 1 && jj <= N && !held(g, lr, jj)) ? row[2 * (jj - 1) + c] : 0.0;
                     };
-                    auto D1 = [&](const double *row) -> double {
-                        if (g->fd_order == 3) return (G(row, j + 1) - G(row, j - 1)) / (2.0 * dr);
-                        return (-G(row, j + 2) + 8.0 * G(row, j + 1) - 8.0 * G(row, j - 1) + G(row, j - 2)) / (12.0 * dr);
+                    auto D1 = [&](const double *row, int lr) -> double {
+                        if (g->fd_order == 3) return (G(row, lr, j + 1) - G(row, lr, j - 1)) / (2.0 * dr);
+                        return (-G(row, lr, j + 2) + 8.0 * G(row, lr, j + 1) - 8.0 * G(row, lr, j - 1) + G(row, lr, j - 2)) / (12.0 * dr);
                     };
-                    s[c] = cm * (D1(flm) - (l / r) * G(flm, j)) + cp * (D1(flp) + ((l + 1) / r) * G(flp, j));
+                    s[c] = cm * (D1(flm, l - 1) - (l / r) * G(flm, l - 1, j)) + cp * (D1(flp, l + 1) + ((l + 1) / r) * G(flp, l + 1, j));
                 }
                 // -i (s0 + i s1) = s1 - i s0
                 out[2L * l * N + 2 * (j - 1)] += e * s[1];
                 out[2L * l * N + 2 * (j - 1) + 1] += -e * s[0];
             }
+            if (held(g, l, j)) { out[2L * l * N + 2 * (j - 1)] = 0.0; out[2L * l * N + 2 * (j - 1) + 1] = 0.0; }
         }
     }
 }
@@ -458,6 +478,14 @@ int oracle_apply_H(const oracle_grid *g, const double *psi, const double *e_fiel
     return 0;
 }
 
+int oracle_is_held(const oracle_grid *g, int l, int j) { return (grid_ok(g) && held(g, l, j)) ? 1 : 0; }
+
+int oracle_project(const oracle_grid *g, double *psi) {
+    if (!grid_ok(g) || !psi) return -1;
+    project_all(g, psi);
+    return 0;
+}
+
 int oracle_dense_H(const oracle_grid *g, double e_field, double *h) {
     if (!grid_ok(g) || !h) return -1;
     const int N = g->n_r, L = g->n_l;
@@ -488,6 +516,7 @@ int oracle_dense_H(const oracle_grid *g, double e_field, double *h) {
                         const int lg = std::max(l, lp);  // l_> of P:94 Eq. 9
                         v = e_field * r_of(g, j) * std::sqrt((double)lg * lg / (4.0 * lg * lg - 1.0));
                     }
+                    if (held(g, l, j) || held(g, lp, jp)) v = 0.0;      // cut-off: rows and columns of held points vanish
                     h[((long)l * N + (j - 1)) * n + ((long)lp * N + (jp - 1))] = v;
                 }
     return 0;
@@ -559,6 +588,7 @@ int oracle_step_taylor(const oracle_grid *g, const oracle_pulse *pulse, double *
                        int order, double t0, double dt, long nsteps, int field_sample,
                        const oracle_obs *obs) {
     if (!grid_ok(g) || !pulse || !psi || order < 1 || nsteps < 0) return -1;
+    project_all(g, psi);       // centrifugal cut-off (if any): the held points are zero from here on
     const long M = n_points(g);
     std::vector<double> term(2 * M), hterm(2 * M);
     long block = 0;
@@ -593,6 +623,7 @@ int oracle_step_taylor(const oracle_grid *g, const oracle_pulse *pulse, double *
 // closed-form ground-state energy of the 3-point scheme pins it).
 int oracle_step_imag(const oracle_grid *g, double *psi, int order, double dt, long nsteps, double *energy_out) {
     if (!grid_ok(g) || !psi || order < 1 || nsteps < 0 || !(dt > 0.0)) return -1;
+    project_all(g, psi);       // centrifugal cut-off (if any): the held points are zero from here on
     const long M = n_points(g);
     std::vector<double> term(2 * M), hterm(2 * M);
     for (long n = 0; n < nsteps; ++n) {
@@ -619,6 +650,7 @@ int oracle_step_imag(const oracle_grid *g, double *psi, int order, double dt, lo
 int oracle_step_rk_fixed(const oracle_grid *g, const oracle_pulse *pulse, double *psi, int tableau,
                          double t0, double dt, long nsteps, double *err_out, const oracle_obs *obs) {
     if (!grid_ok(g) || !pulse || !psi || nsteps < 0 || tableau < 0 || tableau > 5) return -1;
+    project_all(g, psi);       // centrifugal cut-off (if any): the held points are zero from here on
     const Tableau tb = tableau_of(tableau);
     const long MB = n_points(g) * g->batch;
     std::vector<std::vector<double>> k(tb.s, std::vector<double>(2 * MB));
@@ -646,6 +678,7 @@ int oracle_step_rk4(const oracle_grid *g, const oracle_pulse *pulse, double *psi
 int oracle_step_rk_sigma(const oracle_grid *g, const oracle_pulse *pulse, double *psi, int tableau,
                          double t0, double dt, long nsteps, double *sigma_out, const oracle_obs *obs) {
     if (!grid_ok(g) || !pulse || !psi || nsteps < 0 || tableau < 0 || tableau > 5) return -1;
+    project_all(g, psi);       // centrifugal cut-off (if any): the held points are zero from here on
     const Tableau tb = tableau_of(tableau);
     const long M = n_points(g), MB = M * g->batch;
     std::vector<std::vector<double>> k(tb.s, std::vector<double>(2 * MB));
@@ -669,6 +702,7 @@ int oracle_step_rk45(const oracle_grid *g, const oracle_pulse *pulse, double *ps
                      const double *dt_replay, long n_replay,
                      long *n_accept, long *n_reject, double *dt_log, double *err_log, long max_log) {
     if (!grid_ok(g) || !pulse || !psi || rtol <= 0.0) return -1;
+    project_all(g, psi);       // centrifugal cut-off (if any): the held points are zero from here on
     const Tableau tb = tableau_of(1);
     const long MB = n_points(g) * g->batch;
     std::vector<std::vector<double>> k(tb.s, std::vector<double>(2 * MB));
@@ -727,6 +761,7 @@ int oracle_step_lanczos(const oracle_grid *g, const oracle_pulse *pulse, double 
                         int krylov_dim, int taylor_order, double t0, double dt, long nsteps,
                         int field_sample, double beta_tol, const oracle_obs *obs) {
     if (!grid_ok(g) || !pulse || !psi || krylov_dim < 1 || taylor_order < 1 || nsteps < 0) return -1;
+    project_all(g, psi);       // centrifugal cut-off (if any): the held points are zero from here on
     const long M = n_points(g);
     std::vector<double> q(2 * M * krylov_dim), w(2 * M);
     std::vector<double> alpha(krylov_dim), beta(krylov_dim), coef(2 * krylov_dim);

@@ -40,6 +40,10 @@ typedef struct {
     int    batch;     /* B independent members                               */
     double r_offset;  /* the paper's grid `Offset`; 0 normally   */
     int    gauge;     /* 0 length gauge (Eq. 11), 1 velocity gauge (Eq. 12) */
+    double cutoff_lambda; /* centrifugal inner cut-off Lambda (an EXTENSION beyond the paper, motivated
+                         by P:454 "not always stable"): 0 = none; > 0: f_l(r_j) is held at zero wherever
+                         l(l+1)/(2 r_j^2) > Lambda, i.e. H is replaced by its principal sub-matrix on the remaining
+                         points (still real symmetric), which bounds the centrifugal part of rho(H) by Lambda */
 } oracle_grid;
 
 typedef struct {      /* kind 0: E(t) = e0 sin^2(omega t/(2 n_c)) cos(omega t + cep) */
@@ -58,8 +62,15 @@ double oracle_pulse_A(const oracle_pulse *p, double t);
 void   oracle_coupling(int n_l, double *c);
 
 /* out = H(E) psi, matrix-free (Eq. 11 with P:89 Eq. 7, Eq. 9, Eq. 15).
- * psi, out: [B][L][N_r] complex128; e_field: [B]. returns 0 or <0 on bad args. */
+ * psi, out: [B][L][N_r] complex128; e_field: [B]. returns 0 or <0 on bad args.
+ * With a centrifugal cut-off this is P H P: held points read as zero and come out as zero. */
 int oracle_apply_H(const oracle_grid *g, const double *psi, const double *e_field, double *out);
+
+/* Centrifugal cut-off: 1 if point (l, j), j = 1..N_r, is HELD at zero, i.e. cutoff_lambda > 0 and
+ * l(l+1) > 2 Lambda r_j^2 (evaluated as (double)(l(l+1)) > (2.0*Lambda)*(r_j*r_j) with r_j = j*dr + r_offset). */
+int oracle_is_held(const oracle_grid *g, int l, int j);
+/* psi <- P psi: zero the held points of every member (the propagators do this on entry when a cut-off is set). */
+int oracle_project(const oracle_grid *g, double *psi);
 
 /* Dense real-symmetric H for ONE member (g->batch ignored), built entry by entry
  * from the block structure of P:134/P:142 (Fig. 1): h[(l*N_r + j-1)*n + (l'*N_r + j'-1)].

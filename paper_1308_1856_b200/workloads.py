@@ -103,12 +103,18 @@ def pulses(c):
 
 def rho_gershgorin(c, e0_max=None):
     """Upper bound of the spectral radius of H used ONLY to choose a stable step:
-    kappa_G/dr^2 + (L-1)L/(2 dr^2) + E0 r_max, kappa_G = 2 (3-point) or 8/3 (5-point)."""
+    kappa_G/dr^2 + (L-1)L/(2 dr^2) + E0 r_max, kappa_G = 2 (3-point) or 8/3 (5-point).  With a centrifugal inner
+    cut-off c["cutoff_lambda"] > 0 (an extension beyond the paper: points with l(l+1)/(2 r^2) > Lambda are held at
+    zero) the centrifugal part is at most Lambda."""
     if e0_max is None:
         e0_max = max(p[0] for p in pulses(c))
     kg = 2.0 if c["fd_order"] == 3 else 8.0 / 3.0
     dr2 = c["dr"] ** 2
-    return kg / dr2 + (c["n_l"] - 1) * c["n_l"] / (2.0 * dr2) + e0_max * c["n_r"] * c["dr"]
+    cen = (c["n_l"] - 1) * c["n_l"] / (2.0 * dr2)
+    lam = c.get("cutoff_lambda", 0.0)
+    if lam > 0.0:
+        cen = min(cen, lam)
+    return kg / dr2 + cen + e0_max * c["n_r"] * c["dr"]
 
 
 def dt_eff(c, propagator=None, order=None, t_run=None):

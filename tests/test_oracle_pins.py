@@ -825,3 +825,106 @@ def test_P14_rk_methods_convergence_and_sigma():
     _, rel, _ = oracle.step_rk_fixed(g, pulse, psi, 1, t0, 2e-3, 1)
     m_el = g.n_l * g.n_r
     assert abs(s[0] - rel[0] * np.linalg.norm(out) / math.sqrt(m_el)) <= 1e-12 * s[0]
+
+
+# --------------------------------------------------------------- centrifugal inner cut-off (P15, NEXT f4: an extension)
+def plain_held(n_r, dr, n_l, lam):
+    """The definition written out: point (l, j) is held at zero iff l(l+1)/(2 r_j^2) > Lambda."""
+    r = dr * np.arange(1, n_r + 1)
+    l = np.arange(n_l)[:, None]
+    return l * (l + 1) / (2.0 * r[None, :] ** 2) > lam
+
+
+@pytest.mark.parametrize("fd", [3, 5])
+def test_P15_cutoff_is_the_principal_submatrix(fd):
+    """With a cut-off the dense H is the un-cut H on the points that are not held and zero elsewhere (a principal
+    sub-matrix: still exactly symmetric); the matrix-free operator equals it column by column; its spectral radius obeys
+    kappa_G/dr^2 + Lambda + E0 r_max (LAPACK) while the un-cut radius is dominated by the centrifugal term at r_1."""
+    n_r, dr, n_l, lam, e = 60, 0.1, 7, 40.0, 0.07
+    g0 = oracle.make_grid(n_r, dr, n_l, fd)
+    gc = oracle.make_grid(n_r, dr, n_l, fd, cutoff_lambda=lam)
+    held = plain_held(n_r, dr, n_l, lam)
+    assert np.array_equal(oracle.held_mask(gc), held)
+    assert held.sum() > 10 and not held[0].any() and held[-1, 0] and not held[-1, -1]
+    h0, hc = oracle.dense_H(g0, e), oracle.dense_H(gc, e)
+    act = ~held.ravel()
+    expect = np.where(np.outer(act, act), h0, 0.0)
+    assert np.array_equal(hc, expect)
+    assert np.array_equal(hc, hc.T)
+    x = rand_state((1, n_l, n_r), 77)
+    y = oracle.apply_H(gc, x, e)
+    assert np.max(np.abs(y.ravel() - hc @ x.ravel())) <= 1e-12 * np.max(np.abs(y))
+    assert np.count_nonzero(y[0][held]) == 0
+    kg = 2.0 if fd == 3 else 8.0 / 3.0
+    rho_c = np.max(np.abs(np.linalg.eigvalsh(hc)))
+    rho_0 = np.max(np.abs(np.linalg.eigvalsh(h0)))
+    assert rho_c <= kg / dr ** 2 + lam + e * n_r * dr
+    assert rho_0 > (n_l - 1) * n_l / (2 * dr ** 2) and rho_0 > 5 * rho_c
+    # the same bound is what the step-size rule uses
+    c = dict(n_r=n_r, dr=dr, n_l=n_l, fd_order=fd, batch=1, intensity=1e14, lam_nm=800.0, n_cycles=2, cutoff_lambda=lam)
+    c["omega"] = wl.omega_of_nm(800.0)
+    assert wl.rho_gershgorin(c, e0_max=e) >= rho_c
+
+
+def test_P15_cutoff_stabilises_the_step_and_converges_with_lambda():
+    """Purpose and harmlessness of the cut-off (the paper only says Taylor is "not always stable",
+    P:454).  Hydrogen from the discrete 1s state through a whole 2-cycle pulse (omega = 0.6, E0 = 0.25), L = 10:
+    (i) at 2.5/rho of the CUT operator the cut Taylor-4 run keeps the norm to 1e-10 and the held points exactly zero, in
+    13 to 19 times fewer steps, while the un-cut operator overflows at that step; (ii) the 1s population, the dipole and
+    the l <= 2 blocks converge to the un-cut run (at its own, much smaller stable step) as Lambda grows: 3e-2, 2e-3,
+    1e-6 relative at Lambda = 10, 40, 160; (iii) a Lambda that holds no point is bit-identical to no cut-off."""
+    n_r, dr, n_l = 200, 0.1, 10
+    e0, om = 0.25, 0.6
+    c = wl.config("cfg1", n_r=n_r, dr=dr, n_l=n_l, fd_order=3, intensity=e0 ** 2 * wl.AU_INTENSITY_W_CM2)
+    pulses = [(e0, om, 2.0, 0.0)]
+    t_run = 2 * math.pi * 2.0 / om
+    g0 = oracle.make_grid(n_r, dr, n_l, 3)
+    _, phi = oracle.bound_states(g0, 0, 1)
+    st = (np.array([0], dtype=np.int32), phi)
+    psi0 = wl.ground_state(c, phi[0])
+    oracle.set_threads(4)
+    res = {}
+    for lam in (0.0, 10.0, 40.0, 160.0):
+        dt = wl.dt_eff(dict(c, cutoff_lambda=lam), "taylor", 4, t_run=t_run)
+        n = int(round(t_run / dt))
+        g = oracle.make_grid(n_r, dr, n_l, 3, cutoff_lambda=lam)
+        psi, rows = oracle.step_taylor(g, pulses, psi0, 4, 0.0, dt, n, states=st, obs_every=n)
+        assert np.count_nonzero(psi[0][oracle.held_mask(g)]) == 0
+        assert abs(rows[-1, 0, 0] - 1.0) <= 1e-10                        # (i) norm
+        res[lam] = (n, rows[-1, 0], psi)
+    oracle.set_threads(1)
+    assert res[0.0][0] > 12 * res[160.0][0] and res[0.0][0] > 18 * res[10.0][0]
+    dt = t_run / res[40.0][0]
+    bad, _ = oracle.step_taylor(g0, pulses, psi0, 4, 0.0, dt, 400)       # the un-cut operator at the cut run's step
+    assert not np.all(np.isfinite(bad.view(np.float64))) or np.max(np.abs(bad)) > 1e6
+    ref = res[0.0]
+    assert 0.2 < ref[1][3] < 0.5 and abs(ref[1][1]) > 0.1                # the pulse did something (p_1s = 0.313)
+    low = [np.linalg.norm(res[lam][2][0, :3] - ref[2][0, :3]) / np.linalg.norm(ref[2][0, :3]) for lam in (10.0, 40.0, 160.0)]
+    pop = [abs(res[lam][1][3] - ref[1][3]) for lam in (10.0, 40.0, 160.0)]
+    dip = [abs(res[lam][1][1] - ref[1][1]) for lam in (10.0, 40.0, 160.0)]
+    assert low[0] > 10 * low[1] > 100 * low[2] and low[2] <= 1e-5        # (ii)
+    assert pop[0] > pop[1] > pop[2] and pop[2] <= 1e-6 and dip[0] > dip[1] > dip[2] and dip[2] <= 1e-5
+    g_big = oracle.make_grid(n_r, dr, n_l, 3, cutoff_lambda=1e9)          # (iii)
+    assert not oracle.held_mask(g_big).any()
+    a, _ = oracle.step_taylor(g_big, pulses, psi0, 4, 0.0, 1e-4, 20)
+    b, _ = oracle.step_taylor(g0, pulses, psi0, 4, 0.0, 1e-4, 20)
+    assert np.array_equal(a, b)
+
+
+def test_P15_cutoff_in_every_propagator_against_the_dense_exponential():
+    """RK4, Dormand-Prince, Lanczos and imaginary time all go through the same P H P: each against scipy's expm of the
+    cut dense matrix at a frozen field."""
+    n_r, dr, n_l, lam, e = 50, 0.2, 5, 15.0, 0.05
+    g = oracle.make_grid(n_r, dr, n_l, 5, cutoff_lambda=lam)
+    hc = oracle.dense_H(g, e)
+    psi0 = oracle.project(g, rand_state((1, n_l, n_r), 5))
+    psi0 /= math.sqrt(dr * np.sum(np.abs(psi0) ** 2))
+    dt, n = 2e-4, 10                                  # y = dt rho = 0.02: RK4's y^5/120 per step is far below 1e-9
+    exact = (sla.expm(-1j * hc * dt * n) @ psi0.ravel()).reshape(psi0.shape)
+    static = (e, 0.0, 1.0, 0.0)
+    for name, got in (("rk4", oracle.step_rk4(g, static, psi0, 0.0, dt, n)[0]),
+                      ("dp", oracle.step_rk_fixed(g, static, psi0, 1, 0.0, dt, n)[0]),
+                      ("lanczos", oracle.step_lanczos(g, static, psi0, 12, 12, 0.0, dt, n)[0]),
+                      ("taylor", oracle.step_taylor(g, static, psi0, 8, 0.0, dt, n)[0])):
+        assert np.linalg.norm(got - exact) <= 1e-9, name
+        assert np.count_nonzero(got[0][oracle.held_mask(g)]) == 0, name
