@@ -110,6 +110,7 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
     const int gr0 = rbase + r0;                                // global row of this thread's patch row 0
     const double2 z2 = make_double2(0.0, 0.0);
     const bool al32 = !MASK && ((N & 1) == 0) && ((H & 1) == 0) && ((W & 1) == 0);
+    const bool ragged_rows = (csize * NWR * RP != L);
 
     for (int r = threadIdx.x; r < NWR * RP; r += G::NT) {
         const int l = rbase + r;
@@ -150,15 +151,16 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
         armed = false;
     };
     // tile of work item `it` -> stage (one thread; the stage must have been consumed by every thread)
-    auto fetch_item = [&](const int it) {
-        if (TMA && threadIdx.x == 0 && it < n_items) {
-            const int fb = it / n_tiles, ft = it - fb * n_tiles;
+    auto fetch_tile = [&](const int fb, const int ft) {
+        if (TMA && threadIdx.x == 0) {
             fence_proxy_async_smem();
             mbar_expect_tx(&sm.mbar, kStageBytes);
             tma_load_3d(sm.stage, &tmap, 0, rp_start(ft, W, H, N, WT) >> 3, fb * L + rbase, &sm.mbar);
         }
     };
-    fetch_item(cid);
+    const int db = ncl / n_tiles, dtile = ncl - db * n_tiles;
+    int b = cid / n_tiles, t = cid - b * n_tiles;
+    if (cid < n_items) fetch_tile(b, t);
 
     const double wl = (lane == 0) ? 0.0 : 1.0, wrt = (lane == 31) ? 0.0 : 1.0;
     // l-1 / l+1 rows of the neighbouring row groups (or the zero row); the parity offset is 0 for the zero row
@@ -175,13 +177,13 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
     }
 
     int t_cur = -1;
+    double ef_cur = (cid < n_items) ? __ldg(ef + b) : 0.0, ef_next = 0.0;
     double Dq[CP], Cq[CP], Eq[CP];
     bool dom[CP];
 #pragma unroll
     for (int q = 0; q < CP; ++q) { Dq[q] = 0.0; Cq[q] = 0.0; dom[q] = true; }
 
     for (int item = cid; item < n_items; item += ncl) {
-        const int b = item / n_tiles, t = item - b * n_tiles;
         const int start = rp_start(t, W, H, N, WT);
         const double2 *src_g = in + ((size_t)b * L + rbase) * N + start + c0;
         // ---- own patch straight from global memory -------------------------------------------------------------
@@ -189,7 +191,7 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
         if (TMA) {
             if (order < 2 && item != cid) {      // no second order whose barrier could have covered the refill
                 if (armed) bar_wait();
-                fetch_item(item);
+                fetch_tile(b, t);
             }
             mbar_wait(&sm.mbar, tma_phase);
             tma_phase ^= 1u;
@@ -233,7 +235,7 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
         }
         // coupling weights E r_j / c1 for the field value of this step (Taylor) or of RK stage `st`
         auto set_field = [&](const int st) {
-            const double es = inv_c1 * (__ldg(ef + st * g.batch + b) * g.dr);
+            const double es = inv_c1 * (((RK || st) ? __ldg(ef + st * g.batch + b) : ef_cur) * g.dr);
 #pragma unroll
             for (int q = 0; q < CP; ++q) Eq[q] = es * (double)(dom[q] ? start + c0 + q + 1 : 1);
         };
@@ -347,8 +349,13 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                 do_row(Ti, To, 2, Ti[1], Ti[3], a1, a2, ll1[2], pr, odd, first, s, want_out, cg);
             }
             bar_wait();
-            // every value of the stage was consumed by the arithmetic of order 1: fetch the next item
-            if (TMA && k == 2) fetch_item(item + ncl);
+            // every value of the stage was consumed by the arithmetic of order 1: fetch the next item (and its field value)
+            if (TMA && k == 2 && item + ncl < n_items) {
+                int nb = b + db, nt = t + dtile;
+                if (nt >= n_tiles) { nt -= n_tiles; ++nb; }
+                fetch_tile(nb, nt);
+            }
+            if (!RK && k == 1 && item + ncl < n_items) ef_next = __ldg(ef + b + db + ((t + dtile >= n_tiles) ? 1 : 0));
             double2 lo[CP], below[CP];
 #pragma unroll
             for (int q = 0; q < CP; ++q) {
@@ -431,7 +438,7 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
             const int lo_c = t * W - start;                  // first interior column (tile coordinates)
             int wint = N - t * W;
             if (wint > W) wint = W;
-            double2 *dst_g = out + ((size_t)b * L + rbase) * N + start + c0;
+            double2 *dst_g = out + ((size_t)b * L + rbase + r0) * N + start + c0;
             if (MODE != 2 && g.mask != nullptr) {            // absorbing boundary: psi *= exp(-i W dt) (Eq. 18)
 #pragma unroll
                 for (int q = 0; q < CP; ++q) {
@@ -441,23 +448,31 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                     for (int r = 0; r < RP; ++r) { A[r][q].x *= m; A[r][q].y *= m; }
                 }
             }
+            bool in_c[CP], row_ok[RP];
 #pragma unroll
-            for (int q = 0; q < CP; q += 2) {
-                const int c = c0 + q;
-                const bool in0 = c >= lo_c && c < lo_c + wint, in1 = c + 1 >= lo_c && c + 1 < lo_c + wint;
+            for (int q = 0; q < CP; ++q) in_c[q] = c0 + q >= lo_c && c0 + q < lo_c + wint;
 #pragma unroll
-                for (int r = 0; r < RP; ++r) {
-                    if (gr0 + r >= L) continue;
-                    double2 *p = dst_g + (size_t)(r0 + r) * N + q;
-                    if (al32) {
-                        if (in0) stg256(p, A[r][q], A[r][q + 1]);      // interior bounds are even: in0 == in1
-                    } else {
-                        if (in0) p[0] = A[r][q];
-                        if (in1) p[1] = A[r][q + 1];
-                    }
-                }
+            for (int r = 0; r < RP; ++r) row_ok[r] = !ragged_rows || gr0 + r < L;
+            double2 *prow[RP];
+#pragma unroll
+            for (int r = 0; r < RP; ++r) prow[r] = dst_g + (size_t)r * N;
+            if (al32) {                                      // interior bounds are even: in_c[q] == in_c[q + 1]
+#pragma unroll
+                for (int r = 0; r < RP; ++r)
+#pragma unroll
+                    for (int q = 0; q < CP; q += 2)
+                        if (in_c[q] && row_ok[r]) stg256(prow[r] + q, A[r][q], A[r][q + 1]);
+            } else {
+#pragma unroll
+                for (int r = 0; r < RP; ++r)
+#pragma unroll
+                    for (int q = 0; q < CP; ++q)
+                        if (in_c[q] && row_ok[r]) prow[r][q] = A[r][q];
             }
         }
+        b += db; t += dtile;
+        if (t >= n_tiles) { t -= n_tiles; ++b; }
+        ef_cur = ef_next;
     }
     if (armed) bar_wait();     // (cluster: no CTA may exit while a neighbour can still read its shared memory)
 }

@@ -830,3 +830,60 @@ def test_error_codes_and_lifecycle(B):
     assert ei.value.code == -4
     h.close()
     h2.close()
+
+
+# ------------------------------------------------------------------------------------------------- sanitizer selection
+def test_sanitizer_selection(B):
+    """A short walk through every kernel family on small grids (register-patch kernel: direct loads, TMA, cluster +
+    DSMEM, fused RK4, imaginary time, masked; tile kernels: register-staged, TMA, three-source Lanczos pass; RK45
+    controller; observables with many states) -- the selection profiles/ runs under compute-sanitizer (memcheck,
+    racecheck).  It also checks parity, so it is a regular test as well."""
+    import torch
+    cases = [
+        # n_r, n_l, fd, batch, what
+        (264, 16, 3, 3, "taylor"), (300, 16, 5, 2, "taylor"), (264, 40, 3, 1, "taylor"), (100, 3, 3, 1, "taylor"),
+        (264, 16, 5, 2, "rk4"), (264, 40, 3, 1, "imag"), (264, 11, 5, 2, "lanczos"), (260, 6, 3, 1, "lanczos"),
+        (264, 9, 5, 1, "rk45"), (264, 9, 3, 2, "apply"),
+    ]
+    for n_r, n_l, fd, batch, what in cases:
+        c = wl.config("cfg5" if batch > 1 else "cfg1", n_r=n_r, dr=0.1, n_l=n_l, fd_order=fd, batch=batch, order=4)
+        g, h = both(B, c)
+        pulses = wl.pulses(c)
+        h.set_pulse(pulses)
+        st = bound_pack(g, [(0, 0), (1, 0), (0, 1), (2, 0), (1, 1)])
+        h.set_bound_states(*st)
+        psi0 = wl.populated_state(c)
+        h.set_state(psi0)
+        t0, n = 0.5 * c["t_pulse"], 6
+        if what == "taylor":
+            dt = wl.dt_eff(c, "taylor", 4)
+            h.step_taylor(4, t0, dt, n, 2)
+            ref, robs = oracle.step_taylor(g, pulses, psi0, 4, t0, dt, n, states=st, obs_every=2)
+            check_fixed(h.get_state(), ref, h.obs_log(), robs)
+        elif what == "rk4":
+            dt = wl.dt_eff(c, "rk4", 4)
+            h.step_rk4(t0, dt, n, 3)
+            ref, robs = oracle.step_rk4(g, pulses, psi0, t0, dt, n, states=st, obs_every=3)
+            check_fixed(h.get_state(), ref, h.obs_log(), robs)
+        elif what == "imag":
+            dt = 0.2 * wl.dt_eff(c, "taylor", 4)
+            h.step_imag(4, dt, n)
+            assert rel_l2(h.get_state(), oracle.step_imag(g, psi0, 4, dt, n)[0]) <= TOL_PSI
+        elif what == "lanczos":
+            dt = wl.dt_eff(c, "lanczos", 12)
+            h.step_lanczos(6, 12, t0, dt, 3, 1)
+            ref, robs = oracle.step_lanczos(g, pulses, psi0, 6, 12, t0, dt, 3, states=st, obs_every=1)
+            check_fixed(h.get_state(), ref, h.obs_log(), robs)
+        elif what == "rk45":
+            info = h.step_rk45(t0, t0 + 2e-3, 1e-4, 1e-8)
+            ref, _ = oracle.step_rk45(g, pulses, psi0, t0, t0 + 2e-3, 1e-4, 1e-8, dt_replay=info["dt"])
+            assert rel_l2(h.get_state(), ref) <= TOL_PSI
+        else:
+            x = torch.from_numpy(wl.random_state(c)).cuda()
+            y = torch.empty_like(x)
+            for tma in (2, 0):
+                h.set_option("apply_tma", tma)
+                h.apply_H(x, y, 0.05)
+                torch.cuda.synchronize()
+                assert rel_l2(y.cpu().numpy(), oracle.apply_H(g, wl.random_state(c), 0.05)) <= TOL_H
+        h.close()
