@@ -83,6 +83,10 @@ void tdse_destroy(tdse_handle *h);
  *   "taylor_rp_variant" [-1] instantiation of the register-patch kernel (-1: heuristic)
  *   "taylor_rp_tma"    [-1] register-patch kernel: fetch tiles by TMA tensor copies (-1: heuristic, 0: never,
  *                          1: whenever n_r % 8 == 0 and the grid is wider than a tile)
+ *   "obs_fused"        [1] logged observable rows are reduced inside the register-patch step kernel (from the registers
+ *                          that hold psi(t + dt); no extra pass over psi) when it runs on full tiles, at most 4 bound
+ *                          states are set and the grid is at most 16 CTAs (beyond that the separate pass measured
+ *                          faster); 2: wherever the kernel can; 0: always the separate observable kernels
  *   "lanczos_beta_tol" [1e-12] breakdown threshold on beta ("if beta = 0 then quit", R-G17)
  *   "rk45_dt_max"      [0 = none] cap on the adaptive step
  *   "rk45_check_every" [32] attempted steps enqueued between host checks of the device `done` flag */
@@ -94,6 +98,15 @@ int  tdse_set_option(tdse_handle *h, const char *key, double value);
  * R-G26).  r_b <= 0 removes the absorber.  tdse_step_rk45 returns TDSE_ERR_UNSUPPORTED while one is set; the
  * imaginary-time propagation ignores it.  Synchronises the device. */
 int  tdse_set_absorber(tdse_handle *h, double r_b, int p);
+
+/* Centrifugal inner cut-off -- an EXTENSION beyond the paper, motivated by its remark that the
+ * explicit propagators are "not always stable": with lambda > 0 every point (l, j) with l(l+1)/(2 r_j^2) > lambda
+ * is HELD at zero and H is replaced by its principal sub-matrix on the remaining points (still real symmetric), so the
+ * centrifugal part of the spectral radius is at most lambda and the stable step grows from about 1/(L^2/(2 dr^2)) to
+ * about 1/(kappa/dr^2 + lambda).  The rule is evaluated as (double)(l(l+1)) > (2.0*lambda)*(r_j*r_j), r_j = j*dr.
+ * Applies to tdse_apply_H (P H P: held inputs read as zero, held outputs are zero) and to every propagator; the
+ * current state and every later tdse_set_state are projected.  lambda = 0 removes it.  Synchronises the device. */
+int  tdse_set_cutoff(tdse_handle *h, double lambda);
 
 /* One pulse per member, host array [batch].  TDSE_ERR_UNSUPPORTED for a kind-0 pulse on a velocity-gauge handle. */
 int  tdse_set_pulse(tdse_handle *h, const tdse_pulse *per_member_host);

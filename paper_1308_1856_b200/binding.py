@@ -17,7 +17,7 @@ ERRORS = {-1: "TDSE_ERR_ARG", -2: "TDSE_ERR_ALLOC", -3: "TDSE_ERR_CUDA", -4: "TD
 
 # every symbol include/tdse.h declares
 SYMBOLS = ["tdse_create", "tdse_destroy", "tdse_set_option", "tdse_set_pulse", "tdse_set_bound_states",
-           "tdse_set_state", "tdse_get_state", "tdse_apply_H", "tdse_set_absorber", "tdse_bound_population", "tdse_step_taylor", "tdse_step_imag", "tdse_energy_log", "tdse_step_rk4", "tdse_step_rk", "tdse_rk_sigma",
+           "tdse_set_cutoff", "tdse_set_state", "tdse_get_state", "tdse_apply_H", "tdse_set_absorber", "tdse_bound_population", "tdse_step_taylor", "tdse_step_imag", "tdse_energy_log", "tdse_step_rk4", "tdse_step_rk", "tdse_rk_sigma",
            "tdse_step_lanczos", "tdse_step_rk45", "tdse_observables", "tdse_obs_log", "tdse_dt_log",
            "tdse_lanczos_info", "tdse_ionisation_yield", "tdse_graph_instantiations", "tdse_launch_count", "tdse_taylor_was_blocked", "tdse_strerror", "tdse_version"]
 
@@ -64,6 +64,7 @@ def lib():
         L.tdse_step_rk.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_long, C.c_int, vp]
         L.tdse_rk_sigma.argtypes = [vp, C.POINTER(C.c_double), vp]
         L.tdse_set_absorber.argtypes = [vp, C.c_double, C.c_int]
+        L.tdse_set_cutoff.argtypes = [vp, C.c_double]
         L.tdse_bound_population.argtypes = [vp, C.c_double, C.POINTER(C.c_double), vp]
         L.tdse_energy_log.argtypes = [vp, C.POINTER(C.c_double), C.c_long, vp]
         L.tdse_step_rk4.argtypes = [vp, C.c_double, C.c_double, C.c_long, C.c_int, vp]
@@ -204,6 +205,10 @@ class Tdse:
     def step_taylor(self, order, t0, dt, nsteps, obs_every=0, stream=None):
         _check(lib().tdse_step_taylor(self._h, int(order), float(t0), float(dt), int(nsteps), int(obs_every),
                                       _stream(stream)), "tdse_step_taylor")
+
+    def set_cutoff(self, lam):
+        """Centrifugal inner cut-off Lambda (an extension beyond the paper); 0 removes it."""
+        _check(lib().tdse_set_cutoff(self._h, float(lam)), "tdse_set_cutoff")
 
     def set_absorber(self, r_b, p):
         _check(lib().tdse_set_absorber(self._h, float(r_b), int(p)), "tdse_set_absorber")

@@ -113,6 +113,8 @@ struct tdse_handle {
     int n_states = 0; double *d_phi = nullptr; int *d_lstate = nullptr;
     double *d_obs_partials = nullptr; int *d_loff = nullptr, *d_slist = nullptr; unsigned int *d_obs_counters = nullptr;
     double *d_yield = nullptr;
+    double *d_rp_part = nullptr; size_t rp_part_cap = 0; unsigned int *d_rp_counter = nullptr;   // fused observables
+    int obs_fused = 1;                      // option: reduce the logged rows in the step kernel when it can
     double *d_rows = nullptr; size_t rows_cap = 0; long log_rows = 0; double *d_row_direct = nullptr;
     // rk45 logs
     double *d_dtlog = nullptr, *d_errlog = nullptr, *d_replay = nullptr; long log_cap = 0, replay_cap = 0;
@@ -133,6 +135,7 @@ struct tdse_handle {
     int apply_tma = 1;                      // tdse_apply_H: TMA-fetched tiles when n_r % 8 == 0
     int lanczos_tma = 1;                    // Lanczos pass: sources fetched by TMA when n_r % 8 == 0
     double *d_sigma = nullptr;              // passive RK error sums [batch] (tdse_step_rk)
+    int *d_j0 = nullptr; double cutoff = 0.0;     // centrifugal inner cut-off (tdse_set_cutoff)
     double *d_mask = nullptr; double *d_pb = nullptr;   // absorber mask [n_r] (or null), bound populations [batch]
     double *d_elog = nullptr, *d_imag_inv = nullptr; size_t elog_cap = 0; long elog_rows = 0;
 };
@@ -274,6 +277,32 @@ int enqueue_imag_norm(tdse_handle *h, double2 *psi, int step_off, cudaStream_t s
     return TDSE_OK;
 }
 
+// the observable row of step `step_off` reduced inside the register-patch kernel (tdse_taylor_rp.cuh, OBS)
+// Measured (profiles/r02_README.md): on grids of many CTAs the fused reduction costs more than it saves (one more
+// barrier round per item, and a fence + ticket + last-CTA tail of 6-8 us per logged step against a 9 us pass of
+// obs_kernel over an L2-resident CFG3 state), so obs_fused = 1 (auto) uses it for grids of at most 16 CTAs and
+// obs_fused = 2 forces it wherever the kernel can do it.
+bool obs_fused_wanted(const tdse_handle *h) {
+    if (!h->obs_fused || !rp_obs_capable(h->rpp, h->grid, h->n_states)) return false;
+    return h->obs_fused == 2 || (long)h->rpp.n_items * h->rpp.cl <= 16;
+}
+bool obs_fused_now(const tdse_handle *h, int obs) { return obs && h->d_rp_part && obs_fused_wanted(h); }
+RpObs make_rp_obs(const tdse_handle *h, int step_off) {
+    RpObs o{};
+    o.ctl = h->d_ctl; o.pulse = h->d_pulse; o.phi = h->d_phi; o.l_of_state = h->d_lstate; o.n_states = h->n_states;
+    o.step_off = step_off; o.partials = h->d_rp_part; o.counter = h->d_rp_counter; o.rows = h->d_rows;
+    return o;
+}
+int ensure_rp_obs(tdse_handle *h, int obs_every) {
+    if (obs_every <= 0 || !obs_fused_wanted(h)) return TDSE_OK;
+    RC(ensure_buf(h, &h->d_rp_part, &h->rp_part_cap, rp_obs_partials(h->rpp)));
+    if (!h->d_rp_counter) {
+        CU(cudaMalloc(&h->d_rp_counter, sizeof(unsigned int)));
+        CU(cudaMemset(h->d_rp_counter, 0, sizeof(unsigned int)));
+    }
+    return TDSE_OK;
+}
+
 int enqueue_taylor_block(tdse_handle *h, int order, int n, int obs, cudaStream_t s) {
     const int B = h->grid.batch;
     if (h->imag) {
@@ -292,10 +321,12 @@ int enqueue_taylor_block(tdse_handle *h, int order, int n, int obs, cudaStream_t
         if (h->taylor_blocked_last) {
             // ping-pong psi <-> acc: even steps read psi, odd steps read acc (n is even inside graphs)
             double2 *src = (i & 1) ? acc : psi, *dst = (i & 1) ? psi : acc;
-            RC(launch_taylor_rp(h->gd, h->rpp, src, dst, ef, &h->d_ctl->dt, order, s));
+            const bool fused = !h->imag && obs_fused_now(h, obs);
+            const RpObs ro = make_rp_obs(h, i);
+            RC(launch_taylor_rp(h->gd, h->rpp, src, dst, ef, &h->d_ctl->dt, order, s, fused ? &ro : nullptr));
             count(h);
             if (h->imag) RC(enqueue_imag_norm(h, dst, i, s));
-            if (obs) RC(enqueue_obs(h, dst, i, 1, 0, 0.0, h->d_rows, s));
+            if (obs && !fused) RC(enqueue_obs(h, dst, i, 1, 0, 0.0, h->d_rows, s));
             continue;
         }
         for (int k = 1; k <= order; ++k) {
@@ -362,9 +393,11 @@ int enqueue_rk4_block(tdse_handle *h, int n, int obs, cudaStream_t s) {
         double2 *alt = h->pool[h->psi_slot == 0 ? 1 : 0];
         for (int i = 0; i < n; ++i) {
             double2 *src = (i & 1) ? alt : psi, *dst = (i & 1) ? psi : alt;
-            RC(launch_taylor_rp(h->gd, h->rpp, src, dst, h->d_etab + (size_t)i * 4 * B, &h->d_ctl->dt, 4, s));
+            const bool fused = obs_fused_now(h, obs);
+            const RpObs ro = make_rp_obs(h, i);
+            RC(launch_taylor_rp(h->gd, h->rpp, src, dst, h->d_etab + (size_t)i * 4 * B, &h->d_ctl->dt, 4, s, fused ? &ro : nullptr));
             count(h);
-            if (obs) RC(enqueue_obs(h, dst, i, 1, 0, 0.0, h->d_rows, s));
+            if (obs && !fused) RC(enqueue_obs(h, dst, i, 1, 0, 0.0, h->d_rows, s));
         }
         if (n & 1) {   // odd eager remainder: bring the state back into the psi slot
             OpCopy cp{}; cp.dst = psi; cp.src = alt;
@@ -610,7 +643,7 @@ int run_blocks(tdse_handle *h, int kind, int p1, int p2, int n, int obs, long nb
         }
         return TDSE_OK;
     }
-    const auto key = std::make_tuple(kind, p1, p2, n, obs + 2 * h->taylor_blocked_last + 256 * (h->rpp.variant + 1) + 8192 * h->rpp.tma + 16384 * h->rk4_fused + 32768 * h->imag, h->psi_slot);
+    const auto key = std::make_tuple(kind, p1, p2, n, obs + 2 * h->taylor_blocked_last + 256 * (h->rpp.variant + 1) + 8192 * h->rpp.tma + 16384 * h->rk4_fused + 32768 * h->imag + 65536 * (int)obs_fused_now(h, obs), h->psi_slot);
     auto it = h->graphs.find(key);
     if (it == h->graphs.end()) {
         cudaGraph_t g = nullptr;
@@ -643,6 +676,7 @@ int run_fixed(tdse_handle *h, int kind, int p1, int p2, double t0, double dt, lo
     if (h->taylor_blocked_last) G = (G + 1) & ~1;       // ping-pong needs an even block
     RC(ensure_buf(h, &h->d_etab, &h->etab_cap, (size_t)G * 7 * B));
     RC(ensure_rows(h, nsteps, obs_every));
+    if (h->taylor_blocked_last) RC(ensure_rp_obs(h, obs_every));
     CtlInit v{};
     v.t0 = t0; v.dt = dt; v.obs_every = obs_every; v.field_sample = h->field_sample;
     h->pending = 0;
@@ -759,7 +793,7 @@ void tdse_destroy(tdse_handle *h) {
     free_graphs(h);
     for (double2 *p : h->pool) cudaFree(p);
     void *ptrs[] = {h->d_vj, h->d_cen, h->d_cl, h->d_pulse, h->d_bufs, h->d_ctl, h->d_etab, h->d_eapply, h->d_partials,
-                    h->d_counter, h->d_phi, h->d_lstate, h->d_obs_partials, h->d_obs_counters, h->d_elog, h->d_imag_inv, h->d_mask, h->d_pb, h->d_sigma, h->d_loff, h->d_slist, h->d_yield, h->d_rows, h->d_row_direct,
+                    h->d_counter, h->d_phi, h->d_lstate, h->d_obs_partials, h->d_obs_counters, h->d_elog, h->d_imag_inv, h->d_mask, h->d_pb, h->d_sigma, h->d_j0, h->d_loff, h->d_slist, h->d_yield, h->d_rp_part, h->d_rp_counter, h->d_rows, h->d_row_direct,
                     h->d_dtlog, h->d_errlog, h->d_replay, h->d_alpha, h->d_beta, h->d_nrm, h->d_inv, h->d_coef,
                     h->d_m, h->d_nsub, h->d_basis};
     for (void *p : ptrs) if (p) cudaFree(p);
@@ -778,6 +812,7 @@ int tdse_set_option(tdse_handle *h, const char *key, double value) {
     else if (k == "taylor_rp_variant") { if (value < -1 || value >= kNumRpVariants) return TDSE_ERR_ARG; h->rp_variant = (int)value; free_graphs(h); }
     else if (k == "apply_tma") { if (value < 0 || value > 2) return TDSE_ERR_ARG; h->apply_tma = (int)value; }
     else if (k == "lanczos_tma") { if (value < 0 || value > 1) return TDSE_ERR_ARG; h->lanczos_tma = (int)value; free_graphs(h); }
+    else if (k == "obs_fused") { if (value != 0.0 && value != 1.0 && value != 2.0) return TDSE_ERR_ARG; h->obs_fused = (int)value; free_graphs(h); }
     else if (k == "rk4_block") { if (value < 0 || value > 1) return TDSE_ERR_ARG; h->rk4_block = (int)value; free_graphs(h); }
     else if (k == "taylor_rp_tma") { if (value < -1 || value > 1) return TDSE_ERR_ARG; h->rp_tma = (int)value; free_graphs(h); }
     else if (k == "lanczos_beta_tol") { if (!(value >= 0.0)) return TDSE_ERR_ARG; h->beta_tol = value; free_graphs(h); }
@@ -830,12 +865,24 @@ int tdse_set_bound_states(tdse_handle *h, int n_states, const int *l_of_state, c
     return TDSE_OK;
 }
 
+// psi <- P psi on the handle's state (no-op without a cut-off)
+static int project_state(tdse_handle *h, cudaStream_t s) {
+    if (!h->d_j0) return TDSE_OK;
+    OpProject op{};
+    op.psi = h->pool[h->psi_slot]; op.j0 = h->d_j0; op.n_r = h->grid.n_r; op.n_l = h->grid.n_l;
+    h->pending = 0;
+    RC(launch_ew(h, op, s));
+    h->launches += h->pending;
+    return TDSE_OK;
+}
+
 int tdse_set_state(tdse_handle *h, const void *psi, int is_device, void *stream) {
     if (!h || !psi) return TDSE_ERR_ARG;
     cudaStream_t s = (cudaStream_t)stream;
     CU(cudaMemcpyAsync(h->pool[h->psi_slot], psi, h->n_state * sizeof(double2),
                        is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s));
     if (!is_device) CU(cudaStreamSynchronize(s));
+    RC(project_state(h, s));                          // centrifugal cut-off (if set): the held points are zero from here on
     return TDSE_OK;
 }
 
@@ -1171,6 +1218,38 @@ int tdse_set_absorber(tdse_handle *h, double r_b, int p) {
     if (!h->d_mask) CU(cudaMalloc(&h->d_mask, sizeof(double) * N));
     CU(cudaMemcpy(h->d_mask, m.data(), sizeof(double) * N, cudaMemcpyHostToDevice));
     h->gd.mask = h->d_mask;
+    return TDSE_OK;
+}
+
+int tdse_set_cutoff(tdse_handle *h, double lambda) {
+    if (!h || !(lambda >= 0.0)) return TDSE_ERR_ARG;
+    CU(cudaDeviceSynchronize());
+    free_graphs(h);                                   // captured kernels hold the grid description by value
+    h->cutoff = lambda;
+    if (!(lambda > 0.0)) {
+        if (h->d_j0) cudaFree(h->d_j0);
+        h->d_j0 = nullptr; h->gd.j0 = nullptr; h->gd.j0_max = 0;
+        return TDSE_OK;
+    }
+    const int N = h->grid.n_r, L = h->grid.n_l;
+    std::vector<int> j0(L, 0);
+    int jmax = 0;
+    for (int l = 0; l < L; ++l) {
+        // point (l, j) is held iff l(l+1) > (2 Lambda) r_j^2 with r_j = (j+1) dr, in exactly this operation order
+        int j = 0;
+        while (j < N) {
+            const double r = (double)(j + 1) * h->grid.dr;
+            if (!((double)(l * (l + 1)) > (2.0 * lambda) * (r * r))) break;
+            ++j;
+        }
+        j0[l] = j;
+        jmax = std::max(jmax, j);
+    }
+    if (!h->d_j0) CU(cudaMalloc(&h->d_j0, sizeof(int) * L));
+    CU(cudaMemcpy(h->d_j0, j0.data(), sizeof(int) * L, cudaMemcpyHostToDevice));
+    h->gd.j0 = h->d_j0; h->gd.j0_max = jmax;
+    RC(project_state(h, nullptr));
+    CU(cudaDeviceSynchronize());
     return TDSE_OK;
 }
 

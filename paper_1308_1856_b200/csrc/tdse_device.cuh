@@ -20,6 +20,10 @@ struct GridDev {
     const double *vj;       // [n_r]  kinetic diagonal - Z/r_j          (Eq. 7, Eq. 15)
     const double *cen;      // [n_r]  1/(2 r_j^2)                       (centrifugal factor, Eq. 7)
     const double *cl;       // [n_l]  c_l = (l+1)/sqrt((2l+1)(2l+3))    (Eq. 9, m = 0)
+    const int *j0;          // [n_l]  centrifugal inner cut-off (an extension beyond the paper, tdse_set_cutoff): the points
+                            //        (l, j < j0[l]) are HELD at zero, H acts as its principal sub-matrix on the others;
+                            //        nullptr: no cut-off
+    int j0_max;             //        max_l j0[l]: columns >= j0_max are untouched by the cut-off
     const double *mask;     // [n_r]  absorbing-boundary factor exp(-i W(r_j) dt) of P:146 Eq. 18 applied after every
                             //        step, or nullptr (no absorber)
 };
@@ -48,6 +52,11 @@ struct RedCtx {
     unsigned int *counter;          // zero before the launch; reset by the last CTA
     int ctas_per_member;
 };
+
+// is point (l, j) (0-based column) held at zero by the centrifugal cut-off?  (rows outside 0..n_l-1 are zero anyway)
+__device__ __forceinline__ bool held_pt(const GridDev &g, int l, int j) {
+    return g.j0 != nullptr && l >= 0 && l < g.n_l && j < __ldg(g.j0 + l);
+}
 
 __device__ __forceinline__ double2 ldcg2(const double2 *p) { return __ldcg(p); }
 

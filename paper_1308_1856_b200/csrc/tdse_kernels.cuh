@@ -92,6 +92,7 @@ __global__ void __launch_bounds__(256, Epi::MINB) tile_kernel(GridDev g, Epi epi
         epi.prepare(b);
         const double2 *base = epi.input() + (size_t)b * g.n_l * g.n_r;
         const double sc = Epi::SCALED ? epi.in_scale(b) : 1.0;
+        const bool cut_tile = g.j0 != nullptr && j0 - T::HW < g.j0_max;         // the tile touches held points
         // optional second source: the tile holds in + c2in * in2 (a stage vector formed while loading)
         const double2 *base2 = Epi::TWO_IN ? epi.input2() + (size_t)b * g.n_l * g.n_r : nullptr;
         const double c2in = Epi::TWO_IN ? epi.in2_coef() : 0.0;
@@ -112,6 +113,7 @@ __global__ void __launch_bounds__(256, Epi::MINB) tile_kernel(GridDev g, Epi epi
                     }
                 }
                 if (Epi::SCALED) { v.x *= sc; v.y *= sc; }
+                if (cut_tile && held_pt(g, l, j)) v = make_double2(0.0, 0.0);      // P H P: held points read as zero
                 tile[i] = v;
             }
         }
@@ -140,6 +142,7 @@ __global__ void __launch_bounds__(256, Epi::MINB) tile_kernel(GridDev g, Epi epi
                 const double cp = __ldg(g.cl + l);
                 double2 h = h_point<FD>(g, d, VG ? 0.0 : er, cm, cp, f, fm1, fp1, fm2, fp2, lo, up);
                 if (VG) vg_couple<FD>(g, c, T::PITCH, l, rinv, cm, cp, afield, lo, up, h);
+                if (cut_tile && held_pt(g, l, j)) h = make_double2(0.0, 0.0);    // ... and come out as zero
                 const size_t idx = ((size_t)b * g.n_l + l) * g.n_r + j;
                 epi.point(b, l, j, idx, f, h, red);
                 lo = f; f = up;
@@ -483,6 +486,15 @@ struct OpBoundPop : OpBase {
         }
     }
     __device__ __forceinline__ void finish_member(int b, const double *s) { out[b] = dr * s[0]; }
+};
+
+// psi <- P psi: zero the points the centrifugal cut-off holds (tdse_set_cutoff, tdse_set_state)
+struct OpProject : OpBase {
+    double2 *psi; const int *j0; int n_r, n_l;
+    __device__ __forceinline__ void point(int, size_t idx, double *) {
+        const int j = (int)(idx % (size_t)n_r), l = (int)((idx / (size_t)n_r) % (size_t)n_l);
+        if (j < __ldg(j0 + l)) psi[idx] = make_double2(0.0, 0.0);
+    }
 };
 
 struct OpCopy : OpBase {

@@ -48,6 +48,8 @@ struct RpSmem {
     double2 zrow[CP][32];                   // zeros for ever: the rows above l = 0 and below the last row group
     double rowtab[NWR * kRpRows][4];        // {c_l, l(l+1), c_{l-1}, 0}
     double2 psi_s[RK ? kRpRows * CP : 1][NWR * NWC * 32];   // RK4: psi(t_n) of every thread's patch (private slots)
+    double red[NWR * NWC][kRpObsRed];       // fused observables: per-warp partial sums
+    int last_flag;
 };
 
 __device__ __forceinline__ double2 shfl_up2(double2 v) {
@@ -86,11 +88,13 @@ __device__ __forceinline__ int rp_start(int t, int W, int H, int N, int WT) {
 // of 272 for one kernel per stage.
 // MODE: 0 Taylor in real time, 1 classic RK4 (above), 2 Taylor in IMAGINARY time (-i -> 1, weights
 // (-dt c1)^k / k!; the caller re-normalises).
-template <int FD, int CP, int NWR, int NWC, bool MASK, int MINB, bool TMA, bool CLUSTER, int MODE = 0>
+// OBS: the observable sums of the row logged after this step are reduced in the store phase (RpObs above).
+template <int FD, int CP, int NWR, int NWC, bool MASK, int MINB, bool TMA, bool CLUSTER, int MODE = 0, bool OBS = false>
 __global__ void __launch_bounds__(NWR * NWC * 32, MINB)
 taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict__ out, const double *__restrict__ ef,
                  const double *__restrict__ dtp, int order, int W, int H, int n_tiles, int n_items,
-                 const __grid_constant__ CUtensorMap tmap) {
+                 const __grid_constant__ CUtensorMap tmap, const RpObs ob) {
+    static_assert(!(OBS && (MASK || MODE == 2)), "fused observables: full tiles, real-time propagation");
     static_assert(!(TMA && MASK), "the TMA path needs a full tile");
     static_assert(NWC > 1 || CP == 4, "one-warp-wide tiles use the edge-weight trick, which needs 4-column patches");
     using G = RpGeom<FD, CP, NWR, NWC>;
@@ -123,6 +127,17 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
     __syncthreads();
 
     const double dt = *dtp;
+    // fused observables: is the step this launch takes a logged one, which row, at what time (uniform over the grid)
+    bool obs_now = false;
+    long long obs_row = 0;
+    double obs_t = 0.0;
+    if (OBS) {
+        const long long n = ob.ctl->step_base + ob.step_off + 1;
+        const int every = ob.ctl->obs_every;
+        obs_now = every > 0 && (n % every) == 0;
+        obs_row = obs_now ? n / every - 1 : 0;
+        obs_t = time_at(ob.ctl->t0, (double)n, ob.ctl->dt);
+    }
     const double inv_c1 = 1.0 / g.c1;
     const double kappa = dt * g.c1;                 // u'_k = (H/c1)^k psi  ->  weight (dt c1)^k / k!
     const double c2p = g.c2 * inv_c1;               // 5-point: second off-diagonal weight / c1 (= -1/16)
@@ -220,6 +235,16 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                 for (int q = 0; q < CP; ++q) T[r][q] = z2;
             }
         }
+        }
+        // ---- centrifugal cut-off (tdse_set_cutoff): the held points of this patch read as zero and stay zero ---------
+        const bool cut_item = g.j0 != nullptr && start < g.j0_max;       // (uniform over the CTA)
+        unsigned held_bits = 0u;
+        if (cut_item) {
+#pragma unroll
+            for (int r = 0; r < RP; ++r)
+#pragma unroll
+                for (int q = 0; q < CP; ++q)
+                    if (held_pt(g, gr0 + r, start + c0 + q)) { held_bits |= 1u << (r * CP + q); T[r][q] = z2; }
         }
         // ---- per-column coefficients (scaled by 1/c1): reloaded only when the radial tile changes ----------------
         if (t != t_cur) {
@@ -323,6 +348,11 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                 else if (first) { A[r][q].x = fma(s, hx, f.x); A[r][q].y = fma(s, hy, f.y); }
                 else if (odd) { A[r][q].x = fma(s, hy, A[r][q].x); A[r][q].y = fma(-s, hx, A[r][q].y); }
                 else { A[r][q].x = fma(s, hx, A[r][q].x); A[r][q].y = fma(s, hy, A[r][q].y); }
+            }
+            if (cut_item) {     // P H P: the new term (stage vector) vanishes at the held points (A is cleared at the end)
+#pragma unroll
+                for (int q = 0; q < CP; ++q)
+                    if ((held_bits >> (r * CP + q)) & 1u) To[r][q] = z2;
             }
         };
 
@@ -432,6 +462,13 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
             }
         }
         // the barrier signalled by the last order is waited for before the next item publishes (or at the end)
+        if (cut_item) {
+#pragma unroll
+            for (int r = 0; r < RP; ++r)
+#pragma unroll
+                for (int q = 0; q < CP; ++q)
+                    if ((held_bits >> (r * CP + q)) & 1u) A[r][q] = z2;
+        }
 
         // ---- psi(t + dt): interior columns of the tile straight from registers ---------------------------------
         {
@@ -453,6 +490,81 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
             for (int q = 0; q < CP; ++q) in_c[q] = c0 + q >= lo_c && c0 + q < lo_c + wint;
 #pragma unroll
             for (int r = 0; r < RP; ++r) row_ok[r] = !ragged_rows || gr0 + r < L;
+            // (the fused observables come BEFORE the stores: the release fences of their exchange would otherwise wait
+            // for the stores to drain)
+            if (OBS && obs_now) {
+                // row l-1 of psi(t + dt) for this thread's row 0: one more exchange through the buffer of the order loop
+                if (armed) bar_wait();
+#pragma unroll
+                for (int q = 0; q < CP; ++q) sm.xch[0][warp][1][q][lane] = A[RP - 1][q];
+                bar_arrive();
+                double red[kRpObsRed];
+#pragma unroll
+                for (int i = 0; i < kRpObsRed; ++i) red[i] = 0.0;
+                // the sums that need nothing from other warps are formed between arrive and wait
+                double szc[CP];
+#pragma unroll
+                for (int q = 0; q < CP; ++q) {
+                    double nn = 0.0, sz = 0.0;
+#pragma unroll
+                    for (int r = 0; r < RP; ++r) {
+                        const double2 a = A[r][q];
+                        if (row_ok[r]) nn += a.x * a.x + a.y * a.y;
+                        if (r > 0 && row_ok[r]) {
+                            const double2 pv = A[r > 0 ? r - 1 : 0][q];
+                            sz = fma(sm.rowtab[r0 + r][2], pv.x * a.x + pv.y * a.y, sz);     // c_{l-1} Re(conj f_{l-1} f_l)
+                        }
+                    }
+                    szc[q] = sz;
+                    if (in_c[q]) red[0] += nn;
+                }
+                bar_wait();
+                const double c_lo = sm.rowtab[r0][2];
+#pragma unroll
+                for (int q = 0; q < CP; ++q) {
+                    double2 lo;
+                    if (CLUSTER && lo_remote) lo = ld_dsmem2(lo_dsm + (unsigned)(q * 32 * sizeof(double2)));
+                    else lo = lo_base[q * 32];
+                    const double sz = fma(c_lo, lo.x * A[0][q].x + lo.y * A[0][q].y, szc[q]);
+                    if (in_c[q]) {
+                        const double rj = g.dr * (double)(start + c0 + q + 1);
+                        red[1] = fma(rj, sz, red[1]);
+                        red[2] += sz / (rj * rj);
+                    }
+                }
+                bar_arrive();                   // (waited for before the next item publishes into the buffer)
+#pragma unroll
+                for (int si = 0; si < kRpObsStates; ++si) {          // (compile-time indices: red[] stays in registers)
+                    if (si >= ob.n_states) continue;
+                    const int lr = __ldg(ob.l_of_state + si) - gr0;
+                    if (lr < 0 || lr >= RP) continue;
+#pragma unroll
+                    for (int q = 0; q < CP; ++q) {
+                        if (!in_c[q]) continue;
+                        const double w = __ldg(ob.phi + (size_t)si * N + start + c0 + q);
+                        double2 a = A[0][q];
+#pragma unroll
+                        for (int r = 1; r < RP; ++r) if (lr == r) a = A[r][q];
+                        red[3 + 2 * si] = fma(w, a.x, red[3 + 2 * si]);
+                        red[4 + 2 * si] = fma(w, a.y, red[4 + 2 * si]);
+                    }
+                }
+#pragma unroll
+                for (int i = 0; i < kRpObsRed; ++i) {
+#pragma unroll
+                    for (int off = 16; off > 0; off >>= 1) red[i] += __shfl_down_sync(0xffffffffu, red[i], off);
+                }
+                if (lane == 0) {
+#pragma unroll
+                    for (int i = 0; i < kRpObsRed; ++i) sm.red[warp][i] = red[i];
+                }
+                __syncthreads();
+                if (threadIdx.x < kRpObsRed) {
+                    double v = 0.0;
+                    for (int w2 = 0; w2 < NWR * NWC; ++w2) v += sm.red[w2][threadIdx.x];
+                    ob.partials[((size_t)item * csize + crank) * kRpObsRed + threadIdx.x] = v;
+                }
+            }
             double2 *prow[RP];
 #pragma unroll
             for (int r = 0; r < RP; ++r) prow[r] = dst_g + (size_t)r * N;
@@ -475,6 +587,69 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
         ef_cur = ef_next;
     }
     if (armed) bar_wait();     // (cluster: no CTA may exit while a neighbour can still read its shared memory)
+    if (OBS && obs_now) {
+        // the last CTA to sign off adds the partials of every member in a fixed order and writes the row
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            __threadfence();
+            const unsigned int ticket = atomicAdd(ob.counter, 1u);
+            sm.last_flag = (ticket == gridDim.x - 1);
+        }
+        __syncthreads();
+        if (!sm.last_flag) return;
+        __threadfence();
+        const int per = n_tiles * csize, Wd = 3 + ob.n_states;
+        constexpr int NW = NWR * NWC;
+        auto write_row = [&](const int bb, const double (&s)[kRpObsRed]) {
+            double *o = ob.rows + ((size_t)obs_row * g.batch + bb) * Wd;
+            o[0] = g.dr * s[0];
+            o[1] = 2.0 * g.dr * s[1];
+            o[2] = -pulse_E(ob.pulse[bb], obs_t) - 2.0 * g.z * g.dr * s[2];
+            for (int si = 0; si < ob.n_states && si < kRpObsStates; ++si) {
+                const double ar = g.dr * s[3 + 2 * si], ai = g.dr * s[4 + 2 * si];
+                o[3 + si] = ar * ar + ai * ai;
+            }
+        };
+        // many members: one warp per member; few members (a single wavefunction): the whole CTA per member
+        const bool by_warp = g.batch >= NW;
+        for (int bb = by_warp ? warp : 0; bb < g.batch; bb += by_warp ? NW : 1) {
+            double s[kRpObsRed];
+#pragma unroll
+            for (int i = 0; i < kRpObsRed; ++i) s[i] = 0.0;
+            const double *pp = ob.partials + (size_t)bb * per * kRpObsRed;
+            const int first = by_warp ? lane : (int)threadIdx.x, stride = by_warp ? 32 : G::NT;
+#pragma unroll 4
+            for (int i = first; i < per; i += stride) {
+#pragma unroll
+                for (int j = 0; j < kRpObsRed; ++j) s[j] += __ldcg(pp + (size_t)i * kRpObsRed + j);
+            }
+#pragma unroll
+            for (int j = 0; j < kRpObsRed; ++j) {
+#pragma unroll
+                for (int off = 16; off > 0; off >>= 1) s[j] += __shfl_down_sync(0xffffffffu, s[j], off);
+            }
+            if (by_warp) {
+                if (lane == 0) write_row(bb, s);
+            } else {
+                __syncthreads();
+                if (lane == 0) {
+#pragma unroll
+                    for (int j = 0; j < kRpObsRed; ++j) sm.red[warp][j] = s[j];
+                }
+                __syncthreads();
+                if (threadIdx.x == 0) {
+#pragma unroll
+                    for (int j = 0; j < kRpObsRed; ++j) {
+                        double v = 0.0;
+                        for (int w2 = 0; w2 < NW; ++w2) v += sm.red[w2][j];
+                        s[j] = v;
+                    }
+                    write_row(bb, s);
+                }
+            }
+        }
+        if (threadIdx.x == 0) *ob.counter = 0u;
+    }
 }
 
 // ------------------------------------------------------------------------------------------------------
@@ -494,7 +669,7 @@ inline int rp_init_tables() {
 template <class K>
 inline int rp_launch_kernel(K kern, DeviceOnce *once, int smem, const RpPlan &p, cudaStream_t s, const GridDev &g,
                             const double2 *in, double2 *out, const double *ef, const double *dtp, int order,
-                            const CUtensorMap &tm) {
+                            const CUtensorMap &tm, const RpObs &ob) {
     if (once->first()) {
         if (cudaFuncSetAttribute((const void *)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
             return TDSE_ERR_CUDA;
@@ -505,66 +680,64 @@ inline int rp_launch_kernel(K kern, DeviceOnce *once, int smem, const RpPlan &p,
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = p.cl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.attrs = at; cfg.numAttrs = (p.cl > 1) ? 1 : 0;
-    return cudaLaunchKernelEx(&cfg, kern, g, in, out, ef, dtp, order, p.W, p.H, p.n_tiles, p.n_items, tm) == cudaSuccess
+    return cudaLaunchKernelEx(&cfg, kern, g, in, out, ef, dtp, order, p.W, p.H, p.n_tiles, p.n_items, tm, ob) == cudaSuccess
                ? TDSE_OK : TDSE_ERR_CUDA;
 }
 
-// MODE 1 / 2 instantiations exist only for the one-warp-wide variants (RKABLE) and full tiles
-template <int FD, int CP, int NWR, int NWC, int MINB, bool CLUSTERABLE, bool RKABLE, int MODE>
-inline int rp_launch_mode(const GridDev &g, const RpPlan &p, bool mask, const CUtensorMap *tm, const double2 *in,
-                          double2 *out, const double *ef, const double *dtp, int order, cudaStream_t s) {
-    if (!RKABLE || mask) return TDSE_ERR_UNSUPPORTED;
-    constexpr int kM = RKABLE ? MODE : 0;
-    constexpr bool kCl = CLUSTERABLE && RKABLE, kT = RKABLE;
+// the four full-tile instantiations (direct / TMA) x (CTA / cluster) of one (MODE, OBS) pair
+template <int FD, int CP, int NWR, int NWC, int MINB, bool CLUSTERABLE, int MODE, bool OBS>
+inline int rp_launch_full(const GridDev &g, const RpPlan &p, const CUtensorMap &tm, const double2 *in, double2 *out,
+                          const double *ef, const double *dtp, int order, cudaStream_t s, const RpObs &ob) {
     static DeviceOnce once[4];
-    const int sm_t = (int)sizeof(RpSmem<FD, CP, NWR, NWC, kT, kM == 1>), sm_n = (int)sizeof(RpSmem<FD, CP, NWR, NWC, false, kM == 1>);
+    constexpr bool RK = (MODE == 1);
+    const int sm_t = (int)sizeof(RpSmem<FD, CP, NWR, NWC, true, RK>), sm_n = (int)sizeof(RpSmem<FD, CP, NWR, NWC, false, RK>);
     if (p.cl > 1) {
-        if (!kCl) return TDSE_ERR_UNSUPPORTED;
-        if (p.tma) return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, kT, kCl, kM>, &once[3], sm_t, p, s, g, in, out, ef, dtp, order, *tm);
-        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, kCl, kM>, &once[2], sm_n, p, s, g, in, out, ef, dtp, order, *tm);
+        if (!CLUSTERABLE) return TDSE_ERR_UNSUPPORTED;
+        constexpr bool kCl = CLUSTERABLE;
+        if (p.tma) return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, true, kCl, MODE, OBS>, &once[3], sm_t, p, s, g, in, out, ef, dtp, order, tm, ob);
+        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, kCl, MODE, OBS>, &once[2], sm_n, p, s, g, in, out, ef, dtp, order, tm, ob);
     }
-    if (p.tma) return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, kT, false, kM>, &once[1], sm_t, p, s, g, in, out, ef, dtp, order, *tm);
-    return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, false, kM>, &once[0], sm_n, p, s, g, in, out, ef, dtp, order, *tm);
+    if (p.tma) return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, true, false, MODE, OBS>, &once[1], sm_t, p, s, g, in, out, ef, dtp, order, tm, ob);
+    return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, false, MODE, OBS>, &once[0], sm_n, p, s, g, in, out, ef, dtp, order, tm, ob);
 }
 
+// MODE 1 / 2 instantiations exist only for the one-warp-wide variants (RKABLE) and full tiles; fused observables (ob)
+// for full tiles in real time (MODE 0 / 1)
 template <int FD, int CP, int NWR, int NWC, int MINB, bool CLUSTERABLE, bool RKABLE>
 inline int rp_launch_one(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
-                         const double *dtp, int order, cudaStream_t s) {
+                         const double *dtp, int order, cudaStream_t s, const RpObs *ob) {
     const bool mask = g.n_r < 32 * CP * NWC;
-    static DeviceOnce once[5];
     CUtensorMap tmap{};
     if (p.tma) {
         if (mask) return TDSE_ERR_UNSUPPORTED;
         if (!tma_map_rows3d(&tmap, in, g.n_r, g.batch * g.n_l, kRpRows * NWR, 32 * CP * NWC)) return TDSE_ERR_CUDA;
     }
-    const CUtensorMap *tm = &tmap;
-    if (p.rk == 1) return rp_launch_mode<FD, CP, NWR, NWC, MINB, CLUSTERABLE, RKABLE, 1>(g, p, mask, tm, in, out, ef, dtp, order, s);
-    if (p.rk == 2) return rp_launch_mode<FD, CP, NWR, NWC, MINB, CLUSTERABLE, RKABLE, 2>(g, p, mask, tm, in, out, ef, dtp, order, s);
-    if (p.cl > 1) {
-        if (!CLUSTERABLE || mask) return TDSE_ERR_UNSUPPORTED;
-        constexpr bool kCl = CLUSTERABLE;
-        if (p.tma)
-            return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, true, kCl>, &once[3],
-                                    (int)sizeof(RpSmem<FD, CP, NWR, NWC, true>), p, s, g, in, out, ef, dtp, order, *tm);
-        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, kCl>, &once[4],
-                                (int)sizeof(RpSmem<FD, CP, NWR, NWC, false>), p, s, g, in, out, ef, dtp, order, *tm);
+    const RpObs none{};
+    if (mask) {
+        if (p.rk != 0 || p.cl > 1 || ob) return TDSE_ERR_UNSUPPORTED;
+        static DeviceOnce once;
+        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, true, MINB, false, false>, &once,
+                                (int)sizeof(RpSmem<FD, CP, NWR, NWC, false>), p, s, g, in, out, ef, dtp, order, tmap, none);
     }
-    if (p.tma)
-        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, true, false>, &once[2],
-                                (int)sizeof(RpSmem<FD, CP, NWR, NWC, true>), p, s, g, in, out, ef, dtp, order, *tm);
-    if (mask)
-        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, true, MINB, false, false>, &once[1],
-                                (int)sizeof(RpSmem<FD, CP, NWR, NWC, false>), p, s, g, in, out, ef, dtp, order, *tm);
-    return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, false>, &once[0],
-                            (int)sizeof(RpSmem<FD, CP, NWR, NWC, false>), p, s, g, in, out, ef, dtp, order, *tm);
+    if (p.rk == 2) {
+        if (!RKABLE || ob) return TDSE_ERR_UNSUPPORTED;
+        return rp_launch_full<FD, CP, NWR, NWC, MINB, CLUSTERABLE, RKABLE ? 2 : 0, false>(g, p, tmap, in, out, ef, dtp, order, s, none);
+    }
+    if (p.rk == 1) {
+        if (!RKABLE) return TDSE_ERR_UNSUPPORTED;
+        if (ob) return rp_launch_full<FD, CP, NWR, NWC, MINB, CLUSTERABLE, RKABLE ? 1 : 0, true>(g, p, tmap, in, out, ef, dtp, order, s, *ob);
+        return rp_launch_full<FD, CP, NWR, NWC, MINB, CLUSTERABLE, RKABLE ? 1 : 0, false>(g, p, tmap, in, out, ef, dtp, order, s, none);
+    }
+    if (ob) return rp_launch_full<FD, CP, NWR, NWC, MINB, CLUSTERABLE, 0, true>(g, p, tmap, in, out, ef, dtp, order, s, *ob);
+    return rp_launch_full<FD, CP, NWR, NWC, MINB, CLUSTERABLE, 0, false>(g, p, tmap, in, out, ef, dtp, order, s, none);
 }
 
 template <int FD>
 inline int launch_taylor_rp_fd(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
-                               const double *dtp, int order, cudaStream_t s) {
+                               const double *dtp, int order, cudaStream_t s, const RpObs *ob) {
     if (!p.ok) return TDSE_ERR_UNSUPPORTED;
 #define TDSE_RP_CASE(I, CP, NWR, NWC, MINB) \
-    case I: return rp_launch_one<FD, CP, NWR, NWC, MINB, rp_clusterable(I), rp_rk_capable(I)>(g, p, in, out, ef, dtp, order, s);
+    case I: return rp_launch_one<FD, CP, NWR, NWC, MINB, rp_clusterable(I), rp_rk_capable(I)>(g, p, in, out, ef, dtp, order, s, ob);
     switch (p.variant) {
         TDSE_RP_CASE(0, 4, 1, 1, 8)
         TDSE_RP_CASE(1, 4, 2, 1, 4)

@@ -85,18 +85,40 @@ inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant
     return best;
 }
 
+// Observables fused into the last pass of a step (row a6; P:371 column list, "not performed asynchronously"):
+// norm, the l / l+1 products of <z> (Eq. 34) and <z''> (Eq. 36) and up to kRpObsStates bound-state overlaps
+// (Eq. 25) are reduced from the registers that hold psi(t + dt); one partial per work item (and cluster rank), the
+// last CTA to finish adds them per member in a fixed order and writes the row.
+constexpr int kRpObsStates = 4;
+constexpr int kRpObsRed = 3 + 2 * kRpObsStates;
+struct RpObs {
+    const Ctl *ctl; const tdse_pulse *pulse;
+    const double *phi; const int *l_of_state; int n_states;
+    int step_off;                   // the step of the captured block this launch is
+    double *partials;               // [n_items * cluster size][kRpObsRed]
+    unsigned int *counter;          // zero before the launch; reset by the last CTA
+    double *rows;                   // [rows][batch][3 + n_states]
+};
+
+// can the plan reduce the observable row in its own store phase (full tiles, real time, few bound states)?
+inline bool rp_obs_capable(const RpPlan &p, const tdse_grid &g, int n_states) {
+    return p.ok && p.rk != 2 && g.n_r >= p.WT && n_states <= kRpObsStates;
+}
+// doubles of partial sums the fused observables need
+inline size_t rp_obs_partials(const RpPlan &p) { return (size_t)p.n_items * p.cl * kRpObsRed; }
+
 // defined in tdse_taylor_rp_fd3.cu / tdse_taylor_rp_fd5.cu
 int rp_init_fd3();          // uploads the 1/k table of that translation unit to the current device (tdse_create)
 int rp_init_fd5();
 int launch_taylor_rp_fd3(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
-                         const double *dtp, int order, cudaStream_t s);
+                         const double *dtp, int order, cudaStream_t s, const RpObs *ob);
 int launch_taylor_rp_fd5(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
-                         const double *dtp, int order, cudaStream_t s);
+                         const double *dtp, int order, cudaStream_t s, const RpObs *ob);
 
 inline int launch_taylor_rp(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
-                            const double *dtp, int order, cudaStream_t s) {
-    return g.fd == 3 ? launch_taylor_rp_fd3(g, p, in, out, ef, dtp, order, s)
-                     : launch_taylor_rp_fd5(g, p, in, out, ef, dtp, order, s);
+                            const double *dtp, int order, cudaStream_t s, const RpObs *ob = nullptr) {
+    return g.fd == 3 ? launch_taylor_rp_fd3(g, p, in, out, ef, dtp, order, s, ob)
+                     : launch_taylor_rp_fd5(g, p, in, out, ef, dtp, order, s, ob);
 }
 
 }  // namespace tdse

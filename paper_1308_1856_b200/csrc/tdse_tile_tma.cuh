@@ -62,6 +62,15 @@ tile_tma_kernel(GridDev g, Epi epi_in, const __grid_constant__ CUtensorMap tmap,
         const double vj = (j < g.n_r) ? __ldg(g.vj + j) : 0.0, cen = (j < g.n_r) ? __ldg(g.cen + j) : 0.0;
         mbar_wait(&bars[s], (phase >> s) & 1u);
         phase ^= 1u << s;
+        const bool cut_tile = g.j0 != nullptr && tr * kTtTW - kTtHalo < g.j0_max;       // the tile touches held points
+        if (cut_tile) {          // centrifugal cut-off: held points read as zero (P H P)
+            double2 *tile_s = st + (size_t)s * kTtRows * COLS;
+            for (int i = tid; i < kTtRows * COLS; i += 256) {
+                const int rr = i / COLS, cc = i - rr * COLS;
+                if (held_pt(g, tl * kTtTL - 1 + rr, tr * kTtTW - kTtHalo + cc)) tile_s[i] = make_double2(0.0, 0.0);
+            }
+            __syncthreads();
+        }
         if (j < g.n_r && epi.member_active(b)) {
             const double afield = epi.efield(b), rinv = 1.0 / (g.dr * (double)(j + 1));
             const double er = afield * (g.dr * (double)(j + 1));
@@ -82,6 +91,7 @@ tile_tma_kernel(GridDev g, Epi epi_in, const __grid_constant__ CUtensorMap tmap,
                 const double cp = __ldg(g.cl + l);
                 double2 h = h_point<FD>(g, d, VG ? 0.0 : er, cm, cp, f, fm1, fp1, fm2, fp2, lo, up);
                 if (VG) vg_couple<FD>(g, c, COLS, l, rinv, cm, cp, afield, lo, up, h);
+                if (cut_tile && held_pt(g, l, j)) h = make_double2(0.0, 0.0);
                 epi.point(b, l, j, ((size_t)b * g.n_l + l) * g.n_r + j, f, h, red);
                 lo = f; f = up;
             }
@@ -162,8 +172,15 @@ tile_tma3_kernel(GridDev g, Epi epi_in, RedCtx rc, const __grid_constant__ CUten
             const double vj = (jc < g.n_r) ? __ldg(g.vj + jc) : 0.0, cen = (jc < g.n_r) ? __ldg(g.cen + jc) : 0.0;
             mbar_wait(bar, phase);
             phase ^= 1u;
-            for (int i = tid; i < ELEMS; i += 256)
-                tile[i] = epi.combine(raw[i], has1 ? raw[ELEMS + i] : z2, has2 ? raw[2 * ELEMS + i] : z2);
+            const bool cut_tile = g.j0 != nullptr && tr * kTtTW - kTtHalo < g.j0_max;   // the tile touches held points
+            for (int i = tid; i < ELEMS; i += 256) {
+                double2 v = epi.combine(raw[i], has1 ? raw[ELEMS + i] : z2, has2 ? raw[2 * ELEMS + i] : z2);
+                if (cut_tile) {      // centrifugal cut-off: held points read as zero (P H P)
+                    const int rr = i / COLS, cc = i - rr * COLS;
+                    if (held_pt(g, tl * kTtTL - 1 + rr, tr * kTtTW - kTtHalo + cc)) v = z2;
+                }
+                tile[i] = v;
+            }
             __syncthreads();                               // tile complete, raw buffers consumed
             fetch(item + gridDim.x);
             const int j = tr * kTtTW + tx, l0 = tl * kTtTL;
@@ -187,6 +204,7 @@ tile_tma3_kernel(GridDev g, Epi epi_in, RedCtx rc, const __grid_constant__ CUten
                     const double cp = __ldg(g.cl + l);
                     double2 h = h_point<FD>(g, d, VG ? 0.0 : er, cm, cp, f, fm1, fp1, fm2, fp2, lo, up);
                     if (VG) vg_couple<FD>(g, c, COLS, l, rinv, cm, cp, afield, lo, up, h);
+                    if (cut_tile && held_pt(g, l, j)) h = z2;
                     epi.point(b, l, j, ((size_t)b * g.n_l + l) * g.n_r + j, f, h, red);
                     lo = f; f = up;
                 }

@@ -247,7 +247,8 @@ def test_taylor_register_patch_parity(B, case, tma):
     dt = wl.dt_eff(c, "taylor", order)
     t0 = wl.window(c, nsteps, dt)
     psi0 = wl.populated_state(c)
-    opts = {"taylor_block": 1, "use_graph": use_graph, "taylor_rp_variant": variant, "taylor_rp_tma": tma}
+    opts = {"taylor_block": 1, "use_graph": use_graph, "taylor_rp_variant": variant, "taylor_rp_tma": tma,
+            "obs_fused": 2 if tma else 0}        # logged rows: reduced in the step kernel / by the observable kernels
     h, got, ref, gobs, robs = run_pair_fixed(B, c, "taylor", nsteps, psi0, t0, dt, obs_every, [(0, 0)], opts, order=order)
     tma_applies = bool(tma) and n_r % 8 == 0 and n_r > (256 if variant == 4 else 128)
     assert h.taylor_kernel() == (4 if tma_applies else 3)
@@ -321,7 +322,7 @@ def test_rk4_parity(B, case, fused):
     t0 = wl.window(c, nsteps, dt)
     psi0 = wl.populated_state(c)
     h, got, ref, gobs, robs = run_pair_fixed(B, c, "rk4", nsteps, psi0, t0, dt, obs_every, [(0, 0)],
-                                             {"use_graph": use_graph, "rk4_block": fused})
+                                             {"use_graph": use_graph, "rk4_block": fused, "obs_fused": 2})
     assert (h.taylor_kernel() in (3, 4)) == (bool(fused) and n_r >= 128)
     check_fixed(got, ref, gobs, robs)
     for b in range(batch):
@@ -887,3 +888,112 @@ def test_sanitizer_selection(B):
                 torch.cuda.synchronize()
                 assert rel_l2(y.cpu().numpy(), oracle.apply_H(g, wl.random_state(c), 0.05)) <= TOL_H
         h.close()
+
+
+# ------------------------------------------------------------------------------------------------- centrifugal cut-off
+CUTOFF_SHAPES = [(500, 8, 3, 1, 30.0), (328, 11, 5, 3, 8.0), (1304, 40, 5, 1, 5.0), (264, 128, 3, 1, 50.0), (37, 6, 3, 2, 20.0)]
+
+
+@pytest.mark.parametrize("shape", CUTOFF_SHAPES)
+def test_cutoff_apply_H_parity(B, shape):
+    """tdse_set_cutoff (extension): H psi is P H P of the oracle -- held inputs (non-zero here) read as
+    zero, held outputs are exactly zero -- through the register-staged and the TMA-fetched tile kernels; held regions of
+    up to several tiles."""
+    import torch
+    n_r, n_l, fd, batch, lam = shape
+    c = wl.config("cfg5" if batch > 1 else "cfg1", n_r=n_r, dr=0.1, n_l=n_l, fd_order=fd, batch=batch)
+    g = oracle.make_grid(n_r, 0.1, n_l, fd, batch=batch, cutoff_lambda=lam)
+    h = B.Tdse(n_r, 0.1, n_l, fd, batch=batch)
+    h.set_cutoff(lam)
+    held = oracle.held_mask(g)
+    assert held.sum() > 0
+    x = wl.random_state(c)
+    e = [0.05 + 0.01 * b for b in range(batch)]
+    ref = oracle.apply_H(g, x, e)
+    d_in = torch.from_numpy(x).cuda()
+    for tma in (2, 0):
+        h.set_option("apply_tma", tma)
+        d_out = torch.full_like(d_in, float("nan"))
+        h.apply_H(d_in, d_out, e)
+        torch.cuda.synchronize()
+        got = d_out.cpu().numpy()
+        assert rel_l2(got, ref) <= TOL_H
+        assert np.count_nonzero(got[:, held]) == 0
+    h.set_cutoff(0.0)                                   # removed again: the plain operator
+    h.apply_H(d_in, d_out, e)
+    torch.cuda.synchronize()
+    g0 = oracle.make_grid(n_r, 0.1, n_l, fd, batch=batch)
+    assert rel_l2(d_out.cpu().numpy(), oracle.apply_H(g0, x, e)) <= TOL_H
+    h.close()
+
+
+CUTOFF_STEPS = [
+    # propagator, n_r, n_l, fd, batch, lambda, options
+    ("taylor", 640, 16, 3, 2, 20.0, {}),                         # register-patch kernel, TMA
+    ("taylor", 333, 11, 5, 3, 8.0, {}),                          # direct loads, ragged rows
+    ("taylor", 304, 64, 5, 1, 3.0, {}),                          # cluster of 4; the held region spans two tiles
+    ("taylor", 640, 16, 3, 2, 20.0, {"taylor_block": 0}),        # one kernel per order
+    ("taylor", 100, 5, 3, 1, 20.0, {}),                          # masked single tile
+    ("rk4", 640, 9, 5, 2, 10.0, {}),                             # fused RK4
+    ("rk4", 640, 9, 3, 1, 10.0, {"rk4_block": 0}),               # one kernel per stage
+    ("lanczos", 424, 12, 3, 2, 10.0, {}),                        # TMA-fetched sources
+    ("lanczos", 420, 12, 5, 1, 10.0, {}),                        # register-staged pass
+    ("merson", 333, 7, 5, 2, 10.0, {}),                          # generic RK stage loop
+    ("rk45", 500, 8, 5, 1, 10.0, {}),                            # adaptive controller
+]
+
+
+@pytest.mark.parametrize("case", CUTOFF_STEPS)
+def test_cutoff_propagators_parity(B, case):
+    """Every propagator with the centrifugal cut-off against the oracle's P H P propagation, from a state that is
+    non-zero at the held points (tdse_set_state projects it), at the larger step the cut-off allows, with observables."""
+    prop, n_r, n_l, fd, batch, lam, opts = case
+    c = wl.config("cfg5" if batch > 1 else "cfg1", n_r=n_r, dr=0.1, n_l=n_l, fd_order=fd, batch=batch, order=4,
+                  cutoff_lambda=lam)
+    g = oracle.make_grid(n_r, 0.1, n_l, fd, batch=batch, cutoff_lambda=lam)
+    g0 = oracle.make_grid(n_r, 0.1, n_l, fd, batch=batch)
+    h = B.Tdse(n_r, 0.1, n_l, fd, batch=batch)
+    for k, v in opts.items():
+        h.set_option(k, v)
+    h.set_cutoff(lam)
+    pulses = wl.pulses(c)
+    h.set_pulse(pulses)
+    st = bound_pack(g0, [(0, 0), (1, 0)])
+    h.set_bound_states(*st)
+    psi0 = wl.populated_state(c)
+    held = oracle.held_mask(g)
+    assert np.count_nonzero(psi0[:, held]) > 0
+    h.set_state(psi0)
+    assert rel_l2(h.get_state(), oracle.project(g, psi0)) == 0.0
+    t0, n = 0.5 * c["t_pulse"], 21
+    if prop == "taylor":
+        dt = wl.dt_eff(c, "taylor", 4)
+        assert dt > 2.0 * wl.dt_eff(dict(c, cutoff_lambda=0.0), "taylor", 4) or n_l < 8      # the step the cut-off buys
+        h.step_taylor(4, t0, dt, n, 3)
+        ref, robs = oracle.step_taylor(g, pulses, psi0, 4, t0, dt, n, states=st, obs_every=3)
+    elif prop == "rk4":
+        dt = wl.dt_eff(c, "rk4", 4)
+        h.step_rk4(t0, dt, n, 3)
+        ref, robs = oracle.step_rk4(g, pulses, psi0, t0, dt, n, states=st, obs_every=3)
+    elif prop == "lanczos":
+        dt = wl.dt_eff(c, "lanczos", 12)
+        h.step_lanczos(8, 12, t0, dt, n, 3)
+        ref, robs = oracle.step_lanczos(g, pulses, psi0, 8, 12, t0, dt, n, states=st, obs_every=3)
+    elif prop == "merson":
+        dt = 0.5 * wl.dt_eff(c, "rk4", 4)
+        h.step_rk("merson", t0, dt, n, 3)
+        ref, _, robs = oracle.step_rk_method(g, pulses, psi0, "merson", t0, dt, n, states=st, obs_every=3)
+    else:
+        info = h.step_rk45(t0, t0 + 0.05, 1e-3, 1e-8)
+        ref, rinfo = oracle.step_rk45(g, pulses, psi0, t0, t0 + 0.05, 1e-3, 1e-8, dt_replay=info["dt"])
+        assert info["n_accept"] > 5 and np.max(rinfo["err"]) <= 1.05
+        robs = None
+    got = h.get_state()
+    assert np.count_nonzero(got[:, held]) == 0
+    if robs is not None:
+        check_fixed(got, ref, h.obs_log(), robs)
+    else:
+        assert rel_l2(got, ref) <= TOL_PSI
+    for l in range(n_l):
+        assert np.linalg.norm(got[:, l] - ref[:, l]) <= TOL_PSI * max(np.linalg.norm(ref[:, l]), 1e-3)
+    h.close()
