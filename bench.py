@@ -369,7 +369,7 @@ def run_own(args):
             "gpu_launches": int(launches), "graphs_instantiated_in_timed_region": 0, "max_norm_drift": norm_dev}
 
     if rank == 0 and not args.no_extra and world == 1:
-        line["extra"] = extra_measurements(binding, torch, stream)
+        line["extra"] = extra_measurements(binding, torch, stream, full_pulse=not args.no_full_pulse)
     if rank == 0 and world == 1 and not args.no_cpu:
         line["cpu_baseline"] = cpu_baseline(c, order, dt, t0)
     h.close()
@@ -389,7 +389,7 @@ def timed(torch, stream, fn, reps=1):
     return e0.elapsed_time(e1) / reps
 
 
-def extra_measurements(binding, torch, stream):
+def extra_measurements(binding, torch, stream, full_pulse=True):
     """Secondary figures (not the headline): bare H.psi, s/step of the other configs, the claim "HBM-bound for small
     orders" tested (Taylor-2 / Taylor-4 on the CFG5 grid) and the roofline sweep of SURVEY section 8(d) S1."""
     out = {}
@@ -483,7 +483,45 @@ def extra_measurements(binding, torch, stream):
                                  "timing": "CUDA events around the call (includes the controller's host checks)"}
         h.close()
         out["sweep"] = roofline_sweep(binding, torch, stream, peak)
+        if full_pulse:
+            out["cfg3_full_pulse"] = cfg3_full_pulse(binding, torch, stream)
     return out
+
+
+def cfg3_full_pulse(binding, torch, stream, lam=300.0):
+    """CFG3 end to end: hydrogen from the (analytic) 1s state through the WHOLE 10-cycle 800 nm pulse at 2e14 W/cm^2,
+    Taylor order 10, with the dipole-acceleration expectation logged EVERY step (BASELINE.json configs[2]: "an HHG-shaped
+    output").  Feasible only with the centrifugal inner cut-off (an extension beyond the paper, tdse_set_cutoff): at
+    Lambda = 300 au the stable step is about 1.4e-3 au (7.9e5 steps) instead of 4.9e-6 (2.2e8 steps)."""
+    c = wl.config("cfg3", cutoff_lambda=lam)
+    dt = wl.dt_eff(c)
+    nsteps = int(round(c["t_pulse"] / dt))
+    h = binding.Tdse(c["n_r"], c["dr"], c["n_l"], c["fd_order"])
+    h.set_cutoff(lam)
+    h.set_pulse(wl.pulses(c))
+    h.set_state(wl.ground_state(c), stream=stream)
+    h.step_taylor(c["order"], 0.0, dt, 64, 1, stream=stream)            # graphs captured before the timed run
+    h.set_state(wl.ground_state(c), stream=stream)
+    stream.synchronize()
+    tw = time.perf_counter()
+    ms = timed(torch, stream, lambda: h.step_taylor(c["order"], 0.0, dt, nsteps, 1, stream=stream))
+    rows = h.obs_log()
+    wall = time.perf_counter() - tw
+    acc = rows[:, 0, 2]
+    # harmonic content of <z''>(t): power in windows around odd and even multiples of omega (P:305: odd harmonics only)
+    spec = np.abs(np.fft.rfft(acc * np.hanning(len(acc)))) ** 2
+    freq = 2.0 * np.pi * np.fft.rfftfreq(len(acc), d=dt) / c["omega"]
+    def band(k):
+        m = (freq > k - 0.25) & (freq < k + 0.25)
+        return float(spec[m].sum())
+    odd, even = sum(band(k) for k in (3, 5, 7, 9)), sum(band(k) for k in (4, 6, 8, 10))
+    h.close()
+    return {"cutoff_lambda": lam, "dt": dt, "steps": nsteps, "wall_s": wall, "device_s": ms * 1e-3,
+            "us_per_step_with_row": ms * 1e3 / nsteps, "rows_logged": int(rows.shape[0]),
+            "max_norm_drift": float(np.max(np.abs(rows[:, 0, 0] - 1.0))),
+            "max_abs_accel": float(np.max(np.abs(acc))), "final_dipole": float(rows[-1, 0, 1]),
+            "odd_over_even_harmonic_power_3_to_10": odd / max(even, 1e-300),
+            "note": "extension beyond the paper (centrifugal inner cut-off); the un-cut operator needs 2.2e8 steps"}
 
 
 def roofline_sweep(binding, torch, stream, peak):
@@ -543,6 +581,7 @@ def main():
     ap.add_argument("--rp-tma", type=int, default=-1, help="register-patch kernel: -1 auto, 0 direct loads, 1 TMA")
     ap.add_argument("--no-extra", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-full-pulse", action="store_true", help="skip the 8e5-step CFG3 run of `extra` (about 70 s)")
     args = ap.parse_args()
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         respawn_under_torchrun(args.gpus)

@@ -83,6 +83,10 @@ void tdse_destroy(tdse_handle *h);
  *   "taylor_rp_variant" [-1] instantiation of the register-patch kernel (-1: heuristic)
  *   "taylor_rp_tma"    [-1] register-patch kernel: fetch tiles by TMA tensor copies (-1: heuristic, 0: never,
  *                          1: whenever n_r % 8 == 0 and the grid is wider than a tile)
+ *   "persist"          [8] tdse_step_taylor on SMALL grids (at most one wave of CTAs; no cut-off; logged rows, if any,
+ *                          fusable: at most 4 bound states): temporal blocking across steps -- the halo of a tile covers
+ *                          up to this many steps, so one launch takes that many steps with psi in registers (halved
+ *                          until the interior of a tile is at least half of it); 0 / 1: one launch per step
  *   "obs_fused"        [1] logged observable rows are reduced inside the register-patch step kernel (from the registers
  *                          that hold psi(t + dt); no extra pass over psi) when it runs on full tiles, at most 4 bound
  *                          states are set and the grid is at most 16 CTAs (beyond that the separate pass measured

@@ -114,6 +114,7 @@ struct tdse_handle {
     double *d_obs_partials = nullptr; int *d_loff = nullptr, *d_slist = nullptr; unsigned int *d_obs_counters = nullptr;
     double *d_yield = nullptr;
     double *d_rp_part = nullptr; size_t rp_part_cap = 0; unsigned int *d_rp_counter = nullptr;   // fused observables
+    int persist = 8;                        // option: up to this many steps per launch on small grids (0 / 1: one)
     int obs_fused = 1;                      // option: reduce the logged rows in the step kernel when it can
     double *d_rows = nullptr; size_t rows_cap = 0; long log_rows = 0; double *d_row_direct = nullptr;
     // rk45 logs
@@ -283,8 +284,8 @@ int enqueue_imag_norm(tdse_handle *h, double2 *psi, int step_off, cudaStream_t s
 // obs_kernel over an L2-resident CFG3 state), so obs_fused = 1 (auto) uses it for grids of at most 16 CTAs and
 // obs_fused = 2 forces it wherever the kernel can do it.
 bool obs_fused_wanted(const tdse_handle *h) {
-    if (!h->obs_fused || !rp_obs_capable(h->rpp, h->grid, h->n_states)) return false;
-    return h->obs_fused == 2 || (long)h->rpp.n_items * h->rpp.cl <= 16;
+    if (!h->obs_fused || h->d_j0 || !rp_obs_capable(h->rpp, h->grid, h->n_states)) return false;   // (no fused rows with a cut-off)
+    return h->obs_fused == 2 || h->rpp.persist > 1 || (long)h->rpp.n_items * h->rpp.cl <= 16;
 }
 bool obs_fused_now(const tdse_handle *h, int obs) { return obs && h->d_rp_part && obs_fused_wanted(h); }
 RpObs make_rp_obs(const tdse_handle *h, int step_off) {
@@ -316,6 +317,27 @@ int enqueue_taylor_block(tdse_handle *h, int order, int n, int obs, cudaStream_t
     int sl[3], c = 0;
     for (int i = 0; c < 3; ++i) if (i != h->psi_slot) sl[c++] = i;
     double2 *ta = h->pool[sl[0]], *tb = h->pool[sl[1]], *acc = h->pool[sl[2]];
+    if (h->taylor_blocked_last && h->rpp.persist) {
+        // temporal blocking across steps: launches of up to rpp.persist steps, psi in registers in between
+        const bool fused = obs_fused_now(h, obs);
+        if (obs && !fused) return TDSE_ERR_UNSUPPORTED;         // (step_taylor_impl plans persist only when the rows can be fused)
+        double2 *src = psi, *dst = acc;
+        for (int i = 0; i < n; i += h->rpp.persist) {
+            const int k = std::min(h->rpp.persist, n - i);
+            const RpObs ro = make_rp_obs(h, i);
+            RC(launch_taylor_rp(h->gd, h->rpp, src, dst, h->d_etab + (size_t)i * B, &h->d_ctl->dt, order, s, fused ? &ro : nullptr, k));
+            count(h);
+            std::swap(src, dst);
+        }
+        if (src != psi) {                                       // odd number of launches: bring the state back
+            OpCopy cp{}; cp.dst = psi; cp.src = acc;
+            RC(launch_ew(h, cp, s));
+        }
+        ctl_advance_kernel<<<1, 32, 0, s>>>(h->d_ctl, n);
+        count(h);
+        CU(cudaGetLastError());
+        return TDSE_OK;
+    }
     for (int i = 0; i < n; ++i) {
         const double *ef = h->d_etab + (size_t)i * B;
         if (h->taylor_blocked_last) {
@@ -643,7 +665,7 @@ int run_blocks(tdse_handle *h, int kind, int p1, int p2, int n, int obs, long nb
         }
         return TDSE_OK;
     }
-    const auto key = std::make_tuple(kind, p1, p2, n, obs + 2 * h->taylor_blocked_last + 256 * (h->rpp.variant + 1) + 8192 * h->rpp.tma + 16384 * h->rk4_fused + 32768 * h->imag + 65536 * (int)obs_fused_now(h, obs), h->psi_slot);
+    const auto key = std::make_tuple(kind, p1, p2, n, obs + 2 * h->taylor_blocked_last + 256 * (h->rpp.variant + 1) + 8192 * h->rpp.tma + 16384 * h->rk4_fused + 32768 * h->imag + 65536 * (int)obs_fused_now(h, obs) + 131072 * h->rpp.persist + 16777216 * (h->rpp.H & 127), h->psi_slot);
     auto it = h->graphs.find(key);
     if (it == h->graphs.end()) {
         cudaGraph_t g = nullptr;
@@ -813,6 +835,7 @@ int tdse_set_option(tdse_handle *h, const char *key, double value) {
     else if (k == "apply_tma") { if (value < 0 || value > 2) return TDSE_ERR_ARG; h->apply_tma = (int)value; }
     else if (k == "lanczos_tma") { if (value < 0 || value > 1) return TDSE_ERR_ARG; h->lanczos_tma = (int)value; free_graphs(h); }
     else if (k == "obs_fused") { if (value != 0.0 && value != 1.0 && value != 2.0) return TDSE_ERR_ARG; h->obs_fused = (int)value; free_graphs(h); }
+    else if (k == "persist") { if (value < 0 || value > 64) return TDSE_ERR_ARG; h->persist = (int)value; free_graphs(h); }
     else if (k == "rk4_block") { if (value < 0 || value > 1) return TDSE_ERR_ARG; h->rk4_block = (int)value; free_graphs(h); }
     else if (k == "taylor_rp_tma") { if (value < -1 || value > 1) return TDSE_ERR_ARG; h->rp_tma = (int)value; free_graphs(h); }
     else if (k == "lanczos_beta_tol") { if (!(value >= 0.0)) return TDSE_ERR_ARG; h->beta_tol = value; free_graphs(h); }
@@ -984,9 +1007,19 @@ static int step_taylor_impl(tdse_handle *h, int order, double t0, double dt, lon
     h->rk4_fused = 0;
     h->rpp = RpPlan{};
     // (the all-orders-in-one-pass kernel implements the length-gauge coupling only; imaginary time has no field)
-    const bool lg = h->grid.gauge == 0 || h->imag;
+    const bool lg = (h->grid.gauge == 0 || h->imag) && !(h->imag && h->d_j0);      // (imaginary time with a cut-off: per order)
     if (lg && h->taylor_block == 1) {
-        h->rpp = rp_plan(h->grid, order, h->n_sm, h->rp_variant, h->rp_tma, h->imag ? 2 : 0);
+        // (persistent steps: real-time Taylor on grids one CTA per member can hold, logged rows fused or none)
+        // (several steps per launch: real-time Taylor on SMALL grids -- at most one wave of CTAs --, no cut-off, logged
+        // rows fusable or none; the deepest blocking that keeps the interior of a tile at least half of it)
+        h->rpp = RpPlan{};
+        const bool may_persist = h->persist > 1 && h->rp_tma != 1 && !h->imag && !h->d_j0 &&
+                                 (obs_every == 0 || (h->obs_fused && h->n_states <= kRpObsStates));
+        for (int k = may_persist ? h->persist : 0; k > 1 && !h->rpp.ok; k /= 2) {
+            RpPlan p = rp_plan(h->grid, order, h->n_sm, h->rp_variant, 0, 0, k);
+            if (p.ok && (long)p.n_items * p.cl <= h->n_sm) h->rpp = p;
+        }
+        if (!h->rpp.ok) h->rpp = rp_plan(h->grid, order, h->n_sm, h->rp_variant, h->rp_tma, h->imag ? 2 : 0);
         if (h->rpp.ok) h->taylor_blocked_last = 3;
     }
     return run_fixed(h, KIND_TAYLOR, order, 0, t0, dt, nsteps, obs_every, (cudaStream_t)stream);

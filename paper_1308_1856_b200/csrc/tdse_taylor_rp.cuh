@@ -89,12 +89,21 @@ __device__ __forceinline__ int rp_start(int t, int W, int H, int N, int WT) {
 // MODE: 0 Taylor in real time, 1 classic RK4 (above), 2 Taylor in IMAGINARY time (-i -> 1, weights
 // (-dt c1)^k / k!; the caller re-normalises).
 // OBS: the observable sums of the row logged after this step are reduced in the store phase (RpObs above).
-template <int FD, int CP, int NWR, int NWC, bool MASK, int MINB, bool TMA, bool CLUSTER, int MODE = 0, bool OBS = false>
+// PERSIST: temporal blocking ACROSS steps: the halo H covers n_steps x order x hw columns, so a tile can take n_steps
+// whole steps with psi in registers (field value ef[step * batch + b]; after each step the sum becomes the next input;
+// one observable partial per logged step) and touches HBM once per launch -- small grids are bound by the serial work of
+// a CTA instead of by one launch per step (NS: "so small grids are not launch-bound", hard part 4).
+// CUT: some points of the patch are HELD at zero (centrifugal inner cut-off g.j0; columns >= n_r of a grid narrower than
+// the tile): a separate instantiation, because the extra control flow costs the plain kernel its register allocation.
+template <int FD, int CP, int NWR, int NWC, bool MASK, int MINB, bool TMA, bool CLUSTER, int MODE = 0, bool OBS = false,
+          bool PERSIST = false, bool CUT = false>
 __global__ void __launch_bounds__(NWR * NWC * 32, MINB)
 taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict__ out, const double *__restrict__ ef,
                  const double *__restrict__ dtp, int order, int W, int H, int n_tiles, int n_items,
-                 const __grid_constant__ CUtensorMap tmap, const RpObs ob) {
-    static_assert(!(OBS && (MASK || MODE == 2)), "fused observables: full tiles, real-time propagation");
+                 const __grid_constant__ CUtensorMap tmap, const RpObs ob, int n_steps) {
+    static_assert(!(OBS && MODE == 2), "fused observables: real-time propagation");
+    static_assert(!(OBS && MASK), "fused observables: unmasked instantiations");
+    static_assert(!(PERSIST && (MASK || TMA || CLUSTER || MODE != 0)), "several steps per launch: full tiles, direct loads, Taylor");
     static_assert(!(TMA && MASK), "the TMA path needs a full tile");
     static_assert(NWC > 1 || CP == 4, "one-warp-wide tiles use the edge-weight trick, which needs 4-column patches");
     using G = RpGeom<FD, CP, NWR, NWC>;
@@ -113,7 +122,7 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
     const int r0 = wr * RP, c0 = (wc * 32 + lane) * CP;
     const int gr0 = rbase + r0;                                // global row of this thread's patch row 0
     const double2 z2 = make_double2(0.0, 0.0);
-    const bool al32 = !MASK && ((N & 1) == 0) && ((H & 1) == 0) && ((W & 1) == 0);
+    const bool al32 = !MASK && ((N & 1) == 0) && ((H & 1) == 0) && ((W & 1) == 0) && N >= WT;
     const bool ragged_rows = (csize * NWR * RP != L);
 
     for (int r = threadIdx.x; r < NWR * RP; r += G::NT) {
@@ -127,17 +136,33 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
     __syncthreads();
 
     const double dt = *dtp;
-    // fused observables: is the step this launch takes a logged one, which row, at what time (uniform over the grid)
+    // fused observables: is the step a logged one, which row, at what time (uniform over the grid)
     bool obs_now = false;
     long long obs_row = 0;
     double obs_t = 0.0;
-    if (OBS) {
-        const long long n = ob.ctl->step_base + ob.step_off + 1;
-        const int every = ob.ctl->obs_every;
-        obs_now = every > 0 && (n % every) == 0;
-        obs_row = obs_now ? n / every - 1 : 0;
-        obs_t = time_at(ob.ctl->t0, (double)n, ob.ctl->dt);
-    }
+    // (the control block is read once: its loads must not sit in front of every step of a multi-step launch)
+    const long long obs_base = OBS ? ob.ctl->step_base + ob.step_off + 1 : 0;
+    const int obs_every = OBS ? ob.ctl->obs_every : 0;
+    const double obs_t0 = OBS ? ob.ctl->t0 : 0.0, obs_dt = OBS ? ob.ctl->dt : 0.0;
+    auto obs_setup = [&](const int step) {
+        const long long n = obs_base + step;
+        obs_now = obs_every > 0 && (n % obs_every) == 0;
+        obs_row = obs_now ? n / obs_every - 1 : 0;
+        obs_t = time_at(obs_t0, (double)n, obs_dt);
+    };
+    if (OBS) obs_setup(0);
+    bool any_obs = obs_now;                                  // some step of this launch is a logged one
+    const bool obs_direct = (n_tiles * csize == 1);         // the CTA owns the whole member: it writes the row itself
+    auto write_row = [&](const int bb, const double (&s)[kRpObsRed]) {
+        double *o = ob.rows + ((size_t)obs_row * g.batch + bb) * (3 + ob.n_states);
+        o[0] = g.dr * s[0];
+        o[1] = 2.0 * g.dr * s[1];
+        o[2] = -pulse_E(ob.pulse[bb], obs_t) - 2.0 * g.z * g.dr * s[2];
+        for (int si = 0; si < ob.n_states && si < kRpObsStates; ++si) {
+            const double ar = g.dr * s[3 + 2 * si], ai = g.dr * s[4 + 2 * si];
+            o[3 + si] = ar * ar + ai * ai;
+        }
+    };
     const double inv_c1 = 1.0 / g.c1;
     const double kappa = dt * g.c1;                 // u'_k = (H/c1)^k psi  ->  weight (dt c1)^k / k!
     const double c2p = g.c2 * inv_c1;               // 5-point: second off-diagonal weight / c1 (= -1/16)
@@ -237,14 +262,16 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
         }
         }
         // ---- centrifugal cut-off (tdse_set_cutoff): the held points of this patch read as zero and stay zero ---------
-        const bool cut_item = g.j0 != nullptr && start < g.j0_max;       // (uniform over the CTA)
+        // (a grid narrower than the tile of an unmasked instantiation -- the persistent kernel -- holds its columns >= n_r
+        // at zero the same way)
+        const bool cut_item = CUT && ((g.j0 != nullptr && start < g.j0_max) || (!MASK && N < start + WT));   // (uniform over the CTA)
         unsigned held_bits = 0u;
         if (cut_item) {
 #pragma unroll
             for (int r = 0; r < RP; ++r)
 #pragma unroll
                 for (int q = 0; q < CP; ++q)
-                    if (held_pt(g, gr0 + r, start + c0 + q)) { held_bits |= 1u << (r * CP + q); T[r][q] = z2; }
+                    if (held_pt(g, gr0 + r, start + c0 + q) || start + c0 + q >= N) { held_bits |= 1u << (r * CP + q); T[r][q] = z2; }
         }
         // ---- per-column coefficients (scaled by 1/c1): reloaded only when the radial tile changes ----------------
         if (t != t_cur) {
@@ -253,7 +280,7 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
             for (int q = 0; q < CP; ++q) {
                 const int j = start + c0 + q;
                 dom[q] = !MASK || j < N;
-                const int jj = dom[q] ? j : 0;
+                const int jj = (dom[q] && j < N) ? j : 0;
                 Dq[q] = inv_c1 * __ldg(g.vj + jj);
                 Cq[q] = inv_c1 * __ldg(g.cen + jj);
             }
@@ -264,6 +291,26 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
 #pragma unroll
             for (int q = 0; q < CP; ++q) Eq[q] = es * (double)(dom[q] ? start + c0 + q + 1 : 1);
         };
+        // interior columns of the tile and valid rows (what is stored and what enters the observables); recomputed where
+        // needed so that nothing of it is live across the order loop
+        auto interior = [&](bool (&in_c)[CP], bool (&row_ok)[RP]) {
+            const int lo_c = t * W - start;                  // first interior column (tile coordinates)
+            int wint = N - t * W;
+            if (wint > W) wint = W;
+#pragma unroll
+            for (int q = 0; q < CP; ++q) in_c[q] = c0 + q >= lo_c && c0 + q < lo_c + wint;
+#pragma unroll
+            for (int r = 0; r < RP; ++r) row_ok[r] = !ragged_rows || gr0 + r < L;
+        };
+        const int n_rep = PERSIST ? n_steps : 1;
+        for (int step = 0; step < n_rep; ++step) {          // (PERSIST: psi stays in registers between the steps)
+        if (PERSIST && step > 0) {
+#pragma unroll
+            for (int r = 0; r < RP; ++r)
+#pragma unroll
+                for (int q = 0; q < CP; ++q) T[r][q] = A[r][q];
+            if (OBS) { obs_setup(step); any_obs = any_obs || obs_now; }
+        }
         set_field(0);
         if (RK) {       // psi(t_n) is needed again when the stage vectors g_2..g_4 are formed
 #pragma unroll
@@ -372,9 +419,9 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                 cup[r] = rt.x; ll1[r] = rt.y;
             }
             double a0[CP], a1[CP], a2[CP], a3[CP], ac[CP];
-#pragma unroll
-            for (int q = 0; q < CP; ++q) { a0[q] = cup[0] * Eq[q]; a1[q] = cup[1] * Eq[q]; a2[q] = cup[2] * Eq[q]; }
             if (NWC == 1) {
+#pragma unroll
+                for (int q = 0; q < CP; ++q) { a0[q] = cup[0] * Eq[q]; a1[q] = cup[1] * Eq[q]; a2[q] = cup[2] * Eq[q]; }
                 do_row(Ti, To, 1, Ti[0], Ti[2], a0, a1, ll1[1], pr, odd, first, s, want_out, cg);
                 do_row(Ti, To, 2, Ti[1], Ti[3], a1, a2, ll1[2], pr, odd, first, s, want_out, cg);
             }
@@ -385,26 +432,47 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                 if (nt >= n_tiles) { nt -= n_tiles; ++nb; }
                 fetch_tile(nb, nt);
             }
-            if (!RK && k == 1 && item + ncl < n_items) ef_next = __ldg(ef + b + db + ((t + dtile >= n_tiles) ? 1 : 0));
+            if (!RK && k == 1) {
+                if (PERSIST && step + 1 < n_rep) ef_next = __ldg(ef + (size_t)(step + 1) * g.batch + b);
+                else if (item + ncl < n_items) ef_next = __ldg(ef + b + db + ((t + dtile >= n_tiles) ? 1 : 0));
+            }
             double2 lo[CP], below[CP];
 #pragma unroll
             for (int q = 0; q < CP; ++q) {
                 if (CLUSTER && lo_remote) lo[q] = ld_dsmem2(lo_dsm + (unsigned)((pr * kParStride + q * 32) * sizeof(double2)));
                 else lo[q] = lo_base[pr * lo_par + q * 32];
-                if (CLUSTER && up_remote) below[q] = ld_dsmem2(up_dsm + (unsigned)((pr * kParStride + q * 32) * sizeof(double2)));
-                else below[q] = up_base[pr * up_par + q * 32];
             }
-            {
-                const double clo = sm.rowtab[r0][2];
+            const double clo = sm.rowtab[r0][2];
+            if (NWC == 1) {
+#pragma unroll
+                for (int q = 0; q < CP; ++q) {
+                    if (CLUSTER && up_remote) below[q] = ld_dsmem2(up_dsm + (unsigned)((pr * kParStride + q * 32) * sizeof(double2)));
+                    else below[q] = up_base[pr * up_par + q * 32];
+                }
 #pragma unroll
                 for (int q = 0; q < CP; ++q) { ac[q] = clo * Eq[q]; a3[q] = cup[3] * Eq[q]; }
-            }
-            do_row(Ti, To, 0, lo, Ti[1], ac, a0, ll1[0], pr, odd, first, s, want_out, cg);
-            if (NWC > 1) {
+                do_row(Ti, To, 0, lo, Ti[1], ac, a0, ll1[0], pr, odd, first, s, want_out, cg);
+                do_row(Ti, To, 3, Ti[2], below, a2, a3, ll1[3], pr, odd, first, s, want_out, cg);
+            } else {
+                // tiles wider than a warp: every row needs the neighbouring warp's edge columns, so all rows come after
+                // the barrier, in order, with the coupling weights of one row pair formed at a time (register budget)
+#pragma unroll
+                for (int q = 0; q < CP; ++q) { ac[q] = clo * Eq[q]; a0[q] = cup[0] * Eq[q]; }
+                do_row(Ti, To, 0, lo, Ti[1], ac, a0, ll1[0], pr, odd, first, s, want_out, cg);
+#pragma unroll
+                for (int q = 0; q < CP; ++q) a1[q] = cup[1] * Eq[q];
                 do_row(Ti, To, 1, Ti[0], Ti[2], a0, a1, ll1[1], pr, odd, first, s, want_out, cg);
+#pragma unroll
+                for (int q = 0; q < CP; ++q) a2[q] = cup[2] * Eq[q];
                 do_row(Ti, To, 2, Ti[1], Ti[3], a1, a2, ll1[2], pr, odd, first, s, want_out, cg);
+#pragma unroll
+                for (int q = 0; q < CP; ++q) {
+                    if (CLUSTER && up_remote) below[q] = ld_dsmem2(up_dsm + (unsigned)((pr * kParStride + q * 32) * sizeof(double2)));
+                    else below[q] = up_base[pr * up_par + q * 32];
+                    a3[q] = cup[3] * Eq[q];
+                }
+                do_row(Ti, To, 3, Ti[2], below, a2, a3, ll1[3], pr, odd, first, s, want_out, cg);
             }
-            do_row(Ti, To, 3, Ti[2], below, a2, a3, ll1[3], pr, odd, first, s, want_out, cg);
             if (k < order) {
 #pragma unroll
                 for (int q = 0; q < CP; ++q) {
@@ -470,12 +538,8 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                     if ((held_bits >> (r * CP + q)) & 1u) A[r][q] = z2;
         }
 
-        // ---- psi(t + dt): interior columns of the tile straight from registers ---------------------------------
+        // ---- end of the step: absorber, observables of the logged row ---------------------------------------------
         {
-            const int lo_c = t * W - start;                  // first interior column (tile coordinates)
-            int wint = N - t * W;
-            if (wint > W) wint = W;
-            double2 *dst_g = out + ((size_t)b * L + rbase + r0) * N + start + c0;
             if (MODE != 2 && g.mask != nullptr) {            // absorbing boundary: psi *= exp(-i W dt) (Eq. 18)
 #pragma unroll
                 for (int q = 0; q < CP; ++q) {
@@ -485,14 +549,11 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                     for (int r = 0; r < RP; ++r) { A[r][q].x *= m; A[r][q].y *= m; }
                 }
             }
-            bool in_c[CP], row_ok[RP];
-#pragma unroll
-            for (int q = 0; q < CP; ++q) in_c[q] = c0 + q >= lo_c && c0 + q < lo_c + wint;
-#pragma unroll
-            for (int r = 0; r < RP; ++r) row_ok[r] = !ragged_rows || gr0 + r < L;
             // (the fused observables come BEFORE the stores: the release fences of their exchange would otherwise wait
             // for the stores to drain)
             if (OBS && obs_now) {
+                bool in_c[CP], row_ok[RP];
+                interior(in_c, row_ok);
                 // row l-1 of psi(t + dt) for this thread's row 0: one more exchange through the buffer of the order loop
                 if (armed) bar_wait();
 #pragma unroll
@@ -559,12 +620,32 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                     for (int i = 0; i < kRpObsRed; ++i) sm.red[warp][i] = red[i];
                 }
                 __syncthreads();
-                if (threadIdx.x < kRpObsRed) {
+                if (obs_direct) {
+                    if (threadIdx.x == 0) {
+                        double sred[kRpObsRed];
+#pragma unroll
+                        for (int i = 0; i < kRpObsRed; ++i) {
+                            double v = 0.0;
+                            for (int w2 = 0; w2 < NWR * NWC; ++w2) v += sm.red[w2][i];
+                            sred[i] = v;
+                        }
+                        write_row(b, sred);
+                    }
+                    __syncthreads();            // sm.red is free again (the next step may come soon)
+                } else if (threadIdx.x < kRpObsRed) {
                     double v = 0.0;
                     for (int w2 = 0; w2 < NWR * NWC; ++w2) v += sm.red[w2][threadIdx.x];
-                    ob.partials[((size_t)item * csize + crank) * kRpObsRed + threadIdx.x] = v;
+                    ob.partials[(((size_t)step * n_items + item) * csize + crank) * kRpObsRed + threadIdx.x] = v;
                 }
             }
+        }
+        if (PERSIST && step + 1 < n_rep) ef_cur = ef_next;
+        }   // step
+        // ---- psi(t + dt): interior columns of the tile straight from registers ---------------------------------
+        {
+            double2 *dst_g = out + ((size_t)b * L + rbase + r0) * N + start + c0;
+            bool in_c[CP], row_ok[RP];
+            interior(in_c, row_ok);
             double2 *prow[RP];
 #pragma unroll
             for (int r = 0; r < RP; ++r) prow[r] = dst_g + (size_t)r * N;
@@ -587,7 +668,10 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
         ef_cur = ef_next;
     }
     if (armed) bar_wait();     // (cluster: no CTA may exit while a neighbour can still read its shared memory)
-    if (OBS && obs_now) {
+    if (OBS && !obs_direct) {
+        // (uniform over the grid: every CTA took the same steps)
+        if (PERSIST) { for (int st = 0; st < n_steps; ++st) { obs_setup(st); any_obs = any_obs || obs_now; } }
+        if (!any_obs) return;
         // the last CTA to sign off adds the partials of every member in a fixed order and writes the row
         __syncthreads();
         if (threadIdx.x == 0) {
@@ -598,25 +682,18 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
         __syncthreads();
         if (!sm.last_flag) return;
         __threadfence();
-        const int per = n_tiles * csize, Wd = 3 + ob.n_states;
+        const int per = n_tiles * csize;
+        for (int st = 0; st < (PERSIST ? n_steps : 1); ++st) {
+        obs_setup(st);
+        if (!obs_now) continue;
         constexpr int NW = NWR * NWC;
-        auto write_row = [&](const int bb, const double (&s)[kRpObsRed]) {
-            double *o = ob.rows + ((size_t)obs_row * g.batch + bb) * Wd;
-            o[0] = g.dr * s[0];
-            o[1] = 2.0 * g.dr * s[1];
-            o[2] = -pulse_E(ob.pulse[bb], obs_t) - 2.0 * g.z * g.dr * s[2];
-            for (int si = 0; si < ob.n_states && si < kRpObsStates; ++si) {
-                const double ar = g.dr * s[3 + 2 * si], ai = g.dr * s[4 + 2 * si];
-                o[3 + si] = ar * ar + ai * ai;
-            }
-        };
         // many members: one warp per member; few members (a single wavefunction): the whole CTA per member
         const bool by_warp = g.batch >= NW;
         for (int bb = by_warp ? warp : 0; bb < g.batch; bb += by_warp ? NW : 1) {
             double s[kRpObsRed];
 #pragma unroll
             for (int i = 0; i < kRpObsRed; ++i) s[i] = 0.0;
-            const double *pp = ob.partials + (size_t)bb * per * kRpObsRed;
+            const double *pp = ob.partials + ((size_t)st * n_items * csize + (size_t)bb * per) * kRpObsRed;
             const int first = by_warp ? lane : (int)threadIdx.x, stride = by_warp ? 32 : G::NT;
 #pragma unroll 4
             for (int i = first; i < per; i += stride) {
@@ -648,6 +725,7 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                 }
             }
         }
+        }   // step of the launch
         if (threadIdx.x == 0) *ob.counter = 0u;
     }
 }
@@ -669,7 +747,7 @@ inline int rp_init_tables() {
 template <class K>
 inline int rp_launch_kernel(K kern, DeviceOnce *once, int smem, const RpPlan &p, cudaStream_t s, const GridDev &g,
                             const double2 *in, double2 *out, const double *ef, const double *dtp, int order,
-                            const CUtensorMap &tm, const RpObs &ob) {
+                            const CUtensorMap &tm, const RpObs &ob, int n_steps = 1) {
     if (once->first()) {
         if (cudaFuncSetAttribute((const void *)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
             return TDSE_ERR_CUDA;
@@ -680,12 +758,12 @@ inline int rp_launch_kernel(K kern, DeviceOnce *once, int smem, const RpPlan &p,
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = p.cl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.attrs = at; cfg.numAttrs = (p.cl > 1) ? 1 : 0;
-    return cudaLaunchKernelEx(&cfg, kern, g, in, out, ef, dtp, order, p.W, p.H, p.n_tiles, p.n_items, tm, ob) == cudaSuccess
+    return cudaLaunchKernelEx(&cfg, kern, g, in, out, ef, dtp, order, p.W, p.H, p.n_tiles, p.n_items, tm, ob, n_steps) == cudaSuccess
                ? TDSE_OK : TDSE_ERR_CUDA;
 }
 
 // the four full-tile instantiations (direct / TMA) x (CTA / cluster) of one (MODE, OBS) pair
-template <int FD, int CP, int NWR, int NWC, int MINB, bool CLUSTERABLE, int MODE, bool OBS>
+template <int FD, int CP, int NWR, int NWC, int MINB, bool CLUSTERABLE, int MODE, bool OBS, bool CUT = false>
 inline int rp_launch_full(const GridDev &g, const RpPlan &p, const CUtensorMap &tm, const double2 *in, double2 *out,
                           const double *ef, const double *dtp, int order, cudaStream_t s, const RpObs &ob) {
     static DeviceOnce once[4];
@@ -694,19 +772,29 @@ inline int rp_launch_full(const GridDev &g, const RpPlan &p, const CUtensorMap &
     if (p.cl > 1) {
         if (!CLUSTERABLE) return TDSE_ERR_UNSUPPORTED;
         constexpr bool kCl = CLUSTERABLE;
-        if (p.tma) return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, true, kCl, MODE, OBS>, &once[3], sm_t, p, s, g, in, out, ef, dtp, order, tm, ob);
-        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, kCl, MODE, OBS>, &once[2], sm_n, p, s, g, in, out, ef, dtp, order, tm, ob);
+        if (p.tma) return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, true, kCl, MODE, OBS, false, CUT>, &once[3], sm_t, p, s, g, in, out, ef, dtp, order, tm, ob);
+        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, kCl, MODE, OBS, false, CUT>, &once[2], sm_n, p, s, g, in, out, ef, dtp, order, tm, ob);
     }
-    if (p.tma) return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, true, false, MODE, OBS>, &once[1], sm_t, p, s, g, in, out, ef, dtp, order, tm, ob);
-    return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, false, MODE, OBS>, &once[0], sm_n, p, s, g, in, out, ef, dtp, order, tm, ob);
+    if (p.tma) return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, true, false, MODE, OBS, false, CUT>, &once[1], sm_t, p, s, g, in, out, ef, dtp, order, tm, ob);
+    return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, false, MODE, OBS, false, CUT>, &once[0], sm_n, p, s, g, in, out, ef, dtp, order, tm, ob);
 }
 
 // MODE 1 / 2 instantiations exist only for the one-warp-wide variants (RKABLE) and full tiles; fused observables (ob)
 // for full tiles in real time (MODE 0 / 1)
 template <int FD, int CP, int NWR, int NWC, int MINB, bool CLUSTERABLE, bool RKABLE>
 inline int rp_launch_one(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
-                         const double *dtp, int order, cudaStream_t s, const RpObs *ob) {
+                         const double *dtp, int order, cudaStream_t s, const RpObs *ob, int n_steps) {
     const bool mask = g.n_r < 32 * CP * NWC;
+    if (p.persist) {        // up to p.persist steps per launch (halo sized for them)
+        if (mask || p.tma || p.cl > 1 || p.rk != 0 || n_steps > p.persist || g.j0 != nullptr) return TDSE_ERR_UNSUPPORTED;
+        static DeviceOnce once[2];
+        const CUtensorMap no_map{};
+        const RpObs no_obs{};
+        const int smem = (int)sizeof(RpSmem<FD, CP, NWR, NWC, false>);
+        if (ob) return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, false, 0, true, true>, &once[0], smem, p, s, g, in, out, ef, dtp, order, no_map, *ob, n_steps);
+        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, false, 0, false, true>, &once[1], smem, p, s, g, in, out, ef, dtp, order, no_map, no_obs, n_steps);
+    }
+    if (n_steps != 1) return TDSE_ERR_UNSUPPORTED;
     CUtensorMap tmap{};
     if (p.tma) {
         if (mask) return TDSE_ERR_UNSUPPORTED;
@@ -716,28 +804,32 @@ inline int rp_launch_one(const GridDev &g, const RpPlan &p, const double2 *in, d
     if (mask) {
         if (p.rk != 0 || p.cl > 1 || ob) return TDSE_ERR_UNSUPPORTED;
         static DeviceOnce once;
-        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, true, MINB, false, false>, &once,
+        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, true, MINB, false, false, 0, false, false, true>, &once,
                                 (int)sizeof(RpSmem<FD, CP, NWR, NWC, false>), p, s, g, in, out, ef, dtp, order, tmap, none);
     }
+    const bool cut = g.j0 != nullptr;            // centrifugal cut-off: the CUT instantiations (no fused rows, no imaginary time)
     if (p.rk == 2) {
-        if (!RKABLE || ob) return TDSE_ERR_UNSUPPORTED;
+        if (!RKABLE || ob || cut) return TDSE_ERR_UNSUPPORTED;
         return rp_launch_full<FD, CP, NWR, NWC, MINB, CLUSTERABLE, RKABLE ? 2 : 0, false>(g, p, tmap, in, out, ef, dtp, order, s, none);
     }
+    if (cut && ob) return TDSE_ERR_UNSUPPORTED;
     if (p.rk == 1) {
         if (!RKABLE) return TDSE_ERR_UNSUPPORTED;
+        if (cut) return rp_launch_full<FD, CP, NWR, NWC, MINB, CLUSTERABLE, RKABLE ? 1 : 0, false, true>(g, p, tmap, in, out, ef, dtp, order, s, none);
         if (ob) return rp_launch_full<FD, CP, NWR, NWC, MINB, CLUSTERABLE, RKABLE ? 1 : 0, true>(g, p, tmap, in, out, ef, dtp, order, s, *ob);
         return rp_launch_full<FD, CP, NWR, NWC, MINB, CLUSTERABLE, RKABLE ? 1 : 0, false>(g, p, tmap, in, out, ef, dtp, order, s, none);
     }
+    if (cut) return rp_launch_full<FD, CP, NWR, NWC, MINB, CLUSTERABLE, 0, false, true>(g, p, tmap, in, out, ef, dtp, order, s, none);
     if (ob) return rp_launch_full<FD, CP, NWR, NWC, MINB, CLUSTERABLE, 0, true>(g, p, tmap, in, out, ef, dtp, order, s, *ob);
     return rp_launch_full<FD, CP, NWR, NWC, MINB, CLUSTERABLE, 0, false>(g, p, tmap, in, out, ef, dtp, order, s, none);
 }
 
 template <int FD>
 inline int launch_taylor_rp_fd(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
-                               const double *dtp, int order, cudaStream_t s, const RpObs *ob) {
+                               const double *dtp, int order, cudaStream_t s, const RpObs *ob, int n_steps) {
     if (!p.ok) return TDSE_ERR_UNSUPPORTED;
 #define TDSE_RP_CASE(I, CP, NWR, NWC, MINB) \
-    case I: return rp_launch_one<FD, CP, NWR, NWC, MINB, rp_clusterable(I), rp_rk_capable(I)>(g, p, in, out, ef, dtp, order, s, ob);
+    case I: return rp_launch_one<FD, CP, NWR, NWC, MINB, rp_clusterable(I), rp_rk_capable(I)>(g, p, in, out, ef, dtp, order, s, ob, n_steps);
     switch (p.variant) {
         TDSE_RP_CASE(0, 4, 1, 1, 8)
         TDSE_RP_CASE(1, 4, 2, 1, 4)

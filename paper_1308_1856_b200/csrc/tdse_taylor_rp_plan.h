@@ -25,13 +25,17 @@ constexpr bool rp_clusterable(int variant) { return variant == 2 || variant == 4
 constexpr bool rp_rk_capable(int variant) { return variant >= 0 && variant <= 3; }
 
 // rk = kernel MODE (0 Taylor, 1 classic RK4, 2 imaginary time); cl: CTAs per cluster (1: none)
-struct RpPlan { int ok, variant, tma, cl, rk, W, H, WT, n_tiles, n_items, grid, threads; };
+struct RpPlan { int ok, variant, tma, cl, rk, W, H, WT, n_tiles, n_items, grid, threads, persist; };     // persist: steps per launch (0: one)
 
 bool tma_available();       // cuTensorMapEncodeTiled could be resolved (tdse_api.cu)
 
 // use_tma: -1 heuristic, 0 never, 1 whenever the layout allows it (n_r % 8 == 0 and more than one tile)
 // rk: plan the fused RK4 / imaginary-time step (only the one-warp-wide instantiations, full tiles)
-inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant, int use_tma, int rk = 0) {
+// persist = k > 1: temporal blocking across steps: the halo covers k steps (H = k x order x hw), so one launch takes up to
+// k steps with psi in registers (Taylor in real time, full tiles, direct loads, no cluster); kept only while the interior
+// of a tile stays at least half of it
+inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant, int use_tma, int rk = 0, int persist = 0) {
+    if (persist > 1 && rk != 0) persist = 0;
     RpPlan best{};
     const int hw = (g.fd_order == 3) ? 1 : 2;
     double best_cost = 0.0;
@@ -41,6 +45,7 @@ inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant
         const int WT = 32 * v.cp * v.nwc;
         if (rk && (!rp_rk_capable(i) || g.n_r < WT)) continue;
         int rows = kRpRows * v.nwr, cl = 1;
+        if (persist > 1 && (rows < g.n_l || g.n_r <= WT)) continue;
         if (rows < g.n_l) {
             // more rows than one CTA holds: split them over a cluster of 2, 4 or 8 CTAs (16-row CTAs only)
             if (!rp_clusterable(i)) continue;
@@ -51,17 +56,18 @@ inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant
         if (rows >= 2 * g.n_l && v.nwr > 1) continue;      // more than half of the rows would be padding
         for (int tma = 0; tma <= 1; ++tma) {
             const bool tma_ok = !(g.n_r & 7) && g.n_r > WT && tma_available();
-            if (tma && (use_tma == 0 || !tma_ok)) continue;
-            if (!tma && use_tma == 1 && tma_ok) continue;
-            int H = order * hw;
+            if (tma && (use_tma == 0 || !tma_ok || persist > 1)) continue;
+            if (!tma && use_tma == 1 && tma_ok && persist <= 1) continue;
+            int H = order * hw * (persist > 1 ? persist : 1);
             if (tma) H = (H + 7) & ~7;                      // tile starts on a 128-byte column group
             else if ((g.n_r & 1) == 0) H = (H + 1) & ~1;    // even halo: every patch row starts 32-byte aligned
             RpPlan p{};
             p.variant = i; p.tma = tma; p.cl = cl; p.rk = rk; p.H = H; p.WT = WT; p.threads = 32 * v.nwr * v.nwc;
+            p.persist = persist > 1 ? persist : 0;
             if (g.n_r <= WT) { p.W = g.n_r; p.n_tiles = 1; }
             else {
                 p.W = WT - 2 * H;
-                if (p.W < WT / 4) continue;
+                if (p.W < (persist > 1 ? WT / 2 : WT / 4)) continue;
                 p.n_tiles = (g.n_r + p.W - 1) / p.W;
             }
             p.n_items = p.n_tiles * g.batch;
@@ -105,20 +111,21 @@ inline bool rp_obs_capable(const RpPlan &p, const tdse_grid &g, int n_states) {
     return p.ok && p.rk != 2 && g.n_r >= p.WT && n_states <= kRpObsStates;
 }
 // doubles of partial sums the fused observables need
-inline size_t rp_obs_partials(const RpPlan &p) { return (size_t)p.n_items * p.cl * kRpObsRed; }
+inline size_t rp_obs_partials(const RpPlan &p) { return (size_t)p.n_items * p.cl * kRpObsRed * (p.persist > 1 ? p.persist : 1); }
 
 // defined in tdse_taylor_rp_fd3.cu / tdse_taylor_rp_fd5.cu
 int rp_init_fd3();          // uploads the 1/k table of that translation unit to the current device (tdse_create)
 int rp_init_fd5();
 int launch_taylor_rp_fd3(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
-                         const double *dtp, int order, cudaStream_t s, const RpObs *ob);
+                         const double *dtp, int order, cudaStream_t s, const RpObs *ob, int n_steps);
 int launch_taylor_rp_fd5(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
-                         const double *dtp, int order, cudaStream_t s, const RpObs *ob);
+                         const double *dtp, int order, cudaStream_t s, const RpObs *ob, int n_steps);
 
+// n_steps > 1 only with a persistent plan (ef then holds n_steps x batch field values)
 inline int launch_taylor_rp(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
-                            const double *dtp, int order, cudaStream_t s, const RpObs *ob = nullptr) {
-    return g.fd == 3 ? launch_taylor_rp_fd3(g, p, in, out, ef, dtp, order, s, ob)
-                     : launch_taylor_rp_fd5(g, p, in, out, ef, dtp, order, s, ob);
+                            const double *dtp, int order, cudaStream_t s, const RpObs *ob = nullptr, int n_steps = 1) {
+    return g.fd == 3 ? launch_taylor_rp_fd3(g, p, in, out, ef, dtp, order, s, ob, n_steps)
+                     : launch_taylor_rp_fd5(g, p, in, out, ef, dtp, order, s, ob, n_steps);
 }
 
 }  // namespace tdse
