@@ -33,7 +33,7 @@ METRIC = "Gpoint-updates/s of H(t)psi (Taylor step)"
 UNIT = "Gpoint-updates/s"
 L2_BYTES = 126e6                      # B200 L2 (B200_PROFILING.md)
 # FP64 issue roof: 148 SMs x 64 FP64 lanes x clocks.max.sm 1.965 GHz = 18.6 T thread-instructions/s (nominal, from the
-# guide's unit counts and clocks; a DFMA-only probe on this pool measured 18.2 T/s, profiles/r02_probe_fp64_issue.md)
+# guide's unit counts and clocks; a DFMA-only probe on this pool measured 18.2 T/s, profiles/r02_README.md section 2)
 FP64_PEAK_INSTR = 148 * 64 * 1.965e9
 
 
