@@ -102,6 +102,24 @@ def pulse_A(pulse, t):
     return lib().oracle_pulse_A(C.byref(p), float(t))
 
 
+def gl5_field_integral(pulse, ta, tb):
+    """int_ta^tb E dtau by one 5-point Gauss-Legendre rule."""
+    p = _pulse1(pulse)
+    f = lib().oracle_gl5_field_integral
+    f.restype = C.c_double
+    f.argtypes = [C.POINTER(Pulse), C.c_double, C.c_double]
+    return f(C.byref(p), float(ta), float(tb))
+
+
+def vecpot_running(pulse, t0, dt, nsteps):
+    """A(t0 + n dt), n = 0..nsteps, by the running quadrature of P:188 on the field of `pulse`."""
+    p = _pulse1(pulse)
+    out = np.zeros(int(nsteps) + 1)
+    rc = lib().oracle_vecpot_running(C.byref(p), C.c_double(t0), C.c_double(dt), C.c_long(nsteps), _dp(out))
+    assert rc == 0, rc
+    return out
+
+
 def coupling(n_l):
     c = np.zeros(n_l)
     lib().oracle_coupling(int(n_l), _dp(c))

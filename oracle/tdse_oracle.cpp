@@ -21,6 +21,49 @@ static double coupling_field(const oracle_grid *g, const oracle_pulse *p, double
     return g->gauge == 1 ? oracle_pulse_A(p, t) : oracle_pulse_E(p, t);
 }
 
+// ---- vector potential of a pulse given by its FIELD (kind 0) -- P:186-188: "we numerically calculate the potential
+// field A(t), for each time step, as A(t_{n+1}) = A(t_n) - int_{t_n}^{t_n+h} E dtau, where the integral is performed using
+// a standard 5-point Gaussian quadrature" (c dropped), and inside a step A(t_n + c_i h) = A(t_n) -
+// int_{t_n}^{t_n + c_i h} E dtau.  Reading R-V4: a call that starts at t0 > 0 starts from
+// A(t0) = - sum of the same 5-point rule over the panels [m dt, (m+1) dt] from 0 and the last partial panel up to t0.
+static double gl5(const oracle_pulse *p, double ta, double tb) {
+    // nodes and weights of the 5-point Gauss-Legendre rule on [-1, 1] (Abramowitz & Stegun 25.4.30, table 25.4)
+    static const double x[5] = {-0.9061798459386640, -0.5384693101056831, 0.0, 0.5384693101056831, 0.9061798459386640};
+    static const double w[5] = {0.2369268850561891, 0.4786286704993665, 0.5688888888888889, 0.4786286704993665,
+                                0.2369268850561891};
+    const double half = 0.5 * (tb - ta), mid = 0.5 * (tb + ta);
+    double s = 0.0;
+    for (int i = 0; i < 5; ++i) s += w[i] * oracle_pulse_E(p, mid + half * x[i]);
+    return half * s;
+}
+static bool needs_quadrature(const oracle_grid *g, const oracle_pulse *p) {
+    return g->gauge == 1 && p->omega != 0.0 && p->kind == 0;
+}
+struct VecPot {                     // A(t_n) of every member that needs the running quadrature
+    std::vector<double> a;
+    void init(const oracle_grid *g, const oracle_pulse *pulse, double t0, double dt) {
+        a.assign(g->batch, 0.0);
+        for (int b = 0; b < g->batch; ++b) {
+            if (!needs_quadrature(g, &pulse[b]) || !(t0 > 0.0)) continue;
+            const long m = (long)std::floor(t0 / dt);
+            double acc = 0.0;
+            for (long i = 0; i < m; ++i) acc -= gl5(&pulse[b], i * dt, (i + 1) * dt);
+            if (t0 > m * dt) acc -= gl5(&pulse[b], m * dt, t0);
+            a[b] = acc;
+        }
+    }
+    // the time-dependent factor of the coupling at t_n + tau
+    // (t_abs: the same instant as the propagator computes it, used by the pulses that have a closed form)
+    double at(const oracle_grid *g, const oracle_pulse *pulse, int b, double tn, double tau, double t_abs) const {
+        if (!needs_quadrature(g, &pulse[b])) return coupling_field(g, &pulse[b], t_abs);
+        return tau == 0.0 ? a[b] : a[b] - gl5(&pulse[b], tn, tn + tau);
+    }
+    void advance(const oracle_grid *g, const oracle_pulse *pulse, double tn, double h) {
+        for (int b = 0; b < g->batch; ++b)
+            if (needs_quadrature(g, &pulse[b])) a[b] -= gl5(&pulse[b], tn, tn + h);
+    }
+};
+
 namespace {
 
 int g_threads = 1;
@@ -253,7 +296,8 @@ Tableau tableau_of(int id) {
 // *err = max_b ||Delta_b|| / ||psi_new,b||  (0 without an embedded pair).  psi is not modified.
 void rk_step(const oracle_grid *g, const oracle_pulse *pulse, const Tableau &tb, const double *psi,
              double t, double h, std::vector<std::vector<double>> &k, bool k1_valid,
-             std::vector<double> &gbuf, std::vector<double> &hbuf, double *psi_new, double *err) {
+             std::vector<double> &gbuf, std::vector<double> &hbuf, double *psi_new, double *err,
+             const VecPot &vp) {
     const long M = n_points(g);
     const int B = g->batch;
     for (int i = (k1_valid ? 1 : 0); i < tb.s; ++i) {
@@ -265,7 +309,7 @@ void rk_step(const oracle_grid *g, const oracle_pulse *pulse, const Tableau &tb,
         }
         // k_i <- f(t_n + c_i h, g) = -i H(t_n + c_i h) g      (Eq. 17)
         for (int b = 0; b < B; ++b) {
-            const double e = coupling_field(g, &pulse[b], t + tb.c[i] * h);
+            const double e = vp.at(g, pulse, b, t, tb.c[i] * h, t + tb.c[i] * h);   // (P:480 for a pulse given by its field)
             apply_H_member(g, gbuf.data() + 2 * M * b, e, hbuf.data() + 2 * M * b);
         }
         double *ki = k[i].data();
@@ -469,6 +513,21 @@ double oracle_pulse_A(const oracle_pulse *p, double t) {
     return -(p->e0 / p->omega) * s * s * std::sin(p->omega * t + p->cep);
 }
 
+double oracle_gl5_field_integral(const oracle_pulse *p, double ta, double tb) { return gl5(p, ta, tb); }
+
+int oracle_vecpot_running(const oracle_pulse *p, double t0, double dt, long nsteps, double *a_out) {
+    if (!p || !(dt > 0.0) || nsteps < 0 || !a_out) return -1;
+    // the running scheme of P:188 on the field E(t) of this pulse, whatever its kind (for a kind-1 pulse the result can
+    // be compared with its analytic A(t): the paper's Fig. 8)
+    const long m = (t0 > 0.0) ? (long)std::floor(t0 / dt) : 0;
+    double acc = 0.0;
+    for (long i = 0; i < m; ++i) acc -= gl5(p, i * dt, (i + 1) * dt);
+    if (t0 > m * dt) acc -= gl5(p, m * dt, t0);
+    a_out[0] = acc;
+    for (long n = 0; n < nsteps; ++n) { acc -= gl5(p, t0 + n * dt, t0 + (n + 1) * dt); a_out[n + 1] = acc; }
+    return 0;
+}
+
 void oracle_coupling(int n_l, double *c) { for (int l = 0; l < n_l; ++l) c[l] = coupling(l); }
 
 int oracle_apply_H(const oracle_grid *g, const double *psi, const double *e_field, double *out) {
@@ -592,11 +651,13 @@ int oracle_step_taylor(const oracle_grid *g, const oracle_pulse *pulse, double *
     const long M = n_points(g);
     std::vector<double> term(2 * M), hterm(2 * M);
     long block = 0;
+    VecPot vp;
+    vp.init(g, pulse, t0, dt);
     for (long n = 0; n < nsteps; ++n) {
         const double ts = field_sample == 1 ? t0 + n * dt : t0 + (n + 0.5) * dt;  // reading R-G7
         for (int b = 0; b < g->batch; ++b) {
             double *f = psi + 2 * M * b;
-            const double e = coupling_field(g, &pulse[b], ts);
+            const double e = vp.at(g, pulse, b, t0 + n * dt, field_sample == 1 ? 0.0 : 0.5 * dt, ts);
             // F^(0) = F_n; F^(k) = (-i dt/k) H F^(k-1); F_{n+1} = sum_k F^(k)   (Eq. 37)
             std::memcpy(term.data(), f, sizeof(double) * 2 * M);
             for (int k = 1; k <= order; ++k) {
@@ -609,6 +670,7 @@ int oracle_step_taylor(const oracle_grid *g, const oracle_pulse *pulse, double *
                 for (long i = 0; i < 2 * M; ++i) f[i] += term[i];
             }
         }
+        vp.advance(g, pulse, t0 + n * dt, dt);       // A(t_{n+1}) = A(t_n) - int E
         if (obs && obs->obs_every > 0 && (n + 1) % obs->obs_every == 0)
             log_obs(g, pulse, psi, t0 + (n + 1) * dt, obs, block++);
     }
@@ -656,9 +718,12 @@ int oracle_step_rk_fixed(const oracle_grid *g, const oracle_pulse *pulse, double
     std::vector<std::vector<double>> k(tb.s, std::vector<double>(2 * MB));
     std::vector<double> gbuf(2 * MB), hbuf(2 * MB), next(2 * MB);
     long block = 0;
+    VecPot vp;
+    vp.init(g, pulse, t0, dt);
     for (long n = 0; n < nsteps; ++n) {
         double err;
-        rk_step(g, pulse, tb, psi, t0 + n * dt, dt, k, false, gbuf, hbuf, next.data(), &err);
+        rk_step(g, pulse, tb, psi, t0 + n * dt, dt, k, false, gbuf, hbuf, next.data(), &err, vp);
+        vp.advance(g, pulse, t0 + n * dt, dt);
         std::memcpy(psi, next.data(), sizeof(double) * 2 * MB);
         if (err_out) err_out[n] = err;
         if (obs && obs->obs_every > 0 && (n + 1) % obs->obs_every == 0)
@@ -685,9 +750,12 @@ int oracle_step_rk_sigma(const oracle_grid *g, const oracle_pulse *pulse, double
     std::vector<double> gbuf(2 * MB), hbuf(2 * MB), next(2 * MB);
     if (sigma_out) for (int b = 0; b < g->batch; ++b) sigma_out[b] = 0.0;
     long block = 0;
+    VecPot vp;
+    vp.init(g, pulse, t0, dt);
     for (long n = 0; n < nsteps; ++n) {
         double err;
-        rk_step(g, pulse, tb, psi, t0 + n * dt, dt, k, false, gbuf, hbuf, next.data(), &err);   // gbuf <- Delta
+        rk_step(g, pulse, tb, psi, t0 + n * dt, dt, k, false, gbuf, hbuf, next.data(), &err, vp);   // gbuf <- Delta
+        vp.advance(g, pulse, t0 + n * dt, dt);
         std::memcpy(psi, next.data(), sizeof(double) * 2 * MB);
         if (sigma_out && tb.bh)
             for (int b = 0; b < g->batch; ++b) sigma_out[b] += std::sqrt(sumsq(M, gbuf.data() + 2 * M * b) / (double)M);
@@ -710,14 +778,17 @@ int oracle_step_rk45(const oracle_grid *g, const oracle_pulse *pulse, double *ps
     long na = 0, nr = 0;
     double t = t0;
     bool fsal = false;
+    VecPot vp;
+    vp.init(g, pulse, t0, dt_replay ? (n_replay > 0 ? dt_replay[0] : 1.0) : dt_init);
     if (dt_replay) {
         for (long n = 0; n < n_replay; ++n) {
             double err;
             const double h = dt_replay[n];
-            rk_step(g, pulse, tb, psi, t, h, k, fsal, gbuf, hbuf, next.data(), &err);
+            rk_step(g, pulse, tb, psi, t, h, k, fsal, gbuf, hbuf, next.data(), &err, vp);
             std::memcpy(psi, next.data(), sizeof(double) * 2 * MB);
             k[0].swap(k[6]); fsal = true;  // k_7 of this step is k_1 of the next (same time t_{n+1})
             if (na < max_log) { if (dt_log) dt_log[na] = h; if (err_log) err_log[na] = err / rtol; }
+            vp.advance(g, pulse, t, h);
             ++na; t += h;
         }
     } else {
@@ -729,7 +800,7 @@ int oracle_step_rk45(const oracle_grid *g, const oracle_pulse *pulse, double *ps
             bool last = false;
             if (t + h >= t_end) { h = t_end - t; last = true; }  // land on t_end exactly
             double e;
-            rk_step(g, pulse, tb, psi, t, h, k, fsal, gbuf, hbuf, next.data(), &e);
+            rk_step(g, pulse, tb, psi, t, h, k, fsal, gbuf, hbuf, next.data(), &e, vp);
             const double err = e / rtol;
             double fac = 0.9 * std::pow(err, -0.2);
             if (!(fac >= 0.2)) fac = 0.2;   // also catches NaN
@@ -739,6 +810,7 @@ int oracle_step_rk45(const oracle_grid *g, const oracle_pulse *pulse, double *ps
                 k[0].swap(k[6]); fsal = true;
                 if (na < max_log) { if (dt_log) dt_log[na] = h; if (err_log) err_log[na] = err; }
                 ++na;
+                vp.advance(g, pulse, t, h);
                 t = last ? t_end : t + h;
                 if (after_reject && fac > 1.0) fac = 1.0;
                 after_reject = false;
@@ -766,13 +838,17 @@ int oracle_step_lanczos(const oracle_grid *g, const oracle_pulse *pulse, double 
     std::vector<double> q(2 * M * krylov_dim), w(2 * M);
     std::vector<double> alpha(krylov_dim), beta(krylov_dim), coef(2 * krylov_dim);
     long block = 0;
+    VecPot vp;
+    vp.init(g, pulse, t0, dt);
     for (long n = 0; n < nsteps; ++n) {
         const double ts = field_sample == 1 ? t0 + n * dt : t0 + (n + 0.5) * dt;
         for (int b = 0; b < g->batch; ++b) {
             int n_sub;
-            lanczos_member(g, psi + 2 * M * b, coupling_field(g, &pulse[b], ts), krylov_dim, taylor_order,
+            lanczos_member(g, psi + 2 * M * b, vp.at(g, pulse, b, t0 + n * dt, field_sample == 1 ? 0.0 : 0.5 * dt, ts),
+                           krylov_dim, taylor_order,
                            dt, beta_tol, q, w, alpha.data(), beta.data(), coef.data(), &n_sub);
         }
+        vp.advance(g, pulse, t0 + n * dt, dt);
         if (obs && obs->obs_every > 0 && (n + 1) % obs->obs_every == 0)
             log_obs(g, pulse, psi, t0 + (n + 1) * dt, obs, block++);
     }

@@ -56,8 +56,17 @@ typedef struct {      /* kind 0: E(t) = e0 sin^2(omega t/(2 n_c)) cos(omega t + 
 /* --- pieces of H ------------------------------------------------------- */
 double oracle_pulse_E(const oracle_pulse *p, double t);
 /* A(t) with E = -dA/dt (Eq. 20 with the factor c dropped as in P:182); defined for kind 1 pulses and for the
- * static test aid (omega == 0: A = e0); NaN for kind 0 (the running quadrature of P:180 is not implemented). */
+ * static test aid (omega == 0: A = e0); NaN for kind 0, whose A(t) exists only as the running quadrature below. */
 double oracle_pulse_A(const oracle_pulse *p, double t);
+/* Vector potential of a pulse given by its FIELD (kind 0) in the velocity gauge: the running 5-point Gauss-Legendre
+ * quadrature of P:186-188, A(t_{n+1}) = A(t_n) - int_{t_n}^{t_n+h} E dtau (c dropped), and inside a step
+ * A(t_n + c_i h) = A(t_n) - int_{t_n}^{t_n + c_i h} E dtau.  A call that starts at t0 > 0 starts from the same
+ * rule summed over the panels [m dt, (m+1) dt] from 0 and the last partial panel (reading R-V4).  Every propagator uses
+ * this scheme when grid.gauge = 1 and pulse.kind = 0.
+ *   oracle_gl5_field_integral: int_{ta}^{tb} E(tau) dtau by ONE 5-point rule.
+ *   oracle_vecpot_running: a_out[0..nsteps] = A(t0), A(t0 + dt), ... by the running scheme on E(t) of `p` (any kind). */
+double oracle_gl5_field_integral(const oracle_pulse *p, double ta, double tb);
+int    oracle_vecpot_running(const oracle_pulse *p, double t0, double dt, long nsteps, double *a_out);
 /* c[l] = (l+1)/sqrt((2l+1)(2l+3)), l = 0..n_l-1: k_{l,l+1}(m=0) of P:94 Eq. 9 */
 void   oracle_coupling(int n_l, double *c);
 

@@ -718,7 +718,7 @@ def test_P13_vector_potential_pulse_and_gauge_agreement():
     assert np.max(np.abs(num - ana)) < 1e-8
     assert oracle.pulse_A(p, 0.0) == 0.0 and abs(oracle.pulse_A(p, T)) < 1e-15 and oracle.pulse_A(p, T + 1.0) == 0.0
     assert 0.9 * p[0] < np.max(np.abs(ana)) <= 1.05 * p[0]
-    assert math.isnan(oracle.pulse_A((0.05, 0.057, 2.0, 0.0, 0), 1.0))          # kind 0: no A(t) (running quadrature absent)
+    assert math.isnan(oracle.pulse_A((0.05, 0.057, 2.0, 0.0, 0), 1.0))          # kind 0: no closed form here (running quadrature, P16)
     # depletion of 1s by a one-cycle pulse at omega = 0.6 au (one-photon ionisation), both gauges
     n_r, dr, n_l, dt = 400, 0.2, 6, 0.004
     pulse = [(0.15, 0.6, 3.0, 0.0, 1)]
@@ -928,3 +928,81 @@ def test_P15_cutoff_in_every_propagator_against_the_dense_exponential():
                       ("taylor", oracle.step_taylor(g, static, psi0, 8, 0.0, dt, n)[0])):
         assert np.linalg.norm(got - exact) <= 1e-9, name
         assert np.count_nonzero(got[0][oracle.held_mask(g)]) == 0, name
+
+
+# ---------------------------------------------------- vector potential by the running Gauss quadrature (P16, f1 widened)
+def _closed_form_A_kind0(e0, om, nc, t):
+    """A(t) = -int_0^t e0 sin^2(om t'/(2 nc)) cos(om t') dt' in closed form (cep = 0): sin^2 = (1 - cos 2 Om t)/2."""
+    Om = om / (2.0 * nc)
+    return -0.5 * e0 * (np.sin(om * t) / om - np.sin((om + 2 * Om) * t) / (2 * (om + 2 * Om))
+                        - np.sin((om - 2 * Om) * t) / (2 * (om - 2 * Om)))
+
+
+def test_P16_running_quadrature_against_the_analytic_vector_potential():
+    """The paper's Fig. 8: the vector potential from the running 5-point Gauss quadrature of the field
+     against the analytic one -- for the Hann-shaped A (kind 1, E = -dA/dt fed to the quadrature) and for the
+    ordinary sin^2 pulse (kind 0, closed form above); from t = 0 and from a start inside the pulse (reading R-V4); the
+    5-point rule is exact for polynomials of degree 9, so halving a coarse step cuts the error by about 2^10."""
+    p1 = (0.1688, 0.3675, 10.0, 0.0, 1)                 # 1e15 W/cm^2, 10 eV, 10 cycles: the pulse of Fig. 8
+    T = 2 * math.pi * p1[2] / p1[1]
+    dt = 0.05
+    n = int(T / dt)
+    a = oracle.vecpot_running(p1, 0.0, dt, n)
+    ref = np.array([oracle.pulse_A(p1, k * dt) for k in range(n + 1)])
+    assert np.max(np.abs(ref)) > 0.4 and np.max(np.abs(a - ref)) <= 1e-13
+    a = oracle.vecpot_running(p1, 33.37, dt, 500)       # starts inside the pulse, off the panel grid
+    ref = np.array([oracle.pulse_A(p1, 33.37 + k * dt) for k in range(501)])
+    assert np.max(np.abs(a - ref)) <= 1e-13
+    e0, om, nc = 0.0534, 0.057, 4.0
+    p0 = (e0, om, nc, 0.0, 0)
+    T = 2 * math.pi * nc / om
+    for t0 in (0.0, 101.3):
+        a = oracle.vecpot_running(p0, t0, 0.5, 300)
+        ts = t0 + 0.5 * np.arange(301)
+        assert np.max(np.abs(a - _closed_form_A_kind0(e0, om, nc, ts))) <= 1e-13
+    assert abs(oracle.vecpot_running(p0, 0.0, T / 400, 400)[-1]) <= 1e-13        # a whole pulse integrates to zero
+    errs = []
+    for h in (40.0, 20.0):                                                       # coarse panels: convergence order
+        a = oracle.vecpot_running(p0, 0.0, h, int(200 / h))
+        errs.append(abs(a[-1] - _closed_form_A_kind0(e0, om, nc, 200.0)))
+    assert errs[1] < errs[0] / 300
+    # one rule alone: exact on a constant field, antisymmetric in its limits
+    assert abs(oracle.gl5_field_integral((0.3, 0.0, 1.0, 0.0, 0), 1.0, 3.5) - 0.75) <= 1e-15
+    assert oracle.gl5_field_integral(p0, 10.0, 12.0) == -oracle.gl5_field_integral(p0, 12.0, 10.0)
+
+
+def test_P16_velocity_gauge_propagators_with_a_field_pulse():
+    """Velocity-gauge propagation under an ordinary (kind-0) pulse: Taylor and Lanczos freeze H at A(t_n + dt/2) =
+    A(t_n) - int_{t_n}^{t_n+dt/2} E (P:480 with c_i = 1/2), RK4 takes A at its stage times; each against numpy on the
+    independently built dense H (P13) with the CLOSED-FORM A(t) at those times."""
+    n_r, dr, n_l, fd = 30, 0.2, 3, 5
+    e0, om, nc = 0.4, 0.9, 2.0
+    pulse = [(e0, om, nc, 0.0, 0)]
+    g = oracle.make_grid(n_r, dr, n_l, fd, gauge=1)
+    psi0 = rand_state((1, n_l, n_r), 9)
+    psi0 /= math.sqrt(dr * np.sum(np.abs(psi0) ** 2))
+    t0, dt, n = 2.31, 2e-3, 12
+    A = lambda t: float(_closed_form_A_kind0(e0, om, nc, t))
+    H = lambda t: _dense_velocity_H(n_r, dr, n_l, fd, A(t))
+    # Taylor / Lanczos: product of frozen-midpoint exponentials
+    ref = psi0.ravel().copy()
+    for k in range(n):
+        ref = sla.expm(-1j * dt * H(t0 + (k + 0.5) * dt)) @ ref
+    got = oracle.step_taylor(g, pulse, psi0, 14, t0, dt, n)[0]
+    assert np.linalg.norm(got.ravel() - ref) <= 1e-11
+    got = oracle.step_lanczos(g, pulse, psi0, 30, 14, t0, dt, n)[0]
+    assert np.linalg.norm(got.ravel() - ref) <= 1e-9
+    # classic RK4 with H at the stage times, written out in numpy
+    y = psi0.ravel().copy()
+    f = lambda t, v: -1j * (H(t) @ v)
+    for k in range(n):
+        t = t0 + k * dt
+        k1 = f(t, y); k2 = f(t + dt / 2, y + dt / 2 * k1); k3 = f(t + dt / 2, y + dt / 2 * k2); k4 = f(t + dt, y + dt * k3)
+        y = y + dt / 6 * (k1 + 2 * k2 + 2 * k3 + k4)
+    got = oracle.step_rk4(g, pulse, psi0, t0, dt, n)[0]
+    assert np.linalg.norm(got.ravel() - y) <= 1e-12
+    # and the sign convention ties in with the analytic pulses: the SAME physical pulse given as kind 1 (A analytic) and
+    # as its field integrated numerically must propagate identically -- here through apply_H at equal A
+    p1 = (0.2, 0.6, 3.0, 0.0, 1)
+    a_run = oracle.vecpot_running(p1, 0.0, 0.01, 500)[-1]
+    assert abs(a_run - oracle.pulse_A(p1, 5.0)) <= 1e-14
