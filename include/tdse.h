@@ -48,7 +48,7 @@ typedef struct {
     int    n_l;       /* number of partial-wave blocks L, l = 0..n_l-1 (`NumBlocks`)       */
     int    fd_order;  /* 3 or 5 point second derivative (Eq. 15)                            */
     int    gauge;     /* 0 = length gauge (Eq. 11), 1 = velocity gauge (Eq. 12 in reading R-V2,
-                         first derivative of P:119 Eq. 14; needs kind-1 pulses); else TDSE_ERR_UNSUPPORTED */
+                         first derivative of P:119 Eq. 14); else TDSE_ERR_UNSUPPORTED */
     double z_nuc;     /* V(r) = -z_nuc/r                                                   */
     int    batch;     /* B >= 1 independent members sharing the grid                      */
 } tdse_grid;
@@ -57,8 +57,11 @@ typedef struct {      /* E(t) = e0 sin^2(omega t/(2 n_cycles)) cos(omega t + cep
     double e0, omega, n_cycles, cep;   /* else 0 (Eq. 19; R-G8).  omega == 0: static field e0 */
     int kind;         /* 0: as above.  1: the Hann shape is on the vector potential (R-V3):
                          A(t) = -(e0/omega) sin^2(omega t/(2 n_cycles)) sin(omega t + cep), E(t) = -dA/dt.
-                         The velocity gauge (tdse_grid.gauge = 1) needs kind 1 (or the static test aid omega = 0,
-                         whose e0 is then the constant A). */
+                         In the velocity gauge (tdse_grid.gauge = 1) a kind-0 pulse gets its A(t) from the running
+                         5-point Gauss quadrature of the field, A(t_{n+1}) = A(t_n) - int E, with
+                         A(t_n + c_i h) = A(t_n) - int_{t_n}^{t_n + c_i h} E inside a step; a call starting at
+                         t0 > 0 starts from the same rule summed over panels of width dt from 0 (reading R-V4).  The
+                         static test aid omega = 0 has the constant A = e0. */
 } tdse_pulse;
 
 /* Create / destroy.  tdse_create builds the device tables (diagonal of h_l, c_l) and allocates the state
@@ -112,7 +115,7 @@ int  tdse_set_absorber(tdse_handle *h, double r_b, int p);
  * current state and every later tdse_set_state are projected.  lambda = 0 removes it.  Synchronises the device. */
 int  tdse_set_cutoff(tdse_handle *h, double lambda);
 
-/* One pulse per member, host array [batch].  TDSE_ERR_UNSUPPORTED for a kind-0 pulse on a velocity-gauge handle. */
+/* One pulse per member, host array [batch]. */
 int  tdse_set_pulse(tdse_handle *h, const tdse_pulse *per_member_host);
 
 /* Real bound-state vectors for the population observable p_s = |dr sum_j phi_s[j] f_{l_s,j}|^2
@@ -162,7 +165,8 @@ int  tdse_energy_log(tdse_handle *h, double *energy_host, long max_rows, void *s
 /* Embedded Dormand-Prince 5(4) (named P:796; error estimate P:813-833; the adaptive controller is ours,
  * R-C4, the paper's is "not implemented"): err = max_b ||Delta_b||_2 / (rtol ||psi_new,b||_2), accept iff
  * err <= 1, dt_next = dt clamp(0.9 err^(-1/5), 0.2, 5) (<= 1 right after a reject), last step clipped to t_end,
- * FSAL.  If dt_replay != NULL (host [n_replay]) exactly those steps are taken, all accepted.
+ * FSAL.  If dt_replay != NULL (host [n_replay]) exactly those steps are taken, all accepted.  TDSE_ERR_UNSUPPORTED
+ * in the velocity gauge with kind-0 pulses (the running quadrature of A(t) serves the fixed-step propagators).
  * Synchronises `stream`; n_accept / n_reject may be NULL. */
 int  tdse_step_rk45(tdse_handle *h, double t0, double t_end, double dt_init, double rtol,
                     const double *dt_replay, long n_replay, long *n_accept, long *n_reject, void *stream);

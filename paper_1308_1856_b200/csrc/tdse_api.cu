@@ -136,6 +136,7 @@ struct tdse_handle {
     int apply_tma = 1;                      // tdse_apply_H: TMA-fetched tiles when n_r % 8 == 0
     int lanczos_tma = 1;                    // Lanczos pass: sources fetched by TMA when n_r % 8 == 0
     double *d_sigma = nullptr;              // passive RK error sums [batch] (tdse_step_rk)
+    double *d_arun = nullptr; bool vg_quad = false;   // velocity gauge with kind-0 pulses: running A(t_n) per member
     int *d_j0 = nullptr; double cutoff = 0.0;     // centrifugal inner cut-off (tdse_set_cutoff)
     double *d_mask = nullptr; double *d_pb = nullptr;   // absorber mask [n_r] (or null), bound populations [batch]
     double *d_elog = nullptr, *d_imag_inv = nullptr; size_t elog_cap = 0; long elog_rows = 0;
@@ -304,13 +305,32 @@ int ensure_rp_obs(tdse_handle *h, int obs_every) {
     return TDSE_OK;
 }
 
+// field tables of a block of n steps: e_tab[(step*n_stage + stage)*B + b].  mode 0: Taylor / Lanczos (one value per step),
+// 1: classic RK4 stage times, 2: the stage times `cs` of any tableau.  Velocity gauge with pulses given by their field:
+// the running quadrature (field_table_quad_kernel), else the closed-form kernels.
+int enqueue_field_table(tdse_handle *h, int n, int mode, int n_stage, const StageTimes &cs, cudaStream_t s) {
+    const int B = h->grid.batch;
+    if (h->vg_quad) {
+        StageTimes c = cs;
+        if (mode == 1) { c.c[0] = 0.0; c.c[1] = 0.5; c.c[2] = 0.5; c.c[3] = 1.0; }
+        field_table_quad_kernel<<<(B + 63) / 64, 64, 0, s>>>(h->d_ctl, h->d_pulse, B, n, mode == 0 ? 1 : n_stage, c, mode == 0 ? 1 : 0,
+                                                             h->d_etab, h->d_arun);
+    } else if (mode == 2) {
+        field_table_rk_kernel<<<(n * n_stage * B + 255) / 256, 256, 0, s>>>(h->d_ctl, h->d_pulse, B, n, n_stage, cs, h->d_etab, h->gd.gauge);
+    } else {
+        field_table_kernel<<<(n * (mode == 1 ? 4 : 1) * B + 255) / 256, 256, 0, s>>>(h->d_ctl, h->d_pulse, B, n, mode, h->d_etab, h->gd.gauge);
+    }
+    count(h);
+    CU(cudaGetLastError());
+    return TDSE_OK;
+}
+
 int enqueue_taylor_block(tdse_handle *h, int order, int n, int obs, cudaStream_t s) {
     const int B = h->grid.batch;
     if (h->imag) {
         CU(cudaMemsetAsync(h->d_etab, 0, sizeof(double) * (size_t)n * B, s));       // no field
     } else {
-        field_table_kernel<<<(n * B + 255) / 256, 256, 0, s>>>(h->d_ctl, h->d_pulse, B, n, 0, h->d_etab, h->gd.gauge);
-        count(h);
+        RC(enqueue_field_table(h, n, 0, 1, StageTimes{}, s));
     }
     double2 *psi = h->pool[h->psi_slot];
     // scratch: three further pool slots
@@ -407,8 +427,7 @@ void fill_rk_common(tdse_handle *h, E &e, int stage, const double *ef, const dou
 
 int enqueue_rk4_block(tdse_handle *h, int n, int obs, cudaStream_t s) {
     const int B = h->grid.batch;
-    field_table_kernel<<<(n * 4 * B + 255) / 256, 256, 0, s>>>(h->d_ctl, h->d_pulse, B, n, 1, h->d_etab, h->gd.gauge);
-    count(h);
+    RC(enqueue_field_table(h, n, 1, 4, StageTimes{}, s));
     double2 *psi = h->pool[h->psi_slot];
     if (h->rk4_fused) {
         // all four stages in one pass over HBM (taylor_rp_kernel in RK mode); ping-pong psi <-> scratch
@@ -466,8 +485,7 @@ int enqueue_rk_generic_block(tdse_handle *h, int method, int n, int obs, cudaStr
     const RkTab &tb = kRkTabs[method];
     StageTimes cs{};
     for (int i = 0; i < 7; ++i) cs.c[i] = tb.c[i];
-    field_table_rk_kernel<<<(n * tb.s * B + 255) / 256, 256, 0, s>>>(h->d_ctl, h->d_pulse, B, n, tb.s, cs, h->d_etab, h->gd.gauge);
-    count(h);
+    RC(enqueue_field_table(h, n, 2, tb.s, cs, s));
     double2 *psi = h->pool[h->psi_slot];
     for (int i = 0; i < n; ++i) {
         for (int st = 0; st < tb.s; ++st) {
@@ -570,8 +588,7 @@ int enqueue_rk45_block(tdse_handle *h, int n, int first_stage, cudaStream_t s) {
 // written by the same kernel (halo race).
 int enqueue_lanczos_block(tdse_handle *h, int K, int order, int n, int obs, cudaStream_t s) {
     const int B = h->grid.batch;
-    field_table_kernel<<<(n * B + 255) / 256, 256, 0, s>>>(h->d_ctl, h->d_pulse, B, n, 0, h->d_etab, h->gd.gauge);
-    count(h);
+    RC(enqueue_field_table(h, n, 0, 1, StageTimes{}, s));
     double2 *psi = h->pool[h->psi_slot];
     double2 *wbuf[2]; int c = 0;
     for (int i = 0; c < 2; ++i) if (i != h->psi_slot) wbuf[c++] = h->pool[i];
@@ -703,6 +720,11 @@ int run_fixed(tdse_handle *h, int kind, int p1, int p2, double t0, double dt, lo
     v.t0 = t0; v.dt = dt; v.obs_every = obs_every; v.field_sample = h->field_sample;
     h->pending = 0;
     RC(init_ctl(h, v, stream));
+    if (h->vg_quad) {                   // A(t0) of the pulses given by their field (reading R-V4)
+        vecpot_init_kernel<<<B, 256, 0, stream>>>(h->d_ctl, h->d_pulse, h->d_arun);
+        count(h);
+        CU(cudaGetLastError());
+    }
     h->launches += h->pending;
     const int obs = obs_every > 0 ? 1 : 0;
     RC(run_blocks(h, kind, p1, p2, G, obs, nsteps / G, stream));
@@ -815,7 +837,7 @@ void tdse_destroy(tdse_handle *h) {
     free_graphs(h);
     for (double2 *p : h->pool) cudaFree(p);
     void *ptrs[] = {h->d_vj, h->d_cen, h->d_cl, h->d_pulse, h->d_bufs, h->d_ctl, h->d_etab, h->d_eapply, h->d_partials,
-                    h->d_counter, h->d_phi, h->d_lstate, h->d_obs_partials, h->d_obs_counters, h->d_elog, h->d_imag_inv, h->d_mask, h->d_pb, h->d_sigma, h->d_j0, h->d_loff, h->d_slist, h->d_yield, h->d_rp_part, h->d_rp_counter, h->d_rows, h->d_row_direct,
+                    h->d_counter, h->d_phi, h->d_lstate, h->d_obs_partials, h->d_obs_counters, h->d_elog, h->d_imag_inv, h->d_mask, h->d_pb, h->d_sigma, h->d_j0, h->d_arun, h->d_loff, h->d_slist, h->d_yield, h->d_rp_part, h->d_rp_counter, h->d_rows, h->d_row_direct,
                     h->d_dtlog, h->d_errlog, h->d_replay, h->d_alpha, h->d_beta, h->d_nrm, h->d_inv, h->d_coef,
                     h->d_m, h->d_nsub, h->d_basis};
     for (void *p : ptrs) if (p) cudaFree(p);
@@ -847,10 +869,19 @@ int tdse_set_option(tdse_handle *h, const char *key, double value) {
 
 int tdse_set_pulse(tdse_handle *h, const tdse_pulse *p) {
     if (!h || !p) return TDSE_ERR_ARG;
-    if (h->grid.gauge == 1)             // the velocity gauge needs A(t): kind-1 pulses (or the static test aid omega = 0)
-        for (int b = 0; b < h->grid.batch; ++b)
-            if (p[b].omega != 0.0 && p[b].kind != 1) return TDSE_ERR_UNSUPPORTED;
+    bool quad = false;                  // velocity gauge + a pulse given by its field: A(t) by the running quadrature
+    if (h->grid.gauge == 1)
+        for (int b = 0; b < h->grid.batch; ++b) {
+            if (p[b].kind != 0 && p[b].kind != 1) return TDSE_ERR_ARG;
+            if (p[b].omega != 0.0 && p[b].kind == 0) quad = true;
+        }
     CU(cudaDeviceSynchronize());
+    if (quad != h->vg_quad) free_graphs(h);
+    h->vg_quad = quad;
+    if (quad && !h->d_arun) {
+        CU(cudaMalloc(&h->d_arun, sizeof(double) * h->grid.batch));
+        CU(cudaMemset(h->d_arun, 0, sizeof(double) * h->grid.batch));
+    }
     CU(cudaMemcpy(h->d_pulse, p, sizeof(tdse_pulse) * h->grid.batch, cudaMemcpyHostToDevice));
     return TDSE_OK;
 }
@@ -1097,6 +1128,7 @@ int tdse_step_rk45(tdse_handle *h, double t0, double t_end, double dt_init, doub
                    long n_replay, long *n_accept, long *n_reject, void *stream) {
     if (!h || !(rtol > 0.0)) return TDSE_ERR_ARG;
     if (h->d_mask) return TDSE_ERR_UNSUPPORTED;      // the per-step mask of Eq. 18 presumes a fixed dt
+    if (h->vg_quad) return TDSE_ERR_UNSUPPORTED;     // (the running quadrature of A(t) is built for the fixed-step propagators)
     const bool replay = dt_replay != nullptr;
     if (replay ? (n_replay < 0) : (!(dt_init > 0.0) || !(t_end > t0))) return TDSE_ERR_ARG;
     cudaStream_t s = (cudaStream_t)stream;

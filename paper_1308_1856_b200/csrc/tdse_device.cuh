@@ -94,6 +94,25 @@ __device__ inline double pulse_A(const tdse_pulse &p, double t) {
     return -(p.e0 / p.omega) * s * s * sin(__dadd_rn(wt, p.cep));
 }
 
+// Velocity gauge with a pulse given by its FIELD (kind 0): A(t) exists only as the running quadrature of P:186-188,
+// A(t_{n+1}) = A(t_n) - int_{t_n}^{t_n + h} E dtau "using a standard 5-point Gaussian quadrature" (c dropped), and
+// A(t_n + c_i h) = A(t_n) - int_{t_n}^{t_n + c_i h} E dtau inside a step.
+__device__ __forceinline__ bool pulse_needs_quadrature(const tdse_pulse &p, int gauge) {
+    return gauge == 1 && p.omega != 0.0 && p.kind == 0;
+}
+// int_{ta}^{tb} E dtau by ONE 5-point Gauss-Legendre rule
+__device__ inline double gl5_field(const tdse_pulse &p, double ta, double tb) {
+    const double x1 = 0.5384693101056831, x2 = 0.9061798459386640;          // nodes on [-1, 1] (0, +-x1, +-x2)
+    const double w0 = 0.5688888888888889, w1 = 0.4786286704993665, w2 = 0.2369268850561891;
+    const double half = 0.5 * (tb - ta), mid = 0.5 * (tb + ta);
+    double s = w2 * pulse_E(p, mid - half * x2);
+    s += w1 * pulse_E(p, mid - half * x1);
+    s += w0 * pulse_E(p, mid);
+    s += w1 * pulse_E(p, mid + half * x1);
+    s += w2 * pulse_E(p, mid + half * x2);
+    return half * s;
+}
+
 // the time-dependent factor of the coupling: E(t) in the length gauge, A(t) in the velocity gauge
 __device__ inline double pulse_field(const tdse_pulse &p, double t, int gauge) {
     return gauge == 1 ? pulse_A(p, t) : pulse_E(p, t);

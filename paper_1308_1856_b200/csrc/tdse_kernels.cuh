@@ -580,6 +580,63 @@ __global__ void field_table_rk_kernel(const Ctl *ctl, const tdse_pulse *pulse, i
     }
 }
 
+// Velocity gauge, pulses given by their field (kind 0): the field tables come from the running quadrature of P:186-188 /
+// P:480.  a_run[b] holds A(t_n) of the first step of the block and is advanced past its last step; one thread per
+// member walks the steps in order (the sum is sequential by definition).  Members whose pulse has a closed-form A(t)
+// get exactly the values of field_table_kernel / field_table_rk_kernel.  e_tab[(step*n_stage + stage)*B + b].
+// mid_rule: 1 for Taylor / Lanczos (n_stage = 1, sample at t_n + dt/2 or, field_sample = 1, at t_n), 0 for stage times cs.
+__global__ void field_table_quad_kernel(const Ctl *ctl, const tdse_pulse *pulse, int B, int n_steps, int n_stage,
+                                        StageTimes cs, int mid_rule, double *e_tab, double *a_run) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    const tdse_pulse p = pulse[b];
+    const bool quad = pulse_needs_quadrature(p, 1);
+    const double t0 = ctl->t0, dt = ctl->dt;
+    const long long base = ctl->step_base;
+    double a = a_run[b];
+    for (int s = 0; s < n_steps; ++s) {
+        const double n = (double)(base + s);
+        const double tn = time_at(t0, n, dt);
+        for (int st = 0; st < n_stage; ++st) {
+            double v;
+            if (mid_rule) {
+                const bool at_start = ctl->field_sample == 1;
+                if (quad) v = at_start ? a : a - gl5_field(p, tn, tn + 0.5 * dt);
+                else v = pulse_A(p, at_start ? tn : time_at(t0, n + 0.5, dt));
+            } else {
+                const double c = cs.c[st];
+                if (quad) v = (c == 0.0) ? a : a - gl5_field(p, tn, tn + c * dt);
+                else v = pulse_A(p, __dadd_rn(tn, __dmul_rn(c, dt)));
+            }
+            e_tab[((size_t)s * n_stage + st) * B + b] = v;
+        }
+        if (quad) a -= gl5_field(p, tn, tn + dt);
+    }
+    a_run[b] = a;
+}
+
+// A(t0) of the members that need the quadrature (reading R-V4): minus the 5-point rule summed over the panels
+// [m dt, (m+1) dt] from 0 and the last partial panel up to t0.  grid = batch, block = 256.
+__global__ void __launch_bounds__(256) vecpot_init_kernel(const Ctl *ctl, const tdse_pulse *pulse, double *a_run) {
+    __shared__ double red_s[8];
+    const int b = blockIdx.x;
+    const tdse_pulse p = pulse[b];
+    const double t0 = ctl->t0, dt = ctl->dt;
+    double acc[1] = {0.0};
+    const bool quad = pulse_needs_quadrature(p, 1) && t0 > 0.0;
+    long long m = 0;
+    if (quad) {
+        m = (long long)floor(t0 / dt);
+        for (long long i = threadIdx.x; i < m; i += 256) acc[0] -= gl5_field(p, (double)i * dt, (double)(i + 1) * dt);
+    }
+    block_reduce<256, 1>(acc, red_s);
+    if (threadIdx.x == 0) {
+        double a = acc[0];
+        if (quad && t0 > (double)m * dt) a -= gl5_field(p, (double)m * dt, t0);
+        a_run[b] = quad ? a : 0.0;
+    }
+}
+
 __global__ void ctl_init_kernel(Ctl *c, CtlInit v) {
     if (threadIdx.x == 0 && blockIdx.x == 0) {
         c->t0 = v.t0; c->dt = v.dt; c->step_base = 0; c->obs_every = v.obs_every; c->field_sample = v.field_sample;

@@ -560,14 +560,46 @@ def test_gauge_agreement_of_the_ground_state_depletion_on_the_device(B):
     assert abs(dep[0] - dep[1]) <= 0.03 * dep[0]
 
 
-def test_velocity_gauge_needs_a_vector_potential_pulse(B):
-    """A kind-0 pulse has no A(t) here: the handle must refuse it instead of silently producing numbers."""
-    c = wl.config("cfg1", n_r=200, dr=0.2, n_l=4, fd_order=3)
+@pytest.mark.parametrize("prop", ["taylor", "rk4", "lanczos", "cashkarp"])
+def test_velocity_gauge_field_pulse_running_quadrature(B, prop):
+    """Velocity gauge under ORDINARY pulses (kind 0, given by their field): A(t) by the running 5-point Gauss quadrature
+    (P:186-188), A at the midpoint / stage times by P:480, a start inside the pulse (reading R-V4) -- every fixed-step
+    propagator against the oracle, members with different pulses, one of them with an analytic A (kind 1)."""
+    c = wl.config("cfg5", n_r=424, dr=0.1, n_l=7, fd_order=5, batch=3, order=4)
     g, h = both(B, c, gauge=1)
-    with pytest.raises(B.TdseError) as ei:
-        h.set_pulse([(0.05, 0.057, 2.0, 0.0)])
+    pulses = [(0.08, 0.3, 3.0, 0.0, 0), (0.05, 0.45, 2.0, 0.4, 0), (0.06, 0.3, 3.0, 0.2, 1)]
+    h.set_pulse(pulses)
+    g0 = oracle.make_grid(c["n_r"], c["dr"], c["n_l"], c["fd_order"], batch=3)
+    st = bound_pack(g0, [(0, 0), (1, 0)])
+    h.set_bound_states(*st)
+    psi0 = wl.populated_state(c)
+    dt = wl.dt_eff(c, "lanczos" if prop == "lanczos" else "rk4", 12 if prop == "lanczos" else 4)
+    t0, nsteps = 17.3, 37                       # inside all three pulses, not a multiple of dt; odd number of steps
+    h.set_state(psi0)
+    if prop == "taylor":
+        h.step_taylor(4, t0, dt, nsteps, 5)
+        ref, robs = oracle.step_taylor(g, pulses, psi0, 4, t0, dt, nsteps, states=st, obs_every=5)
+    elif prop == "rk4":
+        h.step_rk4(t0, dt, nsteps, 5)
+        ref, robs = oracle.step_rk4(g, pulses, psi0, t0, dt, nsteps, states=st, obs_every=5)
+    elif prop == "lanczos":
+        h.step_lanczos(10, 12, t0, dt, nsteps, 5)
+        ref, robs = oracle.step_lanczos(g, pulses, psi0, 10, 12, t0, dt, nsteps, states=st, obs_every=5)
+    else:
+        h.step_rk("cashkarp", t0, dt, nsteps, 5)
+        ref, _, robs = oracle.step_rk_method(g, pulses, psi0, "cashkarp", t0, dt, nsteps, states=st, obs_every=5)
+    got = h.get_state()
+    check_fixed(got, ref, h.obs_log(), robs)
+    for b in range(3):
+        assert rel_l2(got[b], ref[b]) <= TOL_PSI
+    # a second call continues from its own t0 (the running sum restarts from the panel rule): same as the oracle's
+    t1 = t0 + nsteps * dt
+    h.step_taylor(4, t1, dt, 8)
+    ref2, _ = oracle.step_taylor(g, pulses, ref, 4, t1, dt, 8)
+    assert rel_l2(h.get_state(), ref2) <= TOL_PSI
+    with pytest.raises(B.TdseError) as ei:      # the adaptive propagator is not served by the running quadrature
+        h.step_rk45(t1, t1 + 0.01, 1e-4, 1e-8)
     assert ei.value.code == -5
-    h.set_pulse([(0.05, 0.057, 2.0, 0.0, 1)])         # the same pulse with the Hann shape on A is accepted
     h.close()
 
 
