@@ -63,3 +63,24 @@ def test_product_does_not_import_oracle():
         if f.endswith((".py", ".cpp", ".h")):
             src = open(os.path.join(ROOT, "oracle", f)).read()
             assert "binding" not in src and "libtdse_b200" not in src and "csrc" not in src.replace("csrc/,", ""), f
+
+
+def test_bench_bound_state_inputs_match_the_oracle():
+    """bench.py's product arm may not touch oracle/, so it takes CFG5's bound states (every E < 0 eigenvector of the
+    discrete 3-point h_l) from LAPACK; they must be the same input data the GPU tests take from the oracle's eigen-solver."""
+    import numpy as np
+    import oracle
+    import bench
+    from paper_1308_1856_b200 import workloads as wl
+    c = wl.config("cfg5", n_r=400, n_l=4, batch=1)
+    ls, phis = bench.bound_state_inputs(c)
+    g = oracle.make_grid(c["n_r"], c["dr"], c["n_l"], 3)
+    k = 0
+    for l in range(c["n_l"]):
+        en, phi = oracle.bound_states(g, l, 32, only_negative=True)
+        assert list(ls[k:k + len(en)]) == [l] * len(en)
+        for i in range(len(en)):
+            assert abs(c["dr"] * np.sum(phis[k + i] ** 2) - 1.0) < 1e-12 and phis[k + i][0] > 0
+            assert np.max(np.abs(phis[k + i] - phi[i])) < 1e-8
+        k += len(en)
+    assert k == len(ls) and k >= 6
