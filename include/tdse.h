@@ -123,7 +123,9 @@ int  tdse_set_pulse(tdse_handle *h, const tdse_pulse *per_member_host);
 int  tdse_set_bound_states(tdse_handle *h, int n_states, const int *l_of_state, const double *phi);
 
 /* Copy the whole state [batch][n_l][n_r] complex128 in / out.  is_device = 0: host pointer (the call
- * synchronises `stream`), 1: device pointer (asynchronous on `stream`). */
+ * synchronises `stream`), 1: device pointer (asynchronous on `stream`), 2: PINNED host pointer, asynchronous on
+ * `stream` (the caller keeps the buffer alive and synchronises the stream itself: lets the transfers of one handle
+ * overlap the steps of another, e.g. a batch split over several handles and streams). */
 int  tdse_set_state(tdse_handle *h, const void *psi, int is_device, void *stream);
 int  tdse_get_state(tdse_handle *h, void *psi, int is_device, void *stream);
 

@@ -169,24 +169,29 @@ class Tdse:
         self.n_states = len(l_arr)
 
     # -- state
-    def set_state(self, psi, stream=None):
-        """psi: numpy complex128 array (host) or torch complex128 CUDA tensor, shape [batch][n_l][n_r]."""
+    def set_state(self, psi, stream=None, pinned_async=False):
+        """psi: numpy complex128 array (host) or torch complex128 CUDA tensor, shape [batch][n_l][n_r].
+        pinned_async: the numpy array lives in pinned memory and the copy is left asynchronous on the stream."""
         if isinstance(psi, np.ndarray):
             a = np.ascontiguousarray(psi, dtype=np.complex128)
             assert a.size == int(np.prod(self.shape))
-            _check(lib().tdse_set_state(self._h, C.c_void_p(a.ctypes.data), 0, _stream(stream)), "tdse_set_state")
+            assert not pinned_async or a is psi or a.ctypes.data == psi.ctypes.data
+            _check(lib().tdse_set_state(self._h, C.c_void_p(a.ctypes.data), 2 if pinned_async else 0, _stream(stream)),
+                   "tdse_set_state")
         else:
             t = psi.contiguous()
             assert t.is_cuda and t.numel() == int(np.prod(self.shape)) and t.element_size() == 16
             _check(lib().tdse_set_state(self._h, C.c_void_p(t.data_ptr()), 1, _stream(stream)), "tdse_set_state")
 
-    def get_state(self, out=None, stream=None):
-        """Returns a numpy array (out=None or numpy) or fills the given torch CUDA tensor."""
+    def get_state(self, out=None, stream=None, pinned_async=False):
+        """Returns a numpy array (out=None or numpy) or fills the given torch CUDA tensor.
+        pinned_async: `out` is a pinned numpy array; the copy is left asynchronous on the stream."""
         if out is None:
             out = np.empty(self.shape, dtype=np.complex128)
         if isinstance(out, np.ndarray):
             assert out.flags.c_contiguous and out.dtype == np.complex128
-            _check(lib().tdse_get_state(self._h, C.c_void_p(out.ctypes.data), 0, _stream(stream)), "tdse_get_state")
+            _check(lib().tdse_get_state(self._h, C.c_void_p(out.ctypes.data), 2 if pinned_async else 0, _stream(stream)),
+                   "tdse_get_state")
         else:
             assert out.is_cuda and out.is_contiguous() and out.element_size() == 16
             _check(lib().tdse_get_state(self._h, C.c_void_p(out.data_ptr()), 1, _stream(stream)), "tdse_get_state")

@@ -933,9 +933,10 @@ static int project_state(tdse_handle *h, cudaStream_t s) {
 int tdse_set_state(tdse_handle *h, const void *psi, int is_device, void *stream) {
     if (!h || !psi) return TDSE_ERR_ARG;
     cudaStream_t s = (cudaStream_t)stream;
+    if (is_device < 0 || is_device > 2) return TDSE_ERR_ARG;
     CU(cudaMemcpyAsync(h->pool[h->psi_slot], psi, h->n_state * sizeof(double2),
-                       is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s));
-    if (!is_device) CU(cudaStreamSynchronize(s));
+                       is_device == 1 ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s));
+    if (is_device == 0) CU(cudaStreamSynchronize(s));
     RC(project_state(h, s));                          // centrifugal cut-off (if set): the held points are zero from here on
     return TDSE_OK;
 }
@@ -943,9 +944,10 @@ int tdse_set_state(tdse_handle *h, const void *psi, int is_device, void *stream)
 int tdse_get_state(tdse_handle *h, void *psi, int is_device, void *stream) {
     if (!h || !psi) return TDSE_ERR_ARG;
     cudaStream_t s = (cudaStream_t)stream;
+    if (is_device < 0 || is_device > 2) return TDSE_ERR_ARG;
     CU(cudaMemcpyAsync(psi, h->pool[h->psi_slot], h->n_state * sizeof(double2),
-                       is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, s));
-    if (!is_device) CU(cudaStreamSynchronize(s));
+                       is_device == 1 ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, s));
+    if (is_device == 0) CU(cudaStreamSynchronize(s));
     return TDSE_OK;
 }
 
