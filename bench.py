@@ -536,7 +536,7 @@ def extra_measurements(binding, torch, stream, full_pulse=True):
                                  "us_per_attempted_step": ms * 1e3 / max(att, 1),
                                  "dt_mean": float(np.mean(info["dt"])) if len(info["dt"]) else None,
                                  "gpoint_updates_per_s": pts * 6 * att / (ms * 1e-3) / 1e9,
-                                 "timing": "CUDA events around the call (includes the controller's host checks)"}
+                                 "timing": "CUDA events around the call (one graph launch: the device runs the accept / reject loop)"}
         h.close()
         out["sweep"] = roofline_sweep(binding, torch, stream, peak)
         if full_pulse:

@@ -96,7 +96,10 @@ void tdse_destroy(tdse_handle *h);
  *                          faster); 2: wherever the kernel can; 0: always the separate observable kernels
  *   "lanczos_beta_tol" [1e-12] breakdown threshold on beta ("if beta = 0 then quit", R-G17)
  *   "rk45_dt_max"      [0 = none] cap on the adaptive step
- *   "rk45_check_every" [32] attempted steps enqueued between host checks of the device `done` flag */
+ *   "rk45_loop"        [1] tdse_step_rk45 runs as ONE graph launch: a CUDA-graph WHILE node repeats a block of attempted
+ *                          steps until the device controller is done (no host poll); 0: the host enqueues blocks and
+ *                          polls the `done` flag between them
+ *   "rk45_check_every" [8] attempted steps per block of that loop (or between host checks) */
 int  tdse_set_option(tdse_handle *h, const char *key, double value);
 
 /* Absorbing boundary (Eq. 18): W(r) = (i/dt) ln{1 - cos^p[(pi/2)(1 - r/r_b)]} enters as a split step, i.e.

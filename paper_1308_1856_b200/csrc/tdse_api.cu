@@ -93,7 +93,7 @@ struct tdse_handle {
     size_t n_state = 0;                 // complex elements per state vector (B*L*N)
     cudaError_t last_cuda = cudaSuccess;
     // options
-    int field_sample = 0, use_graph = 1, graph_steps = 16, taylor_block = 1, rk45_check_every = 32;
+    int field_sample = 0, use_graph = 1, graph_steps = 16, taylor_block = 1, rk45_check_every = 8;
     double beta_tol = 1e-12, rk45_dt_max = 0.0;
     // device tables
     double *d_vj = nullptr, *d_cen = nullptr, *d_cl = nullptr;
@@ -128,6 +128,7 @@ struct tdse_handle {
     std::map<std::tuple<int, int, int, int, int, int>, cudaGraphExec_t> graphs;
     std::map<std::tuple<int, int, int, int, int, int>, long> graph_nodes;
     long launches = 0; long pending = 0; long graph_inst = 0; bool capturing = false;
+    cudaGraphExec_t rk45_loop = nullptr; long rk45_loop_nodes = 0; int rk45_loop_G = 0, rk45_use_loop = 1;   // device-driven adaptive run
     int taylor_blocked_last = 0;        // 0: one kernel per order, 3: all orders in one pass (persistent register-patch kernel)
     // blocked Taylor configuration
     RpPlan rpp{}; int n_sm = 148; int rp_variant = -1, rp_tma = -1;
@@ -147,6 +148,7 @@ namespace {
 inline void count(tdse_handle *h) { ++h->pending; }
 
 void free_graphs(tdse_handle *h) {
+    if (h->rk45_loop) { cudaGraphExecDestroy(h->rk45_loop); h->rk45_loop = nullptr; }
     for (auto &kv : h->graphs) cudaGraphExecDestroy(kv.second);
     h->graphs.clear();
     h->graph_nodes.clear();
@@ -657,6 +659,43 @@ int enqueue_lanczos_block(tdse_handle *h, int K, int order, int n, int obs, cuda
     return TDSE_OK;
 }
 
+// The adaptive run as ONE graph launch: a WHILE node whose body is G attempted Dormand-Prince steps followed by the
+// condition kernel (go on while the device controller has not set `done`).  No host poll inside the run (the paper
+// enqueues kernels asynchronously to keep the device busy; its kernel boundaries exist only for global
+// synchronisation, P:484 -- the accept / reject decision is taken by the last CTA of the last stage on the device).
+int build_rk45_loop(tdse_handle *h, int G) {
+    if (h->rk45_loop && h->rk45_loop_G == G) return TDSE_OK;
+    if (h->rk45_loop) { cudaGraphExecDestroy(h->rk45_loop); h->rk45_loop = nullptr; }
+    cudaGraph_t g = nullptr;
+    CU(cudaGraphCreate(&g, 0));
+    auto fail = [&](int rc) { cudaGraphDestroy(g); cudaGetLastError(); return rc; };
+    cudaGraphConditionalHandle handle;
+    if (cudaGraphConditionalHandleCreate(&handle, g, 1, cudaGraphCondAssignDefault) != cudaSuccess) return fail(TDSE_ERR_CUDA);
+    cudaGraphNodeParams np{};
+    np.type = cudaGraphNodeTypeConditional;
+    np.conditional.handle = handle;
+    np.conditional.type = cudaGraphCondTypeWhile;
+    np.conditional.size = 1;
+    cudaGraphNode_t node;
+    if (cudaGraphAddNode(&node, g, nullptr, 0, &np) != cudaSuccess) return fail(TDSE_ERR_CUDA);
+    cudaGraph_t body = np.conditional.phGraph_out[0];
+    if (cudaStreamBeginCaptureToGraph(h->cap_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed) != cudaSuccess)
+        return fail(TDSE_ERR_CUDA);
+    h->pending = 0;
+    int rc = enqueue_rk45_block(h, G, 1, h->cap_stream);
+    rk45_cond_kernel<<<1, 32, 0, h->cap_stream>>>(h->d_ctl, handle);
+    ++h->pending;
+    cudaGraph_t captured = nullptr;
+    const cudaError_t ce = cudaStreamEndCapture(h->cap_stream, &captured);
+    if (rc != TDSE_OK || ce != cudaSuccess) return fail(rc != TDSE_OK ? rc : TDSE_ERR_CUDA);
+    cudaGraphExec_t ex = nullptr;
+    if (cudaGraphInstantiate(&ex, g, 0) != cudaSuccess) return fail(TDSE_ERR_CUDA);
+    cudaGraphDestroy(g);
+    h->rk45_loop = ex; h->rk45_loop_G = G; h->rk45_loop_nodes = h->pending;
+    ++h->graph_inst;
+    return TDSE_OK;
+}
+
 // ---- graph-captured time loop (row a7; NS: "the time loop is captured in a CUDA graph") ------------------
 enum Kind { KIND_TAYLOR = 1, KIND_RK4 = 2, KIND_LANCZOS = 3, KIND_RK45 = 4, KIND_RKGEN = 5 };
 
@@ -863,6 +902,7 @@ int tdse_set_option(tdse_handle *h, const char *key, double value) {
     else if (k == "lanczos_beta_tol") { if (!(value >= 0.0)) return TDSE_ERR_ARG; h->beta_tol = value; free_graphs(h); }
     else if (k == "rk45_dt_max") { if (!(value >= 0.0)) return TDSE_ERR_ARG; h->rk45_dt_max = value; }
     else if (k == "rk45_check_every") { if (value < 1 || value > 1024) return TDSE_ERR_ARG; h->rk45_check_every = (int)value; }
+    else if (k == "rk45_loop") { if (value != 0.0 && value != 1.0) return TDSE_ERR_ARG; h->rk45_use_loop = (int)value; }
     else return TDSE_ERR_ARG;
     return TDSE_OK;
 }
@@ -1179,6 +1219,19 @@ int tdse_step_rk45(tdse_handle *h, double t0, double t_end, double dt_init, doub
     h->launches += h->pending;
     const int G = std::max(1, h->rk45_check_every);
     Ctl hc{};
+    if (h->rk45_use_loop && h->use_graph && build_rk45_loop(h, G) == TDSE_OK) {
+        // device-driven: one graph launch runs blocks of G attempted steps until the controller is done
+        CU(cudaGraphLaunch(h->rk45_loop, s));
+        CU(cudaMemcpyAsync(&hc, h->d_ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, s));
+        CU(cudaStreamSynchronize(s));
+        h->launches += h->rk45_loop_nodes * ((hc.n_attempt - 1 + G - 1) / G);
+        h->psi_slot = h->role_slot[hc.perm[R_PSI]];
+        if (!hc.done) return TDSE_ERR_NONFINITE;            // the loop stopped on a step that is no positive number
+        h->last_accept = (long)hc.n_accept;
+        if (n_accept) *n_accept = (long)hc.n_accept;
+        if (n_reject) *n_reject = (long)hc.n_reject;
+        return TDSE_OK;
+    }
     for (;;) {
         CU(cudaMemcpyAsync(&hc, h->d_ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, s));
         CU(cudaStreamSynchronize(s));

@@ -651,6 +651,15 @@ __global__ void ctl_advance_kernel(Ctl *c, int n) {
     if (threadIdx.x == 0 && blockIdx.x == 0) c->step_base += n;
 }
 
+// Loop condition of the device-driven adaptive run (a CUDA-graph WHILE node around a block of attempted steps): go on
+// while the controller has not finished and its step is still a positive finite number.
+__global__ void rk45_cond_kernel(const Ctl *c, cudaGraphConditionalHandle handle) {
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        const bool stop = c->done || !(c->h > 0.0) || c->n_attempt > (1LL << 40);
+        cudaGraphSetConditional(handle, stop ? 0u : 1u);
+    }
+}
+
 // Start of an attempted Dormand-Prince step: clip the step to t_end (or take the replayed one) and tabulate
 // E_b(t + c_i h) for the 7 stages.  e_tab[stage*B + b].  One block.
 __global__ void rk45_begin_kernel(Ctl *c, const tdse_pulse *pulse, int B, const double *replay, double *e_tab,

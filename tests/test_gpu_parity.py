@@ -759,6 +759,41 @@ def test_rk45_batched_with_rejects(B):
     h.close()
 
 
+@pytest.mark.parametrize("check_every", [1, 5, 8])
+def test_rk45_device_loop_is_the_host_polled_run(B, check_every):
+    """The adaptive run as one graph launch (WHILE node around a block of attempted steps, option rk45_loop = 1) takes
+    exactly the decisions of the host-polled loop: same accepted-dt log, same error log, same reject count, bit-identical
+    state -- and a second run on the same handle re-uses the instantiated loop."""
+    c = wl.config("cfg5", n_r=333, n_l=6, batch=2, fd_order=5)
+    pulses = wl.pulses(c)
+    psi0 = wl.populated_state(c)
+    t0 = 0.5 * c["t_pulse"]
+    out = []
+    for loop in (0, 1):
+        g, h = both(B, c)
+        h.set_pulse(pulses)
+        h.set_option("rk45_loop", loop)
+        h.set_option("rk45_check_every", check_every)
+        h.set_state(psi0)
+        info = h.step_rk45(t0, t0 + 0.03, 5e-3, 1e-9)
+        psi = h.get_state()
+        if loop:
+            n_inst = h.graph_instantiations()
+            h.set_state(psi0)
+            again = h.step_rk45(t0, t0 + 0.03, 5e-3, 1e-9)
+            assert h.graph_instantiations() == n_inst
+            assert np.array_equal(again["dt"], info["dt"]) and np.array_equal(h.get_state(), psi)
+        out.append((info, psi))
+        h.close()
+    (a, pa), (b, pb) = out
+    assert a["n_reject"] >= 1 and a["n_accept"] > 20
+    assert (a["n_accept"], a["n_reject"]) == (b["n_accept"], b["n_reject"])
+    assert np.array_equal(a["dt"], b["dt"]) and np.array_equal(a["err"], b["err"])
+    assert np.array_equal(pa, pb)
+    ref, rinfo = oracle.step_rk45(g, pulses, psi0, t0, t0 + 0.03, 5e-3, 1e-9, dt_replay=b["dt"])
+    assert rel_l2(pb, ref) <= TOL_PSI
+
+
 def test_observables_direct(B):
     c = wl.config("cfg1", batch=2)
     g, h = both(B, c)
