@@ -96,7 +96,12 @@ void tdse_destroy(tdse_handle *h);
  *                          faster); 2: wherever the kernel can; 0: always the separate observable kernels
  *   "lanczos_beta_tol" [1e-12] breakdown threshold on beta ("if beta = 0 then quit", R-G17)
  *   "rk45_dt_max"      [0 = none] cap on the adaptive step
- *   "rk45_loop"        [1] tdse_step_rk45 runs as ONE graph launch: a CUDA-graph WHILE node repeats a block of attempted
+ *   "rk45_persist"     [1] tdse_step_rk45 runs as ONE persistent cooperative kernel when the grid fits the shared memory
+ *                          of the device (batch * n_l * ceil(n_r / #SMs) <= 2048 points per CTA, batch <= 32): psi and
+ *                          k_1..k_7 stay in shared memory from t0 to t_end, neighbouring CTAs hand their edge columns
+ *                          over through flags, every CTA runs the controller (the paper's kernel boundaries are
+ *                          its only global synchronisation); 0, or a larger grid: one kernel per stage, see below
+ *   "rk45_loop"        [1] (stage by stage) tdse_step_rk45 runs as ONE graph launch: a CUDA-graph WHILE node repeats a block of attempted
  *                          steps until the device controller is done (no host poll); 0: the host enqueues blocks and
  *                          polls the `done` flag between them
  *   "rk45_check_every" [8] attempted steps per block of that loop (or between host checks) */
@@ -208,6 +213,9 @@ long tdse_graph_instantiations(tdse_handle *h);
  * 0 one kernel per order, 3 persistent register-patch kernel with direct global loads, 4 the same with TMA tile
  * fetches (3, 4: all orders in one pass). */
 int  tdse_taylor_was_blocked(tdse_handle *h);
+/* 1 if the last tdse_step_rk45 call ran as the single persistent kernel (option "rk45_persist"), 0 if it ran stage by
+ * stage. */
+int  tdse_rk45_was_persistent(tdse_handle *h);
 
 const char *tdse_strerror(int code);
 const char *tdse_version(void);

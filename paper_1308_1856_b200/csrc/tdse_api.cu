@@ -15,6 +15,7 @@
 #include "tdse_kernels.cuh"
 #include "tdse_taylor_rp_plan.h"
 #include "tdse_tile_tma.cuh"
+#include "tdse_rk45_persist.cuh"
 
 using namespace tdse;
 
@@ -128,6 +129,8 @@ struct tdse_handle {
     std::map<std::tuple<int, int, int, int, int, int>, cudaGraphExec_t> graphs;
     std::map<std::tuple<int, int, int, int, int, int>, long> graph_nodes;
     long launches = 0; long pending = 0; long graph_inst = 0; bool capturing = false;
+    int rk45_persist = 1; int rk45_persist_last = 0;     // the whole adaptive run as one persistent kernel (small grids)
+    void *d_rkp_ws = nullptr; size_t rkp_ws_cap = 0;
     cudaGraphExec_t rk45_loop = nullptr; long rk45_loop_nodes = 0; int rk45_loop_G = 0, rk45_use_loop = 1;   // device-driven adaptive run
     int taylor_blocked_last = 0;        // 0: one kernel per order, 3: all orders in one pass (persistent register-patch kernel)
     // blocked Taylor configuration
@@ -697,6 +700,9 @@ int build_rk45_loop(tdse_handle *h, int G) {
 }
 
 // ---- graph-captured time loop (row a7; NS: "the time loop is captured in a CUDA graph") ------------------
+}  // namespace
+namespace tdse { int launch_rk45_persist(const RkpArgs &a, const RkpPlan &p, cudaStream_t s); }
+namespace {
 enum Kind { KIND_TAYLOR = 1, KIND_RK4 = 2, KIND_LANCZOS = 3, KIND_RK45 = 4, KIND_RKGEN = 5 };
 
 int enqueue_block(tdse_handle *h, int kind, int p1, int p2, int n, int obs, cudaStream_t s) {
@@ -878,7 +884,7 @@ void tdse_destroy(tdse_handle *h) {
     void *ptrs[] = {h->d_vj, h->d_cen, h->d_cl, h->d_pulse, h->d_bufs, h->d_ctl, h->d_etab, h->d_eapply, h->d_partials,
                     h->d_counter, h->d_phi, h->d_lstate, h->d_obs_partials, h->d_obs_counters, h->d_elog, h->d_imag_inv, h->d_mask, h->d_pb, h->d_sigma, h->d_j0, h->d_arun, h->d_loff, h->d_slist, h->d_yield, h->d_rp_part, h->d_rp_counter, h->d_rows, h->d_row_direct,
                     h->d_dtlog, h->d_errlog, h->d_replay, h->d_alpha, h->d_beta, h->d_nrm, h->d_inv, h->d_coef,
-                    h->d_m, h->d_nsub, h->d_basis};
+                    h->d_m, h->d_nsub, h->d_basis, h->d_rkp_ws};
     for (void *p : ptrs) if (p) cudaFree(p);
     if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
     cudaGetLastError();
@@ -902,6 +908,7 @@ int tdse_set_option(tdse_handle *h, const char *key, double value) {
     else if (k == "lanczos_beta_tol") { if (!(value >= 0.0)) return TDSE_ERR_ARG; h->beta_tol = value; free_graphs(h); }
     else if (k == "rk45_dt_max") { if (!(value >= 0.0)) return TDSE_ERR_ARG; h->rk45_dt_max = value; }
     else if (k == "rk45_check_every") { if (value < 1 || value > 1024) return TDSE_ERR_ARG; h->rk45_check_every = (int)value; }
+    else if (k == "rk45_persist") { if (value != 0.0 && value != 1.0) return TDSE_ERR_ARG; h->rk45_persist = (int)value; }
     else if (k == "rk45_loop") { if (value != 0.0 && value != 1.0) return TDSE_ERR_ARG; h->rk45_use_loop = (int)value; }
     else return TDSE_ERR_ARG;
     return TDSE_OK;
@@ -1175,11 +1182,23 @@ int tdse_step_rk45(tdse_handle *h, double t0, double t_end, double dt_init, doub
     if (replay ? (n_replay < 0) : (!(dt_init > 0.0) || !(t_end > t0))) return TDSE_ERR_ARG;
     cudaStream_t s = (cudaStream_t)stream;
     const int B = h->grid.batch;
-    RC(ensure_pool(h, kRkRoles));
+    // grids that fit the shared memory of the machine: the whole run is one persistent kernel (tdse_rk45_persist.cuh)
+    RkpPlan pp{};
+    if (h->rk45_persist) {
+        int dev = 0, max_smem = 0, coop = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) == cudaSuccess && coop)
+            pp = rkp_plan(h->grid, h->n_sm, std::min(max_smem - 2048, kRkpMaxSmem));
+    }
+    h->rk45_persist_last = pp.ok;
     h->taylor_blocked_last = 0;
-    rk_roles(h);
-    RC(upload_bufs(h, kRkRoles, s));
-    RC(ensure_buf(h, &h->d_etab, &h->etab_cap, (size_t)std::max(1, h->graph_steps) * 7 * B));
+    if (!pp.ok) {
+        RC(ensure_pool(h, kRkRoles));
+        rk_roles(h);
+        RC(upload_bufs(h, kRkRoles, s));
+        RC(ensure_buf(h, &h->d_etab, &h->etab_cap, (size_t)std::max(1, h->graph_steps) * 7 * B));
+    }
     // logs
     const long want_log = replay ? std::max(1L, n_replay) : (1L << 20);
     if (h->log_cap < want_log) {
@@ -1214,6 +1233,38 @@ int tdse_step_rk45(tdse_handle *h, double t0, double t_end, double dt_init, doub
     if (!replay && v.dt_max > 0.0 && v.h > v.dt_max) v.h = v.dt_max;
     h->pending = 0;
     RC(init_ctl(h, v, s));
+    if (pp.ok) {
+        const size_t part_off = (pp.halo_bytes + 255) & ~(size_t)255, ws_bytes = part_off + pp.part_bytes;
+        if (h->rkp_ws_cap < ws_bytes) {
+            CU(cudaStreamSynchronize(s));
+            if (h->d_rkp_ws) cudaFree(h->d_rkp_ws);
+            h->d_rkp_ws = nullptr; h->rkp_ws_cap = 0;
+            CU(cudaMalloc(&h->d_rkp_ws, ws_bytes));
+            h->rkp_ws_cap = ws_bytes;
+        }
+        char *ws = (char *)h->d_rkp_ws;
+        RkpArgs a{};
+        a.g = h->gd; a.psi = h->pool[h->psi_slot]; a.ctl = h->d_ctl; a.pulse = h->d_pulse; a.replay = h->d_replay;
+        a.dt_log = h->d_dtlog; a.err_log = h->d_errlog;
+        a.halo = (unsigned long long *)ws; a.part = (unsigned long long *)(ws + part_off);
+        a.G = pp.G; a.Wc = pp.Wc; a.R = pp.R; a.pitch = pp.pitch;
+        for (int i = 0; i < 7; ++i) {
+            for (int j = 0; j < 7; ++j) a.a[i][j] = DP_A[i][j];
+            a.d_err[i] = DP_B[i] - DP_BH[i];
+        }
+        CU(cudaMemsetAsync(ws, 0, ws_bytes, s));        // no packet of an earlier run may carry a sequence number of this one
+        RC(launch_rk45_persist(a, pp, s));
+        count(h);
+        h->launches += h->pending;
+        Ctl hc{};
+        CU(cudaMemcpyAsync(&hc, h->d_ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, s));
+        CU(cudaStreamSynchronize(s));
+        if (!hc.done) return TDSE_ERR_NONFINITE;            // the run stopped on a step that is no positive number
+        h->last_accept = (long)hc.n_accept;
+        if (n_accept) *n_accept = (long)hc.n_accept;
+        if (n_reject) *n_reject = (long)hc.n_reject;
+        return TDSE_OK;
+    }
     // the first attempted step needs k_1 (no FSAL yet): run it eagerly with stage 0 included
     RC(enqueue_rk45_block(h, 1, 0, s));
     h->launches += h->pending;
@@ -1391,5 +1442,6 @@ int tdse_bound_population(tdse_handle *h, double r_b, double *out_host, void *st
 }
 
 int tdse_taylor_was_blocked(tdse_handle *h) { return h ? h->taylor_blocked_last + ((h->taylor_blocked_last == 3 && h->rpp.tma) ? 1 : 0) : 0; }
+int tdse_rk45_was_persistent(tdse_handle *h) { return h ? h->rk45_persist_last : 0; }
 
 }  // extern "C"

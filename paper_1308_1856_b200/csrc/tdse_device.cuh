@@ -225,4 +225,46 @@ __device__ __forceinline__ void grid_finish(const RedCtx &rc, int total_ctas, in
     }
 }
 
+// (H f)_{l,j} from the five/seven neighbouring values (Eq. 11).  d = l(l+1)/(2r^2) - Z/r + kinetic diagonal.
+template <int FD>
+__device__ __forceinline__ double2 h_point(const GridDev &g, double d, double er, double cm, double cp,
+                                           double2 f, double2 fm1, double2 fp1, double2 fm2, double2 fp2,
+                                           double2 lo, double2 up) {
+    double2 h;
+    double kx = g.c1 * (fp1.x + fm1.x), ky = g.c1 * (fp1.y + fm1.y);
+    if (FD == 5) {
+        kx = fma(g.c2, fp2.x + fm2.x, kx);
+        ky = fma(g.c2, fp2.y + fm2.y, ky);
+    }
+    const double cx = fma(cp, up.x, cm * lo.x), cy = fma(cp, up.y, cm * lo.y);
+    h.x = fma(er, cx, fma(d, f.x, kx));
+    h.y = fma(er, cy, fma(d, f.y, ky));
+    return h;
+}
+
+// Velocity-gauge coupling added to h (Eq. 12 in reading R-V2; afield = A(t)):
+//   -i A [ c_{l-1} (d/dr - l/r) f_{l-1} + c_l (d/dr + (l+1)/r) f_{l+1} ],  d/dr by P:119 Eq. 14 (R-V1).
+// c points at (l, j) of a shared-memory tile with row pitch `pitch` that holds the rows l-1 and l+1 with their radial halo.
+template <int FD>
+__device__ __forceinline__ void vg_couple(const GridDev &g, const double2 *c, int pitch, int l, double rinv, double cm,
+                                          double cp, double afield, double2 lo, double2 up, double2 &h) {
+    const double2 *cl_ = c - pitch, *cu_ = c + pitch;
+    double dlx, dly, dux, duy;
+    if (FD == 3) {
+        const double w = 0.5 / g.dr;
+        dlx = w * (cl_[1].x - cl_[-1].x); dly = w * (cl_[1].y - cl_[-1].y);
+        dux = w * (cu_[1].x - cu_[-1].x); duy = w * (cu_[1].y - cu_[-1].y);
+    } else {
+        const double w = 1.0 / (12.0 * g.dr);
+        dlx = w * (8.0 * (cl_[1].x - cl_[-1].x) - (cl_[2].x - cl_[-2].x));
+        dly = w * (8.0 * (cl_[1].y - cl_[-1].y) - (cl_[2].y - cl_[-2].y));
+        dux = w * (8.0 * (cu_[1].x - cu_[-1].x) - (cu_[2].x - cu_[-2].x));
+        duy = w * (8.0 * (cu_[1].y - cu_[-1].y) - (cu_[2].y - cu_[-2].y));
+    }
+    const double sx = cm * (dlx - (double)l * rinv * lo.x) + cp * (dux + (double)(l + 1) * rinv * up.x);
+    const double sy = cm * (dly - (double)l * rinv * lo.y) + cp * (duy + (double)(l + 1) * rinv * up.y);
+    h.x = fma(afield, sy, h.x);              // -i (sx + i sy) = sy - i sx
+    h.y = fma(-afield, sx, h.y);
+}
+
 }  // namespace tdse

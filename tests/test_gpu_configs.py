@@ -74,13 +74,16 @@ def test_cfg1_full_pulse_every_step(B):
     h.close()
 
 
-def test_cfg2_adaptive_rk45_full_size(B):
+@pytest.mark.parametrize("persist", [1, 0])
+def test_cfg2_adaptive_rk45_full_size(B, persist):
     """CFG2's second propagator at CFG2's own size (4000 x 32, 5-point): embedded Dormand-Prince 5(4), rtol 1e-8,
-    adaptive dt over a 0.05 au window at the pulse peak.  Protocol R-G20: the oracle replays the accepted-dt sequence of
-    the CUDA run, must itself find err <= 1.05 on every step, and the final states agree to 1e-9."""
+    adaptive dt over a 0.05 au window at the pulse peak, as the persistent cooperative kernel (the default at this size)
+    and stage by stage.  Protocol R-G20: the oracle replays the accepted-dt sequence of the CUDA run, must itself find
+    err <= 1.05 on every step, and the final states agree to 1e-9."""
     c = wl.config("cfg2")
     g = oracle.make_grid(c["n_r"], c["dr"], c["n_l"], c["fd_order"])
     h = B.Tdse(c["n_r"], c["dr"], c["n_l"], c["fd_order"])
+    h.set_option("rk45_persist", persist)
     pulses = wl.pulses(c)
     h.set_pulse(pulses)
     psi0 = wl.populated_state(c)
@@ -88,6 +91,7 @@ def test_cfg2_adaptive_rk45_full_size(B):
     t1 = t0 + 0.05
     h.set_state(psi0)
     info = h.step_rk45(t0, t1, 1e-5, c["rtol"])
+    assert h.rk45_was_persistent() == bool(persist)
     got = h.get_state()
     assert info["n_accept"] > 500 and len(info["dt"]) == info["n_accept"]     # stability-limited: dt ~ 1/rho(H)
     assert abs(np.sum(info["dt"]) - (t1 - t0)) <= 1e-12

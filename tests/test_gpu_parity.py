@@ -706,11 +706,14 @@ def test_lanczos_breakdown_field_free_eigenstate(B):
     h.close()
 
 
-def test_rk45_adaptive_replay_parity(B):
-    """Adaptive DP5(4) on the GPU; the oracle replays the GPU's accepted-dt sequence (R-G20) and must agree on the final
-    state; the oracle's own adaptive run must make the same number of decisions; the GPU replays the oracle's list."""
+@pytest.mark.parametrize("persist", [1, 0])
+def test_rk45_adaptive_replay_parity(B, persist):
+    """Adaptive DP5(4) on the GPU (persist = 1: the whole run as one persistent cooperative kernel, 0: one kernel per
+    stage); the oracle replays the GPU's accepted-dt sequence (R-G20) and must agree on the final state; the oracle's own
+    adaptive run must make the same number of decisions; the GPU replays the oracle's list."""
     c = wl.config("cfg2", n_r=500, n_l=6)
     g, h = both(B, c)
+    h.set_option("rk45_persist", persist)
     pulses = wl.pulses(c)
     h.set_pulse(pulses)
     psi0 = wl.populated_state(c)
@@ -719,6 +722,7 @@ def test_rk45_adaptive_replay_parity(B):
     rtol = 1e-8
     h.set_state(psi0)
     info = h.step_rk45(t0, t1, 1e-4, rtol)
+    assert h.rk45_was_persistent() == bool(persist)
     got = h.get_state()
     assert info["n_accept"] > 20 and len(info["dt"]) == info["n_accept"]
     assert abs(np.sum(info["dt"]) - (t1 - t0)) <= 1e-12
@@ -744,15 +748,20 @@ def test_rk45_adaptive_replay_parity(B):
     h.close()
 
 
-def test_rk45_batched_with_rejects(B):
-    c = wl.config("cfg5", n_r=200, n_l=5, batch=3, fd_order=5)
+@pytest.mark.parametrize("persist,n_r,fd", [(1, 200, 5), (0, 200, 5), (1, 333, 3), (1, 7, 5), (1, 1200, 5)])
+def test_rk45_batched_with_rejects(B, persist, n_r, fd):
+    """Three members, a first step far too large (rejects), both forms of the run; ragged column blocks (333 = 83 x 4 + 1
+    is re-planned so that the last CTA owns a stencil half-width), a grid of one CTA, several points per thread."""
+    c = wl.config("cfg5", n_r=n_r, n_l=5, batch=3, fd_order=fd)
     g, h = both(B, c)
+    h.set_option("rk45_persist", persist)
     pulses = wl.pulses(c)
     h.set_pulse(pulses)
     psi0 = wl.populated_state(c)
     t0 = 0.5 * c["t_pulse"]
     h.set_state(psi0)
     info = h.step_rk45(t0, t0 + 0.02, 5e-3, 1e-9)     # dt_init far too large: forces rejects
+    assert h.rk45_was_persistent() == bool(persist)
     assert info["n_reject"] >= 1
     ref, rinfo = oracle.step_rk45(g, pulses, psi0, t0, t0 + 0.02, 5e-3, 1e-9, dt_replay=info["dt"])
     assert rel_l2(h.get_state(), ref) <= TOL_PSI
@@ -772,6 +781,7 @@ def test_rk45_device_loop_is_the_host_polled_run(B, check_every):
     for loop in (0, 1):
         g, h = both(B, c)
         h.set_pulse(pulses)
+        h.set_option("rk45_persist", 0)
         h.set_option("rk45_loop", loop)
         h.set_option("rk45_check_every", check_every)
         h.set_state(psi0)
