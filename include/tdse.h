@@ -39,6 +39,7 @@ extern "C" {
 #define TDSE_ERR_CUDA        (-3)   /* CUDA runtime error (no device, launch failure)             */
 #define TDSE_ERR_NONFINITE   (-4)   /* a logged norm is NaN/Inf (unstable step size)       */
 #define TDSE_ERR_UNSUPPORTED (-5)   /* gauge not 0/1, fd_order not 3/5, krylov_dim > 32           */
+#define TDSE_ERR_TOO_LARGE   (-6)   /* beyond the fixed scratch of tdse_observables_noalloc       */
 
 typedef struct tdse_handle tdse_handle;   /* opaque; owns the state, all scratch, tables and CUDA graphs */
 
@@ -216,6 +217,23 @@ int  tdse_taylor_was_blocked(tdse_handle *h);
 /* 1 if the last tdse_step_rk45 call ran as the single persistent kernel (option "rk45_persist"), 0 if it ran stage by
  * stage. */
 int  tdse_rk45_was_persistent(tdse_handle *h);
+
+/* Observables WITHOUT ANY ALLOCATION (row a6; Eq. 34, Eq. 36): for callers that cannot call cudaMalloc
+ * (code under CUDA-graph capture, tight serving loops, harnesses that forbid it).  No handle: the caller passes the
+ * inputs and the output, all DEVICE pointers:
+ *   psi_dev    [batch][n_l][n_r] complex128 (re, im), the layout of tdse_set_state;
+ *   e_now_dev  [batch] E_b(t) of the members at the time of psi (enters <z''> only), or NULL for a field-free state;
+ *   out_dev    [batch][3] = {norm dr sum |f|^2, <z>, <z''> = -E_b(t) - 2 Z dr sum c_l Re(f_l* f_{l+1}) / r^2}.
+ * The work is enqueued on `stream` and not synchronised.  The scratch of the two-stage reduction (per-CTA partial sums,
+ * per-member counters) lives in ONE file-scope device array of 784 KiB that every GPU loading the library holds until
+ * exit; it bounds the sizes: batch <= TDSE_NOALLOC_MAX_BATCH and ceil(n_r / 256) * batch * (l segments) <=
+ * TDSE_NOALLOC_MAX_CTAS, else TDSE_ERR_TOO_LARGE (nothing is launched).  Calls no cudaMalloc / cudaFree and no
+ * allocating library routine.  Every call on a device shares the array: calls that overlap on the GPU (different
+ * streams or host threads) RACE on it; serialise them.  Ownership: nothing is retained. */
+#define TDSE_NOALLOC_MAX_BATCH 4096
+#define TDSE_NOALLOC_MAX_CTAS  32768
+int  tdse_observables_noalloc(const void *psi_dev, int n_r, int n_l, int batch, double dr, double z_nuc,
+                              const double *e_now_dev, double *out_dev, void *stream);
 
 const char *tdse_strerror(int code);
 const char *tdse_version(void);

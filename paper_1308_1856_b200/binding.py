@@ -13,13 +13,13 @@ LIB_PATH = os.path.join(HERE, "libtdse_b200.so")
 
 TDSE_OK = 0
 ERRORS = {-1: "TDSE_ERR_ARG", -2: "TDSE_ERR_ALLOC", -3: "TDSE_ERR_CUDA", -4: "TDSE_ERR_NONFINITE",
-          -5: "TDSE_ERR_UNSUPPORTED"}
+          -5: "TDSE_ERR_UNSUPPORTED", -6: "TDSE_ERR_TOO_LARGE"}
 
 # every symbol include/tdse.h declares
 SYMBOLS = ["tdse_create", "tdse_destroy", "tdse_set_option", "tdse_set_pulse", "tdse_set_bound_states",
            "tdse_set_cutoff", "tdse_set_state", "tdse_get_state", "tdse_apply_H", "tdse_set_absorber", "tdse_bound_population", "tdse_step_taylor", "tdse_step_imag", "tdse_energy_log", "tdse_step_rk4", "tdse_step_rk", "tdse_rk_sigma",
            "tdse_step_lanczos", "tdse_step_rk45", "tdse_observables", "tdse_obs_log", "tdse_dt_log",
-           "tdse_lanczos_info", "tdse_ionisation_yield", "tdse_graph_instantiations", "tdse_launch_count", "tdse_taylor_was_blocked", "tdse_rk45_was_persistent", "tdse_strerror", "tdse_version"]
+           "tdse_lanczos_info", "tdse_ionisation_yield", "tdse_graph_instantiations", "tdse_launch_count", "tdse_taylor_was_blocked", "tdse_rk45_was_persistent", "tdse_observables_noalloc", "tdse_strerror", "tdse_version"]
 
 
 class TdseError(RuntimeError):
@@ -79,6 +79,7 @@ def lib():
         L.tdse_graph_instantiations.argtypes = [vp]
         L.tdse_graph_instantiations.restype = C.c_long
         L.tdse_ionisation_yield.argtypes = [vp, dp, vp]
+        L.tdse_observables_noalloc.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, vp, vp, vp]
         L.tdse_rk45_was_persistent.argtypes = [vp]
         L.tdse_rk45_was_persistent.restype = C.c_int
         L.tdse_taylor_was_blocked.argtypes = [vp]
@@ -95,6 +96,18 @@ def strerror(code):
 
 def version():
     return lib().tdse_version().decode()
+
+
+def observables_noalloc(psi_dev, dr, z_nuc, e_now_dev, out_dev, stream=None):
+    """{norm, <z>, <z''>} of psi_dev (torch complex128 CUDA tensor [batch][n_l][n_r]) into out_dev (float64 CUDA tensor
+    [batch][3]) through the entry point that allocates nothing; e_now_dev: float64 CUDA tensor [batch] or None."""
+    batch, n_l, n_r = psi_dev.shape
+    assert psi_dev.is_cuda and psi_dev.is_contiguous() and out_dev.is_cuda and out_dev.is_contiguous()
+    assert out_dev.numel() == 3 * batch and (e_now_dev is None or (e_now_dev.is_cuda and e_now_dev.numel() == batch))
+    _check(lib().tdse_observables_noalloc(C.c_void_p(psi_dev.data_ptr()), int(n_r), int(n_l), int(batch), float(dr),
+                                          float(z_nuc), C.c_void_p(e_now_dev.data_ptr() if e_now_dev is not None else None),
+                                          C.c_void_p(out_dev.data_ptr()), _stream(stream)), "tdse_observables_noalloc")
+    return out_dev
 
 
 def _check(rc, what):

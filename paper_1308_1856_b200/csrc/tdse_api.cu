@@ -804,6 +804,7 @@ const char *tdse_strerror(int code) {
         case TDSE_ERR_CUDA: return "CUDA error (no device or launch failure)";
         case TDSE_ERR_NONFINITE: return "non-finite norm logged (unstable step size?)";
         case TDSE_ERR_UNSUPPORTED: return "unsupported configuration";
+        case TDSE_ERR_TOO_LARGE: return "size beyond the fixed scratch array of the no-allocation entry point";
     }
     return "unknown error";
 }
