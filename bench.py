@@ -525,18 +525,29 @@ def extra_measurements(binding, torch, stream, full_pulse=True):
         t_a = 0.5 * c["t_pulse"]
         h.set_state(psi0, stream=stream)
         h.step_rk45(t_a, t_a + 0.005, 1e-5, 1e-8, stream=stream)          # warm-up (graphs, controller)
-        h.set_state(psi0, stream=stream)
-        stream.synchronize()
-        info = {}
-        ms = timed(torch, stream, lambda: info.update(h.step_rk45(t_a, t_a + 0.05, 1e-5, 1e-8, stream=stream)))
-        att = info["n_accept"] + info["n_reject"]
+        def rk45_run(hh):
+            hh.set_state(psi0, stream=stream)
+            stream.synchronize()
+            info = {}
+            ms = timed(torch, stream, lambda: info.update(hh.step_rk45(t_a, t_a + 0.05, 1e-5, 1e-8, stream=stream)))
+            att = info["n_accept"] + info["n_reject"]
+            return info, ms, att
+        info, ms, att = rk45_run(h)
         pts = c["batch"] * c["n_l"] * c["n_r"]
         out["step_cfg2_rk45"] = {"propagator": "rk45 (Dormand-Prince, adaptive, rtol 1e-8)", "window_au": 0.05,
                                  "n_accept": info["n_accept"], "n_reject": info["n_reject"],
                                  "us_per_attempted_step": ms * 1e3 / max(att, 1),
                                  "dt_mean": float(np.mean(info["dt"])) if len(info["dt"]) else None,
                                  "gpoint_updates_per_s": pts * 6 * att / (ms * 1e-3) / 1e9,
-                                 "timing": "CUDA events around the call (one graph launch: the device runs the accept / reject loop)"}
+                                 "kernel": "one persistent cooperative kernel (psi and k_1..k_7 in shared memory)"
+                                           if h.rk45_was_persistent() else "one kernel per stage",
+                                 "timing": "CUDA events around the call (the device runs the accept / reject loop)"}
+        # the same run stage by stage (one graph launch: WHILE node around blocks of attempted steps)
+        h.set_option("rk45_persist", 0)
+        h.set_state(psi0, stream=stream)
+        h.step_rk45(t_a, t_a + 0.005, 1e-5, 1e-8, stream=stream)
+        info, ms, att = rk45_run(h)
+        out["step_cfg2_rk45"]["stage_by_stage_us_per_attempted_step"] = ms * 1e3 / max(att, 1)
         h.close()
         out["sweep"] = roofline_sweep(binding, torch, stream, peak)
         if full_pulse:

@@ -18,21 +18,24 @@
 // (tile_kernel<EpiRK>): only the order of the reductions differs.  No host interaction between t0 and t_end.
 #pragma once
 
+#include <type_traits>
+
 #include "tdse_device.cuh"
 
 namespace tdse {
 
 constexpr int kRkpThreads = 512;
-constexpr int kRkpMaxPT = 4;            // owned points per thread
+constexpr int kRkpMaxPT = 4;            // owned points per thread (k_1..k_7 in shared memory)
+constexpr int kRkpRegPT = 2;            // ... with psi and k_1..k_7 of the owned points in REGISTERS (the faster form)
 constexpr int kRkpMaxB = 32;            // members
 constexpr int kRkpMaxSmem = 224 * 1024; // dynamic shared memory of a CTA (the kernel has about 1 KB of static data besides)
 
-struct RkpPlan { int ok, G, Wc, R, pitch, smem; size_t halo_bytes, part_bytes; };
+struct RkpPlan { int ok, G, Wc, R, pitch, smem, kreg; size_t halo_bytes, part_bytes; };
 
-inline int rkp_smem_bytes(int R, int Wc, int pitch, int B, int G) {
+inline int rkp_smem_bytes(int R, int Wc, int pitch, int B, int G, int kreg) {
     const int NW = kRkpThreads / 32;
     const size_t P = (size_t)R * Wc;
-    return (int)(sizeof(double2) * (2 * (size_t)(R + 2) * pitch + 9 * P) +
+    return (int)(sizeof(double2) * (2 * (size_t)(R + 2) * pitch + (kreg ? 1 : 9) * P) +
                  sizeof(double) * (7 * B + 56 + 2 * (NW > B ? NW : B) + 2 * B + 2 * (size_t)G * B));
 }
 
@@ -59,7 +62,8 @@ inline RkpPlan rkp_plan(const tdse_grid &g, int n_sm, int max_smem) {
     p.R = (int)R;
     p.pitch = p.Wc + 2 * HW;
     if (R * p.Wc > (long)kRkpThreads * kRkpMaxPT) return p;
-    p.smem = rkp_smem_bytes(p.R, p.Wc, p.pitch, g.batch, p.G);
+    p.kreg = R * p.Wc <= (long)kRkpThreads * kRkpRegPT;
+    p.smem = rkp_smem_bytes(p.R, p.Wc, p.pitch, g.batch, p.G, p.kreg);
     if (p.smem > max_smem) return p;
     p.halo_bytes = (size_t)32 * 2 * p.G * 2 * p.R * HW;        // a complex value = 4 packets of 8 bytes
     p.part_bytes = (size_t)16 * 2 * p.G * g.batch * 2;         // a real value = 2 packets
@@ -87,6 +91,15 @@ __device__ __forceinline__ void ll_send(unsigned long long *dst, double v, unsig
     const unsigned long long w0 = hi | (unsigned int)__double2loint(v), w1 = hi | (unsigned int)__double2hiint(v);
     asm volatile("st.volatile.global.v2.u64 [%0], {%1, %2};" ::"l"(dst), "l"(w0), "l"(w1) : "memory");
 }
+__device__ __forceinline__ void ll_peek(const unsigned long long *src, unsigned long long &w0, unsigned long long &w1) {
+    asm volatile("ld.volatile.global.v2.u64 {%0, %1}, [%2];" : "=l"(w0), "=l"(w1) : "l"(src) : "memory");
+}
+// the value of a packet pair that was peeked at earlier (polls again while the sequence number is not the expected one)
+__device__ __forceinline__ double ll_finish(const unsigned long long *src, unsigned int seq, unsigned long long w0,
+                                            unsigned long long w1) {
+    while ((unsigned int)(w0 >> 32) != seq || (unsigned int)(w1 >> 32) != seq) ll_peek(src, w0, w1);
+    return __hiloint2double((int)(unsigned int)w1, (int)(unsigned int)w0);
+}
 __device__ __forceinline__ double ll_recv(const unsigned long long *src, unsigned int seq) {
     unsigned long long w0, w1;
     do {
@@ -95,19 +108,24 @@ __device__ __forceinline__ double ll_recv(const unsigned long long *src, unsigne
     return __hiloint2double((int)(unsigned int)w1, (int)(unsigned int)w0);
 }
 
-template <int FD, bool VG>
+template <int N> using RkpI = std::integral_constant<int, N>;
+
+// KREG: at most kRkpRegPT points per thread; psi and k_1..k_7 of a thread's points stay in its registers, shared memory
+// holds only the two copies of the stage vector (whose neighbours other threads read).
+template <int FD, bool VG, bool KREG>
 __global__ void __launch_bounds__(kRkpThreads, 1) rk45_persist_kernel(const __grid_constant__ RkpArgs a) {
     constexpr int HW = (FD == 3) ? 1 : 2;
-    constexpr int NT = kRkpThreads, NW = NT / 32, PT = kRkpMaxPT;
+    constexpr int NT = kRkpThreads, NW = NT / 32, PT = KREG ? kRkpRegPT : kRkpMaxPT;
     extern __shared__ __align__(16) unsigned char rkp_smem[];
     const GridDev &g = a.g;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int cta = blockIdx.x, G = a.G, R = a.R, pitch = a.pitch, B = g.batch, L = g.n_l;
     const int c0 = cta * a.Wc, wc = min(a.Wc, g.n_r - c0), P = R * wc, Pcap = R * a.Wc, TS = (R + 2) * pitch;
     double2 *tile = reinterpret_cast<double2 *>(rkp_smem);          // [2][(R + 2)][pitch]: zero rows above and below
-    double2 *psi_s = tile + 2 * (size_t)TS;                         // [P]   (slot p belongs to one thread)
-    double2 *k_s = psi_s + Pcap;                                    // [7][P]
-    double2 *ev = k_s + 7 * (size_t)Pcap;                           // [P] (|Delta|^2, |psi_new|^2), row-major over the owned block
+    double2 *psi_s = tile + 2 * (size_t)TS;                         // [P]   (slot p belongs to one thread)     } not with
+    double2 *k_s = psi_s + (KREG ? 0 : Pcap);                       // [7][P]                                   } KREG
+    double2 *ev = k_s + (KREG ? 0 : 7 * (size_t)Pcap);              // [P] (|Delta|^2, |psi_new|^2), row-major over the owned block
+    double2 kr[KREG ? 7 : 1][PT], pr[PT];                           // KREG: k_1..k_7 and psi of this thread's points
     double *etab = reinterpret_cast<double *>(ev + Pcap);           // [7][B] field values of the stages
     double *coef = etab + 7 * B;                                    // [7][7] h a_{sj}, then [7] h (b_j - bhat_j)
     double *csum = coef + 56;                                       // [max(NW, B)][2] chunk sums
@@ -125,11 +143,12 @@ __global__ void __launch_bounds__(kRkpThreads, 1) rk45_persist_kernel(const __gr
     int tix[PT], bb[PT], nix[PT], sl[PT], sr[PT];
     size_t gix[PT];
     double dd[PT], rj[PT], cm[PT], cp[PT];
-    bool own[PT], held[PT];
+    bool own[PT], held[PT], edge[PT];
 #pragma unroll
     for (int i = 0; i < PT; ++i) {
         const int p = tid + i * NT;
         own[i] = p < P;
+        edge[i] = p < nE;                   // its stencil reaches into a neighbouring CTA's columns
         int row = 0, col = 0;
         if (own[i]) {
             if (p < nE) { row = p / ec; const int e = p - row * ec; col = (e < HW) ? e : wc - (ec - e); }
@@ -161,7 +180,7 @@ __global__ void __launch_bounds__(kRkpThreads, 1) rk45_persist_kernel(const __gr
         if (own[i]) {
             double2 v = a.psi[gix[i]];
             if (held[i]) v = make_double2(0.0, 0.0);
-            psi_s[tid + i * NT] = v;
+            if constexpr (KREG) pr[i] = v; else psi_s[tid + i * NT] = v;
         }
     __syncthreads();
 
@@ -169,7 +188,8 @@ __global__ void __launch_bounds__(kRkpThreads, 1) rk45_persist_kernel(const __gr
     int cur = 0;                // which copy of the tile holds the stage vector being read
     // Form g_{s+1} = psi + sum_{j < s} (h a_{sj}) k_j at the owned points into the OTHER copy of the tile, send the edge
     // points to the neighbours as they are formed, receive theirs into the halo columns, switch the copies.
-    auto form = [&](const int s) {
+    auto form = [&](auto S) {
+        constexpr int s = decltype(S)::value;
         ++n_pub;
         const int par = (int)(n_pub & 1u);
         double2 *tn = tile + (cur ^ 1) * TS;
@@ -178,38 +198,59 @@ __global__ void __launch_bounds__(kRkpThreads, 1) rk45_persist_kernel(const __gr
         for (int i = 0; i < PT; ++i) {
             if (!own[i]) continue;
             const int p = tid + i * NT;
-            double2 acc = psi_s[p];
+            double2 acc;
+            if constexpr (KREG) acc = pr[i]; else acc = psi_s[p];
 #pragma unroll
             for (int j = 0; j < 6; ++j) {
                 if (j < s) {
                     const double aj = coef[s * 7 + j];
-                    if (aj != 0.0) acc = caxpy_r(aj, k_s[(size_t)j * Pcap + p], acc);
+                    double2 kj;
+                    if constexpr (KREG) kj = kr[KREG ? j : 0][i]; else kj = k_s[(size_t)j * Pcap + p];
+                    if (aj != 0.0) acc = caxpy_r(aj, kj, acc);
                 }
             }
             tn[tix[i]] = acc;
             if (sl[i] >= 0) { ll_send(mine + (size_t)sl[i] * 4, acc.x, n_pub); ll_send(mine + (size_t)sl[i] * 4 + 2, acc.y, n_pub); }
             if (sr[i] >= 0) { ll_send(mine + (size_t)(per + sr[i]) * 4, acc.x, n_pub); ll_send(mine + (size_t)(per + sr[i]) * 4 + 2, acc.y, n_pub); }
         }
-        for (int idx = tid; idx < 2 * per; idx += NT) {
-            const int side = idx / per, rem = idx - side * per, row = rem / HW, hh = rem - row * HW;
-            const int nb = side == 0 ? cta - 1 : cta + 1;
-            if (nb < 0 || nb >= G) continue;                   // the wall: the halo stays zero
-            // the left neighbour's RIGHT edge / the right neighbour's LEFT edge
-            const unsigned long long *src = a.halo + ((size_t)(par * G + nb) * 2 * per + (size_t)(1 - side) * per + rem) * 4;
-            double2 v;
-            v.x = ll_recv(src, n_pub);
-            v.y = ll_recv(src + 2, n_pub);
-            tn[(row + 1) * pitch + (side == 0 ? hh : HW + wc + hh)] = v;
+    };
+    // The neighbours' edge columns -> the halo columns of the copy being formed.  The first packets of a thread are
+    // requested BEFORE the interior points are worked on and looked at afterwards: the trip through L2 hides behind them.
+    unsigned long long hw0 = 0, hw1 = 0, hw2 = 0, hw3 = 0;
+    auto halo_src = [&](const int idx, int &dst) -> const unsigned long long * {
+        const int par = (int)(n_pub & 1u);
+        const int side = idx / per, rem = idx - side * per, row = rem / HW, hh = rem - row * HW;
+        const int nb = side == 0 ? cta - 1 : cta + 1;
+        if (nb < 0 || nb >= G) return nullptr;                 // the wall: the halo stays zero
+        dst = (row + 1) * pitch + (side == 0 ? hh : HW + wc + hh);
+        // the left neighbour's RIGHT edge / the right neighbour's LEFT edge
+        return a.halo + ((size_t)(par * G + nb) * 2 * per + (size_t)(1 - side) * per + rem) * 4;
+    };
+    auto halo_request = [&]() {
+        int dst;
+        if (tid < 2 * per) {
+            const unsigned long long *src = halo_src(tid, dst);
+            if (src) { ll_peek(src, hw0, hw1); ll_peek(src + 2, hw2, hw3); }
         }
-        __syncthreads();
-        cur ^= 1;
+    };
+    auto halo_receive = [&]() {
+        double2 *tn = tile + (cur ^ 1) * TS;
+        for (int idx = tid; idx < 2 * per; idx += NT) {
+            int dst;
+            const unsigned long long *src = halo_src(idx, dst);
+            if (!src) continue;
+            double2 v;
+            if (idx == tid) { v.x = ll_finish(src, n_pub, hw0, hw1); v.y = ll_finish(src + 2, n_pub, hw2, hw3); }
+            else { v.x = ll_recv(src, n_pub); v.y = ll_recv(src + 2, n_pub); }
+            tn[dst] = v;
+        }
     };
     // k_s = -i H(t + c_s h) g_s at the owned points, g_s = the vector in the current copy of the tile
-    auto apply = [&](const int s) {
-        const double2 *tc = tile + cur * TS;
+    auto apply = [&](auto S, const double2 *tc, const bool edge_points) {
+        constexpr int s = decltype(S)::value;
 #pragma unroll
         for (int i = 0; i < PT; ++i) {
-            if (!own[i]) continue;
+            if (!own[i] || edge[i] != edge_points) continue;
             const double2 *cpt = tc + tix[i];
             const double2 f = cpt[0], fm1 = cpt[-1], fp1 = cpt[1];
             double2 fm2 = fm1, fp2 = fp1;
@@ -222,8 +263,22 @@ __global__ void __launch_bounds__(kRkpThreads, 1) rk45_persist_kernel(const __gr
                 vg_couple<FD>(g, cpt, pitch, l, 1.0 / rj[i], cm[i], cp[i], afield, lo, up, h);
             }
             if (held[i]) h = make_double2(0.0, 0.0);
-            k_s[(size_t)s * Pcap + tid + i * NT] = make_double2(h.y, -h.x);
+            if constexpr (KREG) kr[KREG ? s : 0][i] = make_double2(h.y, -h.x);
+            else k_s[(size_t)s * Pcap + tid + i * NT] = make_double2(h.y, -h.x);
         }
+    };
+    // one stage: form g_{s+1} (edge points first, sent at once), then k_{s+1} = -i H g_{s+1}: interior points while the
+    // neighbours' packets travel, edge points once they are in
+    auto stage = [&](auto S) {
+        form(S);
+        halo_request();
+        __syncthreads();
+        const double2 *tn = tile + (cur ^ 1) * TS;
+        apply(S, tn, false);
+        halo_receive();
+        __syncthreads();
+        apply(S, tn, true);
+        cur ^= 1;
     };
 
     bool have_k1 = false;
@@ -247,15 +302,16 @@ __global__ void __launch_bounds__(kRkpThreads, 1) rk45_persist_kernel(const __gr
         else if (tid < 56) coef[tid] = hh * a.d_err[tid - 49];
         __syncthreads();
         if (!have_k1) {         // the first attempted step: k_1 = -i H(t) psi (afterwards FSAL supplies it)
-            form(0);
-            apply(0);
+            stage(RkpI<0>{});
             have_k1 = true;
         }
         // ---- stages 2..7: g_{s+1} = psi + h sum_j a_{s+1,j} k_j, then k_{s+1}; the last one is psi_new and k_7 -------------
-        for (int s = 1; s < 7; ++s) {
-            form(s);
-            apply(s);
-        }
+        stage(RkpI<1>{});
+        stage(RkpI<2>{});
+        stage(RkpI<3>{});
+        stage(RkpI<4>{});
+        stage(RkpI<5>{});
+        stage(RkpI<6>{});
         // ---- embedded error estimate: Delta = h sum_j (b_j - bhat_j) k_j against psi_new ---------------------------
         {
             const double2 *tc = tile + cur * TS;
@@ -267,7 +323,9 @@ __global__ void __launch_bounds__(kRkpThreads, 1) rk45_persist_kernel(const __gr
 #pragma unroll
                 for (int j = 0; j < 7; ++j) {
                     const double dj = coef[49 + j];
-                    if (dj != 0.0) d = caxpy_r(dj, k_s[(size_t)j * Pcap + p], d);
+                    double2 kj;
+                    if constexpr (KREG) kj = kr[KREG ? j : 0][i]; else kj = k_s[(size_t)j * Pcap + p];
+                    if (dj != 0.0) d = caxpy_r(dj, kj, d);
                 }
                 const double2 f = tc[tix[i]];
                 ev[nix[i]] = make_double2(d.x * d.x + d.y * d.y, f.x * f.x + f.y * f.y);
@@ -359,8 +417,8 @@ __global__ void __launch_bounds__(kRkpThreads, 1) rk45_persist_kernel(const __gr
             for (int i = 0; i < PT; ++i) {
                 if (!own[i]) continue;
                 const int p = tid + i * NT;
-                psi_s[p] = tc[tix[i]];
-                k_s[p] = k_s[(size_t)6 * Pcap + p];
+                if constexpr (KREG) { pr[i] = tc[tix[i]]; kr[0][i] = kr[KREG ? 6 : 0][i]; }
+                else { psi_s[p] = tc[tix[i]]; k_s[p] = k_s[(size_t)6 * Pcap + p]; }
             }
         }
         __syncthreads();
@@ -368,7 +426,9 @@ __global__ void __launch_bounds__(kRkpThreads, 1) rk45_persist_kernel(const __gr
 
 #pragma unroll
     for (int i = 0; i < PT; ++i)
-        if (own[i]) a.psi[gix[i]] = psi_s[tid + i * NT];
+        if (own[i]) {
+            if constexpr (KREG) a.psi[gix[i]] = pr[i]; else a.psi[gix[i]] = psi_s[tid + i * NT];
+        }
     if (cta == 0 && tid == 0) {
         Ctl &s = *a.ctl;
         s.t = c.t; s.h = c.h; s.done = c.done; s.last = c.last; s.after_reject = c.after_reject;
