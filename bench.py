@@ -539,7 +539,7 @@ def extra_measurements(binding, torch, stream, full_pulse=True):
                                  "us_per_attempted_step": ms * 1e3 / max(att, 1),
                                  "dt_mean": float(np.mean(info["dt"])) if len(info["dt"]) else None,
                                  "gpoint_updates_per_s": pts * 6 * att / (ms * 1e-3) / 1e9,
-                                 "kernel": "one persistent cooperative kernel (psi and k_1..k_7 in shared memory)"
+                                 "kernel": "one persistent cooperative kernel (psi and k_1..k_7 on chip from t0 to t_end)"
                                            if h.rk45_was_persistent() else "one kernel per stage",
                                  "timing": "CUDA events around the call (the device runs the accept / reject loop)"}
         # the same run stage by stage (one graph launch: WHILE node around blocks of attempted steps)
