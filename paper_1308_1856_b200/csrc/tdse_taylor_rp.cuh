@@ -153,11 +153,13 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
     if (OBS) obs_setup(0);
     bool any_obs = obs_now;                                  // some step of this launch is a logged one
     const bool obs_direct = (n_tiles * csize == 1);         // the CTA owns the whole member: it writes the row itself
-    auto write_row = [&](const int bb, const double (&s)[kRpObsRed]) {
+    // (with_field = false: the -E(t) term of <z''> is added afterwards by add_field, many rows at a time)
+    auto write_row = [&](const int bb, const double (&s)[kRpObsRed], const bool with_field) {
         double *o = ob.rows + ((size_t)obs_row * g.batch + bb) * (3 + ob.n_states);
         o[0] = g.dr * s[0];
         o[1] = 2.0 * g.dr * s[1];
-        o[2] = -pulse_E(ob.pulse[bb], obs_t) - 2.0 * g.z * g.dr * s[2];
+        const double acc = 2.0 * g.z * g.dr * s[2];
+        o[2] = with_field ? -pulse_E(ob.pulse[bb], obs_t) - acc : -acc;
         for (int si = 0; si < ob.n_states && si < kRpObsStates; ++si) {
             const double ar = g.dr * s[3 + 2 * si], ai = g.dr * s[4 + 2 * si];
             o[3 + si] = ar * ar + ai * ai;
@@ -629,7 +631,7 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                             for (int w2 = 0; w2 < NWR * NWC; ++w2) v += sm.red[w2][i];
                             sred[i] = v;
                         }
-                        write_row(b, sred);
+                        write_row(b, sred, true);
                     }
                     __syncthreads();            // sm.red is free again (the next step may come soon)
                 } else if (threadIdx.x < kRpObsRed) {
@@ -683,7 +685,28 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
         if (!sm.last_flag) return;
         __threadfence();
         const int per = n_tiles * csize;
-        for (int st = 0; st < (PERSIST ? n_steps : 1); ++st) {
+        const int n_st = PERSIST ? n_steps : 1;
+        if (per <= 16) {
+            // few partials per member (small grids): one THREAD per (step, member) adds them in a fixed order and
+            // writes the row, field value included -- no barriers, every row of the launch at the same time
+            for (int idx = threadIdx.x; idx < n_st * g.batch; idx += G::NT) {
+                const int st = idx / g.batch, bb = idx - st * g.batch;
+                obs_setup(st);
+                if (!obs_now) continue;
+                double s[kRpObsRed];
+#pragma unroll
+                for (int j = 0; j < kRpObsRed; ++j) s[j] = 0.0;
+                const double *pp = ob.partials + ((size_t)st * n_items * csize + (size_t)bb * per) * kRpObsRed;
+                for (int i = 0; i < per; ++i) {
+#pragma unroll
+                    for (int j = 0; j < kRpObsRed; ++j) s[j] += __ldcg(pp + (size_t)i * kRpObsRed + j);
+                }
+                write_row(bb, s, true);
+            }
+            if (threadIdx.x == 0) *ob.counter = 0u;
+            return;
+        }
+        for (int st = 0; st < n_st; ++st) {
         obs_setup(st);
         if (!obs_now) continue;
         constexpr int NW = NWR * NWC;
@@ -706,7 +729,7 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                 for (int off = 16; off > 0; off >>= 1) s[j] += __shfl_down_sync(0xffffffffu, s[j], off);
             }
             if (by_warp) {
-                if (lane == 0) write_row(bb, s);
+                if (lane == 0) write_row(bb, s, false);
             } else {
                 __syncthreads();
                 if (lane == 0) {
@@ -721,11 +744,21 @@ taylor_rp_kernel(GridDev g, const double2 *__restrict__ in, double2 *__restrict_
                         for (int w2 = 0; w2 < NW; ++w2) v += sm.red[w2][j];
                         s[j] = v;
                     }
-                    write_row(bb, s);
+                    write_row(bb, s, false);
                 }
             }
         }
         }   // step of the launch
+        // <z''> = -E(t) - ...: the field values of all rows of the launch, one (step, member) per thread -- a serial
+        // evaluation per row (three divisions, a sine and a cosine in one thread) would cost more than the sums
+        __syncthreads();
+        for (int idx = threadIdx.x; idx < n_st * g.batch; idx += G::NT) {
+            const int st = idx / g.batch, bb = idx - st * g.batch;
+            obs_setup(st);
+            if (!obs_now) continue;
+            double *o = ob.rows + ((size_t)obs_row * g.batch + bb) * (3 + ob.n_states);
+            o[2] = o[2] - pulse_E(ob.pulse[bb], obs_t);
+        }
         if (threadIdx.x == 0) *ob.counter = 0u;
     }
 }
