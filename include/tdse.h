@@ -74,7 +74,8 @@ void tdse_destroy(tdse_handle *h);
 /* Options (all default to the value in brackets):
  *   "field_sample"     [0] 0: H frozen at t_n + dt/2 in Taylor/Lanczos steps, 1: at t_n (R-G7)
  *   "use_graph"        [1] capture blocks of steps in a CUDA graph
- *   "graph_steps"      [16] steps per captured graph
+ *   "graph_steps"      [16] steps per captured graph (four times as many on the small grids whose launches take
+ *                          several steps, option "persist")
  *   "apply_tma"        [1] tdse_apply_H: tiles fetched by TMA tensor copies (zero fill outside the index box by the
  *                          hardware) when n_r % 8 == 0 and the grid is many rounds of
  *                          resident CTAs; 2: whenever the layout allows it; 0: the (l, r) tile kernel
@@ -84,7 +85,8 @@ void tdse_destroy(tdse_handle *h);
  *                          when the grid is at least one 128-column tile wide; 0 one kernel per stage
  *   "taylor_block"     [1] 0: one kernel per Taylor order; 1: temporally blocked step, all orders in one
  *                          pass over HBM (persistent register-patch kernel; n_l <= 128, else falls back to 0)
- *   "taylor_rp_variant" [-1] instantiation of the register-patch kernel (-1: heuristic)
+ *   "taylor_rp_variant" [-1] instantiation of the register-patch kernel (-1: heuristic; 0..4: 16 points per thread,
+ *                          5..7: 8 points per thread, multi-step launches only)
  *   "taylor_rp_tma"    [-1] register-patch kernel: fetch tiles by TMA tensor copies (-1: heuristic, 0: never,
  *                          1: whenever n_r % 8 == 0 and the grid is wider than a tile)
  *   "persist"          [8] tdse_step_taylor on SMALL grids (at most one wave of CTAs; no cut-off; logged rows, if any,
@@ -214,6 +216,11 @@ long tdse_graph_instantiations(tdse_handle *h);
  * 0 one kernel per order, 3 persistent register-patch kernel with direct global loads, 4 the same with TMA tile
  * fetches (3, 4: all orders in one pass). */
 int  tdse_taylor_was_blocked(tdse_handle *h);
+/* Plan of the register-patch kernel the last tdse_step_taylor / tdse_step_rk4 / tdse_step_imag call ran with (any
+ * pointer may be NULL): *variant = instantiation (index into the table of csrc/tdse_taylor_rp_plan.h; -1 if the call did
+ * not use that kernel), *steps_per_launch = steps one launch takes (1, or up to option "persist" on small grids),
+ * *ctas = CTAs of a launch.  Returns TDSE_OK. */
+int  tdse_taylor_plan(tdse_handle *h, int *variant, int *steps_per_launch, int *ctas);
 /* 1 if the last tdse_step_rk45 call ran as the single persistent kernel (option "rk45_persist"), 0 if it ran stage by
  * stage. */
 int  tdse_rk45_was_persistent(tdse_handle *h);

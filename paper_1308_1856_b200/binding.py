@@ -19,7 +19,7 @@ ERRORS = {-1: "TDSE_ERR_ARG", -2: "TDSE_ERR_ALLOC", -3: "TDSE_ERR_CUDA", -4: "TD
 SYMBOLS = ["tdse_create", "tdse_destroy", "tdse_set_option", "tdse_set_pulse", "tdse_set_bound_states",
            "tdse_set_cutoff", "tdse_set_state", "tdse_get_state", "tdse_apply_H", "tdse_set_absorber", "tdse_bound_population", "tdse_step_taylor", "tdse_step_imag", "tdse_energy_log", "tdse_step_rk4", "tdse_step_rk", "tdse_rk_sigma",
            "tdse_step_lanczos", "tdse_step_rk45", "tdse_observables", "tdse_obs_log", "tdse_dt_log",
-           "tdse_lanczos_info", "tdse_ionisation_yield", "tdse_graph_instantiations", "tdse_launch_count", "tdse_taylor_was_blocked", "tdse_rk45_was_persistent", "tdse_observables_noalloc", "tdse_strerror", "tdse_version"]
+           "tdse_lanczos_info", "tdse_ionisation_yield", "tdse_graph_instantiations", "tdse_launch_count", "tdse_taylor_was_blocked", "tdse_rk45_was_persistent", "tdse_taylor_plan", "tdse_observables_noalloc", "tdse_strerror", "tdse_version"]
 
 
 class TdseError(RuntimeError):
@@ -80,6 +80,7 @@ def lib():
         L.tdse_graph_instantiations.restype = C.c_long
         L.tdse_ionisation_yield.argtypes = [vp, dp, vp]
         L.tdse_observables_noalloc.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, vp, vp, vp]
+        L.tdse_taylor_plan.argtypes = [vp, ip, ip, ip]
         L.tdse_rk45_was_persistent.argtypes = [vp]
         L.tdse_rk45_was_persistent.restype = C.c_int
         L.tdse_taylor_was_blocked.argtypes = [vp]
@@ -319,6 +320,12 @@ class Tdse:
 
     def taylor_was_blocked(self):
         return bool(lib().tdse_taylor_was_blocked(self._h))
+
+    def taylor_plan(self):
+        """dict(variant, steps_per_launch, ctas) of the register-patch kernel the last step call ran with."""
+        v, k, n = C.c_int(-1), C.c_int(0), C.c_int(0)
+        _check(lib().tdse_taylor_plan(self._h, C.byref(v), C.byref(k), C.byref(n)), "tdse_taylor_plan")
+        return {"variant": v.value, "steps_per_launch": k.value, "ctas": n.value}
 
     def rk45_was_persistent(self):
         return bool(lib().tdse_rk45_was_persistent(self._h))

@@ -757,6 +757,9 @@ int run_fixed(tdse_handle *h, int kind, int p1, int p2, double t0, double dt, lo
               cudaStream_t stream) {
     const int B = h->grid.batch;
     int G = std::max(1, h->graph_steps);
+    // small grids whose launches take several steps: a graph of four times as many steps (the field-table and counter
+    // kernels and the graph launch itself weigh 15 % of a 16-step block there)
+    if (kind == KIND_TAYLOR && h->taylor_blocked_last && h->rpp.persist > 1) G *= 4;
     if (h->taylor_blocked_last) G = (G + 1) & ~1;       // ping-pong needs an even block
     RC(ensure_buf(h, &h->d_etab, &h->etab_cap, (size_t)G * 7 * B));
     RC(ensure_rows(h, nsteps, obs_every));
@@ -1444,5 +1447,13 @@ int tdse_bound_population(tdse_handle *h, double r_b, double *out_host, void *st
 
 int tdse_taylor_was_blocked(tdse_handle *h) { return h ? h->taylor_blocked_last + ((h->taylor_blocked_last == 3 && h->rpp.tma) ? 1 : 0) : 0; }
 int tdse_rk45_was_persistent(tdse_handle *h) { return h ? h->rk45_persist_last : 0; }
+int tdse_taylor_plan(tdse_handle *h, int *variant, int *steps_per_launch, int *ctas) {
+    if (!h) return TDSE_ERR_ARG;
+    const bool used = h->taylor_blocked_last == 3 || h->rk4_fused;
+    if (variant) *variant = (used && h->rpp.ok) ? h->rpp.variant : -1;
+    if (steps_per_launch) *steps_per_launch = (used && h->rpp.ok && h->rpp.persist > 1) ? h->rpp.persist : 1;
+    if (ctas) *ctas = (used && h->rpp.ok) ? h->rpp.grid : 0;
+    return TDSE_OK;
+}
 
 }  // extern "C"

@@ -814,19 +814,25 @@ inline int rp_launch_full(const GridDev &g, const RpPlan &p, const CUtensorMap &
 
 // MODE 1 / 2 instantiations exist only for the one-warp-wide variants (RKABLE) and full tiles; fused observables (ob)
 // for full tiles in real time (MODE 0 / 1)
+// up to p.persist steps per launch (halo sized for them)
+template <int FD, int CP, int NWR, int NWC, int MINB>
+inline int rp_launch_persist(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
+                             const double *dtp, int order, cudaStream_t s, const RpObs *ob, int n_steps) {
+    const bool mask = g.n_r < 32 * CP * NWC;
+    if (!p.persist || mask || p.tma || p.cl > 1 || p.rk != 0 || n_steps > p.persist || g.j0 != nullptr) return TDSE_ERR_UNSUPPORTED;
+    static DeviceOnce once[2];
+    const CUtensorMap no_map{};
+    const RpObs no_obs{};
+    const int smem = (int)sizeof(RpSmem<FD, CP, NWR, NWC, false>);
+    if (ob) return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, false, 0, true, true>, &once[0], smem, p, s, g, in, out, ef, dtp, order, no_map, *ob, n_steps);
+    return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, false, 0, false, true>, &once[1], smem, p, s, g, in, out, ef, dtp, order, no_map, no_obs, n_steps);
+}
+
 template <int FD, int CP, int NWR, int NWC, int MINB, bool CLUSTERABLE, bool RKABLE>
 inline int rp_launch_one(const GridDev &g, const RpPlan &p, const double2 *in, double2 *out, const double *ef,
                          const double *dtp, int order, cudaStream_t s, const RpObs *ob, int n_steps) {
     const bool mask = g.n_r < 32 * CP * NWC;
-    if (p.persist) {        // up to p.persist steps per launch (halo sized for them)
-        if (mask || p.tma || p.cl > 1 || p.rk != 0 || n_steps > p.persist || g.j0 != nullptr) return TDSE_ERR_UNSUPPORTED;
-        static DeviceOnce once[2];
-        const CUtensorMap no_map{};
-        const RpObs no_obs{};
-        const int smem = (int)sizeof(RpSmem<FD, CP, NWR, NWC, false>);
-        if (ob) return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, false, 0, true, true>, &once[0], smem, p, s, g, in, out, ef, dtp, order, no_map, *ob, n_steps);
-        return rp_launch_kernel(taylor_rp_kernel<FD, CP, NWR, NWC, false, MINB, false, false, 0, false, true>, &once[1], smem, p, s, g, in, out, ef, dtp, order, no_map, no_obs, n_steps);
-    }
+    if (p.persist) return rp_launch_persist<FD, CP, NWR, NWC, MINB>(g, p, in, out, ef, dtp, order, s, ob, n_steps);
     if (n_steps != 1) return TDSE_ERR_UNSUPPORTED;
     CUtensorMap tmap{};
     if (p.tma) {
@@ -869,6 +875,9 @@ inline int launch_taylor_rp_fd(const GridDev &g, const RpPlan &p, const double2 
         TDSE_RP_CASE(2, 4, 4, 1, 2)
         TDSE_RP_CASE(3, 4, 8, 1, 1)
         TDSE_RP_CASE(4, 4, 4, 2, 1)
+        case 5: return rp_launch_persist<FD, 2, 1, 2, 4>(g, p, in, out, ef, dtp, order, s, ob, n_steps);
+        case 6: return rp_launch_persist<FD, 2, 2, 2, 2>(g, p, in, out, ef, dtp, order, s, ob, n_steps);
+        case 7: return rp_launch_persist<FD, 2, 4, 2, 1>(g, p, in, out, ef, dtp, order, s, ob, n_steps);
     }
 #undef TDSE_RP_CASE
     return TDSE_ERR_UNSUPPORTED;

@@ -17,12 +17,17 @@ struct RpVariant { int cp, nwr, nwc, minb; };
 constexpr RpVariant kRpVariants[] = {
     {4, 1, 1, 8}, {4, 2, 1, 4}, {4, 4, 1, 2}, {4, 8, 1, 1},      // 128-column tiles, 4 / 8 / 16 / 32 rows
     {4, 4, 2, 1},                                                // 256-column tile (edge exchange between warps), 16 rows
+    // 8 points per thread, 128-column tiles of two warps, 4 / 8 / 16 rows: only for the multi-step launches of small
+    // grids (persist > 1), whose step time is the latency of one warp's sweep -- half the patch, about half the sweep
+    {2, 1, 2, 4}, {2, 2, 2, 2}, {2, 4, 2, 1},
 };
 constexpr int kNumRpVariants = sizeof(kRpVariants) / sizeof(kRpVariants[0]);
 // the instantiations that also exist as cluster kernels (16 rows per CTA)
 constexpr bool rp_clusterable(int variant) { return variant == 2 || variant == 4; }
 // ... and as fused-RK4 / imaginary-time kernels (one-warp-wide tiles)
 constexpr bool rp_rk_capable(int variant) { return variant >= 0 && variant <= 3; }
+// ... and those that exist only as multi-step (PERSIST) kernels
+constexpr bool rp_persist_only(int variant) { return variant >= 5; }
 
 // rk = kernel MODE (0 Taylor, 1 classic RK4, 2 imaginary time); cl: CTAs per cluster (1: none)
 struct RpPlan { int ok, variant, tma, cl, rk, W, H, WT, n_tiles, n_items, grid, threads, persist; };     // persist: steps per launch (0: one)
@@ -44,6 +49,7 @@ inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant
         const RpVariant &v = kRpVariants[i];
         const int WT = 32 * v.cp * v.nwc;
         if (rk && (!rp_rk_capable(i) || g.n_r < WT)) continue;
+        if (rp_persist_only(i) && persist <= 1) continue;
         int rows = kRpRows * v.nwr, cl = 1;
         if (persist > 1 && (rows < g.n_l || g.n_r <= WT)) continue;
         if (rows < g.n_l) {
@@ -83,6 +89,7 @@ inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant
             const double n_ctas = (double)p.n_items * cl;
             double cost = (double)(rows / cl) * WT * std::max(1.0, n_ctas / n_sm);
             if (force_variant < 0 && v.nwc > 1) cost *= 1.4;
+            if (persist > 1) cost *= v.cp / 4.0;            // latency-bound: the sweep of one warp scales with its patch
             if (cl > 1) cost *= 1.25;
             if (tma) cost *= 0.85;
             if (!best.ok || cost < best_cost) { best = p; best_cost = cost; }

@@ -264,6 +264,39 @@ def test_taylor_register_patch_parity(B, case, tma):
     h.close()
 
 
+# (n_r, n_l, fd, batch, order, nsteps, obs_every, persist, forced variant, expected variant)
+MULTI_STEP_CASES = [
+    (500, 8, 3, 1, 4, 37, 0, 8, -1, 6),          # CFG1's grid: 8 points per thread, 8 rows
+    (500, 8, 3, 1, 4, 37, 1, 8, -1, 6),          # ... with a fused row every step (two bound states)
+    (500, 8, 3, 1, 4, 37, 1, 8, 1, 1),           # ... and the 16-points-per-thread instantiation, forced
+    (400, 3, 5, 2, 3, 21, 2, 4, -1, 5),          # 4-row instantiation, ragged rows, 5-point, two members
+    (600, 13, 3, 1, 2, 50, 5, 16, -1, 7),        # 16-row instantiation, ragged rows, 16 steps per launch
+    (1000, 16, 5, 3, 2, 19, 0, 4, -1, 7),        # several tiles per member, 5-point
+]
+
+
+@pytest.mark.parametrize("case", MULTI_STEP_CASES)
+def test_taylor_several_steps_per_launch(B, case):
+    """Small grids: one launch of the register-patch kernel takes several steps with psi in registers (option "persist",
+    halo sized for them), on the 8-points-per-thread instantiations the plan picks for them or a forced 16-point one;
+    odd step counts (a shorter last launch), fused rows, ragged rows: final state and every logged row against the oracle."""
+    n_r, n_l, fd, batch, order, nsteps, obs_every, persist, variant, expect = case
+    c = wl.config("cfg5" if batch > 1 else "cfg1", n_r=n_r, n_l=n_l, fd_order=fd, batch=batch, order=order)
+    c["propagator"] = "taylor"
+    dt = wl.dt_eff(c, "taylor", order)
+    t0 = wl.window(c, nsteps, dt)
+    psi0 = wl.populated_state(c)
+    opts = {"taylor_block": 1, "persist": persist, "taylor_rp_variant": variant, "obs_fused": 2}
+    h, got, ref, gobs, robs = run_pair_fixed(B, c, "taylor", nsteps, psi0, t0, dt, obs_every, [(0, 0), (1, 0)], opts,
+                                             order=order)
+    plan = h.taylor_plan()
+    assert h.taylor_kernel() == 3 and plan["variant"] == expect and plan["steps_per_launch"] > 1, plan
+    check_fixed(got, ref, gobs, robs)
+    for b in range(batch):
+        assert rel_l2(got[b], ref[b]) <= TOL_PSI
+    h.close()
+
+
 def test_taylor_batched_ragged_obs_every(B):
     c = wl.config("cfg5", n_r=300, batch=5, n_l=11)
     dt = wl.dt_eff(c)
