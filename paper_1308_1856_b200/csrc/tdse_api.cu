@@ -701,7 +701,7 @@ int build_rk45_loop(tdse_handle *h, int G) {
 
 // ---- graph-captured time loop (row a7; NS: "the time loop is captured in a CUDA graph") ------------------
 }  // namespace
-namespace tdse { int launch_rk45_persist(const RkpArgs &a, const RkpPlan &p, cudaStream_t s); }
+namespace tdse { int launch_rk45_persist(const RkpArgs &a, const RkpPlan &p, cudaStream_t s); bool rk45_persist_fits(int fd, int gauge, const RkpPlan &p); }
 namespace {
 enum Kind { KIND_TAYLOR = 1, KIND_RK4 = 2, KIND_LANCZOS = 3, KIND_RK45 = 4, KIND_RKGEN = 5 };
 
@@ -1194,6 +1194,7 @@ int tdse_step_rk45(tdse_handle *h, double t0, double t_end, double dt_init, doub
             cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) == cudaSuccess &&
             cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) == cudaSuccess && coop)
             pp = rkp_plan(h->grid, h->n_sm, std::min(max_smem - 2048, kRkpMaxSmem));
+        if (pp.ok && !rk45_persist_fits(h->grid.fd_order, h->grid.gauge, pp)) pp.ok = 0;     // (a partitioned or shared device)
     }
     h->rk45_persist_last = pp.ok;
     h->taylor_blocked_last = 0;

@@ -22,9 +22,33 @@ static int rkp_launch(const RkpArgs &a, const RkpPlan &p, cudaStream_t s) {
     return TDSE_OK;
 }
 
+// CTAs of this instantiation that can be resident at once on the current device (0: error)
+template <int FD, bool VG, bool KREG>
+static int rkp_resident(const RkpPlan &p) {
+    auto kern = rk45_persist_kernel<FD, VG, KREG>;
+    if (cudaFuncSetAttribute((const void *)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kRkpMaxSmem) != cudaSuccess) return 0;
+    int dev = 0, n_sm = 0, per_sm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)kern, kRkpThreads, (size_t)p.smem) != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
+    return per_sm * n_sm;
+}
+
 template <int FD, bool VG>
 static int rkp_launch_k(const RkpArgs &a, const RkpPlan &p, cudaStream_t s) {
     return p.kreg ? rkp_launch<FD, VG, true>(a, p, s) : rkp_launch<FD, VG, false>(a, p, s);
+}
+
+// can the grid of the plan be co-resident (what the hand-shakes between CTAs need)?  Else the caller runs stage by stage.
+bool rk45_persist_fits(int fd, int gauge, const RkpPlan &p) {
+    int n = 0;
+    if (fd == 3) n = gauge == 1 ? (p.kreg ? rkp_resident<3, true, true>(p) : rkp_resident<3, true, false>(p))
+                                : (p.kreg ? rkp_resident<3, false, true>(p) : rkp_resident<3, false, false>(p));
+    else n = gauge == 1 ? (p.kreg ? rkp_resident<5, true, true>(p) : rkp_resident<5, true, false>(p))
+                        : (p.kreg ? rkp_resident<5, false, true>(p) : rkp_resident<5, false, false>(p));
+    return n >= p.G;
 }
 
 int launch_rk45_persist(const RkpArgs &a, const RkpPlan &p, cudaStream_t s) {
