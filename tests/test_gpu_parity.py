@@ -801,6 +801,29 @@ def test_rk45_batched_with_rejects(B, persist, n_r, fd):
     h.close()
 
 
+@pytest.mark.parametrize("batch,n_l,n_r,fd", [(4, 16, 2500, 5), (32, 2, 600, 3)])
+def test_rk45_persistent_kernel_other_forms(B, batch, n_l, n_r, fd):
+    """The persistent Dormand-Prince kernel where a thread owns more than two points (k_1..k_7 in shared memory instead of
+    registers: 64 rows x 17 columns per CTA) and at the largest member count it takes (32): replay parity R-G20."""
+    c = wl.config("cfg5", n_r=n_r, n_l=n_l, batch=batch, fd_order=fd)
+    g, h = both(B, c)
+    pulses = wl.pulses(c)
+    h.set_pulse(pulses)
+    psi0 = wl.populated_state(c)
+    t0 = 0.5 * c["t_pulse"]
+    h.set_state(psi0)
+    info = h.step_rk45(t0, t0 + 0.01, 2e-3, 1e-9)
+    assert h.rk45_was_persistent()
+    assert info["n_accept"] >= 5 and info["n_reject"] >= 1
+    ref, rinfo = oracle.step_rk45(g, pulses, psi0, t0, t0 + 0.01, 2e-3, 1e-9, dt_replay=info["dt"])
+    assert np.max(rinfo["err"]) <= 1.05
+    got = h.get_state()
+    assert rel_l2(got, ref) <= TOL_PSI
+    for b in range(batch):
+        assert rel_l2(got[b], ref[b]) <= TOL_PSI
+    h.close()
+
+
 @pytest.mark.parametrize("check_every", [1, 5, 8])
 def test_rk45_device_loop_is_the_host_polled_run(B, check_every):
     """The adaptive run as one graph launch (WHILE node around a block of attempted steps, option rk45_loop = 1) takes
