@@ -505,6 +505,13 @@ def extra_measurements(binding, torch, stream, full_pulse=True):
                                    "gpoint_updates_per_s": pts * n_h * nsteps / (ms * 1e-3) / 1e9,
                                    "blocked": h.taylor_was_blocked() if c["propagator"] == "taylor" else None,
                                    "observables_every_step": bool(every)}
+            if c["propagator"] == "rk4":
+                out[f"step_{name}"]["kernel"] = ("persistent on-chip Runge-Kutta kernel (RK4 as an FSAL scheme)"
+                                                if h.rk45_was_persistent() else "four stages fused in the register-patch kernel")
+                h.set_option("rk4_persist", 0)
+                go(nsteps, t0)
+                ms1 = timed(torch, stream, lambda: go(nsteps, t0))
+                out[f"step_{name}"]["us_per_step_fused_register_patch_kernel"] = ms1 * 1e3 / nsteps
             if every:
                 h.step_taylor(c["order"], t0, dt, nsteps, 0, stream=stream)
                 ms0 = timed(torch, stream, lambda: h.step_taylor(c["order"], t0, dt, nsteps, 0, stream=stream))

@@ -99,6 +99,9 @@ void tdse_destroy(tdse_handle *h);
  *                          faster); 2: wherever the kernel can; 0: always the separate observable kernels
  *   "lanczos_beta_tol" [1e-12] breakdown threshold on beta ("if beta = 0 then quit", R-G17)
  *   "rk45_dt_max"      [0 = none] cap on the adaptive step
+ *   "rk4_persist"      [1] tdse_step_rk4 with obs_every = 0 and no absorber runs in the same persistent kernel as
+ *                          "rk45_persist" below when the grid fits on chip (classic RK4 as an FSAL scheme of five stage
+ *                          vectors, field values from a table, one launch per 2048 steps); 0: stage kernels
  *   "rk45_persist"     [1] tdse_step_rk45 runs as ONE persistent cooperative kernel when the grid fits the shared memory
  *                          of the device (batch * n_l * ceil(n_r / #SMs) <= 2048 points per CTA, batch <= 32): psi and
  *                          k_1..k_7 stay in shared memory from t0 to t_end, neighbouring CTAs hand their edge columns
@@ -221,8 +224,8 @@ int  tdse_taylor_was_blocked(tdse_handle *h);
  * not use that kernel), *steps_per_launch = steps one launch takes (1, or up to option "persist" on small grids),
  * *ctas = CTAs of a launch.  Returns TDSE_OK. */
 int  tdse_taylor_plan(tdse_handle *h, int *variant, int *steps_per_launch, int *ctas);
-/* 1 if the last tdse_step_rk45 call ran as the single persistent kernel (option "rk45_persist"), 0 if it ran stage by
- * stage. */
+/* 1 if the last tdse_step_rk45 / tdse_step_rk4 call ran in the persistent on-chip kernel (options "rk45_persist",
+ * "rk4_persist"), 0 if it ran stage by stage. */
 int  tdse_rk45_was_persistent(tdse_handle *h);
 
 /* Observables WITHOUT ANY ALLOCATION (row a6; Eq. 34, Eq. 36): for callers that cannot call cudaMalloc

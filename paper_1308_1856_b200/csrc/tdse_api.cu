@@ -129,7 +129,7 @@ struct tdse_handle {
     std::map<std::tuple<int, int, int, int, int, int>, cudaGraphExec_t> graphs;
     std::map<std::tuple<int, int, int, int, int, int>, long> graph_nodes;
     long launches = 0; long pending = 0; long graph_inst = 0; bool capturing = false;
-    int rk45_persist = 1; int rk45_persist_last = 0;     // the whole adaptive run as one persistent kernel (small grids)
+    int rk45_persist = 1, rk4_persist = 1; int rk45_persist_last = 0;     // the whole adaptive run as one persistent kernel (small grids)
     void *d_rkp_ws = nullptr; size_t rkp_ws_cap = 0;
     cudaGraphExec_t rk45_loop = nullptr; long rk45_loop_nodes = 0; int rk45_loop_G = 0, rk45_use_loop = 1;   // device-driven adaptive run
     int taylor_blocked_last = 0;        // 0: one kernel per order, 3: all orders in one pass (persistent register-patch kernel)
@@ -787,6 +787,40 @@ int run_fixed(tdse_handle *h, int kind, int p1, int p2, double t0, double dt, lo
     return TDSE_OK;
 }
 
+// ---- the persistent on-chip Runge-Kutta kernel (tdse_rk45_persist.cuh) -------------------------------------------------
+// its plan on the current device (ok = 0: the grid does not fit on chip, or the device cannot hold the grid at once)
+RkpPlan rkp_plan_for(tdse_handle *h) {
+    RkpPlan pp{};
+    int dev = 0, max_smem = 0, coop = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess &&
+        cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) == cudaSuccess &&
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) == cudaSuccess && coop)
+        pp = rkp_plan(h->grid, h->n_sm, std::min(max_smem - 2048, kRkpMaxSmem));
+    if (pp.ok && !rk45_persist_fits(h->grid.fd_order, h->grid.gauge, pp)) pp.ok = 0;     // (a partitioned or shared device)
+    return pp;
+}
+
+// workspace of the packets (cleared: no packet of an earlier launch may carry a sequence number of this one) and the
+// arguments every mode shares
+int rkp_prepare(tdse_handle *h, const RkpPlan &pp, RkpArgs &a, cudaStream_t s) {
+    const size_t part_off = (pp.halo_bytes + 255) & ~(size_t)255, ws_bytes = part_off + pp.part_bytes;
+    if (h->rkp_ws_cap < ws_bytes) {
+        CU(cudaStreamSynchronize(s));
+        if (h->d_rkp_ws) cudaFree(h->d_rkp_ws);
+        h->d_rkp_ws = nullptr; h->rkp_ws_cap = 0;
+        CU(cudaMalloc(&h->d_rkp_ws, ws_bytes));
+        h->rkp_ws_cap = ws_bytes;
+    }
+    char *ws = (char *)h->d_rkp_ws;
+    a = RkpArgs{};
+    a.g = h->gd; a.psi = h->pool[h->psi_slot]; a.ctl = h->d_ctl; a.pulse = h->d_pulse; a.replay = h->d_replay;
+    a.dt_log = h->d_dtlog; a.err_log = h->d_errlog;
+    a.halo = (unsigned long long *)ws; a.part = (unsigned long long *)(ws + part_off);
+    a.G = pp.G; a.Wc = pp.Wc; a.R = pp.R; a.pitch = pp.pitch;
+    CU(cudaMemsetAsync(ws, 0, ws_bytes, s));
+    return TDSE_OK;
+}
+
 bool grid_valid(const tdse_grid *g) {
     return g && g->n_r >= 1 && g->n_l >= 1 && g->dr > 0.0 && g->batch >= 1 && g->batch <= 65535 &&
            (long long)g->n_r * g->n_l * g->batch < (1LL << 31) * 8;
@@ -912,6 +946,7 @@ int tdse_set_option(tdse_handle *h, const char *key, double value) {
     else if (k == "lanczos_beta_tol") { if (!(value >= 0.0)) return TDSE_ERR_ARG; h->beta_tol = value; free_graphs(h); }
     else if (k == "rk45_dt_max") { if (!(value >= 0.0)) return TDSE_ERR_ARG; h->rk45_dt_max = value; }
     else if (k == "rk45_check_every") { if (value < 1 || value > 1024) return TDSE_ERR_ARG; h->rk45_check_every = (int)value; }
+    else if (k == "rk4_persist") { if (value != 0.0 && value != 1.0) return TDSE_ERR_ARG; h->rk4_persist = (int)value; }
     else if (k == "rk45_persist") { if (value != 0.0 && value != 1.0) return TDSE_ERR_ARG; h->rk45_persist = (int)value; }
     else if (k == "rk45_loop") { if (value != 0.0 && value != 1.0) return TDSE_ERR_ARG; h->rk45_use_loop = (int)value; }
     else return TDSE_ERR_ARG;
@@ -1111,6 +1146,49 @@ static int step_taylor_impl(tdse_handle *h, int order, double t0, double dt, lon
 
 int tdse_step_rk4(tdse_handle *h, double t0, double dt, long nsteps, int obs_every, void *stream) {
     if (!h || nsteps < 0 || obs_every < 0) return TDSE_ERR_ARG;
+    h->rk45_persist_last = 0;
+    // Grids that fit on chip, no logged rows, no absorber: the whole call runs in the persistent Runge-Kutta kernel, classic
+    // RK4 written as an FSAL scheme of five stage vectors (the fifth is psi_new, its k the k_1 of the next step); field
+    // values of all stage times from a table, a launch per 2048 steps.
+    if (h->rk4_persist && obs_every == 0 && nsteps > 0 && !h->d_mask && !h->vg_quad) {
+        const RkpPlan pp = rkp_plan_for(h);
+        if (pp.ok) {
+            cudaStream_t s = (cudaStream_t)stream;
+            const int B = h->grid.batch, NS = 5;
+            const long chunk = 2048;
+            RC(ensure_pool(h, 1));
+            RC(ensure_buf(h, &h->d_etab, &h->etab_cap, (size_t)std::min(chunk, nsteps) * NS * B));
+            h->taylor_blocked_last = 0; h->rk4_fused = 0; h->rpp = RpPlan{};
+            CtlInit v{};
+            v.t0 = t0; v.dt = dt; v.obs_every = 0; v.field_sample = h->field_sample;
+            h->pending = 0;
+            RC(init_ctl(h, v, s));
+            StageTimes cs{};
+            cs.c[0] = 0.0; cs.c[1] = 0.5; cs.c[2] = 0.5; cs.c[3] = 1.0; cs.c[4] = 1.0;
+            for (long done = 0; done < nsteps;) {
+                const long n = std::min(chunk, nsteps - done);
+                field_table_rk_kernel<<<(unsigned)((n * NS * B + 255) / 256), 256, 0, s>>>(h->d_ctl, h->d_pulse, B, (int)n, NS, cs,
+                                                                                         h->d_etab, h->gd.gauge);
+                count(h);
+                RkpArgs a{};
+                RC(rkp_prepare(h, pp, a, s));
+                a.n_stage = NS; a.fixed = 1; a.n_fixed = n; a.e_tab = h->d_etab;
+                for (int i = 1; i < 4; ++i)
+                    for (int j = 0; j < i; ++j) a.a[i][j] = RK4_A[i][j];
+                for (int j = 0; j < 4; ++j) a.a[4][j] = RK4_B[j];
+                RC(launch_rk45_persist(a, pp, s));
+                count(h);
+                ctl_advance_kernel<<<1, 32, 0, s>>>(h->d_ctl, (int)n);
+                count(h);
+                done += n;
+            }
+            CU(cudaGetLastError());
+            h->launches += h->pending;
+            h->log_rows = 0;
+            h->rk45_persist_last = 1;
+            return TDSE_OK;
+        }
+    }
     RC(ensure_pool(h, 6));
     h->taylor_blocked_last = 0;
     h->rk4_fused = 0;
@@ -1188,14 +1266,7 @@ int tdse_step_rk45(tdse_handle *h, double t0, double t_end, double dt_init, doub
     const int B = h->grid.batch;
     // grids that fit the shared memory of the machine: the whole run is one persistent kernel (tdse_rk45_persist.cuh)
     RkpPlan pp{};
-    if (h->rk45_persist) {
-        int dev = 0, max_smem = 0, coop = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess &&
-            cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) == cudaSuccess &&
-            cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) == cudaSuccess && coop)
-            pp = rkp_plan(h->grid, h->n_sm, std::min(max_smem - 2048, kRkpMaxSmem));
-        if (pp.ok && !rk45_persist_fits(h->grid.fd_order, h->grid.gauge, pp)) pp.ok = 0;     // (a partitioned or shared device)
-    }
+    if (h->rk45_persist) pp = rkp_plan_for(h);
     h->rk45_persist_last = pp.ok;
     h->taylor_blocked_last = 0;
     if (!pp.ok) {
@@ -1239,25 +1310,13 @@ int tdse_step_rk45(tdse_handle *h, double t0, double t_end, double dt_init, doub
     h->pending = 0;
     RC(init_ctl(h, v, s));
     if (pp.ok) {
-        const size_t part_off = (pp.halo_bytes + 255) & ~(size_t)255, ws_bytes = part_off + pp.part_bytes;
-        if (h->rkp_ws_cap < ws_bytes) {
-            CU(cudaStreamSynchronize(s));
-            if (h->d_rkp_ws) cudaFree(h->d_rkp_ws);
-            h->d_rkp_ws = nullptr; h->rkp_ws_cap = 0;
-            CU(cudaMalloc(&h->d_rkp_ws, ws_bytes));
-            h->rkp_ws_cap = ws_bytes;
-        }
-        char *ws = (char *)h->d_rkp_ws;
         RkpArgs a{};
-        a.g = h->gd; a.psi = h->pool[h->psi_slot]; a.ctl = h->d_ctl; a.pulse = h->d_pulse; a.replay = h->d_replay;
-        a.dt_log = h->d_dtlog; a.err_log = h->d_errlog;
-        a.halo = (unsigned long long *)ws; a.part = (unsigned long long *)(ws + part_off);
-        a.G = pp.G; a.Wc = pp.Wc; a.R = pp.R; a.pitch = pp.pitch;
+        RC(rkp_prepare(h, pp, a, s));
+        a.n_stage = 7;
         for (int i = 0; i < 7; ++i) {
             for (int j = 0; j < 7; ++j) a.a[i][j] = DP_A[i][j];
             a.d_err[i] = DP_B[i] - DP_BH[i];
         }
-        CU(cudaMemsetAsync(ws, 0, ws_bytes, s));        // no packet of an earlier run may carry a sequence number of this one
         RC(launch_rk45_persist(a, pp, s));
         count(h);
         h->launches += h->pending;

@@ -81,8 +81,16 @@ struct RkpArgs {
     unsigned long long *halo;     // [2][G][2 sides][R][HW][4] packets: edge columns of the stage vectors (zero before the launch)
     unsigned long long *part;     // [2][G][B][2][2] packets: error-norm partial sums (zero before the launch)
     int G, Wc, R, pitch;
-    double a[7][7];               // a[s][j], j < s: stage vector g_{s+1} (row 6 = the b row: psi_new)
+    double a[7][7];               // a[s][j], j < s: stage vector g_{s+1} (the last row = the b row: psi_new)
     double d_err[7];              // b_j - bhat_j
+    // Every explicit method runs here as an FSAL scheme: its last stage vector is psi_new, whose k is the k_1 of the next
+    // step (Dormand-Prince is one by construction, n_stage = 7; classic RK4 becomes one with n_stage = 5, row 4 = b).
+    int n_stage;                  // k vectors of a step, the closing one included (2..7)
+    // FIXED-step mode (tdse_step_rk4): n_fixed steps of ctl->dt, every one accepted, no error estimate, no exchange of
+    // sums; the field values of all stage times come from e_tab[step][n_stage][batch] (field_table_rk_kernel)
+    int fixed;
+    long long n_fixed;
+    const double *e_tab;
 };
 
 // ---- self-validating packets: {32 bits of data, 32-bit sequence number} per aligned 8-byte word -------------------------
@@ -282,7 +290,20 @@ __global__ void __launch_bounds__(kRkpThreads, 1) rk45_persist_kernel(const __gr
     };
 
     bool have_k1 = false;
-    while (!c.done && !c.stop) {
+    const bool fixed = a.fixed != 0;
+    const int ns = a.n_stage;
+    long long step = 0;
+    if (fixed) {
+        const double hh = a.ctl->dt;
+        if (tid < 49) coef[tid] = hh * a.a[tid / 7][tid % 7];
+        if (tid < ns * B) etab[tid] = __ldg(a.e_tab + tid);
+        __syncthreads();
+    }
+    while (fixed ? step < a.n_fixed : (!c.done && !c.stop)) {
+        double e_next = 0.0;    // fixed: the field value this thread carries over to the next step
+        const bool carries = fixed && tid < ns * B && step + 1 < a.n_fixed;
+        if (carries) e_next = __ldg(a.e_tab + (size_t)(step + 1) * ns * B + tid);
+        if (!fixed) {
         // ---- start of an attempted step: clip the step to t_end (or take the replayed one), field values of the stages
         if (tid == 0) {
             double h = c.h;
@@ -301,17 +322,19 @@ __global__ void __launch_bounds__(kRkpThreads, 1) rk45_persist_kernel(const __gr
         if (tid < 49) coef[tid] = hh * a.a[tid / 7][tid % 7];
         else if (tid < 56) coef[tid] = hh * a.d_err[tid - 49];
         __syncthreads();
+        }
         if (!have_k1) {         // the first attempted step: k_1 = -i H(t) psi (afterwards FSAL supplies it)
             stage(RkpI<0>{});
             have_k1 = true;
         }
         // ---- stages 2..7: g_{s+1} = psi + h sum_j a_{s+1,j} k_j, then k_{s+1}; the last one is psi_new and k_7 -------------
         stage(RkpI<1>{});
-        stage(RkpI<2>{});
-        stage(RkpI<3>{});
-        stage(RkpI<4>{});
-        stage(RkpI<5>{});
-        stage(RkpI<6>{});
+        if (ns > 2) stage(RkpI<2>{});
+        if (ns > 3) stage(RkpI<3>{});
+        if (ns > 4) stage(RkpI<4>{});
+        if (ns > 5) stage(RkpI<5>{});
+        if (ns > 6) stage(RkpI<6>{});
+        if (!fixed) {
         // ---- embedded error estimate: Delta = h sum_j (b_j - bhat_j) k_j against psi_new ---------------------------
         {
             const double2 *tc = tile + cur * TS;
@@ -410,17 +433,31 @@ __global__ void __launch_bounds__(kRkpThreads, 1) rk45_persist_kernel(const __gr
                 if (!c.done && !(hn > 0.0)) c.stop = 1;     // no positive step left: the host reports TDSE_ERR_NONFINITE
             }
         }
-        __syncthreads();
-        if (c.accept) {         // psi <- psi_new (the vector in the tile), k_1 <- k_7 (FSAL: same time t_{n+1})
+        }
+        __syncthreads();        // (fixed: every thread is done with the field values of this step)
+        if (fixed || c.accept) {    // psi <- psi_new (the vector in the tile), k_1 <- the closing k (FSAL: same time t_{n+1})
             const double2 *tc = tile + cur * TS;
 #pragma unroll
             for (int i = 0; i < PT; ++i) {
                 if (!own[i]) continue;
                 const int p = tid + i * NT;
-                if constexpr (KREG) { pr[i] = tc[tix[i]]; kr[0][i] = kr[KREG ? 6 : 0][i]; }
-                else { psi_s[p] = tc[tix[i]]; k_s[p] = k_s[(size_t)6 * Pcap + p]; }
+                if constexpr (KREG) {
+                    pr[i] = tc[tix[i]];
+                    double2 kl = kr[KREG ? 6 : 0][i];
+                    if (ns == 6) kl = kr[KREG ? 5 : 0][i];
+                    if (ns == 5) kl = kr[KREG ? 4 : 0][i];
+                    if (ns == 4) kl = kr[KREG ? 3 : 0][i];
+                    if (ns == 3) kl = kr[KREG ? 2 : 0][i];
+                    if (ns == 2) kl = kr[KREG ? 1 : 0][i];
+                    kr[0][i] = kl;
+                } else {
+                    psi_s[p] = tc[tix[i]];
+                    k_s[p] = k_s[(size_t)(ns - 1) * Pcap + p];
+                }
             }
         }
+        if (carries) etab[tid] = e_next;
+        ++step;
         __syncthreads();
     }
 
@@ -429,7 +466,7 @@ __global__ void __launch_bounds__(kRkpThreads, 1) rk45_persist_kernel(const __gr
         if (own[i]) {
             if constexpr (KREG) a.psi[gix[i]] = pr[i]; else a.psi[gix[i]] = psi_s[tid + i * NT];
         }
-    if (cta == 0 && tid == 0) {
+    if (cta == 0 && tid == 0 && !fixed) {
         Ctl &s = *a.ctl;
         s.t = c.t; s.h = c.h; s.done = c.done; s.last = c.last; s.after_reject = c.after_reject;
         s.n_accept = c.n_accept; s.n_reject = c.n_reject; s.n_attempt = c.n_attempt;

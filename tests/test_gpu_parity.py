@@ -355,12 +355,60 @@ def test_rk4_parity(B, case, fused):
     t0 = wl.window(c, nsteps, dt)
     psi0 = wl.populated_state(c)
     h, got, ref, gobs, robs = run_pair_fixed(B, c, "rk4", nsteps, psi0, t0, dt, obs_every, [(0, 0)],
-                                             {"use_graph": use_graph, "rk4_block": fused, "obs_fused": 2})
-    assert (h.taylor_kernel() in (3, 4)) == (bool(fused) and n_r >= 128)
+                                             {"use_graph": use_graph, "rk4_block": fused, "obs_fused": 2, "rk4_persist": 0})
+    assert (h.taylor_kernel() in (3, 4)) == (bool(fused) and n_r >= 128) and not h.rk45_was_persistent()
     check_fixed(got, ref, gobs, robs)
     for b in range(batch):
         for l in range(n_l):
             assert np.linalg.norm(got[b, l] - ref[b, l]) <= TOL_PSI * max(np.linalg.norm(ref[b, l]), 1e-3)
+    h.close()
+
+
+RK4_PERSIST_CASES = [
+    # n_r, n_l, fd, batch, nsteps, gauge, cutoff
+    (600, 9, 5, 1, 70, 0, 0.0),         # ragged column blocks, k_1..k_5 in registers
+    (333, 5, 3, 3, 41, 0, 0.0),         # batched, 3-point, odd sizes
+    (4000, 32, 5, 1, 24, 0, 0.0),       # CFG2's own grid
+    (200, 4, 5, 2, 2100, 0, 0.0),       # more steps than one launch takes (2048): two launches, two field tables
+    (500, 6, 5, 1, 30, 1, 0.0),         # velocity gauge
+    (500, 8, 3, 1, 30, 0, 10.0),        # centrifugal cut-off
+    (2500, 16, 5, 4, 12, 0, 0.0),       # more than two points per thread: k_1..k_5 in shared memory
+]
+
+
+@pytest.mark.parametrize("case", RK4_PERSIST_CASES)
+def test_rk4_persistent_kernel_parity(B, case):
+    """Classic RK4 on grids that fit on chip and without logged rows: the whole call runs in the persistent Runge-Kutta
+    kernel (RK4 as an FSAL scheme of five stage vectors, field values from a table) -- final state against the oracle's
+    stage-by-stage recursion, and against the stage kernels of the same library."""
+    n_r, n_l, fd, batch, nsteps, gauge, cutoff = case
+    c = wl.config("cfg2", n_r=n_r, n_l=n_l, fd_order=fd, batch=batch, cutoff_lambda=cutoff)
+    dt = wl.dt_eff(c, "rk4", 4)
+    t0 = wl.window(c, nsteps, dt)
+    psi0 = wl.populated_state(c)
+    g = oracle.make_grid(n_r, c["dr"], n_l, fd, gauge=gauge, batch=batch, cutoff_lambda=cutoff)
+    h = B.Tdse(n_r, c["dr"], n_l, fd, gauge=gauge, batch=batch)
+    if cutoff:
+        h.set_cutoff(cutoff)
+        psi0 = oracle.project(g, psi0)
+    pulses = wl.pulses(c)
+    if gauge == 1:          # the velocity gauge takes the Hann-shaped vector potential (pulse kind 1)
+        pulses = [(0.06 + 0.02 * b, 0.3, 3.0, 0.2, 1) for b in range(batch)]
+        t0 = 20.0
+    h.set_pulse(pulses)
+    h.set_state(psi0)
+    h.step_rk4(t0, dt, nsteps)
+    assert h.rk45_was_persistent()
+    got = h.get_state()
+    ref, _ = oracle.step_rk4(g, pulses, psi0, t0, dt, nsteps)
+    assert rel_l2(got, ref) <= TOL_PSI
+    for b in range(batch):
+        assert rel_l2(got[b], ref[b]) <= TOL_PSI
+    h.set_option("rk4_persist", 0)
+    h.set_state(psi0)
+    h.step_rk4(t0, dt, nsteps)
+    assert not h.rk45_was_persistent()
+    assert rel_l2(h.get_state(), got) <= 1e-12
     h.close()
 
 
