@@ -4,10 +4,10 @@
 
 namespace tdse {
 
-template <int FD, bool VG, bool KREG>
-static int rkp_launch(const RkpArgs &a, const RkpPlan &p, cudaStream_t s) {
+template <int FD, bool VG, bool KREG, bool FIXED>
+static int rkp_launch_f(const RkpArgs &a, const RkpPlan &p, cudaStream_t s) {
     static DeviceOnce once;
-    auto kern = rk45_persist_kernel<FD, VG, KREG>;
+    auto kern = rk45_persist_kernel<FD, VG, KREG, FIXED>;
     if (once.first()) {
         if (cudaFuncSetAttribute((const void *)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kRkpMaxSmem) != cudaSuccess)
             return TDSE_ERR_CUDA;
@@ -22,10 +22,17 @@ static int rkp_launch(const RkpArgs &a, const RkpPlan &p, cudaStream_t s) {
     return TDSE_OK;
 }
 
+template <int FD, bool VG, bool KREG>
+static int rkp_launch(const RkpArgs &a, const RkpPlan &p, cudaStream_t s) {
+    if (a.fixed) return rkp_launch_f<FD, VG, KREG, true>(a, p, s);
+    if (a.n_stage != 7) return TDSE_ERR_UNSUPPORTED;        // (the adaptive instantiation is Dormand-Prince's seven stages)
+    return rkp_launch_f<FD, VG, KREG, false>(a, p, s);
+}
+
 // CTAs of this instantiation that can be resident at once on the current device (0: error)
 template <int FD, bool VG, bool KREG>
 static int rkp_resident(const RkpPlan &p) {
-    auto kern = rk45_persist_kernel<FD, VG, KREG>;
+    auto kern = rk45_persist_kernel<FD, VG, KREG, false>;      // (the fixed-step instantiation needs no more than this one)
     if (cudaFuncSetAttribute((const void *)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kRkpMaxSmem) != cudaSuccess) return 0;
     int dev = 0, n_sm = 0, per_sm = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||

@@ -120,7 +120,9 @@ template <int N> using RkpI = std::integral_constant<int, N>;
 
 // KREG: at most kRkpRegPT points per thread; psi and k_1..k_7 of a thread's points stay in its registers, shared memory
 // holds only the two copies of the stage vector (whose neighbours other threads read).
-template <int FD, bool VG, bool KREG>
+// FIXED: the fixed-step mode with any stage count (a separate instantiation: the adaptive Dormand-Prince run keeps its
+// seven stages and its control flow as compile-time facts).
+template <int FD, bool VG, bool KREG, bool FIXED>
 __global__ void __launch_bounds__(kRkpThreads, 1) rk45_persist_kernel(const __grid_constant__ RkpArgs a) {
     constexpr int HW = (FD == 3) ? 1 : 2;
     constexpr int NT = kRkpThreads, NW = NT / 32, PT = KREG ? kRkpRegPT : kRkpMaxPT;
@@ -290,8 +292,8 @@ __global__ void __launch_bounds__(kRkpThreads, 1) rk45_persist_kernel(const __gr
     };
 
     bool have_k1 = false;
-    const bool fixed = a.fixed != 0;
-    const int ns = a.n_stage;
+    constexpr bool fixed = FIXED;
+    const int ns = FIXED ? a.n_stage : 7;
     long long step = 0;
     if (fixed) {
         const double hh = a.ctl->dt;
