@@ -104,9 +104,10 @@ void tdse_destroy(tdse_handle *h);
  *                          vectors, field values from a table, one launch per 2048 steps); 0: stage kernels
  *   "rk45_persist"     [1] tdse_step_rk45 runs as ONE persistent cooperative kernel when the grid fits the shared memory
  *                          of the device (batch * n_l * ceil(n_r / #SMs) <= 2048 points per CTA, batch <= 32): psi and
- *                          k_1..k_7 stay in shared memory from t0 to t_end, neighbouring CTAs hand their edge columns
- *                          over through flags, every CTA runs the controller (the paper's kernel boundaries are
- *                          its only global synchronisation); 0, or a larger grid: one kernel per stage, see below
+ *                          k_1..k_7 stay on chip (registers or shared memory) from t0 to t_end, neighbouring CTAs hand
+ *                          their edge columns over as self-validating packets through L2, every CTA runs the controller
+ *                          (the paper's kernel boundaries are its only global synchronisation); 0, a larger grid
+ *                          or a device that cannot hold the grid at once: one kernel per stage, see below
  *   "rk45_loop"        [1] (stage by stage) tdse_step_rk45 runs as ONE graph launch: a CUDA-graph WHILE node repeats a block of attempted
  *                          steps until the device controller is done (no host poll); 0: the host enqueues blocks and
  *                          polls the `done` flag between them
