@@ -296,7 +296,8 @@ def run_own(args):
         d2h = (pin_out.numel() * 16 + yld.size * 8) / K
         # ---- the same job with the batch split over several handles and streams (members are independent): the
         # pinned-host transfers of one part overlap the steps of another.  Same bytes, same outputs, same ABI calls.
-        ms_e2e, n_parts, yld_p = e2e_pipelined(binding, torch, sharding, c, args, pulses, pinned, pin_out, order, t0, dt, K)
+        ms_e2e, n_parts, yld_p = e2e_pipelined(binding, torch, sharding, c, args, pulses, pinned, pin_out, order, t0, dt, K,
+                                               parts=args.e2e_parts)
         if ms_e2e is None or ms_e2e > ms_e2e_serial:
             ms_e2e, n_parts = ms_e2e_serial, 1
         else:
@@ -653,6 +654,7 @@ def main():
     ap.add_argument("--no-block", action="store_true", help="one kernel per Taylor order (no temporal blocking)")
     ap.add_argument("--rp-variant", type=int, default=-1, help="instantiation of the register-patch kernel")
     ap.add_argument("--rp-tma", type=int, default=-1, help="register-patch kernel: -1 auto, 0 direct loads, 1 TMA")
+    ap.add_argument("--e2e-parts", type=int, default=4, help="handles / streams the end-to-end leg splits the batch over")
     ap.add_argument("--no-extra", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-full-pulse", action="store_true", help="skip the 8e5-step CFG3 run of `extra` (about 70 s)")
