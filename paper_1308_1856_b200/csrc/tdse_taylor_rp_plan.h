@@ -91,7 +91,10 @@ inline RpPlan rp_plan(const tdse_grid &g, int order, int n_sm, int force_variant
             if (force_variant < 0 && v.nwc > 1) cost *= 1.4;
             if (persist > 1) cost *= v.cp / 4.0;            // latency-bound: the sweep of one warp scales with its patch
             if (cl > 1) cost *= 1.25;
-            if (tma) cost *= 0.85;
+            // (a state that stays in L2 gains less from the prefetch than it loses to the halo rounded up to 8 columns:
+            // CFG3 62.1 us per step with direct loads, 88 interior columns, against 63.1 us with TMA tiles, 80)
+            const bool l2_resident = 2.0 * 16.0 * (double)g.n_r * g.n_l * g.batch < 100e6;
+            if (tma) cost *= l2_resident ? 0.93 : 0.85;
             if (!best.ok || cost < best_cost) { best = p; best_cost = cost; }
         }
     }

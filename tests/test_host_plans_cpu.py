@@ -52,8 +52,9 @@ def test_plans_of_the_five_configurations(plans):
     # CFG2: clusters of 2; on chip: 143 CTAs of 28 columns x 32 rows, two points per thread (k in registers)
     assert p2["cl"] == 2 and (p2["k_ok"], p2["G"], p2["Wc"], p2["R"], p2["kreg"]) == (1, 143, 28, 32, 1)
     assert p2["smem"] <= 224 * 1024
-    # CFG3: clusters of 4, halo 20 rounded to 24 for the TMA tile start; CFG4: clusters of 8; neither fits on chip
-    assert (p3["cl"], p3["H"], p3["W"]) == (4, 24, 80) and p3["k_ok"] == 0
+    # CFG3 (L2-resident): clusters of 4, direct loads with the exact halo of 20 columns (TMA tiles would round it up to
+    # 24); CFG4: clusters of 8; neither fits on chip
+    assert (p3["cl"], p3["tma"], p3["H"], p3["W"]) == (4, 0, 20, 88) and p3["k_ok"] == 0
     assert p4["cl"] == 8 and p4["k_ok"] == 0
 
 
